@@ -1,0 +1,233 @@
+"""Pins for the oracle's path (norm -> mask -> backbone -> residual -> GEMMs); not gpu.
+P:n = /root/reference/PAPER.md line n."""
+import itertools
+import math
+from fractions import Fraction
+
+import ml_dtypes
+import numpy as np
+import pytest
+
+import sharq_inputs as si
+from oracle import sharq_oracle as so
+
+F32 = np.float32
+
+
+@pytest.fixture(scope="module")
+def small():
+    T, K, D = 8, 1024, 256
+    x = si.activations(T, K, config=1)
+    g = si.gamma(K)
+    w = si.weight(D, K)
+    return x, g, w
+
+
+# ------------------------------------------------------------------ O1 norm
+def test_canonical_sum_against_fsum_and_special_cases():
+    rng = np.random.default_rng(0)
+    for K in (256, 768, 1024, 3584, 4096):
+        x = rng.standard_normal((3, K)).astype(F32)
+        s = so.canonical_sum(x, squares=True)
+        for t in range(3):
+            exact = math.fsum((float(v) ** 2 for v in x[t]))
+            assert abs(float(s[t]) - exact) <= K * 2.0 ** -24 * exact
+        # powers of two sum exactly whatever the order
+        p = np.ldexp(F32(1), rng.integers(-3, 4, (2, K))).astype(F32)
+        assert np.array_equal(so.canonical_sum(p, squares=False), p.astype(np.float64).sum(1).astype(F32))
+    # order pin: a permutation inside one 8-leaf that changes a naive left-to-right sum
+    x = np.zeros((1, 1024), F32); x[0, 0] = 2.0 ** 24; x[0, 1] = 1.0; x[0, 2] = 1.0
+    assert so.canonical_sum(x, False)[0] == 2.0 ** 24            # (2^24+1)+1 = 2^24 in fp32
+    x[0, 0], x[0, 2] = 1.0, 2.0 ** 24
+    assert so.canonical_sum(x, False)[0] == 2.0 ** 24 + 2        # (1+1)+2^24
+
+
+def test_rmsnorm_against_fp64_and_exact_case():
+    x = si.activations(4, 4096, config=1); g = si.gamma(4096)
+    X = so.bf16_to_f32(so.normalize(x, so.NORM_RMS, g)).astype(np.float64)
+    xf = so.bf16_to_f32(x).astype(np.float64); gf = so.bf16_to_f32(g).astype(np.float64)
+    ref = xf / np.sqrt((xf ** 2).mean(1, keepdims=True) + 1e-6) * gf
+    assert np.abs(X - ref).max() <= np.abs(ref).max() * 2.0 ** -7          # two bf16 roundings
+    assert (np.abs(X - ref) <= np.abs(ref) * (2.0 ** -8 + 2.0 ** -8 + 2.0 ** -15) + 1e-30).all()
+    # exact case: x = +-2 everywhere, gamma = 1, eps = 0 -> X = +-1 exactly
+    s = np.where(np.arange(512) % 3 == 0, -2.0, 2.0).astype(F32)[None, :]
+    X = so.normalize(so.f32_to_bf16(s), so.NORM_RMS, so.f32_to_bf16(np.ones(512, F32)), eps=0.0)
+    assert np.array_equal(so.bf16_to_f32(X), s / 2)
+    # layernorm: mean 0 / unit variance up to bf16
+    xl = so.f32_to_bf16((np.random.default_rng(1).standard_normal((2, 1024)) * 3 + 5).astype(F32))
+    X = so.bf16_to_f32(so.normalize(xl, so.NORM_LAYER, so.f32_to_bf16(np.ones(1024, F32)),
+                                    so.f32_to_bf16(np.zeros(1024, F32)))).astype(np.float64)
+    assert abs(X.mean()) < 1e-2 and abs(X.std() - 1) < 1e-2
+
+
+# ------------------------------------------------------------------ O3 masks
+def _best_mask_bruteforce(scores):
+    """Among the 6 two-of-four masks: lexicographically largest sorted kept scores, then lowest indices."""
+    best = None
+    for c in itertools.combinations(range(4), 2):
+        key = (tuple(sorted((scores[i] for i in c), reverse=True)), tuple(-i for i in c))
+        if best is None or key > best[0]:
+            best = (key, c)
+    return best[1]
+
+
+def test_pair_mask_exhaustive_small_alphabet():
+    """Every chunk of 8 with values in {0,+-1,+-2,+-3} restricted to score patterns: all 4^4 score
+    tuples over 4 distinct magnitudes x all placements of the max inside the pair (every tie pattern)."""
+    vals = so.f32_to_bf16(np.array([0, 1, 2, 3], F32))
+    rows = []
+    for sc in itertools.product(range(4), repeat=4):
+        for lay in range(16):                      # which element of each pair carries the score
+            ch = []
+            for p in range(4):
+                hi, lo = vals[sc[p]], vals[0] if sc[p] == 0 else vals[sc[p] - 1]
+                sign = 0x8000 if (lay >> p) & 1 else 0
+                ch += ([hi | sign, lo] if (lay >> p) & 1 else [lo, hi | sign])
+            rows.append(ch)
+    X = np.array(rows, dtype=np.uint16).reshape(1, -1)
+    keep, nib = so.mask_pair48(X)
+    keep = keep.reshape(-1, 4, 2); nib = nib.reshape(-1)
+    u = (X.reshape(-1, 4, 2) & 0x7FFF).max(-1)
+    for n in range(u.shape[0]):
+        c = _best_mask_bruteforce(u[n].tolist())
+        assert nib[n] == c[0] | (c[1] << 2)
+        assert keep[n].all(1).tolist() == [i in c for i in range(4)]
+        assert (keep[n, :, 0] == keep[n, :, 1]).all()
+
+
+def test_masks_on_random_data_and_24_exhaustive():
+    x = si.activations(16, 1024, config=1)
+    keep, nib = so.mask_pair48(x)
+    assert (keep.reshape(16, -1, 8).sum(-1) == 4).all()                    # exactly N survivors per M
+    assert ((nib & 3) < (nib >> 2)).all()                                  # ascending indices
+    # the largest element of every chunk is in the backbone
+    a = (x & 0x7FFF).reshape(16, -1, 8)
+    assert np.take_along_axis(keep.reshape(16, -1, 8), a.argmax(-1)[..., None], -1).all()
+    k24, n24 = so.mask_24(x)
+    assert (k24.reshape(16, -1, 4).sum(-1) == 2).all()
+    vals = so.f32_to_bf16(np.array([0, -1, 1, 2, -3], F32))
+    allq = np.array(list(itertools.product(vals.tolist(), repeat=4)), dtype=np.uint16).reshape(1, -1)
+    k, n = so.mask_24(allq)
+    u = (allq.reshape(-1, 4) & 0x7FFF)
+    for i in range(u.shape[0]):
+        c = _best_mask_bruteforce(u[i].tolist())
+        assert n[0, i] == c[0] | (c[1] << 2) and k.reshape(-1, 4)[i].tolist() == [j in c for j in range(4)]
+
+
+# ------------------------------------------------------------------ O2/O4-O6 scales, residual
+@pytest.mark.parametrize("fmt", [so.NVFP4, so.MXFP4])
+def test_prepare_invariants(small, fmt):
+    x, g, _ = small
+    p = so.prepare(x, fmt=fmt, gamma_u16=g)
+    T, K = x.shape
+    Xf = so.bf16_to_f32(p["X"]).astype(np.float64)
+    ts = p["ts"].astype(np.float64)
+    if fmt == so.NVFP4:
+        assert np.array_equal(p["ts"], (np.abs(Xf).max(1) / 2688.0).astype(F32))
+    # scale = amax/6 (/ts) rounded to the scale format, evaluated in fp64 (BASELINE.json invariant)
+    a_sp = np.where(p["keep"], np.abs(Xf), 0).reshape(T, -1, 32).max(-1)
+    if fmt == so.NVFP4:
+        want = np.minimum(a_sp / 6 / ts[:, None], 448).astype(F32).astype(ml_dtypes.float8_e4m3fn).view(np.uint8)
+        assert (p["sp_sf"] == want).mean() > 0.999          # fp32 chain vs fp64: only boundary cases differ
+        assert (np.abs(p["sp_sf"].astype(int) - want.astype(int)) <= 1).all()
+        sf = so.e4m3_decode(p["sp_sf"]).astype(np.float64) * ts[:, None]
+        assert (sf * 6 >= a_sp * (1 - 2.0 ** -4) - 1e-30).all()
+    else:
+        sf = so.e8m0_decode(p["sp_sf"]).astype(np.float64)
+        assert (sf * 6 >= a_sp).all() and (sf * 3 < a_sp)[a_sp > 0].all()               # smallest 2^e >= a/6
+    # every code on the grid; residual identity Eq. 8 exact in fp64
+    assert (so.unpack_codes(p["sp_codes"]) < 16).all() and (so.unpack_codes(p["dn_codes"]) < 16).all()
+    assert np.array_equal(p["R"].astype(np.float64) + p["Xsp_tilde"].astype(np.float64), Xf)
+    assert np.array_equal(p["R"][~p["keep"]], so.bf16_to_f32(p["X"])[~p["keep"]])
+    # Xsp_tilde equals what the stored bytes decode to (compression + metadata round trip)
+    back = so.dequant_backbone(p)
+    assert np.allclose(back, p["Xsp_tilde"], rtol=2 ** -22, atol=0)
+    codes, keep2 = so.expand_backbone(p)
+    assert np.array_equal(keep2, p["keep"])
+    # Eq. 12: X - (Xsp~ + R~) == R - R~, and the element error bound of the residual quantizer
+    Rt = so.dequant_residual(p)
+    lhs = Xf - (p["Xsp_tilde"].astype(np.float64) + Rt)
+    rhs = p["R"].astype(np.float64) - Rt
+    assert np.abs(lhs - rhs).max() <= 2.0 ** -40 * np.abs(Xf).max()
+    Gd = p["Gd"]
+    sfd = (so.sf_decode(p["dn_sf"], fmt).astype(np.float64) * ts[:, None]).repeat(Gd, 1)
+    dn = so.unpack_codes(p["dn_codes"]) & 7
+    half_gap = np.array([.25, .25, .25, .25, .5, .5, 1.0, 1.0])[dn]                    # half the e2m1 gap at that code
+    assert (np.abs(rhs)[dn < 7] <= (sfd * half_gap)[dn < 7] * (1 + 1e-6)).all()
+    # outliers isolated: residual block scales are not larger than a plain dense quantizer's
+    p0 = so.prepare(x, fmt=fmt, gamma_u16=g, _force_no_survivors=True)
+    assert so.sf_decode(p["dn_sf"], fmt).astype(np.float64).sum() < so.sf_decode(p0["dn_sf"], fmt).astype(np.float64).sum()
+
+
+def test_dense_only_special_case_equals_independent_nvfp4_quantizer(small):
+    """Empty mask => R = X and the residual path is a plain NVFP4 quantizer: compare with an
+    independent numpy + ml_dtypes implementation (casts done by the library)."""
+    x, g, _ = small
+    p = so.prepare(x, gamma_u16=g, _force_no_survivors=True)
+    Xf = so.bf16_to_f32(p["X"])
+    assert np.array_equal(p["R"], Xf)
+    T, K = Xf.shape
+    ts = (np.abs(Xf).max(1) / F32(2688)).astype(F32)
+    amax = np.abs(Xf).reshape(T, K // 16, 16).max(-1)
+    c6 = np.array([0x3E2AAAAB], np.uint32).view(F32)[0]
+    sf8 = ((amax * c6) * (F32(1) / ts)[:, None]).astype(F32).astype(ml_dtypes.float8_e4m3fn)
+    assert np.array_equal(sf8.view(np.uint8), p["dn_sf"])
+    s_eff = sf8.astype(F32) * ts[:, None]
+    q = (Xf * np.repeat(F32(1) / s_eff, 16, 1)).astype(F32).astype(ml_dtypes.float4_e2m1fn).view(np.uint8) & 0xF
+    assert np.array_equal(q[:, 0::2] | (q[:, 1::2] << 4), p["dn_codes"])
+
+
+def test_static_tensor_scale_and_zero_rows():
+    x = si.activations(4, 512, config=1)
+    x[1] = 0
+    p = so.prepare(x, norm=so.NORM_NONE)
+    assert p["ts"][1] == 1.0 and (p["sp_sf"][1] == 0).all() and (p["dn_codes"][1] == 0).all()
+    ps = so.prepare(x, norm=so.NORM_NONE, x_tensor_scale=0.03125)
+    assert (ps["ts"] == F32(0.03125)).all()
+
+
+# ------------------------------------------------------------------ O8 weights, O7 linear
+@pytest.mark.parametrize("fmt", [so.NVFP4, so.MXFP4, so.HIF4])
+def test_weight_views_share_one_payload(small, fmt):
+    _, _, w = small
+    wq = so.quantize_weight(w, fmt)
+    if fmt == so.NVFP4:
+        assert np.array_equal(wq["sf_dn"][:, 0::2], wq["sf_sp"]) and np.array_equal(wq["sf_dn"][:, 1::2], wq["sf_sp"])
+    assert np.array_equal(so.dequant_weight(wq, "sparse"), so.dequant_weight(wq, "dense"))
+    Wf = so.bf16_to_f32(w).astype(np.float64)
+    err = np.linalg.norm(so.dequant_weight(wq) - Wf) / np.linalg.norm(Wf)
+    assert err < 0.13
+
+
+@pytest.mark.parametrize("fmt", [so.NVFP4, so.MXFP4, so.HIF4])
+def test_linear_against_blas_loops_and_eq13(small, fmt):
+    x, g, w = small
+    p = so.prepare(x, fmt=fmt, gamma_u16=g)
+    wq = so.quantize_weight(w, fmt)
+    Y = so.linear(p, wq)
+    A = so.dequant_backbone(p) + so.dequant_residual(p)                 # Xsp~ + R~
+    Wd = so.dequant_weight(wq)
+    assert np.allclose(Y, A @ Wd.T, rtol=1e-11, atol=1e-11 * np.abs(Y).max())
+    for (t, d) in ((0, 0), (3, 17), (7, 255)):
+        assert math.isclose(so.linear_loops(p, wq, t, d), Y[t, d], rel_tol=1e-11, abs_tol=1e-12)
+    sub = so.linear(p, wq, rows=np.array([1, 5]), cols=np.array([2, 200]))
+    assert np.array_equal(sub, Y[np.ix_([1, 5], [2, 200])])
+    # Eq. 13
+    Xf = so.bf16_to_f32(p["X"]).astype(np.float64)
+    Rt = so.dequant_residual(p)
+    lhs = np.linalg.norm(Xf @ Wd.T - A @ Wd.T)
+    rhs = np.linalg.norm(p["R"].astype(np.float64) - Rt) * np.linalg.svd(Wd, compute_uv=False)[0]
+    assert lhs <= rhs * (1 + 1e-9)
+
+
+def test_qualitative_ordering_of_path_combinations():
+    """P:265, P:288 (Table 5): sparse-only >> plain dense NVFP4 >~ SharQ in activation error."""
+    x = si.activations(32, 4096, config=1); g = si.gamma(4096)
+    p = so.prepare(x, gamma_u16=g)
+    p0 = so.prepare(x, gamma_u16=g, _force_no_survivors=True)
+    Xf = so.bf16_to_f32(p["X"]).astype(np.float64)
+    n = np.linalg.norm
+    e_sparse = n(so.dequant_backbone(p) - Xf) / n(Xf)
+    e_dense = n(so.dequant_residual(p0) - Xf) / n(Xf)
+    e_sharq = n(so.dequant_backbone(p) + so.dequant_residual(p) - Xf) / n(Xf)
+    assert e_sparse > 2 * e_dense and e_dense > 2 * e_sharq
