@@ -1,0 +1,154 @@
+/* sharq.h -- C ABI of the B200-native SharQ per-linear-layer hot path.
+ *
+ * SharQ (arxiv/paper_2606_26587; "P:n" = line n of the paper text): for each linear layer
+ *   Y^ = GEMM_sp(Q_sp(M(X) . X), Q_w,sp(W)) + GEMM_dn(Q_dn(R), Q_w,dn(W)),  R = X - D_sp(Q_sp(X_sp))
+ * (Eq. 6-9).  Three calls make the path (Fig. 2, section 3.4):
+ *   sharq_quantize_weight  offline, once per weight: one FP4 payload + two scale views
+ *   sharq_prepare          per call: norm -> N:M mask -> sparse FP4 backbone -> residual -> dense FP4
+ *   sharq_linear           sparse + dense block-scaled FP4 GEMMs into one accumulator, bf16 epilogue
+ *
+ * Conventions
+ *   - The caller owns every buffer; the library never allocates device memory and keeps no
+ *     mutable global state.  All pointers are DEVICE pointers unless marked "host".
+ *   - Work is enqueued on the caller's CUDA stream (`stream` is a cudaStream_t passed as void*)
+ *     and the call returns without synchronising.
+ *   - Errors are return codes; nothing throws or aborts.  On a non-OK return nothing was launched.
+ *   - Sizes are int64_t, leading dimensions are in ELEMENTS, base pointers 16-byte aligned.
+ *   - bf16 tensors are row-major; "code" tensors hold two 4-bit codes per byte, the element
+ *     with the lower k in the low nibble.
+ *   - Shapes: K % 256 == 0 (8-chunks, 32/64 scale groups, MMA-K 128, 256-wide metadata tile),
+ *     D % 128 == 0 for sharq_linear, T >= 0 (T == 0 returns SHARQ_OK without a launch).
+ *   - Inputs must be finite; NaN/Inf behaviour is deterministic but unspecified.
+ *
+ * Output layouts (config.layout)
+ *   CANONICAL  plain row-major arrays as listed per argument below (what the parity tests read).
+ *   TILED      what sharq_linear consumes (tcgen05 scale-factor / metadata atoms):
+ *     scale factors [R rows, C = K/G columns], rows padded to a multiple of 128:
+ *       byte(r, c) at  ((r/128) * (C/4) + c/4) * 512 + (r%32)*16 + ((r%128)/32)*4 + (c%4)
+ *     sparsity metadata [R rows, K/16 bytes], rows padded to a multiple of 128:
+ *       byte(r, b) at  ((r/128) * (K/256) + b/16) * 2048 + (r%128)*16 + (b%16)
+ *     codes and row scales are identical in both layouts.
+ *   sharq_*_sizes report the padded byte counts for the chosen layout.
+ */
+#ifndef SHARQ_H_
+#define SHARQ_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  SHARQ_OK = 0,
+  SHARQ_EINVAL = 1,     /* null pointer, bad enum, misaligned pointer, unsupported combination */
+  SHARQ_ESHAPE = 2,     /* shape rule violated (see above) */
+  SHARQ_EWORKSPACE = 3, /* workspace too small */
+  SHARQ_EARCH = 4,      /* device is not sm_100 */
+  SHARQ_ECUDA = 5       /* a CUDA runtime / driver call failed (launch not accepted) */
+} sharq_status;
+
+typedef enum { SHARQ_NVFP4 = 0, SHARQ_MXFP4 = 1, SHARQ_HIF4 = 2 } sharq_format;
+/* PAIR48: 4:8 "in pairs" -- the pattern the block-scaled FP4 sparse MMA accepts.
+ * MASK_24: element-wise 2:4, used with HiF4. */
+typedef enum { SHARQ_MASK_PAIR48 = 0, SHARQ_MASK_24 = 1 } sharq_mask;
+typedef enum { SHARQ_NORM_NONE = 0, SHARQ_NORM_RMS = 1, SHARQ_NORM_LAYER = 2 } sharq_norm;
+typedef enum { SHARQ_LAYOUT_CANONICAL = 0, SHARQ_LAYOUT_TILED = 1 } sharq_layout;
+
+typedef struct {
+  int32_t fmt;    /* sharq_format */
+  int32_t mask;   /* sharq_mask; NVFP4/MXFP4 require PAIR48, HIF4 requires MASK_24 */
+  int32_t norm;   /* sharq_norm */
+  float eps;      /* added to the mean square / variance (P:155 RMSNorm / LayerNorm) */
+  int32_t layout; /* sharq_layout of scale-factor and metadata outputs */
+} sharq_config;
+
+/* ---- sizes: host-only pure functions; every out pointer may be NULL --------------------- */
+
+/* Bytes of the outputs of sharq_quantize_weight for W[D,K].  */
+sharq_status sharq_weight_sizes(const sharq_config* cfg, int64_t D, int64_t K, size_t* codes,
+                                size_t* sf_sparse_view, size_t* sf_dense_view, size_t* workspace);
+
+/* Bytes of the outputs of sharq_prepare for x[T,K]. */
+sharq_status sharq_act_sizes(const sharq_config* cfg, int64_t T, int64_t K, size_t* sp_codes,
+                             size_t* sp_sf, size_t* sp_meta, size_t* dn_codes, size_t* dn_sf,
+                             size_t* row_scale);
+
+/* Workspace bytes sharq_linear / sharq_linear_grouped need (may be 0). */
+sharq_status sharq_linear_workspace(const sharq_config* cfg, int64_t T, int64_t D, int64_t K,
+                                    int32_t E, size_t* workspace);
+
+/* ---- sharq_quantize_weight (Fig. 2 "weight preparation") --------------------
+ * W bf16 [D,K], row-major with leading dimension ldw (out-features x in-features).
+ *   codes           [D, K/2] bytes          the single shared FP4 payload
+ *   sf_sparse_view  [D, K/32] e4m3|e8m0     one scale per 32 k   (HiF4: [D, K/64] uint32 words)
+ *   sf_dense_view   [D, K/16] e4m3          every sparse-view scale repeated for its two
+ *                                           16-groups (MXFP4: [D,K/32], equal to the sparse
+ *                                           view; HiF4: equal to the sparse view)
+ *   tensor_scale    1 float                 NVFP4: max|W| / 2688; otherwise 1
+ *   workspace       >= sharq_weight_sizes(...workspace) bytes; used for the max|W| reduction
+ * Scale views follow cfg->layout.  Two kernels (amax, quantize); not on the timed path. */
+sharq_status sharq_quantize_weight(const sharq_config* cfg, const void* W, int64_t D, int64_t K,
+                                   int64_t ldw, void* codes, void* sf_sparse_view,
+                                   void* sf_dense_view, float* tensor_scale, void* workspace,
+                                   size_t workspace_bytes, void* stream);
+
+/* ---- sharq_prepare (Fig. 2 "fused activation preparation") --------------
+ * ONE kernel, one pass over x.  x bf16 [T,K] (ldx elements between rows); gamma/beta bf16 [K]
+ * (NULL when unused).  x_tensor_scale: device pointer to one float (static per-tensor scale,
+ * P:394) or NULL = dynamic per-row scale amax_row/2688 (NVFP4 only; ignored otherwise).
+ *   sp_codes  [T, K/4]  bytes  survivors' FP4 codes, ascending k (Eq. 7)
+ *   sp_sf     [T, K/32] bytes  backbone block scales           (HiF4: [T, K/64] uint32)
+ *   sp_meta   [T, K/16] bytes  one nibble i0|i1<<2 per 8-chunk (MASK_24: [T, K/8], per 4)
+ *   dn_codes  [T, K/2]  bytes  residual FP4 codes of R = X - D_sp(Q_sp(X_sp)) (Eq. 8)
+ *   dn_sf     [T, K/16] bytes  residual block scales (MXFP4: [T,K/32]; HiF4: [T,K/64] uint32)
+ *   row_scale [T] float        the tensor scale each row was quantized with (1 for MXFP4/HiF4)
+ * sp_sf, sp_meta, dn_sf follow cfg->layout. */
+sharq_status sharq_prepare(const sharq_config* cfg, const void* x, int64_t T, int64_t K,
+                           int64_t ldx, const void* gamma, const void* beta,
+                           const float* x_tensor_scale, void* sp_codes, void* sp_sf,
+                           void* sp_meta, void* dn_codes, void* dn_sf, float* row_scale,
+                           void* stream);
+
+/* ---- sharq_linear (Eq. 9) -----------------------------------------------
+ * Y[T,D] = (A_sp . W^T through the sparse view  +  A_dn . W^T through the dense view)
+ *          * row_scale[t] * w_tensor_scale  (+ bias[d])
+ * Inputs are the outputs of sharq_prepare and sharq_quantize_weight made with the SAME config
+ * and layout == SHARQ_LAYOUT_TILED (otherwise SHARQ_EINVAL).  Both GEMMs accumulate into the
+ * same TMEM tile in one kernel ("accumulates directly into this output").
+ * out_dtype: 0 = bf16, 1 = fp32.  bias bf16 [D] or NULL.  ldy in elements.
+ * path: 0 = sparse + dense (SharQ), 1 = sparse only, 2 = dense only (Table 5 rows). */
+sharq_status sharq_linear(const sharq_config* cfg, int64_t T, int64_t D, int64_t K,
+                          const void* sp_codes, const void* sp_sf, const void* sp_meta,
+                          const void* dn_codes, const void* dn_sf, const float* row_scale,
+                          const void* w_codes, const void* w_sf_sparse_view,
+                          const void* w_sf_dense_view, const float* w_tensor_scale,
+                          const void* bias, void* Y, int64_t ldy, int32_t out_dtype, int32_t path,
+                          void* workspace, size_t workspace_bytes, void* stream);
+
+/* ---- sharq_linear_grouped (MoE expert linears) -----------------------------
+ * E experts; `offsets` is a HOST int32[E+1] array: rows [offsets[e], offsets[e+1]) of the
+ * activation tensors belong to expert e.  Every expert's row range must start at a multiple of
+ * 128 in the TILED scale/metadata arrays, i.e. the caller prepares each expert's rows with
+ * sharq_prepare into a 128-row-aligned slot: row r of expert e lives at padded row
+ * pad_offsets[e] + r with pad_offsets[e] = sum_{j<e} roundup(count_j, 128).  Weight tensors are
+ * stacked [E, ...] (each expert's tensors laid out as sharq_quantize_weight writes them);
+ * w_tensor_scale is float[E].  Empty experts are skipped.  Y is [sum roundup(count,128), D]
+ * in the same padded row numbering. */
+sharq_status sharq_linear_grouped(const sharq_config* cfg, int32_t E, const int32_t* offsets_host,
+                                  int64_t D, int64_t K, const void* sp_codes, const void* sp_sf,
+                                  const void* sp_meta, const void* dn_codes, const void* dn_sf,
+                                  const float* row_scale, const void* w_codes,
+                                  const void* w_sf_sparse_view, const void* w_sf_dense_view,
+                                  const float* w_tensor_scale, void* Y, int64_t ldy,
+                                  int32_t out_dtype, void* workspace, size_t workspace_bytes,
+                                  void* stream);
+
+/* Library / build information: returns a static string, e.g. "sharq-b200 0.1 sm_100a". */
+const char* sharq_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SHARQ_H_ */

@@ -1,0 +1,190 @@
+"""Thin Python binding of libsharq.so (include/sharq.h).  Argument marshalling only: every step of
+the SharQ hot path runs in the CUDA kernels behind the C ABI.  PyTorch is used here for device
+memory and streams, nothing else.  There is no CPU fallback: a missing library raises.
+
+Low level  : `capi.sharq_prepare(...)` etc. -- the raw ctypes functions, same names as the header.
+Convenience: `quantize_weight`, `prepare`, `linear`, `linear_grouped` -- allocate the output tensors
+             with the sizes the library reports, pass raw pointers + the current stream.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from ctypes import POINTER, c_char_p, c_float, c_int32, c_int64, c_size_t, c_void_p
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libsharq.so")
+
+OK, EINVAL, ESHAPE, EWORKSPACE, EARCH, ECUDA = range(6)
+NVFP4, MXFP4, HIF4 = 0, 1, 2
+MASK_PAIR48, MASK_24 = 0, 1
+NORM_NONE, NORM_RMS, NORM_LAYER = 0, 1, 2
+LAYOUT_CANONICAL, LAYOUT_TILED = 0, 1
+PATH_SHARQ, PATH_SPARSE_ONLY, PATH_DENSE_ONLY = 0, 1, 2
+_STATUS = {0: "SHARQ_OK", 1: "SHARQ_EINVAL", 2: "SHARQ_ESHAPE", 3: "SHARQ_EWORKSPACE", 4: "SHARQ_EARCH",
+           5: "SHARQ_ECUDA"}
+
+
+class SharqError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        super().__init__(f"{where} returned {_STATUS.get(status, status)}")
+        self.status = status
+
+
+class Config(ctypes.Structure):
+    _fields_ = [("fmt", c_int32), ("mask", c_int32), ("norm", c_int32), ("eps", c_float), ("layout", c_int32)]
+
+
+def make_config(fmt=NVFP4, norm=NORM_RMS, eps=1e-6, layout=LAYOUT_TILED, mask=None) -> Config:
+    if mask is None:
+        mask = MASK_24 if fmt == HIF4 else MASK_PAIR48
+    if fmt == HIF4:
+        layout = LAYOUT_CANONICAL
+    return Config(fmt, mask, norm, eps, layout)
+
+
+def _load() -> ctypes.CDLL:
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(f"{LIB_PATH} is missing: run `python -c 'import __graft_entry__ as g; g.build()'` "
+                          "(there is no fallback path)")
+    lib = ctypes.CDLL(LIB_PATH)
+    P, SZ = c_void_p, POINTER(c_size_t)
+    CFG = POINTER(Config)
+    lib.sharq_version.restype = c_char_p
+    lib.sharq_version.argtypes = []
+    lib.sharq_weight_sizes.argtypes = [CFG, c_int64, c_int64, SZ, SZ, SZ, SZ]
+    lib.sharq_act_sizes.argtypes = [CFG, c_int64, c_int64, SZ, SZ, SZ, SZ, SZ, SZ]
+    lib.sharq_linear_workspace.argtypes = [CFG, c_int64, c_int64, c_int64, c_int32, SZ]
+    lib.sharq_quantize_weight.argtypes = [CFG, P, c_int64, c_int64, c_int64, P, P, P, P, P, c_size_t, P]
+    lib.sharq_prepare.argtypes = [CFG, P, c_int64, c_int64, c_int64, P, P, P, P, P, P, P, P, P, P]
+    lib.sharq_linear.argtypes = [CFG, c_int64, c_int64, c_int64, P, P, P, P, P, P, P, P, P, P, P, P, c_int64,
+                                 c_int32, c_int32, P, c_size_t, P]
+    lib.sharq_linear_grouped.argtypes = [CFG, c_int32, POINTER(c_int32), c_int64, c_int64, P, P, P, P, P, P, P, P,
+                                         P, P, P, c_int64, c_int32, P, c_size_t, P]
+    for name in ("sharq_weight_sizes", "sharq_act_sizes", "sharq_linear_workspace", "sharq_quantize_weight",
+                 "sharq_prepare", "sharq_linear", "sharq_linear_grouped"):
+        getattr(lib, name).restype = c_int32
+    return lib
+
+
+capi = _load()
+EXPORTS = ("sharq_version", "sharq_weight_sizes", "sharq_act_sizes", "sharq_linear_workspace",
+           "sharq_quantize_weight", "sharq_prepare", "sharq_linear", "sharq_linear_grouped")
+
+
+def version() -> str:
+    return capi.sharq_version().decode()
+
+
+def _check(status: int, where: str):
+    if status != OK:
+        raise SharqError(status, where)
+
+
+def _ptr(t):
+    if t is None:
+        return None
+    if isinstance(t, int):
+        return t
+    return t.data_ptr()
+
+
+def _stream():
+    import torch
+    return torch.cuda.current_stream().cuda_stream
+
+
+def weight_sizes(cfg: Config, D: int, K: int):
+    s = [c_size_t() for _ in range(4)]
+    _check(capi.sharq_weight_sizes(ctypes.byref(cfg), D, K, *[ctypes.byref(v) for v in s]), "sharq_weight_sizes")
+    return tuple(v.value for v in s)
+
+
+def act_sizes(cfg: Config, T: int, K: int):
+    s = [c_size_t() for _ in range(6)]
+    _check(capi.sharq_act_sizes(ctypes.byref(cfg), T, K, *[ctypes.byref(v) for v in s]), "sharq_act_sizes")
+    return tuple(v.value for v in s)
+
+
+def linear_workspace(cfg: Config, T: int, D: int, K: int, E: int = 0) -> int:
+    s = c_size_t()
+    _check(capi.sharq_linear_workspace(ctypes.byref(cfg), T, D, K, E, ctypes.byref(s)), "sharq_linear_workspace")
+    return s.value
+
+
+def _bytes(n, device):
+    import torch
+    return torch.empty(max(int(n), 16), dtype=torch.uint8, device=device)
+
+
+def quantize_weight(cfg: Config, W):
+    """W: torch bf16 [D, K] on cuda.  Returns dict(codes, sf_sp, sf_dn, ts_w, D, K) of device tensors."""
+    import torch
+    D, K = W.shape
+    n_codes, n_sp, n_dn, n_ws = weight_sizes(cfg, D, K)
+    dev = W.device
+    out = dict(codes=_bytes(n_codes, dev), sf_sp=_bytes(n_sp, dev), sf_dn=_bytes(n_dn, dev),
+               ts_w=torch.empty(1, dtype=torch.float32, device=dev), D=D, K=K)
+    ws = _bytes(n_ws, dev)
+    _check(capi.sharq_quantize_weight(ctypes.byref(cfg), _ptr(W), D, K, W.stride(0), _ptr(out["codes"]),
+                                      _ptr(out["sf_sp"]), _ptr(out["sf_dn"]), _ptr(out["ts_w"]), _ptr(ws), n_ws,
+                                      _stream()), "sharq_quantize_weight")
+    return out
+
+
+def alloc_act(cfg: Config, T: int, K: int, device):
+    import torch
+    n = act_sizes(cfg, T, K)
+    return dict(sp_codes=_bytes(n[0], device), sp_sf=_bytes(n[1], device), sp_meta=_bytes(n[2], device),
+                dn_codes=_bytes(n[3], device), dn_sf=_bytes(n[4], device),
+                row_scale=torch.empty(max(T, 1), dtype=torch.float32, device=device), T=T, K=K)
+
+
+def prepare(cfg: Config, x, gamma=None, beta=None, x_tensor_scale=None, out=None):
+    """x: torch bf16 [T, K] on cuda; gamma/beta bf16 [K]; x_tensor_scale: 1-element fp32 tensor or None."""
+    T, K = x.shape
+    if out is None:
+        out = alloc_act(cfg, T, K, x.device)
+    _check(capi.sharq_prepare(ctypes.byref(cfg), _ptr(x), T, K, x.stride(0), _ptr(gamma), _ptr(beta),
+                              _ptr(x_tensor_scale), _ptr(out["sp_codes"]), _ptr(out["sp_sf"]), _ptr(out["sp_meta"]),
+                              _ptr(out["dn_codes"]), _ptr(out["dn_sf"]), _ptr(out["row_scale"]), _stream()),
+           "sharq_prepare")
+    return out
+
+
+def linear(cfg: Config, act: dict, wq: dict, bias=None, out_dtype="bf16", path=PATH_SHARQ, Y=None, workspace=None):
+    import torch
+    T, K, D = act["T"], act["K"], wq["D"]
+    dev = act["sp_codes"].device
+    if Y is None:
+        Y = torch.empty((T, D), dtype=torch.bfloat16 if out_dtype == "bf16" else torch.float32, device=dev)
+    n_ws = linear_workspace(cfg, T, D, K)
+    if workspace is None and n_ws:
+        workspace = _bytes(n_ws, dev)
+    _check(capi.sharq_linear(ctypes.byref(cfg), T, D, K, _ptr(act["sp_codes"]), _ptr(act["sp_sf"]),
+                             _ptr(act["sp_meta"]), _ptr(act["dn_codes"]), _ptr(act["dn_sf"]), _ptr(act["row_scale"]),
+                             _ptr(wq["codes"]), _ptr(wq["sf_sp"]), _ptr(wq["sf_dn"]), _ptr(wq["ts_w"]), _ptr(bias),
+                             _ptr(Y), Y.stride(0), 0 if Y.dtype == torch.bfloat16 else 1, path, _ptr(workspace), n_ws,
+                             _stream()), "sharq_linear")
+    return Y
+
+
+def linear_grouped(cfg: Config, offsets, act: dict, wq: dict, D: int, out_dtype="bf16", Y=None, workspace=None):
+    """offsets: host int32 sequence [E+1]; act tensors hold the 128-row-padded expert slots (sharq.h)."""
+    import torch
+    E = len(offsets) - 1
+    K = act["K"]
+    dev = act["sp_codes"].device
+    offs = (c_int32 * (E + 1))(*[int(o) for o in offsets])
+    padded = sum(-(-(int(offsets[e + 1]) - int(offsets[e])) // 128) * 128 for e in range(E))
+    if Y is None:
+        Y = torch.zeros((max(padded, 1), D), dtype=torch.bfloat16 if out_dtype == "bf16" else torch.float32, device=dev)
+    n_ws = linear_workspace(cfg, int(offsets[-1]), D, K, E)
+    if workspace is None:
+        workspace = _bytes(n_ws, dev)
+    _check(capi.sharq_linear_grouped(ctypes.byref(cfg), E, offs, D, K, _ptr(act["sp_codes"]), _ptr(act["sp_sf"]),
+                                     _ptr(act["sp_meta"]), _ptr(act["dn_codes"]), _ptr(act["dn_sf"]),
+                                     _ptr(act["row_scale"]), _ptr(wq["codes"]), _ptr(wq["sf_sp"]), _ptr(wq["sf_dn"]),
+                                     _ptr(wq["ts_w"]), _ptr(Y), Y.stride(0), 0 if Y.dtype == torch.bfloat16 else 1,
+                                     _ptr(workspace), n_ws, _stream()), "sharq_linear_grouped")
+    return Y

@@ -1,0 +1,203 @@
+// C ABI of libsharq.so (include/sharq.h): argument validation, size queries, dispatch.
+// All compute is in prepare.cu / linear.cu; there is no CPU fallback anywhere.
+#include <cuda_runtime.h>
+
+#include "common.cuh"
+
+namespace sharq {
+cudaError_t launch_prepare(const sharq_config* cfg, const void* x, int64_t T, int64_t K, int64_t ldx,
+                           const void* gamma, const void* beta, const float* x_ts, void* sp_codes, void* sp_sf,
+                           void* sp_meta, void* dn_codes, void* dn_sf, float* row_scale, int num_sms,
+                           cudaStream_t st);
+cudaError_t launch_quantize_weight(const sharq_config* cfg, const void* W, int64_t D, int64_t K, int64_t ldw,
+                                   void* codes, void* sf_sp, void* sf_dn, float* ts, void* workspace,
+                                   cudaStream_t st);
+struct LinearArgs {
+  int64_t T, D, K;              // T = rows of this problem (per expert for grouped)
+  const void *sp_codes, *sp_sf, *sp_meta, *dn_codes, *dn_sf;
+  const float* row_scale;
+  const void *w_codes, *w_sf_sp, *w_sf_dn;
+  const float* w_ts;
+  const void* bias;
+  void* Y; int64_t ldy; int out_dtype; int path;
+};
+sharq_status launch_linear(const sharq_config* cfg, const LinearArgs& a, int32_t E, const int32_t* offsets_host,
+                           void* workspace, size_t workspace_bytes, int num_sms, cudaStream_t st);
+size_t linear_workspace_bytes(const sharq_config* cfg, int64_t T, int64_t D, int64_t K, int32_t E);
+}  // namespace sharq
+
+using namespace sharq;
+
+namespace {
+
+bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+sharq_status check_cfg(const sharq_config* cfg) {
+  if (!cfg) return SHARQ_EINVAL;
+  if (cfg->fmt < 0 || cfg->fmt > 2 || cfg->mask < 0 || cfg->mask > 1 || cfg->norm < 0 || cfg->norm > 2 ||
+      cfg->layout < 0 || cfg->layout > 1)
+    return SHARQ_EINVAL;
+  // the block-scaled FP4 sparse MMA only takes the pairwise pattern; HiF4 uses the standard 2:4
+  if (cfg->fmt == SHARQ_HIF4 ? cfg->mask != SHARQ_MASK_24 : cfg->mask != SHARQ_MASK_PAIR48) return SHARQ_EINVAL;
+  if (cfg->fmt == SHARQ_HIF4 && cfg->layout != SHARQ_LAYOUT_CANONICAL) return SHARQ_EINVAL;
+  return SHARQ_OK;
+}
+
+struct DeviceInfo { int ok; int sms; int major; };
+sharq_status device_info(DeviceInfo* out) {
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) return SHARQ_ECUDA;
+  int major = 0, sms = 0;
+  if (cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess) return SHARQ_ECUDA;
+  if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return SHARQ_ECUDA;
+  if (major != 10) return SHARQ_EARCH;
+  out->ok = 1; out->sms = sms; out->major = major;
+  return SHARQ_OK;
+}
+
+int64_t sf_cols(int fmt, bool dense_group, int64_t K) {
+  if (fmt == SHARQ_HIF4) return K / 64 * 4;                       // uint32 words, in bytes
+  if (fmt == SHARQ_NVFP4 && dense_group) return K / 16;
+  return K / 32;
+}
+size_t sf_bytes(const sharq_config* cfg, int64_t rows, int64_t cols_bytes) {
+  return (size_t)((cfg->layout == SHARQ_LAYOUT_TILED) ? round_up(rows, 128) : rows) * (size_t)cols_bytes;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* sharq_version(void) { return "sharq-b200 0.1 sm_100a"; }
+
+sharq_status sharq_weight_sizes(const sharq_config* cfg, int64_t D, int64_t K, size_t* codes, size_t* sf_sparse_view,
+                                size_t* sf_dense_view, size_t* workspace) {
+  sharq_status s = check_cfg(cfg);
+  if (s != SHARQ_OK) return s;
+  if (D < 0 || K <= 0 || K % 256 != 0) return SHARQ_ESHAPE;
+  if (codes) *codes = (size_t)D * (size_t)(K / 2);
+  if (sf_sparse_view) *sf_sparse_view = sf_bytes(cfg, D, sf_cols(cfg->fmt, false, K));
+  if (sf_dense_view) *sf_dense_view = sf_bytes(cfg, D, sf_cols(cfg->fmt, true, K));
+  if (workspace) *workspace = 256;
+  return SHARQ_OK;
+}
+
+sharq_status sharq_act_sizes(const sharq_config* cfg, int64_t T, int64_t K, size_t* sp_codes, size_t* sp_sf,
+                             size_t* sp_meta, size_t* dn_codes, size_t* dn_sf, size_t* row_scale) {
+  sharq_status s = check_cfg(cfg);
+  if (s != SHARQ_OK) return s;
+  if (T < 0 || K <= 0 || K % 256 != 0) return SHARQ_ESHAPE;
+  if (sp_codes) *sp_codes = (size_t)T * (size_t)(K / 4);
+  if (sp_sf) *sp_sf = sf_bytes(cfg, T, sf_cols(cfg->fmt, false, K));
+  if (sp_meta) *sp_meta = sf_bytes(cfg, T, cfg->mask == SHARQ_MASK_24 ? K / 8 : K / 16);
+  if (dn_codes) *dn_codes = (size_t)T * (size_t)(K / 2);
+  if (dn_sf) *dn_sf = sf_bytes(cfg, T, sf_cols(cfg->fmt, true, K));
+  if (row_scale) *row_scale = (size_t)T * sizeof(float);
+  return SHARQ_OK;
+}
+
+sharq_status sharq_linear_workspace(const sharq_config* cfg, int64_t T, int64_t D, int64_t K, int32_t E,
+                                    size_t* workspace) {
+  sharq_status s = check_cfg(cfg);
+  if (s != SHARQ_OK) return s;
+  if (T < 0 || D <= 0 || D % 128 != 0 || K <= 0 || K % 256 != 0 || E < 0) return SHARQ_ESHAPE;
+  if (workspace) *workspace = linear_workspace_bytes(cfg, T, D, K, E);
+  return SHARQ_OK;
+}
+
+sharq_status sharq_quantize_weight(const sharq_config* cfg, const void* W, int64_t D, int64_t K, int64_t ldw,
+                                   void* codes, void* sf_sparse_view, void* sf_dense_view, float* tensor_scale,
+                                   void* workspace, size_t workspace_bytes, void* stream) {
+  sharq_status s = check_cfg(cfg);
+  if (s != SHARQ_OK) return s;
+  if (D < 0 || K <= 0 || K % 256 != 0 || ldw < K || ldw % 8 != 0) return SHARQ_ESHAPE;
+  if (!W || !codes || !sf_sparse_view || !sf_dense_view || !tensor_scale || !workspace) return SHARQ_EINVAL;
+  if (!aligned16(W) || !aligned16(codes) || !aligned16(sf_sparse_view) || !aligned16(sf_dense_view) ||
+      !aligned16(workspace))
+    return SHARQ_EINVAL;
+  if (workspace_bytes < 256) return SHARQ_EWORKSPACE;
+  DeviceInfo di{};
+  if ((s = device_info(&di)) != SHARQ_OK) return s;
+  if (D == 0) return SHARQ_OK;
+  cudaError_t e = launch_quantize_weight(cfg, W, D, K, ldw, codes, sf_sparse_view, sf_dense_view, tensor_scale,
+                                         workspace, (cudaStream_t)stream);
+  return e == cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
+}
+
+sharq_status sharq_prepare(const sharq_config* cfg, const void* x, int64_t T, int64_t K, int64_t ldx,
+                           const void* gamma, const void* beta, const float* x_tensor_scale, void* sp_codes,
+                           void* sp_sf, void* sp_meta, void* dn_codes, void* dn_sf, float* row_scale, void* stream) {
+  sharq_status s = check_cfg(cfg);
+  if (s != SHARQ_OK) return s;
+  if (T < 0 || K <= 0 || K % 256 != 0 || ldx < K || ldx % 8 != 0) return SHARQ_ESHAPE;
+  if (T == 0) return SHARQ_OK;
+  if (!x || !sp_codes || !sp_sf || !sp_meta || !dn_codes || !dn_sf || !row_scale) return SHARQ_EINVAL;
+  if (cfg->norm != SHARQ_NORM_NONE && !gamma) return SHARQ_EINVAL;
+  if (!aligned16(x) || !aligned16(sp_codes) || !aligned16(sp_sf) || !aligned16(sp_meta) || !aligned16(dn_codes) ||
+      !aligned16(dn_sf) || (gamma && !aligned16(gamma)) || (beta && !aligned16(beta)))
+    return SHARQ_EINVAL;
+  if (K > 100 * 1024) return SHARQ_ESHAPE;   // one row must fit in shared memory
+  DeviceInfo di{};
+  if ((s = device_info(&di)) != SHARQ_OK) return s;
+  cudaError_t e = launch_prepare(cfg, x, T, K, ldx, gamma, beta, x_tensor_scale, sp_codes, sp_sf, sp_meta, dn_codes,
+                                 dn_sf, row_scale, di.sms, (cudaStream_t)stream);
+  return e == cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
+}
+
+static sharq_status check_linear(const sharq_config* cfg, int64_t D, int64_t K, const void* const* ptrs, int n,
+                                 int64_t ldy, int32_t out_dtype, int32_t path) {
+  sharq_status s = check_cfg(cfg);
+  if (s != SHARQ_OK) return s;
+  if (cfg->layout != SHARQ_LAYOUT_TILED && cfg->fmt != SHARQ_HIF4) return SHARQ_EINVAL;
+  if (D <= 0 || D % 128 != 0 || K <= 0 || K % 256 != 0 || ldy < D || ldy % 8 != 0) return SHARQ_ESHAPE;
+  if (out_dtype < 0 || out_dtype > 1 || path < 0 || path > 2) return SHARQ_EINVAL;
+  for (int i = 0; i < n; ++i)
+    if (!ptrs[i] || !aligned16(ptrs[i])) return SHARQ_EINVAL;
+  return SHARQ_OK;
+}
+
+sharq_status sharq_linear(const sharq_config* cfg, int64_t T, int64_t D, int64_t K, const void* sp_codes,
+                          const void* sp_sf, const void* sp_meta, const void* dn_codes, const void* dn_sf,
+                          const float* row_scale, const void* w_codes, const void* w_sf_sparse_view,
+                          const void* w_sf_dense_view, const float* w_tensor_scale, const void* bias, void* Y,
+                          int64_t ldy, int32_t out_dtype, int32_t path, void* workspace, size_t workspace_bytes,
+                          void* stream) {
+  const void* ptrs[] = {sp_codes, sp_sf, sp_meta, dn_codes, dn_sf, w_codes, w_sf_sparse_view, w_sf_dense_view, Y};
+  sharq_status s = check_linear(cfg, D, K, ptrs, 9, ldy, out_dtype, path);
+  if (s != SHARQ_OK) return s;
+  if (T < 0) return SHARQ_ESHAPE;
+  if (T == 0) return SHARQ_OK;
+  if (!row_scale || !w_tensor_scale) return SHARQ_EINVAL;
+  if (workspace_bytes < linear_workspace_bytes(cfg, T, D, K, 0)) return SHARQ_EWORKSPACE;
+  DeviceInfo di{};
+  if ((s = device_info(&di)) != SHARQ_OK) return s;
+  LinearArgs a{T, D, K, sp_codes, sp_sf, sp_meta, dn_codes, dn_sf, row_scale, w_codes, w_sf_sparse_view,
+               w_sf_dense_view, w_tensor_scale, bias, Y, ldy, out_dtype, path};
+  return launch_linear(cfg, a, 0, nullptr, workspace, workspace_bytes, di.sms, (cudaStream_t)stream);
+}
+
+sharq_status sharq_linear_grouped(const sharq_config* cfg, int32_t E, const int32_t* offsets_host, int64_t D,
+                                  int64_t K, const void* sp_codes, const void* sp_sf, const void* sp_meta,
+                                  const void* dn_codes, const void* dn_sf, const float* row_scale,
+                                  const void* w_codes, const void* w_sf_sparse_view, const void* w_sf_dense_view,
+                                  const float* w_tensor_scale, void* Y, int64_t ldy, int32_t out_dtype,
+                                  void* workspace, size_t workspace_bytes, void* stream) {
+  const void* ptrs[] = {sp_codes, sp_sf, sp_meta, dn_codes, dn_sf, w_codes, w_sf_sparse_view, w_sf_dense_view, Y};
+  sharq_status s = check_linear(cfg, D, K, ptrs, 9, ldy, out_dtype, 0);
+  if (s != SHARQ_OK) return s;
+  if (E <= 0 || !offsets_host) return SHARQ_EINVAL;
+  if (cfg->fmt == SHARQ_HIF4) return SHARQ_EINVAL;
+  for (int32_t e = 0; e < E; ++e)
+    if (offsets_host[e + 1] < offsets_host[e]) return SHARQ_ESHAPE;
+  if (offsets_host[0] != 0) return SHARQ_ESHAPE;
+  if (!row_scale || !w_tensor_scale) return SHARQ_EINVAL;
+  if (workspace_bytes < linear_workspace_bytes(cfg, offsets_host[E], D, K, E)) return SHARQ_EWORKSPACE;
+  if (!workspace && linear_workspace_bytes(cfg, offsets_host[E], D, K, E) > 0) return SHARQ_EINVAL;
+  DeviceInfo di{};
+  if ((s = device_info(&di)) != SHARQ_OK) return s;
+  LinearArgs a{0, D, K, sp_codes, sp_sf, sp_meta, dn_codes, dn_sf, row_scale, w_codes, w_sf_sparse_view,
+               w_sf_dense_view, w_tensor_scale, nullptr, Y, ldy, out_dtype, 0};
+  return launch_linear(cfg, a, E, offsets_host, workspace, workspace_bytes, di.sms, (cudaStream_t)stream);
+}
+
+}  // extern "C"

@@ -1,0 +1,64 @@
+"""The C-ABI library loads, exports every symbol include/sharq.h declares, and its host-only logic
+(size queries, argument validation) behaves as the header says.  No compute calls (no GPU needed)."""
+import ctypes
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def sq():
+    import __graft_entry__ as g
+    g.build()
+    import paper_2606_26587_b200 as pkg
+    return pkg
+
+
+def test_every_declared_symbol_is_exported(sq):
+    header = open(os.path.join(ROOT, "include", "sharq.h")).read()
+    declared = set(re.findall(r"\b(sharq_[a-z_]+)\s*\(", header))
+    assert declared == set(sq.EXPORTS)
+    for name in declared:
+        assert getattr(sq.capi, name) is not None
+    assert sq.version().startswith("sharq-b200")
+
+
+def test_sizes_follow_the_header(sq):
+    cfg = sq.make_config(sq.NVFP4, layout=sq.LAYOUT_CANONICAL)
+    T, K, D = 16, 4096, 6144
+    assert sq.act_sizes(cfg, T, K) == (T * K // 4, T * K // 32, T * K // 16, T * K // 2, T * K // 16, T * 4)
+    assert sq.weight_sizes(cfg, D, K)[:3] == (D * K // 2, D * K // 32, D * K // 16)
+    cfg_t = sq.make_config(sq.NVFP4, layout=sq.LAYOUT_TILED)
+    assert sq.act_sizes(cfg_t, T, K) == (T * K // 4, 128 * K // 32, 128 * K // 16, T * K // 2, 128 * K // 16, T * 4)
+    # per element: 2 B in + 0.25 + 0.0625 + 0.03125 + 0.5 + 0.0625 out = 2.906 B (DESIGN.md roofline unit)
+    n = sq.act_sizes(cfg, 128, 4096)
+    assert (sum(n[:5]) + 2 * 128 * 4096) / (128 * 4096) == 2.90625
+    cfg_m = sq.make_config(sq.MXFP4, layout=sq.LAYOUT_CANONICAL)
+    assert sq.act_sizes(cfg_m, T, K)[4] == T * K // 32
+    cfg_h = sq.make_config(sq.HIF4)
+    assert sq.act_sizes(cfg_h, T, K) == (T * K // 4, T * K // 16, T * K // 8, T * K // 2, T * K // 16, T * 4)
+
+
+def test_argument_validation_returns_codes_without_touching_cuda(sq):
+    cfg = sq.make_config(sq.NVFP4)
+    null = ctypes.c_void_p(0)
+    f = sq.capi.sharq_prepare
+    # K not a multiple of 256
+    assert f(ctypes.byref(cfg), 16, 4, 1000, 1000, *([16] * 9), null) == sq.ESHAPE
+    # T == 0 is OK and launches nothing
+    assert f(ctypes.byref(cfg), 16, 0, 1024, 1024, *([16] * 9), null) == sq.OK
+    # null output pointer
+    assert f(ctypes.byref(cfg), 16, 4, 1024, 1024, 16, null, null, null, 16, 16, 16, 16, 16, null) == sq.EINVAL
+    # misaligned pointer
+    assert f(ctypes.byref(cfg), 8, 4, 1024, 1024, 16, null, null, 16, 16, 16, 16, 16, 16, null) == sq.EINVAL
+    # element-wise 2:4 with NVFP4 has no tensor-core path on B200 (R2)
+    bad = sq.Config(sq.NVFP4, sq.MASK_24, sq.NORM_NONE, 1e-6, sq.LAYOUT_TILED)
+    with pytest.raises(sq.SharqError):
+        sq.act_sizes(bad, 16, 1024)
+    with pytest.raises(sq.SharqError):
+        sq.act_sizes(cfg, 16, 1000)
+    with pytest.raises(sq.SharqError):
+        sq.linear_workspace(cfg, 16, 100, 1024)          # D % 128

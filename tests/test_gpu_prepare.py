@@ -1,0 +1,111 @@
+"""GPU parity: sharq_prepare and sharq_quantize_weight through the C ABI vs the oracle, bit-exact
+(masks/metadata, packed codes, scale bytes, row scales).  BASELINE.json: "must match bit-exactly"."""
+import numpy as np
+import pytest
+import torch
+
+import sharq_inputs as si
+from oracle import sharq_oracle as so
+from tests.gpu_util import act_to_canonical, to_dev, weight_to_canonical
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def sq():
+    import __graft_entry__ as g
+    g.build()
+    import paper_2606_26587_b200 as pkg
+    return pkg
+
+
+def _compare_act(got, p, what=""):
+    for key in ("sp_meta", "sp_sf", "sp_codes", "dn_sf", "dn_codes"):
+        eq = got[key] == p[key]
+        assert eq.all(), f"{what} {key}: {np.count_nonzero(~eq)} of {eq.size} differ, first at {np.argwhere(~eq)[:3].tolist()}"
+    assert np.array_equal(got["ts"].view(np.uint32), p["ts"].view(np.uint32)), f"{what} row_scale"
+
+
+CASES = [
+    # (fmt, norm, layout, T, K, outlier_mult)   K spans several 1024-blocks and ragged tails (768, 3584)
+    (0, 1, 0, 16, 4096, 50.0), (0, 1, 1, 16, 4096, 50.0), (0, 0, 1, 37, 14336, 50.0), (0, 1, 0, 5, 768, 10.0),
+    (0, 1, 1, 130, 3584, 200.0), (0, 2, 0, 9, 2048, 50.0), (0, 0, 0, 1, 256, 50.0), (0, 1, 0, 300, 1024, 50.0),
+    (1, 1, 0, 16, 4096, 50.0), (1, 0, 1, 33, 3584, 200.0), (1, 2, 0, 7, 768, 10.0), (1, 1, 1, 129, 18944, 50.0),
+    (2, 1, 0, 16, 4096, 50.0), (2, 0, 0, 33, 3584, 200.0), (2, 2, 0, 7, 768, 10.0), (2, 1, 0, 3, 18944, 50.0),
+]
+
+
+@pytest.mark.parametrize("fmt,norm,layout,T,K,mult", CASES)
+def test_prepare_bit_exact(sq, fmt, norm, layout, T, K, mult):
+    x = si.activations(T, K, config=1, outlier_mult=mult, extra=K + T)
+    g, b = si.gamma(K, 1), si.beta(K, 1)
+    cfg = sq.make_config(fmt, norm, 1e-6, layout)
+    act = sq.prepare(cfg, to_dev(x), to_dev(g) if norm else None, to_dev(b) if norm == 2 else None)
+    torch.cuda.synchronize()
+    p = so.prepare(x, fmt=fmt, mask=cfg.mask, norm=norm, gamma_u16=g, beta_u16=b if norm == 2 else None)
+    _compare_act(act_to_canonical(sq, cfg, act, T, K), p, f"fmt{fmt} norm{norm} T{T} K{K}")
+
+
+def test_prepare_edge_cases(sq):
+    """zero rows, -0 / tiny values, exact ties, huge dynamic range, static tensor scale, strided input."""
+    T, K = 12, 1024
+    x = si.activations(T, K, config=1)
+    xf = si.bf16_bits_to_f32(x).copy()
+    xf[0] = 0.0
+    xf[1] = -0.0
+    xf[2] = 1.0                                   # every pair ties
+    xf[3, ::2] = -3.0; xf[3, 1::2] = 3.0
+    xf[4] *= 1e-30
+    xf[5] *= 1e30
+    xf[6, :512] = 0.0
+    xf[7] = np.where(np.arange(K) % 8 < 4, 5.0, -5.0)
+    x = si.to_bf16_bits(xf)
+    x[1] = 0x8000
+    for fmt in (0, 1, 2):
+        cfg = sq.make_config(fmt, sq.NORM_NONE, 1e-6, sq.LAYOUT_CANONICAL)
+        act = sq.prepare(cfg, to_dev(x))
+        p = so.prepare(x, fmt=fmt, mask=cfg.mask, norm=so.NORM_NONE)
+        _compare_act(act_to_canonical(sq, cfg, act, T, K), p, f"edge fmt{fmt}")
+    # static per-tensor scale through a device pointer
+    cfg = sq.make_config(0, sq.NORM_RMS, 1e-6, sq.LAYOUT_CANONICAL)
+    g = si.gamma(K, 1)
+    ts = torch.tensor([0.0078125], dtype=torch.float32, device="cuda")
+    act = sq.prepare(cfg, to_dev(x), to_dev(g), x_tensor_scale=ts)
+    p = so.prepare(x, gamma_u16=g, x_tensor_scale=0.0078125)
+    _compare_act(act_to_canonical(sq, cfg, act, T, K), p, "static ts")
+    # leading dimension > K
+    big = torch.zeros((T, K + 64), dtype=torch.bfloat16, device="cuda")
+    big[:, :K] = to_dev(x)
+    act = sq.prepare(cfg, big[:, :K], to_dev(g))
+    p = so.prepare(x, gamma_u16=g)
+    _compare_act(act_to_canonical(sq, cfg, act, T, K), p, "ldx")
+
+
+@pytest.mark.parametrize("fmt,layout,D,K", [(0, 0, 256, 4096), (0, 1, 384, 3584), (1, 1, 128, 768), (1, 0, 200, 1024),
+                                            (2, 0, 256, 4096), (2, 0, 64, 768)])
+def test_quantize_weight_bit_exact(sq, fmt, layout, D, K):
+    w = si.weight(D, K, config=1, extra=D)
+    cfg = sq.make_config(fmt, sq.NORM_NONE, 1e-6, layout)
+    wq = sq.quantize_weight(cfg, to_dev(w))
+    torch.cuda.synchronize()
+    ref = so.quantize_weight(w, fmt)
+    got = weight_to_canonical(sq, cfg, wq, D, K)
+    for key in ("codes", "sf_sp", "sf_dn"):
+        assert np.array_equal(got[key], ref[key]), key
+    assert np.float32(got["ts_w"]) == ref["ts_w"]
+
+
+def test_prepare_full_size_sampled_rows(sq):
+    """BASELINE configs[2] size (T=4096, K=4096 and K=14336) in the bench launch configuration: the
+    oracle recomputes a seeded sample of rows (rows are independent)."""
+    for (T, K, norm) in ((4096, 4096, 1), (2048, 14336, 0)):
+        x = si.activations(T, K, config=3, outlier_mult=200.0)
+        g = si.gamma(K, 3)
+        cfg = sq.make_config(0, norm, 1e-6, sq.LAYOUT_TILED)
+        act = sq.prepare(cfg, to_dev(x), to_dev(g) if norm else None)
+        torch.cuda.synchronize()
+        got = act_to_canonical(sq, cfg, act, T, K)
+        rows = np.random.default_rng(T + K).choice(T, 48, replace=False)
+        rows[:3] = (0, T - 1, T // 2)
+        p = so.prepare(x[rows], norm=norm, gamma_u16=g)
+        _compare_act({k: v[rows] for k, v in got.items()}, p, f"full T{T} K{K}")
