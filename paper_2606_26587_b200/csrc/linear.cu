@@ -1,7 +1,356 @@
-// placeholder replaced below
+// sharq_linear / sharq_linear_grouped (Eq. 9): the sparse backbone GEMM and the dense
+// residual GEMM of one SharQ linear layer, fused in ONE kernel.
+//
+// Per 128 x BN output tile one CTA streams K in blocks of 256 logical elements through a TMA-fed
+// shared-memory ring.  Each W tile is loaded ONCE per k-block and consumed by both paths (P:157
+// "single shared FP4 weight payload"): two tcgen05.mma.sp (K = 128 logical each, compressed A +
+// metadata in tensor memory, one scale per 32 logical k) and four dense block-scaled tcgen05.mma
+// (K = 64 each, one scale per 16) accumulate into the SAME fp32 TMEM tile ("accumulates
+// directly into this output").  Scale factors and metadata arrive in the tcgen05 atom layouts
+// sharq_prepare / sharq_quantize_weight emit (LAYOUT_TILED) so they go HBM -> smem with 1-D bulk
+// copies and smem -> TMEM with tcgen05.cp, no re-formatting.  Epilogue: TMEM -> registers,
+// y = acc * (row_scale[t] * w_tensor_scale) (+ bias), bf16 or fp32 store.
+//
+// Warp roles (192 threads): warp 0 = TMA producer, warp 1 = MMA issuer (one elected lane),
+// warps 2-5 = epilogue (warp w owns TMEM lanes 32*(w%4)..+31); warp 2 also owns the TMEM allocation.
+#include <cuda.h>
+#include <cuda_runtime.h>
+
 #include "common.cuh"
+#include "tc_ptx.cuh"
+
 namespace sharq {
-struct LinearArgs;
-sharq_status launch_linear(const sharq_config*, const LinearArgs&, int32_t, const int32_t*, void*, size_t, int, cudaStream_t) { return SHARQ_EINVAL; }
-size_t linear_workspace_bytes(const sharq_config*, int64_t, int64_t, int64_t, int32_t) { return 0; }
+
+struct LinearArgs {
+  int64_t T, D, K;
+  const void *sp_codes, *sp_sf, *sp_meta, *dn_codes, *dn_sf;
+  const float* row_scale;
+  const void *w_codes, *w_sf_sp, *w_sf_dn;
+  const float* w_ts;
+  const void* bias;
+  void* Y; int64_t ldy; int out_dtype; int path;
+};
+
+namespace {
+
+constexpr int kMaxExperts = 256;
+constexpr int BM = 128;          // rows of an output tile = TMEM lanes
+constexpr int BK = 256;          // logical k per pipeline stage
+constexpr int kThreads = 192;
+constexpr int kTmemCols = 512;
+
+struct GroupInfo {
+  int32_t E;                               // 0: single problem
+  int32_t blk_prefix[kMaxExperts + 1];     // first 128-row block of expert e (padded row numbering)
+  int32_t count[kMaxExperts];              // valid rows of expert e
+};
+
+struct KParams {
+  const uint8_t *sp_sf, *sp_meta, *dn_sf, *w_sf_sp, *w_sf_dn;
+  const float *row_scale, *w_ts;
+  const uint16_t* bias;
+  void* Y;
+  int64_t ldy;
+  int32_t T, D, K, out_fp32, path;
+};
+
+// ---- shared-memory stage layout -------------------------------------------------------------
+template <int BN, int FMT>
+struct Stage {
+  static constexpr int NB = (BN + 127) / 128;                         // 128-row scale atoms of W per tile
+  static constexpr int SF_DN_BYTES = (FMT == SHARQ_NVFP4) ? 2048 : 1024;  // per 128 rows per k-block
+  static constexpr int A_DN = 0;
+  static constexpr int W = A_DN + BM * 128;
+  static constexpr int A_SP = W + BN * 128;
+  static constexpr int META = A_SP + BM * 64;
+  static constexpr int SFA_SP = META + 2048;
+  static constexpr int SFA_DN = SFA_SP + 1024;
+  static constexpr int SFB_SP = SFA_DN + SF_DN_BYTES;
+  static constexpr int SFB_DN = SFB_SP + NB * 1024;
+  static constexpr int RAW = SFB_DN + NB * SF_DN_BYTES;
+  static constexpr int BYTES = (RAW + 1023) / 1024 * 1024;
+  static constexpr int STAGES = (BN > 128) ? 3 : 4;
+  static constexpr int SMEM = STAGES * BYTES + 1024 /*alignment slack*/ + 256 /*barriers*/;
+  // tensor-memory columns
+  static constexpr int SFB_COLS = NB * 4;          // columns one MMA's B scales occupy
+  static constexpr int ACC = 0;
+  static constexpr int E_COL = 256;
+  static constexpr int SFA_SP_COL = 260;           // 2 MMAs x 4
+  static constexpr int SFA_DN_COL = 268;           // 4 MMAs x 4
+  static constexpr int SFB_SP_COL = 284;           // 2 MMAs x SFB_COLS (<= 16)
+  static constexpr int SFB_DN_COL = 300;           // 4 MMAs x SFB_COLS (<= 32)
+};
+
+template <int BN, int FMT>
+__global__ void __launch_bounds__(kThreads, 1)
+sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_constant__ CUtensorMap tm_a_dn,
+                    const __grid_constant__ CUtensorMap tm_w, const KParams p, const __grid_constant__ GroupInfo g) {
+  using S = Stage<BN, FMT>;
+  constexpr bool NV = (FMT == SHARQ_NVFP4);
+  extern __shared__ uint8_t smem_raw[];
+  const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+  const uint32_t bars = smem_base + S::STAGES * S::BYTES;          // full[S], empty[S], tmem_full, tmem_ptr
+  auto full_bar = [&](int s) { return bars + 8u * s; };
+  auto empty_bar = [&](int s) { return bars + 8u * (S::STAGES + s); };
+  const uint32_t tmem_full_bar = bars + 8u * (2 * S::STAGES);
+  const uint32_t tmem_ptr_smem = bars + 8u * (2 * S::STAGES + 1);
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int n_blk = blockIdx.x, m_blk = blockIdx.y;
+  const int num_kb = p.K / BK;
+  const bool do_sp = p.path != 2, do_dn = p.path != 1;
+
+  // ---- which problem does this 128-row block belong to --------------------------------------
+  int expert = 0, rows_valid;
+  if (g.E > 0) {
+    while (expert + 1 < g.E && g.blk_prefix[expert + 1] <= m_blk) ++expert;
+    rows_valid = min(BM, g.count[expert] - (m_blk - g.blk_prefix[expert]) * BM);
+  } else {
+    rows_valid = min(BM, p.T - m_blk * BM);
+  }
+  const int n0 = n_blk * BN;                        // first output feature of the tile
+  const int w_row0 = expert * p.D + n0;             // row in the stacked [E*D, K/2] weight payload
+
+  if (warp == 0 && lane == 0) {
+    tc::prefetch_tmap(&tm_a_sp);
+    tc::prefetch_tmap(&tm_a_dn);
+    tc::prefetch_tmap(&tm_w);
+  }
+  if (warp == 1 && lane == 0) {
+    for (int s = 0; s < S::STAGES; ++s) {
+      tc::mbar_init(full_bar(s), 1);
+      tc::mbar_init(empty_bar(s), 1);
+    }
+    tc::mbar_init(tmem_full_bar, 1);
+    tc::fence_mbar_init();
+  }
+  if (warp == 2) tc::tmem_alloc<kTmemCols>(tmem_ptr_smem);
+  tc::tc_fence_before();
+  __syncthreads();
+  tc::tc_fence_after();
+  uint32_t tmem_base;
+  asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_ptr_smem));
+
+  if (warp == 0) {
+    // =========================== TMA producer ===============================================
+    if (lane == 0) {
+      const uint64_t pol_act = tc::policy_evict_first(), pol_w = tc::policy_evict_last();
+      const int64_t Kc = p.K;
+      const uint8_t* sfa_sp = p.sp_sf + (size_t)m_blk * (Kc / 128) * 512;
+      const uint8_t* sfa_dn = p.dn_sf + (size_t)m_blk * (Kc / 256) * (S::SF_DN_BYTES);
+      const uint8_t* meta = p.sp_meta + (size_t)m_blk * (Kc / 256) * 2048;
+      const int64_t wblk0 = w_row0 / 128;
+      uint32_t tx = BN * 128;
+      if (do_sp) tx += BM * 64 + 2048 + 1024 + S::NB * 1024;
+      if (do_dn) tx += BM * 128 + S::SF_DN_BYTES + S::NB * S::SF_DN_BYTES;
+      for (int kb = 0; kb < num_kb; ++kb) {
+        const int s = kb % S::STAGES;
+        const uint32_t ph = (kb / S::STAGES) & 1;
+        tc::mbar_wait(empty_bar(s), ph ^ 1);
+        const uint32_t st = smem_base + s * S::BYTES;
+        const uint32_t fb = full_bar(s);
+        tc::mbar_expect_tx(fb, tx);
+        tc::tma_load_2d(st + S::W, &tm_w, fb, kb * 128, w_row0, pol_w);
+        if (do_sp) {
+          tc::tma_load_2d(st + S::A_SP, &tm_a_sp, fb, kb * 64, m_blk * BM, pol_act);
+          tc::bulk_load(st + S::META, meta + (size_t)kb * 2048, 2048, fb, pol_act);
+          tc::bulk_load(st + S::SFA_SP, sfa_sp + (size_t)kb * 1024, 1024, fb, pol_act);
+          for (int nb = 0; nb < S::NB; ++nb)
+            tc::bulk_load(st + S::SFB_SP + nb * 1024,
+                          p.w_sf_sp + ((size_t)(wblk0 + nb) * (Kc / 128) + (size_t)kb * 2) * 512, 1024, fb, pol_w);
+        }
+        if (do_dn) {
+          tc::tma_load_2d(st + S::A_DN, &tm_a_dn, fb, kb * 128, m_blk * BM, pol_act);
+          tc::bulk_load(st + S::SFA_DN, sfa_dn + (size_t)kb * S::SF_DN_BYTES, S::SF_DN_BYTES, fb, pol_act);
+          for (int nb = 0; nb < S::NB; ++nb)
+            tc::bulk_load(st + S::SFB_DN + nb * S::SF_DN_BYTES,
+                          p.w_sf_dn + ((size_t)(wblk0 + nb) * (Kc / 256) + (size_t)kb) * S::SF_DN_BYTES,
+                          S::SF_DN_BYTES, fb, pol_w);
+        }
+      }
+    }
+  } else if (warp == 1) {
+    // =========================== MMA issuer =================================================
+    if (lane == 0) {
+      const uint32_t idesc_sp = tc::idesc_fp4(BM, BN, true, !NV, 0, 0);
+      const uint32_t sfb_shift = (BN < 128) ? (uint32_t)((n0 % 128) / 32) : 0u;   // sub-atom N tiles
+      uint32_t accumulate = 0;
+      for (int kb = 0; kb < num_kb; ++kb) {
+        const int s = kb % S::STAGES;
+        const uint32_t ph = (kb / S::STAGES) & 1;
+        tc::mbar_wait(full_bar(s), ph);
+        tc::tc_fence_after();
+        const uint32_t st = smem_base + s * S::BYTES;
+        if (do_sp) {
+          tc::tc_cp_meta(tmem_base + S::E_COL, tc::smem_desc(st + S::META, 128, 0));
+#pragma unroll
+          for (int a = 0; a < 2; ++a) {
+            tc::tc_cp_sf(tmem_base + S::SFA_SP_COL + 4 * a, tc::smem_desc(st + S::SFA_SP + 512 * a, 128, 0));
+#pragma unroll
+            for (int nb = 0; nb < S::NB; ++nb)
+              tc::tc_cp_sf(tmem_base + S::SFB_SP_COL + S::SFB_COLS * a + 4 * nb,
+                           tc::smem_desc(st + S::SFB_SP + nb * 1024 + 512 * a, 128, 0));
+          }
+#pragma unroll
+          for (int j = 0; j < 2; ++j) {
+            tc::mma_sparse(tmem_base + S::ACC, tc::smem_desc(st + S::A_SP + 32 * j, 512, 4),
+                           tc::smem_desc(st + S::W + 64 * j, 1024, 2), idesc_sp, tmem_base + S::SFA_SP_COL + 4 * j,
+                           tmem_base + S::SFB_SP_COL + S::SFB_COLS * j + sfb_shift, tmem_base + S::E_COL + 2 * j,
+                           accumulate);
+            accumulate = 1;
+          }
+        }
+        if (do_dn) {
+          constexpr int ATOMS = NV ? 4 : 2;
+#pragma unroll
+          for (int a = 0; a < ATOMS; ++a) {
+            tc::tc_cp_sf(tmem_base + S::SFA_DN_COL + 4 * a, tc::smem_desc(st + S::SFA_DN + 512 * a, 128, 0));
+#pragma unroll
+            for (int nb = 0; nb < S::NB; ++nb)
+              tc::tc_cp_sf(tmem_base + S::SFB_DN_COL + S::SFB_COLS * a + 4 * nb,
+                           tc::smem_desc(st + S::SFB_DN + nb * S::SF_DN_BYTES + 512 * a, 128, 0));
+          }
+#pragma unroll
+          for (int j = 0; j < 4; ++j) {
+            const int atom = NV ? j : j / 2;                 // MXFP4: two K=64 MMAs share one 4-scale atom
+            const uint32_t sf_id = NV ? 0u : (uint32_t)(j & 1) * 2u;
+            const uint32_t idesc_dn = tc::idesc_fp4(BM, BN, false, !NV, sf_id, sf_id);
+            tc::mma_dense<NV>(tmem_base + S::ACC, tc::smem_desc(st + S::A_DN + 32 * j, 1024, 2),
+                              tc::smem_desc(st + S::W + 32 * j, 1024, 2), idesc_dn,
+                              tmem_base + S::SFA_DN_COL + 4 * atom,
+                              tmem_base + S::SFB_DN_COL + S::SFB_COLS * atom + sfb_shift, accumulate);
+            accumulate = 1;
+          }
+        }
+        tc::tc_commit(empty_bar(s));                     // smem slot reusable once these MMAs have read it
+      }
+      tc::tc_commit(tmem_full_bar);                      // accumulator complete
+    }
+  } else {
+    // =========================== epilogue ====================================================
+    tc::mbar_wait(tmem_full_bar, 0);
+    tc::tc_fence_after();
+    const int sub = warp & 3;                            // TMEM sub-partition this warp may read
+    const int r_local = sub * 32 + lane;
+    const int64_t row = (int64_t)m_blk * BM + r_local;
+    const bool row_ok = r_local < rows_valid;
+    const float scale = row_ok ? __fmul_rn(p.row_scale[row], p.w_ts[expert]) : 0.0f;
+#pragma unroll 1
+    for (int c = 0; c < BN / 32; ++c) {
+      uint32_t v[32];
+      tc::tmem_ld32(tmem_base + ((uint32_t)(sub * 32) << 16) + S::ACC + c * 32, v);
+      tc::tmem_ld_wait();
+      if (row_ok) {
+        float f[32];
+#pragma unroll
+        for (int i = 0; i < 32; ++i) f[i] = __fmul_rn(__uint_as_float(v[i]), scale);
+        if (p.bias) {
+          const uint16_t* b = p.bias + n0 + c * 32;
+#pragma unroll
+          for (int i = 0; i < 32; ++i) f[i] = __fadd_rn(f[i], __uint_as_float((uint32_t)b[i] << 16));
+        }
+        if (p.out_fp32) {
+          float4* dst = reinterpret_cast<float4*>(static_cast<float*>(p.Y) + row * p.ldy + n0 + c * 32);
+#pragma unroll
+          for (int i = 0; i < 8; ++i) dst[i] = make_float4(f[4 * i], f[4 * i + 1], f[4 * i + 2], f[4 * i + 3]);
+        } else {
+          uint4* dst = reinterpret_cast<uint4*>(static_cast<uint16_t*>(p.Y) + row * p.ldy + n0 + c * 32);
+#pragma unroll
+          for (int i = 0; i < 4; ++i)
+            dst[i] = make_uint4(pack_bf16x2_rn(f[8 * i], f[8 * i + 1]), pack_bf16x2_rn(f[8 * i + 2], f[8 * i + 3]),
+                                pack_bf16x2_rn(f[8 * i + 4], f[8 * i + 5]), pack_bf16x2_rn(f[8 * i + 6], f[8 * i + 7]));
+        }
+      }
+    }
+    tc::tc_fence_before();
+  }
+  __syncthreads();
+  if (warp == 2) {
+    tc::tc_fence_after();
+    tc::tmem_dealloc<kTmemCols>(tmem_base);
+  }
 }
+
+// ---- host: tensor maps + launch ----------------------------------------------------------------
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn encode_fn() {
+  static EncodeTiledFn fn = [] {
+    void* f = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &f, cudaEnableDefault, &q) != cudaSuccess ||
+        q != cudaDriverEntryPointSuccess)
+      f = nullptr;
+    return reinterpret_cast<EncodeTiledFn>(f);
+  }();
+  return fn;
+}
+
+// bytes [rows, row_bytes] row-major -> boxes of box_rows x box_bytes, swizzle = box_bytes (64 or 128)
+bool make_map(CUtensorMap* m, const void* base, uint64_t rows, uint64_t row_bytes, uint32_t box_bytes,
+              uint32_t box_rows) {
+  EncodeTiledFn fn = encode_fn();
+  if (!fn) return false;
+  cuuint64_t dims[2] = {row_bytes, rows};
+  cuuint64_t strides[1] = {row_bytes};
+  cuuint32_t box[2] = {box_bytes, box_rows};
+  cuuint32_t estr[2] = {1, 1};
+  CUtensorMapSwizzle sw = box_bytes == 128 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_64B;
+  return fn(m, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<void*>(base), dims, strides, box, estr,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, sw, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+template <int BN, int FMT>
+sharq_status launch_tiles(const LinearArgs& a, const GroupInfo& g, int64_t rows_total, int64_t m_blocks, int E,
+                          cudaStream_t st) {
+  using S = Stage<BN, FMT>;
+  CUtensorMap tm_sp, tm_dn, tm_w;
+  const int64_t w_rows = (int64_t)(E > 0 ? E : 1) * a.D;
+  if (!make_map(&tm_sp, a.sp_codes, (uint64_t)rows_total, (uint64_t)a.K / 4, 64, BM) ||
+      !make_map(&tm_dn, a.dn_codes, (uint64_t)rows_total, (uint64_t)a.K / 2, 128, BM) ||
+      !make_map(&tm_w, a.w_codes, (uint64_t)w_rows, (uint64_t)a.K / 2, 128, BN < 256 ? BN : 256))
+    return SHARQ_ECUDA;
+  KParams p{(const uint8_t*)a.sp_sf, (const uint8_t*)a.sp_meta, (const uint8_t*)a.dn_sf, (const uint8_t*)a.w_sf_sp,
+            (const uint8_t*)a.w_sf_dn, a.row_scale, a.w_ts, (const uint16_t*)a.bias, a.Y, a.ldy,
+            (int32_t)a.T, (int32_t)a.D, (int32_t)a.K, a.out_dtype, a.path};
+  auto kfn = sharq_linear_kernel<BN, FMT>;
+  if (cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, S::SMEM) != cudaSuccess)
+    return SHARQ_ECUDA;
+  dim3 grid((unsigned)(a.D / BN), (unsigned)m_blocks);
+  kfn<<<grid, kThreads, S::SMEM, st>>>(tm_sp, tm_dn, tm_w, p, g);
+  return cudaGetLastError() == cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
+}
+
+}  // namespace
+
+size_t linear_workspace_bytes(const sharq_config*, int64_t, int64_t, int64_t, int32_t) { return 0; }
+
+sharq_status launch_linear(const sharq_config* cfg, const LinearArgs& a, int32_t E, const int32_t* offsets_host,
+                           void* /*workspace*/, size_t /*workspace_bytes*/, int /*num_sms*/, cudaStream_t st) {
+  if (cfg->fmt == SHARQ_HIF4) return SHARQ_EINVAL;        // HiF4 has no FP4-rate tensor path
+  if (a.K > (int64_t)1 << 24 || a.D > (int64_t)1 << 24) return SHARQ_ESHAPE;
+  GroupInfo g{};
+  int64_t rows_total = a.T, m_blocks = (a.T + BM - 1) / BM;
+  if (E > 0) {
+    if (E > kMaxExperts) return SHARQ_ESHAPE;
+    g.E = E;
+    int32_t blk = 0;
+    for (int e = 0; e < E; ++e) {
+      g.blk_prefix[e] = blk;
+      g.count[e] = offsets_host[e + 1] - offsets_host[e];
+      blk += (g.count[e] + BM - 1) / BM;
+    }
+    g.blk_prefix[E] = blk;
+    m_blocks = blk;
+    rows_total = (int64_t)blk * BM;
+    if (m_blocks == 0) return SHARQ_OK;
+  }
+  if (m_blocks > 65535) return SHARQ_ESHAPE;
+  if (cfg->fmt == SHARQ_NVFP4) return launch_tiles<128, SHARQ_NVFP4>(a, g, rows_total, m_blocks, E, st);
+  return launch_tiles<128, SHARQ_MXFP4>(a, g, rows_total, m_blocks, E, st);
+}
+
+}  // namespace sharq
