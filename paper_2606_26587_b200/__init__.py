@@ -152,6 +152,17 @@ def prepare(cfg: Config, x, gamma=None, beta=None, x_tensor_scale=None, out=None
     return out
 
 
+def act_slot(cfg: Config, act: dict, row0: int, T: int) -> dict:
+    """View of rows [row0, row0+T) of a TILED activation set as raw device pointers (row0 % 128 == 0):
+    lets `prepare(..., out=...)` fill one expert's 128-row-aligned slot (sharq_linear_grouped, sharq.h)."""
+    assert row0 % 128 == 0 and cfg.fmt != HIF4
+    K = act["K"]
+    c_dn = K // 16 if cfg.fmt == NVFP4 else K // 32
+    return dict(sp_codes=act["sp_codes"].data_ptr() + row0 * (K // 4), sp_sf=act["sp_sf"].data_ptr() + row0 * (K // 32),
+                sp_meta=act["sp_meta"].data_ptr() + row0 * (K // 16), dn_codes=act["dn_codes"].data_ptr() + row0 * (K // 2),
+                dn_sf=act["dn_sf"].data_ptr() + row0 * c_dn, row_scale=act["row_scale"].data_ptr() + row0 * 4, T=T, K=K)
+
+
 def linear(cfg: Config, act: dict, wq: dict, bias=None, out_dtype="bf16", path=PATH_SHARQ, Y=None, workspace=None):
     import torch
     T, K, D = act["T"], act["K"], wq["D"]

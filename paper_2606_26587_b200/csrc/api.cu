@@ -163,7 +163,7 @@ sharq_status sharq_linear(const sharq_config* cfg, int64_t T, int64_t D, int64_t
                           int64_t ldy, int32_t out_dtype, int32_t path, void* workspace, size_t workspace_bytes,
                           void* stream) {
   const void* ptrs[] = {sp_codes, sp_sf, sp_meta, dn_codes, dn_sf, w_codes, w_sf_sparse_view, w_sf_dense_view, Y};
-  sharq_status s = check_linear(cfg, D, K, ptrs, 9, ldy, out_dtype, path);
+  sharq_status s = check_linear(cfg, D, K, ptrs, T == 0 ? 0 : 9, ldy, out_dtype, path);
   if (s != SHARQ_OK) return s;
   if (T < 0) return SHARQ_ESHAPE;
   if (T == 0) return SHARQ_OK;

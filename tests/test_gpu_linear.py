@@ -1,0 +1,131 @@
+"""GPU parity: sharq_linear / sharq_linear_grouped through the C ABI vs the oracle's fp64 product of the
+same dequantized operands (Eq. 9).  Bar (BASELINE.json north_star, R15):
+|Y - Y64| <= 1e-3 * max(|Y64|, 1e-2 * rms(Y64)) on the fp32 output; the bf16 output must be the RNE
+rounding of the fp32 output bit for bit."""
+import numpy as np
+import pytest
+import torch
+
+import sharq_inputs as si
+from oracle import sharq_oracle as so
+from tests.gpu_util import to_dev
+
+pytestmark = pytest.mark.gpu
+TOL = 1e-3
+
+
+@pytest.fixture(scope="module")
+def sq():
+    import __graft_entry__ as g
+    g.build()
+    import paper_2606_26587_b200 as pkg
+    return pkg
+
+
+def rel_err(y, y64):
+    den = np.maximum(np.abs(y64), 1e-2 * np.sqrt((y64 ** 2).mean()))
+    return np.abs(y.astype(np.float64) - y64) / den
+
+
+def path_reference(p, q, path):
+    """Table 5's ablation rows: 0 = sparse + dense, 1 = sparse only, 2 = dense only."""
+    A_sp, A_dn = so.dequant_backbone(p, with_ts=False), so.dequant_residual(p, with_ts=False)
+    W_sp, W_dn = so.dequant_weight(q, "sparse", with_ts=False), so.dequant_weight(q, "dense", with_ts=False)
+    acc = (A_sp @ W_sp.T if path != 2 else 0.0) + (A_dn @ W_dn.T if path != 1 else 0.0)
+    return acc * p["ts"].astype(np.float64)[:, None] * np.float64(q["ts_w"])
+
+
+CASES = [
+    # (fmt, norm, T, K, D, mult)   several k-blocks and n-tiles, ragged T (not a multiple of 128), T = 1
+    (0, 1, 16, 4096, 4096, 50.0),      # BASELINE.json configs[0]
+    (0, 1, 1, 4096, 6144, 50.0), (0, 0, 8, 14336, 4096, 50.0), (0, 1, 32, 4096, 28672, 50.0),   # configs[1] shapes
+    (0, 1, 300, 1024, 384, 200.0), (0, 0, 129, 256, 128, 10.0), (0, 1, 257, 3584, 512, 50.0),
+    (1, 1, 16, 4096, 4096, 50.0), (1, 0, 130, 3584, 4608, 200.0), (1, 1, 5, 768, 2048, 10.0),
+]
+
+
+@pytest.mark.parametrize("fmt,norm,T,K,D,mult", CASES)
+def test_linear_vs_oracle(sq, fmt, norm, T, K, D, mult):
+    x = si.activations(T, K, config=2, outlier_mult=mult, extra=T + K)
+    g, w = si.gamma(K, 2), si.weight(D, K, 2, extra=D)
+    cfg = sq.make_config(fmt, norm, 1e-6, sq.LAYOUT_TILED)
+    wq = sq.quantize_weight(cfg, to_dev(w))
+    act = sq.prepare(cfg, to_dev(x), to_dev(g) if norm else None)
+    y32 = sq.linear(cfg, act, wq, out_dtype="fp32")
+    y16 = sq.linear(cfg, act, wq, out_dtype="bf16")
+    torch.cuda.synchronize()
+    p = so.prepare(x, fmt=fmt, norm=norm, gamma_u16=g)
+    q = so.quantize_weight(w, fmt=fmt)
+    err = rel_err(y32.cpu().numpy(), so.linear(p, q))
+    assert err.max() <= TOL, f"max rel err {err.max():.3e} at {np.unravel_index(err.argmax(), err.shape)}"
+    assert torch.equal(y16, y32.to(torch.bfloat16)), "bf16 output is not RNE(fp32 output)"
+
+
+@pytest.mark.parametrize("path", [1, 2])
+def test_linear_single_path_and_bias(sq, path):
+    T, K, D = 70, 1024, 256
+    x, g, w = si.activations(T, K, config=3), si.gamma(K, 3), si.weight(D, K, 3)
+    bias = si.beta(D, 3)
+    cfg = sq.make_config(sq.NVFP4, sq.NORM_RMS, 1e-6, sq.LAYOUT_TILED)
+    wq, act = sq.quantize_weight(cfg, to_dev(w)), sq.prepare(cfg, to_dev(x), to_dev(g))
+    y = sq.linear(cfg, act, wq, out_dtype="fp32", path=path)
+    yb = sq.linear(cfg, act, wq, bias=to_dev(bias), out_dtype="fp32", path=0)
+    torch.cuda.synchronize()
+    p, q = so.prepare(x, gamma_u16=g), so.quantize_weight(w)
+    assert rel_err(y.cpu().numpy(), path_reference(p, q, path)).max() <= TOL
+    assert rel_err(yb.cpu().numpy(), so.linear(p, q, bias_u16=bias)).max() <= TOL
+
+
+def test_linear_strided_output_and_empty(sq):
+    T, K, D = 9, 512, 256
+    x, w = si.activations(T, K, config=3, extra=1), si.weight(D, K, 3, extra=1)
+    cfg = sq.make_config(sq.NVFP4, sq.NORM_NONE, 1e-6, sq.LAYOUT_TILED)
+    wq, act = sq.quantize_weight(cfg, to_dev(w)), sq.prepare(cfg, to_dev(x))
+    big = torch.full((T, D + 64), 7.0, dtype=torch.float32, device="cuda")
+    sq.linear(cfg, act, wq, Y=big[:, :D])
+    torch.cuda.synchronize()
+    assert (big[:, D:] == 7.0).all(), "wrote outside the [T, D] window of a strided Y"
+    p, q = so.prepare(x, norm=0), so.quantize_weight(w)
+    assert rel_err(big[:, :D].cpu().numpy(), so.linear(p, q)).max() <= TOL
+    # T = 0: SHARQ_OK, nothing launched, nothing touched
+    empty = sq.alloc_act(cfg, 0, K, "cuda")
+    y0 = sq.linear(cfg, empty, wq, Y=torch.empty((0, D), dtype=torch.float32, device="cuda"))
+    assert y0.shape == (0, D)
+
+
+def test_linear_rejects_bad_arguments(sq):
+    cfg = sq.make_config(sq.NVFP4, sq.NORM_NONE, 1e-6, sq.LAYOUT_CANONICAL)
+    x, w = si.activations(4, 256, config=3), si.weight(128, 256, 3)
+    wq, act = sq.quantize_weight(cfg, to_dev(w)), sq.prepare(cfg, to_dev(x))
+    with pytest.raises(sq.SharqError) as e:           # canonical layout is not what the GEMM consumes
+        sq.linear(cfg, act, wq)
+    assert e.value.status == sq.EINVAL
+
+
+def test_linear_grouped_moe(sq):
+    """Config 5 shape family, scaled down: experts with 0, 1, ragged and > 128 rows."""
+    E, K, D = 6, 512, 256
+    counts = [0, 1, 130, 37, 0, 128]
+    offsets = np.concatenate([[0], np.cumsum(counts)]).astype(np.int32)
+    cfg = sq.make_config(sq.NVFP4, sq.NORM_NONE, 1e-6, sq.LAYOUT_TILED)
+    pad = [-(-c // 128) * 128 for c in counts]
+    pad_off = np.concatenate([[0], np.cumsum(pad)])
+    act = sq.alloc_act(cfg, int(pad_off[-1]), K, "cuda")
+    ws, xs = [], []
+    for e in range(E):
+        ws.append(si.weight(D, K, 5, extra=e))
+        xs.append(si.activations(counts[e], K, config=5, extra=e))
+        if counts[e]:
+            sq.prepare(cfg, to_dev(xs[e]), out=sq.act_slot(cfg, act, int(pad_off[e]), counts[e]))
+    wqs = [sq.quantize_weight(cfg, to_dev(w)) for w in ws]
+    wq = dict(codes=torch.cat([q["codes"] for q in wqs]), sf_sp=torch.cat([q["sf_sp"] for q in wqs]),
+              sf_dn=torch.cat([q["sf_dn"] for q in wqs]), ts_w=torch.cat([q["ts_w"] for q in wqs]), D=D, K=K)
+    Y = sq.linear_grouped(cfg, offsets, act, wq, D, out_dtype="fp32")
+    torch.cuda.synchronize()
+    Y = Y.cpu().numpy()
+    for e in range(E):
+        if counts[e] == 0:
+            continue
+        p, q = so.prepare(xs[e], norm=0), so.quantize_weight(ws[e])
+        got = Y[pad_off[e]: pad_off[e] + counts[e]]
+        assert rel_err(got, so.linear(p, q)).max() <= TOL, f"expert {e}"
