@@ -15,6 +15,7 @@
 // warps 2-5 = epilogue (warp w owns TMEM lanes 32*(w%4)..+31); warp 2 also owns the TMEM allocation.
 #include <cuda.h>
 #include <cuda_runtime.h>
+#include <stdlib.h>
 
 #include "common.cuh"
 #include "tc_ptx.cuh"
@@ -52,10 +53,14 @@ struct KParams {
   void* Y;
   int64_t ldy;
   int32_t T, D, K, out_fp32, path;
+  int32_t m_blocks, total_tiles;
 };
 
 // ---- shared-memory stage layout -------------------------------------------------------------
-template <int BN, int FMT>
+// SPLIT = the split-K variant for T <= 256 (few output tiles): a thread-block cluster of `splits` CTAs
+// shares one output tile, each CTA runs a slice of K, the partial accumulators are exchanged through
+// distributed shared memory (16-column slices, owner = slice % splits) and summed in rank order.
+template <int BN, int FMT, bool SPLIT>
 struct Stage {
   static constexpr int NB = (BN + 127) / 128;                         // 128-row scale atoms of W per tile
   static constexpr int SF_DN_BYTES = (FMT == SHARQ_NVFP4) ? 2048 : 1024;  // per 128 rows per k-block
@@ -69,47 +74,85 @@ struct Stage {
   static constexpr int SFB_DN = SFB_SP + NB * 1024;
   static constexpr int RAW = SFB_DN + NB * SF_DN_BYTES;
   static constexpr int BYTES = (RAW + 1023) / 1024 * 1024;
-  static constexpr int STAGES = (BN > 128) ? 3 : 4;
-  static constexpr int SMEM = STAGES * BYTES + 1024 /*alignment slack*/ + 256 /*barriers*/;
-  // tensor-memory columns
+  static constexpr int STAGES = SPLIT ? 3 : 4;
+  static constexpr int RECV = SPLIT ? 9 * 8192 : 0;                   // [src][slot][128 rows][16 fp32]
+  static constexpr int SMEM = STAGES * BYTES + RECV + 1024 /*alignment slack*/ + 256 /*barriers*/;
+  // tensor-memory columns: two accumulator stages, then metadata and scale factors
   static constexpr int SFB_COLS = NB * 4;          // columns one MMA's B scales occupy
-  static constexpr int ACC = 0;
+  static constexpr int ACC_STAGES = 2;
   static constexpr int E_COL = 256;
   static constexpr int SFA_SP_COL = 260;           // 2 MMAs x 4
   static constexpr int SFA_DN_COL = 268;           // 4 MMAs x 4
   static constexpr int SFB_SP_COL = 284;           // 2 MMAs x SFB_COLS (<= 16)
   static constexpr int SFB_DN_COL = 300;           // 4 MMAs x SFB_COLS (<= 32)
+  static_assert(BN * ACC_STAGES <= 256, "accumulator stages overlap the scale-factor columns");
 };
 
-template <int BN, int FMT>
+struct Unit { int m_blk, n_blk, expert, rows_valid, kb0, kb1; };
+
+__device__ __forceinline__ Unit decode_unit(const KParams& p, const GroupInfo& g, int tile, int rank, int splits) {
+  Unit u;
+  u.m_blk = tile % p.m_blocks;                     // m fastest: concurrent CTAs share W tiles in L2
+  u.n_blk = tile / p.m_blocks;
+  u.expert = 0;
+  if (g.E > 0) {
+    while (u.expert + 1 < g.E && g.blk_prefix[u.expert + 1] <= u.m_blk) ++u.expert;
+    u.rows_valid = min(BM, g.count[u.expert] - (u.m_blk - g.blk_prefix[u.expert]) * BM);
+  } else {
+    u.rows_valid = min(BM, p.T - u.m_blk * BM);
+  }
+  const int num_kb = p.K / BK;
+  u.kb0 = (int)((int64_t)rank * num_kb / splits);
+  u.kb1 = (int)((int64_t)(rank + 1) * num_kb / splits);
+  return u;
+}
+
+// y = acc * scale (+ bias) for N consecutive output features of one row, bf16 or fp32 store
+template <int N>
+__device__ __forceinline__ void store_row(const KParams& p, int64_t row, int col0, float scale, float (&f)[N]) {
+#pragma unroll
+  for (int i = 0; i < N; ++i) f[i] = __fmul_rn(f[i], scale);
+  if (p.bias) {
+    const uint16_t* b = p.bias + col0;
+#pragma unroll
+    for (int i = 0; i < N; ++i) f[i] = __fadd_rn(f[i], __uint_as_float((uint32_t)b[i] << 16));
+  }
+  if (p.out_fp32) {
+    float4* dst = reinterpret_cast<float4*>(static_cast<float*>(p.Y) + row * p.ldy + col0);
+#pragma unroll
+    for (int i = 0; i < N / 4; ++i) dst[i] = make_float4(f[4 * i], f[4 * i + 1], f[4 * i + 2], f[4 * i + 3]);
+  } else {
+    uint4* dst = reinterpret_cast<uint4*>(static_cast<uint16_t*>(p.Y) + row * p.ldy + col0);
+#pragma unroll
+    for (int i = 0; i < N / 8; ++i)
+      dst[i] = make_uint4(pack_bf16x2_rn(f[8 * i], f[8 * i + 1]), pack_bf16x2_rn(f[8 * i + 2], f[8 * i + 3]),
+                          pack_bf16x2_rn(f[8 * i + 4], f[8 * i + 5]), pack_bf16x2_rn(f[8 * i + 6], f[8 * i + 7]));
+  }
+}
+
+template <int BN, int FMT, bool SPLIT>
 __global__ void __launch_bounds__(kThreads, 1)
 sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_constant__ CUtensorMap tm_a_dn,
                     const __grid_constant__ CUtensorMap tm_w, const KParams p, const __grid_constant__ GroupInfo g) {
-  using S = Stage<BN, FMT>;
+  using S = Stage<BN, FMT, SPLIT>;
   constexpr bool NV = (FMT == SHARQ_NVFP4);
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
-  const uint32_t bars = smem_base + S::STAGES * S::BYTES;          // full[S], empty[S], tmem_full, tmem_ptr
+  const uint32_t recv_base = smem_base + S::STAGES * S::BYTES;
+  const uint32_t bars = recv_base + S::RECV;      // full[STAGES], empty[STAGES], tmem_full[2], tmem_empty[2], ptr
   auto full_bar = [&](int s) { return bars + 8u * s; };
   auto empty_bar = [&](int s) { return bars + 8u * (S::STAGES + s); };
-  const uint32_t tmem_full_bar = bars + 8u * (2 * S::STAGES);
-  const uint32_t tmem_ptr_smem = bars + 8u * (2 * S::STAGES + 1);
+  auto tmem_full_bar = [&](int a) { return bars + 8u * (2 * S::STAGES + a); };
+  auto tmem_empty_bar = [&](int a) { return bars + 8u * (2 * S::STAGES + 2 + a); };
+  const uint32_t tmem_ptr_smem = bars + 8u * (2 * S::STAGES + 4);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int n_blk = blockIdx.x, m_blk = blockIdx.y;
-  const int num_kb = p.K / BK;
   const bool do_sp = p.path != 2, do_dn = p.path != 1;
-
-  // ---- which problem does this 128-row block belong to --------------------------------------
-  int expert = 0, rows_valid;
-  if (g.E > 0) {
-    while (expert + 1 < g.E && g.blk_prefix[expert + 1] <= m_blk) ++expert;
-    rows_valid = min(BM, g.count[expert] - (m_blk - g.blk_prefix[expert]) * BM);
-  } else {
-    rows_valid = min(BM, p.T - m_blk * BM);
-  }
-  const int n0 = n_blk * BN;                        // first output feature of the tile
-  const int w_row0 = expert * p.D + n0;             // row in the stacked [E*D, K/2] weight payload
+  // work distribution: SPLIT -> one tile per cluster, this CTA's k-slice; else persistent round-robin
+  const int rank = SPLIT ? (int)tc::cluster_ctarank() : 0;
+  const int splits = SPLIT ? (int)tc::cluster_nctarank() : 1;
+  const int tile0 = SPLIT ? (int)tc::cluster_id_x() : (int)blockIdx.x;
+  const int tile_step = SPLIT ? p.total_tiles : (int)gridDim.x;
 
   if (warp == 0 && lane == 0) {
     tc::prefetch_tmap(&tm_a_sp);
@@ -121,7 +164,10 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
       tc::mbar_init(full_bar(s), 1);
       tc::mbar_init(empty_bar(s), 1);
     }
-    tc::mbar_init(tmem_full_bar, 1);
+    for (int a = 0; a < 2; ++a) {
+      tc::mbar_init(tmem_full_bar(a), 1);
+      tc::mbar_init(tmem_empty_bar(a), 4);          // one arrival per epilogue warp
+    }
     tc::fence_mbar_init();
   }
   if (warp == 2) tc::tmem_alloc<kTmemCols>(tmem_ptr_smem);
@@ -134,38 +180,44 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
   if (warp == 0) {
     // =========================== TMA producer ===============================================
     if (lane == 0) {
-      const uint64_t pol_act = tc::policy_evict_first(), pol_w = tc::policy_evict_last();
+      const uint64_t pol_act = SPLIT ? tc::policy_evict_last() : tc::policy_evict_normal();
+      const uint64_t pol_w = SPLIT ? tc::policy_evict_first() : tc::policy_evict_normal();
       const int64_t Kc = p.K;
-      const uint8_t* sfa_sp = p.sp_sf + (size_t)m_blk * (Kc / 128) * 512;
-      const uint8_t* sfa_dn = p.dn_sf + (size_t)m_blk * (Kc / 256) * (S::SF_DN_BYTES);
-      const uint8_t* meta = p.sp_meta + (size_t)m_blk * (Kc / 256) * 2048;
-      const int64_t wblk0 = w_row0 / 128;
       uint32_t tx = BN * 128;
       if (do_sp) tx += BM * 64 + 2048 + 1024 + S::NB * 1024;
       if (do_dn) tx += BM * 128 + S::SF_DN_BYTES + S::NB * S::SF_DN_BYTES;
-      for (int kb = 0; kb < num_kb; ++kb) {
-        const int s = kb % S::STAGES;
-        const uint32_t ph = (kb / S::STAGES) & 1;
-        tc::mbar_wait(empty_bar(s), ph ^ 1);
-        const uint32_t st = smem_base + s * S::BYTES;
-        const uint32_t fb = full_bar(s);
-        tc::mbar_expect_tx(fb, tx);
-        tc::tma_load_2d(st + S::W, &tm_w, fb, kb * 128, w_row0, pol_w);
-        if (do_sp) {
-          tc::tma_load_2d(st + S::A_SP, &tm_a_sp, fb, kb * 64, m_blk * BM, pol_act);
-          tc::bulk_load(st + S::META, meta + (size_t)kb * 2048, 2048, fb, pol_act);
-          tc::bulk_load(st + S::SFA_SP, sfa_sp + (size_t)kb * 1024, 1024, fb, pol_act);
-          for (int nb = 0; nb < S::NB; ++nb)
-            tc::bulk_load(st + S::SFB_SP + nb * 1024,
-                          p.w_sf_sp + ((size_t)(wblk0 + nb) * (Kc / 128) + (size_t)kb * 2) * 512, 1024, fb, pol_w);
-        }
-        if (do_dn) {
-          tc::tma_load_2d(st + S::A_DN, &tm_a_dn, fb, kb * 128, m_blk * BM, pol_act);
-          tc::bulk_load(st + S::SFA_DN, sfa_dn + (size_t)kb * S::SF_DN_BYTES, S::SF_DN_BYTES, fb, pol_act);
-          for (int nb = 0; nb < S::NB; ++nb)
-            tc::bulk_load(st + S::SFB_DN + nb * S::SF_DN_BYTES,
-                          p.w_sf_dn + ((size_t)(wblk0 + nb) * (Kc / 256) + (size_t)kb) * S::SF_DN_BYTES,
-                          S::SF_DN_BYTES, fb, pol_w);
+      uint32_t it = 0;                                   // k-blocks issued so far (ring position)
+      for (int tile = tile0; tile < p.total_tiles; tile += tile_step) {
+        const Unit u = decode_unit(p, g, tile, rank, splits);
+        const int w_row0 = u.expert * p.D + u.n_blk * BN;
+        const int64_t wblk0 = w_row0 / 128;
+        const uint8_t* sfa_sp = p.sp_sf + (size_t)u.m_blk * (Kc / 128) * 512;
+        const uint8_t* sfa_dn = p.dn_sf + (size_t)u.m_blk * (Kc / 256) * (S::SF_DN_BYTES);
+        const uint8_t* meta = p.sp_meta + (size_t)u.m_blk * (Kc / 256) * 2048;
+        for (int kb = u.kb0; kb < u.kb1; ++kb, ++it) {
+          const int s = it % S::STAGES;
+          const uint32_t ph = (it / S::STAGES) & 1;
+          tc::mbar_wait(empty_bar(s), ph ^ 1);
+          const uint32_t st = smem_base + s * S::BYTES;
+          const uint32_t fb = full_bar(s);
+          tc::mbar_expect_tx(fb, tx);
+          tc::tma_load_2d(st + S::W, &tm_w, fb, kb * 128, w_row0, pol_w);
+          if (do_sp) {
+            tc::tma_load_2d(st + S::A_SP, &tm_a_sp, fb, kb * 64, u.m_blk * BM, pol_act);
+            tc::bulk_load(st + S::META, meta + (size_t)kb * 2048, 2048, fb, pol_act);
+            tc::bulk_load(st + S::SFA_SP, sfa_sp + (size_t)kb * 1024, 1024, fb, pol_act);
+            for (int nb = 0; nb < S::NB; ++nb)
+              tc::bulk_load(st + S::SFB_SP + nb * 1024,
+                            p.w_sf_sp + ((size_t)(wblk0 + nb) * (Kc / 128) + (size_t)kb * 2) * 512, 1024, fb, pol_w);
+          }
+          if (do_dn) {
+            tc::tma_load_2d(st + S::A_DN, &tm_a_dn, fb, kb * 128, u.m_blk * BM, pol_act);
+            tc::bulk_load(st + S::SFA_DN, sfa_dn + (size_t)kb * S::SF_DN_BYTES, S::SF_DN_BYTES, fb, pol_act);
+            for (int nb = 0; nb < S::NB; ++nb)
+              tc::bulk_load(st + S::SFB_DN + nb * S::SF_DN_BYTES,
+                            p.w_sf_dn + ((size_t)(wblk0 + nb) * (Kc / 256) + (size_t)kb) * S::SF_DN_BYTES,
+                            S::SF_DN_BYTES, fb, pol_w);
+          }
         }
       }
     }
@@ -173,96 +225,151 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
     // =========================== MMA issuer =================================================
     if (lane == 0) {
       const uint32_t idesc_sp = tc::idesc_fp4(BM, BN, true, !NV, 0, 0);
-      const uint32_t sfb_shift = (BN < 128) ? (uint32_t)((n0 % 128) / 32) : 0u;   // sub-atom N tiles
-      uint32_t accumulate = 0;
-      for (int kb = 0; kb < num_kb; ++kb) {
-        const int s = kb % S::STAGES;
-        const uint32_t ph = (kb / S::STAGES) & 1;
-        tc::mbar_wait(full_bar(s), ph);
+      uint32_t it = 0, n_unit = 0;
+      for (int tile = tile0; tile < p.total_tiles; tile += tile_step, ++n_unit) {
+        const Unit u = decode_unit(p, g, tile, rank, splits);
+        const uint32_t sfb_shift = (BN < 128) ? (uint32_t)(((u.n_blk * BN) % 128) / 32) : 0u;   // sub-atom N tiles
+        const uint32_t as = n_unit & 1u;                                  // accumulator stage
+        const uint32_t acc = tmem_base + as * BN;
+        tc::mbar_wait(tmem_empty_bar(as), ((n_unit >> 1) & 1u) ^ 1u);     // epilogue has drained this stage
         tc::tc_fence_after();
-        const uint32_t st = smem_base + s * S::BYTES;
-        if (do_sp) {
-          tc::tc_cp_meta(tmem_base + S::E_COL, tc::smem_desc(st + S::META, 128, 0));
+        uint32_t accumulate = 0;
+        for (int kb = u.kb0; kb < u.kb1; ++kb, ++it) {
+          const int s = it % S::STAGES;
+          const uint32_t ph = (it / S::STAGES) & 1;
+          tc::mbar_wait(full_bar(s), ph);
+          tc::tc_fence_after();
+          const uint32_t st = smem_base + s * S::BYTES;
+          if (do_sp) {
+            tc::tc_cp_meta(tmem_base + S::E_COL, tc::smem_desc(st + S::META, 128, 0));
 #pragma unroll
-          for (int a = 0; a < 2; ++a) {
-            tc::tc_cp_sf(tmem_base + S::SFA_SP_COL + 4 * a, tc::smem_desc(st + S::SFA_SP + 512 * a, 128, 0));
+            for (int a = 0; a < 2; ++a) {
+              tc::tc_cp_sf(tmem_base + S::SFA_SP_COL + 4 * a, tc::smem_desc(st + S::SFA_SP + 512 * a, 128, 0));
 #pragma unroll
-            for (int nb = 0; nb < S::NB; ++nb)
-              tc::tc_cp_sf(tmem_base + S::SFB_SP_COL + S::SFB_COLS * a + 4 * nb,
-                           tc::smem_desc(st + S::SFB_SP + nb * 1024 + 512 * a, 128, 0));
+              for (int nb = 0; nb < S::NB; ++nb)
+                tc::tc_cp_sf(tmem_base + S::SFB_SP_COL + S::SFB_COLS * a + 4 * nb,
+                             tc::smem_desc(st + S::SFB_SP + nb * 1024 + 512 * a, 128, 0));
+            }
+#pragma unroll
+            for (int j = 0; j < 2; ++j) {
+              tc::mma_sparse(acc, tc::smem_desc(st + S::A_SP + 32 * j, 512, 4),
+                             tc::smem_desc(st + S::W + 64 * j, 1024, 2), idesc_sp, tmem_base + S::SFA_SP_COL + 4 * j,
+                             tmem_base + S::SFB_SP_COL + S::SFB_COLS * j + sfb_shift, tmem_base + S::E_COL + 2 * j,
+                             accumulate);
+              accumulate = 1;
+            }
           }
+          if (do_dn) {
+            constexpr int ATOMS = NV ? 4 : 2;
 #pragma unroll
-          for (int j = 0; j < 2; ++j) {
-            tc::mma_sparse(tmem_base + S::ACC, tc::smem_desc(st + S::A_SP + 32 * j, 512, 4),
-                           tc::smem_desc(st + S::W + 64 * j, 1024, 2), idesc_sp, tmem_base + S::SFA_SP_COL + 4 * j,
-                           tmem_base + S::SFB_SP_COL + S::SFB_COLS * j + sfb_shift, tmem_base + S::E_COL + 2 * j,
-                           accumulate);
-            accumulate = 1;
+            for (int a = 0; a < ATOMS; ++a) {
+              tc::tc_cp_sf(tmem_base + S::SFA_DN_COL + 4 * a, tc::smem_desc(st + S::SFA_DN + 512 * a, 128, 0));
+#pragma unroll
+              for (int nb = 0; nb < S::NB; ++nb)
+                tc::tc_cp_sf(tmem_base + S::SFB_DN_COL + S::SFB_COLS * a + 4 * nb,
+                             tc::smem_desc(st + S::SFB_DN + nb * S::SF_DN_BYTES + 512 * a, 128, 0));
+            }
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+              const int atom = NV ? j : j / 2;               // MXFP4: two K=64 MMAs share one 4-scale atom
+              const uint32_t sf_id = NV ? 0u : (uint32_t)(j & 1) * 2u;
+              const uint32_t idesc_dn = tc::idesc_fp4(BM, BN, false, !NV, sf_id, sf_id);
+              tc::mma_dense<NV>(acc, tc::smem_desc(st + S::A_DN + 32 * j, 1024, 2),
+                                tc::smem_desc(st + S::W + 32 * j, 1024, 2), idesc_dn,
+                                tmem_base + S::SFA_DN_COL + 4 * atom,
+                                tmem_base + S::SFB_DN_COL + S::SFB_COLS * atom + sfb_shift, accumulate);
+              accumulate = 1;
+            }
           }
+          tc::tc_commit(empty_bar(s));                   // smem slot reusable once these MMAs have read it
         }
-        if (do_dn) {
-          constexpr int ATOMS = NV ? 4 : 2;
-#pragma unroll
-          for (int a = 0; a < ATOMS; ++a) {
-            tc::tc_cp_sf(tmem_base + S::SFA_DN_COL + 4 * a, tc::smem_desc(st + S::SFA_DN + 512 * a, 128, 0));
-#pragma unroll
-            for (int nb = 0; nb < S::NB; ++nb)
-              tc::tc_cp_sf(tmem_base + S::SFB_DN_COL + S::SFB_COLS * a + 4 * nb,
-                           tc::smem_desc(st + S::SFB_DN + nb * S::SF_DN_BYTES + 512 * a, 128, 0));
-          }
-#pragma unroll
-          for (int j = 0; j < 4; ++j) {
-            const int atom = NV ? j : j / 2;                 // MXFP4: two K=64 MMAs share one 4-scale atom
-            const uint32_t sf_id = NV ? 0u : (uint32_t)(j & 1) * 2u;
-            const uint32_t idesc_dn = tc::idesc_fp4(BM, BN, false, !NV, sf_id, sf_id);
-            tc::mma_dense<NV>(tmem_base + S::ACC, tc::smem_desc(st + S::A_DN + 32 * j, 1024, 2),
-                              tc::smem_desc(st + S::W + 32 * j, 1024, 2), idesc_dn,
-                              tmem_base + S::SFA_DN_COL + 4 * atom,
-                              tmem_base + S::SFB_DN_COL + S::SFB_COLS * atom + sfb_shift, accumulate);
-            accumulate = 1;
-          }
-        }
-        tc::tc_commit(empty_bar(s));                     // smem slot reusable once these MMAs have read it
+        tc::tc_commit(tmem_full_bar(as));                // accumulator complete
       }
-      tc::tc_commit(tmem_full_bar);                      // accumulator complete
     }
   } else {
     // =========================== epilogue ====================================================
-    tc::mbar_wait(tmem_full_bar, 0);
-    tc::tc_fence_after();
     const int sub = warp & 3;                            // TMEM sub-partition this warp may read
     const int r_local = sub * 32 + lane;
-    const int64_t row = (int64_t)m_blk * BM + r_local;
-    const bool row_ok = r_local < rows_valid;
-    const float scale = row_ok ? __fmul_rn(p.row_scale[row], p.w_ts[expert]) : 0.0f;
+    const uint32_t lane_addr = tmem_base + ((uint32_t)(sub * 32) << 16);
+    if constexpr (!SPLIT) {
+      uint32_t n_unit = 0;
+      for (int tile = tile0; tile < p.total_tiles; tile += tile_step, ++n_unit) {
+        const Unit u = decode_unit(p, g, tile, 0, 1);
+        const uint32_t as = n_unit & 1u;
+        const int64_t row = (int64_t)u.m_blk * BM + r_local;
+        const bool row_ok = r_local < u.rows_valid;
+        const float scale = row_ok ? __fmul_rn(p.row_scale[row], p.w_ts[u.expert]) : 0.0f;
+        tc::mbar_wait(tmem_full_bar(as), (n_unit >> 1) & 1u);
+        tc::tc_fence_after();
 #pragma unroll 1
-    for (int c = 0; c < BN / 32; ++c) {
-      uint32_t v[32];
-      tc::tmem_ld32(tmem_base + ((uint32_t)(sub * 32) << 16) + S::ACC + c * 32, v);
-      tc::tmem_ld_wait();
-      if (row_ok) {
-        float f[32];
+        for (int c = 0; c < BN / 32; ++c) {
+          uint32_t v[32];
+          tc::tmem_ld32(lane_addr + as * BN + c * 32, v);
+          tc::tmem_ld_wait();
+          if (row_ok) {
+            float f[32];
 #pragma unroll
-        for (int i = 0; i < 32; ++i) f[i] = __fmul_rn(__uint_as_float(v[i]), scale);
-        if (p.bias) {
-          const uint16_t* b = p.bias + n0 + c * 32;
-#pragma unroll
-          for (int i = 0; i < 32; ++i) f[i] = __fadd_rn(f[i], __uint_as_float((uint32_t)b[i] << 16));
+            for (int i = 0; i < 32; ++i) f[i] = __uint_as_float(v[i]);
+            store_row<32>(p, row, u.n_blk * BN + c * 32, scale, f);
+          }
         }
-        if (p.out_fp32) {
-          float4* dst = reinterpret_cast<float4*>(static_cast<float*>(p.Y) + row * p.ldy + n0 + c * 32);
-#pragma unroll
-          for (int i = 0; i < 8; ++i) dst[i] = make_float4(f[4 * i], f[4 * i + 1], f[4 * i + 2], f[4 * i + 3]);
-        } else {
-          uint4* dst = reinterpret_cast<uint4*>(static_cast<uint16_t*>(p.Y) + row * p.ldy + n0 + c * 32);
+        tc::tc_fence_before();
+        __syncwarp();
+        if (lane == 0) tc::mbar_arrive(tmem_empty_bar(as));
+      }
+    } else {
+      // ---- split-K: scatter 16-column slices of the partial accumulator to their owner CTAs ----
+      const Unit u = decode_unit(p, g, tile0, rank, splits);
+      const bool row_ok = r_local < u.rows_valid;
+      const int slots = (BN / 16 + splits - 1) / splits;
+      tc::mbar_wait(tmem_full_bar(0), 0);
+      tc::tc_fence_after();
+#pragma unroll 1
+      for (int j = 0; j < BN / 16; ++j) {
+        uint32_t v[16];
+        tc::tmem_ld16(lane_addr + j * 16, v);
+        tc::tmem_ld_wait();
+        if (row_ok) {
+          const uint32_t local = recv_base + (uint32_t)(((rank * slots + j / splits) * BM + r_local) * 64);
+          const uint32_t remote = tc::map_to_cta(local, (uint32_t)(j % splits));
 #pragma unroll
           for (int i = 0; i < 4; ++i)
-            dst[i] = make_uint4(pack_bf16x2_rn(f[8 * i], f[8 * i + 1]), pack_bf16x2_rn(f[8 * i + 2], f[8 * i + 3]),
-                                pack_bf16x2_rn(f[8 * i + 4], f[8 * i + 5]), pack_bf16x2_rn(f[8 * i + 6], f[8 * i + 7]));
+            tc::st_cluster_v4(remote + 16 * i, __uint_as_float(v[4 * i]), __uint_as_float(v[4 * i + 1]),
+                              __uint_as_float(v[4 * i + 2]), __uint_as_float(v[4 * i + 3]));
+        }
+      }
+      tc::tc_fence_before();
+    }
+  }
+  if constexpr (SPLIT) {
+    __syncwarp();
+    tc::cluster_sync_all();                              // partial slices have landed in their owners
+    if (warp >= 2) {
+      const Unit u = decode_unit(p, g, tile0, rank, splits);
+      const int r_local = (warp & 3) * 32 + lane;
+      if (r_local < u.rows_valid) {
+        const int64_t row = (int64_t)u.m_blk * BM + r_local;
+        const float scale = __fmul_rn(p.row_scale[row], p.w_ts[u.expert]);
+        const int slots = (BN / 16 + splits - 1) / splits;
+        for (int slot = 0; slot < slots; ++slot) {
+          const int j = slot * splits + rank;            // the slices this CTA owns
+          if (j >= BN / 16) break;
+          float f[16];
+#pragma unroll
+          for (int i = 0; i < 16; ++i) f[i] = 0.0f;
+          for (int src = 0; src < splits; ++src) {       // fixed order: deterministic sum
+            const uint32_t a = recv_base + (uint32_t)(((src * slots + slot) * BM + r_local) * 64);
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+              const float4 t = tc::ld_shared_v4(a + 16 * i);
+              f[4 * i] = __fadd_rn(f[4 * i], t.x); f[4 * i + 1] = __fadd_rn(f[4 * i + 1], t.y);
+              f[4 * i + 2] = __fadd_rn(f[4 * i + 2], t.z); f[4 * i + 3] = __fadd_rn(f[4 * i + 3], t.w);
+            }
+          }
+          store_row<16>(p, row, u.n_blk * BN + j * 16, scale, f);
         }
       }
     }
-    tc::tc_fence_before();
   }
   __syncthreads();
   if (warp == 2) {
@@ -303,25 +410,59 @@ bool make_map(CUtensorMap* m, const void* base, uint64_t rows, uint64_t row_byte
             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
+// Number of K-splits (cluster size) for a launch with `tiles` output tiles: only when the tiles alone
+// leave most SMs idle, and only sizes whose slice exchange fits the receive buffer (2, 3, 4, 8).
+int choose_splits(int64_t tiles, int num_kb, int num_sms) {
+  if (tiles * 2 > num_sms) return 1;
+  const int cand[4] = {8, 4, 3, 2};
+  for (int c : cand) {
+    if (c == 8 && tiles * 8 > 128) continue;             // 8-CTA clusters: two per GPC at most
+    if (tiles * c <= num_sms && num_kb >= 2 * c) return c;
+  }
+  return 1;
+}
+
 template <int BN, int FMT>
 sharq_status launch_tiles(const LinearArgs& a, const GroupInfo& g, int64_t rows_total, int64_t m_blocks, int E,
-                          cudaStream_t st) {
-  using S = Stage<BN, FMT>;
+                          int num_sms, cudaStream_t st) {
   CUtensorMap tm_sp, tm_dn, tm_w;
   const int64_t w_rows = (int64_t)(E > 0 ? E : 1) * a.D;
   if (!make_map(&tm_sp, a.sp_codes, (uint64_t)rows_total, (uint64_t)a.K / 4, 64, BM) ||
       !make_map(&tm_dn, a.dn_codes, (uint64_t)rows_total, (uint64_t)a.K / 2, 128, BM) ||
       !make_map(&tm_w, a.w_codes, (uint64_t)w_rows, (uint64_t)a.K / 2, 128, BN < 256 ? BN : 256))
     return SHARQ_ECUDA;
+  const int64_t tiles = m_blocks * (a.D / BN);
   KParams p{(const uint8_t*)a.sp_sf, (const uint8_t*)a.sp_meta, (const uint8_t*)a.dn_sf, (const uint8_t*)a.w_sf_sp,
             (const uint8_t*)a.w_sf_dn, a.row_scale, a.w_ts, (const uint16_t*)a.bias, a.Y, a.ldy,
-            (int32_t)a.T, (int32_t)a.D, (int32_t)a.K, a.out_dtype, a.path};
-  auto kfn = sharq_linear_kernel<BN, FMT>;
+            (int32_t)a.T, (int32_t)a.D, (int32_t)a.K, a.out_dtype, a.path, (int32_t)m_blocks, (int32_t)tiles};
+  const int splits = choose_splits(tiles, (int)(a.K / BK), num_sms);
+  cudaLaunchConfig_t lc{};
+  cudaLaunchAttribute attr[1];
+  lc.blockDim = dim3(kThreads);
+  lc.stream = st;
+  if (splits > 1) {
+    using S = Stage<BN, FMT, true>;
+    auto kfn = sharq_linear_kernel<BN, FMT, true>;
+    if (cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, S::SMEM) != cudaSuccess)
+      return SHARQ_ECUDA;
+    lc.gridDim = dim3((unsigned)(tiles * splits));
+    lc.dynamicSmemBytes = S::SMEM;
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = (unsigned)splits;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    lc.attrs = attr;
+    lc.numAttrs = 1;
+    return cudaLaunchKernelEx(&lc, kfn, tm_sp, tm_dn, tm_w, p, g) == cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
+  }
+  using S = Stage<BN, FMT, false>;
+  auto kfn = sharq_linear_kernel<BN, FMT, false>;
   if (cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, S::SMEM) != cudaSuccess)
     return SHARQ_ECUDA;
-  dim3 grid((unsigned)(a.D / BN), (unsigned)m_blocks);
-  kfn<<<grid, kThreads, S::SMEM, st>>>(tm_sp, tm_dn, tm_w, p, g);
-  return cudaGetLastError() == cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
+  lc.gridDim = dim3((unsigned)(tiles < num_sms ? tiles : num_sms));      // persistent: one CTA per SM
+  if (const char* dbg = getenv("SHARQ_DEBUG_GRID")) lc.gridDim = dim3((unsigned)atoi(dbg));
+  lc.dynamicSmemBytes = S::SMEM;
+  return cudaLaunchKernelEx(&lc, kfn, tm_sp, tm_dn, tm_w, p, g) == cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
 }
 
 }  // namespace
@@ -329,7 +470,7 @@ sharq_status launch_tiles(const LinearArgs& a, const GroupInfo& g, int64_t rows_
 size_t linear_workspace_bytes(const sharq_config*, int64_t, int64_t, int64_t, int32_t) { return 0; }
 
 sharq_status launch_linear(const sharq_config* cfg, const LinearArgs& a, int32_t E, const int32_t* offsets_host,
-                           void* /*workspace*/, size_t /*workspace_bytes*/, int /*num_sms*/, cudaStream_t st) {
+                           void* /*workspace*/, size_t /*workspace_bytes*/, int num_sms, cudaStream_t st) {
   if (cfg->fmt == SHARQ_HIF4) return SHARQ_EINVAL;        // HiF4 has no FP4-rate tensor path
   if (a.K > (int64_t)1 << 24 || a.D > (int64_t)1 << 24) return SHARQ_ESHAPE;
   GroupInfo g{};
@@ -348,9 +489,9 @@ sharq_status launch_linear(const sharq_config* cfg, const LinearArgs& a, int32_t
     rows_total = (int64_t)blk * BM;
     if (m_blocks == 0) return SHARQ_OK;
   }
-  if (m_blocks > 65535) return SHARQ_ESHAPE;
-  if (cfg->fmt == SHARQ_NVFP4) return launch_tiles<128, SHARQ_NVFP4>(a, g, rows_total, m_blocks, E, st);
-  return launch_tiles<128, SHARQ_MXFP4>(a, g, rows_total, m_blocks, E, st);
+  if (m_blocks * (a.D / 128) > (int64_t)1 << 30) return SHARQ_ESHAPE;
+  if (cfg->fmt == SHARQ_NVFP4) return launch_tiles<128, SHARQ_NVFP4>(a, g, rows_total, m_blocks, E, num_sms, st);
+  return launch_tiles<128, SHARQ_MXFP4>(a, g, rows_total, m_blocks, E, num_sms, st);
 }
 
 }  // namespace sharq
