@@ -378,6 +378,232 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
   }
 }
 
+// ---- CTA-pair kernel (cta_group::2): 256 x 256 output tile per cluster of two CTAs ---------------------
+// For T >= 256 the 128 x 128 kernel is bound by shared-memory refill latency (48 KB per 384 MMA cycles).
+// Here each CTA stages its own 128 rows of A but only HALF of the 256-row W tile, and one tcgen05.mma
+// with M = 256, N = 256 consumes both CTAs' shared memory: same bytes per stage, twice the MMA work.
+template <int FMT>
+struct PairStage {
+  static constexpr int SF_DN_BYTES = (FMT == SHARQ_NVFP4) ? 2048 : 1024;
+  static constexpr int A_DN = 0;
+  static constexpr int W = A_DN + BM * 128;              // this CTA's 128 rows of the 256-row W tile
+  static constexpr int A_SP = W + 128 * 128;
+  static constexpr int META = A_SP + BM * 64;
+  static constexpr int SFA_SP = META + 2048;
+  static constexpr int SFA_DN = SFA_SP + 1024;
+  static constexpr int SFB_SP = SFA_DN + SF_DN_BYTES;    // all 256 W rows: both CTAs need every B scale
+  static constexpr int SFB_DN = SFB_SP + 2 * 1024;
+  static constexpr int RAW = SFB_DN + 2 * SF_DN_BYTES;
+  static constexpr int BYTES = (RAW + 1023) / 1024 * 1024;
+  static constexpr int STAGES = 4;
+  static constexpr int SMEM = STAGES * BYTES + 1024 + 256;
+  static constexpr int BN = 256;
+  static constexpr int SFB_COLS = 8;
+  static constexpr int E_COL = 256, SFA_SP_COL = 260, SFA_DN_COL = 268, SFB_SP_COL = 284, SFB_DN_COL = 300;
+};
+
+template <int FMT>
+__global__ void __launch_bounds__(kThreads, 1)
+sharq_linear_pair_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_constant__ CUtensorMap tm_a_dn,
+                         const __grid_constant__ CUtensorMap tm_w, const KParams p) {
+  using S = PairStage<FMT>;
+  constexpr bool NV = (FMT == SHARQ_NVFP4);
+  extern __shared__ uint8_t smem_raw[];
+  const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+  const uint32_t bars = smem_base + S::STAGES * S::BYTES;
+  auto full_bar = [&](int s) { return bars + 8u * s; };                       // used in the leader CTA
+  auto full1_bar = [&](int s) { return bars + 8u * (S::STAGES + s); };        // CTA 1: its own bulk copies
+  auto empty_bar = [&](int s) { return bars + 8u * (2 * S::STAGES + s); };
+  const uint32_t tmem_full_bar = bars + 8u * (3 * S::STAGES);
+  const uint32_t tmem_empty_bar = bars + 8u * (3 * S::STAGES + 1);            // leader CTA
+  const uint32_t tmem_ptr_smem = bars + 8u * (3 * S::STAGES + 2);
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int rank = (int)tc::cluster_ctarank();
+  const bool do_sp = p.path != 2, do_dn = p.path != 1;
+  const int num_kb = p.K / BK;
+  const int m_pairs = (p.m_blocks + 1) / 2;
+  const int total = m_pairs * (p.D / S::BN);
+  const int tile0 = (int)tc::cluster_id_x(), tile_step = (int)(gridDim.x >> 1);
+
+  if (warp == 0 && lane == 0) {
+    tc::prefetch_tmap(&tm_a_sp);
+    tc::prefetch_tmap(&tm_a_dn);
+    tc::prefetch_tmap(&tm_w);
+  }
+  if (warp == 1 && lane == 0) {
+    for (int s = 0; s < S::STAGES; ++s) {
+      tc::mbar_init(full_bar(s), 2);             // leader producer's expect_tx + CTA 1's relay
+      tc::mbar_init(full1_bar(s), 1);
+      tc::mbar_init(empty_bar(s), 1);
+    }
+    tc::mbar_init(tmem_full_bar, 1);
+    tc::mbar_init(tmem_empty_bar, 8);            // four epilogue warps in each CTA
+    tc::fence_mbar_init();
+  }
+  if (warp == 2) tc::tmem_alloc_pair<kTmemCols>(tmem_ptr_smem);
+  tc::tc_fence_before();
+  __syncwarp();
+  tc::cluster_sync_all();                        // peer barriers initialised before any remote signal
+  tc::tc_fence_after();
+  uint32_t tmem_base;
+  asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_ptr_smem));
+
+  if (warp == 0) {
+    // =========================== TMA producer (both CTAs) ===================================
+    if (lane == 0) {
+      const uint64_t pol = tc::policy_evict_normal();
+      const int64_t Kc = p.K;
+      const uint32_t tx_tensor = 2u * (128 * 128 + (do_sp ? BM * 64 : 0) + (do_dn ? BM * 128 : 0));
+      const uint32_t tx_bulk = (do_sp ? 2048 + 1024 + 2 * 1024 : 0) + (do_dn ? 3 * S::SF_DN_BYTES : 0);
+      uint32_t it = 0;
+      for (int tile = tile0; tile < total; tile += tile_step) {
+        const int m_blk = 2 * (tile % m_pairs) + rank, n_blk = tile / m_pairs;
+        const int m_sf = min(m_blk, p.m_blocks - 1);       // a ragged pair's second CTA: valid memory, unused rows
+        const int n0 = n_blk * S::BN;
+        const int64_t wblk0 = n0 / 128;
+        const uint8_t* sfa_sp = p.sp_sf + (size_t)m_sf * (Kc / 128) * 512;
+        const uint8_t* sfa_dn = p.dn_sf + (size_t)m_sf * (Kc / 256) * (S::SF_DN_BYTES);
+        const uint8_t* meta = p.sp_meta + (size_t)m_sf * (Kc / 256) * 2048;
+        for (int kb = 0; kb < num_kb; ++kb, ++it) {
+          const int s = it % S::STAGES;
+          const uint32_t ph = (it / S::STAGES) & 1;
+          tc::mbar_wait(empty_bar(s), ph ^ 1);
+          const uint32_t st = smem_base + s * S::BYTES;
+          const uint32_t fb = full_bar(s);                  // tensor loads: leader's barrier (peer bit cleared)
+          const uint32_t lb = rank == 0 ? fb : full1_bar(s);   // bulk copies: a barrier of this CTA
+          tc::mbar_expect_tx(lb, rank == 0 ? tx_tensor + tx_bulk : tx_bulk);
+          tc::tma_load_2d_pair(st + S::W, &tm_w, fb, kb * 128, n0 + rank * 128, pol);
+          if (do_sp) {
+            tc::tma_load_2d_pair(st + S::A_SP, &tm_a_sp, fb, kb * 64, m_blk * BM, pol);
+            tc::bulk_load(st + S::META, meta + (size_t)kb * 2048, 2048, lb, pol);
+            tc::bulk_load(st + S::SFA_SP, sfa_sp + (size_t)kb * 1024, 1024, lb, pol);
+#pragma unroll
+            for (int nb = 0; nb < 2; ++nb)
+              tc::bulk_load(st + S::SFB_SP + nb * 1024,
+                            p.w_sf_sp + ((size_t)(wblk0 + nb) * (Kc / 128) + (size_t)kb * 2) * 512, 1024, lb, pol);
+          }
+          if (do_dn) {
+            tc::tma_load_2d_pair(st + S::A_DN, &tm_a_dn, fb, kb * 128, m_blk * BM, pol);
+            tc::bulk_load(st + S::SFA_DN, sfa_dn + (size_t)kb * S::SF_DN_BYTES, S::SF_DN_BYTES, lb, pol);
+#pragma unroll
+            for (int nb = 0; nb < 2; ++nb)
+              tc::bulk_load(st + S::SFB_DN + nb * S::SF_DN_BYTES,
+                            p.w_sf_dn + ((size_t)(wblk0 + nb) * (Kc / 256) + (size_t)kb) * S::SF_DN_BYTES,
+                            S::SF_DN_BYTES, lb, pol);
+          }
+        }
+      }
+    }
+  } else if (warp == 1) {
+    if (lane == 0 && rank == 1) {
+      // ===================== CTA 1: relay "my scale factors / metadata have landed" ===============
+      uint32_t it = 0;
+      for (int tile = tile0; tile < total; tile += tile_step)
+        for (int kb = 0; kb < num_kb; ++kb, ++it) {
+          const int s = it % S::STAGES;
+          tc::mbar_wait(full1_bar(s), (it / S::STAGES) & 1);
+          tc::mbar_arrive_cluster(tc::map_to_cta(full_bar(s), 0));
+        }
+    } else if (lane == 0) {
+      // =========================== MMA issuer (leader CTA) ===================================
+      const uint32_t idesc_sp = tc::idesc_fp4(256, S::BN, true, !NV, 0, 0);
+      uint32_t it = 0, n_unit = 0;
+      for (int tile = tile0; tile < total; tile += tile_step, ++n_unit) {
+        tc::mbar_wait(tmem_empty_bar, (n_unit & 1u) ^ 1u);    // both CTAs' epilogues drained the accumulator
+        tc::tc_fence_after();
+        uint32_t accumulate = 0;
+        for (int kb = 0; kb < num_kb; ++kb, ++it) {
+          const int s = it % S::STAGES;
+          tc::mbar_wait(full_bar(s), (it / S::STAGES) & 1);
+          tc::tc_fence_after();
+          const uint32_t st = smem_base + s * S::BYTES;
+          if (do_sp) {
+            tc::tc_cp_meta_pair(tmem_base + S::E_COL, tc::smem_desc(st + S::META, 128, 0));
+#pragma unroll
+            for (int a = 0; a < 2; ++a) {
+              tc::tc_cp_sf_pair(tmem_base + S::SFA_SP_COL + 4 * a, tc::smem_desc(st + S::SFA_SP + 512 * a, 128, 0));
+#pragma unroll
+              for (int nb = 0; nb < 2; ++nb)
+                tc::tc_cp_sf_pair(tmem_base + S::SFB_SP_COL + S::SFB_COLS * a + 4 * nb,
+                                  tc::smem_desc(st + S::SFB_SP + nb * 1024 + 512 * a, 128, 0));
+            }
+#pragma unroll
+            for (int j = 0; j < 2; ++j) {
+              tc::mma_sparse_pair(tmem_base, tc::smem_desc(st + S::A_SP + 32 * j, 512, 4),
+                                  tc::smem_desc(st + S::W + 64 * j, 1024, 2), idesc_sp,
+                                  tmem_base + S::SFA_SP_COL + 4 * j, tmem_base + S::SFB_SP_COL + S::SFB_COLS * j,
+                                  tmem_base + S::E_COL + 2 * j, accumulate);
+              accumulate = 1;
+            }
+          }
+          if (do_dn) {
+            constexpr int ATOMS = NV ? 4 : 2;
+#pragma unroll
+            for (int a = 0; a < ATOMS; ++a) {
+              tc::tc_cp_sf_pair(tmem_base + S::SFA_DN_COL + 4 * a, tc::smem_desc(st + S::SFA_DN + 512 * a, 128, 0));
+#pragma unroll
+              for (int nb = 0; nb < 2; ++nb)
+                tc::tc_cp_sf_pair(tmem_base + S::SFB_DN_COL + S::SFB_COLS * a + 4 * nb,
+                                  tc::smem_desc(st + S::SFB_DN + nb * S::SF_DN_BYTES + 512 * a, 128, 0));
+            }
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+              const int atom = NV ? j : j / 2;
+              const uint32_t sf_id = NV ? 0u : (uint32_t)(j & 1) * 2u;
+              const uint32_t idesc_dn = tc::idesc_fp4(256, S::BN, false, !NV, sf_id, sf_id);
+              tc::mma_dense_pair<NV>(tmem_base, tc::smem_desc(st + S::A_DN + 32 * j, 1024, 2),
+                                     tc::smem_desc(st + S::W + 32 * j, 1024, 2), idesc_dn,
+                                     tmem_base + S::SFA_DN_COL + 4 * atom,
+                                     tmem_base + S::SFB_DN_COL + S::SFB_COLS * atom, accumulate);
+              accumulate = 1;
+            }
+          }
+          tc::tc_commit_pair(empty_bar(s), 3);              // frees this slot in BOTH CTAs
+        }
+        tc::tc_commit_pair(tmem_full_bar, 3);
+      }
+    }
+  } else {
+    // =========================== epilogue (both CTAs) ==========================================
+    const int sub = warp & 3;
+    const int r_local = sub * 32 + lane;
+    const uint32_t lane_addr = tmem_base + ((uint32_t)(sub * 32) << 16);
+    const uint32_t empty_remote = tc::map_to_cta(tmem_empty_bar, 0);
+    uint32_t n_unit = 0;
+    for (int tile = tile0; tile < total; tile += tile_step, ++n_unit) {
+      const int m_blk = 2 * (tile % m_pairs) + rank, n_blk = tile / m_pairs;
+      const int64_t row = (int64_t)m_blk * BM + r_local;
+      const bool row_ok = row < p.T;
+      const float scale = row_ok ? __fmul_rn(p.row_scale[row], p.w_ts[0]) : 0.0f;
+      tc::mbar_wait(tmem_full_bar, n_unit & 1u);
+      tc::tc_fence_after();
+#pragma unroll 1
+      for (int c = 0; c < S::BN / 32; ++c) {
+        uint32_t v[32];
+        tc::tmem_ld32(lane_addr + c * 32, v);
+        tc::tmem_ld_wait();
+        if (row_ok) {
+          float f[32];
+#pragma unroll
+          for (int i = 0; i < 32; ++i) f[i] = __uint_as_float(v[i]);
+          store_row<32>(p, row, n_blk * S::BN + c * 32, scale, f);
+        }
+      }
+      tc::tc_fence_before();
+      __syncwarp();
+      if (lane == 0) tc::mbar_arrive_cluster(empty_remote);
+    }
+  }
+  tc::tc_fence_before();
+  __syncwarp();
+  tc::cluster_sync_all();                        // the peer may still be reading / being written by the pair MMA
+  if (warp == 2) {
+    tc::tc_fence_after();
+    tc::tmem_dealloc_pair<kTmemCols>(tmem_base);
+  }
+}
+
 // ---- host: tensor maps + launch ----------------------------------------------------------------
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
@@ -435,6 +661,32 @@ sharq_status launch_tiles(const LinearArgs& a, const GroupInfo& g, int64_t rows_
   KParams p{(const uint8_t*)a.sp_sf, (const uint8_t*)a.sp_meta, (const uint8_t*)a.dn_sf, (const uint8_t*)a.w_sf_sp,
             (const uint8_t*)a.w_sf_dn, a.row_scale, a.w_ts, (const uint16_t*)a.bias, a.Y, a.ldy,
             (int32_t)a.T, (int32_t)a.D, (int32_t)a.K, a.out_dtype, a.path, (int32_t)m_blocks, (int32_t)tiles};
+  const char* no_pair = getenv("SHARQ_DEBUG_NO_PAIR");
+  const char* force_pair = getenv("SHARQ_DEBUG_FORCE_PAIR");
+  const bool pair_worth = ((m_blocks + 1) / 2) * (a.D / 256) >= num_sms / 4 || (force_pair && force_pair[0] == '1');
+  if (E == 0 && m_blocks >= 2 && a.D % 256 == 0 && BN == 128 && pair_worth && !(no_pair && no_pair[0] == '1')) {
+    using P = PairStage<FMT>;
+    CUtensorMap tm_wp;
+    if (!make_map(&tm_wp, a.w_codes, (uint64_t)w_rows, (uint64_t)a.K / 2, 128, 128)) return SHARQ_ECUDA;
+    auto kfn = sharq_linear_pair_kernel<FMT>;
+    if (cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, P::SMEM) != cudaSuccess)
+      return SHARQ_ECUDA;
+    const int64_t pair_tiles = ((m_blocks + 1) / 2) * (a.D / 256);
+    const int64_t clusters = pair_tiles < num_sms / 2 ? pair_tiles : num_sms / 2;
+    cudaLaunchConfig_t lp{};
+    cudaLaunchAttribute at[1];
+    lp.blockDim = dim3(kThreads);
+    lp.gridDim = dim3((unsigned)(2 * clusters));
+    lp.dynamicSmemBytes = P::SMEM;
+    lp.stream = st;
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = 2;
+    at[0].val.clusterDim.y = 1;
+    at[0].val.clusterDim.z = 1;
+    lp.attrs = at;
+    lp.numAttrs = 1;
+    return cudaLaunchKernelEx(&lp, kfn, tm_sp, tm_dn, tm_wp, p) == cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
+  }
   const int splits = choose_splits(tiles, (int)(a.K / BK), num_sms);
   cudaLaunchConfig_t lc{};
   cudaLaunchAttribute attr[1];
