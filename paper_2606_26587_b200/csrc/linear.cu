@@ -179,7 +179,8 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
 
   if (warp == 0) {
     // =========================== TMA producer ===============================================
-    if (lane == 0) {
+    {
+      const bool lead = tc::elect_one() != 0;          // whole warp runs the loop, one lane issues
       const uint64_t pol_act = SPLIT ? tc::policy_evict_last() : tc::policy_evict_normal();
       const uint64_t pol_w = SPLIT ? tc::policy_evict_first() : tc::policy_evict_normal();
       const int64_t Kc = p.K;
@@ -200,21 +201,21 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
           tc::mbar_wait(empty_bar(s), ph ^ 1);
           const uint32_t st = smem_base + s * S::BYTES;
           const uint32_t fb = full_bar(s);
-          tc::mbar_expect_tx(fb, tx);
-          tc::tma_load_2d(st + S::W, &tm_w, fb, kb * 128, w_row0, pol_w);
+          if (lead) tc::mbar_expect_tx(fb, tx);
+          if (lead) tc::tma_load_2d(st + S::W, &tm_w, fb, kb * 128, w_row0, pol_w);
           if (do_sp) {
-            tc::tma_load_2d(st + S::A_SP, &tm_a_sp, fb, kb * 64, u.m_blk * BM, pol_act);
-            tc::bulk_load(st + S::META, meta + (size_t)kb * 2048, 2048, fb, pol_act);
-            tc::bulk_load(st + S::SFA_SP, sfa_sp + (size_t)kb * 1024, 1024, fb, pol_act);
+            if (lead) tc::tma_load_2d(st + S::A_SP, &tm_a_sp, fb, kb * 64, u.m_blk * BM, pol_act);
+            if (lead) tc::bulk_load(st + S::META, meta + (size_t)kb * 2048, 2048, fb, pol_act);
+            if (lead) tc::bulk_load(st + S::SFA_SP, sfa_sp + (size_t)kb * 1024, 1024, fb, pol_act);
             for (int nb = 0; nb < S::NB; ++nb)
-              tc::bulk_load(st + S::SFB_SP + nb * 1024,
+              if (lead) tc::bulk_load(st + S::SFB_SP + nb * 1024,
                             p.w_sf_sp + ((size_t)(wblk0 + nb) * (Kc / 128) + (size_t)kb * 2) * 512, 1024, fb, pol_w);
           }
           if (do_dn) {
-            tc::tma_load_2d(st + S::A_DN, &tm_a_dn, fb, kb * 128, u.m_blk * BM, pol_act);
-            tc::bulk_load(st + S::SFA_DN, sfa_dn + (size_t)kb * S::SF_DN_BYTES, S::SF_DN_BYTES, fb, pol_act);
+            if (lead) tc::tma_load_2d(st + S::A_DN, &tm_a_dn, fb, kb * 128, u.m_blk * BM, pol_act);
+            if (lead) tc::bulk_load(st + S::SFA_DN, sfa_dn + (size_t)kb * S::SF_DN_BYTES, S::SF_DN_BYTES, fb, pol_act);
             for (int nb = 0; nb < S::NB; ++nb)
-              tc::bulk_load(st + S::SFB_DN + nb * S::SF_DN_BYTES,
+              if (lead) tc::bulk_load(st + S::SFB_DN + nb * S::SF_DN_BYTES,
                             p.w_sf_dn + ((size_t)(wblk0 + nb) * (Kc / 256) + (size_t)kb) * S::SF_DN_BYTES,
                             S::SF_DN_BYTES, fb, pol_w);
           }
@@ -223,7 +224,8 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
     }
   } else if (warp == 1) {
     // =========================== MMA issuer =================================================
-    if (lane == 0) {
+    {
+      const bool lead = tc::elect_one() != 0;
       const uint32_t idesc_sp = tc::idesc_fp4(BM, BN, true, !NV, 0, 0);
       uint32_t it = 0, n_unit = 0;
       for (int tile = tile0; tile < p.total_tiles; tile += tile_step, ++n_unit) {
@@ -241,18 +243,18 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
           tc::tc_fence_after();
           const uint32_t st = smem_base + s * S::BYTES;
           if (do_sp) {
-            tc::tc_cp_meta(tmem_base + S::E_COL, tc::smem_desc(st + S::META, 128, 0));
+            if (lead) tc::tc_cp_meta(tmem_base + S::E_COL, tc::smem_desc(st + S::META, 128, 0));
 #pragma unroll
             for (int a = 0; a < 2; ++a) {
-              tc::tc_cp_sf(tmem_base + S::SFA_SP_COL + 4 * a, tc::smem_desc(st + S::SFA_SP + 512 * a, 128, 0));
+              if (lead) tc::tc_cp_sf(tmem_base + S::SFA_SP_COL + 4 * a, tc::smem_desc(st + S::SFA_SP + 512 * a, 128, 0));
 #pragma unroll
               for (int nb = 0; nb < S::NB; ++nb)
-                tc::tc_cp_sf(tmem_base + S::SFB_SP_COL + S::SFB_COLS * a + 4 * nb,
+                if (lead) tc::tc_cp_sf(tmem_base + S::SFB_SP_COL + S::SFB_COLS * a + 4 * nb,
                              tc::smem_desc(st + S::SFB_SP + nb * 1024 + 512 * a, 128, 0));
             }
 #pragma unroll
             for (int j = 0; j < 2; ++j) {
-              tc::mma_sparse(acc, tc::smem_desc(st + S::A_SP + 32 * j, 512, 4),
+              if (lead) tc::mma_sparse(acc, tc::smem_desc(st + S::A_SP + 32 * j, 512, 4),
                              tc::smem_desc(st + S::W + 64 * j, 1024, 2), idesc_sp, tmem_base + S::SFA_SP_COL + 4 * j,
                              tmem_base + S::SFB_SP_COL + S::SFB_COLS * j + sfb_shift, tmem_base + S::E_COL + 2 * j,
                              accumulate);
@@ -263,10 +265,10 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
             constexpr int ATOMS = NV ? 4 : 2;
 #pragma unroll
             for (int a = 0; a < ATOMS; ++a) {
-              tc::tc_cp_sf(tmem_base + S::SFA_DN_COL + 4 * a, tc::smem_desc(st + S::SFA_DN + 512 * a, 128, 0));
+              if (lead) tc::tc_cp_sf(tmem_base + S::SFA_DN_COL + 4 * a, tc::smem_desc(st + S::SFA_DN + 512 * a, 128, 0));
 #pragma unroll
               for (int nb = 0; nb < S::NB; ++nb)
-                tc::tc_cp_sf(tmem_base + S::SFB_DN_COL + S::SFB_COLS * a + 4 * nb,
+                if (lead) tc::tc_cp_sf(tmem_base + S::SFB_DN_COL + S::SFB_COLS * a + 4 * nb,
                              tc::smem_desc(st + S::SFB_DN + nb * S::SF_DN_BYTES + 512 * a, 128, 0));
             }
 #pragma unroll
@@ -274,16 +276,16 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
               const int atom = NV ? j : j / 2;               // MXFP4: two K=64 MMAs share one 4-scale atom
               const uint32_t sf_id = NV ? 0u : (uint32_t)(j & 1) * 2u;
               const uint32_t idesc_dn = tc::idesc_fp4(BM, BN, false, !NV, sf_id, sf_id);
-              tc::mma_dense<NV>(acc, tc::smem_desc(st + S::A_DN + 32 * j, 1024, 2),
+              if (lead) tc::mma_dense<NV>(acc, tc::smem_desc(st + S::A_DN + 32 * j, 1024, 2),
                                 tc::smem_desc(st + S::W + 32 * j, 1024, 2), idesc_dn,
                                 tmem_base + S::SFA_DN_COL + 4 * atom,
                                 tmem_base + S::SFB_DN_COL + S::SFB_COLS * atom + sfb_shift, accumulate);
               accumulate = 1;
             }
           }
-          tc::tc_commit(empty_bar(s));                   // smem slot reusable once these MMAs have read it
+          if (lead) tc::tc_commit(empty_bar(s));                   // smem slot reusable once these MMAs have read it
         }
-        tc::tc_commit(tmem_full_bar(as));                // accumulator complete
+        if (lead) tc::tc_commit(tmem_full_bar(as));                // accumulator complete
       }
     }
   } else {
@@ -451,7 +453,8 @@ sharq_linear_pair_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __gr
 
   if (warp == 0) {
     // =========================== TMA producer (both CTAs) ===================================
-    if (lane == 0) {
+    {
+      const bool lead = tc::elect_one() != 0;
       const uint64_t pol = tc::policy_evict_normal();
       const int64_t Kc = p.K;
       const uint32_t tx_tensor = 2u * (128 * 128 + (do_sp ? BM * 64 : 0) + (do_dn ? BM * 128 : 0));
@@ -472,23 +475,23 @@ sharq_linear_pair_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __gr
           const uint32_t st = smem_base + s * S::BYTES;
           const uint32_t fb = full_bar(s);                  // tensor loads: leader's barrier (peer bit cleared)
           const uint32_t lb = rank == 0 ? fb : full1_bar(s);   // bulk copies: a barrier of this CTA
-          tc::mbar_expect_tx(lb, rank == 0 ? tx_tensor + tx_bulk : tx_bulk);
-          tc::tma_load_2d_pair(st + S::W, &tm_w, fb, kb * 128, n0 + rank * 128, pol);
+          if (lead) tc::mbar_expect_tx(lb, rank == 0 ? tx_tensor + tx_bulk : tx_bulk);
+          if (lead) tc::tma_load_2d_pair(st + S::W, &tm_w, fb, kb * 128, n0 + rank * 128, pol);
           if (do_sp) {
-            tc::tma_load_2d_pair(st + S::A_SP, &tm_a_sp, fb, kb * 64, m_blk * BM, pol);
-            tc::bulk_load(st + S::META, meta + (size_t)kb * 2048, 2048, lb, pol);
-            tc::bulk_load(st + S::SFA_SP, sfa_sp + (size_t)kb * 1024, 1024, lb, pol);
+            if (lead) tc::tma_load_2d_pair(st + S::A_SP, &tm_a_sp, fb, kb * 64, m_blk * BM, pol);
+            if (lead) tc::bulk_load(st + S::META, meta + (size_t)kb * 2048, 2048, lb, pol);
+            if (lead) tc::bulk_load(st + S::SFA_SP, sfa_sp + (size_t)kb * 1024, 1024, lb, pol);
 #pragma unroll
             for (int nb = 0; nb < 2; ++nb)
-              tc::bulk_load(st + S::SFB_SP + nb * 1024,
+              if (lead) tc::bulk_load(st + S::SFB_SP + nb * 1024,
                             p.w_sf_sp + ((size_t)(wblk0 + nb) * (Kc / 128) + (size_t)kb * 2) * 512, 1024, lb, pol);
           }
           if (do_dn) {
-            tc::tma_load_2d_pair(st + S::A_DN, &tm_a_dn, fb, kb * 128, m_blk * BM, pol);
-            tc::bulk_load(st + S::SFA_DN, sfa_dn + (size_t)kb * S::SF_DN_BYTES, S::SF_DN_BYTES, lb, pol);
+            if (lead) tc::tma_load_2d_pair(st + S::A_DN, &tm_a_dn, fb, kb * 128, m_blk * BM, pol);
+            if (lead) tc::bulk_load(st + S::SFA_DN, sfa_dn + (size_t)kb * S::SF_DN_BYTES, S::SF_DN_BYTES, lb, pol);
 #pragma unroll
             for (int nb = 0; nb < 2; ++nb)
-              tc::bulk_load(st + S::SFB_DN + nb * S::SF_DN_BYTES,
+              if (lead) tc::bulk_load(st + S::SFB_DN + nb * S::SF_DN_BYTES,
                             p.w_sf_dn + ((size_t)(wblk0 + nb) * (Kc / 256) + (size_t)kb) * S::SF_DN_BYTES,
                             S::SF_DN_BYTES, lb, pol);
           }
@@ -496,7 +499,8 @@ sharq_linear_pair_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __gr
       }
     }
   } else if (warp == 1) {
-    if (lane == 0 && rank == 1) {
+    if (rank == 1) {
+      if (lane == 0) {
       // ===================== CTA 1: relay "my scale factors / metadata have landed" ===============
       uint32_t it = 0;
       for (int tile = tile0; tile < total; tile += tile_step)
@@ -505,7 +509,9 @@ sharq_linear_pair_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __gr
           tc::mbar_wait(full1_bar(s), (it / S::STAGES) & 1);
           tc::mbar_arrive_cluster(tc::map_to_cta(full_bar(s), 0));
         }
-    } else if (lane == 0) {
+    }
+    } else {
+      const bool lead = tc::elect_one() != 0;
       // =========================== MMA issuer (leader CTA) ===================================
       const uint32_t idesc_sp = tc::idesc_fp4(256, S::BN, true, !NV, 0, 0);
       uint32_t it = 0, n_unit = 0;
@@ -519,18 +525,18 @@ sharq_linear_pair_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __gr
           tc::tc_fence_after();
           const uint32_t st = smem_base + s * S::BYTES;
           if (do_sp) {
-            tc::tc_cp_meta_pair(tmem_base + S::E_COL, tc::smem_desc(st + S::META, 128, 0));
+            if (lead) tc::tc_cp_meta_pair(tmem_base + S::E_COL, tc::smem_desc(st + S::META, 128, 0));
 #pragma unroll
             for (int a = 0; a < 2; ++a) {
-              tc::tc_cp_sf_pair(tmem_base + S::SFA_SP_COL + 4 * a, tc::smem_desc(st + S::SFA_SP + 512 * a, 128, 0));
+              if (lead) tc::tc_cp_sf_pair(tmem_base + S::SFA_SP_COL + 4 * a, tc::smem_desc(st + S::SFA_SP + 512 * a, 128, 0));
 #pragma unroll
               for (int nb = 0; nb < 2; ++nb)
-                tc::tc_cp_sf_pair(tmem_base + S::SFB_SP_COL + S::SFB_COLS * a + 4 * nb,
+                if (lead) tc::tc_cp_sf_pair(tmem_base + S::SFB_SP_COL + S::SFB_COLS * a + 4 * nb,
                                   tc::smem_desc(st + S::SFB_SP + nb * 1024 + 512 * a, 128, 0));
             }
 #pragma unroll
             for (int j = 0; j < 2; ++j) {
-              tc::mma_sparse_pair(tmem_base, tc::smem_desc(st + S::A_SP + 32 * j, 512, 4),
+              if (lead) tc::mma_sparse_pair(tmem_base, tc::smem_desc(st + S::A_SP + 32 * j, 512, 4),
                                   tc::smem_desc(st + S::W + 64 * j, 1024, 2), idesc_sp,
                                   tmem_base + S::SFA_SP_COL + 4 * j, tmem_base + S::SFB_SP_COL + S::SFB_COLS * j,
                                   tmem_base + S::E_COL + 2 * j, accumulate);
@@ -541,10 +547,10 @@ sharq_linear_pair_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __gr
             constexpr int ATOMS = NV ? 4 : 2;
 #pragma unroll
             for (int a = 0; a < ATOMS; ++a) {
-              tc::tc_cp_sf_pair(tmem_base + S::SFA_DN_COL + 4 * a, tc::smem_desc(st + S::SFA_DN + 512 * a, 128, 0));
+              if (lead) tc::tc_cp_sf_pair(tmem_base + S::SFA_DN_COL + 4 * a, tc::smem_desc(st + S::SFA_DN + 512 * a, 128, 0));
 #pragma unroll
               for (int nb = 0; nb < 2; ++nb)
-                tc::tc_cp_sf_pair(tmem_base + S::SFB_DN_COL + S::SFB_COLS * a + 4 * nb,
+                if (lead) tc::tc_cp_sf_pair(tmem_base + S::SFB_DN_COL + S::SFB_COLS * a + 4 * nb,
                                   tc::smem_desc(st + S::SFB_DN + nb * S::SF_DN_BYTES + 512 * a, 128, 0));
             }
 #pragma unroll
@@ -552,16 +558,16 @@ sharq_linear_pair_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __gr
               const int atom = NV ? j : j / 2;
               const uint32_t sf_id = NV ? 0u : (uint32_t)(j & 1) * 2u;
               const uint32_t idesc_dn = tc::idesc_fp4(256, S::BN, false, !NV, sf_id, sf_id);
-              tc::mma_dense_pair<NV>(tmem_base, tc::smem_desc(st + S::A_DN + 32 * j, 1024, 2),
+              if (lead) tc::mma_dense_pair<NV>(tmem_base, tc::smem_desc(st + S::A_DN + 32 * j, 1024, 2),
                                      tc::smem_desc(st + S::W + 32 * j, 1024, 2), idesc_dn,
                                      tmem_base + S::SFA_DN_COL + 4 * atom,
                                      tmem_base + S::SFB_DN_COL + S::SFB_COLS * atom, accumulate);
               accumulate = 1;
             }
           }
-          tc::tc_commit_pair(empty_bar(s), 3);              // frees this slot in BOTH CTAs
+          if (lead) tc::tc_commit_pair(empty_bar(s), 3);              // frees this slot in BOTH CTAs
         }
-        tc::tc_commit_pair(tmem_full_bar, 3);
+        if (lead) tc::tc_commit_pair(tmem_full_bar, 3);
       }
     }
   } else {

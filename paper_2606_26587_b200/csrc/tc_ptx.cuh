@@ -32,6 +32,16 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
   while (!mbar_try_wait(bar, parity)) {}
 }
 
+// one lane of a converged warp (the same lane every time): tcgen05 / TMA instructions are issued under
+// this predicate so that their operands stay warp-uniform (uniform registers, no per-lane moves)
+__device__ __forceinline__ uint32_t elect_one() {
+  uint32_t pred;
+  asm volatile("{ .reg .pred p;\n\t"
+               "elect.sync _|p, 0xffffffff;\n\t"
+               "selp.u32 %0, 1, 0, p; }" : "=r"(pred));
+  return pred;
+}
+
 // ---- TMA ------------------------------------------------------------------------------------
 __device__ __forceinline__ void prefetch_tmap(const void* tmap) {
   asm volatile("prefetch.tensormap [%0];" ::"l"(tmap) : "memory");
