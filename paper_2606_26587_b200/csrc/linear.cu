@@ -407,14 +407,16 @@ struct PairStage {
 template <int FMT>
 __global__ void __launch_bounds__(kThreads, 1)
 sharq_linear_pair_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_constant__ CUtensorMap tm_a_dn,
-                         const __grid_constant__ CUtensorMap tm_w, const KParams p) {
+                         const __grid_constant__ CUtensorMap tm_w, const __grid_constant__ CUtensorMap tm_sfa_sp,
+                         const __grid_constant__ CUtensorMap tm_sfa_dn, const __grid_constant__ CUtensorMap tm_meta,
+                         const __grid_constant__ CUtensorMap tm_sfb_sp, const __grid_constant__ CUtensorMap tm_sfb_dn,
+                         const KParams p) {
   using S = PairStage<FMT>;
   constexpr bool NV = (FMT == SHARQ_NVFP4);
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
   const uint32_t bars = smem_base + S::STAGES * S::BYTES;
   auto full_bar = [&](int s) { return bars + 8u * s; };                       // used in the leader CTA
-  auto full1_bar = [&](int s) { return bars + 8u * (S::STAGES + s); };        // CTA 1: its own bulk copies
   auto empty_bar = [&](int s) { return bars + 8u * (2 * S::STAGES + s); };
   const uint32_t tmem_full_bar = bars + 8u * (3 * S::STAGES);
   const uint32_t tmem_empty_bar = bars + 8u * (3 * S::STAGES + 1);            // leader CTA
@@ -432,11 +434,15 @@ sharq_linear_pair_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __gr
     tc::prefetch_tmap(&tm_a_sp);
     tc::prefetch_tmap(&tm_a_dn);
     tc::prefetch_tmap(&tm_w);
+    tc::prefetch_tmap(&tm_sfa_sp);
+    tc::prefetch_tmap(&tm_sfa_dn);
+    tc::prefetch_tmap(&tm_meta);
+    tc::prefetch_tmap(&tm_sfb_sp);
+    tc::prefetch_tmap(&tm_sfb_dn);
   }
   if (warp == 1 && lane == 0) {
     for (int s = 0; s < S::STAGES; ++s) {
-      tc::mbar_init(full_bar(s), 2);             // leader producer's expect_tx + CTA 1's relay
-      tc::mbar_init(full1_bar(s), 1);
+      tc::mbar_init(full_bar(s), 1);             // leader's expect_tx; every load of the pair completes here
       tc::mbar_init(empty_bar(s), 1);
     }
     tc::mbar_init(tmem_full_bar, 1);
@@ -457,60 +463,47 @@ sharq_linear_pair_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __gr
       const bool lead = tc::elect_one() != 0;
       const uint64_t pol = tc::policy_evict_normal();
       const int64_t Kc = p.K;
-      const uint32_t tx_tensor = 2u * (128 * 128 + (do_sp ? BM * 64 : 0) + (do_dn ? BM * 128 : 0));
-      const uint32_t tx_bulk = (do_sp ? 2048 + 1024 + 2 * 1024 : 0) + (do_dn ? 3 * S::SF_DN_BYTES : 0);
+      // every load of the pair (tiles, scale-factor atoms, metadata) is a cta_group::2 tensor copy whose
+      // complete_tx lands on the LEADER's full barrier: no cross-CTA hand-off inside the ring
+      const uint32_t tx = 2u * (128 * 128 + (do_sp ? BM * 64 + 2048 + 1024 + 2 * 1024 : 0) +
+                                (do_dn ? BM * 128 + 3 * S::SF_DN_BYTES : 0));
+      constexpr int DN_ROWS = S::SF_DN_BYTES / 1024;       // 1024-byte rows of the scale-factor tensor maps
+      const int kq = p.K / 256;
       uint32_t it = 0;
       for (int tile = tile0; tile < total; tile += tile_step) {
         const int m_blk = 2 * (tile % m_pairs) + rank, n_blk = tile / m_pairs;
         const int m_sf = min(m_blk, p.m_blocks - 1);       // a ragged pair's second CTA: valid memory, unused rows
         const int n0 = n_blk * S::BN;
-        const int64_t wblk0 = n0 / 128;
-        const uint8_t* sfa_sp = p.sp_sf + (size_t)m_sf * (Kc / 128) * 512;
-        const uint8_t* sfa_dn = p.dn_sf + (size_t)m_sf * (Kc / 256) * (S::SF_DN_BYTES);
-        const uint8_t* meta = p.sp_meta + (size_t)m_sf * (Kc / 256) * 2048;
+        const int wblk0 = n0 / 128;
         for (int kb = 0; kb < num_kb; ++kb, ++it) {
           const int s = it % S::STAGES;
           const uint32_t ph = (it / S::STAGES) & 1;
           tc::mbar_wait(empty_bar(s), ph ^ 1);
           const uint32_t st = smem_base + s * S::BYTES;
-          const uint32_t fb = full_bar(s);                  // tensor loads: leader's barrier (peer bit cleared)
-          const uint32_t lb = rank == 0 ? fb : full1_bar(s);   // bulk copies: a barrier of this CTA
-          if (lead) tc::mbar_expect_tx(lb, rank == 0 ? tx_tensor + tx_bulk : tx_bulk);
+          const uint32_t fb = full_bar(s);
+          if (lead && rank == 0) tc::mbar_expect_tx(fb, tx);
           if (lead) tc::tma_load_2d_pair(st + S::W, &tm_w, fb, kb * 128, n0 + rank * 128, pol);
           if (do_sp) {
             if (lead) tc::tma_load_2d_pair(st + S::A_SP, &tm_a_sp, fb, kb * 64, m_blk * BM, pol);
-            if (lead) tc::bulk_load(st + S::META, meta + (size_t)kb * 2048, 2048, lb, pol);
-            if (lead) tc::bulk_load(st + S::SFA_SP, sfa_sp + (size_t)kb * 1024, 1024, lb, pol);
+            if (lead) tc::tma_load_2d_pair(st + S::META, &tm_meta, fb, 0, (m_sf * kq + kb) * 2, pol);
+            if (lead) tc::tma_load_2d_pair(st + S::SFA_SP, &tm_sfa_sp, fb, 0, m_sf * kq + kb, pol);
 #pragma unroll
             for (int nb = 0; nb < 2; ++nb)
-              if (lead) tc::bulk_load(st + S::SFB_SP + nb * 1024,
-                            p.w_sf_sp + ((size_t)(wblk0 + nb) * (Kc / 128) + (size_t)kb * 2) * 512, 1024, lb, pol);
+              if (lead) tc::tma_load_2d_pair(st + S::SFB_SP + nb * 1024, &tm_sfb_sp, fb, 0, (wblk0 + nb) * kq + kb, pol);
           }
           if (do_dn) {
             if (lead) tc::tma_load_2d_pair(st + S::A_DN, &tm_a_dn, fb, kb * 128, m_blk * BM, pol);
-            if (lead) tc::bulk_load(st + S::SFA_DN, sfa_dn + (size_t)kb * S::SF_DN_BYTES, S::SF_DN_BYTES, lb, pol);
+            if (lead) tc::tma_load_2d_pair(st + S::SFA_DN, &tm_sfa_dn, fb, 0, (m_sf * kq + kb) * DN_ROWS, pol);
 #pragma unroll
             for (int nb = 0; nb < 2; ++nb)
-              if (lead) tc::bulk_load(st + S::SFB_DN + nb * S::SF_DN_BYTES,
-                            p.w_sf_dn + ((size_t)(wblk0 + nb) * (Kc / 256) + (size_t)kb) * S::SF_DN_BYTES,
-                            S::SF_DN_BYTES, lb, pol);
+              if (lead) tc::tma_load_2d_pair(st + S::SFB_DN + nb * S::SF_DN_BYTES, &tm_sfb_dn, fb, 0,
+                                             ((wblk0 + nb) * kq + kb) * DN_ROWS, pol);
           }
         }
       }
     }
   } else if (warp == 1) {
-    if (rank == 1) {
-      if (lane == 0) {
-      // ===================== CTA 1: relay "my scale factors / metadata have landed" ===============
-      uint32_t it = 0;
-      for (int tile = tile0; tile < total; tile += tile_step)
-        for (int kb = 0; kb < num_kb; ++kb, ++it) {
-          const int s = it % S::STAGES;
-          tc::mbar_wait(full1_bar(s), (it / S::STAGES) & 1);
-          tc::mbar_arrive_cluster(tc::map_to_cta(full_bar(s), 0));
-        }
-    }
-    } else {
+    if (rank == 0) {
       const bool lead = tc::elect_one() != 0;
       // =========================== MMA issuer (leader CTA) ===================================
       const uint32_t idesc_sp = tc::idesc_fp4(256, S::BN, true, !NV, 0, 0);
@@ -654,6 +647,19 @@ int choose_splits(int64_t tiles, int num_kb, int num_sms) {
   return 1;
 }
 
+// scale-factor / metadata array as a 2-D tensor of 1024-byte rows (256 x u32), boxes of `box_rows` rows
+bool make_map_rows1k(CUtensorMap* m, const void* base, uint64_t bytes, uint32_t box_rows) {
+  EncodeTiledFn fn = encode_fn();
+  if (!fn || bytes % 1024 != 0) return false;
+  cuuint64_t dims[2] = {256, bytes / 1024};
+  cuuint64_t strides[1] = {1024};
+  cuuint32_t box[2] = {256, box_rows};
+  cuuint32_t estr[2] = {1, 1};
+  return fn(m, CU_TENSOR_MAP_DATA_TYPE_UINT32, 2, const_cast<void*>(base), dims, strides, box, estr,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
 template <int BN, int FMT>
 sharq_status launch_tiles(const LinearArgs& a, const GroupInfo& g, int64_t rows_total, int64_t m_blocks, int E,
                           int num_sms, cudaStream_t st) {
@@ -672,8 +678,17 @@ sharq_status launch_tiles(const LinearArgs& a, const GroupInfo& g, int64_t rows_
   const bool pair_worth = ((m_blocks + 1) / 2) * (a.D / 256) >= num_sms / 4 || (force_pair && force_pair[0] == '1');
   if (E == 0 && m_blocks >= 2 && a.D % 256 == 0 && BN == 128 && pair_worth && !(no_pair && no_pair[0] == '1')) {
     using P = PairStage<FMT>;
-    CUtensorMap tm_wp;
-    if (!make_map(&tm_wp, a.w_codes, (uint64_t)w_rows, (uint64_t)a.K / 2, 128, 128)) return SHARQ_ECUDA;
+    CUtensorMap tm_wp, tm_sfa_sp, tm_sfa_dn, tm_meta, tm_sfb_sp, tm_sfb_dn;
+    const uint64_t act_rows = (uint64_t)m_blocks * 128, kk = (uint64_t)a.K;
+    const uint32_t dn_rows = P::SF_DN_BYTES / 1024;
+    const uint64_t dn_div = (FMT == SHARQ_NVFP4) ? 16 : 32;
+    if (!make_map(&tm_wp, a.w_codes, (uint64_t)w_rows, kk / 2, 128, 128) ||
+        !make_map_rows1k(&tm_sfa_sp, a.sp_sf, act_rows * kk / 32, 1) ||
+        !make_map_rows1k(&tm_sfa_dn, a.dn_sf, act_rows * kk / dn_div, dn_rows) ||
+        !make_map_rows1k(&tm_meta, a.sp_meta, act_rows * kk / 16, 2) ||
+        !make_map_rows1k(&tm_sfb_sp, a.w_sf_sp, (uint64_t)a.D * kk / 32, 1) ||
+        !make_map_rows1k(&tm_sfb_dn, a.w_sf_dn, (uint64_t)a.D * kk / dn_div, dn_rows))
+      return SHARQ_ECUDA;
     auto kfn = sharq_linear_pair_kernel<FMT>;
     if (cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, P::SMEM) != cudaSuccess)
       return SHARQ_ECUDA;
@@ -691,7 +706,7 @@ sharq_status launch_tiles(const LinearArgs& a, const GroupInfo& g, int64_t rows_
     at[0].val.clusterDim.z = 1;
     lp.attrs = at;
     lp.numAttrs = 1;
-    return cudaLaunchKernelEx(&lp, kfn, tm_sp, tm_dn, tm_wp, p) == cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
+    return cudaLaunchKernelEx(&lp, kfn, tm_sp, tm_dn, tm_wp, tm_sfa_sp, tm_sfa_dn, tm_meta, tm_sfb_sp, tm_sfb_dn, p) == cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
   }
   const int splits = choose_splits(tiles, (int)(a.K / BK), num_sms);
   cudaLaunchConfig_t lc{};
