@@ -54,6 +54,9 @@ struct KParams {
   int64_t ldy;
   int32_t T, D, K, out_fp32, path;
   int32_t m_blocks, total_tiles;
+  int32_t a_rows;     // rows of the activation TMA boxes: 128, or roundup(T, 8) when T < 128 (out-of-bounds
+                      // rows are zero-filled slowly; rows beyond the box keep stale smem, which only feeds
+                      // accumulator rows that are never stored)
 };
 
 // ---- shared-memory stage layout -------------------------------------------------------------
@@ -185,8 +188,8 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
       const uint64_t pol_w = SPLIT ? tc::policy_evict_first() : tc::policy_evict_normal();
       const int64_t Kc = p.K;
       uint32_t tx = BN * 128;
-      if (do_sp) tx += BM * 64 + 2048 + 1024 + S::NB * 1024;
-      if (do_dn) tx += BM * 128 + S::SF_DN_BYTES + S::NB * S::SF_DN_BYTES;
+      if (do_sp) tx += p.a_rows * 64 + 2048 + 1024 + S::NB * 1024;
+      if (do_dn) tx += p.a_rows * 128 + S::SF_DN_BYTES + S::NB * S::SF_DN_BYTES;
       uint32_t it = 0;                                   // k-blocks issued so far (ring position)
       for (int tile = tile0; tile < p.total_tiles; tile += tile_step) {
         const Unit u = decode_unit(p, g, tile, rank, splits);
@@ -665,14 +668,15 @@ sharq_status launch_tiles(const LinearArgs& a, const GroupInfo& g, int64_t rows_
                           int num_sms, cudaStream_t st) {
   CUtensorMap tm_sp, tm_dn, tm_w;
   const int64_t w_rows = (int64_t)(E > 0 ? E : 1) * a.D;
-  if (!make_map(&tm_sp, a.sp_codes, (uint64_t)rows_total, (uint64_t)a.K / 4, 64, BM) ||
-      !make_map(&tm_dn, a.dn_codes, (uint64_t)rows_total, (uint64_t)a.K / 2, 128, BM) ||
+  const uint32_t a_rows = (m_blocks == 1 && rows_total < BM) ? (uint32_t)((rows_total + 7) / 8 * 8) : BM;
+  if (!make_map(&tm_sp, a.sp_codes, (uint64_t)rows_total, (uint64_t)a.K / 4, 64, a_rows) ||
+      !make_map(&tm_dn, a.dn_codes, (uint64_t)rows_total, (uint64_t)a.K / 2, 128, a_rows) ||
       !make_map(&tm_w, a.w_codes, (uint64_t)w_rows, (uint64_t)a.K / 2, 128, BN < 256 ? BN : 256))
     return SHARQ_ECUDA;
   const int64_t tiles = m_blocks * (a.D / BN);
   KParams p{(const uint8_t*)a.sp_sf, (const uint8_t*)a.sp_meta, (const uint8_t*)a.dn_sf, (const uint8_t*)a.w_sf_sp,
             (const uint8_t*)a.w_sf_dn, a.row_scale, a.w_ts, (const uint16_t*)a.bias, a.Y, a.ldy,
-            (int32_t)a.T, (int32_t)a.D, (int32_t)a.K, a.out_dtype, a.path, (int32_t)m_blocks, (int32_t)tiles};
+            (int32_t)a.T, (int32_t)a.D, (int32_t)a.K, a.out_dtype, a.path, (int32_t)m_blocks, (int32_t)tiles, (int32_t)a_rows};
   const char* no_pair = getenv("SHARQ_DEBUG_NO_PAIR");
   const char* force_pair = getenv("SHARQ_DEBUG_FORCE_PAIR");
   const bool pair_worth = ((m_blocks + 1) / 2) * (a.D / 256) >= num_sms / 4 || (force_pair && force_pair[0] == '1');
