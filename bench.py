@@ -243,6 +243,10 @@ def run_ours(args):
 
     pk = peaks()
     n_sets = 3                                            # 3 x 116 MB of weights: > 126 MB L2 between re-reads
+    if args.extras_only:
+        wl = Workload(sq, rank, [], n_sets)
+        print(json.dumps({"extras_only": True, "extras": prefill_extras(sq, wl, pk, args.steps)}))
+        return
     wl = Workload(sq, rank, DECODE_T, n_sets)
     steps, warmup = args.steps, max(args.warmup, 3)
 
@@ -465,6 +469,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--headline-only", action="store_true",
                     help="time only the whole-step region (short run for ncu launch lists / captures)")
+    ap.add_argument("--extras-only", action="store_true",
+                    help="only the prefill (T=4096) linear and T=8192 prepare measurements (short run for ncu)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

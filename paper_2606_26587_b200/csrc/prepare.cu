@@ -11,6 +11,7 @@
 // Numerics follow DESIGN.md R1-R8 exactly (the oracle in oracle/ restates them in numpy); every
 // rounding is an explicit *_rn intrinsic so no FMA contraction can change a bit.
 #include <cuda_fp16.h>
+#include <stdlib.h>
 
 #include "common.cuh"
 
@@ -503,6 +504,177 @@ __global__ void __launch_bounds__(512) sharq_prepare_kernel(const PrepParams p) 
   cp_async_wait<0>();
 }
 
+// ---- row-per-CTA kernel (NVFP4 / MXFP4, K <= 32768) ---------------------------------------------------
+// Warp w of the CTA owns the 1024-element block w of the row and every lane keeps its 32 contiguous
+// elements in registers from the first load to the last store: no shared-memory staging of the row, so
+// occupancy is set by registers only and a single row (decode, T = 1) is spread over K/1024 warps.  The
+// row statistics keep DESIGN.md R1's order: every lane publishes its four 8-chunk leaves, warp 0 adds
+// them in ascending (block, chunk) order per lane slot and runs the butterfly; the result is broadcast.
+constexpr int kRowMaxWarps = 32;
+
+struct RowShared {
+  float leaf[kRowMaxWarps][4][32];
+  uint32_t amax[kRowMaxWarps];
+  float stat;
+};
+
+__device__ __forceinline__ float row_reduce_ordered(RowShared& sh, const float (&leaf)[4], int warp, int lane,
+                                                    int nwarps) {
+#pragma unroll
+  for (int j = 0; j < 4; ++j) sh.leaf[warp][j][lane] = leaf[j];
+  __syncthreads();
+  if (warp == 0) {
+    float acc = 0.0f;
+    for (int b = 0; b < nwarps; ++b) {
+#pragma unroll
+      for (int j = 0; j < 4; ++j) acc = __fadd_rn(acc, sh.leaf[b][j][lane]);
+    }
+    acc = warp_sum_butterfly(acc);
+    if (lane == 0) sh.stat = acc;
+  }
+  __syncthreads();
+  const float r = sh.stat;
+  __syncthreads();            // sh.leaf / sh.stat may be rewritten by the next reduction
+  return r;
+}
+
+template <int FMT, int NORM, int MAXT, int MINB>
+__global__ void __launch_bounds__(MAXT, MINB) sharq_prepare_row_kernel(const PrepParams p) {
+  __shared__ RowShared sh;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
+  const int64_t K = p.K;
+  const uint32_t k0 = (uint32_t)warp * 1024u + (uint32_t)lane * 32u;
+  const bool act = (int64_t)k0 < K;
+  const float Kf = (float)K;
+  const float static_ts = (FMT == SHARQ_NVFP4 && p.x_ts != nullptr) ? *p.x_ts : 0.0f;
+  const bool need_rowmax = (FMT == SHARQ_NVFP4) && (p.x_ts == nullptr);
+
+  // gamma / beta of this lane's 32 columns stay in registers across rows
+  uint32_t G[16], Bt[16];
+  if (NORM != SHARQ_NORM_NONE && act) {
+    const uint4* g4 = reinterpret_cast<const uint4*>(p.gamma + k0);
+#pragma unroll
+    for (int s = 0; s < 4; ++s) {
+      const uint4 g = __ldg(g4 + s);
+      G[4 * s] = g.x; G[4 * s + 1] = g.y; G[4 * s + 2] = g.z; G[4 * s + 3] = g.w;
+    }
+    if (NORM == SHARQ_NORM_LAYER && p.beta) {
+      const uint4* b4 = reinterpret_cast<const uint4*>(p.beta + k0);
+#pragma unroll
+      for (int s = 0; s < 4; ++s) {
+        const uint4 g = __ldg(b4 + s);
+        Bt[4 * s] = g.x; Bt[4 * s + 1] = g.y; Bt[4 * s + 2] = g.z; Bt[4 * s + 3] = g.w;
+      }
+    }
+  }
+
+  for (int64_t row = blockIdx.x; row < p.T; row += gridDim.x) {
+    uint32_t X[16];
+    if (act) {
+      const uint4* src = reinterpret_cast<const uint4*>(p.x + row * p.ldx + k0);
+#pragma unroll
+      for (int s = 0; s < 4; ++s) {
+        const uint4 v = __ldcs(src + s);
+        X[4 * s] = v.x; X[4 * s + 1] = v.y; X[4 * s + 2] = v.z; X[4 * s + 3] = v.w;
+      }
+    } else {
+#pragma unroll
+      for (int i = 0; i < 16; ++i) X[i] = 0u;
+    }
+
+    // ---- O1 statistics in the canonical order (R1) and normalisation (R3)
+    if (NORM != SHARQ_NORM_NONE) {
+      float mu = 0.0f, leaf[4];
+      if (NORM == SHARQ_NORM_LAYER) {
+#pragma unroll
+        for (int c = 0; c < 4; ++c) leaf[c] = act ? leaf8<false>(&X[4 * c]) : 0.0f;
+        mu = __fdiv_rn(row_reduce_ordered(sh, leaf, warp, lane, nwarps), Kf);
+      }
+#pragma unroll
+      for (int c = 0; c < 4; ++c) {
+        float l = 0.0f;
+        if (act) {
+          if (NORM == SHARQ_NORM_RMS) {
+            l = leaf8<true>(&X[4 * c]);
+          } else {
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+              const float cl = __fsub_rn(bf16lo_to_f32(X[4 * c + i]), mu), ch = __fsub_rn(bf16hi_to_f32(X[4 * c + i]), mu);
+              l = __fadd_rn(l, __fmul_rn(cl, cl));
+              l = __fadd_rn(l, __fmul_rn(ch, ch));
+            }
+          }
+        }
+        leaf[c] = l;
+      }
+      const float S = row_reduce_ordered(sh, leaf, warp, lane, nwarps);
+      const float rstd = __frcp_rn(__fsqrt_rn(__fadd_rn(__fdiv_rn(S, Kf), p.eps)));
+      if (act) {
+#pragma unroll
+        for (int i = 0; i < 16; ++i) {
+          float lo = bf16lo_to_f32(X[i]), hi = bf16hi_to_f32(X[i]);
+          if (NORM == SHARQ_NORM_LAYER) { lo = __fsub_rn(lo, mu); hi = __fsub_rn(hi, mu); }
+          const uint32_t h = pack_bf16x2_rn(__fmul_rn(lo, rstd), __fmul_rn(hi, rstd));
+          uint32_t v = mul_bf16x2_rn(h, G[i]);
+          if (NORM == SHARQ_NORM_LAYER && p.beta) v = add_bf16x2_rn(v, Bt[i]);
+          X[i] = v;
+        }
+      }
+    }
+
+    // ---- O2 per-row tensor scale
+    float ts = 1.0f, inv_ts = 1.0f;
+    if (need_rowmax) {
+      uint32_t amax = 0;
+#pragma unroll
+      for (int i = 0; i < 16; ++i) {
+        const uint32_t a = X[i] & 0x7FFF7FFFu;
+        amax = max(amax, max(a & 0xFFFFu, a >> 16));
+      }
+      amax = warp_max_u32(amax);
+      if (lane == 0) sh.amax[warp] = amax;
+      __syncthreads();
+      amax = warp_max_u32(lane < nwarps ? sh.amax[lane] : 0u);
+      __syncthreads();
+      ts = (amax == 0u) ? 1.0f : __fdiv_rn(__uint_as_float(amax << 16), 2688.0f);
+    }
+    if (FMT == SHARQ_NVFP4) {
+      if (p.x_ts != nullptr) ts = static_ts;
+      inv_ts = __frcp_rn(ts);
+    }
+    if (threadIdx.x == 0) p.row_scale[row] = ts;
+
+    // ---- O3-O7 mask, backbone, residual, stores
+    if (act) quantize_block_e2m1<FMT>(p, row, k0, X, ts, inv_ts);
+  }
+}
+
+template <int FMT>
+static cudaError_t launch_row_kernel(int norm, const PrepParams& p, int num_sms, cudaStream_t st) {
+  const int warps = (int)((p.K + 1023) / 1024);
+  const dim3 block((unsigned)warps * 32);
+  int per_sm = 2048 / (warps * 32);                       // thread limit; registers trim it further at launch
+  if (per_sm < 1) per_sm = 1;
+  if (per_sm > 8) per_sm = 8;
+  int64_t ctas = (int64_t)num_sms * per_sm;
+  if (ctas > p.T) ctas = p.T;
+  const dim3 grid((unsigned)ctas);
+#define SHARQ_ROW(N, MAXT, MINB) sharq_prepare_row_kernel<FMT, N, MAXT, MINB><<<grid, block, 0, st>>>(p)
+#define SHARQ_ROW_N(MAXT, MINB)                                              \
+  {                                                                          \
+    if (norm == SHARQ_NORM_NONE) SHARQ_ROW(SHARQ_NORM_NONE, MAXT, MINB);     \
+    else if (norm == SHARQ_NORM_RMS) SHARQ_ROW(SHARQ_NORM_RMS, MAXT, MINB);  \
+    else SHARQ_ROW(SHARQ_NORM_LAYER, MAXT, MINB);                            \
+  }
+  if (warps <= 4) SHARQ_ROW_N(128, 5)            // <= 102 registers, 20 warps / SM
+  else if (warps <= 8) SHARQ_ROW_N(256, 3)       // <= 85 registers
+  else if (warps <= 16) SHARQ_ROW_N(512, 1)      // <= 128 registers
+  else SHARQ_ROW_N(1024, 1)                      // <= 64 registers
+#undef SHARQ_ROW_N
+#undef SHARQ_ROW
+  return cudaGetLastError();
+}
+
 template <int FMT>
 static cudaError_t launch_norm(int norm, const PrepParams& p, dim3 grid, dim3 block, size_t smem, cudaStream_t st) {
 #define SHARQ_LAUNCH(N)                                                                                        \
@@ -531,6 +703,11 @@ cudaError_t launch_prepare(const sharq_config* cfg, const void* x, int64_t T, in
   p.dn_codes = (uint8_t*)dn_codes; p.dn_sf = (uint8_t*)dn_sf; p.row_scale = row_scale;
   p.eps = cfg->eps; p.tiled = (cfg->layout == SHARQ_LAYOUT_TILED);
   p.row_bytes = (uint32_t)(K * 2);
+  if (cfg->fmt != SHARQ_HIF4 && K <= 1024 * kRowMaxWarps && !getenv("SHARQ_DEBUG_OLD_PREPARE")) {
+    p.nbuf = 0;
+    return cfg->fmt == SHARQ_NVFP4 ? launch_row_kernel<SHARQ_NVFP4>(cfg->norm, p, num_sms, st)
+                                   : launch_row_kernel<SHARQ_MXFP4>(cfg->norm, p, num_sms, st);
+  }
   // warps per CTA: as many double-buffered rows as fit in ~200 KB, else single-buffered
   const size_t budget = 200 * 1024;
   int nbuf = 2;
