@@ -179,6 +179,7 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
   tc::tc_fence_after();
   uint32_t tmem_base;
   asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_ptr_smem));
+  tc::grid_launch_dependents();                          // the next kernel may start its own prologue
 
   if (warp == 0) {
     // =========================== TMA producer ===============================================
@@ -191,6 +192,7 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
       if (do_sp) tx += p.a_rows * 64 + 2048 + 1024 + S::NB * 1024;
       if (do_dn) tx += p.a_rows * 128 + S::SF_DN_BYTES + S::NB * S::SF_DN_BYTES;
       uint32_t it = 0;                                   // k-blocks issued so far (ring position)
+      bool dep_synced = false;
       for (int tile = tile0; tile < p.total_tiles; tile += tile_step) {
         const Unit u = decode_unit(p, g, tile, rank, splits);
         const int w_row0 = u.expert * p.D + u.n_blk * BN;
@@ -198,32 +200,58 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
         const uint8_t* sfa_sp = p.sp_sf + (size_t)u.m_blk * (Kc / 128) * 512;
         const uint8_t* sfa_dn = p.dn_sf + (size_t)u.m_blk * (Kc / 256) * (S::SF_DN_BYTES);
         const uint8_t* meta = p.sp_meta + (size_t)u.m_blk * (Kc / 256) * 2048;
-        for (int kb = u.kb0; kb < u.kb1; ++kb, ++it) {
+        // weight side of k-block kb (codes + both scale views): independent of the preceding kernel
+        auto load_w = [&](int kb, uint32_t st, uint32_t fb) {
+          if (lead) tc::tma_load_2d(st + S::W, &tm_w, fb, kb * 128, w_row0, pol_w);
+          for (int nb = 0; nb < S::NB; ++nb) {
+            if (do_sp && lead)
+              tc::bulk_load(st + S::SFB_SP + nb * 1024,
+                            p.w_sf_sp + ((size_t)(wblk0 + nb) * (Kc / 128) + (size_t)kb * 2) * 512, 1024, fb, pol_w);
+            if (do_dn && lead)
+              tc::bulk_load(st + S::SFB_DN + nb * S::SF_DN_BYTES,
+                            p.w_sf_dn + ((size_t)(wblk0 + nb) * (Kc / 256) + (size_t)kb) * S::SF_DN_BYTES,
+                            S::SF_DN_BYTES, fb, pol_w);
+          }
+        };
+        // activation side: written by sharq_prepare, only after griddepcontrol.wait
+        auto load_a = [&](int kb, uint32_t st, uint32_t fb) {
+          if (do_sp) {
+            if (lead) tc::tma_load_2d(st + S::A_SP, &tm_a_sp, fb, kb * 64, u.m_blk * BM, pol_act);
+            if (lead) tc::bulk_load(st + S::META, meta + (size_t)kb * 2048, 2048, fb, pol_act);
+            if (lead) tc::bulk_load(st + S::SFA_SP, sfa_sp + (size_t)kb * 1024, 1024, fb, pol_act);
+          }
+          if (do_dn) {
+            if (lead) tc::tma_load_2d(st + S::A_DN, &tm_a_dn, fb, kb * 128, u.m_blk * BM, pol_act);
+            if (lead) tc::bulk_load(st + S::SFA_DN, sfa_dn + (size_t)kb * S::SF_DN_BYTES, S::SF_DN_BYTES, fb, pol_act);
+          }
+        };
+        int kb = u.kb0;
+        if (!dep_synced) {
+          // programmatic dependent launch: stream the first STAGES weight k-blocks while the kernel that
+          // produces the activations (sharq_prepare) is still finishing, then wait for it
+          const int n_early = min(S::STAGES, u.kb1 - u.kb0);
+          for (int i = 0; i < n_early; ++i) {
+            if (lead) tc::mbar_expect_tx(full_bar(i), tx);
+            load_w(kb + i, smem_base + i * S::BYTES, full_bar(i));
+          }
+          tc::grid_dependency_wait();
+          dep_synced = true;
+          for (int i = 0; i < n_early; ++i) load_a(kb + i, smem_base + i * S::BYTES, full_bar(i));
+          kb += n_early;
+          it += n_early;
+        }
+        for (; kb < u.kb1; ++kb, ++it) {
           const int s = it % S::STAGES;
           const uint32_t ph = (it / S::STAGES) & 1;
           tc::mbar_wait(empty_bar(s), ph ^ 1);
           const uint32_t st = smem_base + s * S::BYTES;
           const uint32_t fb = full_bar(s);
           if (lead) tc::mbar_expect_tx(fb, tx);
-          if (lead) tc::tma_load_2d(st + S::W, &tm_w, fb, kb * 128, w_row0, pol_w);
-          if (do_sp) {
-            if (lead) tc::tma_load_2d(st + S::A_SP, &tm_a_sp, fb, kb * 64, u.m_blk * BM, pol_act);
-            if (lead) tc::bulk_load(st + S::META, meta + (size_t)kb * 2048, 2048, fb, pol_act);
-            if (lead) tc::bulk_load(st + S::SFA_SP, sfa_sp + (size_t)kb * 1024, 1024, fb, pol_act);
-            for (int nb = 0; nb < S::NB; ++nb)
-              if (lead) tc::bulk_load(st + S::SFB_SP + nb * 1024,
-                            p.w_sf_sp + ((size_t)(wblk0 + nb) * (Kc / 128) + (size_t)kb * 2) * 512, 1024, fb, pol_w);
-          }
-          if (do_dn) {
-            if (lead) tc::tma_load_2d(st + S::A_DN, &tm_a_dn, fb, kb * 128, u.m_blk * BM, pol_act);
-            if (lead) tc::bulk_load(st + S::SFA_DN, sfa_dn + (size_t)kb * S::SF_DN_BYTES, S::SF_DN_BYTES, fb, pol_act);
-            for (int nb = 0; nb < S::NB; ++nb)
-              if (lead) tc::bulk_load(st + S::SFB_DN + nb * S::SF_DN_BYTES,
-                            p.w_sf_dn + ((size_t)(wblk0 + nb) * (Kc / 256) + (size_t)kb) * S::SF_DN_BYTES,
-                            S::SF_DN_BYTES, fb, pol_w);
-          }
+          load_w(kb, st, fb);
+          load_a(kb, st, fb);
         }
       }
+      if (!dep_synced) tc::grid_dependency_wait();
     }
   } else if (warp == 1) {
     // =========================== MMA issuer =================================================
@@ -293,6 +321,7 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
     }
   } else {
     // =========================== epilogue ====================================================
+    tc::grid_dependency_wait();                          // row_scale is sharq_prepare's; Y may still be read
     const int sub = warp & 3;                            // TMEM sub-partition this warp may read
     const int r_local = sub * 32 + lane;
     const uint32_t lane_addr = tmem_base + ((uint32_t)(sub * 32) << 16);
@@ -459,6 +488,8 @@ sharq_linear_pair_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __gr
   tc::tc_fence_after();
   uint32_t tmem_base;
   asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_ptr_smem));
+  tc::grid_launch_dependents();
+  tc::grid_dependency_wait();
 
   if (warp == 0) {
     // =========================== TMA producer (both CTAs) ===================================
@@ -699,7 +730,9 @@ sharq_status launch_tiles(const LinearArgs& a, const GroupInfo& g, int64_t rows_
     const int64_t pair_tiles = ((m_blocks + 1) / 2) * (a.D / 256);
     const int64_t clusters = pair_tiles < num_sms / 2 ? pair_tiles : num_sms / 2;
     cudaLaunchConfig_t lp{};
-    cudaLaunchAttribute at[1];
+    cudaLaunchAttribute at[2];
+    at[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[1].val.programmaticStreamSerializationAllowed = 1;
     lp.blockDim = dim3(kThreads);
     lp.gridDim = dim3((unsigned)(2 * clusters));
     lp.dynamicSmemBytes = P::SMEM;
@@ -709,12 +742,16 @@ sharq_status launch_tiles(const LinearArgs& a, const GroupInfo& g, int64_t rows_
     at[0].val.clusterDim.y = 1;
     at[0].val.clusterDim.z = 1;
     lp.attrs = at;
-    lp.numAttrs = 1;
+    lp.numAttrs = 2;
     return cudaLaunchKernelEx(&lp, kfn, tm_sp, tm_dn, tm_wp, tm_sfa_sp, tm_sfa_dn, tm_meta, tm_sfb_sp, tm_sfb_dn, p) == cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
   }
   const int splits = choose_splits(tiles, (int)(a.K / BK), num_sms);
   cudaLaunchConfig_t lc{};
-  cudaLaunchAttribute attr[1];
+  cudaLaunchAttribute attr[2];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  lc.attrs = attr;
+  lc.numAttrs = 1;
   lc.blockDim = dim3(kThreads);
   lc.stream = st;
   if (splits > 1) {
@@ -724,12 +761,11 @@ sharq_status launch_tiles(const LinearArgs& a, const GroupInfo& g, int64_t rows_
       return SHARQ_ECUDA;
     lc.gridDim = dim3((unsigned)(tiles * splits));
     lc.dynamicSmemBytes = S::SMEM;
-    attr[0].id = cudaLaunchAttributeClusterDimension;
-    attr[0].val.clusterDim.x = (unsigned)splits;
-    attr[0].val.clusterDim.y = 1;
-    attr[0].val.clusterDim.z = 1;
-    lc.attrs = attr;
-    lc.numAttrs = 1;
+    attr[1].id = cudaLaunchAttributeClusterDimension;
+    attr[1].val.clusterDim.x = (unsigned)splits;
+    attr[1].val.clusterDim.y = 1;
+    attr[1].val.clusterDim.z = 1;
+    lc.numAttrs = 2;
     return cudaLaunchKernelEx(&lc, kfn, tm_sp, tm_dn, tm_w, p, g) == cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
   }
   using S = Stage<BN, FMT, false>;

@@ -512,36 +512,45 @@ __global__ void __launch_bounds__(512) sharq_prepare_kernel(const PrepParams p) 
 // them in ascending (block, chunk) order per lane slot and runs the butterfly; the result is broadcast.
 constexpr int kRowMaxWarps = 32;
 
+// dynamic shared memory: leaf[nwarps][4][32] floats, then amax[32] words, then one float
 struct RowShared {
-  float leaf[kRowMaxWarps][4][32];
-  uint32_t amax[kRowMaxWarps];
-  float stat;
+  float* leaf;
+  uint32_t* amax;
+  float* stat;
 };
 
 __device__ __forceinline__ float row_reduce_ordered(RowShared& sh, const float (&leaf)[4], int warp, int lane,
                                                     int nwarps) {
 #pragma unroll
-  for (int j = 0; j < 4; ++j) sh.leaf[warp][j][lane] = leaf[j];
+  for (int j = 0; j < 4; ++j) sh.leaf[(warp * 4 + j) * 32 + lane] = leaf[j];
   __syncthreads();
   if (warp == 0) {
     float acc = 0.0f;
     for (int b = 0; b < nwarps; ++b) {
 #pragma unroll
-      for (int j = 0; j < 4; ++j) acc = __fadd_rn(acc, sh.leaf[b][j][lane]);
+      for (int j = 0; j < 4; ++j) acc = __fadd_rn(acc, sh.leaf[(b * 4 + j) * 32 + lane]);
     }
     acc = warp_sum_butterfly(acc);
-    if (lane == 0) sh.stat = acc;
+    if (lane == 0) *sh.stat = acc;
   }
   __syncthreads();
-  const float r = sh.stat;
+  const float r = *sh.stat;
   __syncthreads();            // sh.leaf / sh.stat may be rewritten by the next reduction
   return r;
 }
 
 template <int FMT, int NORM, int MAXT, int MINB>
 __global__ void __launch_bounds__(MAXT, MINB) sharq_prepare_row_kernel(const PrepParams p) {
-  __shared__ RowShared sh;
+  extern __shared__ __align__(16) uint8_t row_smem[];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
+  RowShared sh;
+  sh.leaf = reinterpret_cast<float*>(row_smem);
+  sh.amax = reinterpret_cast<uint32_t*>(row_smem + (size_t)nwarps * 512);
+  sh.stat = reinterpret_cast<float*>(row_smem + (size_t)nwarps * 512 + 128);
+  // programmatic dependent launch: let the GEMM that follows start streaming its weights now; our own
+  // inputs (and the operand buffers we overwrite) belong to the kernels before us
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  asm volatile("griddepcontrol.wait;" ::: "memory");
   const int64_t K = p.K;
   const uint32_t k0 = (uint32_t)warp * 1024u + (uint32_t)lane * 32u;
   const bool act = (int64_t)k0 < K;
@@ -659,7 +668,14 @@ static cudaError_t launch_row_kernel(int norm, const PrepParams& p, int num_sms,
   int64_t ctas = (int64_t)num_sms * per_sm;
   if (ctas > p.T) ctas = p.T;
   const dim3 grid((unsigned)ctas);
-#define SHARQ_ROW(N, MAXT, MINB) sharq_prepare_row_kernel<FMT, N, MAXT, MINB><<<grid, block, 0, st>>>(p)
+  cudaLaunchConfig_t lc{};
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  lc.gridDim = grid; lc.blockDim = block; lc.stream = st; lc.attrs = attr; lc.numAttrs = 1;
+  lc.dynamicSmemBytes = (size_t)warps * 512 + 128 + 16;
+  cudaError_t err = cudaSuccess;
+#define SHARQ_ROW(N, MAXT, MINB) err = cudaLaunchKernelEx(&lc, sharq_prepare_row_kernel<FMT, N, MAXT, MINB>, p)
 #define SHARQ_ROW_N(MAXT, MINB)                                              \
   {                                                                          \
     if (norm == SHARQ_NORM_NONE) SHARQ_ROW(SHARQ_NORM_NONE, MAXT, MINB);     \
@@ -672,7 +688,7 @@ static cudaError_t launch_row_kernel(int norm, const PrepParams& p, int num_sms,
   else SHARQ_ROW_N(1024, 1)                      // <= 64 registers
 #undef SHARQ_ROW_N
 #undef SHARQ_ROW
-  return cudaGetLastError();
+  return err;
 }
 
 template <int FMT>

@@ -42,6 +42,12 @@ __device__ __forceinline__ uint32_t elect_one() {
   return pred;
 }
 
+// ---- programmatic dependent launch -------------------------------------------------------------
+// wait: all memory of the kernels this one depends on is visible afterwards (no-op without the
+// launch attribute).  launch_dependents: the next kernel in the stream may start launching.
+__device__ __forceinline__ void grid_dependency_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void grid_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
 // ---- TMA ------------------------------------------------------------------------------------
 __device__ __forceinline__ void prefetch_tmap(const void* tmap) {
   asm volatile("prefetch.tensormap [%0];" ::"l"(tmap) : "memory");
