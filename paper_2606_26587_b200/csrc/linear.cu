@@ -670,13 +670,31 @@ bool make_map(CUtensorMap* m, const void* base, uint64_t rows, uint64_t row_byte
 }
 
 // Number of K-splits (cluster size) for a launch with `tiles` output tiles: only when the tiles alone
-// leave most SMs idle, and only sizes whose slice exchange fits the receive buffer (2, 3, 4, 8).
+// leave most SMs idle, only sizes whose slice exchange fits the receive buffer (2, 3, 4, 8), and only if
+// all `tiles` clusters are co-resident in ONE wave (cluster placement is per GPC, so tiles * S <= SMs is
+// not enough: cudaOccupancyMaxActiveClusters decides).
+template <int BN, int FMT>
 int choose_splits(int64_t tiles, int num_kb, int num_sms) {
   if (tiles * 2 > num_sms) return 1;
+  using S = Stage<BN, FMT, true>;
+  static int max_clusters[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};      // per cluster size, queried once
   const int cand[4] = {8, 4, 3, 2};
   for (int c : cand) {
-    if (c == 8 && tiles * 8 > 128) continue;             // 8-CTA clusters: two per GPC at most
-    if (tiles * c <= num_sms && num_kb >= 2 * c) return c;
+    if (tiles * c > num_sms || num_kb < 2 * c) continue;
+    if (max_clusters[c] == 0) {
+      cudaLaunchConfig_t lc{};
+      cudaLaunchAttribute at[1];
+      at[0].id = cudaLaunchAttributeClusterDimension;
+      at[0].val.clusterDim.x = (unsigned)c; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+      lc.gridDim = dim3((unsigned)(c * num_sms)); lc.blockDim = dim3(kThreads); lc.dynamicSmemBytes = S::SMEM;
+      lc.attrs = at; lc.numAttrs = 1;
+      int n = 0;
+      auto kfn = sharq_linear_kernel<BN, FMT, true>;
+      cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, S::SMEM);
+      if (cudaOccupancyMaxActiveClusters(&n, kfn, &lc) != cudaSuccess || n <= 0) n = -1;
+      max_clusters[c] = n;
+    }
+    if (max_clusters[c] >= tiles) return c;
   }
   return 1;
 }
@@ -745,7 +763,7 @@ sharq_status launch_tiles(const LinearArgs& a, const GroupInfo& g, int64_t rows_
     lp.numAttrs = 2;
     return cudaLaunchKernelEx(&lp, kfn, tm_sp, tm_dn, tm_wp, tm_sfa_sp, tm_sfa_dn, tm_meta, tm_sfb_sp, tm_sfb_dn, p) == cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
   }
-  const int splits = choose_splits(tiles, (int)(a.K / BK), num_sms);
+  const int splits = choose_splits<BN, FMT>(tiles, (int)(a.K / BK), num_sms);
   cudaLaunchConfig_t lc{};
   cudaLaunchAttribute attr[2];
   attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
