@@ -519,23 +519,26 @@ struct RowShared {
   float* stat;
 };
 
+// `slot` alternates between consecutive reductions so that the values of one reduction are never
+// overwritten before every warp has read them: two barriers per reduction, none after the read.
 __device__ __forceinline__ float row_reduce_ordered(RowShared& sh, const float (&leaf)[4], int warp, int lane,
-                                                    int nwarps) {
+                                                    int nwarps, uint32_t& slot) {
+  float* buf = sh.leaf + (size_t)slot * nwarps * 128;
 #pragma unroll
-  for (int j = 0; j < 4; ++j) sh.leaf[(warp * 4 + j) * 32 + lane] = leaf[j];
+  for (int j = 0; j < 4; ++j) buf[(warp * 4 + j) * 32 + lane] = leaf[j];
   __syncthreads();
   if (warp == 0) {
     float acc = 0.0f;
     for (int b = 0; b < nwarps; ++b) {
 #pragma unroll
-      for (int j = 0; j < 4; ++j) acc = __fadd_rn(acc, sh.leaf[(b * 4 + j) * 32 + lane]);
+      for (int j = 0; j < 4; ++j) acc = __fadd_rn(acc, buf[(b * 4 + j) * 32 + lane]);
     }
     acc = warp_sum_butterfly(acc);
-    if (lane == 0) *sh.stat = acc;
+    if (lane == 0) sh.stat[slot] = acc;
   }
   __syncthreads();
-  const float r = *sh.stat;
-  __syncthreads();            // sh.leaf / sh.stat may be rewritten by the next reduction
+  const float r = sh.stat[slot];
+  slot ^= 1u;
   return r;
 }
 
@@ -544,9 +547,10 @@ __global__ void __launch_bounds__(MAXT, MINB) sharq_prepare_row_kernel(const Pre
   extern __shared__ __align__(16) uint8_t row_smem[];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
   RowShared sh;
-  sh.leaf = reinterpret_cast<float*>(row_smem);
-  sh.amax = reinterpret_cast<uint32_t*>(row_smem + (size_t)nwarps * 512);
-  sh.stat = reinterpret_cast<float*>(row_smem + (size_t)nwarps * 512 + 128);
+  sh.leaf = reinterpret_cast<float*>(row_smem);                                   // [2][nwarps][4][32]
+  sh.amax = reinterpret_cast<uint32_t*>(row_smem + (size_t)nwarps * 1024);        // [2][32]
+  sh.stat = reinterpret_cast<float*>(row_smem + (size_t)nwarps * 1024 + 256);     // [2]
+  uint32_t red_slot = 0, amax_slot = 0;
   // programmatic dependent launch: let the GEMM that follows start streaming its weights now; our own
   // inputs (and the operand buffers we overwrite) belong to the kernels before us
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
@@ -579,6 +583,8 @@ __global__ void __launch_bounds__(MAXT, MINB) sharq_prepare_row_kernel(const Pre
 
   for (int64_t row = blockIdx.x; row < p.T; row += gridDim.x) {
     uint32_t X[16];
+    if (act && (lane & 1) == 0 && row + gridDim.x < p.T)      // next row of this CTA: 128-byte line -> L2
+      asm volatile("prefetch.global.L2 [%0];" ::"l"(p.x + (row + gridDim.x) * p.ldx + k0));
     if (act) {
       const uint4* src = reinterpret_cast<const uint4*>(p.x + row * p.ldx + k0);
 #pragma unroll
@@ -597,7 +603,7 @@ __global__ void __launch_bounds__(MAXT, MINB) sharq_prepare_row_kernel(const Pre
       if (NORM == SHARQ_NORM_LAYER) {
 #pragma unroll
         for (int c = 0; c < 4; ++c) leaf[c] = act ? leaf8<false>(&X[4 * c]) : 0.0f;
-        mu = __fdiv_rn(row_reduce_ordered(sh, leaf, warp, lane, nwarps), Kf);
+        mu = __fdiv_rn(row_reduce_ordered(sh, leaf, warp, lane, nwarps, red_slot), Kf);
       }
 #pragma unroll
       for (int c = 0; c < 4; ++c) {
@@ -616,7 +622,7 @@ __global__ void __launch_bounds__(MAXT, MINB) sharq_prepare_row_kernel(const Pre
         }
         leaf[c] = l;
       }
-      const float S = row_reduce_ordered(sh, leaf, warp, lane, nwarps);
+      const float S = row_reduce_ordered(sh, leaf, warp, lane, nwarps, red_slot);
       const float rstd = __frcp_rn(__fsqrt_rn(__fadd_rn(__fdiv_rn(S, Kf), p.eps)));
       if (act) {
 #pragma unroll
@@ -641,10 +647,10 @@ __global__ void __launch_bounds__(MAXT, MINB) sharq_prepare_row_kernel(const Pre
         amax = max(amax, max(a & 0xFFFFu, a >> 16));
       }
       amax = warp_max_u32(amax);
-      if (lane == 0) sh.amax[warp] = amax;
+      if (lane == 0) sh.amax[amax_slot * 32 + warp] = amax;
       __syncthreads();
-      amax = warp_max_u32(lane < nwarps ? sh.amax[lane] : 0u);
-      __syncthreads();
+      amax = warp_max_u32(lane < nwarps ? sh.amax[amax_slot * 32 + lane] : 0u);
+      amax_slot ^= 1u;                           // the next row writes the other half: no second barrier
       ts = (amax == 0u) ? 1.0f : __fdiv_rn(__uint_as_float(amax << 16), 2688.0f);
     }
     if (FMT == SHARQ_NVFP4) {
@@ -673,7 +679,7 @@ static cudaError_t launch_row_kernel(int norm, const PrepParams& p, int num_sms,
   attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
   attr[0].val.programmaticStreamSerializationAllowed = 1;
   lc.gridDim = grid; lc.blockDim = block; lc.stream = st; lc.attrs = attr; lc.numAttrs = 1;
-  lc.dynamicSmemBytes = (size_t)warps * 512 + 128 + 16;
+  lc.dynamicSmemBytes = (size_t)warps * 1024 + 256 + 16;
   cudaError_t err = cudaSuccess;
 #define SHARQ_ROW(N, MAXT, MINB) err = cudaLaunchKernelEx(&lc, sharq_prepare_row_kernel<FMT, N, MAXT, MINB>, p)
 #define SHARQ_ROW_N(MAXT, MINB)                                              \
