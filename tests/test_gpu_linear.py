@@ -129,3 +129,71 @@ def test_linear_grouped_moe(sq):
         p, q = so.prepare(xs[e], norm=0), so.quantize_weight(ws[e])
         got = Y[pad_off[e]: pad_off[e] + counts[e]]
         assert rel_err(got, so.linear(p, q)).max() <= TOL, f"expert {e}"
+
+
+def test_prefill_full_size_sampled(sq):
+    """BASELINE.json configs[2] size, in the launch configuration bench.py times (CTA-pair 256x256 kernel,
+    persistent over all SMs): T = 4096, K = 4096, D = 6144.  The oracle computes a seeded sample of rows
+    (each row of prepare and linear is independent) and output features one by one."""
+    T, K, D = 4096, 4096, 6144
+    x, g, w = si.activations(T, K, config=3, outlier_mult=200.0), si.gamma(K, 3), si.weight(D, K, 3, extra=7)
+    cfg = sq.make_config(sq.NVFP4, sq.NORM_RMS, 1e-6, sq.LAYOUT_TILED)
+    wq = sq.quantize_weight(cfg, to_dev(w))
+    act = sq.prepare(cfg, to_dev(x), to_dev(g))
+    y32 = sq.linear(cfg, act, wq, out_dtype="fp32")
+    y16 = sq.linear(cfg, act, wq, out_dtype="bf16")
+    torch.cuda.synchronize()
+    rng = np.random.Generator(np.random.Philox(si.seed_for(3, 99)))
+    rows = np.sort(rng.choice(T, size=40, replace=False))
+    rows[:4] = [0, 127, 128, T - 1]                       # tile corners
+    rows = np.unique(rows)
+    cols = np.unique(np.concatenate([rng.choice(D, size=250, replace=False), [0, 127, 128, 255, 256, D - 1]]))
+    p = so.prepare(x[rows], gamma_u16=g)
+    q = so.quantize_weight(w)
+    # prepare outputs of the sampled rows, bit for bit (codes are row-major in both layouts)
+    assert np.array_equal(act["sp_codes"].cpu().numpy().reshape(T, K // 4)[rows], p["sp_codes"])
+    assert np.array_equal(act["dn_codes"].cpu().numpy().reshape(T, K // 2)[rows], p["dn_codes"])
+    y64 = so.linear(p, q, cols=cols)
+    got = y32.cpu().numpy()[np.ix_(rows, cols)]
+    den = np.maximum(np.abs(y64), 1e-2 * np.sqrt((y64 ** 2).mean()))
+    err = np.abs(got - y64) / den
+    assert err.max() <= TOL, err.max()
+    assert torch.equal(y16, y32.to(torch.bfloat16))
+
+
+def test_moe_config5_size_sampled(sq):
+    """BASELINE.json configs[4]: Qwen3-30B-A3B-shaped experts (gate+up 2048 -> 1536), 128 experts, seeded
+    top-8 routing of 4096 tokens (0 .. ~600 rows per expert); three experts checked against the oracle."""
+    E, K, D = 128, 2048, 1536
+    ids, offsets, order = si.moe_routing()
+    counts = np.diff(offsets)
+    assert counts.sum() == 4096 * 8 and counts.min() >= 0
+    cfg = sq.make_config(sq.NVFP4, sq.NORM_NONE, 1e-6, sq.LAYOUT_TILED)
+    pad_off = np.concatenate([[0], np.cumsum(-(-counts // 128) * 128)])
+    act = sq.alloc_act(cfg, int(pad_off[-1]), K, "cuda")
+    tokens = si.activations(4096, K, config=5)
+    routed_token = (order // 8).astype(np.int64)            # token of every routed row, grouped by expert
+    check = [int(np.argmax(counts)), int(np.argmin(counts)), 77]
+    ws = {}
+    wq_parts = []
+    for e in range(E):
+        w = si.weight(D, K, 5, extra=e) if e in check else si.weight(D, K, 5, extra=e % 3 + 1000)
+        if e in check:
+            ws[e] = w
+        wq_parts.append(sq.quantize_weight(cfg, to_dev(w)))
+        if counts[e]:
+            xe = tokens[routed_token[offsets[e]: offsets[e + 1]]]
+            sq.prepare(cfg, to_dev(xe), out=sq.act_slot(cfg, act, int(pad_off[e]), int(counts[e])))
+    wq = dict(codes=torch.cat([q["codes"] for q in wq_parts]), sf_sp=torch.cat([q["sf_sp"] for q in wq_parts]),
+              sf_dn=torch.cat([q["sf_dn"] for q in wq_parts]), ts_w=torch.cat([q["ts_w"] for q in wq_parts]), D=D, K=K)
+    Y = sq.linear_grouped(cfg, offsets, act, wq, D, out_dtype="fp32")
+    torch.cuda.synchronize()
+    Y = Y.cpu().numpy()
+    for e in check:
+        if counts[e] == 0:
+            continue
+        xe = tokens[routed_token[offsets[e]: offsets[e + 1]]]
+        y64 = so.linear(so.prepare(xe, norm=0), so.quantize_weight(ws[e]))
+        got = Y[pad_off[e]: pad_off[e] + counts[e]]
+        den = np.maximum(np.abs(y64), 1e-2 * np.sqrt((y64 ** 2).mean()))
+        assert (np.abs(got - y64) / den).max() <= TOL, f"expert {e}"
