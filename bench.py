@@ -248,7 +248,10 @@ def run_ours(args):
     n_sets = 3                                            # 3 x 116 MB of weights: > 126 MB L2 between re-reads
     if args.extras_only:
         wl = Workload(sq, rank, [], n_sets)
-        print(json.dumps({"extras_only": True, "extras": prefill_extras(sq, wl, pk, args.steps)}))
+        ex = prefill_extras(sq, wl, pk, args.steps)
+        if not args.short_extras:
+            ex.update(config_extras(sq, wl, pk, args.steps))
+        print(json.dumps({"extras_only": True, "extras": ex}))
         return
     wl = Workload(sq, rank, DECODE_T, n_sets)
     steps, warmup = args.steps, max(args.warmup, 3)
@@ -308,6 +311,8 @@ def run_ours(args):
             layers[f"{n}_T{T}"] = dict(us=round(ms * 1e3, 2), tflops=round(layer_flops(T, K, D) / ms / 1e9, 1))
 
     extras = prefill_extras(sq, wl, pk, steps) if rank == 0 else {}
+    if rank == 0:
+        extras.update(config_extras(sq, wl, pk, steps))
 
     # ---- e2e: activations start in pinned host memory, Y read back, plain stream launches --------
     xh = {k: v.cpu().pin_memory() for k, v in wl.x.items()}
@@ -383,6 +388,80 @@ def prefill_extras(sq, wl, pk, steps):
         out["prepare"][f"T{Tp}_K{K}_{'rms' if norm else 'none'}"] = dict(
             us=round(ms * 1e3, 1), GBps=round(gbs, 1), frac_of_hbm=round(gbs / pk["hbm"], 4))
         del xs, acts
+    return out
+
+
+QWEN = [("qkv", 3584, 4608, 1), ("o", 3584, 3584, 0), ("gate_up", 3584, 37888, 1), ("down", 18944, 3584, 0)]
+
+
+def config_extras(sq, wl, pk, steps):
+    """BASELINE.json configs[2] (T sweep), configs[3] (Qwen2.5-7B shapes x formats) and configs[4] (MoE
+    grouped): sharq_linear alone and sharq_prepare alone, CUDA events, rotating weights where they exist."""
+    import torch
+    p_dn, p_sp = 4 * pk["bf16_sustained"] * 1e12, 8 * pk["bf16_sustained"] * 1e12
+    out = {"config3_T_sweep": {}, "config4_qwen_formats": {}, "config5_moe": {}}
+
+    def lin_entry(ms, T, K, D, fmt=0):
+        fl = layer_flops(T, K, D)
+        return dict(us=round(ms * 1e3, 1), effective_tflops=round(fl / ms / 1e9, 1),
+                    frac_of_fp4_roofline=round((fl / p_dn + fl / p_sp) / (ms * 1e-3), 4),
+                    GBps=round(linear_bytes(T, K, D, fmt) / ms / 1e6, 1))
+
+    for T in (2048, 8192):                       # T = 4096 is in linear_T4096
+        for i, (n, K, D, norm) in enumerate(LLAMA):
+            x = device_activations(T, K, BASE_SEED + 300 + i, outlier_mult=(10.0, 50.0, 200.0)[i % 3])
+            act = sq.prepare(wl.cfg[n], x, wl.gamma[K] if norm else None)
+            Y = torch.empty((T, D), dtype=torch.bfloat16, device="cuda")
+            reps = [lambda r=r: sq.linear(wl.cfg[n], act, wl.wq[r][n], Y=Y) for r in range(wl.n_sets)]
+            out["config3_T_sweep"][f"{n}_T{T}"] = lin_entry(timed(reps, max(steps // 2, 8), 3, lambda: None), T, K, D)
+            del x, act, Y
+    T = 4096
+    for fmt, fname in ((sq.NVFP4, "nvfp4"), (sq.MXFP4, "mxfp4")):
+        for i, (n, K, D, norm) in enumerate(QWEN):
+            cfg = sq.make_config(fmt, sq.NORM_RMS if norm else sq.NORM_NONE, 1e-6, sq.LAYOUT_TILED)
+            wqs = [sq.quantize_weight(cfg, device_weight(D, K, BASE_SEED + 400 + 10 * r + i)) for r in range(2)]
+            x = device_activations(T, K, BASE_SEED + 450 + i)
+            g = device_gamma(K, BASE_SEED + 460)
+            act = sq.alloc_act(cfg, T, K, "cuda")
+            Y = torch.empty((T, D), dtype=torch.bfloat16, device="cuda")
+            ms_p = timed([lambda: sq.prepare(cfg, x, g if norm else None, out=act)], max(steps // 2, 8), 3, lambda: None)
+            ms_l = timed([lambda r=r: sq.linear(cfg, act, wqs[r], Y=Y) for r in range(2)], max(steps // 2, 8), 3, lambda: None)
+            e = lin_entry(ms_l, T, K, D, fmt)
+            e["prepare_us"] = round(ms_p * 1e3, 1)
+            e["prepare_GBps"] = round(prepare_bytes(T, K, fmt) / ms_p / 1e6, 1)
+            out["config4_qwen_formats"][f"{fname}_{n}"] = e
+            del wqs, x, act, Y
+    # configs[4]: 4096 tokens, 128 experts, top-8 of a seeded softmax router; rows grouped by expert into
+    # 128-row-aligned slots; gate+up 2048 -> 1536 and down 768 -> 2048 as ONE grouped launch each
+    E = 128
+    gen = torch.Generator(device="cuda").manual_seed(BASE_SEED + 500)
+    logits = torch.randn((4096, E), generator=gen, device="cuda")
+    top = torch.topk(torch.softmax(logits, dim=1), 8, dim=1).indices.reshape(-1)
+    counts = torch.bincount(top, minlength=E).cpu().numpy()
+    offsets = np.concatenate([[0], np.cumsum(counts)]).astype(np.int32)
+    padded = int((-(-counts // 128) * 128).sum())
+    for n, K, D in (("gate_up", 2048, 1536), ("down", 768, 2048)):
+        cfg = sq.make_config(sq.NVFP4, sq.NORM_NONE, 1e-6, sq.LAYOUT_TILED)
+        parts = [sq.quantize_weight(cfg, device_weight(D, K, BASE_SEED + 510 + e % 8)) for e in range(E)]
+        wq = dict(codes=torch.cat([q["codes"] for q in parts]), sf_sp=torch.cat([q["sf_sp"] for q in parts]),
+                  sf_dn=torch.cat([q["sf_dn"] for q in parts]), ts_w=torch.cat([q["ts_w"] for q in parts]), D=D, K=K)
+        del parts
+        x = device_activations(padded, K, BASE_SEED + 520)          # every slot row filled: prepare is per row
+        act = sq.alloc_act(cfg, padded, K, "cuda")
+        Y = torch.empty((padded, D), dtype=torch.bfloat16, device="cuda")
+        ms_p = timed([lambda: sq.prepare(cfg, x, out=act)], max(steps // 2, 8), 3, lambda: None)
+        ms_l = timed([lambda: sq.linear_grouped(cfg, offsets, act, wq, D, Y=Y)], max(steps // 2, 8), 3, lambda: None)
+        rows = int(counts.sum())
+        w_bytes = E * K * D * (0.5 + 1 / 32)
+        by = w_bytes + rows * K * 0.90625 + 2.0 * rows * D
+        out["config5_moe"][n] = dict(us=round(ms_l * 1e3, 1), rows=rows, padded_rows=padded,
+                                     effective_tflops=round(2.0 * rows * K * D / ms_l / 1e9, 1),
+                                     GBps=round(by / ms_l / 1e6, 1), frac_of_hbm=round(by / ms_l / 1e6 / pk["hbm"], 4),
+                                     prepare_us=round(ms_p * 1e3, 1),
+                                     prepare_GBps=round(prepare_bytes(padded, K) / ms_p / 1e6, 1),
+                                     note="weights (all experts) are L2-resident across repeats: 201 / 101 MB")
+        del wq, x, act, Y
+    out["config5_moe"]["rows_per_expert"] = dict(min=int(counts.min()), max=int(counts.max()))
     return out
 
 
@@ -475,6 +554,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--headline-only", action="store_true",
                     help="time only the whole-step region (short run for ncu launch lists / captures)")
+    ap.add_argument("--short-extras", action="store_true", help="with --extras-only: skip configs 3-5")
     ap.add_argument("--extras-only", action="store_true",
                     help="only the prefill (T=4096) linear and T=8192 prepare measurements (short run for ncu)")
     args = ap.parse_args()

@@ -99,7 +99,12 @@ __device__ __forceinline__ Unit decode_unit(const KParams& p, const GroupInfo& g
   u.n_blk = tile / p.m_blocks;
   u.expert = 0;
   if (g.E > 0) {
-    while (u.expert + 1 < g.E && g.blk_prefix[u.expert + 1] <= u.m_blk) ++u.expert;
+    int lo = 0, hi = g.E - 1;                      // last expert whose first block is <= m_blk (binary search)
+    while (lo < hi) {
+      const int mid = (lo + hi + 1) >> 1;
+      if (g.blk_prefix[mid] <= u.m_blk) lo = mid; else hi = mid - 1;
+    }
+    u.expert = lo;
     u.rows_valid = min(BM, g.count[u.expert] - (u.m_blk - g.blk_prefix[u.expert]) * BM);
   } else {
     u.rows_valid = min(BM, p.T - u.m_blk * BM);
