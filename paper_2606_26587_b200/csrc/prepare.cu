@@ -150,19 +150,22 @@ __device__ __forceinline__ void quantize_block_e2m1(const PrepParams& p, int64_t
 #pragma unroll
   for (int c = 0; c < 4; ++c) {
     uint32_t bytes = 0;  // byte q = the two codes of pair q
+    const uint32_t keep = (1u << i0[c]) | (1u << i1[c]);
 #pragma unroll
     for (int q = 0; q < 4; ++q) {
       const float xl = bf16lo_to_f32(X[4 * c + q]), xh = bf16hi_to_f32(X[4 * c + q]);
       const uint32_t b = cvt_e2m1x2(__fmul_rn(xl, bs.inv), __fmul_rn(xh, bs.inv));
       bytes |= b << (8 * q);
-      // ---- O5 dequantise and residual; dropped pairs subtract +0 (x - +0 == x bit for bit)
+      // ---- O5 dequantise and residual; a dropped pair keeps R = X bit for bit
       float dl, dh;
       e2m1x2_to_f32(b, dl, dh);
-      const bool kept = (q == (int)i0[c]) || (q == (int)i1[c]);
-      dl = kept ? __fmul_rn(dl, bs.s_eff) : 0.0f;
-      dh = kept ? __fmul_rn(dh, bs.s_eff) : 0.0f;
-      R[8 * c + 2 * q] = __fsub_rn(xl, dl);
-      R[8 * c + 2 * q + 1] = __fsub_rn(xh, dh);
+      float rl = xl, rh = xh;
+      if (keep & (1u << q)) {
+        rl = __fsub_rn(xl, __fmul_rn(dl, bs.s_eff));
+        rh = __fsub_rn(xh, __fmul_rn(dh, bs.s_eff));
+      }
+      R[8 * c + 2 * q] = rl;
+      R[8 * c + 2 * q + 1] = rh;
     }
     // compress: survivors in ascending k, byte 2c = pair i0, byte 2c+1 = pair i1
     const uint32_t two = __byte_perm(bytes, 0u, i0[c] | (i1[c] << 4) | 0x4400u);
