@@ -803,11 +803,18 @@ sharq_status launch_tiles(const LinearArgs& a, const GroupInfo& g, int64_t rows_
 
 }  // namespace
 
-size_t linear_workspace_bytes(const sharq_config*, int64_t, int64_t, int64_t, int32_t) { return 0; }
+size_t hif4_linear_workspace_bytes(int64_t T, int64_t D, int64_t K);
+sharq_status launch_linear_hif4(const LinearArgs& a, void* workspace, size_t workspace_bytes, int num_sms,
+                                cudaStream_t st);
+
+size_t linear_workspace_bytes(const sharq_config* cfg, int64_t T, int64_t D, int64_t K, int32_t) {
+  return cfg->fmt == SHARQ_HIF4 ? hif4_linear_workspace_bytes(T, D, K) : 0;   // bf16 copies of A and W
+}
 
 sharq_status launch_linear(const sharq_config* cfg, const LinearArgs& a, int32_t E, const int32_t* offsets_host,
-                           void* /*workspace*/, size_t /*workspace_bytes*/, int num_sms, cudaStream_t st) {
-  if (cfg->fmt == SHARQ_HIF4) return SHARQ_EINVAL;        // HiF4 has no FP4-rate tensor path
+                           void* workspace, size_t workspace_bytes, int num_sms, cudaStream_t st) {
+  if (cfg->fmt == SHARQ_HIF4)                             // no FP4-rate tensor path: exact bf16 emulation
+    return E > 0 ? SHARQ_EINVAL : launch_linear_hif4(a, workspace, workspace_bytes, num_sms, st);
   if (a.K > (int64_t)1 << 24 || a.D > (int64_t)1 << 24) return SHARQ_ESHAPE;
   GroupInfo g{};
   int64_t rows_total = a.T, m_blocks = (a.T + BM - 1) / BM;

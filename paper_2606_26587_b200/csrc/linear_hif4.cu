@@ -1,0 +1,325 @@
+// sharq_linear for HiF4.
+//
+// B200's tcgen05 has no S1P2 element / E6M2 scale format, so HiF4 has no FP4-rate tensor path.  Every
+// HiF4 value E6M2 * 2^(E1_8 + E1_16) * S1P2 = (4 + m) * k * 2^(E - 52 + shift) with (4 + m) * k <= 49
+// has at most 6 significant bits, i.e. it is EXACT in bf16.  The path is therefore:
+//   1. hif4_dequant_*  : codes + 32-bit unit metadata -> bf16 (exact), activations as [T, 2K] =
+//                        [backbone with zeros at dropped positions | residual], weights as [D, K];
+//   2. hif4_gemm_kernel: dense bf16 tcgen05.mma (kind::f16, fp32 accumulate) over the 2K-long rows, the
+//                        W tile reused for both halves (k and k + K read the same weight columns):
+//                        Y = A_sp W^T + A_dn W^T in one accumulator.
+// Roofline denominator: the measured bf16 tensor peak.  The 2:4 sparse bf16 MMA for the backbone half
+// (which would save a quarter of the MMA time) is not used yet: the zeros are multiplied densely.
+#include <cuda.h>
+#include <cuda_runtime.h>
+
+#include "common.cuh"
+#include "tc_ptx.cuh"
+
+namespace sharq {
+
+struct LinearArgs {
+  int64_t T, D, K;
+  const void *sp_codes, *sp_sf, *sp_meta, *dn_codes, *dn_sf;
+  const float* row_scale;
+  const void *w_codes, *w_sf_sp, *w_sf_dn;
+  const float* w_ts;
+  const void* bias;
+  void* Y; int64_t ldy; int out_dtype; int path;
+};
+
+namespace {
+
+// bf16 bits of one decoded HiF4 element (Eq. 15): code = S1P2 nibble, word = E6M2 | E1_8<<8 | E1_16<<16,
+// i = position inside the 64-element unit.
+__device__ __forceinline__ uint32_t hif4_to_bf16(uint32_t code, uint32_t word, uint32_t i) {
+  const uint32_t k = code & 7u;
+  const uint32_t n = (4u + (word & 3u)) * k;                               // <= 49: exact
+  const int shift = (int)((word >> (8 + (i >> 3))) & 1u) + (int)((word >> (16 + (i >> 2))) & 1u);
+  const int p = (int)((word >> 2) & 63u) - 52 + shift;                     // value = n * 2^p
+  const float v = __fmul_rn((float)n, __uint_as_float((uint32_t)(p + 127) << 23));
+  return (__float_as_uint(v) >> 16) | ((code & 8u) << 12);                 // exact in bf16; sign of the code
+}
+
+// activations: one thread per 8 logical k (two 2:4 groups)
+__global__ void hif4_dequant_act_kernel(const uint8_t* __restrict__ sp_codes, const uint32_t* __restrict__ sp_sf,
+                                        const uint8_t* __restrict__ sp_meta, const uint8_t* __restrict__ dn_codes,
+                                        const uint32_t* __restrict__ dn_sf, uint16_t* __restrict__ A, int64_t T,
+                                        int64_t K, int path) {
+  tc::grid_dependency_wait();
+  const int64_t n8 = K >> 3;
+  for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < T * n8;
+       idx += (int64_t)gridDim.x * blockDim.x) {
+    const int64_t t = idx / n8, c = idx % n8;          // k = 8c .. 8c+7
+    const uint32_t unit_i = (uint32_t)((8 * c) & 63);
+    uint32_t sp[8], dn[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) sp[i] = 0u, dn[i] = 0u;
+    if (path != 2) {
+      const uint32_t word = sp_sf[t * (K >> 6) + (c >> 3)];
+      const uint32_t meta = sp_meta[t * (K >> 3) + c];                 // two nibbles: groups 2c, 2c+1
+      const uint32_t codes = *reinterpret_cast<const uint16_t*>(sp_codes + t * (K >> 2) + 2 * c);
+#pragma unroll
+      for (int g = 0; g < 2; ++g) {
+        const uint32_t nib = (meta >> (4 * g)) & 15u, i0 = nib & 3u, i1 = nib >> 2;
+        const uint32_t byte = (codes >> (8 * g)) & 255u;
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+          uint32_t v = 0u;
+          if ((uint32_t)e == i0) v = hif4_to_bf16(byte & 15u, word, unit_i + 4 * g + e);
+          if ((uint32_t)e == i1) v = hif4_to_bf16(byte >> 4, word, unit_i + 4 * g + e);
+          sp[4 * g + e] = v;
+        }
+      }
+    }
+    if (path != 1) {
+      const uint32_t word = dn_sf[t * (K >> 6) + (c >> 3)];
+      const uint32_t codes = *reinterpret_cast<const uint32_t*>(dn_codes + t * (K >> 1) + 4 * c);
+#pragma unroll
+      for (int e = 0; e < 8; ++e) dn[e] = hif4_to_bf16((codes >> (4 * e)) & 15u, word, unit_i + e);
+    }
+    uint16_t* row = A + t * (2 * K);
+    *reinterpret_cast<uint4*>(row + 8 * c) =
+        make_uint4(sp[0] | sp[1] << 16, sp[2] | sp[3] << 16, sp[4] | sp[5] << 16, sp[6] | sp[7] << 16);
+    *reinterpret_cast<uint4*>(row + K + 8 * c) =
+        make_uint4(dn[0] | dn[1] << 16, dn[2] | dn[3] << 16, dn[4] | dn[5] << 16, dn[6] | dn[7] << 16);
+  }
+}
+
+__global__ void hif4_dequant_weight_kernel(const uint8_t* __restrict__ codes, const uint32_t* __restrict__ sf,
+                                           uint16_t* __restrict__ W, int64_t D, int64_t K) {
+  const int64_t n8 = K >> 3;
+  for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < D * n8;
+       idx += (int64_t)gridDim.x * blockDim.x) {
+    const int64_t d = idx / n8, c = idx % n8;
+    const uint32_t word = sf[d * (K >> 6) + (c >> 3)];
+    const uint32_t cw = *reinterpret_cast<const uint32_t*>(codes + d * (K >> 1) + 4 * c);
+    uint32_t v[8];
+#pragma unroll
+    for (int e = 0; e < 8; ++e) v[e] = hif4_to_bf16((cw >> (4 * e)) & 15u, word, (uint32_t)((8 * c) & 63) + e);
+    *reinterpret_cast<uint4*>(W + d * K + 8 * c) =
+        make_uint4(v[0] | v[1] << 16, v[2] | v[3] << 16, v[4] | v[5] << 16, v[6] | v[7] << 16);
+  }
+}
+
+// ---- dense bf16 GEMM: Y[T, D] = A[T, 2K] * [W | W]^T, 128 x BN tiles, persistent, 2 TMEM accumulators ---
+constexpr int GM = 128, GK = 64, kGemmThreads = 192;
+
+struct GemmParams {
+  const float *row_scale, *w_ts;
+  const uint16_t* bias;
+  void* Y;
+  int64_t ldy;
+  int32_t T, D, K, out_fp32, m_blocks, total_tiles;
+};
+
+__device__ __forceinline__ uint32_t idesc_bf16(uint32_t M, uint32_t N) {
+  return (1u << 4) /*fp32 accumulate*/ | (1u << 7) /*A bf16*/ | (1u << 10) /*B bf16*/ | ((N >> 3) << 17) |
+         ((M >> 4) << 24);
+}
+__device__ __forceinline__ void mma_bf16(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc,
+                                         uint32_t accumulate) {
+  asm volatile("{ .reg .pred p;\n\t"
+               "setp.ne.b32 p, %4, 0;\n\t"
+               "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p; }"
+               ::"r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate) : "memory");
+}
+
+template <int BN>
+__global__ void __launch_bounds__(kGemmThreads, 1)
+hif4_gemm_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant__ CUtensorMap tm_w,
+                 const GemmParams p) {
+  constexpr int A_BYTES = GM * 128, B_BYTES = BN * 128, STAGE = A_BYTES + B_BYTES;
+  constexpr int STAGES = (BN == 256) ? 4 : 6;
+  extern __shared__ uint8_t smem_raw[];
+  const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+  const uint32_t bars = smem_base + STAGES * STAGE;
+  auto full_bar = [&](int s) { return bars + 8u * s; };
+  auto empty_bar = [&](int s) { return bars + 8u * (STAGES + s); };
+  auto tmem_full_bar = [&](int a) { return bars + 8u * (2 * STAGES + a); };
+  auto tmem_empty_bar = [&](int a) { return bars + 8u * (2 * STAGES + 2 + a); };
+  const uint32_t tmem_ptr_smem = bars + 8u * (2 * STAGES + 4);
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int num_kb = 2 * p.K / GK, half_kb = p.K / GK;
+
+  if (warp == 0 && lane == 0) {
+    tc::prefetch_tmap(&tm_a);
+    tc::prefetch_tmap(&tm_w);
+  }
+  if (warp == 1 && lane == 0) {
+    for (int s = 0; s < STAGES; ++s) {
+      tc::mbar_init(full_bar(s), 1);
+      tc::mbar_init(empty_bar(s), 1);
+    }
+    for (int a = 0; a < 2; ++a) {
+      tc::mbar_init(tmem_full_bar(a), 1);
+      tc::mbar_init(tmem_empty_bar(a), 4);
+    }
+    tc::fence_mbar_init();
+  }
+  if (warp == 2) tc::tmem_alloc<512>(tmem_ptr_smem);
+  tc::tc_fence_before();
+  __syncthreads();
+  tc::tc_fence_after();
+  uint32_t tmem_base;
+  asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_ptr_smem));
+  tc::grid_dependency_wait();                            // A / W were dequantised by the kernels before us
+
+  if (warp == 0) {
+    const bool lead = tc::elect_one() != 0;
+    const uint64_t pol = tc::policy_evict_normal();
+    uint32_t it = 0;
+    for (int tile = blockIdx.x; tile < p.total_tiles; tile += gridDim.x) {
+      const int m_blk = tile % p.m_blocks, n_blk = tile / p.m_blocks;
+      for (int kb = 0; kb < num_kb; ++kb, ++it) {
+        const int s = it % STAGES;
+        tc::mbar_wait(empty_bar(s), ((it / STAGES) & 1) ^ 1);
+        const uint32_t st = smem_base + s * STAGE;
+        if (lead) tc::mbar_expect_tx(full_bar(s), STAGE);
+        if (lead) tc::tma_load_2d(st, &tm_a, full_bar(s), kb * GK, m_blk * GM, pol);
+        if (lead) tc::tma_load_2d(st + A_BYTES, &tm_w, full_bar(s), (kb % half_kb) * GK, n_blk * BN, pol);
+      }
+    }
+  } else if (warp == 1) {
+    const bool lead = tc::elect_one() != 0;
+    const uint32_t idesc = idesc_bf16(GM, BN);
+    uint32_t it = 0, n_unit = 0;
+    for (int tile = blockIdx.x; tile < p.total_tiles; tile += gridDim.x, ++n_unit) {
+      const uint32_t as = n_unit & 1u;
+      tc::mbar_wait(tmem_empty_bar(as), ((n_unit >> 1) & 1u) ^ 1u);
+      tc::tc_fence_after();
+      uint32_t accumulate = 0;
+      for (int kb = 0; kb < num_kb; ++kb, ++it) {
+        const int s = it % STAGES;
+        tc::mbar_wait(full_bar(s), (it / STAGES) & 1);
+        tc::tc_fence_after();
+        const uint32_t st = smem_base + s * STAGE;
+#pragma unroll
+        for (int j = 0; j < GK / 16; ++j) {              // UMMA K = 16 bf16 = 32 bytes
+          if (lead) mma_bf16(tmem_base + as * BN, tc::smem_desc(st + 32 * j, 1024, 2),
+                             tc::smem_desc(st + A_BYTES + 32 * j, 1024, 2), idesc, accumulate);
+          accumulate = 1;
+        }
+        if (lead) tc::tc_commit(empty_bar(s));
+      }
+      if (lead) tc::tc_commit(tmem_full_bar(as));
+    }
+  } else {
+    const int sub = warp & 3, r_local = sub * 32 + lane;
+    const uint32_t lane_addr = tmem_base + ((uint32_t)(sub * 32) << 16);
+    uint32_t n_unit = 0;
+    for (int tile = blockIdx.x; tile < p.total_tiles; tile += gridDim.x, ++n_unit) {
+      const int m_blk = tile % p.m_blocks, n_blk = tile / p.m_blocks;
+      const uint32_t as = n_unit & 1u;
+      const int64_t row = (int64_t)m_blk * GM + r_local;
+      const bool row_ok = row < p.T;
+      const float scale = row_ok ? __fmul_rn(p.row_scale[row], p.w_ts[0]) : 0.0f;
+      tc::mbar_wait(tmem_full_bar(as), (n_unit >> 1) & 1u);
+      tc::tc_fence_after();
+#pragma unroll 1
+      for (int c = 0; c < BN / 32; ++c) {
+        uint32_t v[32];
+        tc::tmem_ld32(lane_addr + as * BN + c * 32, v);
+        tc::tmem_ld_wait();
+        if (row_ok) {
+          const int col0 = n_blk * BN + c * 32;
+          float f[32];
+#pragma unroll
+          for (int i = 0; i < 32; ++i) f[i] = __fmul_rn(__uint_as_float(v[i]), scale);
+          if (p.bias) {
+#pragma unroll
+            for (int i = 0; i < 32; ++i) f[i] = __fadd_rn(f[i], __uint_as_float((uint32_t)p.bias[col0 + i] << 16));
+          }
+          if (p.out_fp32) {
+            float4* dst = reinterpret_cast<float4*>(static_cast<float*>(p.Y) + row * p.ldy + col0);
+#pragma unroll
+            for (int i = 0; i < 8; ++i) dst[i] = make_float4(f[4 * i], f[4 * i + 1], f[4 * i + 2], f[4 * i + 3]);
+          } else {
+            uint4* dst = reinterpret_cast<uint4*>(static_cast<uint16_t*>(p.Y) + row * p.ldy + col0);
+#pragma unroll
+            for (int i = 0; i < 4; ++i)
+              dst[i] = make_uint4(pack_bf16x2_rn(f[8 * i], f[8 * i + 1]), pack_bf16x2_rn(f[8 * i + 2], f[8 * i + 3]),
+                                  pack_bf16x2_rn(f[8 * i + 4], f[8 * i + 5]), pack_bf16x2_rn(f[8 * i + 6], f[8 * i + 7]));
+          }
+        }
+      }
+      tc::tc_fence_before();
+      __syncwarp();
+      if (lane == 0) tc::mbar_arrive(tmem_empty_bar(as));
+    }
+  }
+  __syncthreads();
+  if (warp == 2) {
+    tc::tc_fence_after();
+    tc::tmem_dealloc<512>(tmem_base);
+  }
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+bool make_bf16_map(CUtensorMap* m, const void* base, uint64_t rows, uint64_t cols, uint32_t box_rows) {
+  static EncodeTiledFn fn = [] {
+    void* f = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &f, cudaEnableDefault, &q) != cudaSuccess ||
+        q != cudaDriverEntryPointSuccess)
+      f = nullptr;
+    return reinterpret_cast<EncodeTiledFn>(f);
+  }();
+  if (!fn) return false;
+  cuuint64_t dims[2] = {cols, rows};
+  cuuint64_t strides[1] = {cols * 2};
+  cuuint32_t box[2] = {GK, box_rows};
+  cuuint32_t estr[2] = {1, 1};
+  return fn(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(base), dims, strides, box, estr,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+template <int BN>
+sharq_status launch_gemm(const CUtensorMap& tm_a, const CUtensorMap& tm_w, const GemmParams& p, int num_sms,
+                         cudaStream_t st) {
+  constexpr int STAGES = (BN == 256) ? 4 : 6;
+  constexpr int SMEM = STAGES * (GM * 128 + BN * 128) + 1024 + 256;
+  auto kfn = hif4_gemm_kernel<BN>;
+  if (cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM) != cudaSuccess) return SHARQ_ECUDA;
+  const int grid = p.total_tiles < num_sms ? p.total_tiles : num_sms;
+  kfn<<<grid, kGemmThreads, SMEM, st>>>(tm_a, tm_w, p);
+  return cudaGetLastError() == cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
+}
+
+}  // namespace
+
+size_t hif4_linear_workspace_bytes(int64_t T, int64_t D, int64_t K) {
+  const int64_t Tp = round_up(T, 128);
+  return (size_t)Tp * (size_t)(2 * K) * 2 + (size_t)D * (size_t)K * 2 + 256;
+}
+
+sharq_status launch_linear_hif4(const LinearArgs& a, void* workspace, size_t workspace_bytes, int num_sms,
+                                cudaStream_t st) {
+  if (!workspace || workspace_bytes < hif4_linear_workspace_bytes(a.T, a.D, a.K)) return SHARQ_EWORKSPACE;
+  if (a.K > (int64_t)1 << 24 || a.D > (int64_t)1 << 24 || a.T > (int64_t)1 << 30) return SHARQ_ESHAPE;
+  const int64_t Tp = round_up(a.T, 128);
+  uint16_t* A = reinterpret_cast<uint16_t*>((reinterpret_cast<uintptr_t>(workspace) + 127) & ~(uintptr_t)127);
+  uint16_t* W = A + (size_t)Tp * (size_t)(2 * a.K);
+  const int64_t na = a.T * (a.K >> 3), nw = a.D * (a.K >> 3);
+  hif4_dequant_act_kernel<<<(unsigned)((na + 255) / 256 < 8192 ? (na + 255) / 256 : 8192), 256, 0, st>>>(
+      (const uint8_t*)a.sp_codes, (const uint32_t*)a.sp_sf, (const uint8_t*)a.sp_meta, (const uint8_t*)a.dn_codes,
+      (const uint32_t*)a.dn_sf, A, a.T, a.K, a.path);
+  hif4_dequant_weight_kernel<<<(unsigned)((nw + 255) / 256 < 16384 ? (nw + 255) / 256 : 16384), 256, 0, st>>>(
+      (const uint8_t*)a.w_codes, (const uint32_t*)a.w_sf_sp, W, a.D, a.K);
+  if (cudaGetLastError() != cudaSuccess) return SHARQ_ECUDA;
+  CUtensorMap tm_a, tm_w;
+  const bool wide = a.D % 256 == 0;
+  if (!make_bf16_map(&tm_a, A, (uint64_t)Tp, (uint64_t)(2 * a.K), GM) ||
+      !make_bf16_map(&tm_w, W, (uint64_t)a.D, (uint64_t)a.K, wide ? 256 : 128))
+    return SHARQ_ECUDA;
+  const int64_t m_blocks = Tp / 128;
+  GemmParams p{a.row_scale, a.w_ts, (const uint16_t*)a.bias, a.Y, a.ldy, (int32_t)a.T, (int32_t)a.D, (int32_t)a.K,
+               a.out_dtype, (int32_t)m_blocks, (int32_t)(m_blocks * (a.D / (wide ? 256 : 128)))};
+  return wide ? launch_gemm<256>(tm_a, tm_w, p, num_sms, st) : launch_gemm<128>(tm_a, tm_w, p, num_sms, st);
+}
+
+}  // namespace sharq

@@ -41,6 +41,8 @@ CASES = [
     (0, 1, 1, 4096, 6144, 50.0), (0, 0, 8, 14336, 4096, 50.0), (0, 1, 32, 4096, 28672, 50.0),   # configs[1] shapes
     (0, 1, 300, 1024, 384, 200.0), (0, 0, 129, 256, 128, 10.0), (0, 1, 257, 3584, 512, 50.0),
     (1, 1, 16, 4096, 4096, 50.0), (1, 0, 130, 3584, 4608, 200.0), (1, 1, 5, 768, 2048, 10.0),
+    # HiF4: exact bf16 emulation path (128- and 256-wide tiles, ragged T)
+    (2, 1, 16, 4096, 4096, 50.0), (2, 0, 130, 768, 384, 10.0), (2, 1, 300, 3584, 512, 200.0),
 ]
 
 
