@@ -416,7 +416,7 @@ def config_extras(sq, wl, pk, steps):
             out["config3_T_sweep"][f"{n}_T{T}"] = lin_entry(timed(reps, max(steps // 2, 8), 3, lambda: None), T, K, D)
             del x, act, Y
     T = 4096
-    for fmt, fname in ((sq.NVFP4, "nvfp4"), (sq.MXFP4, "mxfp4")):
+    for fmt, fname in ((sq.NVFP4, "nvfp4"), (sq.MXFP4, "mxfp4"), (sq.HIF4, "hif4")):
         for i, (n, K, D, norm) in enumerate(QWEN):
             cfg = sq.make_config(fmt, sq.NORM_RMS if norm else sq.NORM_NONE, 1e-6, sq.LAYOUT_TILED)
             wqs = [sq.quantize_weight(cfg, device_weight(D, K, BASE_SEED + 400 + 10 * r + i)) for r in range(2)]
@@ -425,8 +425,16 @@ def config_extras(sq, wl, pk, steps):
             act = sq.alloc_act(cfg, T, K, "cuda")
             Y = torch.empty((T, D), dtype=torch.bfloat16, device="cuda")
             ms_p = timed([lambda: sq.prepare(cfg, x, g if norm else None, out=act)], max(steps // 2, 8), 3, lambda: None)
-            ms_l = timed([lambda r=r: sq.linear(cfg, act, wqs[r], Y=Y) for r in range(2)], max(steps // 2, 8), 3, lambda: None)
+            ws = sq._bytes(sq.linear_workspace(cfg, T, D, K), "cuda") if fmt == sq.HIF4 else None
+            ms_l = timed([lambda r=r: sq.linear(cfg, act, wqs[r], Y=Y, workspace=ws) for r in range(2)],
+                         max(steps // 2, 8), 3, lambda: None)
             e = lin_entry(ms_l, T, K, D, fmt)
+            if fmt == sq.HIF4:                   # no FP4-rate tensor path for HiF4: bf16 roofline (dense + 2:4 sparse)
+                fl = layer_flops(T, K, D)
+                pb = pk["bf16_sustained"] * 1e12
+                del e["frac_of_fp4_roofline"]
+                e["frac_of_bf16_roofline"] = round((fl / pb + fl / (2 * pb)) / (ms_l * 1e-3), 4)
+                e["note"] = "dequantise (A and W, every call) + dense bf16 GEMM over 2K"
             e["prepare_us"] = round(ms_p * 1e3, 1)
             e["prepare_GBps"] = round(prepare_bytes(T, K, fmt) / ms_p / 1e6, 1)
             out["config4_qwen_formats"][f"{fname}_{n}"] = e

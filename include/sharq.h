@@ -118,7 +118,13 @@ sharq_status sharq_prepare(const sharq_config* cfg, const void* x, int64_t T, in
  * and layout == SHARQ_LAYOUT_TILED (otherwise SHARQ_EINVAL).  Both GEMMs accumulate into the
  * same TMEM tile in one kernel ("accumulates directly into this output").
  * out_dtype: 0 = bf16, 1 = fp32.  bias bf16 [D] or NULL.  ldy in elements.
- * path: 0 = sparse + dense (SharQ), 1 = sparse only, 2 = dense only (Table 5 rows). */
+ * path: 0 = sparse + dense (SharQ), 1 = sparse only, 2 = dense only (Table 5 rows).
+ * HiF4 (layout CANONICAL): tcgen05 has no S1P2 / E6M2 formats, so the operands are dequantised to bf16
+ * (exact: every HiF4 value has <= 6 significant bits) into `workspace` and multiplied by a dense bf16
+ * tensor-core GEMM with fp32 accumulation; workspace >= sharq_linear_workspace(...) bytes is required.
+ * NVFP4 / MXFP4 need no workspace (it may be NULL).  Kernels are launched with programmatic dependent
+ * launch: the weight stream of sharq_linear may start while the preceding kernel of the stream (normally
+ * sharq_prepare) is still draining; all reads of activation operands wait for it to complete. */
 sharq_status sharq_linear(const sharq_config* cfg, int64_t T, int64_t D, int64_t K,
                           const void* sp_codes, const void* sp_sf, const void* sp_meta,
                           const void* dn_codes, const void* dn_sf, const float* row_scale,
