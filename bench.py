@@ -148,7 +148,7 @@ class Workload:
         self.sq, self.Ts, self.n_sets = sq, Ts, n_sets
         self.cfg = {n: sq.make_config(sq.NVFP4, sq.NORM_RMS if norm else sq.NORM_NONE, 1e-6, sq.LAYOUT_TILED)
                     for n, _, _, norm in LLAMA}
-        seed = BASE_SEED * 1000 + 97 * rank
+        seed = rank_seed(rank)
         self.wq = []
         for r in range(n_sets):
             ws = {}
@@ -218,6 +218,21 @@ def timed(replays, steps, warmup, barrier):
     return e0.elapsed_time(e1) / steps          # ms per call
 
 
+def reduce_max_over_ranks(value, dist, device):
+    """A step takes as long as its slowest rank: MAX all-reduce of the per-rank device time."""
+    if dist is None:
+        return value
+    import torch
+    t = torch.tensor([value], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def rank_seed(rank):
+    """Rows are sharded across ranks with replicated weight SHAPES: every rank draws its own batch."""
+    return BASE_SEED * 1000 + 97 * rank
+
+
 def run_ours(args):
     import torch
     import __graft_entry__ as ge
@@ -238,11 +253,7 @@ def run_ours(args):
         torch.cuda.synchronize()
 
     def max_over_ranks(v):
-        if dist is None:
-            return v
-        t = torch.tensor([v], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+        return reduce_max_over_ranks(v, dist, "cuda")
 
     pk = peaks()
     n_sets = 3                                            # 3 x 116 MB of weights: > 126 MB L2 between re-reads
