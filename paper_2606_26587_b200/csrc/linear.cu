@@ -63,23 +63,31 @@ struct KParams {
 // SPLIT = the split-K variant for T <= 256 (few output tiles): a thread-block cluster of `splits` CTAs
 // shares one output tile, each CTA runs a slice of K, the partial accumulators are exchanged through
 // distributed shared memory (16-column slices, owner = slice % splits) and summed in rank order.
-template <int BN, int FMT, bool SPLIT>
+// AR = rows reserved for the activation tiles (16 / 64 / 128): for T < 128 only roundup(T, 8) rows are loaded,
+// and a smaller reservation leaves room for more ring stages, i.e. more weight bytes in flight per SM (the
+// decode shapes are bound by exactly that).  The MMA still reads 128 rows; rows beyond the loaded ones are
+// whatever follows in shared memory and only reach accumulator rows that are never stored.
+template <int BN, int FMT, bool SPLIT, int AR>
 struct Stage {
   static constexpr int NB = (BN + 127) / 128;                         // 128-row scale atoms of W per tile
   static constexpr int SF_DN_BYTES = (FMT == SHARQ_NVFP4) ? 2048 : 1024;  // per 128 rows per k-block
+  static constexpr int A_DN_BYTES = AR * 128 < 1024 ? 1024 : AR * 128;
+  static constexpr int A_SP_BYTES = AR * 64 < 1024 ? 1024 : AR * 64;
   static constexpr int A_DN = 0;
-  static constexpr int W = A_DN + BM * 128;
+  static constexpr int W = A_DN + A_DN_BYTES;
   static constexpr int A_SP = W + BN * 128;
-  static constexpr int META = A_SP + BM * 64;
+  static constexpr int META = A_SP + A_SP_BYTES;
   static constexpr int SFA_SP = META + 2048;
   static constexpr int SFA_DN = SFA_SP + 1024;
   static constexpr int SFB_SP = SFA_DN + SF_DN_BYTES;
   static constexpr int SFB_DN = SFB_SP + NB * 1024;
   static constexpr int RAW = SFB_DN + NB * SF_DN_BYTES;
   static constexpr int BYTES = (RAW + 1023) / 1024 * 1024;
-  static constexpr int STAGES = SPLIT ? 3 : 4;
-  static constexpr int RECV = SPLIT ? 9 * 8192 : 0;                   // [src][slot][128 rows][16 fp32]
-  static constexpr int SMEM = STAGES * BYTES + RECV + 1024 /*alignment slack*/ + 256 /*barriers*/;
+  static constexpr int RECV = SPLIT ? 9 * AR * 64 : 0;                // [src][slot][AR rows][16 fp32]
+  static constexpr int PAD = AR < 128 ? 128 * 128 : 0;               // the MMA's over-read behind the last stage
+  static constexpr int FIT = (232448 - 1024 - 256 - RECV - PAD) / BYTES;
+  static constexpr int STAGES = FIT > 8 ? 8 : FIT;
+  static constexpr int SMEM = STAGES * BYTES + PAD + RECV + 1024 /*alignment slack*/ + 256 /*barriers*/;
   // tensor-memory columns: two accumulator stages, then metadata and scale factors
   static constexpr int SFB_COLS = NB * 4;          // columns one MMA's B scales occupy
   static constexpr int ACC_STAGES = 2;
@@ -138,15 +146,15 @@ __device__ __forceinline__ void store_row(const KParams& p, int64_t row, int col
   }
 }
 
-template <int BN, int FMT, bool SPLIT>
+template <int BN, int FMT, bool SPLIT, int AR>
 __global__ void __launch_bounds__(kThreads, 1)
 sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_constant__ CUtensorMap tm_a_dn,
                     const __grid_constant__ CUtensorMap tm_w, const KParams p, const __grid_constant__ GroupInfo g) {
-  using S = Stage<BN, FMT, SPLIT>;
+  using S = Stage<BN, FMT, SPLIT, AR>;
   constexpr bool NV = (FMT == SHARQ_NVFP4);
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
-  const uint32_t recv_base = smem_base + S::STAGES * S::BYTES;
+  const uint32_t recv_base = smem_base + S::STAGES * S::BYTES + S::PAD;
   const uint32_t bars = recv_base + S::RECV;      // full[STAGES], empty[STAGES], tmem_full[2], tmem_empty[2], ptr
   auto full_bar = [&](int s) { return bars + 8u * s; };
   auto empty_bar = [&](int s) { return bars + 8u * (S::STAGES + s); };
@@ -369,7 +377,7 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
         tc::tmem_ld16(lane_addr + j * 16, v);
         tc::tmem_ld_wait();
         if (row_ok) {
-          const uint32_t local = recv_base + (uint32_t)(((rank * slots + j / splits) * BM + r_local) * 64);
+          const uint32_t local = recv_base + (uint32_t)(((rank * slots + j / splits) * AR + r_local) * 64);
           const uint32_t remote = tc::map_to_cta(local, (uint32_t)(j % splits));
 #pragma unroll
           for (int i = 0; i < 4; ++i)
@@ -397,7 +405,7 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
 #pragma unroll
           for (int i = 0; i < 16; ++i) f[i] = 0.0f;
           for (int src = 0; src < splits; ++src) {       // fixed order: deterministic sum
-            const uint32_t a = recv_base + (uint32_t)(((src * slots + slot) * BM + r_local) * 64);
+            const uint32_t a = recv_base + (uint32_t)(((src * slots + slot) * AR + r_local) * 64);
 #pragma unroll
             for (int i = 0; i < 4; ++i) {
               const float4 t = tc::ld_shared_v4(a + 16 * i);
@@ -678,10 +686,10 @@ bool make_map(CUtensorMap* m, const void* base, uint64_t rows, uint64_t row_byte
 // leave most SMs idle, only sizes whose slice exchange fits the receive buffer (2, 3, 4, 8), and only if
 // all `tiles` clusters are co-resident in ONE wave (cluster placement is per GPC, so tiles * S <= SMs is
 // not enough: cudaOccupancyMaxActiveClusters decides).
-template <int BN, int FMT>
+template <int BN, int FMT, int AR>
 int choose_splits(int64_t tiles, int num_kb, int num_sms) {
   if (tiles * 2 > num_sms) return 1;
-  using S = Stage<BN, FMT, true>;
+  using S = Stage<BN, FMT, true, AR>;
   static int max_clusters[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};      // per cluster size, queried once
   const int cand[4] = {8, 4, 3, 2};
   for (int c : cand) {
@@ -694,7 +702,7 @@ int choose_splits(int64_t tiles, int num_kb, int num_sms) {
       lc.gridDim = dim3((unsigned)(c * num_sms)); lc.blockDim = dim3(kThreads); lc.dynamicSmemBytes = S::SMEM;
       lc.attrs = at; lc.numAttrs = 1;
       int n = 0;
-      auto kfn = sharq_linear_kernel<BN, FMT, true>;
+      auto kfn = sharq_linear_kernel<BN, FMT, true, AR>;
       cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, S::SMEM);
       if (cudaOccupancyMaxActiveClusters(&n, kfn, &lc) != cudaSuccess || n <= 0) n = -1;
       max_clusters[c] = n;
@@ -702,6 +710,43 @@ int choose_splits(int64_t tiles, int num_kb, int num_sms) {
     if (max_clusters[c] >= tiles) return c;
   }
   return 1;
+}
+
+template <int BN, int FMT, int AR>
+sharq_status launch_1cta(const LinearArgs& a, const KParams& p, const GroupInfo& g, const CUtensorMap& tm_sp,
+                         const CUtensorMap& tm_dn, const CUtensorMap& tm_w, int64_t tiles, int num_sms,
+                         cudaStream_t st) {
+  const int splits = choose_splits<BN, FMT, AR>(tiles, (int)(a.K / BK), num_sms);
+  cudaLaunchConfig_t lc{};
+  cudaLaunchAttribute attr[2];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  lc.attrs = attr;
+  lc.numAttrs = 1;
+  lc.blockDim = dim3(kThreads);
+  lc.stream = st;
+  if (splits > 1) {
+    using S = Stage<BN, FMT, true, AR>;
+    auto kfn = sharq_linear_kernel<BN, FMT, true, AR>;
+    if (cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, S::SMEM) != cudaSuccess)
+      return SHARQ_ECUDA;
+    lc.gridDim = dim3((unsigned)(tiles * splits));
+    lc.dynamicSmemBytes = S::SMEM;
+    attr[1].id = cudaLaunchAttributeClusterDimension;
+    attr[1].val.clusterDim.x = (unsigned)splits;
+    attr[1].val.clusterDim.y = 1;
+    attr[1].val.clusterDim.z = 1;
+    lc.numAttrs = 2;
+    return cudaLaunchKernelEx(&lc, kfn, tm_sp, tm_dn, tm_w, p, g) == cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
+  }
+  using S = Stage<BN, FMT, false, AR>;
+  auto kfn = sharq_linear_kernel<BN, FMT, false, AR>;
+  if (cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, S::SMEM) != cudaSuccess)
+    return SHARQ_ECUDA;
+  lc.gridDim = dim3((unsigned)(tiles < num_sms ? tiles : num_sms));      // persistent: one CTA per SM
+  if (const char* dbg = getenv("SHARQ_DEBUG_GRID")) lc.gridDim = dim3((unsigned)atoi(dbg));
+  lc.dynamicSmemBytes = S::SMEM;
+  return cudaLaunchKernelEx(&lc, kfn, tm_sp, tm_dn, tm_w, p, g) == cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
 }
 
 // scale-factor / metadata array as a 2-D tensor of 1024-byte rows (256 x u32), boxes of `box_rows` rows
@@ -768,37 +813,9 @@ sharq_status launch_tiles(const LinearArgs& a, const GroupInfo& g, int64_t rows_
     lp.numAttrs = 2;
     return cudaLaunchKernelEx(&lp, kfn, tm_sp, tm_dn, tm_wp, tm_sfa_sp, tm_sfa_dn, tm_meta, tm_sfb_sp, tm_sfb_dn, p) == cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
   }
-  const int splits = choose_splits<BN, FMT>(tiles, (int)(a.K / BK), num_sms);
-  cudaLaunchConfig_t lc{};
-  cudaLaunchAttribute attr[2];
-  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-  attr[0].val.programmaticStreamSerializationAllowed = 1;
-  lc.attrs = attr;
-  lc.numAttrs = 1;
-  lc.blockDim = dim3(kThreads);
-  lc.stream = st;
-  if (splits > 1) {
-    using S = Stage<BN, FMT, true>;
-    auto kfn = sharq_linear_kernel<BN, FMT, true>;
-    if (cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, S::SMEM) != cudaSuccess)
-      return SHARQ_ECUDA;
-    lc.gridDim = dim3((unsigned)(tiles * splits));
-    lc.dynamicSmemBytes = S::SMEM;
-    attr[1].id = cudaLaunchAttributeClusterDimension;
-    attr[1].val.clusterDim.x = (unsigned)splits;
-    attr[1].val.clusterDim.y = 1;
-    attr[1].val.clusterDim.z = 1;
-    lc.numAttrs = 2;
-    return cudaLaunchKernelEx(&lc, kfn, tm_sp, tm_dn, tm_w, p, g) == cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
-  }
-  using S = Stage<BN, FMT, false>;
-  auto kfn = sharq_linear_kernel<BN, FMT, false>;
-  if (cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, S::SMEM) != cudaSuccess)
-    return SHARQ_ECUDA;
-  lc.gridDim = dim3((unsigned)(tiles < num_sms ? tiles : num_sms));      // persistent: one CTA per SM
-  if (const char* dbg = getenv("SHARQ_DEBUG_GRID")) lc.gridDim = dim3((unsigned)atoi(dbg));
-  lc.dynamicSmemBytes = S::SMEM;
-  return cudaLaunchKernelEx(&lc, kfn, tm_sp, tm_dn, tm_w, p, g) == cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
+  if (a_rows <= 16) return launch_1cta<BN, FMT, 16>(a, p, g, tm_sp, tm_dn, tm_w, tiles, num_sms, st);
+  if (a_rows <= 64) return launch_1cta<BN, FMT, 64>(a, p, g, tm_sp, tm_dn, tm_w, tiles, num_sms, st);
+  return launch_1cta<BN, FMT, 128>(a, p, g, tm_sp, tm_dn, tm_w, tiles, num_sms, st);
 }
 
 }  // namespace
