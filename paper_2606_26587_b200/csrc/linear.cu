@@ -820,6 +820,7 @@ sharq_status launch_tiles(const LinearArgs& a, const GroupInfo& g, int64_t rows_
 
 }  // namespace
 
+sharq_status launch_linear_decode(const LinearArgs& a, int num_sms, cudaStream_t st);
 size_t hif4_linear_workspace_bytes(int64_t T, int64_t D, int64_t K);
 sharq_status launch_linear_hif4(const LinearArgs& a, void* workspace, size_t workspace_bytes, int num_sms,
                                 cudaStream_t st);
@@ -833,6 +834,8 @@ sharq_status launch_linear(const sharq_config* cfg, const LinearArgs& a, int32_t
   if (cfg->fmt == SHARQ_HIF4)                             // no FP4-rate tensor path: exact bf16 emulation
     return E > 0 ? SHARQ_EINVAL : launch_linear_hif4(a, workspace, workspace_bytes, num_sms, st);
   if (a.K > (int64_t)1 << 24 || a.D > (int64_t)1 << 24) return SHARQ_ESHAPE;
+  if (cfg->fmt == SHARQ_NVFP4 && E == 0 && a.T <= 64 && !getenv("SHARQ_DEBUG_NO_DECODE"))
+    return launch_linear_decode(a, num_sms, st);          // swapped operands: MMA cost follows T
   GroupInfo g{};
   int64_t rows_total = a.T, m_blocks = (a.T + BM - 1) / BM;
   if (E > 0) {

@@ -306,3 +306,15 @@ __device__ __forceinline__ void mma_sparse_pair(uint32_t d_tmem, uint64_t adesc,
 
 }  // namespace tc
 }  // namespace sharq
+
+namespace sharq {
+namespace tc {
+// 32 lanes x 8 consecutive fp32 columns
+__device__ __forceinline__ void tmem_ld8(uint32_t taddr, uint32_t (&r)[8]) {
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
+               : "r"(taddr)
+               : "memory");
+}
+}  // namespace tc
+}  // namespace sharq
