@@ -16,6 +16,7 @@
 // 2-5 = backbone expanders during the main loop, then epilogue.
 #include <cuda.h>
 #include <cuda_runtime.h>
+#include <stdlib.h>
 
 #include "common.cuh"
 #include "tc_ptx.cuh"
@@ -45,6 +46,8 @@ struct DParams {
   void* Y;
   int64_t ldy;
   int32_t T, D, K, out_fp32, path, n_cols, tiles;     // n_cols = roundup(T, 8): the MMA's N
+  int32_t no_mma;     // experiment: consume the ring without issuing any tensor-core work
+  int32_t w_tiled;    // weight codes stored as [D/128][K/256] tiles of 128 rows x 128 B (16 KB contiguous)
 };
 
 template <int NMAX, bool SPLIT>
@@ -134,7 +137,8 @@ sharq_linear_decode_kernel(const __grid_constant__ CUtensorMap tm_w, const __gri
     for (int tile = tile0; tile < p.tiles; tile += tile_step) {
       const int n0 = tile * 128;                                      // first output feature of the tile
       auto load_w = [&](int kb, uint32_t st, uint32_t fb) {
-        if (lead) tc::tma_load_2d(st + S::W, &tm_w, fb, kb * 128, n0, pol_w);
+        if (lead) tc::tma_load_2d(st + S::W, &tm_w, fb, p.w_tiled ? 0 : kb * 128,
+                                  p.w_tiled ? (tile * (p.K / 256) + kb) * 128 : n0, pol_w);
         if (lead) tc::bulk_load(st + S::SFA, p.w_sf_dn + ((size_t)tile * (Kc / 256) + (size_t)kb) * 2048, 2048, fb, pol_w);
       };
       auto load_a = [&](int kb, uint32_t st, uint32_t fb) {
@@ -189,6 +193,10 @@ sharq_linear_decode_kernel(const __grid_constant__ CUtensorMap tm_w, const __gri
         if (do_sp) tc::mbar_wait(exp_bar(s), ph);
         tc::tc_fence_after();
         const uint32_t st = smem_base + s * S::BYTES;
+        if (p.no_mma) {
+          if (lead) tc::mbar_arrive(empty_bar(s));
+          continue;
+        }
 #pragma unroll
         for (int a = 0; a < 4; ++a) {
           if (lead) tc::tc_cp_sf(tmem_base + S::SFA_COL + 4 * a, tc::smem_desc(st + S::SFA + 512 * a, 128, 0));
@@ -423,7 +431,9 @@ sharq_status launch_decode(const LinearArgs& a, const DParams& p, const CUtensor
 sharq_status launch_linear_decode(const LinearArgs& a, int num_sms, cudaStream_t st) {
   const int n_cols = (int)((a.T + 7) / 8 * 8);
   CUtensorMap tm_w, tm_dn, tm_spc;
-  if (!make_byte_map(&tm_w, a.w_codes, (uint64_t)a.D, (uint64_t)a.K / 2, 128, 128, CU_TENSOR_MAP_SWIZZLE_128B) ||
+  const bool w_tiled = getenv("SHARQ_EXP_WTILED") != nullptr;
+  if (!(w_tiled ? make_byte_map(&tm_w, a.w_codes, (uint64_t)a.D * (uint64_t)(a.K / 256), 128, 128, 128, CU_TENSOR_MAP_SWIZZLE_128B)
+                : make_byte_map(&tm_w, a.w_codes, (uint64_t)a.D, (uint64_t)a.K / 2, 128, 128, CU_TENSOR_MAP_SWIZZLE_128B)) ||
       !make_byte_map(&tm_dn, a.dn_codes, (uint64_t)a.T, (uint64_t)a.K / 2, 128, (uint32_t)n_cols,
                      CU_TENSOR_MAP_SWIZZLE_128B) ||
       !make_byte_map(&tm_spc, a.sp_codes, (uint64_t)a.T, (uint64_t)a.K / 4, 64, (uint32_t)n_cols,
@@ -431,7 +441,7 @@ sharq_status launch_linear_decode(const LinearArgs& a, int num_sms, cudaStream_t
     return SHARQ_ECUDA;
   DParams p{(const uint8_t*)a.sp_sf, (const uint8_t*)a.sp_meta, (const uint8_t*)a.dn_sf, (const uint8_t*)a.w_sf_dn,
             a.row_scale, a.w_ts, (const uint16_t*)a.bias, a.Y, a.ldy, (int32_t)a.T, (int32_t)a.D, (int32_t)a.K,
-            a.out_dtype, a.path, n_cols, (int32_t)(a.D / 128)};
+            a.out_dtype, a.path, n_cols, (int32_t)(a.D / 128), getenv("SHARQ_EXP_NOMMA") ? 1 : 0, w_tiled ? 1 : 0};
   return n_cols <= 16 ? launch_decode<16>(a, p, tm_w, tm_dn, tm_spc, num_sms, st)
                       : launch_decode<64>(a, p, tm_w, tm_dn, tm_spc, num_sms, st);
 }

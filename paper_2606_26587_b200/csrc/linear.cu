@@ -83,20 +83,22 @@ struct Stage {
   static constexpr int SFB_DN = SFB_SP + NB * 1024;
   static constexpr int RAW = SFB_DN + NB * SF_DN_BYTES;
   static constexpr int BYTES = (RAW + 1023) / 1024 * 1024;
-  static constexpr int RECV = SPLIT ? 9 * AR * 64 : 0;                // [src][slot][AR rows][16 fp32]
+  static constexpr int NSL = BN / 16;                                 // 16-column slices of the accumulator
+  static constexpr int RECV = SPLIT ? (NSL + 2) * AR * 64 : 0;        // [src][slot][AR rows][16 fp32]; S*ceil(NSL/S) <= NSL+2 for S in {2,3,4,8}
   static constexpr int PAD = AR < 128 ? 128 * 128 : 0;               // the MMA's over-read behind the last stage
   static constexpr int FIT = (232448 - 1024 - 256 - RECV - PAD) / BYTES;
   static constexpr int STAGES = FIT > 8 ? 8 : FIT;
   static constexpr int SMEM = STAGES * BYTES + PAD + RECV + 1024 /*alignment slack*/ + 256 /*barriers*/;
   // tensor-memory columns: two accumulator stages, then metadata and scale factors
   static constexpr int SFB_COLS = NB * 4;          // columns one MMA's B scales occupy
-  static constexpr int ACC_STAGES = 2;
+  static constexpr int ACC_STAGES = BN > 128 ? 1 : 2;
   static constexpr int E_COL = 256;
   static constexpr int SFA_SP_COL = 260;           // 2 MMAs x 4
   static constexpr int SFA_DN_COL = 268;           // 4 MMAs x 4
   static constexpr int SFB_SP_COL = 284;           // 2 MMAs x SFB_COLS (<= 16)
   static constexpr int SFB_DN_COL = 300;           // 4 MMAs x SFB_COLS (<= 32)
   static_assert(BN * ACC_STAGES <= 256, "accumulator stages overlap the scale-factor columns");
+  static_assert(STAGES >= 2, "shared memory: fewer than two ring stages");
 };
 
 struct Unit { int m_blk, n_blk, expert, rows_valid, kb0, kb1; };
@@ -275,9 +277,9 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
       for (int tile = tile0; tile < p.total_tiles; tile += tile_step, ++n_unit) {
         const Unit u = decode_unit(p, g, tile, rank, splits);
         const uint32_t sfb_shift = (BN < 128) ? (uint32_t)(((u.n_blk * BN) % 128) / 32) : 0u;   // sub-atom N tiles
-        const uint32_t as = n_unit & 1u;                                  // accumulator stage
+        const uint32_t as = n_unit % S::ACC_STAGES;                       // accumulator stage
         const uint32_t acc = tmem_base + as * BN;
-        tc::mbar_wait(tmem_empty_bar(as), ((n_unit >> 1) & 1u) ^ 1u);     // epilogue has drained this stage
+        tc::mbar_wait(tmem_empty_bar(as), ((n_unit / S::ACC_STAGES) & 1u) ^ 1u);   // epilogue has drained this stage
         tc::tc_fence_after();
         uint32_t accumulate = 0;
         for (int kb = u.kb0; kb < u.kb1; ++kb, ++it) {
@@ -342,11 +344,11 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
       uint32_t n_unit = 0;
       for (int tile = tile0; tile < p.total_tiles; tile += tile_step, ++n_unit) {
         const Unit u = decode_unit(p, g, tile, 0, 1);
-        const uint32_t as = n_unit & 1u;
+        const uint32_t as = n_unit % S::ACC_STAGES;
         const int64_t row = (int64_t)u.m_blk * BM + r_local;
         const bool row_ok = r_local < u.rows_valid;
         const float scale = row_ok ? __fmul_rn(p.row_scale[row], p.w_ts[u.expert]) : 0.0f;
-        tc::mbar_wait(tmem_full_bar(as), (n_unit >> 1) & 1u);
+        tc::mbar_wait(tmem_full_bar(as), (n_unit / S::ACC_STAGES) & 1u);
         tc::tc_fence_after();
 #pragma unroll 1
         for (int c = 0; c < BN / 32; ++c) {
@@ -815,12 +817,12 @@ sharq_status launch_tiles(const LinearArgs& a, const GroupInfo& g, int64_t rows_
   }
   if (a_rows <= 16) return launch_1cta<BN, FMT, 16>(a, p, g, tm_sp, tm_dn, tm_w, tiles, num_sms, st);
   if (a_rows <= 64) return launch_1cta<BN, FMT, 64>(a, p, g, tm_sp, tm_dn, tm_w, tiles, num_sms, st);
-  return launch_1cta<BN, FMT, 128>(a, p, g, tm_sp, tm_dn, tm_w, tiles, num_sms, st);
+  if constexpr (BN == 128) return launch_1cta<BN, FMT, 128>(a, p, g, tm_sp, tm_dn, tm_w, tiles, num_sms, st);
+  return SHARQ_EINVAL;                                   // 256-wide tiles are for T <= 64 only
 }
 
 }  // namespace
 
-sharq_status launch_linear_decode(const LinearArgs& a, int num_sms, cudaStream_t st);
 size_t hif4_linear_workspace_bytes(int64_t T, int64_t D, int64_t K);
 sharq_status launch_linear_hif4(const LinearArgs& a, void* workspace, size_t workspace_bytes, int num_sms,
                                 cudaStream_t st);
@@ -834,8 +836,6 @@ sharq_status launch_linear(const sharq_config* cfg, const LinearArgs& a, int32_t
   if (cfg->fmt == SHARQ_HIF4)                             // no FP4-rate tensor path: exact bf16 emulation
     return E > 0 ? SHARQ_EINVAL : launch_linear_hif4(a, workspace, workspace_bytes, num_sms, st);
   if (a.K > (int64_t)1 << 24 || a.D > (int64_t)1 << 24) return SHARQ_ESHAPE;
-  if (cfg->fmt == SHARQ_NVFP4 && E == 0 && a.T <= 64 && !getenv("SHARQ_DEBUG_NO_DECODE"))
-    return launch_linear_decode(a, num_sms, st);          // swapped operands: MMA cost follows T
   GroupInfo g{};
   int64_t rows_total = a.T, m_blocks = (a.T + BM - 1) / BM;
   if (E > 0) {
@@ -853,6 +853,14 @@ sharq_status launch_linear(const sharq_config* cfg, const LinearArgs& a, int32_t
     if (m_blocks == 0) return SHARQ_OK;
   }
   if (m_blocks * (a.D / 128) > (int64_t)1 << 30) return SHARQ_ESHAPE;
+  // T <= 64: 128 x 256 tiles halve the per-column cost of the scale-factor copies and of the M = 128 MMA
+  // (the decode launches are bound by tensor-pipe issue per k-block, not by HBM)
+  // ... and only pays when the 128-wide tiles would need a second round on the SMs (measured: with fewer
+  // tiles than SMs the narrower tiles + deeper K-split win)
+  if (E == 0 && a.T <= 64 && a.D % 256 == 0 && a.D / 128 > num_sms && !getenv("SHARQ_DEBUG_NO_WIDE")) {
+    if (cfg->fmt == SHARQ_NVFP4) return launch_tiles<256, SHARQ_NVFP4>(a, g, rows_total, m_blocks, E, num_sms, st);
+    return launch_tiles<256, SHARQ_MXFP4>(a, g, rows_total, m_blocks, E, num_sms, st);
+  }
   if (cfg->fmt == SHARQ_NVFP4) return launch_tiles<128, SHARQ_NVFP4>(a, g, rows_total, m_blocks, E, num_sms, st);
   return launch_tiles<128, SHARQ_MXFP4>(a, g, rows_total, m_blocks, E, num_sms, st);
 }
