@@ -431,50 +431,57 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
 // For T >= 256 the 128 x 128 kernel is bound by shared-memory refill latency (48 KB per 384 MMA cycles).
 // Here each CTA stages its own 128 rows of A but only HALF of the 256-row W tile, and one tcgen05.mma
 // with M = 256, N = 256 consumes both CTAs' shared memory: same bytes per stage, twice the MMA work.
-template <int FMT>
+// PBN = tile width: 192 -> two TMEM accumulator stages (2 x 192 + 76 scale / metadata columns <= 512), so the
+// epilogue of tile i overlaps the main loop of tile i+1, and finer wave quantisation; 256 -> one stage.
+template <int FMT, int PBN>
 struct PairStage {
   static constexpr int SF_DN_BYTES = (FMT == SHARQ_NVFP4) ? 2048 : 1024;
+  static constexpr int BN = PBN;
+  static constexpr int HALF = PBN / 2;                   // W rows this CTA stages
   static constexpr int A_DN = 0;
-  static constexpr int W = A_DN + BM * 128;              // this CTA's 128 rows of the 256-row W tile
-  static constexpr int A_SP = W + 128 * 128;
+  static constexpr int W = A_DN + BM * 128;
+  static constexpr int A_SP = W + HALF * 128;
   static constexpr int META = A_SP + BM * 64;
   static constexpr int SFA_SP = META + 2048;
   static constexpr int SFA_DN = SFA_SP + 1024;
-  static constexpr int SFB_SP = SFA_DN + SF_DN_BYTES;    // all 256 W rows: both CTAs need every B scale
+  static constexpr int SFB_SP = SFA_DN + SF_DN_BYTES;    // two 128-row atoms rows: both CTAs need every B scale
   static constexpr int SFB_DN = SFB_SP + 2 * 1024;
   static constexpr int RAW = SFB_DN + 2 * SF_DN_BYTES;
   static constexpr int BYTES = (RAW + 1023) / 1024 * 1024;
   static constexpr int STAGES = 4;
   static constexpr int SMEM = STAGES * BYTES + 1024 + 256;
-  static constexpr int BN = 256;
+  static constexpr int ACC_STAGES = PBN <= 192 ? 2 : 1;
   static constexpr int SFB_COLS = 8;
-  static constexpr int E_COL = 256, SFA_SP_COL = 260, SFA_DN_COL = 268, SFB_SP_COL = 284, SFB_DN_COL = 300;
+  static constexpr int SF0 = PBN * ACC_STAGES;           // first column after the accumulators
+  static constexpr int E_COL = SF0, SFA_SP_COL = SF0 + 4, SFA_DN_COL = SF0 + 12, SFB_SP_COL = SF0 + 28,
+                       SFB_DN_COL = SF0 + 44;
+  static_assert(SF0 + 76 <= 512, "tensor memory");
 };
 
-template <int FMT>
+template <int FMT, int PBN>
 __global__ void __launch_bounds__(kThreads, 1)
 sharq_linear_pair_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_constant__ CUtensorMap tm_a_dn,
                          const __grid_constant__ CUtensorMap tm_w, const __grid_constant__ CUtensorMap tm_sfa_sp,
                          const __grid_constant__ CUtensorMap tm_sfa_dn, const __grid_constant__ CUtensorMap tm_meta,
                          const __grid_constant__ CUtensorMap tm_sfb_sp, const __grid_constant__ CUtensorMap tm_sfb_dn,
                          const KParams p) {
-  using S = PairStage<FMT>;
+  using S = PairStage<FMT, PBN>;
   constexpr bool NV = (FMT == SHARQ_NVFP4);
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
   const uint32_t bars = smem_base + S::STAGES * S::BYTES;
   auto full_bar = [&](int s) { return bars + 8u * s; };                       // used in the leader CTA
   auto empty_bar = [&](int s) { return bars + 8u * (2 * S::STAGES + s); };
-  const uint32_t tmem_full_bar = bars + 8u * (3 * S::STAGES);
-  const uint32_t tmem_empty_bar = bars + 8u * (3 * S::STAGES + 1);            // leader CTA
-  const uint32_t tmem_ptr_smem = bars + 8u * (3 * S::STAGES + 2);
+  auto tmem_full_bar = [&](int a) { return bars + 8u * (3 * S::STAGES + a); };
+  auto tmem_empty_bar = [&](int a) { return bars + 8u * (3 * S::STAGES + 2 + a); };   // leader CTA
+  const uint32_t tmem_ptr_smem = bars + 8u * (3 * S::STAGES + 4);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int rank = (int)tc::cluster_ctarank();
   const bool do_sp = p.path != 2, do_dn = p.path != 1;
   const int num_kb = p.K / BK;
   const int m_pairs = (p.m_blocks + 1) / 2;
-  const int total = m_pairs * (p.D / S::BN);
+  const int total = m_pairs * ((p.D + S::BN - 1) / S::BN);      // the last tile may be ragged in N
   const int tile0 = (int)tc::cluster_id_x(), tile_step = (int)(gridDim.x >> 1);
 
   if (warp == 0 && lane == 0) {
@@ -492,8 +499,10 @@ sharq_linear_pair_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __gr
       tc::mbar_init(full_bar(s), 1);             // leader's expect_tx; every load of the pair completes here
       tc::mbar_init(empty_bar(s), 1);
     }
-    tc::mbar_init(tmem_full_bar, 1);
-    tc::mbar_init(tmem_empty_bar, 8);            // four epilogue warps in each CTA
+    for (int a = 0; a < 2; ++a) {
+      tc::mbar_init(tmem_full_bar(a), 1);
+      tc::mbar_init(tmem_empty_bar(a), 8);       // four epilogue warps in each CTA
+    }
     tc::fence_mbar_init();
   }
   if (warp == 2) tc::tmem_alloc_pair<kTmemCols>(tmem_ptr_smem);
@@ -514,7 +523,7 @@ sharq_linear_pair_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __gr
       const int64_t Kc = p.K;
       // every load of the pair (tiles, scale-factor atoms, metadata) is a cta_group::2 tensor copy whose
       // complete_tx lands on the LEADER's full barrier: no cross-CTA hand-off inside the ring
-      const uint32_t tx = 2u * (128 * 128 + (do_sp ? BM * 64 + 2048 + 1024 + 2 * 1024 : 0) +
+      const uint32_t tx = 2u * (S::HALF * 128 + (do_sp ? BM * 64 + 2048 + 1024 + 2 * 1024 : 0) +
                                 (do_dn ? BM * 128 + 3 * S::SF_DN_BYTES : 0));
       constexpr int DN_ROWS = S::SF_DN_BYTES / 1024;       // 1024-byte rows of the scale-factor tensor maps
       const int kq = p.K / 256;
@@ -531,7 +540,7 @@ sharq_linear_pair_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __gr
           const uint32_t st = smem_base + s * S::BYTES;
           const uint32_t fb = full_bar(s);
           if (lead && rank == 0) tc::mbar_expect_tx(fb, tx);
-          if (lead) tc::tma_load_2d_pair(st + S::W, &tm_w, fb, kb * 128, n0 + rank * 128, pol);
+          if (lead) tc::tma_load_2d_pair(st + S::W, &tm_w, fb, kb * 128, n0 + rank * S::HALF, pol);
           if (do_sp) {
             if (lead) tc::tma_load_2d_pair(st + S::A_SP, &tm_a_sp, fb, kb * 64, m_blk * BM, pol);
             if (lead) tc::tma_load_2d_pair(st + S::META, &tm_meta, fb, 0, (m_sf * kq + kb) * 2, pol);
@@ -558,7 +567,10 @@ sharq_linear_pair_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __gr
       const uint32_t idesc_sp = tc::idesc_fp4(256, S::BN, true, !NV, 0, 0);
       uint32_t it = 0, n_unit = 0;
       for (int tile = tile0; tile < total; tile += tile_step, ++n_unit) {
-        tc::mbar_wait(tmem_empty_bar, (n_unit & 1u) ^ 1u);    // both CTAs' epilogues drained the accumulator
+        const uint32_t as = n_unit % S::ACC_STAGES;
+        const uint32_t acc = tmem_base + as * S::BN;
+        const uint32_t sfb_shift = (uint32_t)((((tile / m_pairs) * S::BN) % 128) / 32);   // tile starts inside a 128-row atom
+        tc::mbar_wait(tmem_empty_bar(as), ((n_unit / S::ACC_STAGES) & 1u) ^ 1u);   // both CTAs' epilogues drained it
         tc::tc_fence_after();
         uint32_t accumulate = 0;
         for (int kb = 0; kb < num_kb; ++kb, ++it) {
@@ -578,9 +590,10 @@ sharq_linear_pair_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __gr
             }
 #pragma unroll
             for (int j = 0; j < 2; ++j) {
-              if (lead) tc::mma_sparse_pair(tmem_base, tc::smem_desc(st + S::A_SP + 32 * j, 512, 4),
+              if (lead) tc::mma_sparse_pair(acc, tc::smem_desc(st + S::A_SP + 32 * j, 512, 4),
                                   tc::smem_desc(st + S::W + 64 * j, 1024, 2), idesc_sp,
-                                  tmem_base + S::SFA_SP_COL + 4 * j, tmem_base + S::SFB_SP_COL + S::SFB_COLS * j,
+                                  tmem_base + S::SFA_SP_COL + 4 * j,
+                                  tmem_base + S::SFB_SP_COL + S::SFB_COLS * j + sfb_shift,
                                   tmem_base + S::E_COL + 2 * j, accumulate);
               accumulate = 1;
             }
@@ -600,16 +613,16 @@ sharq_linear_pair_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __gr
               const int atom = NV ? j : j / 2;
               const uint32_t sf_id = NV ? 0u : (uint32_t)(j & 1) * 2u;
               const uint32_t idesc_dn = tc::idesc_fp4(256, S::BN, false, !NV, sf_id, sf_id);
-              if (lead) tc::mma_dense_pair<NV>(tmem_base, tc::smem_desc(st + S::A_DN + 32 * j, 1024, 2),
+              if (lead) tc::mma_dense_pair<NV>(acc, tc::smem_desc(st + S::A_DN + 32 * j, 1024, 2),
                                      tc::smem_desc(st + S::W + 32 * j, 1024, 2), idesc_dn,
                                      tmem_base + S::SFA_DN_COL + 4 * atom,
-                                     tmem_base + S::SFB_DN_COL + S::SFB_COLS * atom, accumulate);
+                                     tmem_base + S::SFB_DN_COL + S::SFB_COLS * atom + sfb_shift, accumulate);
               accumulate = 1;
             }
           }
           if (lead) tc::tc_commit_pair(empty_bar(s), 3);              // frees this slot in BOTH CTAs
         }
-        if (lead) tc::tc_commit_pair(tmem_full_bar, 3);
+        if (lead) tc::tc_commit_pair(tmem_full_bar(as), 3);
       }
     }
   } else {
@@ -617,21 +630,21 @@ sharq_linear_pair_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __gr
     const int sub = warp & 3;
     const int r_local = sub * 32 + lane;
     const uint32_t lane_addr = tmem_base + ((uint32_t)(sub * 32) << 16);
-    const uint32_t empty_remote = tc::map_to_cta(tmem_empty_bar, 0);
     uint32_t n_unit = 0;
     for (int tile = tile0; tile < total; tile += tile_step, ++n_unit) {
       const int m_blk = 2 * (tile % m_pairs) + rank, n_blk = tile / m_pairs;
       const int64_t row = (int64_t)m_blk * BM + r_local;
       const bool row_ok = row < p.T;
       const float scale = row_ok ? __fmul_rn(p.row_scale[row], p.w_ts[0]) : 0.0f;
-      tc::mbar_wait(tmem_full_bar, n_unit & 1u);
+      const uint32_t as = n_unit % S::ACC_STAGES;
+      tc::mbar_wait(tmem_full_bar(as), (n_unit / S::ACC_STAGES) & 1u);
       tc::tc_fence_after();
 #pragma unroll 1
       for (int c = 0; c < S::BN / 32; ++c) {
         uint32_t v[32];
-        tc::tmem_ld32(lane_addr + c * 32, v);
+        tc::tmem_ld32(lane_addr + as * S::BN + c * 32, v);
         tc::tmem_ld_wait();
-        if (row_ok) {
+        if (row_ok && n_blk * S::BN + c * 32 < p.D) {
           float f[32];
 #pragma unroll
           for (int i = 0; i < 32; ++i) f[i] = __uint_as_float(v[i]);
@@ -640,7 +653,7 @@ sharq_linear_pair_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __gr
       }
       tc::tc_fence_before();
       __syncwarp();
-      if (lane == 0) tc::mbar_arrive_cluster(empty_remote);
+      if (lane == 0) tc::mbar_arrive_cluster(tc::map_to_cta(tmem_empty_bar(as), 0));
     }
   }
   tc::tc_fence_before();
@@ -764,6 +777,44 @@ bool make_map_rows1k(CUtensorMap* m, const void* base, uint64_t bytes, uint32_t 
             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
+template <int FMT, int PBN>
+sharq_status launch_pair(const LinearArgs& a, const KParams& p, const CUtensorMap& tm_sp, const CUtensorMap& tm_dn,
+                         int64_t m_blocks, int num_sms, cudaStream_t st) {
+  using P = PairStage<FMT, PBN>;
+  CUtensorMap tm_wp, tm_sfa_sp, tm_sfa_dn, tm_meta, tm_sfb_sp, tm_sfb_dn;
+  const uint64_t act_rows = (uint64_t)m_blocks * 128, kk = (uint64_t)a.K;
+  const uint32_t dn_rows = P::SF_DN_BYTES / 1024;
+  const uint64_t dn_div = (FMT == SHARQ_NVFP4) ? 16 : 32;
+  if (!make_map(&tm_wp, a.w_codes, (uint64_t)a.D, kk / 2, 128, P::HALF) ||
+      !make_map_rows1k(&tm_sfa_sp, a.sp_sf, act_rows * kk / 32, 1) ||
+      !make_map_rows1k(&tm_sfa_dn, a.dn_sf, act_rows * kk / dn_div, dn_rows) ||
+      !make_map_rows1k(&tm_meta, a.sp_meta, act_rows * kk / 16, 2) ||
+      !make_map_rows1k(&tm_sfb_sp, a.w_sf_sp, (uint64_t)a.D * kk / 32, 1) ||
+      !make_map_rows1k(&tm_sfb_dn, a.w_sf_dn, (uint64_t)a.D * kk / dn_div, dn_rows))
+    return SHARQ_ECUDA;
+  auto kfn = sharq_linear_pair_kernel<FMT, PBN>;
+  if (cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, P::SMEM) != cudaSuccess)
+    return SHARQ_ECUDA;
+  const int64_t pair_tiles = ((m_blocks + 1) / 2) * ((a.D + PBN - 1) / PBN);
+  const int64_t clusters = pair_tiles < num_sms / 2 ? pair_tiles : num_sms / 2;
+  cudaLaunchConfig_t lp{};
+  cudaLaunchAttribute at[2];
+  at[0].id = cudaLaunchAttributeClusterDimension;
+  at[0].val.clusterDim.x = 2;
+  at[0].val.clusterDim.y = 1;
+  at[0].val.clusterDim.z = 1;
+  at[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[1].val.programmaticStreamSerializationAllowed = 1;
+  lp.blockDim = dim3(kThreads);
+  lp.gridDim = dim3((unsigned)(2 * clusters));
+  lp.dynamicSmemBytes = P::SMEM;
+  lp.stream = st;
+  lp.attrs = at;
+  lp.numAttrs = 2;
+  return cudaLaunchKernelEx(&lp, kfn, tm_sp, tm_dn, tm_wp, tm_sfa_sp, tm_sfa_dn, tm_meta, tm_sfb_sp, tm_sfb_dn, p) ==
+                 cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
+}
+
 template <int BN, int FMT>
 sharq_status launch_tiles(const LinearArgs& a, const GroupInfo& g, int64_t rows_total, int64_t m_blocks, int E,
                           int num_sms, cudaStream_t st) {
@@ -781,39 +832,17 @@ sharq_status launch_tiles(const LinearArgs& a, const GroupInfo& g, int64_t rows_
   const char* no_pair = getenv("SHARQ_DEBUG_NO_PAIR");
   const char* force_pair = getenv("SHARQ_DEBUG_FORCE_PAIR");
   const bool pair_worth = ((m_blocks + 1) / 2) * (a.D / 256) >= num_sms / 4 || (force_pair && force_pair[0] == '1');
-  if (E == 0 && m_blocks >= 2 && a.D % 256 == 0 && BN == 128 && pair_worth && !(no_pair && no_pair[0] == '1')) {
-    using P = PairStage<FMT>;
-    CUtensorMap tm_wp, tm_sfa_sp, tm_sfa_dn, tm_meta, tm_sfb_sp, tm_sfb_dn;
-    const uint64_t act_rows = (uint64_t)m_blocks * 128, kk = (uint64_t)a.K;
-    const uint32_t dn_rows = P::SF_DN_BYTES / 1024;
-    const uint64_t dn_div = (FMT == SHARQ_NVFP4) ? 16 : 32;
-    if (!make_map(&tm_wp, a.w_codes, (uint64_t)w_rows, kk / 2, 128, 128) ||
-        !make_map_rows1k(&tm_sfa_sp, a.sp_sf, act_rows * kk / 32, 1) ||
-        !make_map_rows1k(&tm_sfa_dn, a.dn_sf, act_rows * kk / dn_div, dn_rows) ||
-        !make_map_rows1k(&tm_meta, a.sp_meta, act_rows * kk / 16, 2) ||
-        !make_map_rows1k(&tm_sfb_sp, a.w_sf_sp, (uint64_t)a.D * kk / 32, 1) ||
-        !make_map_rows1k(&tm_sfb_dn, a.w_sf_dn, (uint64_t)a.D * kk / dn_div, dn_rows))
-      return SHARQ_ECUDA;
-    auto kfn = sharq_linear_pair_kernel<FMT>;
-    if (cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, P::SMEM) != cudaSuccess)
-      return SHARQ_ECUDA;
-    const int64_t pair_tiles = ((m_blocks + 1) / 2) * (a.D / 256);
-    const int64_t clusters = pair_tiles < num_sms / 2 ? pair_tiles : num_sms / 2;
-    cudaLaunchConfig_t lp{};
-    cudaLaunchAttribute at[2];
-    at[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    at[1].val.programmaticStreamSerializationAllowed = 1;
-    lp.blockDim = dim3(kThreads);
-    lp.gridDim = dim3((unsigned)(2 * clusters));
-    lp.dynamicSmemBytes = P::SMEM;
-    lp.stream = st;
-    at[0].id = cudaLaunchAttributeClusterDimension;
-    at[0].val.clusterDim.x = 2;
-    at[0].val.clusterDim.y = 1;
-    at[0].val.clusterDim.z = 1;
-    lp.attrs = at;
-    lp.numAttrs = 2;
-    return cudaLaunchKernelEx(&lp, kfn, tm_sp, tm_dn, tm_wp, tm_sfa_sp, tm_sfa_dn, tm_meta, tm_sfb_sp, tm_sfb_dn, p) == cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
+  if (E == 0 && m_blocks >= 2 && BN == 128 && pair_worth && !(no_pair && no_pair[0] == '1')) {
+    // tile width by a two-term cost model fitted on the box (us): rounds x (k-blocks x 0.43 + exposed
+    // epilogue), the epilogue being hidden by the second TMEM accumulator only for 192-wide tiles
+    const int64_t clusters = num_sms / 2, m_pairs = (m_blocks + 1) / 2;
+    const double per_kb = 0.43 * (double)(a.K / BK);
+    const double cost192 = (double)((m_pairs * ((a.D + 191) / 192) + clusters - 1) / clusters) * (per_kb + 0.3);
+    const double cost256 = (double)((m_pairs * ((a.D + 255) / 256) + clusters - 1) / clusters) * (per_kb + 2.0);
+    int width = (a.D % 256 != 0 || cost192 < cost256) ? 192 : 256;
+    if (const char* pbn = getenv("SHARQ_DEBUG_PAIR_BN")) width = (atoi(pbn) == 256 && a.D % 256 == 0) ? 256 : 192;
+    if (width == 256) return launch_pair<FMT, 256>(a, p, tm_sp, tm_dn, m_blocks, num_sms, st);
+    return launch_pair<FMT, 192>(a, p, tm_sp, tm_dn, m_blocks, num_sms, st);
   }
   if (a_rows <= 16) return launch_1cta<BN, FMT, 16>(a, p, g, tm_sp, tm_dn, tm_w, tiles, num_sms, st);
   if (a_rows <= 64) return launch_1cta<BN, FMT, 64>(a, p, g, tm_sp, tm_dn, tm_w, tiles, num_sms, st);
