@@ -672,6 +672,7 @@ static cudaError_t launch_row_kernel(int norm, const PrepParams& p, int num_sms,
   const int warps = (int)((p.K + 1023) / 1024);
   const dim3 block((unsigned)warps * 32);
   int per_sm = 2048 / (warps * 32);                       // thread limit; registers trim it further at launch
+  if (const char* e = getenv("SHARQ_DEBUG_ROW_PER_SM")) per_sm = atoi(e);
   if (per_sm < 1) per_sm = 1;
   if (per_sm > 8) per_sm = 8;
   int64_t ctas = (int64_t)num_sms * per_sm;
@@ -691,9 +692,20 @@ static cudaError_t launch_row_kernel(int norm, const PrepParams& p, int num_sms,
     else if (norm == SHARQ_NORM_RMS) SHARQ_ROW(SHARQ_NORM_RMS, MAXT, MINB);  \
     else SHARQ_ROW(SHARQ_NORM_LAYER, MAXT, MINB);                            \
   }
-  if (warps <= 4) SHARQ_ROW_N(128, 5)            // <= 102 registers, 20 warps / SM
-  else if (warps <= 8) SHARQ_ROW_N(256, 3)       // <= 85 registers
-  else if (warps <= 16) SHARQ_ROW_N(512, 1)      // <= 128 registers
+#ifndef SHARQ_ROW_MINB_128
+#define SHARQ_ROW_MINB_128 8
+#endif
+#ifndef SHARQ_ROW_MINB_256
+#define SHARQ_ROW_MINB_256 3
+#endif
+#ifndef SHARQ_ROW_MINB_512
+#define SHARQ_ROW_MINB_512 2
+#endif
+  // occupancy beats register comfort here (measured: 64 registers with a few spills and 28-32 warps / SM is
+  // up to 19 % faster than 96-128 registers with 14-20 warps: the kernel is issue bound with long stalls)
+  if (warps <= 4) SHARQ_ROW_N(128, SHARQ_ROW_MINB_128)
+  else if (warps <= 8) SHARQ_ROW_N(256, SHARQ_ROW_MINB_256)
+  else if (warps <= 16) SHARQ_ROW_N(512, SHARQ_ROW_MINB_512)
   else SHARQ_ROW_N(1024, 1)                      // <= 64 registers
 #undef SHARQ_ROW_N
 #undef SHARQ_ROW
