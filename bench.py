@@ -301,8 +301,14 @@ def run_ours(args):
     n_lin = len(DECODE_T) * len(LLAMA)
     lin_bytes = sum(linear_bytes(T, K, D) for T in DECODE_T for _, K, D, _ in LLAMA)
     ach = lin_bytes / (ms_lin * 1e-3) / 1e9
-    roofline = dict(kernel="sharq_linear_kernel<128,NVFP4>", bound="hbm", achieved=round(ach, 1), peak=pk["hbm"],
-                    unit="GB/s", frac=round(ach / pk["hbm"], 4), traffic=None, peak_source=pk["source"],
+    traffic = None                                        # per-launch DRAM bytes from the committed ncu capture
+    tpath = os.path.join(ROOT, "profiles", "linear_decode_traffic_r1.json")
+    if os.path.exists(tpath):
+        with open(tpath) as f:
+            traffic = json.load(f).get("traffic_bytes_per_launch")
+    roofline = dict(kernel="sharq_linear (the 20 launches of the step: 128-wide split-K cluster / persistent, "
+                           "256-wide and CTA-pair variants)", bound="hbm", achieved=round(ach, 1), peak=pk["hbm"],
+                    unit="GB/s", frac=round(ach / pk["hbm"], 4), traffic=traffic, peak_source=pk["source"],
                     launches_per_step=n_lin, avg_launch_us=round(ms_lin * 1e3 / n_lin, 2),
                     algorithmic_bytes_per_launch=round(lin_bytes / n_lin),
                     share_of_step=round(ms_lin / ms_step, 3))
