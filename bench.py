@@ -387,6 +387,32 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def mma_issue_peaks(sq):
+    """FP4 tensor peaks measured on this GPU by the library's MMA issue-rate probe (sharq_mma_peak_launch):
+    dense-only, sparse-only, and the fused per-k-block sequence with its scale-factor copies; `burst` = one
+    2 ms launch, `sustained` = the last of back-to-back launches over ~1.5 s (power-capped clocks)."""
+    import torch
+    n_sm = torch.cuda.get_device_properties(0).multi_processor_count
+    out = {}
+    for name, mode in (("dense", 1), ("sparse", 2), ("fused_with_sf_copies", 7)):
+        paths = (1 if mode & 1 else 0) + (1 if mode & 2 else 0)
+        res = {}
+        for kind, iters, secs in (("burst", 4000, 0.0), ("sustained", 40000, 1.5)):
+            sq.mma_peak_launch(mode, 100)
+            torch.cuda.synchronize()
+            t_end = time.time() + secs
+            while True:
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(); sq.mma_peak_launch(mode, iters); e1.record()
+                torch.cuda.synchronize()
+                if time.time() >= t_end:
+                    break
+            ms = e0.elapsed_time(e1)
+            res[kind] = round(paths * 2.0 * 128 * 256 * 256 * iters * (n_sm // 2 * 2) / ms / 1e9, 1)
+        out[name] = res
+    return out
+
+
 def prefill_extras(sq, wl, pk, steps):
     """configs[2] family at T = 4096 (compute-bound) and the prep kernel's HBM rate: reported beside the
     headline, same kernels, CUDA events.  FP4 tensor peak = measured bf16 peak x 4 (dense, nominal ratio
@@ -396,6 +422,11 @@ def prefill_extras(sq, wl, pk, steps):
            "peak_note": f"4x / 8x the {pk['source']} sustained bf16 cuBLAS rate", "linear_T4096": {}, "prepare": {}}
     T = PREFILL_T
     p_dn, p_sp = 4 * pk["bf16_sustained"] * 1e12, 8 * pk["bf16_sustained"] * 1e12
+    mp = mma_issue_peaks(sq)
+    out["mma_issue_probe_tflops"] = mp
+    out["mma_issue_probe_note"] = ("sharq_mma_peak_launch: the GEMM's own per-k-block tcgen05 sequence on smem-resident "
+                                   "bytes (nominal 2MNK flop per path); frac_of_mma_probe uses the sustained dense and sparse rates")
+    q_dn, q_sp = mp["dense"]["sustained"] * 1e12, mp["sparse"]["sustained"] * 1e12
     for i, (n, K, D, norm) in enumerate(LLAMA):
         x = device_activations(T, K, BASE_SEED + 50 + i)
         act = sq.alloc_act(wl.cfg[n], T, K, "cuda")
@@ -406,7 +437,8 @@ def prefill_extras(sq, wl, pk, steps):
         fl = layer_flops(T, K, D)
         t_min = fl / p_dn + fl / p_sp
         out["linear_T4096"][n] = dict(us=round(ms * 1e3, 1), effective_tflops=round(fl / ms / 1e9, 1),
-                                      frac_of_fp4_roofline=round(t_min / (ms * 1e-3), 4))
+                                      frac_of_fp4_roofline=round(t_min / (ms * 1e-3), 4),
+                                      frac_of_mma_probe=round((fl / q_dn + fl / q_sp) / (ms * 1e-3), 4))
         del x, act, Y
     for K, norm in ((4096, 1), (14336, 0)):
         Tp = 8192

@@ -151,6 +151,14 @@ sharq_status sharq_linear_grouped(const sharq_config* cfg, int32_t E, const int3
                                   int32_t out_dtype, void* workspace, size_t workspace_bytes,
                                   void* stream);
 
+/* ---- diagnostics: tensor-pipe issue-rate probe (not part of the hot path) -------------------------
+ * Launches, on every SM pair, `iters` repetitions of the per-k-block (256 logical k) instruction sequence
+ * of the CTA-pair GEMM on shared-memory-resident bytes: mode bit 1 = the 4 dense block-scaled MMAs, bit 2 =
+ * the 2 sparse MMAs, bit 4 = the scale-factor / metadata tcgen05.cp copies; M = 256, N = 256 per pair, no
+ * loads, no epilogue.  The caller times it (CUDA events): nominal flop per path = 2 * 128 * 256 * 256 *
+ * iters * (number of SMs).  Gives the applicable FP4 tensor peak of the GPU. */
+sharq_status sharq_mma_peak_launch(int32_t mode, int32_t iters, void* stream);
+
 /* Library / build information: returns a static string, e.g. "sharq-b200 0.1 sm_100a". */
 const char* sharq_version(void);
 

@@ -61,6 +61,8 @@ def _load() -> ctypes.CDLL:
                                  c_int32, c_int32, P, c_size_t, P]
     lib.sharq_linear_grouped.argtypes = [CFG, c_int32, POINTER(c_int32), c_int64, c_int64, P, P, P, P, P, P, P, P,
                                          P, P, P, c_int64, c_int32, P, c_size_t, P]
+    lib.sharq_mma_peak_launch.argtypes = [c_int32, c_int32, P]
+    lib.sharq_mma_peak_launch.restype = c_int32
     for name in ("sharq_weight_sizes", "sharq_act_sizes", "sharq_linear_workspace", "sharq_quantize_weight",
                  "sharq_prepare", "sharq_linear", "sharq_linear_grouped"):
         getattr(lib, name).restype = c_int32
@@ -69,7 +71,8 @@ def _load() -> ctypes.CDLL:
 
 capi = _load()
 EXPORTS = ("sharq_version", "sharq_weight_sizes", "sharq_act_sizes", "sharq_linear_workspace",
-           "sharq_quantize_weight", "sharq_prepare", "sharq_linear", "sharq_linear_grouped")
+           "sharq_quantize_weight", "sharq_prepare", "sharq_linear", "sharq_linear_grouped",
+           "sharq_mma_peak_launch")
 
 
 def version() -> str:
@@ -110,6 +113,11 @@ def linear_workspace(cfg: Config, T: int, D: int, K: int, E: int = 0) -> int:
     s = c_size_t()
     _check(capi.sharq_linear_workspace(ctypes.byref(cfg), T, D, K, E, ctypes.byref(s)), "sharq_linear_workspace")
     return s.value
+
+
+def mma_peak_launch(mode: int, iters: int):
+    """Diagnostics: launch the tensor-pipe issue-rate probe on the current stream (see sharq.h)."""
+    _check(capi.sharq_mma_peak_launch(mode, iters, _stream()), "sharq_mma_peak_launch")
 
 
 def _bytes(n, device):

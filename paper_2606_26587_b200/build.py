@@ -8,7 +8,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libsharq.so")
-SOURCES = ["api.cu", "prepare.cu", "linear.cu", "linear_hif4.cu"]
+SOURCES = ["api.cu", "prepare.cu", "linear.cu", "linear_hif4.cu", "mma_peak.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-cudart", "static"]
 
