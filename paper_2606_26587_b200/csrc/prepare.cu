@@ -91,13 +91,20 @@ __device__ __forceinline__ float leaf8(const uint32_t* v) {
   return acc;
 }
 
+// x * y >> 32 as an integer multiply (FMA pipe): the ALU pipe is the kernel's bottleneck
+__device__ __forceinline__ uint32_t mulhi_u32(uint32_t x, uint32_t y) {
+  uint32_t r;
+  asm("mul.hi.u32 %0, %1, %2;" : "=r"(r) : "r"(x), "r"(y));
+  return r;
+}
+
 // top-2-of-4 on keys (score << 2 | 3 - p): returns nibble i0 | i1 << 2 and the best key.
 __device__ __forceinline__ void top2of4(uint32_t k0, uint32_t k1, uint32_t k2, uint32_t k3, uint32_t& i0,
                                         uint32_t& i1, uint32_t& best) {
   uint32_t m01 = max(k0, k1), n01 = min(k0, k1), m23 = max(k2, k3), n23 = min(k2, k3);
-  uint32_t t1 = max(m01, m23), lo = min(m01, m23);
-  uint32_t alt = (m01 > m23) ? n01 : n23;
-  uint32_t t2 = max(lo, alt);
+  uint32_t t1 = max(m01, m23);
+  // second largest of two sorted pairs: the smaller group maximum or the larger group minimum
+  uint32_t t2 = max(min(m01, m23), max(n01, n23));
   uint32_t a = (t1 & 3u) ^ 3u, b = (t2 & 3u) ^ 3u;
   i0 = min(a, b);
   i1 = max(a, b);
@@ -135,8 +142,8 @@ __device__ __forceinline__ void quantize_block_e2m1(const PrepParams& p, int64_t
 #pragma unroll
     for (int q = 0; q < 4; ++q) {
       const uint32_t a = X[4 * c + q] & 0x7FFF7FFFu;
-      const uint32_t s = max(a & 0xFFFFu, a >> 16);
-      key[q] = (s << 2) | (3u - q);
+      const uint32_t s = max(a & 0xFFFFu, mulhi_u32(a, 65536u));        // a >> 16 on the FMA pipe
+      key[q] = s * 4u + (3u - q);
     }
     uint32_t best;
     top2of4(key[0], key[1], key[2], key[3], i0[c], i1[c], best);
@@ -643,12 +650,10 @@ __global__ void __launch_bounds__(MAXT, MINB) sharq_prepare_row_kernel(const Pre
     // ---- O2 per-row tensor scale
     float ts = 1.0f, inv_ts = 1.0f;
     if (need_rowmax) {
-      uint32_t amax = 0;
+      uint32_t amax2 = 0;                        // both bf16 halves at once (packed unsigned 16-bit max)
 #pragma unroll
-      for (int i = 0; i < 16; ++i) {
-        const uint32_t a = X[i] & 0x7FFF7FFFu;
-        amax = max(amax, max(a & 0xFFFFu, a >> 16));
-      }
+      for (int i = 0; i < 16; ++i) amax2 = __vmaxu2(amax2, X[i] & 0x7FFF7FFFu);
+      uint32_t amax = max(amax2 & 0xFFFFu, amax2 >> 16);
       amax = warp_max_u32(amax);
       if (lane == 0) sh.amax[amax_slot * 32 + warp] = amax;
       __syncthreads();
