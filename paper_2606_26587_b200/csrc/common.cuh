@@ -53,6 +53,19 @@ __device__ __forceinline__ uint32_t cvt_e2m1x2(float lo, float hi) {
       : "=r"(r) : "f"(hi), "f"(lo));
   return r;
 }
+// eight fp32 -> one word of eight E2M1 codes (element 0 in the low nibble), RNE, saturating
+__device__ __forceinline__ uint32_t cvt_e2m1x8(float v0, float v1, float v2, float v3, float v4, float v5, float v6,
+                                               float v7) {
+  uint32_t r;
+  asm("{ .reg .b8 t0, t1, t2, t3;\n\t"
+      "cvt.rn.satfinite.e2m1x2.f32 t0, %2, %1;\n\t"
+      "cvt.rn.satfinite.e2m1x2.f32 t1, %4, %3;\n\t"
+      "cvt.rn.satfinite.e2m1x2.f32 t2, %6, %5;\n\t"
+      "cvt.rn.satfinite.e2m1x2.f32 t3, %8, %7;\n\t"
+      "mov.b32 %0, {t0, t1, t2, t3}; }"
+      : "=r"(r) : "f"(v0), "f"(v1), "f"(v2), "f"(v3), "f"(v4), "f"(v5), "f"(v6), "f"(v7));
+  return r;
+}
 // one byte of two E2M1 codes -> two fp32 values
 __device__ __forceinline__ void e2m1x2_to_f32(uint32_t byte, float& lo, float& hi) {
   uint32_t h2;

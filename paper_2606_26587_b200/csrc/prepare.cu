@@ -156,20 +156,26 @@ __device__ __forceinline__ void quantize_block_e2m1(const PrepParams& p, int64_t
   uint32_t sp_word[2] = {0u, 0u};
 #pragma unroll
   for (int c = 0; c < 4; ++c) {
-    uint32_t bytes = 0;  // byte q = the two codes of pair q
+    float xs[8];
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+      xs[2 * q] = bf16lo_to_f32(X[4 * c + q]);
+      xs[2 * q + 1] = bf16hi_to_f32(X[4 * c + q]);
+    }
+    // all four pairs of the chunk in one word: byte q = the two codes of pair q
+    const uint32_t bytes = cvt_e2m1x8(__fmul_rn(xs[0], bs.inv), __fmul_rn(xs[1], bs.inv), __fmul_rn(xs[2], bs.inv),
+                                      __fmul_rn(xs[3], bs.inv), __fmul_rn(xs[4], bs.inv), __fmul_rn(xs[5], bs.inv),
+                                      __fmul_rn(xs[6], bs.inv), __fmul_rn(xs[7], bs.inv));
     const uint32_t keep = (1u << i0[c]) | (1u << i1[c]);
 #pragma unroll
     for (int q = 0; q < 4; ++q) {
-      const float xl = bf16lo_to_f32(X[4 * c + q]), xh = bf16hi_to_f32(X[4 * c + q]);
-      const uint32_t b = cvt_e2m1x2(__fmul_rn(xl, bs.inv), __fmul_rn(xh, bs.inv));
-      bytes |= b << (8 * q);
       // ---- O5 dequantise and residual; a dropped pair keeps R = X bit for bit
       float dl, dh;
-      e2m1x2_to_f32(b, dl, dh);
-      float rl = xl, rh = xh;
+      e2m1x2_to_f32((bytes >> (8 * q)) & 0xFFu, dl, dh);
+      float rl = xs[2 * q], rh = xs[2 * q + 1];
       if (keep & (1u << q)) {
-        rl = __fsub_rn(xl, __fmul_rn(dl, bs.s_eff));
-        rh = __fsub_rn(xh, __fmul_rn(dh, bs.s_eff));
+        rl = __fsub_rn(rl, __fmul_rn(dl, bs.s_eff));
+        rh = __fsub_rn(rh, __fmul_rn(dh, bs.s_eff));
       }
       R[8 * c + 2 * q] = rl;
       R[8 * c + 2 * q + 1] = rh;
@@ -194,13 +200,11 @@ __device__ __forceinline__ void quantize_block_e2m1(const PrepParams& p, int64_t
     dn_sf[g] = ds.code;
 #pragma unroll
     for (int w = 0; w < GD / 8; ++w) {
-      uint32_t word = 0;
-#pragma unroll
-      for (int j = 0; j < 4; ++j) {
-        const int e = g * GD + w * 8 + 2 * j;
-        word |= cvt_e2m1x2(__fmul_rn(R[e], ds.inv), __fmul_rn(R[e + 1], ds.inv)) << (8 * j);
-      }
-      dn_word[g * (GD / 8) + w] = word;
+      const int e = g * GD + w * 8;
+      dn_word[g * (GD / 8) + w] =
+          cvt_e2m1x8(__fmul_rn(R[e], ds.inv), __fmul_rn(R[e + 1], ds.inv), __fmul_rn(R[e + 2], ds.inv),
+                     __fmul_rn(R[e + 3], ds.inv), __fmul_rn(R[e + 4], ds.inv), __fmul_rn(R[e + 5], ds.inv),
+                     __fmul_rn(R[e + 6], ds.inv), __fmul_rn(R[e + 7], ds.inv));
     }
   }
 
