@@ -105,8 +105,14 @@ struct Unit { int m_blk, n_blk, expert, rows_valid, kb0, kb1; };
 
 __device__ __forceinline__ Unit decode_unit(const KParams& p, const GroupInfo& g, int tile, int rank, int splits) {
   Unit u;
-  u.m_blk = tile % p.m_blocks;                     // m fastest: concurrent CTAs share W tiles in L2
-  u.n_blk = tile / p.m_blocks;
+  if (g.E > 0) {                                   // experts: n fastest, so concurrent CTAs share one expert's
+    const int n_tiles = p.total_tiles / p.m_blocks;  // A block and weights instead of streaming 50 experts at once
+    u.n_blk = tile % n_tiles;
+    u.m_blk = tile / n_tiles;
+  } else {
+    u.m_blk = tile % p.m_blocks;                   // m fastest: concurrent CTAs share W tiles in L2
+    u.n_blk = tile / p.m_blocks;
+  }
   u.expert = 0;
   if (g.E > 0) {
     int lo = 0, hi = g.E - 1;                      // last expert whose first block is <= m_blk (binary search)
