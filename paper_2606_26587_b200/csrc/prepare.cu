@@ -672,7 +672,11 @@ __global__ void __launch_bounds__(MAXT, MINB) sharq_prepare_row_kernel(const Pre
     if (threadIdx.x == 0) p.row_scale[row] = ts;
 
     // ---- O3-O7 mask, backbone, residual, stores
-    if (act) quantize_block_e2m1<FMT>(p, row, k0, X, ts, inv_ts);
+    if constexpr (FMT == SHARQ_HIF4) {
+      quantize_block_hif4(p, row, k0, X, lane, act);     // two lanes share a 64-element unit: all lanes take part
+    } else {
+      if (act) quantize_block_e2m1<FMT>(p, row, k0, X, ts, inv_ts);
+    }
   }
 }
 
@@ -749,10 +753,11 @@ cudaError_t launch_prepare(const sharq_config* cfg, const void* x, int64_t T, in
   p.dn_codes = (uint8_t*)dn_codes; p.dn_sf = (uint8_t*)dn_sf; p.row_scale = row_scale;
   p.eps = cfg->eps; p.tiled = (cfg->layout == SHARQ_LAYOUT_TILED);
   p.row_bytes = (uint32_t)(K * 2);
-  if (cfg->fmt != SHARQ_HIF4 && K <= 1024 * kRowMaxWarps && !getenv("SHARQ_DEBUG_OLD_PREPARE")) {
+  if (K <= 1024 * kRowMaxWarps && !getenv("SHARQ_DEBUG_OLD_PREPARE")) {
     p.nbuf = 0;
-    return cfg->fmt == SHARQ_NVFP4 ? launch_row_kernel<SHARQ_NVFP4>(cfg->norm, p, num_sms, st)
-                                   : launch_row_kernel<SHARQ_MXFP4>(cfg->norm, p, num_sms, st);
+    if (cfg->fmt == SHARQ_NVFP4) return launch_row_kernel<SHARQ_NVFP4>(cfg->norm, p, num_sms, st);
+    if (cfg->fmt == SHARQ_MXFP4) return launch_row_kernel<SHARQ_MXFP4>(cfg->norm, p, num_sms, st);
+    return launch_row_kernel<SHARQ_HIF4>(cfg->norm, p, num_sms, st);
   }
   // warps per CTA: as many double-buffered rows as fit in ~200 KB, else single-buffered
   const size_t budget = 200 * 1024;
