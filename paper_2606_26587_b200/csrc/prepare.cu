@@ -130,30 +130,52 @@ __device__ __forceinline__ BlockScale block_scale(float amax, float ts, float in
   return r;
 }
 
-// One lane, 32 contiguous elements X[16] (packed bf16 pairs): mask, backbone, residual, stores.
-template <int FMT>
-__device__ __forceinline__ void quantize_block_e2m1(const PrepParams& p, int64_t row, uint32_t k0,
-                                                    const uint32_t (&X)[16], float ts, float inv_ts) {
-  // ---- O3 pairwise 4:8 mask: per chunk of 8, keep the two pairs with the largest max(|a|,|b|)
-  uint32_t i0[4], i1[4], amax_bits = 0;
+__device__ __forceinline__ uint32_t mullo_u32(uint32_t x, uint32_t y) {   // x * y on the FMA pipe (no shift)
+  uint32_t r;
+  asm("mul.lo.u32 %0, %1, %2;" : "=r"(r) : "r"(x), "r"(y));
+  return r;
+}
+
+// O3 for one lane's 32 elements: what the later steps need from the mask, small enough to stay in registers
+// across the row-scale reduction.  sel[w] is the byte-permute selector that compresses chunks 2w and 2w+1
+// (nibbles: i0, i1 of chunk 2w, then 4 + i0, 4 + i1 of chunk 2w+1); keep bit 4c+q = pair q of chunk c
+// survives; amax_bits = the largest bf16 magnitude of the lane's block (the best pair of a chunk is always
+// kept, so this is both the backbone group amax and the lane's share of the row amax).
+struct MaskSel { uint32_t sel[2]; uint32_t keep; uint32_t meta16; uint32_t amax_bits; };
+
+__device__ __forceinline__ void mask_block_e2m1(const uint32_t (&X)[16], MaskSel& ms) {
+  ms.sel[0] = ms.sel[1] = 0u;
+  ms.keep = 0u; ms.meta16 = 0u; ms.amax_bits = 0u;
 #pragma unroll
   for (int c = 0; c < 4; ++c) {
     uint32_t key[4];
 #pragma unroll
     for (int q = 0; q < 4; ++q) {
-      const uint32_t a = X[4 * c + q] & 0x7FFF7FFFu;
-      const uint32_t s = max(a & 0xFFFFu, mulhi_u32(a, 65536u));        // a >> 16 on the FMA pipe
-      key[q] = s * 4u + (3u - q);
+      // the sign bits fall off the top: the upper 15 bits of x << 17 / x << 1 are |lo| / |hi|; their
+      // unsigned maximum has max(|lo|, |hi|) in its upper 15 bits.  Shifts as multiplies: FMA pipe.
+      const uint32_t m = max(mullo_u32(X[4 * c + q], 131072u), mullo_u32(X[4 * c + q], 2u));
+      key[q] = mullo_u32(mulhi_u32(m, 32768u), 4u) + (3u - q);
     }
-    uint32_t best;
-    top2of4(key[0], key[1], key[2], key[3], i0[c], i1[c], best);
-    amax_bits = max(amax_bits, best >> 2);
+    uint32_t i0, i1, best;
+    top2of4(key[0], key[1], key[2], key[3], i0, i1, best);
+    ms.amax_bits = max(ms.amax_bits, best >> 2);
+    ms.keep |= ((1u << i0) | (1u << i1)) << (4 * c);
+    ms.meta16 |= (i0 | (i1 << 2)) << (4 * c);
+    const uint32_t two = (c & 1) ? (i0 | (i1 << 4)) + 0x44u : (i0 | (i1 << 4));
+    ms.sel[c >> 1] |= two << (8 * (c & 1));
   }
+}
+
+// One lane, 32 contiguous elements X[16] (packed bf16 pairs): backbone, residual, stores (O4-O7).
+template <int FMT>
+__device__ __forceinline__ void quantize_tail_e2m1(const PrepParams& p, int64_t row, uint32_t k0,
+                                                   const uint32_t (&X)[16], const MaskSel& ms, float ts,
+                                                   float inv_ts) {
   // ---- O4 backbone scale over the 16 survivors of this 32-group
-  const BlockScale bs = block_scale<FMT>(__uint_as_float(amax_bits << 16), ts, inv_ts);
+  const BlockScale bs = block_scale<FMT>(__uint_as_float(ms.amax_bits << 16), ts, inv_ts);
 
   float R[32];
-  uint32_t sp_word[2] = {0u, 0u};
+  uint32_t bytes[4];
 #pragma unroll
   for (int c = 0; c < 4; ++c) {
     float xs[8];
@@ -163,29 +185,28 @@ __device__ __forceinline__ void quantize_block_e2m1(const PrepParams& p, int64_t
       xs[2 * q + 1] = bf16hi_to_f32(X[4 * c + q]);
     }
     // all four pairs of the chunk in one word: byte q = the two codes of pair q
-    const uint32_t bytes = cvt_e2m1x8(__fmul_rn(xs[0], bs.inv), __fmul_rn(xs[1], bs.inv), __fmul_rn(xs[2], bs.inv),
-                                      __fmul_rn(xs[3], bs.inv), __fmul_rn(xs[4], bs.inv), __fmul_rn(xs[5], bs.inv),
-                                      __fmul_rn(xs[6], bs.inv), __fmul_rn(xs[7], bs.inv));
-    const uint32_t keep = (1u << i0[c]) | (1u << i1[c]);
+    bytes[c] = cvt_e2m1x8(__fmul_rn(xs[0], bs.inv), __fmul_rn(xs[1], bs.inv), __fmul_rn(xs[2], bs.inv),
+                          __fmul_rn(xs[3], bs.inv), __fmul_rn(xs[4], bs.inv), __fmul_rn(xs[5], bs.inv),
+                          __fmul_rn(xs[6], bs.inv), __fmul_rn(xs[7], bs.inv));
 #pragma unroll
     for (int q = 0; q < 4; ++q) {
       // ---- O5 dequantise and residual; a dropped pair keeps R = X bit for bit
       float dl, dh;
-      e2m1x2_to_f32((bytes >> (8 * q)) & 0xFFu, dl, dh);
+      e2m1x2_to_f32((bytes[c] >> (8 * q)) & 0xFFu, dl, dh);
       float rl = xs[2 * q], rh = xs[2 * q + 1];
-      if (keep & (1u << q)) {
+      if (ms.keep & (1u << (4 * c + q))) {
         rl = __fsub_rn(rl, __fmul_rn(dl, bs.s_eff));
         rh = __fsub_rn(rh, __fmul_rn(dh, bs.s_eff));
       }
       R[8 * c + 2 * q] = rl;
       R[8 * c + 2 * q + 1] = rh;
     }
-    // compress: survivors in ascending k, byte 2c = pair i0, byte 2c+1 = pair i1
-    const uint32_t two = __byte_perm(bytes, 0u, i0[c] | (i1[c] << 4) | 0x4400u);
-    sp_word[c >> 1] |= two << (16 * (c & 1));
   }
-  const uint32_t meta16 = (i0[0] | (i1[0] << 2)) | ((i0[1] | (i1[1] << 2)) << 4) | ((i0[2] | (i1[2] << 2)) << 8) |
-                          ((i0[3] | (i1[3] << 2)) << 12);
+  // compress: survivors in ascending k; one byte permute per two chunks
+  uint32_t sp_word[2];
+  sp_word[0] = __byte_perm(bytes[0], bytes[1], ms.sel[0]);
+  sp_word[1] = __byte_perm(bytes[2], bytes[3], ms.sel[1]);
+  const uint32_t meta16 = ms.meta16;
 
   // ---- O6 residual: NVFP4 two groups of 16, MXFP4 one group of 32
   uint32_t dn_word[4];
@@ -230,6 +251,14 @@ __device__ __forceinline__ void quantize_block_e2m1(const PrepParams& p, int64_t
     else
       p.dn_sf[row * (K >> 5) + g32] = (uint8_t)dn_sf[0];
   }
+}
+
+template <int FMT>
+__device__ __forceinline__ void quantize_block_e2m1(const PrepParams& p, int64_t row, uint32_t k0,
+                                                    const uint32_t (&X)[16], float ts, float inv_ts) {
+  MaskSel ms;
+  mask_block_e2m1(X, ms);
+  quantize_tail_e2m1<FMT>(p, row, k0, X, ms, ts, inv_ts);
 }
 
 // ---- HiF4: Algorithm 1 on a 64-element unit shared by two lanes (32 elements each) -------
@@ -653,12 +682,14 @@ __global__ void __launch_bounds__(MAXT, MINB) sharq_prepare_row_kernel(const Pre
 
     // ---- O2 per-row tensor scale
     float ts = 1.0f, inv_ts = 1.0f;
+    // the mask needs no scale: it runs first and its best pair scores give the lane's share of the row amax
+    MaskSel ms;
+    ms.amax_bits = 0u;
+    if constexpr (FMT != SHARQ_HIF4) {
+      if (act) mask_block_e2m1(X, ms);
+    }
     if (need_rowmax) {
-      uint32_t amax2 = 0;                        // both bf16 halves at once (packed unsigned 16-bit max)
-#pragma unroll
-      for (int i = 0; i < 16; ++i) amax2 = __vmaxu2(amax2, X[i] & 0x7FFF7FFFu);
-      uint32_t amax = max(amax2 & 0xFFFFu, amax2 >> 16);
-      amax = warp_max_u32(amax);
+      uint32_t amax = warp_max_u32(ms.amax_bits);
       if (lane == 0) sh.amax[amax_slot * 32 + warp] = amax;
       __syncthreads();
       amax = warp_max_u32(lane < nwarps ? sh.amax[amax_slot * 32 + lane] : 0u);
@@ -675,7 +706,7 @@ __global__ void __launch_bounds__(MAXT, MINB) sharq_prepare_row_kernel(const Pre
     if constexpr (FMT == SHARQ_HIF4) {
       quantize_block_hif4(p, row, k0, X, lane, act);     // two lanes share a 64-element unit: all lanes take part
     } else {
-      if (act) quantize_block_e2m1<FMT>(p, row, k0, X, ts, inv_ts);
+      if (act) quantize_tail_e2m1<FMT>(p, row, k0, X, ms, ts, inv_ts);
     }
   }
 }
