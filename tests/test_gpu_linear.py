@@ -199,3 +199,46 @@ def test_moe_config5_size_sampled(sq):
         got = Y[pad_off[e]: pad_off[e] + counts[e]]
         den = np.maximum(np.abs(y64), 1e-2 * np.sqrt((y64 ** 2).mean()))
         assert (np.abs(got - y64) / den).max() <= TOL, f"expert {e}"
+
+
+def _sampled_check(sq, fmt, norm, T, K, D, config, mult, n_rows, n_cols, seed_extra):
+    """Full-size launch, oracle on a seeded sample: prepare and linear are independent per activation row
+     and per weight row (Eq. 9), except for the NVFP4 weight tensor scale max|W| / 2688,
+    so the sampled weight rows always include the row that holds max|W|."""
+    x, g, w = si.activations(T, K, config=config, outlier_mult=mult, extra=seed_extra), si.gamma(K, config), \
+        si.weight(D, K, config, extra=seed_extra + 1)
+    cfg = sq.make_config(fmt, norm, 1e-6, sq.LAYOUT_TILED)
+    wq = sq.quantize_weight(cfg, to_dev(w))
+    act = sq.prepare(cfg, to_dev(x), to_dev(g) if norm else None)
+    y32 = sq.linear(cfg, act, wq, out_dtype="fp32")
+    y16 = sq.linear(cfg, act, wq, out_dtype="bf16")
+    torch.cuda.synchronize()
+    rng = np.random.Generator(np.random.Philox(si.seed_for(config, 1000 + seed_extra)))
+    rows = np.unique(np.concatenate([rng.choice(T, size=min(n_rows, T), replace=False),
+                                     [0, min(127, T - 1), min(128, T - 1), T - 1]]))
+    w_mag = w & np.uint16(0x7FFF)                                  # bf16 magnitudes order like integers
+    top_row = int(np.unravel_index(int(w_mag.argmax()), w_mag.shape)[0])
+    cols = np.unique(np.concatenate([rng.choice(D, size=n_cols, replace=False),
+                                     [0, 127, 128, 191, 192, 255, 256, D - 1, top_row]]))
+    p = so.prepare(x[rows], fmt=fmt, norm=norm, gamma_u16=g)
+    q = so.quantize_weight(w[cols], fmt=fmt)
+    y64 = so.linear(p, q)
+    got = y32.cpu().numpy()[np.ix_(rows, cols)]
+    err = rel_err(got, y64)
+    assert err.max() <= TOL, f"max rel err {err.max():.3e}"
+    assert torch.equal(y16, y32.to(torch.bfloat16))
+
+
+@pytest.mark.parametrize("T,K,D", [(256, 4096, 28672), (128, 14336, 4096), (256, 14336, 4096), (128, 4096, 6144)])
+def test_decode_full_size_sampled(sq, T, K, D):
+    """BASELINE.json configs[1] at its two largest token counts, in the launch configurations bench.py
+    times there: CTA-pair tiles (T = 256), 128-row split-K clusters and the persistent 128-wide kernel."""
+    _sampled_check(sq, 0, 1 if K == 4096 else 0, T, K, D, config=2, mult=50.0, n_rows=24, n_cols=200,
+                   seed_extra=T + D)
+
+
+@pytest.mark.parametrize("fmt", [0, 1, 2])
+def test_qwen_config4_full_size_sampled(sq, fmt):
+    """BASELINE.json configs[3]: Qwen2.5-7B down projection 18944 -> 3584 at T = 4096 in all three formats
+    (the longest K of the five configs: 74 k-blocks, ragged against every pipeline depth)."""
+    _sampled_check(sq, fmt, 0, 4096, 18944, 3584, config=4, mult=50.0, n_rows=16, n_cols=120, seed_extra=fmt)
