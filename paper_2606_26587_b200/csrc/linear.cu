@@ -380,17 +380,23 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
       tc::mbar_wait(tmem_full_bar(0), 0);
       tc::tc_fence_after();
 #pragma unroll 1
-      for (int j = 0; j < BN / 16; ++j) {
-        uint32_t v[16];
-        tc::tmem_ld16(lane_addr + j * 16, v);
+      for (int jj = 0; jj < BN / 32; ++jj) {             // two 16-column slices per tensor-memory load
+        uint32_t v[32];
+        tc::tmem_ld32(lane_addr + jj * 32, v);
         tc::tmem_ld_wait();
         if (row_ok) {
-          const uint32_t local = recv_base + (uint32_t)(((rank * slots + j / splits) * AR + r_local) * 64);
-          const uint32_t remote = tc::map_to_cta(local, (uint32_t)(j % splits));
+          const uint32_t sw = ((uint32_t)r_local >> 1) & 3u;   // rows are 64 B apart: rotate the 16-byte chunks
 #pragma unroll
-          for (int i = 0; i < 4; ++i)
-            tc::st_cluster_v4(remote + 16 * i, __uint_as_float(v[4 * i]), __uint_as_float(v[4 * i + 1]),
-                              __uint_as_float(v[4 * i + 2]), __uint_as_float(v[4 * i + 3]));
+          for (int h = 0; h < 2; ++h) {
+            const int j = 2 * jj + h;
+            const uint32_t local = recv_base + (uint32_t)(((rank * slots + j / splits) * AR + r_local) * 64);
+            const uint32_t remote = tc::map_to_cta(local, (uint32_t)(j % splits));
+#pragma unroll
+            for (int i = 0; i < 4; ++i)
+              tc::st_cluster_v4(remote + 16 * ((uint32_t)i ^ sw), __uint_as_float(v[16 * h + 4 * i]),
+                                __uint_as_float(v[16 * h + 4 * i + 1]), __uint_as_float(v[16 * h + 4 * i + 2]),
+                                __uint_as_float(v[16 * h + 4 * i + 3]));
+          }
         }
       }
       tc::tc_fence_before();
@@ -416,7 +422,7 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
             const uint32_t a = recv_base + (uint32_t)(((src * slots + slot) * AR + r_local) * 64);
 #pragma unroll
             for (int i = 0; i < 4; ++i) {
-              const float4 t = tc::ld_shared_v4(a + 16 * i);
+              const float4 t = tc::ld_shared_v4(a + 16 * ((uint32_t)i ^ (((uint32_t)r_local >> 1) & 3u)));
               f[4 * i] = __fadd_rn(f[4 * i], t.x); f[4 * i + 1] = __fadd_rn(f[4 * i + 1], t.y);
               f[4 * i + 2] = __fadd_rn(f[4 * i + 2], t.z); f[4 * i + 3] = __fadd_rn(f[4 * i + 3], t.w);
             }
