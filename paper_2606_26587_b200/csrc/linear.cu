@@ -743,7 +743,9 @@ template <int BN, int FMT, int AR>
 sharq_status launch_1cta(const LinearArgs& a, const KParams& p, const GroupInfo& g, const CUtensorMap& tm_sp,
                          const CUtensorMap& tm_dn, const CUtensorMap& tm_w, int64_t tiles, int num_sms,
                          cudaStream_t st) {
-  const int splits = choose_splits<BN, FMT, AR>(tiles, (int)(a.K / BK), num_sms);
+  constexpr bool kSplitFits = !(BN == 256 && AR == 128);   // no room for the exchange buffers; never needed there
+  int splits = 1;
+  if constexpr (kSplitFits) splits = choose_splits<BN, FMT, AR>(tiles, (int)(a.K / BK), num_sms);
   cudaLaunchConfig_t lc{};
   cudaLaunchAttribute attr[2];
   attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
@@ -752,7 +754,7 @@ sharq_status launch_1cta(const LinearArgs& a, const KParams& p, const GroupInfo&
   lc.numAttrs = 1;
   lc.blockDim = dim3(kThreads);
   lc.stream = st;
-  if (splits > 1) {
+  if constexpr (kSplitFits) if (splits > 1) {
     using S = Stage<BN, FMT, true, AR>;
     auto kfn = sharq_linear_kernel<BN, FMT, true, AR>;
     if (cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, S::SMEM) != cudaSuccess)
@@ -858,8 +860,7 @@ sharq_status launch_tiles(const LinearArgs& a, const GroupInfo& g, int64_t rows_
   }
   if (a_rows <= 16) return launch_1cta<BN, FMT, 16>(a, p, g, tm_sp, tm_dn, tm_w, tiles, num_sms, st);
   if (a_rows <= 64) return launch_1cta<BN, FMT, 64>(a, p, g, tm_sp, tm_dn, tm_w, tiles, num_sms, st);
-  if constexpr (BN == 128) return launch_1cta<BN, FMT, 128>(a, p, g, tm_sp, tm_dn, tm_w, tiles, num_sms, st);
-  return SHARQ_EINVAL;                                   // 256-wide tiles are for T <= 64 only
+  return launch_1cta<BN, FMT, 128>(a, p, g, tm_sp, tm_dn, tm_w, tiles, num_sms, st);
 }
 
 }  // namespace
@@ -894,11 +895,12 @@ sharq_status launch_linear(const sharq_config* cfg, const LinearArgs& a, int32_t
     if (m_blocks == 0) return SHARQ_OK;
   }
   if (m_blocks * (a.D / 128) > (int64_t)1 << 30) return SHARQ_ESHAPE;
-  // T <= 64: 128 x 256 tiles halve the per-column cost of the scale-factor copies and of the M = 128 MMA
+  // T <= 128 (one m-block): 128 x 256 tiles halve the per-column cost of the scale-factor copies and of the M = 128 MMA
   // (the decode launches are bound by tensor-pipe issue per k-block, not by HBM)
   // ... and only pays when the 128-wide tiles would need a second round on the SMs (measured: with fewer
   // tiles than SMs the narrower tiles + deeper K-split win)
-  if (E == 0 && a.T <= 64 && a.D % 256 == 0 && a.D / 128 > num_sms && !getenv("SHARQ_DEBUG_NO_WIDE")) {
+  const char* wide_t = getenv("SHARQ_DEBUG_WIDE_T");
+  if (E == 0 && a.T <= (wide_t ? atoi(wide_t) : 128) && a.D % 256 == 0 && a.D / 128 > num_sms && !getenv("SHARQ_DEBUG_NO_WIDE")) {
     if (cfg->fmt == SHARQ_NVFP4) return launch_tiles<256, SHARQ_NVFP4>(a, g, rows_total, m_blocks, E, num_sms, st);
     return launch_tiles<256, SHARQ_MXFP4>(a, g, rows_total, m_blocks, E, num_sms, st);
   }

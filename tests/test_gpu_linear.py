@@ -229,10 +229,12 @@ def _sampled_check(sq, fmt, norm, T, K, D, config, mult, n_rows, n_cols, seed_ex
     assert torch.equal(y16, y32.to(torch.bfloat16))
 
 
-@pytest.mark.parametrize("T,K,D", [(256, 4096, 28672), (128, 14336, 4096), (256, 14336, 4096), (128, 4096, 6144)])
+@pytest.mark.parametrize("T,K,D", [(256, 4096, 28672), (128, 4096, 28672), (100, 4096, 28672), (128, 14336, 4096), (256, 14336, 4096),
+                                   (128, 4096, 6144)])
 def test_decode_full_size_sampled(sq, T, K, D):
     """BASELINE.json configs[1] at its two largest token counts, in the launch configurations bench.py
-    times there: CTA-pair tiles (T = 256), 128-row split-K clusters and the persistent 128-wide kernel."""
+    times there: CTA-pair tiles (T = 256), 128 x 256 tiles with full and ragged 128-row activation boxes,
+    128-row split-K clusters and the persistent 128-wide kernel."""
     _sampled_check(sq, 0, 1 if K == 4096 else 0, T, K, D, config=2, mult=50.0, n_rows=24, n_cols=200,
                    seed_extra=T + D)
 
