@@ -154,7 +154,10 @@ __device__ __forceinline__ void store_row(const KParams& p, int64_t row, int col
   }
 }
 
-template <int BN, int FMT, bool SPLIT, int AR>
+// MC = true (grouped GEMM): a cluster of two CTAs works on two neighbouring n-tiles of the same 128-row block in
+// lock step; each CTA fetches half of the shared activation operands and multicasts them to both (the many
+// short tiles of the expert GEMMs are bound by L2 -> SM traffic, 60 % of which is the activation side).
+template <int BN, int FMT, bool SPLIT, int AR, bool MC = false>
 __global__ void __launch_bounds__(kThreads, 1)
 sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_constant__ CUtensorMap tm_a_dn,
                     const __grid_constant__ CUtensorMap tm_w, const KParams p, const __grid_constant__ GroupInfo g) {
@@ -173,9 +176,11 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const bool do_sp = p.path != 2, do_dn = p.path != 1;
   // work distribution: SPLIT -> one tile per cluster, this CTA's k-slice; else persistent round-robin
-  const int rank = SPLIT ? (int)tc::cluster_ctarank() : 0;
+  static_assert(!(SPLIT && MC), "split-K clusters and multicast clusters are separate variants");
+  const int crank = (SPLIT || MC) ? (int)tc::cluster_ctarank() : 0;
+  const int rank = SPLIT ? crank : 0;                  // k-slice owner (split-K only)
   const int splits = SPLIT ? (int)tc::cluster_nctarank() : 1;
-  const int tile0 = SPLIT ? (int)tc::cluster_id_x() : (int)blockIdx.x;
+  const int tile0 = SPLIT ? (int)tc::cluster_id_x() : MC ? 2 * (int)tc::cluster_id_x() + crank : (int)blockIdx.x;
   const int tile_step = SPLIT ? p.total_tiles : (int)gridDim.x;
 
   if (warp == 0 && lane == 0) {
@@ -186,7 +191,7 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
   if (warp == 1 && lane == 0) {
     for (int s = 0; s < S::STAGES; ++s) {
       tc::mbar_init(full_bar(s), 1);
-      tc::mbar_init(empty_bar(s), 1);
+      tc::mbar_init(empty_bar(s), MC ? 2 : 1);      // MC: both CTAs of the cluster must have consumed the slot
     }
     for (int a = 0; a < 2; ++a) {
       tc::mbar_init(tmem_full_bar(a), 1);
@@ -196,7 +201,12 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
   }
   if (warp == 2) tc::tmem_alloc<kTmemCols>(tmem_ptr_smem);
   tc::tc_fence_before();
-  __syncthreads();
+  if constexpr (MC) {
+    __syncwarp();
+    tc::cluster_sync_all();                          // the peer's barriers exist before anything is sent to them
+  } else {
+    __syncthreads();
+  }
   tc::tc_fence_after();
   uint32_t tmem_base;
   asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_ptr_smem));
@@ -236,6 +246,19 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
         };
         // activation side: written by sharq_prepare, only after griddepcontrol.wait
         auto load_a = [&](int kb, uint32_t st, uint32_t fb) {
+          if constexpr (MC) {
+            // same 128-row block in both CTAs: CTA 0 fetches the dense side, CTA 1 the sparse side, for both
+            if (do_sp && crank == 1) {
+              if (lead) tc::tma_load_2d_mc(st + S::A_SP, &tm_a_sp, fb, kb * 64, u.m_blk * BM, 3, pol_act);
+              if (lead) tc::bulk_load_mc(st + S::META, meta + (size_t)kb * 2048, 2048, fb, 3, pol_act);
+              if (lead) tc::bulk_load_mc(st + S::SFA_SP, sfa_sp + (size_t)kb * 1024, 1024, fb, 3, pol_act);
+            }
+            if (do_dn && crank == 0) {
+              if (lead) tc::tma_load_2d_mc(st + S::A_DN, &tm_a_dn, fb, kb * 128, u.m_blk * BM, 3, pol_act);
+              if (lead) tc::bulk_load_mc(st + S::SFA_DN, sfa_dn + (size_t)kb * S::SF_DN_BYTES, S::SF_DN_BYTES, fb, 3, pol_act);
+            }
+            return;
+          }
           if (do_sp) {
             if (lead) tc::tma_load_2d(st + S::A_SP, &tm_a_sp, fb, kb * 64, u.m_blk * BM, pol_act);
             if (lead) tc::bulk_load(st + S::META, meta + (size_t)kb * 2048, 2048, fb, pol_act);
@@ -335,7 +358,11 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
               accumulate = 1;
             }
           }
-          if (lead) tc::tc_commit(empty_bar(s));                   // smem slot reusable once these MMAs have read it
+          if constexpr (MC) {
+            if (lead) tc::tc_commit_mc(empty_bar(s), 3);           // ... in BOTH CTAs: either may refill the other's slot
+          } else {
+            if (lead) tc::tc_commit(empty_bar(s));                 // smem slot reusable once these MMAs have read it
+          }
         }
         if (lead) tc::tc_commit(tmem_full_bar(as));                // accumulator complete
       }
@@ -431,6 +458,10 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
         }
       }
     }
+  }
+  if constexpr (MC) {
+    __syncwarp();
+    tc::cluster_sync_all();                              // the peer may still multicast into / signal this CTA
   }
   __syncthreads();
   if (warp == 2) {
@@ -778,6 +809,32 @@ sharq_status launch_1cta(const LinearArgs& a, const KParams& p, const GroupInfo&
   return cudaLaunchKernelEx(&lc, kfn, tm_sp, tm_dn, tm_w, p, g) == cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
 }
 
+// grouped GEMM: persistent clusters of two CTAs on neighbouring n-tiles, activation operands multicast
+template <int FMT>
+sharq_status launch_mc(const KParams& p, const GroupInfo& g, const CUtensorMap& tm_sp, const CUtensorMap& tm_dn,
+                       const CUtensorMap& tm_w, int64_t tiles, int num_sms, cudaStream_t st) {
+  using S = Stage<128, FMT, false, 128>;
+  auto kfn = sharq_linear_kernel<128, FMT, false, 128, true>;
+  if (cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, S::SMEM) != cudaSuccess)
+    return SHARQ_ECUDA;
+  const int64_t clusters = tiles / 2 < num_sms / 2 ? tiles / 2 : num_sms / 2;
+  cudaLaunchConfig_t lc{};
+  cudaLaunchAttribute attr[2];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  attr[1].id = cudaLaunchAttributeClusterDimension;
+  attr[1].val.clusterDim.x = 2;
+  attr[1].val.clusterDim.y = 1;
+  attr[1].val.clusterDim.z = 1;
+  lc.attrs = attr;
+  lc.numAttrs = 2;
+  lc.blockDim = dim3(kThreads);
+  lc.gridDim = dim3((unsigned)(2 * clusters));
+  lc.dynamicSmemBytes = S::SMEM;
+  lc.stream = st;
+  return cudaLaunchKernelEx(&lc, kfn, tm_sp, tm_dn, tm_w, p, g) == cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
+}
+
 // scale-factor / metadata array as a 2-D tensor of 1024-byte rows (256 x u32), boxes of `box_rows` rows
 bool make_map_rows1k(CUtensorMap* m, const void* base, uint64_t bytes, uint32_t box_rows) {
   EncodeTiledFn fn = encode_fn();
@@ -810,7 +867,8 @@ sharq_status launch_pair(const LinearArgs& a, const KParams& p, const CUtensorMa
   if (cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, P::SMEM) != cudaSuccess)
     return SHARQ_ECUDA;
   const int64_t pair_tiles = ((m_blocks + 1) / 2) * ((a.D + PBN - 1) / PBN);
-  const int64_t clusters = pair_tiles < num_sms / 2 ? pair_tiles : num_sms / 2;
+  int64_t clusters = pair_tiles < num_sms / 2 ? pair_tiles : num_sms / 2;
+  if (const char* dbg = getenv("SHARQ_DEBUG_PAIR_CLUSTERS")) clusters = atoi(dbg) < clusters ? atoi(dbg) : clusters;
   cudaLaunchConfig_t lp{};
   cudaLaunchAttribute at[2];
   at[0].id = cudaLaunchAttributeClusterDimension;
@@ -857,6 +915,11 @@ sharq_status launch_tiles(const LinearArgs& a, const GroupInfo& g, int64_t rows_
     if (const char* pbn = getenv("SHARQ_DEBUG_PAIR_BN")) width = (atoi(pbn) == 256 && a.D % 256 == 0) ? 256 : 192;
     if (width == 256) return launch_pair<FMT, 256>(a, p, tm_sp, tm_dn, m_blocks, num_sms, st);
     return launch_pair<FMT, 192>(a, p, tm_sp, tm_dn, m_blocks, num_sms, st);
+  }
+  if constexpr (BN == 128) {
+    // experts: n-tiles of one 128-row block are consecutive (decode_unit), so tiles 2j and 2j+1 share activations
+    if (E > 0 && (a.D / BN) % 2 == 0 && a_rows == (uint32_t)BM && !getenv("SHARQ_DEBUG_NO_MC"))
+      return launch_mc<FMT>(p, g, tm_sp, tm_dn, tm_w, tiles, num_sms, st);
   }
   if (a_rows <= 16) return launch_1cta<BN, FMT, 16>(a, p, g, tm_sp, tm_dn, tm_w, tiles, num_sms, st);
   if (a_rows <= 64) return launch_1cta<BN, FMT, 64>(a, p, g, tm_sp, tm_dn, tm_w, tiles, num_sms, st);

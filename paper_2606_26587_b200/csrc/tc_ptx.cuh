@@ -96,6 +96,25 @@ __device__ __forceinline__ void tmem_dealloc(uint32_t taddr) {       // whole wa
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
 // all previously issued tcgen05.mma / tcgen05.cp of this thread arrive on `bar` when complete
+// multicast variants (cta_group::1 kernels in a cluster): the bytes land at the same offset in every CTA of
+// `mask` and complete_tx is signalled on the barrier at the same offset in each of them
+__device__ __forceinline__ void tma_load_2d_mc(uint32_t dst, const void* tmap, uint32_t bar, int32_t c0, int32_t c1,
+                                               uint16_t mask, uint64_t policy) {
+  asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes.multicast::cluster"
+               ".L2::cache_hint [%0], [%1, {%3, %4}], [%2], %5, %6;"
+               ::"r"(dst), "l"(tmap), "r"(bar), "r"(c0), "r"(c1), "h"(mask), "l"(policy) : "memory");
+}
+__device__ __forceinline__ void bulk_load_mc(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar,
+                                             uint16_t mask, uint64_t policy) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.multicast::cluster.L2::cache_hint "
+               "[%0], [%1], %2, [%3], %4, %5;"
+               ::"r"(dst), "l"(src), "r"(bytes), "r"(bar), "h"(mask), "l"(policy) : "memory");
+}
+// commit whose arrival is delivered to the barrier at this offset in every CTA of `mask`
+__device__ __forceinline__ void tc_commit_mc(uint32_t bar, uint16_t mask) {
+  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;"
+               ::"r"(bar), "h"(mask) : "memory");
+}
 __device__ __forceinline__ void tc_commit(uint32_t bar) {
   asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
 }
