@@ -605,22 +605,18 @@ __global__ void __launch_bounds__(MAXT, MINB) sharq_prepare_row_kernel(const Pre
   const float static_ts = (FMT == SHARQ_NVFP4 && p.x_ts != nullptr) ? *p.x_ts : 0.0f;
   const bool need_rowmax = (FMT == SHARQ_NVFP4) && (p.x_ts == nullptr);
 
-  // gamma / beta of this lane's 32 columns stay in registers across rows
-  uint32_t G[16], Bt[16];
+  // gamma / beta of this lane's 32 columns: parked in shared memory as [4][threads] 16-byte words (conflict
+  // free), not in registers: at 64 registers / thread the 16-32 words would spill to local memory
+  uint4* g_sm = reinterpret_cast<uint4*>(row_smem + (size_t)nwarps * 1024 + 256 + 16);
+  uint4* b_sm = g_sm + 4 * blockDim.x;
   if (NORM != SHARQ_NORM_NONE && act) {
     const uint4* g4 = reinterpret_cast<const uint4*>(p.gamma + k0);
 #pragma unroll
-    for (int s = 0; s < 4; ++s) {
-      const uint4 g = __ldg(g4 + s);
-      G[4 * s] = g.x; G[4 * s + 1] = g.y; G[4 * s + 2] = g.z; G[4 * s + 3] = g.w;
-    }
+    for (int s = 0; s < 4; ++s) g_sm[s * blockDim.x + threadIdx.x] = __ldg(g4 + s);
     if (NORM == SHARQ_NORM_LAYER && p.beta) {
       const uint4* b4 = reinterpret_cast<const uint4*>(p.beta + k0);
 #pragma unroll
-      for (int s = 0; s < 4; ++s) {
-        const uint4 g = __ldg(b4 + s);
-        Bt[4 * s] = g.x; Bt[4 * s + 1] = g.y; Bt[4 * s + 2] = g.z; Bt[4 * s + 3] = g.w;
-      }
+      for (int s = 0; s < 4; ++s) b_sm[s * blockDim.x + threadIdx.x] = __ldg(b4 + s);
     }
   }
 
@@ -669,13 +665,24 @@ __global__ void __launch_bounds__(MAXT, MINB) sharq_prepare_row_kernel(const Pre
       const float rstd = __frcp_rn(__fsqrt_rn(__fadd_rn(__fdiv_rn(S, Kf), p.eps)));
       if (act) {
 #pragma unroll
-        for (int i = 0; i < 16; ++i) {
-          float lo = bf16lo_to_f32(X[i]), hi = bf16hi_to_f32(X[i]);
-          if (NORM == SHARQ_NORM_LAYER) { lo = __fsub_rn(lo, mu); hi = __fsub_rn(hi, mu); }
-          const uint32_t h = pack_bf16x2_rn(__fmul_rn(lo, rstd), __fmul_rn(hi, rstd));
-          uint32_t v = mul_bf16x2_rn(h, G[i]);
-          if (NORM == SHARQ_NORM_LAYER && p.beta) v = add_bf16x2_rn(v, Bt[i]);
-          X[i] = v;
+        for (int s4 = 0; s4 < 4; ++s4) {
+          const uint4 gq = g_sm[s4 * blockDim.x + threadIdx.x];
+          const uint32_t G[4] = {gq.x, gq.y, gq.z, gq.w};
+          uint32_t Bt[4] = {0u, 0u, 0u, 0u};
+          if (NORM == SHARQ_NORM_LAYER && p.beta) {
+            const uint4 bq = b_sm[s4 * blockDim.x + threadIdx.x];
+            Bt[0] = bq.x; Bt[1] = bq.y; Bt[2] = bq.z; Bt[3] = bq.w;
+          }
+#pragma unroll
+          for (int j = 0; j < 4; ++j) {
+            const int i = 4 * s4 + j;
+            float lo = bf16lo_to_f32(X[i]), hi = bf16hi_to_f32(X[i]);
+            if (NORM == SHARQ_NORM_LAYER) { lo = __fsub_rn(lo, mu); hi = __fsub_rn(hi, mu); }
+            const uint32_t h = pack_bf16x2_rn(__fmul_rn(lo, rstd), __fmul_rn(hi, rstd));
+            uint32_t v = mul_bf16x2_rn(h, G[j]);
+            if (NORM == SHARQ_NORM_LAYER && p.beta) v = add_bf16x2_rn(v, Bt[j]);
+            X[i] = v;
+          }
         }
       }
     }
@@ -727,9 +734,15 @@ static cudaError_t launch_row_kernel(int norm, const PrepParams& p, int num_sms,
   attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
   attr[0].val.programmaticStreamSerializationAllowed = 1;
   lc.gridDim = grid; lc.blockDim = block; lc.stream = st; lc.attrs = attr; lc.numAttrs = 1;
-  lc.dynamicSmemBytes = (size_t)warps * 1024 + 256 + 16;
+  lc.dynamicSmemBytes = (size_t)warps * 1024 + 256 + 16 + (norm != SHARQ_NORM_NONE ? (size_t)warps * 32 * 128 : 0);   // + gamma, beta
   cudaError_t err = cudaSuccess;
-#define SHARQ_ROW(N, MAXT, MINB) err = cudaLaunchKernelEx(&lc, sharq_prepare_row_kernel<FMT, N, MAXT, MINB>, p)
+#define SHARQ_ROW(N, MAXT, MINB)                                                                              \
+  do {                                                                                                        \
+    auto kfn = sharq_prepare_row_kernel<FMT, N, MAXT, MINB>;                                                  \
+    if (lc.dynamicSmemBytes > 48 * 1024)                                                                      \
+      err = cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)lc.dynamicSmemBytes); \
+    if (err == cudaSuccess) err = cudaLaunchKernelEx(&lc, kfn, p);                                            \
+  } while (0)
 #define SHARQ_ROW_N(MAXT, MINB)                                              \
   {                                                                          \
     if (norm == SHARQ_NORM_NONE) SHARQ_ROW(SHARQ_NORM_NONE, MAXT, MINB);     \
