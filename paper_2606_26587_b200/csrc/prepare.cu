@@ -725,7 +725,7 @@ static cudaError_t launch_row_kernel(int norm, const PrepParams& p, int num_sms,
   int per_sm = 2048 / (warps * 32);                       // thread limit; registers trim it further at launch
   if (const char* e = getenv("SHARQ_DEBUG_ROW_PER_SM")) per_sm = atoi(e);
   if (per_sm < 1) per_sm = 1;
-  if (per_sm > 8) per_sm = 8;
+  if (per_sm > 32) per_sm = 32;                           // grid = about twice the resident CTAs (finer tail); 32 one-warp CTAs for short rows
   int64_t ctas = (int64_t)num_sms * per_sm;
   if (ctas > p.T) ctas = p.T;
   const dim3 grid((unsigned)ctas);
