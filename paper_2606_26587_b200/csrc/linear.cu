@@ -780,7 +780,7 @@ sharq_status launch_1cta(const LinearArgs& a, const KParams& p, const GroupInfo&
   cudaLaunchConfig_t lc{};
   cudaLaunchAttribute attr[2];
   attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  attr[0].val.programmaticStreamSerializationAllowed = getenv("SHARQ_DEBUG_NO_PDL") ? 0 : 1;
   lc.attrs = attr;
   lc.numAttrs = 1;
   lc.blockDim = dim3(kThreads);
@@ -821,7 +821,7 @@ sharq_status launch_mc(const KParams& p, const GroupInfo& g, const CUtensorMap& 
   cudaLaunchConfig_t lc{};
   cudaLaunchAttribute attr[2];
   attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  attr[0].val.programmaticStreamSerializationAllowed = getenv("SHARQ_DEBUG_NO_PDL") ? 0 : 1;
   attr[1].id = cudaLaunchAttributeClusterDimension;
   attr[1].val.clusterDim.x = 2;
   attr[1].val.clusterDim.y = 1;
@@ -876,7 +876,7 @@ sharq_status launch_pair(const LinearArgs& a, const KParams& p, const CUtensorMa
   at[0].val.clusterDim.y = 1;
   at[0].val.clusterDim.z = 1;
   at[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-  at[1].val.programmaticStreamSerializationAllowed = 1;
+  at[1].val.programmaticStreamSerializationAllowed = getenv("SHARQ_DEBUG_NO_PDL") ? 0 : 1;
   lp.blockDim = dim3(kThreads);
   lp.gridDim = dim3((unsigned)(2 * clusters));
   lp.dynamicSmemBytes = P::SMEM;

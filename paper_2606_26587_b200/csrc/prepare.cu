@@ -732,7 +732,7 @@ static cudaError_t launch_row_kernel(int norm, const PrepParams& p, int num_sms,
   cudaLaunchConfig_t lc{};
   cudaLaunchAttribute attr[1];
   attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  attr[0].val.programmaticStreamSerializationAllowed = getenv("SHARQ_DEBUG_NO_PDL") ? 0 : 1;
   lc.gridDim = grid; lc.blockDim = block; lc.stream = st; lc.attrs = attr; lc.numAttrs = 1;
   lc.dynamicSmemBytes = (size_t)warps * 1024 + 256 + 16 + (norm != SHARQ_NORM_NONE ? (size_t)warps * 32 * 128 : 0);   // + gamma, beta
   cudaError_t err = cudaSuccess;
