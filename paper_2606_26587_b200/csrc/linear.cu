@@ -38,6 +38,13 @@ constexpr int kMaxExperts = 256;
 constexpr int BM = 128;          // rows of an output tile = TMEM lanes
 constexpr int BK = 256;          // logical k per pipeline stage
 constexpr int kThreads = 192;
+
+#ifdef SHARQ_DEBUG_TS                                    // experiments only: per-CTA phase timestamps (SM clocks)
+__device__ long long g_dbg_ts[1024 * 16];
+#define SHARQ_TS(i) do { if ((threadIdx.x & 31) == 0 && blockIdx.x < 1024) g_dbg_ts[blockIdx.x * 16 + (i)] = clock64(); } while (0)
+#else
+#define SHARQ_TS(i) do { } while (0)
+#endif
 constexpr int kTmemCols = 512;
 
 struct GroupInfo {
@@ -174,6 +181,7 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
   const uint32_t tmem_ptr_smem = bars + 8u * (2 * S::STAGES + 4);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  if (warp == 0) SHARQ_TS(0);
   const bool do_sp = p.path != 2, do_dn = p.path != 1;
   // work distribution: SPLIT -> one tile per cluster, this CTA's k-slice; else persistent round-robin
   static_assert(!(SPLIT && MC), "split-K clusters and multicast clusters are separate variants");
@@ -211,7 +219,9 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
   uint32_t tmem_base;
   asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_ptr_smem));
   tc::grid_launch_dependents();                          // the next kernel may start its own prologue
+  if (warp == 0) SHARQ_TS(1);
 
+  float split_scale = 0.0f;
   if (warp == 0) {
     // =========================== TMA producer ===============================================
     {
@@ -278,7 +288,9 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
             if (lead) tc::mbar_expect_tx(full_bar(i), tx);
             load_w(kb + i, smem_base + i * S::BYTES, full_bar(i));
           }
+          SHARQ_TS(2);
           tc::grid_dependency_wait();
+          SHARQ_TS(3);
           dep_synced = true;
           for (int i = 0; i < n_early; ++i) load_a(kb + i, smem_base + i * S::BYTES, full_bar(i));
           kb += n_early;
@@ -315,6 +327,8 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
           const int s = it % S::STAGES;
           const uint32_t ph = (it / S::STAGES) & 1;
           tc::mbar_wait(full_bar(s), ph);
+          if (it == 0) SHARQ_TS(4);
+          if (kb == u.kb1 - 1) SHARQ_TS(5);
           tc::tc_fence_after();
           const uint32_t st = smem_base + s * S::BYTES;
           if (do_sp) {
@@ -404,25 +418,39 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
       const Unit u = decode_unit(p, g, tile0, rank, splits);
       const bool row_ok = r_local < u.rows_valid;
       const int slots = (BN / 16 + splits - 1) / splits;
+      // the output scale of this thread's row, fetched while the main loop runs (used after the exchange)
+      if (row_ok) split_scale = __fmul_rn(p.row_scale[(int64_t)u.m_blk * BM + r_local], p.w_ts[u.expert]);
       tc::mbar_wait(tmem_full_bar(0), 0);
+      if (warp == 2) SHARQ_TS(6);
       tc::tc_fence_after();
 #pragma unroll 1
-      for (int jj = 0; jj < BN / 32; ++jj) {             // two 16-column slices per tensor-memory load
-        uint32_t v[32];
-        tc::tmem_ld32(lane_addr + jj * 32, v);
+      for (int j4 = 0; j4 < BN / 64; ++j4) {              // four 16-column slices (two tensor-memory loads) in flight
+        uint32_t v[64];
+        tc::tmem_ld32(lane_addr + j4 * 64, *reinterpret_cast<uint32_t(*)[32]>(&v[0]));
+        tc::tmem_ld32(lane_addr + j4 * 64 + 32, *reinterpret_cast<uint32_t(*)[32]>(&v[32]));
         tc::tmem_ld_wait();
         if (row_ok) {
-          const uint32_t sw = ((uint32_t)r_local >> 1) & 3u;   // rows are 64 B apart: rotate the 16-byte chunks
+          // exchange layout [src][slot][16-byte chunk][row]: the 32 lanes of one store are 512 contiguous
+          // bytes (full lines on the SM-to-SM network, no bank conflicts on either side)
 #pragma unroll
-          for (int h = 0; h < 2; ++h) {
-            const int j = 2 * jj + h;
-            const uint32_t local = recv_base + (uint32_t)(((rank * slots + j / splits) * AR + r_local) * 64);
-            const uint32_t remote = tc::map_to_cta(local, (uint32_t)(j % splits));
+          for (int h = 0; h < 4; ++h) {
+            const int j = 4 * j4 + h;
+            const uint32_t local = recv_base + (uint32_t)((rank * slots + j / splits) * AR * 64 + r_local * 16);
+            const int owner = j % splits;
+            if (owner == rank) {                         // this CTA's own slices never leave its shared memory
 #pragma unroll
-            for (int i = 0; i < 4; ++i)
-              tc::st_cluster_v4(remote + 16 * ((uint32_t)i ^ sw), __uint_as_float(v[16 * h + 4 * i]),
-                                __uint_as_float(v[16 * h + 4 * i + 1]), __uint_as_float(v[16 * h + 4 * i + 2]),
-                                __uint_as_float(v[16 * h + 4 * i + 3]));
+              for (int i = 0; i < 4; ++i)
+                tc::st_shared_v4(local + (uint32_t)(i * AR * 16), __uint_as_float(v[16 * h + 4 * i]),
+                                 __uint_as_float(v[16 * h + 4 * i + 1]), __uint_as_float(v[16 * h + 4 * i + 2]),
+                                 __uint_as_float(v[16 * h + 4 * i + 3]));
+            } else {
+              const uint32_t remote = tc::map_to_cta(local, (uint32_t)owner);
+#pragma unroll
+              for (int i = 0; i < 4; ++i)
+                tc::st_cluster_v4(remote + (uint32_t)(i * AR * 16), __uint_as_float(v[16 * h + 4 * i]),
+                                  __uint_as_float(v[16 * h + 4 * i + 1]), __uint_as_float(v[16 * h + 4 * i + 2]),
+                                  __uint_as_float(v[16 * h + 4 * i + 3]));
+            }
           }
         }
       }
@@ -431,13 +459,15 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
   }
   if constexpr (SPLIT) {
     __syncwarp();
+    if (warp == 2) SHARQ_TS(7);
     tc::cluster_sync_all();                              // partial slices have landed in their owners
+    if (warp == 2) SHARQ_TS(8);
     if (warp >= 2) {
       const Unit u = decode_unit(p, g, tile0, rank, splits);
       const int r_local = (warp & 3) * 32 + lane;
       if (r_local < u.rows_valid) {
         const int64_t row = (int64_t)u.m_blk * BM + r_local;
-        const float scale = __fmul_rn(p.row_scale[row], p.w_ts[u.expert]);
+        const float scale = split_scale;
         const int slots = (BN / 16 + splits - 1) / splits;
         for (int slot = 0; slot < slots; ++slot) {
           const int j = slot * splits + rank;            // the slices this CTA owns
@@ -445,13 +475,25 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
           float f[16];
 #pragma unroll
           for (int i = 0; i < 16; ++i) f[i] = 0.0f;
-          for (int src = 0; src < splits; ++src) {       // fixed order: deterministic sum
-            const uint32_t a = recv_base + (uint32_t)(((src * slots + slot) * AR + r_local) * 64);
+          for (int s0 = 0; s0 < splits; s0 += 4) {       // fixed order: deterministic sum; four sources' loads in flight
+            float4 t[4][4];
 #pragma unroll
-            for (int i = 0; i < 4; ++i) {
-              const float4 t = tc::ld_shared_v4(a + 16 * ((uint32_t)i ^ (((uint32_t)r_local >> 1) & 3u)));
-              f[4 * i] = __fadd_rn(f[4 * i], t.x); f[4 * i + 1] = __fadd_rn(f[4 * i + 1], t.y);
-              f[4 * i + 2] = __fadd_rn(f[4 * i + 2], t.z); f[4 * i + 3] = __fadd_rn(f[4 * i + 3], t.w);
+            for (int q = 0; q < 4; ++q) {
+              if (s0 + q < splits) {
+                const uint32_t a = recv_base + (uint32_t)(((s0 + q) * slots + slot) * AR * 64 + r_local * 16);
+#pragma unroll
+                for (int i = 0; i < 4; ++i) t[q][i] = tc::ld_shared_v4(a + (uint32_t)(i * AR * 16));
+              }
+            }
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+              if (s0 + q < splits) {
+#pragma unroll
+                for (int i = 0; i < 4; ++i) {
+                  f[4 * i] = __fadd_rn(f[4 * i], t[q][i].x); f[4 * i + 1] = __fadd_rn(f[4 * i + 1], t[q][i].y);
+                  f[4 * i + 2] = __fadd_rn(f[4 * i + 2], t[q][i].z); f[4 * i + 3] = __fadd_rn(f[4 * i + 3], t[q][i].w);
+                }
+              }
             }
           }
           store_row<16>(p, row, u.n_blk * BN + j * 16, scale, f);
@@ -463,6 +505,7 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
     __syncwarp();
     tc::cluster_sync_all();                              // the peer may still multicast into / signal this CTA
   }
+  if (warp == 2) SHARQ_TS(9);
   __syncthreads();
   if (warp == 2) {
     tc::tc_fence_after();
@@ -971,4 +1014,9 @@ sharq_status launch_linear(const sharq_config* cfg, const LinearArgs& a, int32_t
   return launch_tiles<128, SHARQ_MXFP4>(a, g, rows_total, m_blocks, E, num_sms, st);
 }
 
+#ifdef SHARQ_DEBUG_TS
+extern "C" int sharq_debug_read_ts(long long* host_out) {
+  return (int)cudaMemcpyFromSymbol(host_out, g_dbg_ts, sizeof(long long) * 1024 * 16);
+}
+#endif
 }  // namespace sharq
