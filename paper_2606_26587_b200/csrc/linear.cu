@@ -631,17 +631,14 @@ sharq_linear_pair_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __gr
             if (lead) tc::tma_load_2d_pair(st + S::A_SP, &tm_a_sp, fb, kb * 64, m_blk * BM, pol);
             if (lead) tc::tma_load_2d_pair(st + S::META, &tm_meta, fb, 0, (m_sf * kq + kb) * 2, pol);
             if (lead) tc::tma_load_2d_pair(st + S::SFA_SP, &tm_sfa_sp, fb, 0, m_sf * kq + kb, pol);
-#pragma unroll
-            for (int nb = 0; nb < 2; ++nb)
-              if (lead) tc::tma_load_2d_pair(st + S::SFB_SP + nb * 1024, &tm_sfb_sp, fb, 0, (wblk0 + nb) * kq + kb, pol);
+            // both CTAs need the B scales of all 256 rows: each fetches one 128-row atom row for both
+            if (lead) tc::tma_load_2d_pair_mc(st + S::SFB_SP + rank * 1024, &tm_sfb_sp, fb, 0, (wblk0 + rank) * kq + kb, 3, pol);
           }
           if (do_dn) {
             if (lead) tc::tma_load_2d_pair(st + S::A_DN, &tm_a_dn, fb, kb * 128, m_blk * BM, pol);
             if (lead) tc::tma_load_2d_pair(st + S::SFA_DN, &tm_sfa_dn, fb, 0, (m_sf * kq + kb) * DN_ROWS, pol);
-#pragma unroll
-            for (int nb = 0; nb < 2; ++nb)
-              if (lead) tc::tma_load_2d_pair(st + S::SFB_DN + nb * S::SF_DN_BYTES, &tm_sfb_dn, fb, 0,
-                                             ((wblk0 + nb) * kq + kb) * DN_ROWS, pol);
+            if (lead) tc::tma_load_2d_pair_mc(st + S::SFB_DN + rank * S::SF_DN_BYTES, &tm_sfb_dn, fb, 0,
+                                              ((wblk0 + rank) * kq + kb) * DN_ROWS, 3, pol);
           }
         }
       }
