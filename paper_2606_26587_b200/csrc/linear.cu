@@ -18,6 +18,7 @@
 #include <stdlib.h>
 
 #include "common.cuh"
+#include "debug_env.h"
 #include "tc_ptx.cuh"
 
 namespace sharq {
@@ -820,7 +821,7 @@ sharq_status launch_1cta(const LinearArgs& a, const KParams& p, const GroupInfo&
   cudaLaunchConfig_t lc{};
   cudaLaunchAttribute attr[2];
   attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-  attr[0].val.programmaticStreamSerializationAllowed = getenv("SHARQ_DEBUG_NO_PDL") ? 0 : 1;
+  attr[0].val.programmaticStreamSerializationAllowed = debug_env().no_pdl ? 0 : 1;
   lc.attrs = attr;
   lc.numAttrs = 1;
   lc.blockDim = dim3(kThreads);
@@ -844,7 +845,7 @@ sharq_status launch_1cta(const LinearArgs& a, const KParams& p, const GroupInfo&
   if (cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, S::SMEM) != cudaSuccess)
     return SHARQ_ECUDA;
   lc.gridDim = dim3((unsigned)(tiles < num_sms ? tiles : num_sms));      // persistent: one CTA per SM
-  if (const char* dbg = getenv("SHARQ_DEBUG_GRID")) lc.gridDim = dim3((unsigned)atoi(dbg));
+  if (debug_env().grid > 0) lc.gridDim = dim3((unsigned)debug_env().grid);
   lc.dynamicSmemBytes = S::SMEM;
   return cudaLaunchKernelEx(&lc, kfn, tm_sp, tm_dn, tm_w, p, g) == cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
 }
@@ -861,7 +862,7 @@ sharq_status launch_mc(const KParams& p, const GroupInfo& g, const CUtensorMap& 
   cudaLaunchConfig_t lc{};
   cudaLaunchAttribute attr[2];
   attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-  attr[0].val.programmaticStreamSerializationAllowed = getenv("SHARQ_DEBUG_NO_PDL") ? 0 : 1;
+  attr[0].val.programmaticStreamSerializationAllowed = debug_env().no_pdl ? 0 : 1;
   attr[1].id = cudaLaunchAttributeClusterDimension;
   attr[1].val.clusterDim.x = 2;
   attr[1].val.clusterDim.y = 1;
@@ -908,7 +909,7 @@ sharq_status launch_pair(const LinearArgs& a, const KParams& p, const CUtensorMa
     return SHARQ_ECUDA;
   const int64_t pair_tiles = ((m_blocks + 1) / 2) * ((a.D + PBN - 1) / PBN);
   int64_t clusters = pair_tiles < num_sms / 2 ? pair_tiles : num_sms / 2;
-  if (const char* dbg = getenv("SHARQ_DEBUG_PAIR_CLUSTERS")) clusters = atoi(dbg) < clusters ? atoi(dbg) : clusters;
+  if (debug_env().pair_clusters > 0 && debug_env().pair_clusters < clusters) clusters = debug_env().pair_clusters;
   cudaLaunchConfig_t lp{};
   cudaLaunchAttribute at[2];
   at[0].id = cudaLaunchAttributeClusterDimension;
@@ -916,7 +917,7 @@ sharq_status launch_pair(const LinearArgs& a, const KParams& p, const CUtensorMa
   at[0].val.clusterDim.y = 1;
   at[0].val.clusterDim.z = 1;
   at[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-  at[1].val.programmaticStreamSerializationAllowed = getenv("SHARQ_DEBUG_NO_PDL") ? 0 : 1;
+  at[1].val.programmaticStreamSerializationAllowed = debug_env().no_pdl ? 0 : 1;
   lp.blockDim = dim3(kThreads);
   lp.gridDim = dim3((unsigned)(2 * clusters));
   lp.dynamicSmemBytes = P::SMEM;
@@ -941,10 +942,8 @@ sharq_status launch_tiles(const LinearArgs& a, const GroupInfo& g, int64_t rows_
   KParams p{(const uint8_t*)a.sp_sf, (const uint8_t*)a.sp_meta, (const uint8_t*)a.dn_sf, (const uint8_t*)a.w_sf_sp,
             (const uint8_t*)a.w_sf_dn, a.row_scale, a.w_ts, (const uint16_t*)a.bias, a.Y, a.ldy,
             (int32_t)a.T, (int32_t)a.D, (int32_t)a.K, a.out_dtype, a.path, (int32_t)m_blocks, (int32_t)tiles, (int32_t)a_rows};
-  const char* no_pair = getenv("SHARQ_DEBUG_NO_PAIR");
-  const char* force_pair = getenv("SHARQ_DEBUG_FORCE_PAIR");
-  const bool pair_worth = ((m_blocks + 1) / 2) * (a.D / 256) >= num_sms / 4 || (force_pair && force_pair[0] == '1');
-  if (E == 0 && m_blocks >= 2 && BN == 128 && pair_worth && !(no_pair && no_pair[0] == '1')) {
+  const bool pair_worth = ((m_blocks + 1) / 2) * (a.D / 256) >= num_sms / 4 || debug_env().force_pair;
+  if (E == 0 && m_blocks >= 2 && BN == 128 && pair_worth && !debug_env().no_pair) {
     // tile width by a two-term cost model fitted on the box (us): rounds x (k-blocks x 0.43 + exposed
     // epilogue), the epilogue being hidden by the second TMEM accumulator only for 192-wide tiles
     const int64_t clusters = num_sms / 2, m_pairs = (m_blocks + 1) / 2;
@@ -952,13 +951,13 @@ sharq_status launch_tiles(const LinearArgs& a, const GroupInfo& g, int64_t rows_
     const double cost192 = (double)((m_pairs * ((a.D + 191) / 192) + clusters - 1) / clusters) * (per_kb + 0.3);
     const double cost256 = (double)((m_pairs * ((a.D + 255) / 256) + clusters - 1) / clusters) * (per_kb + 2.0);
     int width = (a.D % 256 != 0 || cost192 < cost256) ? 192 : 256;
-    if (const char* pbn = getenv("SHARQ_DEBUG_PAIR_BN")) width = (atoi(pbn) == 256 && a.D % 256 == 0) ? 256 : 192;
+    if (debug_env().pair_bn > 0) width = (debug_env().pair_bn == 256 && a.D % 256 == 0) ? 256 : 192;
     if (width == 256) return launch_pair<FMT, 256>(a, p, tm_sp, tm_dn, m_blocks, num_sms, st);
     return launch_pair<FMT, 192>(a, p, tm_sp, tm_dn, m_blocks, num_sms, st);
   }
   if constexpr (BN == 128) {
     // experts: n-tiles of one 128-row block are consecutive (decode_unit), so tiles 2j and 2j+1 share activations
-    if (E > 0 && (a.D / BN) % 2 == 0 && a_rows == (uint32_t)BM && !getenv("SHARQ_DEBUG_NO_MC"))
+    if (E > 0 && (a.D / BN) % 2 == 0 && a_rows == (uint32_t)BM && !debug_env().no_mc)
       return launch_mc<FMT>(p, g, tm_sp, tm_dn, tm_w, tiles, num_sms, st);
   }
   if (a_rows <= 16) return launch_1cta<BN, FMT, 16>(a, p, g, tm_sp, tm_dn, tm_w, tiles, num_sms, st);
@@ -1002,8 +1001,7 @@ sharq_status launch_linear(const sharq_config* cfg, const LinearArgs& a, int32_t
   // (the decode launches are bound by tensor-pipe issue per k-block, not by HBM)
   // ... and only pays when the 128-wide tiles would need a second round on the SMs (measured: with fewer
   // tiles than SMs the narrower tiles + deeper K-split win)
-  const char* wide_t = getenv("SHARQ_DEBUG_WIDE_T");
-  if (E == 0 && a.T <= (wide_t ? atoi(wide_t) : 128) && a.D % 256 == 0 && a.D / 128 > num_sms && !getenv("SHARQ_DEBUG_NO_WIDE")) {
+  if (E == 0 && a.T <= debug_env().wide_t && a.D % 256 == 0 && a.D / 128 > num_sms && !debug_env().no_wide) {
     if (cfg->fmt == SHARQ_NVFP4) return launch_tiles<256, SHARQ_NVFP4>(a, g, rows_total, m_blocks, E, num_sms, st);
     return launch_tiles<256, SHARQ_MXFP4>(a, g, rows_total, m_blocks, E, num_sms, st);
   }

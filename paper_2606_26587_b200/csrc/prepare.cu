@@ -14,6 +14,7 @@
 #include <stdlib.h>
 
 #include "common.cuh"
+#include "debug_env.h"
 
 namespace sharq {
 
@@ -723,7 +724,7 @@ static cudaError_t launch_row_kernel(int norm, const PrepParams& p, int num_sms,
   const int warps = (int)((p.K + 1023) / 1024);
   const dim3 block((unsigned)warps * 32);
   int per_sm = 2048 / (warps * 32);                       // thread limit; registers trim it further at launch
-  if (const char* e = getenv("SHARQ_DEBUG_ROW_PER_SM")) per_sm = atoi(e);
+  if (debug_env().row_per_sm > 0) per_sm = debug_env().row_per_sm;
   if (per_sm < 1) per_sm = 1;
   if (per_sm > 32) per_sm = 32;                           // grid = about twice the resident CTAs (finer tail); 32 one-warp CTAs for short rows
   int64_t ctas = (int64_t)num_sms * per_sm;
@@ -732,7 +733,7 @@ static cudaError_t launch_row_kernel(int norm, const PrepParams& p, int num_sms,
   cudaLaunchConfig_t lc{};
   cudaLaunchAttribute attr[1];
   attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-  attr[0].val.programmaticStreamSerializationAllowed = getenv("SHARQ_DEBUG_NO_PDL") ? 0 : 1;
+  attr[0].val.programmaticStreamSerializationAllowed = debug_env().no_pdl ? 0 : 1;
   lc.gridDim = grid; lc.blockDim = block; lc.stream = st; lc.attrs = attr; lc.numAttrs = 1;
   lc.dynamicSmemBytes = (size_t)warps * 1024 + 256 + 16 + (norm != SHARQ_NORM_NONE ? (size_t)warps * 32 * 128 : 0);   // + gamma, beta
   cudaError_t err = cudaSuccess;
@@ -797,7 +798,7 @@ cudaError_t launch_prepare(const sharq_config* cfg, const void* x, int64_t T, in
   p.dn_codes = (uint8_t*)dn_codes; p.dn_sf = (uint8_t*)dn_sf; p.row_scale = row_scale;
   p.eps = cfg->eps; p.tiled = (cfg->layout == SHARQ_LAYOUT_TILED);
   p.row_bytes = (uint32_t)(K * 2);
-  if (K <= 1024 * kRowMaxWarps && !getenv("SHARQ_DEBUG_OLD_PREPARE")) {
+  if (K <= 1024 * kRowMaxWarps && !debug_env().old_prepare) {
     p.nbuf = 0;
     if (cfg->fmt == SHARQ_NVFP4) return launch_row_kernel<SHARQ_NVFP4>(cfg->norm, p, num_sms, st);
     if (cfg->fmt == SHARQ_MXFP4) return launch_row_kernel<SHARQ_MXFP4>(cfg->norm, p, num_sms, st);
