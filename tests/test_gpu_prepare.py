@@ -32,6 +32,9 @@ CASES = [
     (0, 1, 1, 130, 3584, 200.0), (0, 2, 0, 9, 2048, 50.0), (0, 0, 0, 1, 256, 50.0), (0, 1, 0, 300, 1024, 50.0),
     (1, 1, 0, 16, 4096, 50.0), (1, 0, 1, 33, 3584, 200.0), (1, 2, 0, 7, 768, 10.0), (1, 1, 1, 129, 18944, 50.0),
     (2, 1, 0, 16, 4096, 50.0), (2, 0, 0, 33, 3584, 200.0), (2, 2, 0, 7, 768, 10.0), (2, 1, 0, 3, 18944, 50.0),
+    # the widest row one CTA covers (32 warps) and the first K beyond it (warp-per-row kernel, row in smem)
+    (0, 1, 1, 3, 32768, 50.0), (0, 1, 1, 3, 33792, 50.0), (0, 2, 0, 150, 33792, 50.0), (1, 0, 0, 2, 33792, 200.0),
+    (2, 1, 0, 2, 33792, 50.0),
 ]
 
 
