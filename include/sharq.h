@@ -133,25 +133,6 @@ sharq_status sharq_linear(const sharq_config* cfg, int64_t T, int64_t D, int64_t
                           const void* bias, void* Y, int64_t ldy, int32_t out_dtype, int32_t path,
                           void* workspace, size_t workspace_bytes, void* stream);
 
-/* ---- sharq_prepare_linear: sharq_prepare followed by sharq_linear as ONE launch ----------
- * Same results, bit for bit, as sharq_prepare(cfg, x, T, K, ldx, gamma, NULL, x_tensor_scale, <operands>)
- * followed by sharq_linear(cfg, T, D, K, <operands>, <weights>, bias, Y, ldy, out_dtype, 0, ...); the
- * prepared operands are still written to the caller's buffers (device, layout TILED).  For decode-sized
- * problems (T <= 128, K <= 16384, NVFP4 / MXFP4, no norm or RMSNorm) extra warps of the GEMM's CTAs prepare
- * the rows while the weight stream is already running, and a device-scope counter releases the activation
- * loads: one launch and one kernel-to-kernel dependency less per layer.  Every other case is issued as the
- * two launches.  `sync`: device int32[2], zero before the first call; every call leaves it zero, so one
- * buffer serves all calls of a stream (calls that may run concurrently need their own).  LayerNorm (beta)
- * is not offered here: use the two calls.  Error behaviour as the two calls. */
-sharq_status sharq_prepare_linear(const sharq_config* cfg, const void* x, int64_t T, int64_t K, int64_t ldx,
-                                  const void* gamma, const float* x_tensor_scale, void* sp_codes,
-                                  void* sp_sf, void* sp_meta, void* dn_codes, void* dn_sf,
-                                  float* row_scale, int64_t D, const void* w_codes,
-                                  const void* w_sf_sparse_view, const void* w_sf_dense_view,
-                                  const float* w_tensor_scale, const void* bias, void* Y, int64_t ldy,
-                                  int32_t out_dtype, int32_t* sync, void* workspace,
-                                  size_t workspace_bytes, void* stream);
-
 /* ---- sharq_linear_grouped (MoE expert linears) -----------------------------
  * E experts; `offsets` is a HOST int32[E+1] array: rows [offsets[e], offsets[e+1]) of the
  * activation tensors belong to expert e.  Every expert's row range must start at a multiple of

@@ -61,8 +61,6 @@ def _load() -> ctypes.CDLL:
                                  c_int32, c_int32, P, c_size_t, P]
     lib.sharq_linear_grouped.argtypes = [CFG, c_int32, POINTER(c_int32), c_int64, c_int64, P, P, P, P, P, P, P, P,
                                          P, P, P, c_int64, c_int32, P, c_size_t, P]
-    lib.sharq_prepare_linear.argtypes = [CFG, P, c_int64, c_int64, c_int64, P, P, P, P, P, P, P, P, c_int64, P, P, P, P,
-                                         P, P, c_int64, c_int32, P, P, c_size_t, P]
     lib.sharq_mma_peak_launch.argtypes = [c_int32, c_int32, P]
     lib.sharq_mma_peak_launch.restype = c_int32
     for name in ("sharq_weight_sizes", "sharq_act_sizes", "sharq_linear_workspace", "sharq_quantize_weight",
@@ -74,7 +72,7 @@ def _load() -> ctypes.CDLL:
 capi = _load()
 EXPORTS = ("sharq_version", "sharq_weight_sizes", "sharq_act_sizes", "sharq_linear_workspace",
            "sharq_quantize_weight", "sharq_prepare", "sharq_linear", "sharq_linear_grouped",
-           "sharq_prepare_linear", "sharq_mma_peak_launch")
+           "sharq_mma_peak_launch")
 
 
 def version() -> str:
@@ -188,34 +186,6 @@ def linear(cfg: Config, act: dict, wq: dict, bias=None, out_dtype="bf16", path=P
                              _ptr(Y), Y.stride(0), 0 if Y.dtype == torch.bfloat16 else 1, path, _ptr(workspace), n_ws,
                              _stream()), "sharq_linear")
     return Y
-
-
-def alloc_sync(device):
-    """The two zeroed device counters sharq_prepare_linear needs (one buffer per stream is enough)."""
-    import torch
-    return torch.zeros(2, dtype=torch.int32, device=device)
-
-
-def prepare_linear(cfg: Config, x, gamma, wq: dict, sync, x_tensor_scale=None, bias=None, out_dtype="bf16", act=None,
-                   Y=None, workspace=None):
-    """sharq_prepare + sharq_linear in one call (one launch for T <= 128, see sharq.h); returns (act, Y)."""
-    import torch
-    T, K = x.shape
-    D = wq["D"]
-    if act is None:
-        act = alloc_act(cfg, T, K, x.device)
-    if Y is None:
-        Y = torch.empty((T, D), dtype=torch.bfloat16 if out_dtype == "bf16" else torch.float32, device=x.device)
-    n_ws = linear_workspace(cfg, T, D, K)
-    if workspace is None and n_ws:
-        workspace = _bytes(n_ws, x.device)
-    _check(capi.sharq_prepare_linear(ctypes.byref(cfg), _ptr(x), T, K, x.stride(0), _ptr(gamma), _ptr(x_tensor_scale),
-                                     _ptr(act["sp_codes"]), _ptr(act["sp_sf"]), _ptr(act["sp_meta"]),
-                                     _ptr(act["dn_codes"]), _ptr(act["dn_sf"]), _ptr(act["row_scale"]), D,
-                                     _ptr(wq["codes"]), _ptr(wq["sf_sp"]), _ptr(wq["sf_dn"]), _ptr(wq["ts_w"]),
-                                     _ptr(bias), _ptr(Y), Y.stride(0), 0 if Y.dtype == torch.bfloat16 else 1,
-                                     _ptr(sync), _ptr(workspace), n_ws, _stream()), "sharq_prepare_linear")
-    return act, Y
 
 
 def linear_grouped(cfg: Config, offsets, act: dict, wq: dict, D: int, out_dtype="bf16", Y=None, workspace=None):

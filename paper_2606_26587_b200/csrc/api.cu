@@ -24,10 +24,6 @@ struct LinearArgs {
 sharq_status launch_linear(const sharq_config* cfg, const LinearArgs& a, int32_t E, const int32_t* offsets_host,
                            void* workspace, size_t workspace_bytes, int num_sms, cudaStream_t st);
 size_t linear_workspace_bytes(const sharq_config* cfg, int64_t T, int64_t D, int64_t K, int32_t E);
-bool fused_prepare_linear_applies(const sharq_config* cfg, int64_t T, int64_t D, int64_t K, int32_t path);
-sharq_status launch_prepare_linear(const sharq_config* cfg, const void* x, int64_t ldx, const void* gamma,
-                                   const float* x_ts, const LinearArgs& a, int32_t* sync, int num_sms,
-                                   cudaStream_t st);
 }  // namespace sharq
 
 using namespace sharq;
@@ -178,38 +174,6 @@ sharq_status sharq_linear(const sharq_config* cfg, int64_t T, int64_t D, int64_t
   LinearArgs a{T, D, K, sp_codes, sp_sf, sp_meta, dn_codes, dn_sf, row_scale, w_codes, w_sf_sparse_view,
                w_sf_dense_view, w_tensor_scale, bias, Y, ldy, out_dtype, path};
   return launch_linear(cfg, a, 0, nullptr, workspace, workspace_bytes, di.sms, (cudaStream_t)stream);
-}
-
-sharq_status sharq_prepare_linear(const sharq_config* cfg, const void* x, int64_t T, int64_t K, int64_t ldx,
-                                  const void* gamma, const float* x_tensor_scale, void* sp_codes, void* sp_sf,
-                                  void* sp_meta, void* dn_codes, void* dn_sf, float* row_scale, int64_t D,
-                                  const void* w_codes, const void* w_sf_sparse_view, const void* w_sf_dense_view,
-                                  const float* w_tensor_scale, const void* bias, void* Y, int64_t ldy,
-                                  int32_t out_dtype, int32_t* sync, void* workspace, size_t workspace_bytes,
-                                  void* stream) {
-  sharq_status s = check_cfg(cfg);
-  if (s != SHARQ_OK) return s;
-  if (cfg->norm == SHARQ_NORM_LAYER) return SHARQ_EINVAL;
-  if (!sync) return SHARQ_EINVAL;
-  if (T >= 1 && K > 0 && K % 256 == 0 && fused_prepare_linear_applies(cfg, T, D, K, 0)) {
-    // the one-launch path: validate exactly what the two calls would
-    if (ldx < K || ldx % 8 != 0) return SHARQ_ESHAPE;
-    if (!x || !row_scale || !w_tensor_scale) return SHARQ_EINVAL;
-    if (cfg->norm != SHARQ_NORM_NONE && !gamma) return SHARQ_EINVAL;
-    if (!aligned16(x) || (gamma && !aligned16(gamma))) return SHARQ_EINVAL;
-    const void* ptrs[] = {sp_codes, sp_sf, sp_meta, dn_codes, dn_sf, w_codes, w_sf_sparse_view, w_sf_dense_view, Y};
-    if ((s = check_linear(cfg, D, K, ptrs, 9, ldy, out_dtype, 0)) != SHARQ_OK) return s;
-    DeviceInfo di{};
-    if ((s = device_info(&di)) != SHARQ_OK) return s;
-    LinearArgs a{T, D, K, sp_codes, sp_sf, sp_meta, dn_codes, dn_sf, row_scale, w_codes, w_sf_sparse_view,
-                 w_sf_dense_view, w_tensor_scale, bias, Y, ldy, out_dtype, 0};
-    return launch_prepare_linear(cfg, x, ldx, gamma, x_tensor_scale, a, sync, di.sms, (cudaStream_t)stream);
-  }
-  s = sharq_prepare(cfg, x, T, K, ldx, gamma, nullptr, x_tensor_scale, sp_codes, sp_sf, sp_meta, dn_codes, dn_sf,
-                    row_scale, stream);
-  if (s != SHARQ_OK) return s;
-  return sharq_linear(cfg, T, D, K, sp_codes, sp_sf, sp_meta, dn_codes, dn_sf, row_scale, w_codes, w_sf_sparse_view,
-                      w_sf_dense_view, w_tensor_scale, bias, Y, ldy, out_dtype, 0, workspace, workspace_bytes, stream);
 }
 
 sharq_status sharq_linear_grouped(const sharq_config* cfg, int32_t E, const int32_t* offsets_host, int64_t D,

@@ -16,7 +16,6 @@ struct DebugEnv {
   int no_wide;         // SHARQ_DEBUG_NO_WIDE: never use 128 x 256 tiles
   int row_per_sm;      // SHARQ_DEBUG_ROW_PER_SM: prepare grid = this many CTAs per SM (0 = default)
   int old_prepare;     // SHARQ_DEBUG_OLD_PREPARE: warp-per-row prepare kernel for every K
-  int no_fused;        // SHARQ_DEBUG_NO_FUSED: sharq_prepare_linear always as two launches
 };
 
 inline const DebugEnv& debug_env() {
@@ -38,7 +37,6 @@ inline const DebugEnv& debug_env() {
     d.no_wide = flag("SHARQ_DEBUG_NO_WIDE");
     d.row_per_sm = num("SHARQ_DEBUG_ROW_PER_SM", 0);
     d.old_prepare = flag("SHARQ_DEBUG_OLD_PREPARE");
-    d.no_fused = flag("SHARQ_DEBUG_NO_FUSED");
     return d;
   }();
   return e;

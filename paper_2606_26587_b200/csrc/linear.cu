@@ -19,7 +19,6 @@
 
 #include "common.cuh"
 #include "debug_env.h"
-#include "prepare_device.cuh"
 #include "tc_ptx.cuh"
 
 namespace sharq {
@@ -55,14 +54,6 @@ struct GroupInfo {
   int32_t count[kMaxExperts];              // valid rows of expert e
 };
 
-// sharq_prepare_linear: what the in-kernel prepare needs (null pointer = plain sharq_linear)
-struct FusedArgs {
-  PrepParams pp;
-  int32_t* sync;       // two device counters, zero before the first launch; every launch leaves them zero
-  int32_t norm;        // SHARQ_NORM_NONE or SHARQ_NORM_RMS
-  int32_t warps;       // K / 1024 rounded up: prepare warps per CTA
-};
-
 struct KParams {
   const uint8_t *sp_sf, *sp_meta, *dn_sf, *w_sf_sp, *w_sf_dn;
   const float *row_scale, *w_ts;
@@ -84,10 +75,7 @@ struct KParams {
 // and a smaller reservation leaves room for more ring stages, i.e. more weight bytes in flight per SM (the
 // decode shapes are bound by exactly that).  The MMA still reads 128 rows; rows beyond the loaded ones are
 // whatever follows in shared memory and only reach accumulator rows that are never stored.
-constexpr int kPrepSmem = 24 * 1024;   // fused kernel: shared memory of the in-kernel sharq_prepare rows
-constexpr int kMaxPrepWarps = 16;      // fused kernel: K <= 16384
-
-template <int BN, int FMT, bool SPLIT, int AR, int EXTRA = 0>
+template <int BN, int FMT, bool SPLIT, int AR>
 struct Stage {
   static constexpr int NB = (BN + 127) / 128;                         // 128-row scale atoms of W per tile
   static constexpr int SF_DN_BYTES = (FMT == SHARQ_NVFP4) ? 2048 : 1024;  // per 128 rows per k-block
@@ -106,9 +94,9 @@ struct Stage {
   static constexpr int NSL = BN / 16;                                 // 16-column slices of the accumulator
   static constexpr int RECV = SPLIT ? (NSL + 2) * AR * 64 : 0;        // [src][slot][AR rows][16 fp32]; S*ceil(NSL/S) <= NSL+2 for S in {2,3,4,8}
   static constexpr int PAD = AR < 128 ? 128 * 128 : 0;               // the MMA's over-read behind the last stage
-  static constexpr int FIT = (232448 - 1024 - 256 - RECV - PAD - EXTRA) / BYTES;
+  static constexpr int FIT = (232448 - 1024 - 256 - RECV - PAD) / BYTES;
   static constexpr int STAGES = FIT > 8 ? 8 : FIT;
-  static constexpr int SMEM = STAGES * BYTES + PAD + RECV + 1024 /*alignment slack*/ + 256 /*barriers*/ + EXTRA;
+  static constexpr int SMEM = STAGES * BYTES + PAD + RECV + 1024 /*alignment slack*/ + 256 /*barriers*/;
   // tensor-memory columns: two accumulator stages, then metadata and scale factors
   static constexpr int SFB_COLS = NB * 4;          // columns one MMA's B scales occupy
   static constexpr int ACC_STAGES = BN > 128 ? 1 : 2;
@@ -177,19 +165,11 @@ __device__ __forceinline__ void store_row(const KParams& p, int64_t row, int col
 // MC = true (grouped GEMM): a cluster of two CTAs works on two neighbouring n-tiles of the same 128-row block in
 // lock step; each CTA fetches half of the shared activation operands and multicasts them to both (the many
 // short tiles of the expert GEMMs are bound by L2 -> SM traffic, 60 % of which is the activation side).
-//
-// FUSED = true (sharq_prepare_linear, T <= 128): warps 6.. of every CTA run sharq_prepare for the rows
-// blockIdx.x, blockIdx.x + gridDim.x, ... (prepare_rows, named barrier 2) while warp 0 already streams the
-// weights; a device-scope counter (release / acquire) tells every CTA's producer when all T rows are in
-// global memory, then the activation loads start.  One launch and one dependency hop less per layer.
-// All CTAs are co-resident (one per SM, grid <= SM count), so the spin cannot deadlock.
-template <int BN, int FMT, bool SPLIT, int AR, bool MC = false, bool FUSED = false>
-__global__ void __launch_bounds__(FUSED ? kThreads + 32 * kMaxPrepWarps : kThreads, 1)
+template <int BN, int FMT, bool SPLIT, int AR, bool MC = false>
+__global__ void __launch_bounds__(kThreads, 1)
 sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_constant__ CUtensorMap tm_a_dn,
-                    const __grid_constant__ CUtensorMap tm_w, const KParams p, const __grid_constant__ GroupInfo g,
-                    const PrepParams pp, int32_t* sync, int32_t prep_norm) {
-  using S = Stage<BN, FMT, SPLIT, AR, FUSED ? kPrepSmem : 0>;
-  static_assert(!(FUSED && MC), "the fused kernel is for dense single-problem launches");
+                    const __grid_constant__ CUtensorMap tm_w, const KParams p, const __grid_constant__ GroupInfo g) {
+  using S = Stage<BN, FMT, SPLIT, AR>;
   constexpr bool NV = (FMT == SHARQ_NVFP4);
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
@@ -311,24 +291,6 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
           }
           SHARQ_TS(2);
           tc::grid_dependency_wait();
-          if constexpr (FUSED) {
-            // all T rows prepared (by the extra warps of this launch's CTAs) and visible: acquire the counter,
-            // order the generic-proxy writes before the tensor copies that follow, then count this CTA as
-            // past the wait; the last one re-arms the two counters for the next launch
-            if (lead) {
-              int32_t seen;
-              do {
-                asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(seen) : "l"(sync) : "memory");
-              } while (seen < p.T);
-              asm volatile("fence.proxy.async;" ::: "memory");
-              if (atomicAdd(sync + 1, 1) == (int32_t)gridDim.x - 1) {
-                sync[0] = 0;
-                sync[1] = 0;
-                __threadfence();
-              }
-            }
-            __syncwarp();
-          }
           SHARQ_TS(3);
           dep_synced = true;
           for (int i = 0; i < n_early; ++i) load_a(kb + i, smem_base + i * S::BYTES, full_bar(i));
@@ -420,7 +382,7 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
         if (lead) tc::tc_commit(tmem_full_bar(as));                // accumulator complete
       }
     }
-  } else if (warp < 6) {
+  } else {
     // =========================== epilogue ====================================================
     tc::grid_dependency_wait();                          // row_scale is sharq_prepare's; Y may still be read
     const int sub = warp & 3;                            // TMEM sub-partition this warp may read
@@ -433,12 +395,9 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
         const uint32_t as = n_unit % S::ACC_STAGES;
         const int64_t row = (int64_t)u.m_blk * BM + r_local;
         const bool row_ok = r_local < u.rows_valid;
-        float scale = 0.0f;
-        if (!FUSED && row_ok) scale = __fmul_rn(p.row_scale[row], p.w_ts[u.expert]);
+        const float scale = row_ok ? __fmul_rn(p.row_scale[row], p.w_ts[u.expert]) : 0.0f;
         tc::mbar_wait(tmem_full_bar(as), (n_unit / S::ACC_STAGES) & 1u);
         tc::tc_fence_after();
-        // fused: the row scale is written by this launch; a full accumulator implies it has landed (L2 read)
-        if (FUSED && row_ok) scale = __fmul_rn(__ldcg(p.row_scale + row), p.w_ts[u.expert]);
 #pragma unroll 1
         for (int c = 0; c < BN / 32; ++c) {
           uint32_t v[32];
@@ -461,9 +420,8 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
       const bool row_ok = r_local < u.rows_valid;
       const int slots = (BN / 16 + splits - 1) / splits;
       // the output scale of this thread's row, fetched while the main loop runs (used after the exchange)
-      if (!FUSED && row_ok) split_scale = __fmul_rn(p.row_scale[(int64_t)u.m_blk * BM + r_local], p.w_ts[u.expert]);
+      if (row_ok) split_scale = __fmul_rn(p.row_scale[(int64_t)u.m_blk * BM + r_local], p.w_ts[u.expert]);
       tc::mbar_wait(tmem_full_bar(0), 0);
-      if (FUSED && row_ok) split_scale = __fmul_rn(__ldcg(p.row_scale + (int64_t)u.m_blk * BM + r_local), p.w_ts[u.expert]);
       if (warp == 2) SHARQ_TS(6);
       tc::tc_fence_after();
 #pragma unroll 1
@@ -499,30 +457,13 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
       }
       tc::tc_fence_before();
     }
-  } else {
-    // =========================== in-kernel sharq_prepare (FUSED only: warps 6 ..) ==================
-    if constexpr (FUSED) {
-      tc::grid_dependency_wait();                        // x belongs to the kernels before this one
-      const int ptid = (int)threadIdx.x - kThreads, pthreads = (int)blockDim.x - kThreads;
-      uint8_t* prep_smem = smem_raw + (bars + 256u - smem_u32(smem_raw));
-      if (prep_norm == SHARQ_NORM_RMS)
-        prepare_rows<FMT, SHARQ_NORM_RMS, 2>(pp, prep_smem, ptid, pthreads, (int64_t)blockIdx.x, (int64_t)gridDim.x);
-      else
-        prepare_rows<FMT, SHARQ_NORM_NONE, 2>(pp, prep_smem, ptid, pthreads, (int64_t)blockIdx.x, (int64_t)gridDim.x);
-      __threadfence();                                   // every thread's stores, device scope
-      named_bar_sync<2>(pthreads);
-      if (ptid == 0 && (int64_t)blockIdx.x < pp.T) {
-        const int32_t mine = (int32_t)((pp.T - 1 - (int64_t)blockIdx.x) / (int64_t)gridDim.x + 1);
-        asm volatile("red.release.gpu.global.add.s32 [%0], %1;" ::"l"(sync), "r"(mine) : "memory");
-      }
-    }
   }
   if constexpr (SPLIT) {
     __syncwarp();
     if (warp == 2) SHARQ_TS(7);
     tc::cluster_sync_all();                              // partial slices have landed in their owners
     if (warp == 2) SHARQ_TS(8);
-    if (warp >= 2 && warp < 6) {
+    if (warp >= 2) {
       const Unit u = decode_unit(p, g, tile0, rank, splits);
       const int r_local = (warp & 3) * 32 + lane;
       if (r_local < u.rows_valid) {
@@ -844,10 +785,10 @@ bool make_map(CUtensorMap* m, const void* base, uint64_t rows, uint64_t row_byte
 // leave most SMs idle, only sizes whose slice exchange fits the receive buffer (2, 3, 4, 8), and only if
 // all `tiles` clusters are co-resident in ONE wave (cluster placement is per GPC, so tiles * S <= SMs is
 // not enough: cudaOccupancyMaxActiveClusters decides).
-template <int BN, int FMT, int AR, bool FUSED>
+template <int BN, int FMT, int AR>
 int choose_splits(int64_t tiles, int num_kb, int num_sms) {
   if (tiles * 2 > num_sms) return 1;
-  using S = Stage<BN, FMT, true, AR, FUSED ? kPrepSmem : 0>;
+  using S = Stage<BN, FMT, true, AR>;
   static int max_clusters[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};      // per cluster size, queried once
   const int cand[4] = {8, 4, 3, 2};
   for (int c : cand) {
@@ -857,12 +798,10 @@ int choose_splits(int64_t tiles, int num_kb, int num_sms) {
       cudaLaunchAttribute at[1];
       at[0].id = cudaLaunchAttributeClusterDimension;
       at[0].val.clusterDim.x = (unsigned)c; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
-      lc.gridDim = dim3((unsigned)(c * num_sms));
-      lc.blockDim = dim3(FUSED ? kThreads + 32 * kMaxPrepWarps : kThreads);
-      lc.dynamicSmemBytes = S::SMEM;
+      lc.gridDim = dim3((unsigned)(c * num_sms)); lc.blockDim = dim3(kThreads); lc.dynamicSmemBytes = S::SMEM;
       lc.attrs = at; lc.numAttrs = 1;
       int n = 0;
-      auto kfn = sharq_linear_kernel<BN, FMT, true, AR, false, FUSED>;
+      auto kfn = sharq_linear_kernel<BN, FMT, true, AR>;
       cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, S::SMEM);
       if (cudaOccupancyMaxActiveClusters(&n, kfn, &lc) != cudaSuccess || n <= 0) n = -1;
       max_clusters[c] = n;
@@ -872,28 +811,24 @@ int choose_splits(int64_t tiles, int num_kb, int num_sms) {
   return 1;
 }
 
-template <int BN, int FMT, int AR, bool FUSED>
-sharq_status launch_1cta_impl(const LinearArgs& a, const KParams& p, const GroupInfo& g, const CUtensorMap& tm_sp,
-                              const CUtensorMap& tm_dn, const CUtensorMap& tm_w, int64_t tiles, int num_sms,
-                              cudaStream_t st, const FusedArgs* fz) {
+template <int BN, int FMT, int AR>
+sharq_status launch_1cta(const LinearArgs& a, const KParams& p, const GroupInfo& g, const CUtensorMap& tm_sp,
+                         const CUtensorMap& tm_dn, const CUtensorMap& tm_w, int64_t tiles, int num_sms,
+                         cudaStream_t st) {
   constexpr bool kSplitFits = !(BN == 256 && AR == 128);   // no room for the exchange buffers; never needed there
-  constexpr int kExtra = FUSED ? kPrepSmem : 0;
   int splits = 1;
-  if constexpr (kSplitFits) splits = choose_splits<BN, FMT, AR, FUSED>(tiles, (int)(a.K / BK), num_sms);
+  if constexpr (kSplitFits) splits = choose_splits<BN, FMT, AR>(tiles, (int)(a.K / BK), num_sms);
   cudaLaunchConfig_t lc{};
   cudaLaunchAttribute attr[2];
   attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
   attr[0].val.programmaticStreamSerializationAllowed = debug_env().no_pdl ? 0 : 1;
   lc.attrs = attr;
   lc.numAttrs = 1;
-  lc.blockDim = dim3(FUSED ? kThreads + 32 * fz->warps : kThreads);
+  lc.blockDim = dim3(kThreads);
   lc.stream = st;
-  const PrepParams pp = FUSED ? fz->pp : PrepParams{};
-  int32_t* sync = FUSED ? fz->sync : nullptr;
-  const int32_t norm = FUSED ? fz->norm : 0;
   if constexpr (kSplitFits) if (splits > 1) {
-    using S = Stage<BN, FMT, true, AR, kExtra>;
-    auto kfn = sharq_linear_kernel<BN, FMT, true, AR, false, FUSED>;
+    using S = Stage<BN, FMT, true, AR>;
+    auto kfn = sharq_linear_kernel<BN, FMT, true, AR>;
     if (cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, S::SMEM) != cudaSuccess)
       return SHARQ_ECUDA;
     lc.gridDim = dim3((unsigned)(tiles * splits));
@@ -903,24 +838,16 @@ sharq_status launch_1cta_impl(const LinearArgs& a, const KParams& p, const Group
     attr[1].val.clusterDim.y = 1;
     attr[1].val.clusterDim.z = 1;
     lc.numAttrs = 2;
-    return cudaLaunchKernelEx(&lc, kfn, tm_sp, tm_dn, tm_w, p, g, pp, sync, norm) == cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
+    return cudaLaunchKernelEx(&lc, kfn, tm_sp, tm_dn, tm_w, p, g) == cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
   }
-  using S = Stage<BN, FMT, false, AR, kExtra>;
-  auto kfn = sharq_linear_kernel<BN, FMT, false, AR, false, FUSED>;
+  using S = Stage<BN, FMT, false, AR>;
+  auto kfn = sharq_linear_kernel<BN, FMT, false, AR>;
   if (cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, S::SMEM) != cudaSuccess)
     return SHARQ_ECUDA;
   lc.gridDim = dim3((unsigned)(tiles < num_sms ? tiles : num_sms));      // persistent: one CTA per SM
   if (debug_env().grid > 0) lc.gridDim = dim3((unsigned)debug_env().grid);
   lc.dynamicSmemBytes = S::SMEM;
-  return cudaLaunchKernelEx(&lc, kfn, tm_sp, tm_dn, tm_w, p, g, pp, sync, norm) == cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
-}
-
-template <int BN, int FMT, int AR>
-sharq_status launch_1cta(const LinearArgs& a, const KParams& p, const GroupInfo& g, const CUtensorMap& tm_sp,
-                         const CUtensorMap& tm_dn, const CUtensorMap& tm_w, int64_t tiles, int num_sms,
-                         cudaStream_t st, const FusedArgs* fz) {
-  if (fz) return launch_1cta_impl<BN, FMT, AR, true>(a, p, g, tm_sp, tm_dn, tm_w, tiles, num_sms, st, fz);
-  return launch_1cta_impl<BN, FMT, AR, false>(a, p, g, tm_sp, tm_dn, tm_w, tiles, num_sms, st, nullptr);
+  return cudaLaunchKernelEx(&lc, kfn, tm_sp, tm_dn, tm_w, p, g) == cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
 }
 
 // grouped GEMM: persistent clusters of two CTAs on neighbouring n-tiles, activation operands multicast
@@ -946,8 +873,7 @@ sharq_status launch_mc(const KParams& p, const GroupInfo& g, const CUtensorMap& 
   lc.gridDim = dim3((unsigned)(2 * clusters));
   lc.dynamicSmemBytes = S::SMEM;
   lc.stream = st;
-  return cudaLaunchKernelEx(&lc, kfn, tm_sp, tm_dn, tm_w, p, g, PrepParams{}, (int32_t*)nullptr, (int32_t)0) == cudaSuccess
-             ? SHARQ_OK : SHARQ_ECUDA;
+  return cudaLaunchKernelEx(&lc, kfn, tm_sp, tm_dn, tm_w, p, g) == cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
 }
 
 // scale-factor / metadata array as a 2-D tensor of 1024-byte rows (256 x u32), boxes of `box_rows` rows
@@ -1004,7 +930,7 @@ sharq_status launch_pair(const LinearArgs& a, const KParams& p, const CUtensorMa
 
 template <int BN, int FMT>
 sharq_status launch_tiles(const LinearArgs& a, const GroupInfo& g, int64_t rows_total, int64_t m_blocks, int E,
-                          int num_sms, cudaStream_t st, const FusedArgs* fz) {
+                          int num_sms, cudaStream_t st) {
   CUtensorMap tm_sp, tm_dn, tm_w;
   const int64_t w_rows = (int64_t)(E > 0 ? E : 1) * a.D;
   const uint32_t a_rows = (m_blocks == 1 && rows_total < BM) ? (uint32_t)((rows_total + 7) / 8 * 8) : BM;
@@ -1034,9 +960,9 @@ sharq_status launch_tiles(const LinearArgs& a, const GroupInfo& g, int64_t rows_
     if (E > 0 && (a.D / BN) % 2 == 0 && a_rows == (uint32_t)BM && !debug_env().no_mc)
       return launch_mc<FMT>(p, g, tm_sp, tm_dn, tm_w, tiles, num_sms, st);
   }
-  if (a_rows <= 16) return launch_1cta<BN, FMT, 16>(a, p, g, tm_sp, tm_dn, tm_w, tiles, num_sms, st, fz);
-  if (a_rows <= 64) return launch_1cta<BN, FMT, 64>(a, p, g, tm_sp, tm_dn, tm_w, tiles, num_sms, st, fz);
-  return launch_1cta<BN, FMT, 128>(a, p, g, tm_sp, tm_dn, tm_w, tiles, num_sms, st, fz);
+  if (a_rows <= 16) return launch_1cta<BN, FMT, 16>(a, p, g, tm_sp, tm_dn, tm_w, tiles, num_sms, st);
+  if (a_rows <= 64) return launch_1cta<BN, FMT, 64>(a, p, g, tm_sp, tm_dn, tm_w, tiles, num_sms, st);
+  return launch_1cta<BN, FMT, 128>(a, p, g, tm_sp, tm_dn, tm_w, tiles, num_sms, st);
 }
 
 }  // namespace
@@ -1049,9 +975,8 @@ size_t linear_workspace_bytes(const sharq_config* cfg, int64_t T, int64_t D, int
   return cfg->fmt == SHARQ_HIF4 ? hif4_linear_workspace_bytes(T, D, K) : 0;   // bf16 copies of A and W
 }
 
-static sharq_status launch_linear_impl(const sharq_config* cfg, const LinearArgs& a, int32_t E,
-                                       const int32_t* offsets_host, void* workspace, size_t workspace_bytes,
-                                       int num_sms, cudaStream_t st, const FusedArgs* fz) {
+sharq_status launch_linear(const sharq_config* cfg, const LinearArgs& a, int32_t E, const int32_t* offsets_host,
+                           void* workspace, size_t workspace_bytes, int num_sms, cudaStream_t st) {
   if (cfg->fmt == SHARQ_HIF4)                             // no FP4-rate tensor path: exact bf16 emulation
     return E > 0 ? SHARQ_EINVAL : launch_linear_hif4(a, workspace, workspace_bytes, num_sms, st);
   if (a.K > (int64_t)1 << 24 || a.D > (int64_t)1 << 24) return SHARQ_ESHAPE;
@@ -1077,11 +1002,11 @@ static sharq_status launch_linear_impl(const sharq_config* cfg, const LinearArgs
   // ... and only pays when the 128-wide tiles would need a second round on the SMs (measured: with fewer
   // tiles than SMs the narrower tiles + deeper K-split win)
   if (E == 0 && a.T <= debug_env().wide_t && a.D % 256 == 0 && a.D / 128 > num_sms && !debug_env().no_wide) {
-    if (cfg->fmt == SHARQ_NVFP4) return launch_tiles<256, SHARQ_NVFP4>(a, g, rows_total, m_blocks, E, num_sms, st, fz);
-    return launch_tiles<256, SHARQ_MXFP4>(a, g, rows_total, m_blocks, E, num_sms, st, fz);
+    if (cfg->fmt == SHARQ_NVFP4) return launch_tiles<256, SHARQ_NVFP4>(a, g, rows_total, m_blocks, E, num_sms, st);
+    return launch_tiles<256, SHARQ_MXFP4>(a, g, rows_total, m_blocks, E, num_sms, st);
   }
-  if (cfg->fmt == SHARQ_NVFP4) return launch_tiles<128, SHARQ_NVFP4>(a, g, rows_total, m_blocks, E, num_sms, st, fz);
-  return launch_tiles<128, SHARQ_MXFP4>(a, g, rows_total, m_blocks, E, num_sms, st, fz);
+  if (cfg->fmt == SHARQ_NVFP4) return launch_tiles<128, SHARQ_NVFP4>(a, g, rows_total, m_blocks, E, num_sms, st);
+  return launch_tiles<128, SHARQ_MXFP4>(a, g, rows_total, m_blocks, E, num_sms, st);
 }
 
 #ifdef SHARQ_DEBUG_TS
@@ -1089,35 +1014,4 @@ extern "C" int sharq_debug_read_ts(long long* host_out) {
   return (int)cudaMemcpyFromSymbol(host_out, g_dbg_ts, sizeof(long long) * 1024 * 16);
 }
 #endif
-sharq_status launch_linear(const sharq_config* cfg, const LinearArgs& a, int32_t E, const int32_t* offsets_host,
-                           void* workspace, size_t workspace_bytes, int num_sms, cudaStream_t st) {
-  return launch_linear_impl(cfg, a, E, offsets_host, workspace, workspace_bytes, num_sms, st, nullptr);
-}
-
-// sharq_prepare_linear: true when the one-launch path applies (otherwise the caller launches the two kernels)
-bool fused_prepare_linear_applies(const sharq_config* cfg, int64_t T, int64_t D, int64_t K, int32_t path) {
-  if (cfg->fmt == SHARQ_HIF4 || cfg->layout != SHARQ_LAYOUT_TILED || cfg->mask != SHARQ_MASK_PAIR48) return false;
-  if (cfg->norm != SHARQ_NORM_NONE && cfg->norm != SHARQ_NORM_RMS) return false;
-  if (T < 1 || T > 128 || K > 1024 * kMaxPrepWarps || path != 0) return false;
-  const int64_t warps = (K + 1023) / 1024;
-  const int64_t smem = warps * 1024 + 272 + (cfg->norm != SHARQ_NORM_NONE ? warps * 32 * 128 : 0);
-  return smem <= kPrepSmem && !debug_env().no_fused;
-}
-
-sharq_status launch_prepare_linear(const sharq_config* cfg, const void* x, int64_t ldx, const void* gamma,
-                                   const float* x_ts, const LinearArgs& a, int32_t* sync, int num_sms,
-                                   cudaStream_t st) {
-  FusedArgs fz{};
-  PrepParams& p = fz.pp;
-  p.x = (const uint16_t*)x; p.ldx = ldx; p.T = a.T; p.K = a.K;
-  p.gamma = (const uint16_t*)gamma; p.beta = nullptr; p.x_ts = x_ts;
-  p.sp_codes = (uint8_t*)a.sp_codes; p.sp_sf = (uint8_t*)a.sp_sf; p.sp_meta = (uint8_t*)a.sp_meta;
-  p.dn_codes = (uint8_t*)a.dn_codes; p.dn_sf = (uint8_t*)a.dn_sf; p.row_scale = (float*)a.row_scale;
-  p.eps = cfg->eps; p.tiled = 1; p.nbuf = 0; p.row_bytes = (uint32_t)(a.K * 2);
-  fz.sync = sync;
-  fz.norm = cfg->norm;
-  fz.warps = (int32_t)((a.K + 1023) / 1024);
-  return launch_linear_impl(cfg, a, 0, nullptr, nullptr, 0, num_sms, st, &fz);
-}
-
 }  // namespace sharq
