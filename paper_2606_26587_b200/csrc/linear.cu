@@ -944,12 +944,14 @@ sharq_status launch_tiles(const LinearArgs& a, const GroupInfo& g, int64_t rows_
             (int32_t)a.T, (int32_t)a.D, (int32_t)a.K, a.out_dtype, a.path, (int32_t)m_blocks, (int32_t)tiles, (int32_t)a_rows};
   const bool pair_worth = ((m_blocks + 1) / 2) * (a.D / 256) >= num_sms / 4 || debug_env().force_pair;
   if (E == 0 && m_blocks >= 2 && BN == 128 && pair_worth && !debug_env().no_pair) {
-    // tile width by a two-term cost model fitted on the box (us): rounds x (k-blocks x 0.43 + exposed
-    // epilogue), the epilogue being hidden by the second TMEM accumulator only for 192-wide tiles
+    // tile width by a cost model fitted on the box over the eight Llama / Qwen prefill shapes at T = 2048 ..
+    // 8192 (us per round of 74 tiles): 256-wide 0.54 per k-block + 4.5 (one TMEM accumulator: drain and pipeline
+    // refill exposed), 192-wide 0.50 per k-block + 1.5 (drain hidden by the second accumulator, but more
+    // activation re-reads per output, which costs on long K)
     const int64_t clusters = num_sms / 2, m_pairs = (m_blocks + 1) / 2;
-    const double per_kb = 0.43 * (double)(a.K / BK);
-    const double cost192 = (double)((m_pairs * ((a.D + 191) / 192) + clusters - 1) / clusters) * (per_kb + 0.3);
-    const double cost256 = (double)((m_pairs * ((a.D + 255) / 256) + clusters - 1) / clusters) * (per_kb + 2.0);
+    const double kb = (double)(a.K / BK);
+    const double cost192 = (double)((m_pairs * ((a.D + 191) / 192) + clusters - 1) / clusters) * (0.4975 * kb + 1.54);
+    const double cost256 = (double)((m_pairs * ((a.D + 255) / 256) + clusters - 1) / clusters) * (0.5375 * kb + 4.5);
     int width = (a.D % 256 != 0 || cost192 < cost256) ? 192 : 256;
     if (debug_env().pair_bn > 0) width = (debug_env().pair_bn == 256 && a.D % 256 == 0) ? 256 : 192;
     if (width == 256) return launch_pair<FMT, 256>(a, p, tm_sp, tm_dn, m_blocks, num_sms, st);
