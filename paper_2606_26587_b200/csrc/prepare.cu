@@ -176,6 +176,41 @@ __global__ void __launch_bounds__(MAXT, MINB) sharq_prepare_row_kernel(const Pre
 }
 
 template <int FMT>
+static cudaError_t launch_row_kernel(int norm, const PrepParams& p, int num_sms, cudaStream_t st);
+
+// The row kernel indexes with 32 bits: at most 2^31 / max(ldx, K) rows (a multiple of 128, so the tiled
+// layouts split at tile boundaries) per launch; larger problems run as several launches on row ranges.
+template <int FMT>
+static cudaError_t launch_row_chunks(int norm, const PrepParams& p0, int num_sms, cudaStream_t st) {
+  const int64_t widest = p0.ldx > p0.K ? p0.ldx : p0.K;
+  int64_t max_rows = ((int64_t(1) << 31) / widest) & ~int64_t(127);
+  if (debug_env().prep_chunk_rows > 0) max_rows = (int64_t)debug_env().prep_chunk_rows & ~int64_t(127);
+  if (max_rows < 128) return cudaErrorInvalidValue;
+  const int64_t K = p0.K;
+  for (int64_t r0 = 0; r0 < p0.T; r0 += max_rows) {
+    PrepParams p = p0;
+    p.T = (p0.T - r0 < max_rows) ? p0.T - r0 : max_rows;
+    p.x = p0.x + r0 * p0.ldx;
+    p.sp_codes = p0.sp_codes + r0 * (K >> 2);
+    p.dn_codes = p0.dn_codes + r0 * (K >> 1);
+    p.row_scale = p0.row_scale + r0;
+    if (FMT == SHARQ_HIF4) {                       // canonical only: metadata K/8 bytes, scale words K/64 per row
+      p.sp_meta = p0.sp_meta + r0 * (K >> 3);
+      p.sp_sf = p0.sp_sf + r0 * (K >> 6) * 4;
+      p.dn_sf = p0.dn_sf + r0 * (K >> 6) * 4;
+    } else {                                       // r0 % 128 == 0: both layouts advance by whole rows / tiles
+      const int64_t c_dn = (FMT == SHARQ_NVFP4) ? (K >> 4) : (K >> 5);
+      p.sp_meta = p0.sp_meta + r0 * (K >> 4);
+      p.sp_sf = p0.sp_sf + r0 * (K >> 5);
+      p.dn_sf = p0.dn_sf + r0 * c_dn;
+    }
+    const cudaError_t e = launch_row_kernel<FMT>(norm, p, num_sms, st);
+    if (e != cudaSuccess) return e;
+  }
+  return cudaSuccess;
+}
+
+template <int FMT>
 static cudaError_t launch_row_kernel(int norm, const PrepParams& p, int num_sms, cudaStream_t st) {
   const int warps = (int)((p.K + 1023) / 1024);
   const dim3 block((unsigned)warps * 32);
@@ -191,7 +226,8 @@ static cudaError_t launch_row_kernel(int norm, const PrepParams& p, int num_sms,
   attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
   attr[0].val.programmaticStreamSerializationAllowed = debug_env().no_pdl ? 0 : 1;
   lc.gridDim = grid; lc.blockDim = block; lc.stream = st; lc.attrs = attr; lc.numAttrs = 1;
-  lc.dynamicSmemBytes = (size_t)warps * 1024 + 256 + 16 + (norm != SHARQ_NORM_NONE ? (size_t)warps * 32 * 128 : 0);   // + gamma, beta
+  lc.dynamicSmemBytes = (size_t)warps * 1024 + 256 + 16 + 64                                           // leaves, amax, stat, mask table
+                        + (size_t)warps * 32 * (norm == SHARQ_NORM_LAYER ? 128 : norm == SHARQ_NORM_RMS ? 64 : 0);   // gamma, beta
   cudaError_t err = cudaSuccess;
 #define SHARQ_ROW(N, MAXT, MINB)                                                                              \
   do {                                                                                                        \
@@ -256,9 +292,9 @@ cudaError_t launch_prepare(const sharq_config* cfg, const void* x, int64_t T, in
   p.row_bytes = (uint32_t)(K * 2);
   if (K <= 1024 * kRowMaxWarps && !debug_env().old_prepare) {
     p.nbuf = 0;
-    if (cfg->fmt == SHARQ_NVFP4) return launch_row_kernel<SHARQ_NVFP4>(cfg->norm, p, num_sms, st);
-    if (cfg->fmt == SHARQ_MXFP4) return launch_row_kernel<SHARQ_MXFP4>(cfg->norm, p, num_sms, st);
-    return launch_row_kernel<SHARQ_HIF4>(cfg->norm, p, num_sms, st);
+    if (cfg->fmt == SHARQ_NVFP4) return launch_row_chunks<SHARQ_NVFP4>(cfg->norm, p, num_sms, st);
+    if (cfg->fmt == SHARQ_MXFP4) return launch_row_chunks<SHARQ_MXFP4>(cfg->norm, p, num_sms, st);
+    return launch_row_chunks<SHARQ_HIF4>(cfg->norm, p, num_sms, st);
   }
   // warps per CTA: as many double-buffered rows as fit in ~200 KB, else single-buffered
   const size_t budget = 200 * 1024;
