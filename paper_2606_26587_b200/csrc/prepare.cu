@@ -290,6 +290,7 @@ cudaError_t launch_prepare(const sharq_config* cfg, const void* x, int64_t T, in
   p.dn_codes = (uint8_t*)dn_codes; p.dn_sf = (uint8_t*)dn_sf; p.row_scale = row_scale;
   p.eps = cfg->eps; p.tiled = (cfg->layout == SHARQ_LAYOUT_TILED);
   p.row_bytes = (uint32_t)(K * 2);
+  p.idx_tags = 0x0004080Cu;
   if (K <= 1024 * kRowMaxWarps && !debug_env().old_prepare) {
     p.nbuf = 0;
     if (cfg->fmt == SHARQ_NVFP4) return launch_row_chunks<SHARQ_NVFP4>(cfg->norm, p, num_sms, st);
