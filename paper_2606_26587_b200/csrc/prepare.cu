@@ -172,7 +172,7 @@ __global__ void __launch_bounds__(MAXT, MINB) sharq_prepare_row_kernel(const Pre
   // inputs (and the operand buffers we overwrite) belong to the kernels before us
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   asm volatile("griddepcontrol.wait;" ::: "memory");
-  prepare_rows<FMT, NORM, 0>(p, row_smem, (int)threadIdx.x, (int)blockDim.x, (int64_t)blockIdx.x, (int64_t)gridDim.x);
+  prepare_rows<FMT, NORM, 0, (MAXT >= 512)>(p, row_smem, (int)threadIdx.x, (int)blockDim.x, (int64_t)blockIdx.x, (int64_t)gridDim.x);
 }
 
 template <int FMT>
@@ -227,7 +227,8 @@ static cudaError_t launch_row_kernel(int norm, const PrepParams& p, int num_sms,
   attr[0].val.programmaticStreamSerializationAllowed = debug_env().no_pdl ? 0 : 1;
   lc.gridDim = grid; lc.blockDim = block; lc.stream = st; lc.attrs = attr; lc.numAttrs = 1;
   lc.dynamicSmemBytes = (size_t)warps * 1024 + 256 + 16 + 64                                           // leaves, amax, stat, mask table
-                        + (size_t)warps * 32 * (norm == SHARQ_NORM_LAYER ? 128 : norm == SHARQ_NORM_RMS ? 64 : 0);   // gamma, beta
+                        + (size_t)warps * 32 * (norm == SHARQ_NORM_LAYER ? 128 : norm == SHARQ_NORM_RMS ? 64 : 0)    // gamma, beta
+                        + (FMT == SHARQ_NVFP4 && warps > 8 ? (size_t)warps * 32 * 128 + 512 + 16 : 0);   // lagged loop: parked row (2 stages), amax slots, mbarriers
   cudaError_t err = cudaSuccess;
 #define SHARQ_ROW(N, MAXT, MINB)                                                                              \
   do {                                                                                                        \
