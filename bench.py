@@ -469,12 +469,13 @@ def prefill_extras(sq, wl, pk, steps):
         reps = [lambda j=j: sq.prepare(wl.cfg[n], xs[j], wl.gamma[K] if norm else None, out=acts[j]) for j in range(3)]
         ms = timed(reps, max(steps, 12), 3, lambda: None)
         gbs = prepare_bytes(Tp, K) / (ms * 1e-3) / 1e9
-        # the kernel is ALU / issue bound, not HBM bound (profiles/prepare_r1_ncu_full.md, final capture:
-        # smsp__inst_executed x 32 / elements = 31.4 thread-instructions per element with RMSNorm, 24.3 without;
+        # the kernel is ALU / issue bound, not HBM bound (profiles/prepare_r1_ncu_full.md, last capture:
+        # smsp__inst_executed x 32 / elements = 25.3 thread-instructions per element with RMSNorm (K = 4096),
+        # 20.5 without (K = 14336, lagged loop);
         # DRAM traffic = algorithmic bytes): second roofline = issue slots, 148 SMs x 4 schedulers x 32 lanes
         # x 1.965 GHz
         issue_peak = 148 * 128 * 1.965e9
-        ipe = 31.4 if norm else 24.3
+        ipe = 25.3 if norm else 20.5
         out["prepare"][f"T{Tp}_K{K}_{'rms' if norm else 'none'}"] = dict(
             us=round(ms * 1e3, 1), GBps=round(gbs, 1), frac_of_hbm=round(gbs / pk["hbm"], 4),
             alu=dict(bound="alu", achieved=round(Tp * K * ipe / (ms * 1e-3) / 1e12, 2), peak=round(issue_peak / 1e12, 2),
