@@ -112,3 +112,30 @@ def test_prepare_full_size_sampled_rows(sq):
         rows[:3] = (0, T - 1, T // 2)
         p = so.prepare(x[rows], norm=norm, gamma_u16=g)
         _compare_act({k: v[rows] for k, v in got.items()}, p, f"full T{T} K{K}")
+
+
+@pytest.mark.parametrize("T,K,norm,static_ts,layout", [
+    (3000, 9216, 1, None, 1),        # 9 warps per row: lagged loop, RMSNorm, 3 rows per CTA
+    (2500, 18944, 2, None, 0),       # 19 warps, LayerNorm, canonical layout, 5-6 rows per CTA
+    (2500, 14336, 0, 0.0625, 1),     # lagged loop without the row-amax exchange (static tensor scale)
+    (5000, 8192, 1, None, 1),        # 8 warps: the widest row of the blocking loop, several rows per CTA
+])
+def test_prepare_many_rows_per_cta_sampled(sq, T, K, norm, static_ts, layout):
+    """More rows than CTAs, so every CTA runs several iterations of the software-pipelined row loop (next row
+    fetched inside the tail; for K > 8192 the lagged loop whose row-amax exchange is waited for one iteration
+    later).  Rows are independent: the oracle recomputes a seeded sample, first and last rows included."""
+    x = si.activations(T, K, config=2, outlier_mult=50.0, extra=T + K)
+    g, b = si.gamma(K, 2), si.beta(K, 2)
+    cfg = sq.make_config(0, norm, 1e-6, layout)
+    ts = None if static_ts is None else torch.tensor([static_ts], dtype=torch.float32, device="cuda")
+    act = sq.prepare(cfg, to_dev(x), to_dev(g) if norm else None, to_dev(b) if norm == 2 else None, x_tensor_scale=ts)
+    torch.cuda.synchronize()
+    got = act_to_canonical(sq, cfg, act, T, K)
+    rows = np.random.default_rng(T + K).choice(T, 40, replace=False)
+    rows[:4] = (0, 1, T - 1, T - 2)
+    p = so.prepare(x[rows], norm=norm, gamma_u16=g if norm else None, beta_u16=b if norm == 2 else None,
+                   x_tensor_scale=static_ts)
+    _compare_act({k: v[rows] for k, v in got.items()}, p, f"T{T} K{K} norm{norm}")
+    # rows outside the sample: every pair-4:8 metadata nibble is one of the six valid codes (no stale tile bytes)
+    nib = np.concatenate([got["sp_meta"] & 0xF, got["sp_meta"] >> 4], axis=1)
+    assert np.isin(nib, [0x4, 0x8, 0xC, 0x9, 0xD, 0xE]).all()
