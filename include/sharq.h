@@ -111,6 +111,24 @@ sharq_status sharq_prepare(const sharq_config* cfg, const void* x, int64_t T, in
                            void* sp_meta, void* dn_codes, void* dn_sf, float* row_scale,
                            void* stream);
 
+/* ---- sharq_prepare_add (the paper's own lever was folding the
+ * neighbouring elementwise operator into the preparation kernel) ----------------------------
+ * sharq_prepare with the transformer's residual-stream add fused in front of the norm:
+ *     h[t,k] = bf16( x[t,k] + residual[t,k] )      one rounding of the exact sum, ties to even
+ * h is written to sum_out (bf16 [T,K], ldo elements between rows: the new residual stream) and is the
+ * activation that norm -> mask -> backbone -> residual -> stores see; every output is exactly what
+ * sharq_prepare would produce from h.  sum_out may alias residual (in-place stream update: each
+ * element is read and written by the same thread) but not x.  One kernel, one pass: 2 + 2 B/element
+ * more HBM traffic than sharq_prepare, against a separate add kernel's 6 B/element plus a launch.
+ * x, residual, sum_out: 32-byte aligned, ldx / ldr / ldo multiples of 16 (256-bit accesses), else
+ * SHARQ_EINVAL / SHARQ_ESHAPE; K <= 32768 (one row per CTA), else SHARQ_ESHAPE. */
+sharq_status sharq_prepare_add(const sharq_config* cfg, const void* x, const void* residual,
+                               int64_t T, int64_t K, int64_t ldx, int64_t ldr, void* sum_out,
+                               int64_t ldo, const void* gamma, const void* beta,
+                               const float* x_tensor_scale, void* sp_codes, void* sp_sf,
+                               void* sp_meta, void* dn_codes, void* dn_sf, float* row_scale,
+                               void* stream);
+
 /* ---- sharq_linear (Eq. 9) -----------------------------------------------
  * Y[T,D] = (A_sp . W^T through the sparse view  +  A_dn . W^T through the dense view)
  *          * row_scale[t] * w_tensor_scale  (+ bias[d])

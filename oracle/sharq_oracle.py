@@ -71,6 +71,16 @@ def _bf16_add(a_u16, b_u16):
     return f32_to_bf16(bf16_to_f32(a_u16) + bf16_to_f32(b_u16))
 
 
+def residual_add(x_u16, r_u16):
+    """h = bf16(x + r): the transformer's residual-stream add that `sharq_prepare_add` folds in front of the
+    norm (the paper's own lever is folding the neighbouring elementwise operator into the
+    preparation kernel).  ONE rounding of the exact sum, ties to even.  Computed as an fp32 add
+    followed by RNE to bf16; the two roundings equal one: the fp32 add only rounds when the smaller addend lies
+    below 2^-16 of the larger, far from any bf16 tie point of the larger (pinned against exact rationals in
+    tests/test_oracle_path.py)."""
+    return _bf16_add(np.asarray(x_u16, dtype=U16), np.asarray(r_u16, dtype=U16))
+
+
 # --------------------------------------------------------------------------------------------
 # element / scale codecs
 # --------------------------------------------------------------------------------------------

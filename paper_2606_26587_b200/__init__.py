@@ -57,6 +57,7 @@ def _load() -> ctypes.CDLL:
     lib.sharq_linear_workspace.argtypes = [CFG, c_int64, c_int64, c_int64, c_int32, SZ]
     lib.sharq_quantize_weight.argtypes = [CFG, P, c_int64, c_int64, c_int64, P, P, P, P, P, c_size_t, P]
     lib.sharq_prepare.argtypes = [CFG, P, c_int64, c_int64, c_int64, P, P, P, P, P, P, P, P, P, P]
+    lib.sharq_prepare_add.argtypes = [CFG, P, P, c_int64, c_int64, c_int64, c_int64, P, c_int64, P, P, P, P, P, P, P, P, P, P]
     lib.sharq_linear.argtypes = [CFG, c_int64, c_int64, c_int64, P, P, P, P, P, P, P, P, P, P, P, P, c_int64,
                                  c_int32, c_int32, P, c_size_t, P]
     lib.sharq_linear_grouped.argtypes = [CFG, c_int32, POINTER(c_int32), c_int64, c_int64, P, P, P, P, P, P, P, P,
@@ -64,14 +65,14 @@ def _load() -> ctypes.CDLL:
     lib.sharq_mma_peak_launch.argtypes = [c_int32, c_int32, P]
     lib.sharq_mma_peak_launch.restype = c_int32
     for name in ("sharq_weight_sizes", "sharq_act_sizes", "sharq_linear_workspace", "sharq_quantize_weight",
-                 "sharq_prepare", "sharq_linear", "sharq_linear_grouped"):
+                 "sharq_prepare", "sharq_prepare_add", "sharq_linear", "sharq_linear_grouped"):
         getattr(lib, name).restype = c_int32
     return lib
 
 
 capi = _load()
 EXPORTS = ("sharq_version", "sharq_weight_sizes", "sharq_act_sizes", "sharq_linear_workspace",
-           "sharq_quantize_weight", "sharq_prepare", "sharq_linear", "sharq_linear_grouped",
+           "sharq_quantize_weight", "sharq_prepare", "sharq_prepare_add", "sharq_linear", "sharq_linear_grouped",
            "sharq_mma_peak_launch")
 
 
@@ -158,6 +159,21 @@ def prepare(cfg: Config, x, gamma=None, beta=None, x_tensor_scale=None, out=None
                               _ptr(out["dn_codes"]), _ptr(out["dn_sf"]), _ptr(out["row_scale"]), _stream()),
            "sharq_prepare")
     return out
+
+
+def prepare_add(cfg: Config, x, residual, gamma=None, beta=None, x_tensor_scale=None, out=None, sum_out=None):
+    """sharq_prepare_add: h = bf16(x + residual) written to sum_out (default: in place over `residual`), then the
+    preparation path on h.  Returns (act, sum_out)."""
+    T, K = x.shape
+    if out is None:
+        out = alloc_act(cfg, T, K, x.device)
+    if sum_out is None:
+        sum_out = residual
+    _check(capi.sharq_prepare_add(ctypes.byref(cfg), _ptr(x), _ptr(residual), T, K, x.stride(0), residual.stride(0),
+                                  _ptr(sum_out), sum_out.stride(0), _ptr(gamma), _ptr(beta), _ptr(x_tensor_scale),
+                                  _ptr(out["sp_codes"]), _ptr(out["sp_sf"]), _ptr(out["sp_meta"]), _ptr(out["dn_codes"]),
+                                  _ptr(out["dn_sf"]), _ptr(out["row_scale"]), _stream()), "sharq_prepare_add")
+    return out, sum_out
 
 
 def act_slot(cfg: Config, act: dict, row0: int, T: int) -> dict:

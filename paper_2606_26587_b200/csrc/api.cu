@@ -8,7 +8,7 @@ namespace sharq {
 cudaError_t launch_prepare(const sharq_config* cfg, const void* x, int64_t T, int64_t K, int64_t ldx,
                            const void* gamma, const void* beta, const float* x_ts, void* sp_codes, void* sp_sf,
                            void* sp_meta, void* dn_codes, void* dn_sf, float* row_scale, int num_sms,
-                           cudaStream_t st);
+                           cudaStream_t st, const void* residual, int64_t ldr, void* sum_out, int64_t ldo);
 cudaError_t launch_quantize_weight(const sharq_config* cfg, const void* W, int64_t D, int64_t K, int64_t ldw,
                                    void* codes, void* sf_sp, void* sf_dn, float* ts, void* workspace,
                                    cudaStream_t st);
@@ -140,7 +140,31 @@ sharq_status sharq_prepare(const sharq_config* cfg, const void* x, int64_t T, in
   DeviceInfo di{};
   if ((s = device_info(&di)) != SHARQ_OK) return s;
   cudaError_t e = launch_prepare(cfg, x, T, K, ldx, gamma, beta, x_tensor_scale, sp_codes, sp_sf, sp_meta, dn_codes,
-                                 dn_sf, row_scale, di.sms, (cudaStream_t)stream);
+                                 dn_sf, row_scale, di.sms, (cudaStream_t)stream, nullptr, 0, nullptr, 0);
+  return e == cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
+}
+
+sharq_status sharq_prepare_add(const sharq_config* cfg, const void* x, const void* residual, int64_t T, int64_t K,
+                               int64_t ldx, int64_t ldr, void* sum_out, int64_t ldo, const void* gamma,
+                               const void* beta, const float* x_tensor_scale, void* sp_codes, void* sp_sf,
+                               void* sp_meta, void* dn_codes, void* dn_sf, float* row_scale, void* stream) {
+  sharq_status s = check_cfg(cfg);
+  if (s != SHARQ_OK) return s;
+  if (T < 0 || K <= 0 || K % 256 != 0 || K > 32768) return SHARQ_ESHAPE;
+  if (ldx < K || ldr < K || ldo < K || ldx % 16 != 0 || ldr % 16 != 0 || ldo % 16 != 0) return SHARQ_ESHAPE;
+  if (T == 0) return SHARQ_OK;
+  if (!x || !residual || !sum_out || !sp_codes || !sp_sf || !sp_meta || !dn_codes || !dn_sf || !row_scale) return SHARQ_EINVAL;
+  if (cfg->norm != SHARQ_NORM_NONE && !gamma) return SHARQ_EINVAL;
+  auto aligned32 = [](const void* q) { return ((uintptr_t)q & 31u) == 0; };
+  if (!aligned32(x) || !aligned32(residual) || !aligned32(sum_out)) return SHARQ_EINVAL;
+  if (!aligned16(sp_codes) || !aligned16(sp_sf) || !aligned16(sp_meta) || !aligned16(dn_codes) || !aligned16(dn_sf) ||
+      (gamma && !aligned16(gamma)) || (beta && !aligned16(beta)))
+    return SHARQ_EINVAL;
+  if (sum_out == x) return SHARQ_EINVAL;   // x is re-read by the software pipeline one row ahead; residual may alias sum_out
+  DeviceInfo di{};
+  if ((s = device_info(&di)) != SHARQ_OK) return s;
+  cudaError_t e = launch_prepare(cfg, x, T, K, ldx, gamma, beta, x_tensor_scale, sp_codes, sp_sf, sp_meta, dn_codes,
+                                 dn_sf, row_scale, di.sms, (cudaStream_t)stream, residual, ldr, sum_out, ldo);
   return e == cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
 }
 

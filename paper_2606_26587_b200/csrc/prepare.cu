@@ -182,7 +182,8 @@ static cudaError_t launch_row_kernel(int norm, const PrepParams& p, int num_sms,
 // layouts split at tile boundaries) per launch; larger problems run as several launches on row ranges.
 template <int FMT>
 static cudaError_t launch_row_chunks(int norm, const PrepParams& p0, int num_sms, cudaStream_t st) {
-  const int64_t widest = p0.ldx > p0.K ? p0.ldx : p0.K;
+  int64_t widest = p0.ldx > p0.K ? p0.ldx : p0.K;
+  if (p0.res) { if (p0.ldr > widest) widest = p0.ldr; if (p0.ldo > widest) widest = p0.ldo; }
   int64_t max_rows = ((int64_t(1) << 31) / widest) & ~int64_t(127);
   if (debug_env().prep_chunk_rows > 0) max_rows = (int64_t)debug_env().prep_chunk_rows & ~int64_t(127);
   if (max_rows < 128) return cudaErrorInvalidValue;
@@ -191,6 +192,7 @@ static cudaError_t launch_row_chunks(int norm, const PrepParams& p0, int num_sms
     PrepParams p = p0;
     p.T = (p0.T - r0 < max_rows) ? p0.T - r0 : max_rows;
     p.x = p0.x + r0 * p0.ldx;
+    if (p0.res) { p.res = p0.res + r0 * p0.ldr; p.sum_out = p0.sum_out + r0 * p0.ldo; }
     p.sp_codes = p0.sp_codes + r0 * (K >> 2);
     p.dn_codes = p0.dn_codes + r0 * (K >> 1);
     p.row_scale = p0.row_scale + r0;
@@ -283,8 +285,9 @@ static cudaError_t launch_norm(int norm, const PrepParams& p, dim3 grid, dim3 bl
 cudaError_t launch_prepare(const sharq_config* cfg, const void* x, int64_t T, int64_t K, int64_t ldx,
                            const void* gamma, const void* beta, const float* x_ts, void* sp_codes, void* sp_sf,
                            void* sp_meta, void* dn_codes, void* dn_sf, float* row_scale, int num_sms,
-                           cudaStream_t st) {
+                           cudaStream_t st, const void* residual, int64_t ldr, void* sum_out, int64_t ldo) {
   PrepParams p;
+  p.res = (const uint16_t*)residual; p.sum_out = (uint16_t*)sum_out; p.ldr = ldr; p.ldo = ldo;
   p.x = (const uint16_t*)x; p.ldx = ldx; p.T = T; p.K = K;
   p.gamma = (const uint16_t*)gamma; p.beta = (const uint16_t*)beta; p.x_ts = x_ts;
   p.sp_codes = (uint8_t*)sp_codes; p.sp_sf = (uint8_t*)sp_sf; p.sp_meta = (uint8_t*)sp_meta;
@@ -292,7 +295,11 @@ cudaError_t launch_prepare(const sharq_config* cfg, const void* x, int64_t T, in
   p.eps = cfg->eps; p.tiled = (cfg->layout == SHARQ_LAYOUT_TILED);
   p.row_bytes = (uint32_t)(K * 2);
   p.idx_tags = 0x0004080Cu;
-  if (K <= 1024 * kRowMaxWarps && !debug_env().old_prepare) {
+  // the row kernel reads 32 bytes per load: rows must start on 32-byte boundaries, otherwise (16-byte aligned
+  // input, the C ABI's minimum) the warp-per-row kernel with its 16-byte cp.async takes the call
+  const bool wide_ok = ((uintptr_t)x % 32 == 0) && (ldx % 16 == 0);
+  if (residual && (!wide_ok || K > 1024 * kRowMaxWarps)) return cudaErrorInvalidValue;   // checked by the C ABI
+  if (K <= 1024 * kRowMaxWarps && wide_ok && (!debug_env().old_prepare || residual)) {
     p.nbuf = 0;
     if (cfg->fmt == SHARQ_NVFP4) return launch_row_chunks<SHARQ_NVFP4>(cfg->norm, p, num_sms, st);
     if (cfg->fmt == SHARQ_MXFP4) return launch_row_chunks<SHARQ_MXFP4>(cfg->norm, p, num_sms, st);

@@ -139,3 +139,50 @@ def test_prepare_many_rows_per_cta_sampled(sq, T, K, norm, static_ts, layout):
     # rows outside the sample: every pair-4:8 metadata nibble is one of the six valid codes (no stale tile bytes)
     nib = np.concatenate([got["sp_meta"] & 0xF, got["sp_meta"] >> 4], axis=1)
     assert np.isin(nib, [0x4, 0x8, 0xC, 0x9, 0xD, 0xE]).all()
+
+
+@pytest.mark.parametrize("fmt,norm,T,K,inplace", [
+    (0, 1, 16, 4096, True),          # configs[0] shape: residual add + RMSNorm, in-place stream update
+    (0, 1, 2100, 4096, False),       # several rows per CTA, blocking loop
+    (0, 2, 700, 14336, True),        # lagged loop, LayerNorm
+    (1, 1, 33, 3584, False),         # MXFP4, ragged K
+    (2, 0, 9, 768, True),            # HiF4, no norm
+])
+def test_prepare_add_bit_exact(sq, fmt, norm, T, K, inplace):
+    """sharq_prepare_add: the new residual stream equals the oracle's bf16(x + r) bit for bit and
+    every prepared output equals the oracle's preparation of that sum."""
+    x = si.activations(T, K, config=4, outlier_mult=50.0, extra=T)
+    r = si.activations(T, K, config=5, outlier_mult=10.0, extra=K)
+    g, b = si.gamma(K, 4), si.beta(K, 4)
+    cfg = sq.make_config(fmt, norm, 1e-6, sq.LAYOUT_CANONICAL if fmt == 2 else sq.LAYOUT_TILED)
+    xd, rd = to_dev(x), to_dev(r)
+    out = None if inplace else torch.empty_like(rd)
+    act, h_dev = sq.prepare_add(cfg, xd, rd, to_dev(g) if norm else None, to_dev(b) if norm == 2 else None, sum_out=out)
+    torch.cuda.synchronize()
+    h = so.residual_add(x, r)
+    assert np.array_equal(h_dev.view(torch.int16).cpu().numpy().view(np.uint16), h), "residual stream"
+    if not inplace:
+        assert np.array_equal(rd.view(torch.int16).cpu().numpy().view(np.uint16), r), "residual input was modified"
+    rows = np.arange(T) if T * K <= 600_000 else np.unique(np.r_[0, 1, T - 1, np.random.default_rng(T).choice(T, 40, replace=False)])
+    p = so.prepare(h[rows], fmt=fmt, mask=cfg.mask, norm=norm, gamma_u16=g if norm else None, beta_u16=b if norm == 2 else None)
+    got = act_to_canonical(sq, cfg, act, T, K)
+    _compare_act({k: v[rows] for k, v in got.items()}, p, f"add fmt{fmt} norm{norm} T{T} K{K}")
+
+
+def test_prepare_rows_not_32_byte_aligned(sq):
+    """The C ABI asks for 16-byte alignment only; the row kernel reads 32 bytes per load, so rows that start on an
+    odd 16-byte boundary are served by the warp-per-row kernel.  Same bytes out."""
+    T, K = 19, 2048
+    x = si.activations(T, K, config=1, extra=7)
+    g = si.gamma(K, 1)
+    cfg = sq.make_config(0, sq.NORM_RMS, 1e-6, sq.LAYOUT_TILED)
+    buf = torch.zeros((T * (K + 8) + 8,), dtype=torch.bfloat16, device="cuda")
+    view = buf[8:].view(T, K + 8)[:, :K]                    # base + 16 bytes, ldx = K + 8
+    view.copy_(to_dev(x))
+    assert view.data_ptr() % 32 == 16
+    act = sq.prepare(cfg, view, to_dev(g))
+    torch.cuda.synchronize()
+    p = so.prepare(x, gamma_u16=g)
+    _compare_act(act_to_canonical(sq, cfg, act, T, K), p, "misaligned")
+    with pytest.raises(sq.SharqError):
+        sq.prepare_add(cfg, view, to_dev(x), to_dev(g))

@@ -231,3 +231,50 @@ def test_qualitative_ordering_of_path_combinations():
     e_dense = n(so.dequant_residual(p0) - Xf) / n(Xf)
     e_sharq = n(so.dequant_backbone(p) + so.dequant_residual(p) - Xf) / n(Xf)
     assert e_sparse > 2 * e_dense and e_dense > 2 * e_sharq
+
+
+def _nearest_bf16_exact(v: Fraction) -> int:
+    """Nearest bf16 bit pattern of an exact rational (ties to even), by brute force over the two neighbours."""
+    if v == 0:
+        return 0
+    sign = 0x8000 if v < 0 else 0
+    a = abs(v)
+    e = math.floor(math.log2(float(a))) if a >= Fraction(1, 2 ** 120) else -126
+    while Fraction(2) ** e > a:
+        e -= 1
+    while Fraction(2) ** (e + 1) <= a:
+        e += 1
+    e = max(e, -126)                                   # subnormals share the spacing of the lowest binade
+    ulp = Fraction(2) ** (e - 7)
+    q, r = divmod(a, ulp)
+    q = int(q)
+    if r * 2 > ulp or (r * 2 == ulp and (q & 1)):
+        q += 1
+    val = q * ulp
+    bits = int(np.float32(float(val)).view(np.uint32)) >> 16      # val is a bf16 value: exact in fp32
+    return sign | bits
+
+
+def test_residual_add_is_one_rounding_of_the_exact_sum():
+    """sharq_prepare_add's h = bf16(x + r): the oracle's fp32 add + RNE equals the exactly
+    rounded rational sum, on random pairs and on pairs built to stress the double rounding (exponent gaps of
+    8..24 around tie points) and cancellation."""
+    rng = np.random.default_rng(26587)
+    a = si.to_bf16_bits((rng.standard_normal(3000) * 10.0 ** rng.integers(-6, 6, 3000)).astype(np.float32))
+    b = si.to_bf16_bits((rng.standard_normal(3000) * 10.0 ** rng.integers(-6, 6, 3000)).astype(np.float32))
+    # adversarial: big = 1.xxxxxxx * 2^0, small = +-(2^-8 +- 2^-k), +-2^-9 ..., and near cancellation
+    big = (0x3F80 + rng.integers(0, 128, 600)).astype(np.uint16)
+    gaps = rng.integers(8, 26, 600)
+    small_f = np.ldexp(1.0, -gaps) * rng.choice([1.0, -1.0, 1.5, -1.5, 1.0078125, 0.9921875], 600)
+    small = si.to_bf16_bits(small_f.astype(np.float32))
+    a = np.concatenate([a, big, big, np.array([0x0001, 0x8001, 0x0080, 0x7F7F], np.uint16)])
+    b = np.concatenate([b, small, (big ^ 0x8000) + rng.integers(0, 3, 600).astype(np.uint16),
+                        np.array([0x0001, 0x0001, 0x8001, 0x0000], np.uint16)])
+    got = so.residual_add(a, b)
+    fa, fb = si.bf16_bits_to_f32(a), si.bf16_bits_to_f32(b)
+    for i in range(a.size):
+        exact = Fraction(float(fa[i])) + Fraction(float(fb[i]))
+        want = _nearest_bf16_exact(exact)
+        if exact == 0:                                 # x + (-x) = +0 under round-to-nearest
+            want = 0x8000 if (a[i] & 0x8000 and b[i] & 0x8000) else 0
+        assert int(got[i]) == want, (hex(a[i]), hex(b[i]), hex(got[i]), hex(want))
