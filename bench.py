@@ -482,6 +482,26 @@ def prefill_extras(sq, wl, pk, steps):
                      unit="T thread-instructions/s", frac=round(Tp * K * ipe / (ms * 1e-3) / issue_peak, 4),
                      instr_per_element=ipe))
         del xs, acts
+    # residual-stream add fused into the preparation (sharq_prepare_add) against the same work
+    # as two launches (a bf16 add kernel, then sharq_prepare).  Algorithmic bytes of the fused pass: the prepare
+    # bytes + 2 (residual read) + 2 (new stream written) per element.
+    Tp, K = 8192, 4096
+    xs = [device_activations(Tp, K, BASE_SEED + 90 + j) for j in range(3)]
+    rs = [device_activations(Tp, K, BASE_SEED + 95 + j, outlier_mult=10.0) for j in range(3)]
+    acts = [sq.alloc_act(wl.cfg["qkv"], Tp, K, "cuda") for _ in xs]
+    fused = [lambda j=j: sq.prepare_add(wl.cfg["qkv"], xs[j], rs[j], wl.gamma[K], out=acts[j]) for j in range(3)]
+    ms_f = timed(fused, max(steps, 12), 3, lambda: None)
+
+    def unfused(j):
+        rs[j].add_(xs[j])
+        sq.prepare(wl.cfg["qkv"], rs[j], wl.gamma[K], out=acts[j])
+    ms_u = timed([lambda j=j: unfused(j) for j in range(3)], max(steps, 12), 3, lambda: None)
+    by = prepare_bytes(Tp, K) + 4.0 * Tp * K
+    out["prepare_add"] = {f"T{Tp}_K{K}_rms": dict(us=round(ms_f * 1e3, 1), GBps=round(by / (ms_f * 1e-3) / 1e9, 1),
+                                               frac_of_hbm=round(by / (ms_f * 1e-3) / 1e9 / pk["hbm"], 4),
+                                               unfused_us=round(ms_u * 1e3, 1),
+                                               unfused_note="torch bf16 add_ kernel + sharq_prepare (two launches)")}
+    del xs, rs, acts
     return out
 
 
