@@ -54,6 +54,16 @@ def test_argument_validation_returns_codes_without_touching_cuda(sq):
     assert f(ctypes.byref(cfg), 16, 4, 1024, 1024, 16, null, null, null, 16, 16, 16, 16, 16, null) == sq.EINVAL
     # misaligned pointer
     assert f(ctypes.byref(cfg), 8, 4, 1024, 1024, 16, null, null, 16, 16, 16, 16, 16, 16, null) == sq.EINVAL
+    # sharq_prepare_add: (cfg, x, residual, T, K, ldx, ldr, sum_out, ldo, gamma, beta, x_ts, 6 outputs, stream)
+    g = sq.capi.sharq_prepare_add
+    ok_ptrs = [32] * 9                                    # gamma, beta, x_ts, sp_codes ... row_scale
+    assert g(ctypes.byref(cfg), 32, 64, 0, 1024, 1024, 1024, 96, 1024, *ok_ptrs, null) == sq.OK          # T == 0
+    assert g(ctypes.byref(cfg), 32, 64, 4, 1000, 1008, 1008, 96, 1008, *ok_ptrs, null) == sq.ESHAPE      # K % 256
+    assert g(ctypes.byref(cfg), 32, 64, 4, 1024, 1032, 1024, 96, 1024, *ok_ptrs, null) == sq.ESHAPE      # ldx % 16
+    assert g(ctypes.byref(cfg), 32, 64, 4, 33792, 33792, 33792, 96, 33792, *ok_ptrs, null) == sq.ESHAPE  # K > 32768
+    assert g(ctypes.byref(cfg), 16, 64, 4, 1024, 1024, 1024, 96, 1024, *ok_ptrs, null) == sq.EINVAL      # x 16-byte aligned only
+    assert g(ctypes.byref(cfg), 32, null, 4, 1024, 1024, 1024, 96, 1024, *ok_ptrs, null) == sq.EINVAL    # no residual
+    assert g(ctypes.byref(cfg), 32, 64, 4, 1024, 1024, 1024, 32, 1024, *ok_ptrs, null) == sq.EINVAL      # sum_out aliases x
     # element-wise 2:4 with NVFP4 has no tensor-core path on B200 (R2)
     bad = sq.Config(sq.NVFP4, sq.MASK_24, sq.NORM_NONE, 1e-6, sq.LAYOUT_TILED)
     with pytest.raises(sq.SharqError):
