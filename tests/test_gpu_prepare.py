@@ -119,6 +119,7 @@ def test_prepare_full_size_sampled_rows(sq):
     (2500, 18944, 2, None, 0),       # 19 warps, LayerNorm, canonical layout, 5-6 rows per CTA
     (2500, 14336, 0, 0.0625, 1),     # lagged loop without the row-amax exchange (static tensor scale)
     (5000, 8192, 1, None, 1),        # 8 warps: the widest row of the blocking loop, several rows per CTA
+    (500, 32768, 1, None, 1),        # 32 warps (the widest one-CTA row), lagged loop, two rows in most CTAs
 ])
 def test_prepare_many_rows_per_cta_sampled(sq, T, K, norm, static_ts, layout):
     """More rows than CTAs, so every CTA runs several iterations of the software-pipelined row loop (next row
