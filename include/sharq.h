@@ -6,6 +6,8 @@
  *   sharq_quantize_weight  offline, once per weight: one FP4 payload + two scale views
  *   sharq_prepare          per call: norm -> N:M mask -> sparse FP4 backbone -> residual -> dense FP4
  *   sharq_linear           sparse + dense block-scaled FP4 GEMMs into one accumulator, bf16 epilogue
+ * plus sharq_linear_grouped (the same over the row ranges of E experts, MoE) and sharq_prepare_add
+ * (sharq_prepare with the residual-stream add fused in front of the norm).
  *
  * Conventions
  *   - The caller owns every buffer; the library never allocates device memory and keeps no
@@ -14,6 +16,8 @@
  *     and the call returns without synchronising.
  *   - Errors are return codes; nothing throws or aborts.  On a non-OK return nothing was launched.
  *   - Sizes are int64_t, leading dimensions are in ELEMENTS, base pointers 16-byte aligned.
+ *     (sharq_prepare is fastest when x is 32-byte aligned with ldx % 16 == 0: rows that start on an odd
+ *     16-byte boundary are served by a slower kernel, same results.)
  *   - bf16 tensors are row-major; "code" tensors hold two 4-bit codes per byte, the element
  *     with the lower k in the low nibble.
  *   - Shapes: K % 256 == 0 (8-chunks, 32/64 scale groups, MMA-K 128, 256-wide metadata tile),
