@@ -278,3 +278,125 @@ def test_residual_add_is_one_rounding_of_the_exact_sum():
         if exact == 0:                                 # x + (-x) = +0 under round-to-nearest
             want = 0x8000 if (a[i] & 0x8000 and b[i] & 0x8000) else 0
         assert int(got[i]) == want, (hex(a[i]), hex(b[i]), hex(got[i]), hex(want))
+
+
+# ------------------------------------------------------------------ O1 LayerNorm branch (R3)
+def _rne_bf16_fraction(v: Fraction) -> Fraction:
+    """Nearest bf16 value (8 significant bits, ties to the even significand) of an exact rational, by search."""
+    if v == 0:
+        return Fraction(0)
+    s, a = (-1 if v < 0 else 1), abs(v)
+    e = 0
+    while Fraction(2) ** (e + 1) <= a:
+        e += 1
+    while Fraction(2) ** e > a:
+        e -= 1
+    q = Fraction(2) ** (e - 7)                       # spacing of the bf16 grid in [2^e, 2^(e+1))
+    n = a / q
+    lo = n.numerator // n.denominator
+    r = n - lo
+    if r > Fraction(1, 2) or (r == Fraction(1, 2) and lo % 2 == 1):
+        lo += 1
+    return s * lo * q
+
+
+def _layernorm_fp64(x_u16, g_u16, b_u16, eps, variant="paper"):
+    """fp64 ((x - mu) / sqrt(var + eps)) * gamma + beta (P:155 'LayerNorm'), and the plausible mistakes the pin
+    must reject: beta sign flipped, beta added before gamma, unbiased (N - 1) variance."""
+    xf = so.bf16_to_f32(x_u16).astype(np.float64)
+    g = so.bf16_to_f32(g_u16).astype(np.float64)
+    b = so.bf16_to_f32(b_u16).astype(np.float64)
+    mu = xf.mean(1, keepdims=True)
+    N = xf.shape[1]
+    var = ((xf - mu) ** 2).sum(1, keepdims=True) / (N - 1 if variant == "nm1" else N)
+    n = (xf - mu) / np.sqrt(var + eps)
+    if variant == "beta_sign":
+        return n * g - b, n * g
+    if variant == "beta_first":
+        return (n + b) * g, n * g
+    return n * g + b, n * g
+
+
+@pytest.mark.parametrize("K", [16, 256, 1024])
+def test_layernorm_against_fp64_with_affine_and_mutations(K):
+    """gamma != 1, beta != 0: the oracle's LayerNorm branch stays inside the three-bf16-rounding error bound of the
+    fp64 definition on EVERY element, and each plausible mistake (beta sign, beta before gamma, N - 1 variance, at
+    K = 16 where it moves every element by 3 %) violates the same bound on the same data, so the pin does discriminate."""
+    rng = np.random.default_rng(K)
+    x = so.f32_to_bf16((rng.standard_normal((6, K)) * 3 + 5).astype(F32))
+    g = so.f32_to_bf16((rng.random(K) + 0.5).astype(F32))
+    b = so.f32_to_bf16(rng.standard_normal(K).astype(F32))
+    eps = 1e-6
+    X = so.bf16_to_f32(so.normalize(x, so.NORM_LAYER, g, b, eps)).astype(np.float64)
+
+    def within(ref, ng):
+        # h = bf16(c*rstd), v = bf16(h*gamma): 2 x 2^-8 relative on |n*gamma| (+ fp32 slack); final bf16(v + beta):
+        # 2^-8 relative on the result
+        bound = np.abs(ng) * (2.0 ** -7 + 2.0 ** -14) + (np.abs(ref) + np.abs(ng) * 2.0 ** -7) * 2.0 ** -8 + 1e-30
+        return np.abs(X - ref) <= bound
+
+    ref, ng = _layernorm_fp64(x, g, b, eps)
+    assert within(ref, ng).all()
+    for variant in ("beta_sign", "beta_first") + (("nm1",) if K == 16 else ()):
+        bad, ng_bad = _layernorm_fp64(x, g, b, eps, variant)
+        assert (~within(bad, ng_bad)).mean() > 0.25, variant          # a large share of elements must fail
+
+
+def test_layernorm_exact_power_of_two_case():
+    """x = +-2^j balanced -> mu = 0, var = 4^j, rstd = 2^-j exactly (eps = 0); gamma = 2^a, beta = 2^b:
+    X = +-2^a + 2^b, exactly representable in bf16 for |a - b| <= 6.  By hand, no arithmetic of the oracle."""
+    K = 512
+    for j, a, bexp in ((3, 1, -2), (-4, -1, 2), (0, 0, 0), (5, 3, -3)):
+        sgn = np.where(np.arange(K) % 2 == 0, 1.0, -1.0)
+        x = so.f32_to_bf16((sgn * 2.0 ** j).astype(F32))[None, :]
+        g = so.f32_to_bf16(np.full(K, 2.0 ** a, F32))
+        b = so.f32_to_bf16(np.full(K, 2.0 ** bexp, F32))
+        X = so.bf16_to_f32(so.normalize(x, so.NORM_LAYER, g, b, eps=0.0))[0]
+        assert np.array_equal(X, (sgn * 2.0 ** a + 2.0 ** bexp).astype(F32)), (j, a, bexp)
+    # beta sign and gamma/beta order on an asymmetric hand case: x = {+2^j, -2^j}, gamma = 4, beta = -0.5 -> {3.5, -4.5}
+    x = so.f32_to_bf16(np.array([[8.0, -8.0] * 128], F32))
+    X = so.bf16_to_f32(so.normalize(x, so.NORM_LAYER, so.f32_to_bf16(np.full(256, 4.0, F32)),
+                                    so.f32_to_bf16(np.full(256, -0.5, F32)), eps=0.0))[0]
+    assert np.array_equal(X, np.array([3.5, -4.5] * 128, F32))
+
+
+def test_layernorm_rounding_points_in_exact_rationals():
+    """DESIGN.md R3's rounding points, X = bf16(bf16(bf16(c * rstd) * gamma) + beta) with c = x - mu in fp32, on a
+    hand-made row where each of the bf16 roundings changes the answer in some columns: x in {+-1, +-7} balanced -> mu = 0,
+    var = 25, rstd = RN(1 / 5) in fp32.  Expected values computed in exact rational arithmetic with a brute-force
+    nearest-bf16 search; the variants that skip a rounding are shown to differ, so the pin is sensitive to them."""
+    K = 256
+    vals = np.array([1.0, -1.0, 7.0, -7.0] * (K // 4), F32)
+    x = so.f32_to_bf16(vals)[None, :]
+    rng = np.random.default_rng(7)
+    g = so.f32_to_bf16((rng.random(K) + 0.5).astype(F32))       # per-column gamma / beta: bf16 values, exact rationals
+    b = so.f32_to_bf16((rng.standard_normal(K) * 0.1).astype(F32))
+    X = so.bf16_to_f32(so.normalize(x, so.NORM_LAYER, g, b, eps=0.0))[0]
+    rstd = F32(1.0) / F32(5.0)                                   # sqrt(25) = 5 exactly; the one fp32 value RN(1/5)
+    skipped = {"h": 0, "v": 0}
+    for i, xv in enumerate(vals.tolist()):
+        gq, bq = Fraction(float(so.bf16_to_f32(g[i:i + 1])[0])), Fraction(float(so.bf16_to_f32(b[i:i + 1])[0]))
+        n32 = Fraction(float(F32(xv) * rstd))                    # fp32 product c * rstd (one RN)
+        h = _rne_bf16_fraction(n32)
+        v = _rne_bf16_fraction(h * gq)
+        want = _rne_bf16_fraction(v + bq)
+        assert Fraction(float(X[i])) == want, (i, xv)
+        skipped["h"] += _rne_bf16_fraction(_rne_bf16_fraction(n32 * gq) + bq) != want
+        skipped["v"] += _rne_bf16_fraction(h * gq + bq) != want
+    assert skipped["h"] > 10 and skipped["v"] > 10, skipped
+
+
+def test_hif4_residual_is_x_minus_decoded_backbone():
+    """Eq. 8 on the HiF4 path, directly: R + D_sp(Q_sp(M (.) X)) == X exactly in fp64 wherever the
+    subtraction was exact, dropped positions carry X bit for bit, and the stored backbone decodes (Eq. 15,
+    P:467) to the same values the residual was formed against."""
+    x = si.activations(6, 1024, config=4)
+    p = so.prepare(x, fmt=so.HIF4, mask=so.MASK_24, norm=so.NORM_NONE)
+    Xf = so.bf16_to_f32(p["X"]).astype(np.float64)
+    d = so.dequant_backbone(p)                                     # rebuilt from sp_codes / sp_meta / sp_sf only
+    assert np.array_equal(d, p["Xsp_tilde"].astype(np.float64))
+    assert np.array_equal(p["R"][~p["keep"]].view(np.uint32), so.bf16_to_f32(p["X"])[~p["keep"]].view(np.uint32))
+    assert (p["keep"].reshape(6, -1, 4).sum(-1) == 2).all()
+    exact = p["R"].astype(np.float64) + d == Xf
+    assert exact.mean() > 0.999                                    # fp32 subtraction of nearby values: Sterbenz
+    assert np.abs(p["R"].astype(np.float64) + d - Xf).max() <= np.abs(Xf).max() * 2.0 ** -24
