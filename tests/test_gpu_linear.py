@@ -215,12 +215,15 @@ def _sampled_check(sq, fmt, norm, T, K, D, config, mult, n_rows, n_cols, seed_ex
     y16 = sq.linear(cfg, act, wq, out_dtype="bf16")
     torch.cuda.synchronize()
     rng = np.random.Generator(np.random.Philox(si.seed_for(config, 1000 + seed_extra)))
+    last_blk = (T - 1) // 128 * 128                                # first row of the (possibly ragged) last 128-row block
     rows = np.unique(np.concatenate([rng.choice(T, size=min(n_rows, T), replace=False),
-                                     [0, min(127, T - 1), min(128, T - 1), T - 1]]))
+                                     [0, min(127, T - 1), min(128, T - 1), min(255, T - 1), min(256, T - 1),
+                                      last_blk, max(last_blk - 1, 0), T - 1]]))
     w_mag = w & np.uint16(0x7FFF)                                  # bf16 magnitudes order like integers
     top_row = int(np.unravel_index(int(w_mag.argmax()), w_mag.shape)[0])
+    # tile corners of the 128- / 192- / 256-wide variants and the tail of a ragged last N tile
     cols = np.unique(np.concatenate([rng.choice(D, size=n_cols, replace=False),
-                                     [0, 127, 128, 191, 192, 255, 256, D - 1, top_row]]))
+                                     [0, 127, 128, 191, 192, 255, 256, D - 64, D - 33, D - 2, D - 1, top_row]]))
     p = so.prepare(x[rows], fmt=fmt, norm=norm, gamma_u16=g)
     q = so.quantize_weight(w[cols], fmt=fmt)
     y64 = so.linear(p, q)
@@ -245,3 +248,64 @@ def test_qwen_config4_full_size_sampled(sq, fmt):
     """BASELINE.json configs[3]: Qwen2.5-7B down projection 18944 -> 3584 at T = 4096 in all three formats
     (the longest K of the five configs: 74 k-blocks, ragged against every pipeline depth)."""
     _sampled_check(sq, fmt, 0, 4096, 18944, 3584, config=4, mult=50.0, n_rows=16, n_cols=120, seed_extra=fmt)
+
+
+PREFILL_VARIANTS = [
+    # (fmt, norm, T, K, D, mult)  every (shape, T, format) family bench.py times at prefill sizes, by launch variant
+    (0, 0, 4096, 4096, 4096, 50.0),     # Llama o: CTA-pair tiles; 192-wide -> 22 n-tiles, ragged last (TMA zero fill)
+    (0, 1, 4096, 4096, 28672, 50.0),    # Llama gate+up: 150 n-tiles of 192, ragged last
+    (0, 0, 4096, 3584, 3584, 50.0),     # Qwen o: D % 256 != 0 -> 192-wide, 19 tiles, ragged last
+    (0, 1, 4000, 4096, 6144, 50.0),     # pair kernel, ragged T: 32 row blocks, last one 32 rows
+    (0, 1, 2049, 4096, 6144, 200.0),    # pair kernel, ODD number of 128-row blocks (17), last block one row
+    (0, 0, 2177, 14336, 4096, 50.0),    # long K (256-wide by the cost model), ragged T
+    (0, 0, 2048, 14336, 4096, 10.0),    # configs[2] T = 2048, outliers x10
+    (0, 0, 8192, 14336, 4096, 200.0),   # configs[2] T = 8192, outliers x200
+    (0, 1, 8192, 4096, 6144, 10.0),     # configs[2] T = 8192 qkv, outliers x10
+    (0, 1, 2048, 4096, 28672, 10.0),    # configs[2] T = 2048 gate+up
+    (0, 1, 4096, 3584, 4608, 50.0),     # configs[3] Qwen qkv, NVFP4
+    (1, 1, 4096, 3584, 4608, 50.0),     #                       MXFP4
+    (1, 0, 4096, 3584, 3584, 50.0),     # configs[3] Qwen o, MXFP4
+    (0, 1, 4096, 3584, 37888, 50.0),    # configs[3] Qwen gate+up, NVFP4
+    (1, 1, 4096, 3584, 37888, 50.0),    #                          MXFP4
+]
+
+
+@pytest.mark.parametrize("fmt,norm,T,K,D,mult", PREFILL_VARIANTS)
+def test_prefill_launch_variants_sampled(sq, fmt, norm, T, K, D, mult):
+    """BASELINE.json configs[2] / configs[3] at full size in the launch configuration bench.py times: the CTA-pair
+    kernel with 192- and 256-wide tiles, a ragged last N tile, ragged T and an odd number of 128-row blocks.
+    The sampled output features always include the last 64 columns (the tail of a ragged last tile) and the
+    sampled rows the first / last rows of the last row block."""
+    _sampled_check(sq, fmt, norm, T, K, D, config=3, mult=mult, n_rows=20, n_cols=160, seed_extra=T + D + fmt)
+
+
+def test_moe_config5_down_projection_sampled(sq):
+    """BASELINE.json configs[4], the expert DOWN projection 768 -> 2048 (3 k-blocks, multicast clusters): the
+    32768 routed rows are prepared per row into the experts' 128-row-aligned slots; three experts are checked."""
+    E, K, D = 128, 768, 2048
+    ids, offsets, order = si.moe_routing()
+    counts = np.diff(offsets)
+    cfg = sq.make_config(sq.NVFP4, sq.NORM_NONE, 1e-6, sq.LAYOUT_TILED)
+    pad_off = np.concatenate([[0], np.cumsum(-(-counts // 128) * 128)])
+    act = sq.alloc_act(cfg, int(pad_off[-1]), K, "cuda")
+    x = si.activations(int(offsets[-1]), K, config=5, extra=3)      # routed rows, already grouped by expert
+    check = [int(np.argmax(counts)), int(np.argmin(counts)), 5]
+    ws, wq_parts = {}, []
+    for e in range(E):
+        w = si.weight(D, K, 5, extra=2000 + e) if e in check else si.weight(D, K, 5, extra=3000 + e % 3)
+        if e in check:
+            ws[e] = w
+        wq_parts.append(sq.quantize_weight(cfg, to_dev(w)))
+        if counts[e]:
+            sq.prepare(cfg, to_dev(x[offsets[e]: offsets[e + 1]]), out=sq.act_slot(cfg, act, int(pad_off[e]), int(counts[e])))
+    wq = dict(codes=torch.cat([q["codes"] for q in wq_parts]), sf_sp=torch.cat([q["sf_sp"] for q in wq_parts]),
+              sf_dn=torch.cat([q["sf_dn"] for q in wq_parts]), ts_w=torch.cat([q["ts_w"] for q in wq_parts]), D=D, K=K)
+    Y = sq.linear_grouped(cfg, offsets, act, wq, D, out_dtype="fp32")
+    torch.cuda.synchronize()
+    Y = Y.cpu().numpy()
+    for e in check:
+        if counts[e] == 0:
+            continue
+        y64 = so.linear(so.prepare(x[offsets[e]: offsets[e + 1]], norm=0), so.quantize_weight(ws[e]))
+        got = Y[pad_off[e]: pad_off[e] + counts[e]]
+        assert rel_err(got, y64).max() <= TOL, f"expert {e}"
