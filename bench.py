@@ -572,7 +572,8 @@ def config_extras(sq, wl, pk, steps):
         act = sq.alloc_act(cfg, padded, K, "cuda")
         Y = torch.empty((padded, D), dtype=torch.bfloat16, device="cuda")
         ms_p = timed([lambda: sq.prepare(cfg, x, out=act)], max(steps // 2, 8), 3, lambda: None)
-        ms_l = timed([lambda: sq.linear_grouped(cfg, offsets, act, wq, D, Y=Y)], max(steps // 2, 8), 3, lambda: None)
+        offs_dev = torch.from_numpy(offsets).cuda()
+        ms_l = timed([lambda: sq.linear_grouped(cfg, offs_dev, act, wq, D, Y=Y)], max(steps // 2, 8), 3, lambda: None)
         rows = int(counts.sum())
         w_bytes = E * K * D * (0.5 + 1 / 32)
         by = w_bytes + rows * K * 0.90625 + 2.0 * rows * D

@@ -6,12 +6,17 @@
  *   sharq_quantize_weight  offline, once per weight: one FP4 payload + two scale views
  *   sharq_prepare          per call: norm -> N:M mask -> sparse FP4 backbone -> residual -> dense FP4
  *   sharq_linear           sparse + dense block-scaled FP4 GEMMs into one accumulator, bf16 epilogue
- * plus sharq_linear_grouped (the same over the row ranges of E experts, MoE) and sharq_prepare_add
- * (sharq_prepare with the residual-stream add fused in front of the norm).
+ * plus sharq_linear_grouped (the same over the row ranges of E experts, MoE), sharq_prepare_add
+ * (sharq_prepare with the residual-stream add fused in front of the norm), host-only size / plan queries
+ * (sharq_weight_sizes, sharq_act_sizes, sharq_linear_workspace, sharq_linear_plan), sharq_act_init and the test
+ * helpers sharq_untile_sf / sharq_untile_meta.  The tensor-pipe probe lives in sharq_diag.h.
  *
  * Conventions
  *   - The caller owns every buffer; the library never allocates device memory and keeps no
- *     mutable global state.  All pointers are DEVICE pointers unless marked "host".
+ *     state between calls: every entry point is thread-safe and reads no environment variable.  (The only
+ *     process-wide data are memoised answers of the CUDA runtime about a device -- a driver entry point,
+ *     "opt-in shared memory is set for this kernel", cluster occupancy -- keyed by device ordinal, filled
+ *     lock-free and idempotently.)  All pointers are DEVICE pointers unless marked "host".
  *   - Work is enqueued on the caller's CUDA stream (`stream` is a cudaStream_t passed as void*)
  *     and the call returns without synchronising.
  *   - Errors are return codes; nothing throws or aborts.  On a non-OK return nothing was launched.
@@ -21,7 +26,7 @@
  *   - bf16 tensors are row-major; "code" tensors hold two 4-bit codes per byte, the element
  *     with the lower k in the low nibble.
  *   - Shapes: K % 256 == 0 (8-chunks, 32/64 scale groups, MMA-K 128, 256-wide metadata tile),
- *     D % 128 == 0 for sharq_linear, T >= 0 (T == 0 returns SHARQ_OK without a launch).
+ *     D % 128 == 0 for sharq_linear, T >= 0 (T == 0 returns SHARQ_OK without a launch), T < 2^30.
  *   - Inputs must be finite; NaN/Inf behaviour is deterministic but unspecified.
  *
  * Output layouts (config.layout)
@@ -32,7 +37,10 @@
  *     sparsity metadata [R rows, K/16 bytes], rows padded to a multiple of 128:
  *       byte(r, b) at  ((r/128) * (K/256) + b/16) * 2048 + (r%128)*16 + (b%16)
  *     codes and row scales are identical in both layouts.
- *   sharq_*_sizes report the padded byte counts for the chosen layout.
+ *   sharq_*_sizes report the padded byte counts for the chosen layout.  sharq_prepare writes the bytes of rows
+ *   0 .. T-1 only; the pad rows of the last 128-row tile are read by sharq_linear's tensor-memory copies (their
+ *   products land in accumulator rows that are never stored), so they must hold VALID bytes: initialise the TILED
+ *   scale / metadata buffers once with sharq_act_init (any later sharq_prepare output keeps them valid).
  */
 #ifndef SHARQ_H_
 #define SHARQ_H_
@@ -62,7 +70,9 @@ typedef enum { SHARQ_LAYOUT_CANONICAL = 0, SHARQ_LAYOUT_TILED = 1 } sharq_layout
 
 typedef struct {
   int32_t fmt;    /* sharq_format */
-  int32_t mask;   /* sharq_mask; NVFP4/MXFP4 require PAIR48, HIF4 requires MASK_24 */
+  int32_t mask;   /* sharq_mask.  HIF4 requires MASK_24.  NVFP4 / MXFP4: PAIR48 is the pattern the B200 sparse FP4
+                     MMA accepts; MASK_24 (element-wise 2:4) is accepted by sharq_prepare / sharq_act_sizes with
+                     layout CANONICAL only (oracle-checkable encoding; sharq_linear returns SHARQ_ESHAPE for it) */
   int32_t norm;   /* sharq_norm */
   float eps;      /* added to the mean square / variance (P:155 RMSNorm / LayerNorm) */
   int32_t layout; /* sharq_layout of scale-factor and metadata outputs */
@@ -104,7 +114,8 @@ sharq_status sharq_quantize_weight(const sharq_config* cfg, const void* W, int64
  * P:394) or NULL = dynamic per-row scale amax_row/2688 (NVFP4 only; ignored otherwise).
  *   sp_codes  [T, K/4]  bytes  survivors' FP4 codes, ascending k (Eq. 7)
  *   sp_sf     [T, K/32] bytes  backbone block scales           (HiF4: [T, K/64] uint32)
- *   sp_meta   [T, K/16] bytes  one nibble i0|i1<<2 per 8-chunk (MASK_24: [T, K/8], per 4)
+ *   sp_meta   [T, K/16] bytes  one nibble i0|i1<<2 per 8-chunk (MASK_24: [T, K/8], one nibble per 4 elements;
+ *                              the backbone scale group stays 32 logical k = 16 survivors)
  *   dn_codes  [T, K/2]  bytes  residual FP4 codes of R = X - D_sp(Q_sp(X_sp)) (Eq. 8)
  *   dn_sf     [T, K/16] bytes  residual block scales (MXFP4: [T,K/32]; HiF4: [T,K/64] uint32)
  *   row_scale [T] float        the tensor scale each row was quantized with (1 for MXFP4/HiF4)
@@ -156,30 +167,47 @@ sharq_status sharq_linear(const sharq_config* cfg, int64_t T, int64_t D, int64_t
                           void* workspace, size_t workspace_bytes, void* stream);
 
 /* ---- sharq_linear_grouped (MoE expert linears) -----------------------------
- * E experts; `offsets` is a HOST int32[E+1] array: rows [offsets[e], offsets[e+1]) of the
- * activation tensors belong to expert e.  Every expert's row range must start at a multiple of
- * 128 in the TILED scale/metadata arrays, i.e. the caller prepares each expert's rows with
- * sharq_prepare into a 128-row-aligned slot: row r of expert e lives at padded row
- * pad_offsets[e] + r with pad_offsets[e] = sum_{j<e} roundup(count_j, 128).  Weight tensors are
- * stacked [E, ...] (each expert's tensors laid out as sharq_quantize_weight writes them);
- * w_tensor_scale is float[E].  Empty experts are skipped.  Y is [sum roundup(count,128), D]
- * in the same padded row numbering. */
-sharq_status sharq_linear_grouped(const sharq_config* cfg, int32_t E, const int32_t* offsets_host,
-                                  int64_t D, int64_t K, const void* sp_codes, const void* sp_sf,
-                                  const void* sp_meta, const void* dn_codes, const void* dn_sf,
-                                  const float* row_scale, const void* w_codes,
+ * E experts (E <= 1024); `offsets` is a DEVICE int32[E+1] array (e.g. the router's output, no host copy and no
+ * synchronisation needed): rows [offsets[e], offsets[e+1]) of the routed batch belong to expert e,
+ * offsets[0] == 0, non-decreasing (a negative count is treated as 0).  Every expert's row range starts at a
+ * multiple of 128 in the activation tensors, i.e. the caller prepares each expert's rows with sharq_prepare into
+ * a 128-row-aligned slot: row r of expert e lives at padded row pad_offsets[e] + r with
+ * pad_offsets[e] = sum_{j<e} roundup(count_j, 128).  `padded_rows` = the row capacity of those activation
+ * buffers and of Y (a multiple of 128, >= sum roundup(count, 128); e.g. roundup(total, 128) + 128 * E always
+ * suffices); row blocks beyond it are not computed.  Weight tensors are stacked [E, ...] (each expert's tensors
+ * laid out as sharq_quantize_weight writes them); w_tensor_scale is float[E].  Empty experts are skipped.  Y is
+ * [padded_rows, D] in the same padded row numbering.  One launch; every CTA derives the expert table from
+ * `offsets` in its shared memory. */
+sharq_status sharq_linear_grouped(const sharq_config* cfg, int32_t E, const int32_t* offsets,
+                                  int64_t padded_rows, int64_t D, int64_t K, const void* sp_codes,
+                                  const void* sp_sf, const void* sp_meta, const void* dn_codes,
+                                  const void* dn_sf, const float* row_scale, const void* w_codes,
                                   const void* w_sf_sparse_view, const void* w_sf_dense_view,
-                                  const float* w_tensor_scale, void* Y, int64_t ldy,
-                                  int32_t out_dtype, void* workspace, size_t workspace_bytes,
-                                  void* stream);
+                                  const float* w_tensor_scale, void* Y, int64_t ldy, int32_t out_dtype,
+                                  void* workspace, size_t workspace_bytes, void* stream);
 
-/* ---- diagnostics: tensor-pipe issue-rate probe (not part of the hot path) -------------------------
- * Launches, on every SM pair, `iters` repetitions of the per-k-block (256 logical k) instruction sequence
- * of the CTA-pair GEMM on shared-memory-resident bytes: mode bit 1 = the 4 dense block-scaled MMAs, bit 2 =
- * the 2 sparse MMAs, bit 4 = the scale-factor / metadata tcgen05.cp copies; M = 256, N = 256 per pair, no
- * loads, no epilogue.  The caller times it (CUDA events): nominal flop per path = 2 * 128 * 256 * 256 *
- * iters * (number of SMs).  Gives the applicable FP4 tensor peak of the GPU. */
-sharq_status sharq_mma_peak_launch(int32_t mode, int32_t iters, void* stream);
+/* ---- sharq_act_init: one-time initialisation of TILED activation scale / metadata buffers ----------
+ * Fills sp_sf and dn_sf with zero scales and sp_meta with the valid nibble 0x4 (pairs 0 and 1) for all
+ * roundup(T, 128) rows, so that the pad rows sharq_prepare never writes hold defined operands (see "Output
+ * layouts").  Three memsets on `stream`; layout CANONICAL: nothing to do, returns SHARQ_OK. */
+sharq_status sharq_act_init(const sharq_config* cfg, int64_t T, int64_t K, void* sp_sf, void* sp_meta,
+                            void* dn_sf, void* stream);
+
+/* ---- sharq_linear_plan: which kernel variant a sharq_linear / sharq_linear_grouped call launches ---------
+ * Host-only query (needs the current device for its SM count / cluster occupancy; launches nothing).
+ * E == 0: sharq_linear(T, D, K); E > 0: sharq_linear_grouped with padded_rows = T.  Writes a zero-terminated
+ * description into buf (at most n bytes), e.g. "pair bn=192 stages=4 tiles=2400 grid=148 cluster=2".
+ * kinds: "tile" (128-row tiles, persistent or split-K cluster), "pair" (CTA-pair 256-row tiles), "grouped-mc"
+ * (multicast clusters of two), "hif4-bf16".  The parity tests use it to name the variant they cover. */
+sharq_status sharq_linear_plan(const sharq_config* cfg, int64_t T, int64_t D, int64_t K, int32_t E, char* buf,
+                               size_t n);
+
+/* ---- test helpers (not on the timed path) ---------------------------------------------
+ * Map the TILED layouts back to canonical row-major arrays for byte comparison (device -> device).
+ *   sharq_untile_sf   tiled scale factors, R rows x C columns (C % 4 == 0) -> canonical [R, C] bytes
+ *   sharq_untile_meta tiled sparsity metadata of R rows, K logical columns   -> canonical [R, K/16] bytes */
+sharq_status sharq_untile_sf(const void* tiled, int64_t R, int64_t C, void* canonical, void* stream);
+sharq_status sharq_untile_meta(const void* tiled, int64_t R, int64_t K, void* canonical, void* stream);
 
 /* Library / build information: returns a static string, e.g. "sharq-b200 0.1 sm_100a". */
 const char* sharq_version(void);

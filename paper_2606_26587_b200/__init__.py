@@ -13,7 +13,7 @@ import os
 from ctypes import POINTER, c_char_p, c_float, c_int32, c_int64, c_size_t, c_void_p
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libsharq.so")
+LIB_PATH = os.environ.get("SHARQ_LIB") or os.path.join(_HERE, "libsharq.so")   # SHARQ_LIB: another build of the same ABI
 
 OK, EINVAL, ESHAPE, EWORKSPACE, EARCH, ECUDA = range(6)
 NVFP4, MXFP4, HIF4 = 0, 1, 2
@@ -60,20 +60,23 @@ def _load() -> ctypes.CDLL:
     lib.sharq_prepare_add.argtypes = [CFG, P, P, c_int64, c_int64, c_int64, c_int64, P, c_int64, P, P, P, P, P, P, P, P, P, P]
     lib.sharq_linear.argtypes = [CFG, c_int64, c_int64, c_int64, P, P, P, P, P, P, P, P, P, P, P, P, c_int64,
                                  c_int32, c_int32, P, c_size_t, P]
-    lib.sharq_linear_grouped.argtypes = [CFG, c_int32, POINTER(c_int32), c_int64, c_int64, P, P, P, P, P, P, P, P,
+    lib.sharq_linear_grouped.argtypes = [CFG, c_int32, P, c_int64, c_int64, c_int64, P, P, P, P, P, P, P, P,
                                          P, P, P, c_int64, c_int32, P, c_size_t, P]
-    lib.sharq_mma_peak_launch.argtypes = [c_int32, c_int32, P]
-    lib.sharq_mma_peak_launch.restype = c_int32
-    for name in ("sharq_weight_sizes", "sharq_act_sizes", "sharq_linear_workspace", "sharq_quantize_weight",
-                 "sharq_prepare", "sharq_prepare_add", "sharq_linear", "sharq_linear_grouped"):
+    lib.sharq_act_init.argtypes = [CFG, c_int64, c_int64, P, P, P, P]
+    lib.sharq_linear_plan.argtypes = [CFG, c_int64, c_int64, c_int64, c_int32, ctypes.c_char_p, c_size_t]
+    lib.sharq_untile_sf.argtypes = [P, c_int64, c_int64, P, P]
+    lib.sharq_untile_meta.argtypes = [P, c_int64, c_int64, P, P]
+    lib.sharq_mma_peak_launch.argtypes = [c_int32, c_int32, P]           # include/sharq_diag.h
+    for name in EXPORTS[1:]:
         getattr(lib, name).restype = c_int32
     return lib
 
 
-capi = _load()
+# every symbol include/sharq.h declares, then include/sharq_diag.h's
 EXPORTS = ("sharq_version", "sharq_weight_sizes", "sharq_act_sizes", "sharq_linear_workspace",
            "sharq_quantize_weight", "sharq_prepare", "sharq_prepare_add", "sharq_linear", "sharq_linear_grouped",
-           "sharq_mma_peak_launch")
+           "sharq_act_init", "sharq_linear_plan", "sharq_untile_sf", "sharq_untile_meta", "sharq_mma_peak_launch")
+capi = _load()
 
 
 def version() -> str:
@@ -121,6 +124,28 @@ def mma_peak_launch(mode: int, iters: int):
     _check(capi.sharq_mma_peak_launch(mode, iters, _stream()), "sharq_mma_peak_launch")
 
 
+def linear_plan(cfg: Config, T: int, D: int, K: int, E: int = 0) -> str:
+    """Which kernel variant sharq_linear (E == 0) / sharq_linear_grouped (E > 0, T = padded rows) launches."""
+    buf = ctypes.create_string_buffer(256)
+    _check(capi.sharq_linear_plan(ctypes.byref(cfg), T, D, K, E, buf, 256), "sharq_linear_plan")
+    return buf.value.decode()
+
+
+def untile_sf(tiled, R: int, C: int):
+    """TILED scale factors (device uint8) -> canonical [R, C] device tensor, through the C ABI."""
+    import torch
+    out = torch.empty((R, C), dtype=torch.uint8, device=tiled.device)
+    _check(capi.sharq_untile_sf(_ptr(tiled), R, C, _ptr(out), _stream()), "sharq_untile_sf")
+    return out
+
+
+def untile_meta(tiled, R: int, K: int):
+    import torch
+    out = torch.empty((R, K // 16), dtype=torch.uint8, device=tiled.device)
+    _check(capi.sharq_untile_meta(_ptr(tiled), R, K, _ptr(out), _stream()), "sharq_untile_meta")
+    return out
+
+
 def _bytes(n, device):
     import torch
     return torch.empty(max(int(n), 16), dtype=torch.uint8, device=device)
@@ -144,9 +169,13 @@ def quantize_weight(cfg: Config, W):
 def alloc_act(cfg: Config, T: int, K: int, device):
     import torch
     n = act_sizes(cfg, T, K)
-    return dict(sp_codes=_bytes(n[0], device), sp_sf=_bytes(n[1], device), sp_meta=_bytes(n[2], device),
-                dn_codes=_bytes(n[3], device), dn_sf=_bytes(n[4], device),
-                row_scale=torch.empty(max(T, 1), dtype=torch.float32, device=device), T=T, K=K)
+    out = dict(sp_codes=_bytes(n[0], device), sp_sf=_bytes(n[1], device), sp_meta=_bytes(n[2], device),
+               dn_codes=_bytes(n[3], device), dn_sf=_bytes(n[4], device),
+               row_scale=torch.empty(max(T, 1), dtype=torch.float32, device=device), T=T, K=K)
+    if T > 0:   # pad rows of the TILED scale / metadata tiles must hold valid operands (sharq.h "Output layouts")
+        _check(capi.sharq_act_init(ctypes.byref(cfg), T, K, _ptr(out["sp_sf"]), _ptr(out["sp_meta"]), _ptr(out["dn_sf"]),
+                                   _stream()), "sharq_act_init")
+    return out
 
 
 def prepare(cfg: Config, x, gamma=None, beta=None, x_tensor_scale=None, out=None):
@@ -205,21 +234,20 @@ def linear(cfg: Config, act: dict, wq: dict, bias=None, out_dtype="bf16", path=P
 
 
 def linear_grouped(cfg: Config, offsets, act: dict, wq: dict, D: int, out_dtype="bf16", Y=None, workspace=None):
-    """offsets: host int32 sequence [E+1]; act tensors hold the 128-row-padded expert slots (sharq.h)."""
+    """offsets: DEVICE int32 tensor [E+1] (a host sequence is uploaded first); act tensors hold the 128-row-padded
+    expert slots (sharq.h), act["T"] = their row capacity (a multiple of 128)."""
     import torch
-    E = len(offsets) - 1
     K = act["K"]
     dev = act["sp_codes"].device
-    offs = (c_int32 * (E + 1))(*[int(o) for o in offsets])
-    padded = sum(-(-(int(offsets[e + 1]) - int(offsets[e])) // 128) * 128 for e in range(E))
+    if not isinstance(offsets, torch.Tensor):
+        offsets = torch.tensor([int(o) for o in offsets], dtype=torch.int32, device=dev)
+    E = offsets.numel() - 1
+    padded = act["T"] // 128 * 128
     if Y is None:
         Y = torch.zeros((max(padded, 1), D), dtype=torch.bfloat16 if out_dtype == "bf16" else torch.float32, device=dev)
-    n_ws = linear_workspace(cfg, int(offsets[-1]), D, K, E)
-    if workspace is None:
-        workspace = _bytes(n_ws, dev)
-    _check(capi.sharq_linear_grouped(ctypes.byref(cfg), E, offs, D, K, _ptr(act["sp_codes"]), _ptr(act["sp_sf"]),
-                                     _ptr(act["sp_meta"]), _ptr(act["dn_codes"]), _ptr(act["dn_sf"]),
+    _check(capi.sharq_linear_grouped(ctypes.byref(cfg), E, _ptr(offsets), padded, D, K, _ptr(act["sp_codes"]),
+                                     _ptr(act["sp_sf"]), _ptr(act["sp_meta"]), _ptr(act["dn_codes"]), _ptr(act["dn_sf"]),
                                      _ptr(act["row_scale"]), _ptr(wq["codes"]), _ptr(wq["sf_sp"]), _ptr(wq["sf_dn"]),
                                      _ptr(wq["ts_w"]), _ptr(Y), Y.stride(0), 0 if Y.dtype == torch.bfloat16 else 1,
-                                     _ptr(workspace), n_ws, _stream()), "sharq_linear_grouped")
+                                     _ptr(workspace), 0, _stream()), "sharq_linear_grouped")
     return Y

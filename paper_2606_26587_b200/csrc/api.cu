@@ -1,8 +1,10 @@
 // C ABI of libsharq.so (include/sharq.h): argument validation, size queries, dispatch.
 // All compute is in prepare.cu / linear.cu; there is no CPU fallback anywhere.
 #include <cuda_runtime.h>
+#include <stdio.h>
 
 #include "common.cuh"
+#include "linear_args.h"
 
 namespace sharq {
 cudaError_t launch_prepare(const sharq_config* cfg, const void* x, int64_t T, int64_t K, int64_t ldx,
@@ -12,17 +14,10 @@ cudaError_t launch_prepare(const sharq_config* cfg, const void* x, int64_t T, in
 cudaError_t launch_quantize_weight(const sharq_config* cfg, const void* W, int64_t D, int64_t K, int64_t ldw,
                                    void* codes, void* sf_sp, void* sf_dn, float* ts, void* workspace,
                                    cudaStream_t st);
-struct LinearArgs {
-  int64_t T, D, K;              // T = rows of this problem (per expert for grouped)
-  const void *sp_codes, *sp_sf, *sp_meta, *dn_codes, *dn_sf;
-  const float* row_scale;
-  const void *w_codes, *w_sf_sp, *w_sf_dn;
-  const float* w_ts;
-  const void* bias;
-  void* Y; int64_t ldy; int out_dtype; int path;
-};
-sharq_status launch_linear(const sharq_config* cfg, const LinearArgs& a, int32_t E, const int32_t* offsets_host,
-                           void* workspace, size_t workspace_bytes, int num_sms, cudaStream_t st);
+sharq_status launch_linear(const sharq_config* cfg, const LinearArgs& a, int32_t E, const int32_t* offsets,
+                           void* workspace, size_t workspace_bytes, int num_sms, int dev, cudaStream_t st,
+                           LinearPlan* plan_only);
+cudaError_t launch_untile(const void* tiled, int64_t R, int64_t C, void* canonical, int meta, cudaStream_t st);
 size_t linear_workspace_bytes(const sharq_config* cfg, int64_t T, int64_t D, int64_t K, int32_t E);
 }  // namespace sharq
 
@@ -37,13 +32,14 @@ sharq_status check_cfg(const sharq_config* cfg) {
   if (cfg->fmt < 0 || cfg->fmt > 2 || cfg->mask < 0 || cfg->mask > 1 || cfg->norm < 0 || cfg->norm > 2 ||
       cfg->layout < 0 || cfg->layout > 1)
     return SHARQ_EINVAL;
-  // the block-scaled FP4 sparse MMA only takes the pairwise pattern; HiF4 uses the standard 2:4
-  if (cfg->fmt == SHARQ_HIF4 ? cfg->mask != SHARQ_MASK_24 : cfg->mask != SHARQ_MASK_PAIR48) return SHARQ_EINVAL;
-  if (cfg->fmt == SHARQ_HIF4 && cfg->layout != SHARQ_LAYOUT_CANONICAL) return SHARQ_EINVAL;
+  // HiF4 uses the standard 2:4; for NVFP4 / MXFP4 the element-wise 2:4 is an encoding the oracle can check
+  // (sharq_prepare, canonical layout) but not one the block-scaled FP4 sparse MMA takes (check_linear refuses it)
+  if (cfg->fmt == SHARQ_HIF4 && cfg->mask != SHARQ_MASK_24) return SHARQ_EINVAL;
+  if (cfg->mask == SHARQ_MASK_24 && cfg->layout != SHARQ_LAYOUT_CANONICAL) return SHARQ_EINVAL;
   return SHARQ_OK;
 }
 
-struct DeviceInfo { int ok; int sms; int major; };
+struct DeviceInfo { int ok; int sms; int major; int dev; };
 sharq_status device_info(DeviceInfo* out) {
   int dev = 0;
   if (cudaGetDevice(&dev) != cudaSuccess) return SHARQ_ECUDA;
@@ -51,7 +47,7 @@ sharq_status device_info(DeviceInfo* out) {
   if (cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess) return SHARQ_ECUDA;
   if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return SHARQ_ECUDA;
   if (major != 10) return SHARQ_EARCH;
-  out->ok = 1; out->sms = sms; out->major = major;
+  out->ok = 1; out->sms = sms; out->major = major; out->dev = dev;
   return SHARQ_OK;
 }
 
@@ -101,6 +97,7 @@ sharq_status sharq_linear_workspace(const sharq_config* cfg, int64_t T, int64_t 
   sharq_status s = check_cfg(cfg);
   if (s != SHARQ_OK) return s;
   if (T < 0 || D <= 0 || D % 128 != 0 || K <= 0 || K % 256 != 0 || E < 0) return SHARQ_ESHAPE;
+  if (cfg->fmt != SHARQ_HIF4 && cfg->mask != SHARQ_MASK_PAIR48) return SHARQ_ESHAPE;
   if (workspace) *workspace = linear_workspace_bytes(cfg, T, D, K, E);
   return SHARQ_OK;
 }
@@ -151,6 +148,7 @@ sharq_status sharq_prepare_add(const sharq_config* cfg, const void* x, const voi
   sharq_status s = check_cfg(cfg);
   if (s != SHARQ_OK) return s;
   if (T < 0 || K <= 0 || K % 256 != 0 || K > 32768) return SHARQ_ESHAPE;
+  if (cfg->fmt != SHARQ_HIF4 && cfg->mask != SHARQ_MASK_PAIR48) return SHARQ_EINVAL;   // the fused add has no 2:4 E2M1 variant
   if (ldx < K || ldr < K || ldo < K || ldx % 16 != 0 || ldr % 16 != 0 || ldo % 16 != 0) return SHARQ_ESHAPE;
   if (T == 0) return SHARQ_OK;
   if (!x || !residual || !sum_out || !sp_codes || !sp_sf || !sp_meta || !dn_codes || !dn_sf || !row_scale) return SHARQ_EINVAL;
@@ -172,6 +170,7 @@ static sharq_status check_linear(const sharq_config* cfg, int64_t D, int64_t K, 
                                  int64_t ldy, int32_t out_dtype, int32_t path) {
   sharq_status s = check_cfg(cfg);
   if (s != SHARQ_OK) return s;
+  if (cfg->fmt != SHARQ_HIF4 && cfg->mask != SHARQ_MASK_PAIR48) return SHARQ_ESHAPE;   // no element-wise 2:4 FP4 MMA
   if (cfg->layout != SHARQ_LAYOUT_TILED && cfg->fmt != SHARQ_HIF4) return SHARQ_EINVAL;
   if (D <= 0 || D % 128 != 0 || K <= 0 || K % 256 != 0 || ldy < D || ldy % 8 != 0) return SHARQ_ESHAPE;
   if (out_dtype < 0 || out_dtype > 1 || path < 0 || path > 2) return SHARQ_EINVAL;
@@ -189,7 +188,7 @@ sharq_status sharq_linear(const sharq_config* cfg, int64_t T, int64_t D, int64_t
   const void* ptrs[] = {sp_codes, sp_sf, sp_meta, dn_codes, dn_sf, w_codes, w_sf_sparse_view, w_sf_dense_view, Y};
   sharq_status s = check_linear(cfg, D, K, ptrs, T == 0 ? 0 : 9, ldy, out_dtype, path);
   if (s != SHARQ_OK) return s;
-  if (T < 0) return SHARQ_ESHAPE;
+  if (T < 0 || T >= (int64_t)1 << 30) return SHARQ_ESHAPE;
   if (T == 0) return SHARQ_OK;
   if (!row_scale || !w_tensor_scale) return SHARQ_EINVAL;
   if (workspace_bytes < linear_workspace_bytes(cfg, T, D, K, 0)) return SHARQ_EWORKSPACE;
@@ -197,11 +196,11 @@ sharq_status sharq_linear(const sharq_config* cfg, int64_t T, int64_t D, int64_t
   if ((s = device_info(&di)) != SHARQ_OK) return s;
   LinearArgs a{T, D, K, sp_codes, sp_sf, sp_meta, dn_codes, dn_sf, row_scale, w_codes, w_sf_sparse_view,
                w_sf_dense_view, w_tensor_scale, bias, Y, ldy, out_dtype, path};
-  return launch_linear(cfg, a, 0, nullptr, workspace, workspace_bytes, di.sms, (cudaStream_t)stream);
+  return launch_linear(cfg, a, 0, nullptr, workspace, workspace_bytes, di.sms, di.dev, (cudaStream_t)stream, nullptr);
 }
 
-sharq_status sharq_linear_grouped(const sharq_config* cfg, int32_t E, const int32_t* offsets_host, int64_t D,
-                                  int64_t K, const void* sp_codes, const void* sp_sf, const void* sp_meta,
+sharq_status sharq_linear_grouped(const sharq_config* cfg, int32_t E, const int32_t* offsets, int64_t padded_rows,
+                                  int64_t D, int64_t K, const void* sp_codes, const void* sp_sf, const void* sp_meta,
                                   const void* dn_codes, const void* dn_sf, const float* row_scale,
                                   const void* w_codes, const void* w_sf_sparse_view, const void* w_sf_dense_view,
                                   const float* w_tensor_scale, void* Y, int64_t ldy, int32_t out_dtype,
@@ -209,19 +208,68 @@ sharq_status sharq_linear_grouped(const sharq_config* cfg, int32_t E, const int3
   const void* ptrs[] = {sp_codes, sp_sf, sp_meta, dn_codes, dn_sf, w_codes, w_sf_sparse_view, w_sf_dense_view, Y};
   sharq_status s = check_linear(cfg, D, K, ptrs, 9, ldy, out_dtype, 0);
   if (s != SHARQ_OK) return s;
-  if (E <= 0 || !offsets_host) return SHARQ_EINVAL;
+  if (E <= 0 || !offsets) return SHARQ_EINVAL;
   if (cfg->fmt == SHARQ_HIF4) return SHARQ_EINVAL;
-  for (int32_t e = 0; e < E; ++e)
-    if (offsets_host[e + 1] < offsets_host[e]) return SHARQ_ESHAPE;
-  if (offsets_host[0] != 0) return SHARQ_ESHAPE;
+  if (E > 1024 || padded_rows < 0 || padded_rows % 128 != 0 || padded_rows >= (int64_t)1 << 30) return SHARQ_ESHAPE;
   if (!row_scale || !w_tensor_scale) return SHARQ_EINVAL;
-  if (workspace_bytes < linear_workspace_bytes(cfg, offsets_host[E], D, K, E)) return SHARQ_EWORKSPACE;
-  if (!workspace && linear_workspace_bytes(cfg, offsets_host[E], D, K, E) > 0) return SHARQ_EINVAL;
+  (void)workspace; (void)workspace_bytes;                  // NVFP4 / MXFP4 need none
+  if (padded_rows == 0) return SHARQ_OK;
   DeviceInfo di{};
   if ((s = device_info(&di)) != SHARQ_OK) return s;
-  LinearArgs a{0, D, K, sp_codes, sp_sf, sp_meta, dn_codes, dn_sf, row_scale, w_codes, w_sf_sparse_view,
+  LinearArgs a{padded_rows, D, K, sp_codes, sp_sf, sp_meta, dn_codes, dn_sf, row_scale, w_codes, w_sf_sparse_view,
                w_sf_dense_view, w_tensor_scale, nullptr, Y, ldy, out_dtype, 0};
-  return launch_linear(cfg, a, E, offsets_host, workspace, workspace_bytes, di.sms, (cudaStream_t)stream);
+  return launch_linear(cfg, a, E, offsets, workspace, workspace_bytes, di.sms, di.dev, (cudaStream_t)stream, nullptr);
+}
+
+sharq_status sharq_linear_plan(const sharq_config* cfg, int64_t T, int64_t D, int64_t K, int32_t E, char* buf,
+                               size_t n) {
+  sharq_status s = check_linear(cfg, D, K, nullptr, 0, D, 0, 0);
+  if (s != SHARQ_OK) return s;
+  if (!buf || n == 0 || T < 0 || E < 0 || T >= (int64_t)1 << 30) return SHARQ_EINVAL;
+  if (E > 0 && (T % 128 != 0 || E > 1024 || cfg->fmt == SHARQ_HIF4)) return SHARQ_ESHAPE;
+  DeviceInfo di{};
+  if ((s = device_info(&di)) != SHARQ_OK) return s;
+  LinearPlan pl{};
+  pl.kind = -1;
+  LinearArgs a{T, D, K, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr,
+               nullptr, nullptr, D, 0, 0};
+  if (T > 0) {
+    s = launch_linear(cfg, a, E, nullptr, nullptr, 0, di.sms, di.dev, nullptr, &pl);
+    if (s != SHARQ_OK) return s;
+  }
+  static const char* const kinds[] = {"tile", "pair", "grouped-mc", "hif4-bf16"};
+  if (pl.kind < 0) snprintf(buf, n, "none");
+  else snprintf(buf, n, "%s bn=%d act_rows=%d splits=%d stages=%d tiles=%lld grid=%lld cluster=%d", kinds[pl.kind],
+                pl.bn, pl.act_rows, pl.splits, pl.stages, (long long)pl.tiles, (long long)pl.grid, pl.cluster);
+  return SHARQ_OK;
+}
+
+sharq_status sharq_act_init(const sharq_config* cfg, int64_t T, int64_t K, void* sp_sf, void* sp_meta, void* dn_sf,
+                            void* stream) {
+  size_t n_sf = 0, n_meta = 0, n_dn = 0;
+  sharq_status s = sharq_act_sizes(cfg, T, K, nullptr, &n_sf, &n_meta, nullptr, &n_dn, nullptr);
+  if (s != SHARQ_OK) return s;
+  if (cfg->layout != SHARQ_LAYOUT_TILED || T == 0) return SHARQ_OK;
+  if (!sp_sf || !sp_meta || !dn_sf) return SHARQ_EINVAL;
+  cudaStream_t st = (cudaStream_t)stream;
+  if (cudaMemsetAsync(sp_sf, 0, n_sf, st) != cudaSuccess || cudaMemsetAsync(dn_sf, 0, n_dn, st) != cudaSuccess ||
+      cudaMemsetAsync(sp_meta, 0x44, n_meta, st) != cudaSuccess)
+    return SHARQ_ECUDA;
+  return SHARQ_OK;
+}
+
+sharq_status sharq_untile_sf(const void* tiled, int64_t R, int64_t C, void* canonical, void* stream) {
+  if (R < 0 || C <= 0 || C % 4 != 0) return SHARQ_ESHAPE;
+  if (R == 0) return SHARQ_OK;
+  if (!tiled || !canonical) return SHARQ_EINVAL;
+  return launch_untile(tiled, R, C, canonical, 0, (cudaStream_t)stream) == cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
+}
+
+sharq_status sharq_untile_meta(const void* tiled, int64_t R, int64_t K, void* canonical, void* stream) {
+  if (R < 0 || K <= 0 || K % 256 != 0) return SHARQ_ESHAPE;
+  if (R == 0) return SHARQ_OK;
+  if (!tiled || !canonical) return SHARQ_EINVAL;
+  return launch_untile(tiled, R, K / 16, canonical, 1, (cudaStream_t)stream) == cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
 }
 
 }  // extern "C"

@@ -1,4 +1,6 @@
-// Debug / experiment switches (environment variables, read ONCE per process; none is needed in production).
+// Experiment switches.  The DEFAULT build has none: debug_env() returns compile-time constants and the library reads
+// no environment variable.  Only a build with -DSHARQ_EXPERIMENTS (never shipped; used for sweeps and ablations)
+// reads the SHARQ_DEBUG_* variables below, once per process.
 #pragma once
 #include <cstdlib>
 
@@ -19,6 +21,10 @@ struct DebugEnv {
   int prep_chunk_rows; // SHARQ_DEBUG_PREP_CHUNK_ROWS: rows per launch of the row-per-CTA prepare kernel (tests; 0 = 2^31 / width)
 };
 
+#ifndef SHARQ_EXPERIMENTS
+constexpr DebugEnv kNoDebug{0, 0, 0, 0, 0, 0, 0, 128, 0, 0, 0, 0};
+inline constexpr const DebugEnv& debug_env() { return kNoDebug; }
+#else
 inline const DebugEnv& debug_env() {
   static const DebugEnv e = [] {
     auto num = [](const char* name, int dflt) {
@@ -43,5 +49,6 @@ inline const DebugEnv& debug_env() {
   }();
   return e;
 }
+#endif
 
 }  // namespace sharq

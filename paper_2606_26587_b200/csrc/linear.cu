@@ -17,30 +17,23 @@
 #include <cuda_runtime.h>
 #include <stdlib.h>
 
+#include <atomic>
+
 #include "common.cuh"
 #include "debug_env.h"
+#include "linear_args.h"
 #include "tc_ptx.cuh"
 
 namespace sharq {
 
-struct LinearArgs {
-  int64_t T, D, K;
-  const void *sp_codes, *sp_sf, *sp_meta, *dn_codes, *dn_sf;
-  const float* row_scale;
-  const void *w_codes, *w_sf_sp, *w_sf_dn;
-  const float* w_ts;
-  const void* bias;
-  void* Y; int64_t ldy; int out_dtype; int path;
-};
-
 namespace {
 
-constexpr int kMaxExperts = 256;
+constexpr int kMaxExperts = 1024;  // the expert table lives in shared memory (2 x (E + 1) words per CTA)
 constexpr int BM = 128;          // rows of an output tile = TMEM lanes
 constexpr int BK = 256;          // logical k per pipeline stage
 constexpr int kThreads = 192;
 
-#ifdef SHARQ_DEBUG_TS                                    // experiments only: per-CTA phase timestamps (SM clocks)
+#if defined(SHARQ_EXPERIMENTS) && defined(SHARQ_DEBUG_TS)   // experiments only: per-CTA phase timestamps (SM clocks)
 __device__ long long g_dbg_ts[1024 * 16];
 #define SHARQ_TS(i) do { if ((threadIdx.x & 31) == 0 && blockIdx.x < 1024) g_dbg_ts[blockIdx.x * 16 + (i)] = clock64(); } while (0)
 #else
@@ -48,10 +41,13 @@ __device__ long long g_dbg_ts[1024 * 16];
 #endif
 constexpr int kTmemCols = 512;
 
-struct GroupInfo {
-  int32_t E;                               // 0: single problem
-  int32_t blk_prefix[kMaxExperts + 1];     // first 128-row block of expert e (padded row numbering)
-  int32_t count[kMaxExperts];              // valid rows of expert e
+// Grouped (MoE) launches: the expert table is built by every CTA in its own shared memory from the DEVICE array
+// `offsets` (no host copy of the routing result, no device -> host synchronisation after the router):
+// offs[e] = offsets[e], pref[e] = first 128-row block of expert e in the padded row numbering.
+struct GroupTab {
+  const int32_t* offs;                     // shared memory, E + 1 entries (nullptr: single problem)
+  const int32_t* pref;                     // shared memory, E + 1 entries
+  int32_t E;
 };
 
 struct KParams {
@@ -61,7 +57,10 @@ struct KParams {
   void* Y;
   int64_t ldy;
   int32_t T, D, K, out_fp32, path;
-  int32_t m_blocks, total_tiles;
+  int32_t m_blocks, total_tiles;   // grouped: m_blocks = capacity of the activation buffers in 128-row blocks, and
+                                   // both are replaced inside the kernel by the values the expert table gives
+  const int32_t* offsets;          // grouped: device int32[E + 1] (nullptr otherwise)
+  int32_t E;
   int32_t a_rows;     // rows of the activation TMA boxes: 128, or roundup(T, 8) when T < 128 (out-of-bounds
                       // rows are zero-filled slowly; rows beyond the box keep stale smem, which only feeds
                       // accumulator rows that are never stored)
@@ -94,9 +93,10 @@ struct Stage {
   static constexpr int NSL = BN / 16;                                 // 16-column slices of the accumulator
   static constexpr int RECV = SPLIT ? (NSL + 2) * AR * 64 : 0;        // [src][slot][AR rows][16 fp32]; S*ceil(NSL/S) <= NSL+2 for S in {2,3,4,8}
   static constexpr int PAD = AR < 128 ? 128 * 128 : 0;               // the MMA's over-read behind the last stage
-  static constexpr int FIT = (232448 - 1024 - 256 - RECV - PAD) / BYTES;
+  static constexpr int GRP = (!SPLIT && AR == 128 && BN == 128) ? 2 * (kMaxExperts + 1) * 4 + 8 : 0;   // expert table (grouped)
+  static constexpr int FIT = (232448 - 1024 - 256 - RECV - PAD - GRP) / BYTES;
   static constexpr int STAGES = FIT > 8 ? 8 : FIT;
-  static constexpr int SMEM = STAGES * BYTES + PAD + RECV + 1024 /*alignment slack*/ + 256 /*barriers*/;
+  static constexpr int SMEM = STAGES * BYTES + PAD + RECV + 1024 /*alignment slack*/ + 256 /*barriers*/ + GRP;
   // tensor-memory columns: two accumulator stages, then metadata and scale factors
   static constexpr int SFB_COLS = NB * 4;          // columns one MMA's B scales occupy
   static constexpr int ACC_STAGES = BN > 128 ? 1 : 2;
@@ -111,25 +111,26 @@ struct Stage {
 
 struct Unit { int m_blk, n_blk, expert, rows_valid, kb0, kb1; };
 
-__device__ __forceinline__ Unit decode_unit(const KParams& p, const GroupInfo& g, int tile, int rank, int splits) {
+__device__ __forceinline__ Unit decode_unit(const KParams& p, const GroupTab& g, int m_blocks, int total_tiles,
+                                            int tile, int rank, int splits) {
   Unit u;
   if (g.E > 0) {                                   // experts: n fastest, so concurrent CTAs share one expert's
-    const int n_tiles = p.total_tiles / p.m_blocks;  // A block and weights instead of streaming 50 experts at once
+    const int n_tiles = total_tiles / m_blocks;    // A block and weights instead of streaming 50 experts at once
     u.n_blk = tile % n_tiles;
     u.m_blk = tile / n_tiles;
   } else {
-    u.m_blk = tile % p.m_blocks;                   // m fastest: concurrent CTAs share W tiles in L2
-    u.n_blk = tile / p.m_blocks;
+    u.m_blk = tile % m_blocks;                     // m fastest: concurrent CTAs share W tiles in L2
+    u.n_blk = tile / m_blocks;
   }
   u.expert = 0;
   if (g.E > 0) {
     int lo = 0, hi = g.E - 1;                      // last expert whose first block is <= m_blk (binary search)
     while (lo < hi) {
       const int mid = (lo + hi + 1) >> 1;
-      if (g.blk_prefix[mid] <= u.m_blk) lo = mid; else hi = mid - 1;
+      if (g.pref[mid] <= u.m_blk) lo = mid; else hi = mid - 1;
     }
     u.expert = lo;
-    u.rows_valid = min(BM, g.count[u.expert] - (u.m_blk - g.blk_prefix[u.expert]) * BM);
+    u.rows_valid = min(BM, (g.offs[lo + 1] - g.offs[lo]) - (u.m_blk - g.pref[lo]) * BM);
   } else {
     u.rows_valid = min(BM, p.T - u.m_blk * BM);
   }
@@ -168,7 +169,7 @@ __device__ __forceinline__ void store_row(const KParams& p, int64_t row, int col
 template <int BN, int FMT, bool SPLIT, int AR, bool MC = false>
 __global__ void __launch_bounds__(kThreads, 1)
 sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_constant__ CUtensorMap tm_a_dn,
-                    const __grid_constant__ CUtensorMap tm_w, const KParams p, const __grid_constant__ GroupInfo g) {
+                    const __grid_constant__ CUtensorMap tm_w, const KParams p) {
   using S = Stage<BN, FMT, SPLIT, AR>;
   constexpr bool NV = (FMT == SHARQ_NVFP4);
   extern __shared__ uint8_t smem_raw[];
@@ -180,6 +181,7 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
   auto tmem_full_bar = [&](int a) { return bars + 8u * (2 * S::STAGES + a); };
   auto tmem_empty_bar = [&](int a) { return bars + 8u * (2 * S::STAGES + 2 + a); };
   const uint32_t tmem_ptr_smem = bars + 8u * (2 * S::STAGES + 4);
+  int32_t* grp_tab = reinterpret_cast<int32_t*>(smem_raw + (bars + 256u - smem_u32(smem_raw)));   // offs[E+1], pref[E+1]
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   if (warp == 0) SHARQ_TS(0);
@@ -190,7 +192,8 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
   const int rank = SPLIT ? crank : 0;                  // k-slice owner (split-K only)
   const int splits = SPLIT ? (int)tc::cluster_nctarank() : 1;
   const int tile0 = SPLIT ? (int)tc::cluster_id_x() : MC ? 2 * (int)tc::cluster_id_x() + crank : (int)blockIdx.x;
-  const int tile_step = SPLIT ? p.total_tiles : (int)gridDim.x;
+  int m_blocks = p.m_blocks, total_tiles = p.total_tiles;
+  GroupTab g{nullptr, nullptr, 0};
 
   if (warp == 0 && lane == 0) {
     tc::prefetch_tmap(&tm_a_sp);
@@ -221,6 +224,48 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
   asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_ptr_smem));
   tc::grid_launch_dependents();                          // the next kernel may start its own prologue
   if (warp == 0) SHARQ_TS(1);
+  bool dep_synced = false;
+  if constexpr (S::GRP > 0) {
+    if (p.E > 0) {
+      // expert table from the DEVICE offsets (they may be the router's output: wait for the preceding kernel).
+      // Every CTA builds its own copy: E + 1 loads, one warp scan.
+      tc::grid_dependency_wait();
+      dep_synced = true;
+      int32_t* offs = grp_tab;
+      int32_t* pref = grp_tab + (kMaxExperts + 1);
+      for (int i = threadIdx.x; i <= p.E; i += kThreads) offs[i] = p.offsets[i];
+      __syncthreads();
+      if (warp == 0) {
+        const int per = (p.E + 31) / 32;               // lane l scans experts [l * per, l * per + per)
+        int sum = 0;
+        for (int i = 0; i < per; ++i) {
+          const int e = lane * per + i;
+          if (e < p.E) sum += (max(offs[e + 1] - offs[e], 0) + BM - 1) / BM;
+        }
+        int incl = sum;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+          const int t = __shfl_up_sync(0xffffffffu, incl, d);
+          if (lane >= d) incl += t;
+        }
+        int run = incl - sum;
+        for (int i = 0; i < per; ++i) {
+          const int e = lane * per + i;
+          if (e < p.E) {
+            pref[e] = run;
+            run += (max(offs[e + 1] - offs[e], 0) + BM - 1) / BM;
+          }
+        }
+        if (lane == 31) pref[p.E] = incl;
+      }
+      __syncthreads();
+      g.offs = offs; g.pref = pref; g.E = p.E;
+      const int n_tiles = p.total_tiles;               // grouped: the host passes the n-tiles per row block here
+      m_blocks = min(pref[p.E], p.m_blocks);           // never beyond the caller's buffers
+      total_tiles = m_blocks * n_tiles;
+    }
+  }
+  const int tile_step = SPLIT ? total_tiles : (int)gridDim.x;
 
   float split_scale = 0.0f;
   if (warp == 0) {
@@ -234,9 +279,8 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
       if (do_sp) tx += p.a_rows * 64 + 2048 + 1024 + S::NB * 1024;
       if (do_dn) tx += p.a_rows * 128 + S::SF_DN_BYTES + S::NB * S::SF_DN_BYTES;
       uint32_t it = 0;                                   // k-blocks issued so far (ring position)
-      bool dep_synced = false;
-      for (int tile = tile0; tile < p.total_tiles; tile += tile_step) {
-        const Unit u = decode_unit(p, g, tile, rank, splits);
+      for (int tile = tile0; tile < total_tiles; tile += tile_step) {
+        const Unit u = decode_unit(p, g, m_blocks, total_tiles, tile, rank, splits);
         const int w_row0 = u.expert * p.D + u.n_blk * BN;
         const int64_t wblk0 = w_row0 / 128;
         const uint8_t* sfa_sp = p.sp_sf + (size_t)u.m_blk * (Kc / 128) * 512;
@@ -316,8 +360,8 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
       const bool lead = tc::elect_one() != 0;
       const uint32_t idesc_sp = tc::idesc_fp4(BM, BN, true, !NV, 0, 0);
       uint32_t it = 0, n_unit = 0;
-      for (int tile = tile0; tile < p.total_tiles; tile += tile_step, ++n_unit) {
-        const Unit u = decode_unit(p, g, tile, rank, splits);
+      for (int tile = tile0; tile < total_tiles; tile += tile_step, ++n_unit) {
+        const Unit u = decode_unit(p, g, m_blocks, total_tiles, tile, rank, splits);
         const uint32_t sfb_shift = (BN < 128) ? (uint32_t)(((u.n_blk * BN) % 128) / 32) : 0u;   // sub-atom N tiles
         const uint32_t as = n_unit % S::ACC_STAGES;                       // accumulator stage
         const uint32_t acc = tmem_base + as * BN;
@@ -390,8 +434,8 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
     const uint32_t lane_addr = tmem_base + ((uint32_t)(sub * 32) << 16);
     if constexpr (!SPLIT) {
       uint32_t n_unit = 0;
-      for (int tile = tile0; tile < p.total_tiles; tile += tile_step, ++n_unit) {
-        const Unit u = decode_unit(p, g, tile, 0, 1);
+      for (int tile = tile0; tile < total_tiles; tile += tile_step, ++n_unit) {
+        const Unit u = decode_unit(p, g, m_blocks, total_tiles, tile, 0, 1);
         const uint32_t as = n_unit % S::ACC_STAGES;
         const int64_t row = (int64_t)u.m_blk * BM + r_local;
         const bool row_ok = r_local < u.rows_valid;
@@ -416,7 +460,7 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
       }
     } else {
       // ---- split-K: scatter 16-column slices of the partial accumulator to their owner CTAs ----
-      const Unit u = decode_unit(p, g, tile0, rank, splits);
+      const Unit u = decode_unit(p, g, m_blocks, total_tiles, tile0, rank, splits);
       const bool row_ok = r_local < u.rows_valid;
       const int slots = (BN / 16 + splits - 1) / splits;
       // the output scale of this thread's row, fetched while the main loop runs (used after the exchange)
@@ -464,7 +508,7 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
     tc::cluster_sync_all();                              // partial slices have landed in their owners
     if (warp == 2) SHARQ_TS(8);
     if (warp >= 2) {
-      const Unit u = decode_unit(p, g, tile0, rank, splits);
+      const Unit u = decode_unit(p, g, m_blocks, total_tiles, tile0, rank, splits);
       const int r_local = (warp & 3) * 32 + lane;
       if (r_local < u.rows_valid) {
         const int64_t row = (int64_t)u.m_blk * BM + r_local;
@@ -754,8 +798,8 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
-EncodeTiledFn encode_fn() {
-  static EncodeTiledFn fn = [] {
+EncodeTiledFn encode_fn() {                       // driver entry point, resolved once (C++11 thread-safe static)
+  static const EncodeTiledFn fn = [] {
     void* f = nullptr;
     cudaDriverEntryPointQueryResult q;
     if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &f, cudaEnableDefault, &q) != cudaSuccess ||
@@ -781,43 +825,63 @@ bool make_map(CUtensorMap* m, const void* base, uint64_t rows, uint64_t row_byte
             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
+// Device facts the launcher derives once per (kernel variant, device) and then only reads: "the opt-in shared
+// memory size of this kernel is set" and "this many clusters of size c are co-resident".  They are answers of the
+// CUDA runtime about the device, not library state: lock-free, filled idempotently (two threads racing compute the
+// same value), keyed by the device ordinal, a failed query is not cached.
+constexpr int kMaxDevices = 64;
+inline cudaError_t set_smem_once(std::atomic<uint64_t>& done, const void* kfn, int smem, int dev) {
+  if (dev >= 0 && dev < kMaxDevices && ((done.load(std::memory_order_acquire) >> dev) & 1u)) return cudaSuccess;
+  const cudaError_t e = cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+  if (e == cudaSuccess && dev >= 0 && dev < kMaxDevices) done.fetch_or(uint64_t(1) << dev, std::memory_order_release);
+  return e;
+}
+
 // Number of K-splits (cluster size) for a launch with `tiles` output tiles: only when the tiles alone
 // leave most SMs idle, only sizes whose slice exchange fits the receive buffer (2, 3, 4, 8), and only if
 // all `tiles` clusters are co-resident in ONE wave (cluster placement is per GPC, so tiles * S <= SMs is
 // not enough: cudaOccupancyMaxActiveClusters decides).
 template <int BN, int FMT, int AR>
-int choose_splits(int64_t tiles, int num_kb, int num_sms) {
+int choose_splits(int64_t tiles, int num_kb, int num_sms, int dev) {
   if (tiles * 2 > num_sms) return 1;
   using S = Stage<BN, FMT, true, AR>;
-  static int max_clusters[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};      // per cluster size, queried once
+  static std::atomic<int> max_clusters[kMaxDevices][9];          // 0 = not queried yet (zero-initialised)
+  static std::atomic<uint64_t> smem_set{0};
   const int cand[4] = {8, 4, 3, 2};
   for (int c : cand) {
     if (tiles * c > num_sms || num_kb < 2 * c) continue;
-    if (max_clusters[c] == 0) {
+    int n = (dev >= 0 && dev < kMaxDevices) ? max_clusters[dev][c].load(std::memory_order_relaxed) : 0;
+    if (n == 0) {
       cudaLaunchConfig_t lc{};
       cudaLaunchAttribute at[1];
       at[0].id = cudaLaunchAttributeClusterDimension;
       at[0].val.clusterDim.x = (unsigned)c; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
       lc.gridDim = dim3((unsigned)(c * num_sms)); lc.blockDim = dim3(kThreads); lc.dynamicSmemBytes = S::SMEM;
       lc.attrs = at; lc.numAttrs = 1;
-      int n = 0;
       auto kfn = sharq_linear_kernel<BN, FMT, true, AR>;
-      cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, S::SMEM);
-      if (cudaOccupancyMaxActiveClusters(&n, kfn, &lc) != cudaSuccess || n <= 0) n = -1;
-      max_clusters[c] = n;
+      if (set_smem_once(smem_set, (const void*)kfn, S::SMEM, dev) != cudaSuccess) continue;
+      if (cudaOccupancyMaxActiveClusters(&n, kfn, &lc) != cudaSuccess || n <= 0) continue;   // not cached: asked again
+      if (dev >= 0 && dev < kMaxDevices) max_clusters[dev][c].store(n, std::memory_order_relaxed);
     }
-    if (max_clusters[c] >= tiles) return c;
+    if (n >= tiles) return c;
   }
   return 1;
 }
 
+struct LaunchEnv { int num_sms; int dev; cudaStream_t st; LinearPlan* plan_only; };
+
+inline void fill_plan(LinearPlan* pl, int kind, int bn, int ar, int splits, int stages, int64_t tiles, int64_t grid,
+                      int cluster) {
+  pl->kind = kind; pl->bn = bn; pl->act_rows = ar; pl->splits = splits; pl->stages = stages; pl->tiles = tiles;
+  pl->grid = grid; pl->cluster = cluster;
+}
+
 template <int BN, int FMT, int AR>
-sharq_status launch_1cta(const LinearArgs& a, const KParams& p, const GroupInfo& g, const CUtensorMap& tm_sp,
-                         const CUtensorMap& tm_dn, const CUtensorMap& tm_w, int64_t tiles, int num_sms,
-                         cudaStream_t st) {
+sharq_status launch_1cta(const LinearArgs& a, const KParams& p, const CUtensorMap& tm_sp,
+                         const CUtensorMap& tm_dn, const CUtensorMap& tm_w, int64_t tiles, const LaunchEnv& env) {
   constexpr bool kSplitFits = !(BN == 256 && AR == 128);   // no room for the exchange buffers; never needed there
   int splits = 1;
-  if constexpr (kSplitFits) splits = choose_splits<BN, FMT, AR>(tiles, (int)(a.K / BK), num_sms);
+  if constexpr (kSplitFits) if (p.E == 0) splits = choose_splits<BN, FMT, AR>(tiles, (int)(a.K / BK), env.num_sms, env.dev);
   cudaLaunchConfig_t lc{};
   cudaLaunchAttribute attr[2];
   attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
@@ -825,12 +889,13 @@ sharq_status launch_1cta(const LinearArgs& a, const KParams& p, const GroupInfo&
   lc.attrs = attr;
   lc.numAttrs = 1;
   lc.blockDim = dim3(kThreads);
-  lc.stream = st;
+  lc.stream = env.st;
   if constexpr (kSplitFits) if (splits > 1) {
     using S = Stage<BN, FMT, true, AR>;
     auto kfn = sharq_linear_kernel<BN, FMT, true, AR>;
-    if (cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, S::SMEM) != cudaSuccess)
-      return SHARQ_ECUDA;
+    if (env.plan_only) { fill_plan(env.plan_only, 0, BN, AR, splits, S::STAGES, tiles, tiles * splits, splits); return SHARQ_OK; }
+    static std::atomic<uint64_t> smem_set{0};
+    if (set_smem_once(smem_set, (const void*)kfn, S::SMEM, env.dev) != cudaSuccess) return SHARQ_ECUDA;
     lc.gridDim = dim3((unsigned)(tiles * splits));
     lc.dynamicSmemBytes = S::SMEM;
     attr[1].id = cudaLaunchAttributeClusterDimension;
@@ -838,27 +903,30 @@ sharq_status launch_1cta(const LinearArgs& a, const KParams& p, const GroupInfo&
     attr[1].val.clusterDim.y = 1;
     attr[1].val.clusterDim.z = 1;
     lc.numAttrs = 2;
-    return cudaLaunchKernelEx(&lc, kfn, tm_sp, tm_dn, tm_w, p, g) == cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
+    return cudaLaunchKernelEx(&lc, kfn, tm_sp, tm_dn, tm_w, p) == cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
   }
   using S = Stage<BN, FMT, false, AR>;
   auto kfn = sharq_linear_kernel<BN, FMT, false, AR>;
-  if (cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, S::SMEM) != cudaSuccess)
-    return SHARQ_ECUDA;
-  lc.gridDim = dim3((unsigned)(tiles < num_sms ? tiles : num_sms));      // persistent: one CTA per SM
-  if (debug_env().grid > 0) lc.gridDim = dim3((unsigned)debug_env().grid);
+  int64_t grid = tiles < env.num_sms ? tiles : env.num_sms;      // persistent: one CTA per SM
+  if (debug_env().grid > 0) grid = debug_env().grid;
+  if (env.plan_only) { fill_plan(env.plan_only, 0, BN, AR, 1, S::STAGES, tiles, grid, 1); return SHARQ_OK; }
+  static std::atomic<uint64_t> smem_set{0};
+  if (set_smem_once(smem_set, (const void*)kfn, S::SMEM, env.dev) != cudaSuccess) return SHARQ_ECUDA;
+  lc.gridDim = dim3((unsigned)grid);
   lc.dynamicSmemBytes = S::SMEM;
-  return cudaLaunchKernelEx(&lc, kfn, tm_sp, tm_dn, tm_w, p, g) == cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
+  return cudaLaunchKernelEx(&lc, kfn, tm_sp, tm_dn, tm_w, p) == cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
 }
 
 // grouped GEMM: persistent clusters of two CTAs on neighbouring n-tiles, activation operands multicast
 template <int FMT>
-sharq_status launch_mc(const KParams& p, const GroupInfo& g, const CUtensorMap& tm_sp, const CUtensorMap& tm_dn,
-                       const CUtensorMap& tm_w, int64_t tiles, int num_sms, cudaStream_t st) {
+sharq_status launch_mc(const KParams& p, const CUtensorMap& tm_sp, const CUtensorMap& tm_dn,
+                       const CUtensorMap& tm_w, int64_t tiles, const LaunchEnv& env) {
   using S = Stage<128, FMT, false, 128>;
   auto kfn = sharq_linear_kernel<128, FMT, false, 128, true>;
-  if (cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, S::SMEM) != cudaSuccess)
-    return SHARQ_ECUDA;
-  const int64_t clusters = tiles / 2 < num_sms / 2 ? tiles / 2 : num_sms / 2;
+  const int64_t clusters = tiles / 2 < env.num_sms / 2 ? tiles / 2 : env.num_sms / 2;
+  if (env.plan_only) { fill_plan(env.plan_only, 2, 128, 128, 1, S::STAGES, tiles, 2 * clusters, 2); return SHARQ_OK; }
+  static std::atomic<uint64_t> smem_set{0};
+  if (set_smem_once(smem_set, (const void*)kfn, S::SMEM, env.dev) != cudaSuccess) return SHARQ_ECUDA;
   cudaLaunchConfig_t lc{};
   cudaLaunchAttribute attr[2];
   attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
@@ -872,8 +940,8 @@ sharq_status launch_mc(const KParams& p, const GroupInfo& g, const CUtensorMap& 
   lc.blockDim = dim3(kThreads);
   lc.gridDim = dim3((unsigned)(2 * clusters));
   lc.dynamicSmemBytes = S::SMEM;
-  lc.stream = st;
-  return cudaLaunchKernelEx(&lc, kfn, tm_sp, tm_dn, tm_w, p, g) == cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
+  lc.stream = env.st;
+  return cudaLaunchKernelEx(&lc, kfn, tm_sp, tm_dn, tm_w, p) == cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
 }
 
 // scale-factor / metadata array as a 2-D tensor of 1024-byte rows (256 x u32), boxes of `box_rows` rows
@@ -891,25 +959,27 @@ bool make_map_rows1k(CUtensorMap* m, const void* base, uint64_t bytes, uint32_t 
 
 template <int FMT, int PBN>
 sharq_status launch_pair(const LinearArgs& a, const KParams& p, const CUtensorMap& tm_sp, const CUtensorMap& tm_dn,
-                         int64_t m_blocks, int num_sms, cudaStream_t st) {
+                         int64_t m_blocks, const LaunchEnv& env) {
   using P = PairStage<FMT, PBN>;
+  const int64_t pair_tiles = ((m_blocks + 1) / 2) * ((a.D + PBN - 1) / PBN);
+  int64_t clusters = pair_tiles < env.num_sms / 2 ? pair_tiles : env.num_sms / 2;
+  if (debug_env().pair_clusters > 0 && debug_env().pair_clusters < clusters) clusters = debug_env().pair_clusters;
+  if (env.plan_only) { fill_plan(env.plan_only, 1, PBN, 128, 1, P::STAGES, pair_tiles, 2 * clusters, 2); return SHARQ_OK; }
   CUtensorMap tm_wp, tm_sfa_sp, tm_sfa_dn, tm_meta, tm_sfb_sp, tm_sfb_dn;
   const uint64_t act_rows = (uint64_t)m_blocks * 128, kk = (uint64_t)a.K;
   const uint32_t dn_rows = P::SF_DN_BYTES / 1024;
   const uint64_t dn_div = (FMT == SHARQ_NVFP4) ? 16 : 32;
+  const uint64_t w_rows_pad = (uint64_t)round_up(a.D, 128);       // the scale views are padded to whole 128-row atoms
   if (!make_map(&tm_wp, a.w_codes, (uint64_t)a.D, kk / 2, 128, P::HALF) ||
       !make_map_rows1k(&tm_sfa_sp, a.sp_sf, act_rows * kk / 32, 1) ||
       !make_map_rows1k(&tm_sfa_dn, a.dn_sf, act_rows * kk / dn_div, dn_rows) ||
       !make_map_rows1k(&tm_meta, a.sp_meta, act_rows * kk / 16, 2) ||
-      !make_map_rows1k(&tm_sfb_sp, a.w_sf_sp, (uint64_t)a.D * kk / 32, 1) ||
-      !make_map_rows1k(&tm_sfb_dn, a.w_sf_dn, (uint64_t)a.D * kk / dn_div, dn_rows))
+      !make_map_rows1k(&tm_sfb_sp, a.w_sf_sp, w_rows_pad * kk / 32, 1) ||
+      !make_map_rows1k(&tm_sfb_dn, a.w_sf_dn, w_rows_pad * kk / dn_div, dn_rows))
     return SHARQ_ECUDA;
   auto kfn = sharq_linear_pair_kernel<FMT, PBN>;
-  if (cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, P::SMEM) != cudaSuccess)
-    return SHARQ_ECUDA;
-  const int64_t pair_tiles = ((m_blocks + 1) / 2) * ((a.D + PBN - 1) / PBN);
-  int64_t clusters = pair_tiles < num_sms / 2 ? pair_tiles : num_sms / 2;
-  if (debug_env().pair_clusters > 0 && debug_env().pair_clusters < clusters) clusters = debug_env().pair_clusters;
+  static std::atomic<uint64_t> smem_set{0};
+  if (set_smem_once(smem_set, (const void*)kfn, P::SMEM, env.dev) != cudaSuccess) return SHARQ_ECUDA;
   cudaLaunchConfig_t lp{};
   cudaLaunchAttribute at[2];
   at[0].id = cudaLaunchAttributeClusterDimension;
@@ -921,27 +991,32 @@ sharq_status launch_pair(const LinearArgs& a, const KParams& p, const CUtensorMa
   lp.blockDim = dim3(kThreads);
   lp.gridDim = dim3((unsigned)(2 * clusters));
   lp.dynamicSmemBytes = P::SMEM;
-  lp.stream = st;
+  lp.stream = env.st;
   lp.attrs = at;
   lp.numAttrs = 2;
   return cudaLaunchKernelEx(&lp, kfn, tm_sp, tm_dn, tm_wp, tm_sfa_sp, tm_sfa_dn, tm_meta, tm_sfb_sp, tm_sfb_dn, p) ==
                  cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
 }
 
+// rows_total = rows the activation tensor maps cover (T; grouped: the capacity of the caller's padded buffers)
 template <int BN, int FMT>
-sharq_status launch_tiles(const LinearArgs& a, const GroupInfo& g, int64_t rows_total, int64_t m_blocks, int E,
-                          int num_sms, cudaStream_t st) {
+sharq_status launch_tiles(const LinearArgs& a, int64_t rows_total, int64_t m_blocks, int E, const int32_t* offsets,
+                          const LaunchEnv& env) {
+  const int num_sms = env.num_sms;
   CUtensorMap tm_sp, tm_dn, tm_w;
   const int64_t w_rows = (int64_t)(E > 0 ? E : 1) * a.D;
-  const uint32_t a_rows = (m_blocks == 1 && rows_total < BM) ? (uint32_t)((rows_total + 7) / 8 * 8) : BM;
-  if (!make_map(&tm_sp, a.sp_codes, (uint64_t)rows_total, (uint64_t)a.K / 4, 64, a_rows) ||
-      !make_map(&tm_dn, a.dn_codes, (uint64_t)rows_total, (uint64_t)a.K / 2, 128, a_rows) ||
-      !make_map(&tm_w, a.w_codes, (uint64_t)w_rows, (uint64_t)a.K / 2, 128, BN < 256 ? BN : 256))
+  const uint32_t a_rows = (E == 0 && m_blocks == 1 && rows_total < BM) ? (uint32_t)((rows_total + 7) / 8 * 8) : BM;
+  if (!env.plan_only &&
+      (!make_map(&tm_sp, a.sp_codes, (uint64_t)rows_total, (uint64_t)a.K / 4, 64, a_rows) ||
+       !make_map(&tm_dn, a.dn_codes, (uint64_t)rows_total, (uint64_t)a.K / 2, 128, a_rows) ||
+       !make_map(&tm_w, a.w_codes, (uint64_t)w_rows, (uint64_t)a.K / 2, 128, BN < 256 ? BN : 256)))
     return SHARQ_ECUDA;
-  const int64_t tiles = m_blocks * (a.D / BN);
+  const int64_t n_tiles = a.D / BN;
+  const int64_t tiles = m_blocks * n_tiles;                  // grouped: an upper bound (the kernel knows the real count)
   KParams p{(const uint8_t*)a.sp_sf, (const uint8_t*)a.sp_meta, (const uint8_t*)a.dn_sf, (const uint8_t*)a.w_sf_sp,
             (const uint8_t*)a.w_sf_dn, a.row_scale, a.w_ts, (const uint16_t*)a.bias, a.Y, a.ldy,
-            (int32_t)a.T, (int32_t)a.D, (int32_t)a.K, a.out_dtype, a.path, (int32_t)m_blocks, (int32_t)tiles, (int32_t)a_rows};
+            (int32_t)a.T, (int32_t)a.D, (int32_t)a.K, a.out_dtype, a.path, (int32_t)m_blocks,
+            (int32_t)(E > 0 ? n_tiles : tiles), offsets, (int32_t)E, (int32_t)a_rows};
   const bool pair_worth = ((m_blocks + 1) / 2) * (a.D / 256) >= num_sms / 4 || debug_env().force_pair;
   if (E == 0 && m_blocks >= 2 && BN == 128 && pair_worth && !debug_env().no_pair) {
     // tile width by a cost model fitted on the box over the eight Llama / Qwen prefill shapes at T = 2048 ..
@@ -954,17 +1029,16 @@ sharq_status launch_tiles(const LinearArgs& a, const GroupInfo& g, int64_t rows_
     const double cost256 = (double)((m_pairs * ((a.D + 255) / 256) + clusters - 1) / clusters) * (0.5375 * kb + 4.5);
     int width = (a.D % 256 != 0 || cost192 < cost256) ? 192 : 256;
     if (debug_env().pair_bn > 0) width = (debug_env().pair_bn == 256 && a.D % 256 == 0) ? 256 : 192;
-    if (width == 256) return launch_pair<FMT, 256>(a, p, tm_sp, tm_dn, m_blocks, num_sms, st);
-    return launch_pair<FMT, 192>(a, p, tm_sp, tm_dn, m_blocks, num_sms, st);
+    if (width == 256) return launch_pair<FMT, 256>(a, p, tm_sp, tm_dn, m_blocks, env);
+    return launch_pair<FMT, 192>(a, p, tm_sp, tm_dn, m_blocks, env);
   }
   if constexpr (BN == 128) {
     // experts: n-tiles of one 128-row block are consecutive (decode_unit), so tiles 2j and 2j+1 share activations
-    if (E > 0 && (a.D / BN) % 2 == 0 && a_rows == (uint32_t)BM && !debug_env().no_mc)
-      return launch_mc<FMT>(p, g, tm_sp, tm_dn, tm_w, tiles, num_sms, st);
+    if (E > 0 && n_tiles % 2 == 0 && !debug_env().no_mc) return launch_mc<FMT>(p, tm_sp, tm_dn, tm_w, tiles, env);
   }
-  if (a_rows <= 16) return launch_1cta<BN, FMT, 16>(a, p, g, tm_sp, tm_dn, tm_w, tiles, num_sms, st);
-  if (a_rows <= 64) return launch_1cta<BN, FMT, 64>(a, p, g, tm_sp, tm_dn, tm_w, tiles, num_sms, st);
-  return launch_1cta<BN, FMT, 128>(a, p, g, tm_sp, tm_dn, tm_w, tiles, num_sms, st);
+  if (a_rows <= 16) return launch_1cta<BN, FMT, 16>(a, p, tm_sp, tm_dn, tm_w, tiles, env);
+  if (a_rows <= 64) return launch_1cta<BN, FMT, 64>(a, p, tm_sp, tm_dn, tm_w, tiles, env);
+  return launch_1cta<BN, FMT, 128>(a, p, tm_sp, tm_dn, tm_w, tiles, env);
 }
 
 }  // namespace
@@ -977,25 +1051,28 @@ size_t linear_workspace_bytes(const sharq_config* cfg, int64_t T, int64_t D, int
   return cfg->fmt == SHARQ_HIF4 ? hif4_linear_workspace_bytes(T, D, K) : 0;   // bf16 copies of A and W
 }
 
-sharq_status launch_linear(const sharq_config* cfg, const LinearArgs& a, int32_t E, const int32_t* offsets_host,
-                           void* workspace, size_t workspace_bytes, int num_sms, cudaStream_t st) {
-  if (cfg->fmt == SHARQ_HIF4)                             // no FP4-rate tensor path: exact bf16 emulation
-    return E > 0 ? SHARQ_EINVAL : launch_linear_hif4(a, workspace, workspace_bytes, num_sms, st);
-  if (a.K > (int64_t)1 << 24 || a.D > (int64_t)1 << 24) return SHARQ_ESHAPE;
-  GroupInfo g{};
+// E > 0: grouped; `offsets` is the DEVICE int32[E + 1] array, a.T the row capacity of the padded activation buffers.
+// plan_only != nullptr: fill it with the launch configuration this call would use and launch nothing.
+sharq_status launch_linear(const sharq_config* cfg, const LinearArgs& a, int32_t E, const int32_t* offsets,
+                           void* workspace, size_t workspace_bytes, int num_sms, int dev, cudaStream_t st,
+                           LinearPlan* plan_only) {
+  if (cfg->fmt == SHARQ_HIF4) {                           // no FP4-rate tensor path: exact bf16 emulation
+    if (E > 0) return SHARQ_EINVAL;
+    if (plan_only) {
+      const int bn = a.D % 256 == 0 ? 256 : 128;
+      const int64_t tiles = ((a.T + 127) / 128) * (a.D / bn);
+      fill_plan(plan_only, 3, bn, 128, 1, bn == 256 ? 4 : 6, tiles, tiles < num_sms ? tiles : num_sms, 1);
+      return SHARQ_OK;
+    }
+    return launch_linear_hif4(a, workspace, workspace_bytes, num_sms, st);
+  }
+  if (a.K > (int64_t)1 << 24 || a.D > (int64_t)1 << 24 || a.T > (int64_t)1 << 30) return SHARQ_ESHAPE;
+  const LaunchEnv env{num_sms, dev, st, plan_only};
   int64_t rows_total = a.T, m_blocks = (a.T + BM - 1) / BM;
   if (E > 0) {
     if (E > kMaxExperts) return SHARQ_ESHAPE;
-    g.E = E;
-    int32_t blk = 0;
-    for (int e = 0; e < E; ++e) {
-      g.blk_prefix[e] = blk;
-      g.count[e] = offsets_host[e + 1] - offsets_host[e];
-      blk += (g.count[e] + BM - 1) / BM;
-    }
-    g.blk_prefix[E] = blk;
-    m_blocks = blk;
-    rows_total = (int64_t)blk * BM;
+    m_blocks = a.T / BM;                                  // whole 128-row blocks of the caller's buffers
+    rows_total = m_blocks * BM;
     if (m_blocks == 0) return SHARQ_OK;
   }
   if (m_blocks * (a.D / 128) > (int64_t)1 << 30) return SHARQ_ESHAPE;
@@ -1004,14 +1081,14 @@ sharq_status launch_linear(const sharq_config* cfg, const LinearArgs& a, int32_t
   // ... and only pays when the 128-wide tiles would need a second round on the SMs (measured: with fewer
   // tiles than SMs the narrower tiles + deeper K-split win)
   if (E == 0 && a.T <= debug_env().wide_t && a.D % 256 == 0 && a.D / 128 > num_sms && !debug_env().no_wide) {
-    if (cfg->fmt == SHARQ_NVFP4) return launch_tiles<256, SHARQ_NVFP4>(a, g, rows_total, m_blocks, E, num_sms, st);
-    return launch_tiles<256, SHARQ_MXFP4>(a, g, rows_total, m_blocks, E, num_sms, st);
+    if (cfg->fmt == SHARQ_NVFP4) return launch_tiles<256, SHARQ_NVFP4>(a, rows_total, m_blocks, E, offsets, env);
+    return launch_tiles<256, SHARQ_MXFP4>(a, rows_total, m_blocks, E, offsets, env);
   }
-  if (cfg->fmt == SHARQ_NVFP4) return launch_tiles<128, SHARQ_NVFP4>(a, g, rows_total, m_blocks, E, num_sms, st);
-  return launch_tiles<128, SHARQ_MXFP4>(a, g, rows_total, m_blocks, E, num_sms, st);
+  if (cfg->fmt == SHARQ_NVFP4) return launch_tiles<128, SHARQ_NVFP4>(a, rows_total, m_blocks, E, offsets, env);
+  return launch_tiles<128, SHARQ_MXFP4>(a, rows_total, m_blocks, E, offsets, env);
 }
 
-#ifdef SHARQ_DEBUG_TS
+#if defined(SHARQ_EXPERIMENTS) && defined(SHARQ_DEBUG_TS)
 extern "C" int sharq_debug_read_ts(long long* host_out) {
   return (int)cudaMemcpyFromSymbol(host_out, g_dbg_ts, sizeof(long long) * 1024 * 16);
 }

@@ -14,19 +14,10 @@
 #include <cuda_runtime.h>
 
 #include "common.cuh"
+#include "linear_args.h"
 #include "tc_ptx.cuh"
 
 namespace sharq {
-
-struct LinearArgs {
-  int64_t T, D, K;
-  const void *sp_codes, *sp_sf, *sp_meta, *dn_codes, *dn_sf;
-  const float* row_scale;
-  const void *w_codes, *w_sf_sp, *w_sf_dn;
-  const float* w_ts;
-  const void* bias;
-  void* Y; int64_t ldy; int out_dtype; int path;
-};
 
 namespace {
 

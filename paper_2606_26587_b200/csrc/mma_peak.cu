@@ -6,6 +6,7 @@
 // result is the ceiling of the GEMM's main loop on this GPU at the clocks of the moment.
 #include <cuda_runtime.h>
 
+#include "../../include/sharq_diag.h"
 #include "common.cuh"
 #include "tc_ptx.cuh"
 

@@ -150,7 +150,8 @@ __global__ void __launch_bounds__(512) sharq_prepare_kernel(const PrepParams p) 
       if (FMT == SHARQ_HIF4) {
         quantize_block_hif4(p, row, (uint32_t)k0, X, lane, act);
       } else if (act) {
-        quantize_block_e2m1<FMT>(p, row, (uint32_t)k0, X, ts, inv_ts);
+        if (p.mask24) quantize_block_e2m1_24<FMT>(p, row, (uint32_t)k0, X, ts, inv_ts);
+        else quantize_block_e2m1<FMT>(p, row, (uint32_t)k0, X, ts, inv_ts);
       }
     }
     __syncwarp();   // all lanes are done with `buf` before it is refilled
@@ -295,11 +296,12 @@ cudaError_t launch_prepare(const sharq_config* cfg, const void* x, int64_t T, in
   p.eps = cfg->eps; p.tiled = (cfg->layout == SHARQ_LAYOUT_TILED);
   p.row_bytes = (uint32_t)(K * 2);
   p.idx_tags = 0x0004080Cu;
+  p.mask24 = (cfg->fmt != SHARQ_HIF4 && cfg->mask == SHARQ_MASK_24) ? 1 : 0;
   // the row kernel reads 32 bytes per load: rows must start on 32-byte boundaries, otherwise (16-byte aligned
   // input, the C ABI's minimum) the warp-per-row kernel with its 16-byte cp.async takes the call
   const bool wide_ok = ((uintptr_t)x % 32 == 0) && (ldx % 16 == 0);
-  if (residual && (!wide_ok || K > 1024 * kRowMaxWarps)) return cudaErrorInvalidValue;   // checked by the C ABI
-  if (K <= 1024 * kRowMaxWarps && wide_ok && (!debug_env().old_prepare || residual)) {
+  if (residual && (!wide_ok || K > 1024 * kRowMaxWarps || p.mask24)) return cudaErrorInvalidValue;   // checked by the C ABI
+  if (K <= 1024 * kRowMaxWarps && wide_ok && !p.mask24 && (!debug_env().old_prepare || residual)) {
     p.nbuf = 0;
     if (cfg->fmt == SHARQ_NVFP4) return launch_row_chunks<SHARQ_NVFP4>(cfg->norm, p, num_sms, st);
     if (cfg->fmt == SHARQ_MXFP4) return launch_row_chunks<SHARQ_MXFP4>(cfg->norm, p, num_sms, st);
@@ -437,6 +439,22 @@ cudaError_t launch_quantize_weight(const sharq_config* cfg, const void* W, int64
   else if (cfg->fmt == SHARQ_MXFP4) SHARQ_WQ(SHARQ_MXFP4);
   else SHARQ_WQ(SHARQ_HIF4);
 #undef SHARQ_WQ
+  return cudaGetLastError();
+}
+
+// ---- test helpers: TILED -> canonical (include/sharq.h "Output layouts"); pure index maps --------------------------
+__global__ void untile_kernel(const uint8_t* __restrict__ tiled, int64_t R, int64_t C, uint8_t* __restrict__ canonical,
+                              int meta) {
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < R * C; i += (int64_t)gridDim.x * blockDim.x) {
+    const int64_t r = i / C, c = i % C;
+    canonical[i] = tiled[meta ? meta_tiled_offset(r, c, C * 16) : sf_tiled_offset(r, c, C)];
+  }
+}
+
+cudaError_t launch_untile(const void* tiled, int64_t R, int64_t C, void* canonical, int meta, cudaStream_t st) {
+  const int64_t n = R * C;
+  const unsigned blocks = (unsigned)((n + 255) / 256 < 4096 ? (n + 255) / 256 : 4096);
+  untile_kernel<<<blocks, 256, 0, st>>>((const uint8_t*)tiled, R, C, (uint8_t*)canonical, meta);
   return cudaGetLastError();
 }
 

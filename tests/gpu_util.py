@@ -39,10 +39,19 @@ def act_to_canonical(sq, cfg, act, T, K):
         out["sp_meta"] = host(act["sp_meta"], T * K // 8).reshape(T, K // 8)
         return out
     Cd = K // 16 if fmt == sq.NVFP4 else K // 32
-    if cfg.layout == sq.LAYOUT_TILED:
-        out["sp_sf"] = untile_sf(host(act["sp_sf"]), T, K // 32)
-        out["dn_sf"] = untile_sf(host(act["dn_sf"]), T, Cd)
-        out["sp_meta"] = untile_meta(host(act["sp_meta"]), T, K)
+    if cfg.mask == sq.MASK_24:                              # element-wise 2:4 on E2M1: canonical only, K/8 metadata bytes
+        out["sp_sf"] = host(act["sp_sf"], T * K // 32).reshape(T, K // 32)
+        out["dn_sf"] = host(act["dn_sf"], T * Cd).reshape(T, Cd)
+        out["sp_meta"] = host(act["sp_meta"], T * K // 8).reshape(T, K // 8)
+    elif cfg.layout == sq.LAYOUT_TILED:
+        # through the C ABI's own helpers (sharq_untile_sf / sharq_untile_meta) AND the numpy restatement of the
+        # header's formulas: the two must agree, so neither the kernel's tiling nor the helper can drift alone
+        out["sp_sf"] = host(sq.untile_sf(act["sp_sf"], T, K // 32))
+        out["dn_sf"] = host(sq.untile_sf(act["dn_sf"], T, Cd))
+        out["sp_meta"] = host(sq.untile_meta(act["sp_meta"], T, K))
+        assert np.array_equal(out["sp_sf"], untile_sf(host(act["sp_sf"]), T, K // 32))
+        assert np.array_equal(out["dn_sf"], untile_sf(host(act["dn_sf"]), T, Cd))
+        assert np.array_equal(out["sp_meta"], untile_meta(host(act["sp_meta"]), T, K))
     else:
         out["sp_sf"] = host(act["sp_sf"], T * K // 32).reshape(T, K // 32)
         out["dn_sf"] = host(act["dn_sf"], T * Cd).reshape(T, Cd)
@@ -58,8 +67,10 @@ def weight_to_canonical(sq, cfg, wq, D, K):
         return out
     Cd = K // 16 if cfg.fmt == sq.NVFP4 else K // 32
     if cfg.layout == sq.LAYOUT_TILED:
-        out["sf_sp"] = untile_sf(host(wq["sf_sp"]), D, K // 32)
-        out["sf_dn"] = untile_sf(host(wq["sf_dn"]), D, Cd)
+        out["sf_sp"] = host(sq.untile_sf(wq["sf_sp"], D, K // 32))
+        out["sf_dn"] = host(sq.untile_sf(wq["sf_dn"], D, Cd))
+        assert np.array_equal(out["sf_sp"], untile_sf(host(wq["sf_sp"]), D, K // 32))
+        assert np.array_equal(out["sf_dn"], untile_sf(host(wq["sf_dn"]), D, Cd))
     else:
         out["sf_sp"] = host(wq["sf_sp"], D * K // 32).reshape(D, K // 32)
         out["sf_dn"] = host(wq["sf_dn"], D * Cd).reshape(D, Cd)

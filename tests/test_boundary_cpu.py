@@ -18,8 +18,10 @@ def sq():
 
 
 def test_every_declared_symbol_is_exported(sq):
-    header = open(os.path.join(ROOT, "include", "sharq.h")).read()
-    declared = set(re.findall(r"\b(sharq_[a-z_]+)\s*\(", header))
+    declared = set()
+    for h in ("sharq.h", "sharq_diag.h"):
+        text = re.sub(r"/\*.*?\*/", "", open(os.path.join(ROOT, "include", h)).read(), flags=re.S)   # comments mention calls too
+        declared |= set(re.findall(r"\b(sharq_[a-z0-9_]+)\s*\(", text))
     assert declared == set(sq.EXPORTS)
     for name in declared:
         assert getattr(sq.capi, name) is not None
@@ -64,10 +66,28 @@ def test_argument_validation_returns_codes_without_touching_cuda(sq):
     assert g(ctypes.byref(cfg), 16, 64, 4, 1024, 1024, 1024, 96, 1024, *ok_ptrs, null) == sq.EINVAL      # x 16-byte aligned only
     assert g(ctypes.byref(cfg), 32, null, 4, 1024, 1024, 1024, 96, 1024, *ok_ptrs, null) == sq.EINVAL    # no residual
     assert g(ctypes.byref(cfg), 32, 64, 4, 1024, 1024, 1024, 32, 1024, *ok_ptrs, null) == sq.EINVAL      # sum_out aliases x
-    # element-wise 2:4 with NVFP4 has no tensor-core path on B200 (R2)
+    # element-wise 2:4 with NVFP4 / MXFP4: accepted by sharq_prepare / sharq_act_sizes in the canonical layout
+    # (metadata K/8 bytes per row), refused by everything on the GEMM side: B200 has no such FP4 MMA (R2)
+    m24 = sq.Config(sq.NVFP4, sq.MASK_24, sq.NORM_NONE, 1e-6, sq.LAYOUT_CANONICAL)
+    assert sq.act_sizes(m24, 16, 1024) == (16 * 256, 16 * 32, 16 * 128, 16 * 512, 16 * 64, 64)
+    assert f(ctypes.byref(m24), 16, 0, 1024, 1024, *([16] * 9), null) == sq.OK
+    with pytest.raises(sq.SharqError) as e:
+        sq.linear_workspace(m24, 16, 128, 1024)
+    assert e.value.status == sq.ESHAPE
     bad = sq.Config(sq.NVFP4, sq.MASK_24, sq.NORM_NONE, 1e-6, sq.LAYOUT_TILED)
     with pytest.raises(sq.SharqError):
         sq.act_sizes(bad, 16, 1024)
+    # sharq_linear_grouped: offsets is a device pointer; E, padded_rows are validated on the host
+    lg = sq.capi.sharq_linear_grouped
+    ptrs9 = [16] * 10                                     # 5 activation operands, row_scale, 3 weight tensors, ts_w
+    assert lg(ctypes.byref(cfg), 4, 16, 100, 128, 256, *ptrs9, 16, 128, 0, null, 0, null) == sq.ESHAPE     # padded_rows % 128
+    assert lg(ctypes.byref(cfg), 2000, 16, 128, 128, 256, *ptrs9, 16, 128, 0, null, 0, null) == sq.ESHAPE  # E > 1024
+    assert lg(ctypes.byref(cfg), 4, null, 128, 128, 256, *ptrs9, 16, 128, 0, null, 0, null) == sq.EINVAL   # no offsets
+    assert lg(ctypes.byref(cfg), 4, 16, 0, 128, 256, *ptrs9, 16, 128, 0, null, 0, null) == sq.OK           # nothing to do
+    # untile helpers: shape rules
+    assert sq.capi.sharq_untile_sf(16, 4, 6, 16, null) == sq.ESHAPE
+    assert sq.capi.sharq_untile_meta(16, 4, 1000, 16, null) == sq.ESHAPE
+    assert sq.capi.sharq_untile_sf(16, 0, 8, 16, null) == sq.OK
     with pytest.raises(sq.SharqError):
         sq.act_sizes(cfg, 16, 1000)
     with pytest.raises(sq.SharqError):

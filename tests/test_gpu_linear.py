@@ -276,7 +276,68 @@ def test_prefill_launch_variants_sampled(sq, fmt, norm, T, K, D, mult):
     kernel with 192- and 256-wide tiles, a ragged last N tile, ragged T and an odd number of 128-row blocks.
     The sampled output features always include the last 64 columns (the tail of a ragged last tile) and the
     sampled rows the first / last rows of the last row block."""
+    plan = sq.linear_plan(sq.make_config(fmt, norm, 1e-6, sq.LAYOUT_TILED), T, D, K)
+    assert plan.startswith("pair "), plan                           # every prefill shape runs on CTA-pair tiles
+    if D % 256 != 0:
+        assert "bn=256" not in plan, plan                           # a ragged last N tile
     _sampled_check(sq, fmt, norm, T, K, D, config=3, mult=mult, n_rows=20, n_cols=160, seed_extra=T + D + fmt)
+
+
+def test_linear_plan_names_the_variants_the_tests_cover(sq):
+    """sharq_linear_plan: the decode / prefill / MoE shapes of BASELINE.json map onto the kernel variants the parity
+    tests above run (split-K clusters, 128 x 256 tiles, persistent tiles, CTA pairs of both widths, multicast)."""
+    cfg = sq.make_config(0, 0, 1e-6, sq.LAYOUT_TILED)
+    plans = {name: sq.linear_plan(cfg, T, D, K, E) for name, (T, D, K, E) in dict(
+        o_T1=(1, 4096, 4096, 0), gate_up_T128=(128, 28672, 4096, 0), down_T256=(256, 4096, 14336, 0),
+        o_T4096=(4096, 4096, 4096, 0), down_T4096=(4096, 4096, 14336, 0), moe_gate_up=(40576, 1536, 2048, 128),
+        moe_down=(40576, 2048, 768, 128)).items()}
+    assert plans["o_T1"].startswith("tile bn=128 act_rows=16") and "splits=1 " not in plans["o_T1"], plans
+    assert plans["gate_up_T128"].startswith("tile bn=256"), plans
+    assert plans["o_T4096"].startswith("pair "), plans
+    assert plans["down_T4096"].startswith("pair "), plans
+    assert plans["moe_gate_up"].startswith("grouped-mc") and plans["moe_down"].startswith("grouped-mc"), plans
+    assert sq.linear_plan(sq.make_config(2, 0), 4096, 3584, 18944).startswith("hif4-bf16")
+
+
+def test_linear_grouped_device_offsets_and_spare_capacity(sq):
+    """sharq_linear_grouped reads `offsets` on the DEVICE (no host copy): a device tensor, buffers larger than the
+    padded total (roundup(total, 128) + 128 E), an odd number of n-tiles (the non-multicast grouped path) and a
+    capacity that is too SMALL (extra row blocks are skipped, nothing is written beyond the buffers)."""
+    E, K = 5, 512
+    counts = [3, 0, 257, 128, 64]
+    offsets = np.concatenate([[0], np.cumsum(counts)]).astype(np.int32)
+    pad_off = np.concatenate([[0], np.cumsum([-(-c // 128) * 128 for c in counts])])
+    cap = int(-(-offsets[-1] // 128) * 128 + 128 * E)
+    cfg = sq.make_config(sq.NVFP4, sq.NORM_NONE, 1e-6, sq.LAYOUT_TILED)
+    for D in (256, 384):                                            # 2 n-tiles (multicast clusters) / 3 (plain persistent)
+        act = sq.alloc_act(cfg, cap, K, "cuda")
+        ws, xs = [], []
+        for e in range(E):
+            ws.append(si.weight(D, K, 5, extra=50 + e))
+            xs.append(si.activations(counts[e], K, config=5, extra=60 + e))
+            if counts[e]:
+                sq.prepare(cfg, to_dev(xs[e]), out=sq.act_slot(cfg, act, int(pad_off[e]), counts[e]))
+        wqs = [sq.quantize_weight(cfg, to_dev(w)) for w in ws]
+        wq = dict(codes=torch.cat([q["codes"] for q in wqs]), sf_sp=torch.cat([q["sf_sp"] for q in wqs]),
+                  sf_dn=torch.cat([q["sf_dn"] for q in wqs]), ts_w=torch.cat([q["ts_w"] for q in wqs]), D=D, K=K)
+        offs_dev = torch.from_numpy(offsets).cuda()
+        Y = torch.full((cap, D), 7.0, dtype=torch.float32, device="cuda")
+        sq.linear_grouped(cfg, offs_dev, act, wq, D, Y=Y)
+        torch.cuda.synchronize()
+        Yh = Y.cpu().numpy()
+        for e in range(E):
+            if counts[e]:
+                y64 = so.linear(so.prepare(xs[e], norm=0), so.quantize_weight(ws[e]))
+                assert rel_err(Yh[pad_off[e]: pad_off[e] + counts[e]], y64).max() <= TOL, f"D{D} expert {e}"
+        assert (Yh[pad_off[-1]:] == 7.0).all(), "rows beyond the padded total were written"
+        # capacity of 4 row blocks only (experts 0, 2 (two of its three blocks... all three), 3 need 1 + 3 + 1 + 1 = 6)
+        small = dict(act, T=4 * 128)
+        Y2 = torch.full((cap, D), 7.0, dtype=torch.float32, device="cuda")
+        sq.linear_grouped(cfg, offs_dev, small, wq, D, Y=Y2)
+        torch.cuda.synchronize()
+        Y2h = Y2.cpu().numpy()
+        assert (Y2h[4 * 128:] == 7.0).all(), "row blocks beyond padded_rows were computed"
+        assert np.array_equal(Y2h[:3], Yh[:3])
 
 
 def test_moe_config5_down_projection_sampled(sq):

@@ -187,3 +187,35 @@ def test_prepare_rows_not_32_byte_aligned(sq):
     _compare_act(act_to_canonical(sq, cfg, act, T, K), p, "misaligned")
     with pytest.raises(sq.SharqError):
         sq.prepare_add(cfg, view, to_dev(x), to_dev(g))
+
+
+@pytest.mark.parametrize("fmt,norm,T,K", [(0, 1, 16, 4096), (0, 0, 37, 3584), (1, 1, 9, 768), (1, 2, 5, 33792), (0, 2, 130, 1024)])
+def test_prepare_mask24_on_e2m1_formats_bit_exact(sq, fmt, norm, T, K):
+    """SHARQ_MASK_24 (element-wise 2:4, P:95 / P:124) with NVFP4 / MXFP4: accepted by sharq_prepare,
+    canonical layout, metadata K/8 bytes per row; sharq_linear refuses it (no such FP4 MMA on B200)."""
+    x = si.activations(T, K, config=1, outlier_mult=50.0, extra=3 * K + T)
+    g, b = si.gamma(K, 1), si.beta(K, 1)
+    cfg = sq.make_config(fmt, norm, 1e-6, sq.LAYOUT_CANONICAL, mask=sq.MASK_24)
+    act = sq.prepare(cfg, to_dev(x), to_dev(g) if norm else None, to_dev(b) if norm == 2 else None)
+    torch.cuda.synchronize()
+    p = so.prepare(x, fmt=fmt, mask=so.MASK_24, norm=norm, gamma_u16=g, beta_u16=b if norm == 2 else None)
+    assert p["sp_meta"].shape == (T, K // 8)
+    _compare_act(act_to_canonical(sq, cfg, act, T, K), p, f"mask24 fmt{fmt} norm{norm} T{T} K{K}")
+    w = sq.quantize_weight(sq.make_config(fmt, 0, 1e-6, sq.LAYOUT_CANONICAL, mask=sq.MASK_24), to_dev(si.weight(128, K, 1)))
+    with pytest.raises(sq.SharqError) as e:
+        sq.linear(cfg, act, w)
+    assert e.value.status == sq.ESHAPE
+
+
+def test_tiled_pad_rows_are_initialised(sq):
+    """TILED scale / metadata buffers are padded to 128 rows; alloc_act -> sharq_act_init gives the pad rows valid
+    operands (zero scales, metadata nibble 0x4) and sharq_prepare leaves them alone."""
+    T, K = 5, 512
+    cfg = sq.make_config(0, 0, 1e-6, sq.LAYOUT_TILED)
+    act = sq.prepare(cfg, to_dev(si.activations(T, K, config=1)))
+    torch.cuda.synchronize()
+    sf = sq.untile_sf(act["sp_sf"], 128, K // 32).cpu().numpy()
+    dn = sq.untile_sf(act["dn_sf"], 128, K // 16).cpu().numpy()
+    meta = sq.untile_meta(act["sp_meta"], 128, K).cpu().numpy()
+    assert (sf[T:] == 0).all() and (dn[T:] == 0).all() and (meta[T:] == 0x44).all()
+    assert (meta[:T] != 0).all()
