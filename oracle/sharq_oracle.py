@@ -397,6 +397,101 @@ def prepare(x_u16, fmt=NVFP4, mask=MASK_PAIR48, norm=NORM_RMS, gamma_u16=None, b
 
 
 # --------------------------------------------------------------------------------------------
+# Path combinations of the ablation (Table 5): Dense+Dense and Sparse+Sparse
+# --------------------------------------------------------------------------------------------
+PATH_SHARQ, PATH_SPARSE_ONLY, PATH_DENSE_ONLY, PATH_DENSE_DENSE, PATH_SPARSE_SPARSE = 0, 1, 2, 3, 4
+
+
+def mask_pair48_f32(R):
+    """Pairwise 4:8 on an fp32 tensor (the second sparse path of Sparse+Sparse masks the RESIDUAL, which is
+    fp32): score of a pair = max of the two 31-bit magnitude patterns (monotone in |r| for finite values),
+    top 2 of 4 pairs, ties to the lower pair index -- DESIGN.md R4 carried over to fp32 (R17)."""
+    R = np.ascontiguousarray(R, dtype=F32)
+    T, K = R.shape
+    u = (R.view(U32) & U32(0x7FFFFFFF)).reshape(T, K // 8, 4, 2)
+    keep_pair = _top2_of_4(u.max(axis=-1))
+    return np.repeat(keep_pair, 2, axis=-1).reshape(T, K), _nibbles(keep_pair)
+
+
+def _dense_quantize(V, fmt, ts, inv_ts):
+    """One dense FP4 path (Eq. 3): per group of Gd (16 NVFP4 / 32 MXFP4) scale = amax/6 in the scale
+    format, codes = RNE e2m1.  Returns (codes packed [T,K/2], sf [T,K/Gd], dequantised fp32 [T,K])."""
+    T, K = V.shape
+    Gd = 16 if fmt == NVFP4 else 32
+    a = np.abs(V).reshape(T, K // Gd, Gd).max(axis=-1)
+    sf, s_eff, inv = _block_scale(a, fmt, ts, inv_ts)
+    code = e2m1_encode(V * np.repeat(inv, Gd, axis=1))
+    d = (e2m1_decode(code) * np.repeat(s_eff, Gd, axis=1)).astype(F32)
+    return pack_codes(code), sf, d
+
+
+def _sparse_quantize(V, keep, fmt, ts, inv_ts):
+    """One sparse FP4 path (Eq. 7): scale per 32 logical k over the survivors, survivors' codes in
+    ascending k.  Returns (codes packed [T,K/4], sf [T,K/32], dequantised fp32 [T,K], 0 at dropped k)."""
+    T, K = V.shape
+    a = np.where(keep, np.abs(V), F32(0)).reshape(T, K // 32, 32).max(axis=-1)
+    sf, s_eff, inv = _block_scale(a, fmt, ts, inv_ts)
+    with np.errstate(over="ignore"):
+        code = e2m1_encode(V * np.repeat(inv, 32, axis=1))
+    d = np.where(keep, e2m1_decode(code) * np.repeat(s_eff, 32, axis=1), F32(0)).astype(F32)
+    return pack_codes(code[keep].reshape(T, K // 2)), sf, d
+
+
+def prepare_paths(x_u16, path, fmt=NVFP4, norm=NORM_RMS, gamma_u16=None, beta_u16=None, eps=1e-6,
+                  x_tensor_scale=None):
+    """The two-path decompositions of Table 5, each X ~= A0 + A1 with A1 quantised from the residual
+    of A0 exactly as in Eq. 8: R = X - D(Q(.)), one row tensor scale for both paths (R5).
+      PATH_DENSE_DENSE   A0 = dense FP4 of X,                 A1 = dense FP4 of R   ("two dense NVFP4 paths")
+      PATH_SPARSE_SPARSE A0 = SharQ's sparse backbone of X,   A1 = sparse FP4 of R under its own pairwise 4:8
+                         mask M(R) ("two sparse paths"; the part of R outside M(R) is lost)
+    Returns dict(X, ts, a0_codes, a0_sf, a0_meta, a1_codes, a1_sf, a1_meta, A0, A1 (fp32 dequantised, without
+    nothing folded: they include ts), R); metas are None for dense paths."""
+    assert fmt in (NVFP4, MXFP4) and path in (PATH_DENSE_DENSE, PATH_SPARSE_SPARSE)
+    x_u16 = np.asarray(x_u16, dtype=U16)
+    X = normalize(x_u16, norm, gamma_u16, beta_u16, eps)
+    Xf = bf16_to_f32(X)
+    ts, inv_ts = tensor_scale(X, fmt, x_tensor_scale)
+    if path == PATH_DENSE_DENSE:
+        a0_codes, a0_sf, d0 = _dense_quantize(Xf, fmt, ts, inv_ts)
+        R = (Xf - d0).astype(F32)
+        a1_codes, a1_sf, d1 = _dense_quantize(R, fmt, ts, inv_ts)
+        a0_meta = a1_meta = None
+    else:
+        keep0, nib0 = mask_pair48(X)
+        a0_codes, a0_sf, d0 = _sparse_quantize(Xf, keep0, fmt, ts, inv_ts)
+        R = np.where(keep0, Xf - d0, Xf).astype(F32)
+        keep1, nib1 = mask_pair48_f32(R)
+        a1_codes, a1_sf, d1 = _sparse_quantize(R, keep1, fmt, ts, inv_ts)
+        a0_meta, a1_meta = pack_nibbles(nib0), pack_nibbles(nib1)
+    return dict(X=X, ts=ts, R=R, A0=d0, A1=d1, a0_codes=a0_codes, a0_sf=a0_sf, a0_meta=a0_meta,
+                a1_codes=a1_codes, a1_sf=a1_sf, a1_meta=a1_meta, fmt=fmt, path=path)
+
+
+def linear_paths(pp, wq, rows=None, cols=None):
+    """Eq. 9 for a Table 5 combination, fp64, rebuilt from the STORED operands only: both dense paths go
+    through the weight's dense scale view, both sparse paths through the sparse view (same values, R7)."""
+    fmt, path = pp["fmt"], pp["path"]
+    ops = []
+    for i in (0, 1):
+        if path == PATH_DENSE_DENSE:
+            view = dict(dn_codes=pp[f"a{i}_codes"], dn_sf=pp[f"a{i}_sf"], ts=pp["ts"], fmt=fmt,
+                        Gd=16 if fmt == NVFP4 else 32)
+            ops.append(dequant_residual(view, with_ts=False))
+        else:
+            view = dict(sp_codes=pp[f"a{i}_codes"], sp_sf=pp[f"a{i}_sf"], sp_meta=pp[f"a{i}_meta"], ts=pp["ts"],
+                        fmt=fmt, mask=MASK_PAIR48, Gs=32)
+            ops.append(dequant_backbone(view, with_ts=False))
+    W = dequant_weight(wq, "dense" if path == PATH_DENSE_DENSE else "sparse", with_ts=False)
+    ts = pp["ts"].astype(np.float64)
+    A0, A1 = ops
+    if rows is not None:
+        A0, A1, ts = A0[rows], A1[rows], ts[rows]
+    if cols is not None:
+        W = W[cols]
+    return (A0 @ W.T + A1 @ W.T) * ts[:, None] * np.float64(wq["ts_w"])
+
+
+# --------------------------------------------------------------------------------------------
 # sharq_quantize_weight (P:130 Fig. 2 caption, P:157; DESIGN.md R7)
 # --------------------------------------------------------------------------------------------
 def quantize_weight(w_u16, fmt=NVFP4):

@@ -400,3 +400,67 @@ def test_hif4_residual_is_x_minus_decoded_backbone():
     exact = p["R"].astype(np.float64) + d == Xf
     assert exact.mean() > 0.999                                    # fp32 subtraction of nearby values: Sterbenz
     assert np.abs(p["R"].astype(np.float64) + d - Xf).max() <= np.abs(Xf).max() * 2.0 ** -24
+
+
+# ------------------------------------------------------------------ Table 5 path combinations
+@pytest.mark.parametrize("fmt", [so.NVFP4, so.MXFP4])
+def test_dense_dense_paths(fmt):
+    """Dense+Dense: the first path is a plain dense quantiser of X -- byte for byte the 'dense-only special case' of
+    prepare() (itself pinned against ml_dtypes) -- and the second path is the same quantiser applied to the exact
+    residual; the two-path error is far below the one-path error (6.63 vs the NVFP4 baseline's 6.95)."""
+    x = si.activations(8, 1024, config=1); g = si.gamma(1024)
+    pp = so.prepare_paths(x, so.PATH_DENSE_DENSE, fmt=fmt, gamma_u16=g)
+    p0 = so.prepare(x, fmt=fmt, gamma_u16=g, _force_no_survivors=True)
+    assert np.array_equal(pp["a0_codes"], p0["dn_codes"]) and np.array_equal(pp["a0_sf"], p0["dn_sf"])
+    Xf = so.bf16_to_f32(pp["X"]).astype(np.float64)
+    assert np.array_equal(pp["R"].astype(np.float64) + pp["A0"].astype(np.float64), Xf)          # Eq. 8, exact
+    # second path = the dense quantiser on R: re-run it through prepare()'s own dense branch on a bf16-free route
+    Gd = 16 if fmt == so.NVFP4 else 32
+    ts = pp["ts"]; inv_ts = (F32(1) / ts).astype(F32)
+    a = np.abs(pp["R"]).reshape(8, -1, Gd).max(-1)
+    sf, s_eff, inv = so._block_scale(a, fmt, ts, inv_ts)
+    assert np.array_equal(sf, pp["a1_sf"])
+    assert (so.sf_decode(pp["a1_sf"], fmt).astype(np.float64) * ts[:, None] * 6 >= a * (1 - 2.0 ** -4)).all()
+    n = np.linalg.norm
+    e1 = n(pp["A0"].astype(np.float64) - Xf) / n(Xf)
+    e2 = n(pp["A0"].astype(np.float64) + pp["A1"].astype(np.float64) - Xf) / n(Xf)
+    assert e2 < e1 / 4
+
+
+@pytest.mark.parametrize("fmt", [so.NVFP4, so.MXFP4])
+def test_sparse_sparse_paths_and_table5_ordering(fmt):
+    """Sparse+Sparse: first path == SharQ's backbone bit for bit; the second mask is an exact top-2-of-4 on |R|
+    (brute force), its survivors are exactly N of M; and the reconstruction errors order as Table 5 does:
+    Sparse >> Sparse+Sparse > SharQ, Dense+Dense ~ SharQ (P:265, P:288)."""
+    x = si.activations(16, 2048, config=1); g = si.gamma(2048)
+    ps = so.prepare_paths(x, so.PATH_SPARSE_SPARSE, fmt=fmt, gamma_u16=g)
+    p = so.prepare(x, fmt=fmt, gamma_u16=g)
+    for k0, k1 in (("a0_codes", "sp_codes"), ("a0_sf", "sp_sf"), ("a0_meta", "sp_meta")):
+        assert np.array_equal(ps[k0], p[k1])
+    assert np.array_equal(ps["R"], p["R"])
+    keep1, nib1 = so.mask_pair48_f32(ps["R"])
+    assert (keep1.reshape(16, -1, 8).sum(-1) == 4).all()
+    score = np.abs(ps["R"]).reshape(16, -1, 4, 2).max(-1)
+    for t in range(2):
+        for c in range(score.shape[1]):
+            best = _best_mask_bruteforce(score[t, c].tolist())
+            assert nib1[t, c] == best[0] | (best[1] << 2)
+    assert (ps["A1"][~keep1] == 0).all()
+    # stored operands decode to A0 / A1 (linear_paths sees what the kernels see)
+    w = si.weight(64, 2048); wq = so.quantize_weight(w, fmt)
+    Wd = so.dequant_weight(wq)
+    Y = so.linear_paths(ps, wq)
+    # (A0 / A1 carry s_eff = RN(sf * ts) in fp32, the stored operands the exact product: 2^-24 relative per term)
+    assert np.allclose(Y, (ps["A0"].astype(np.float64) + ps["A1"].astype(np.float64)) @ Wd.T, rtol=1e-6,
+                       atol=1e-6 * np.abs(Y).max())
+    Xf = so.bf16_to_f32(p["X"]).astype(np.float64)
+    n = np.linalg.norm
+    e_sparse = n(p["Xsp_tilde"].astype(np.float64) - Xf) / n(Xf)
+    e_ss = n(ps["A0"].astype(np.float64) + ps["A1"].astype(np.float64) - Xf) / n(Xf)
+    e_sharq = n(so.dequant_backbone(p) + so.dequant_residual(p) - Xf) / n(Xf)
+    pd = so.prepare_paths(x, so.PATH_DENSE_DENSE, fmt=fmt, gamma_u16=g)
+    e_dd = n(pd["A0"].astype(np.float64) + pd["A1"].astype(np.float64) - Xf) / n(Xf)
+    assert e_sparse > 3 * e_ss > 3 * e_sharq and e_dd < 1.5 * e_sharq
+    Yd = so.linear_paths(pd, wq)
+    assert np.allclose(Yd, (pd["A0"].astype(np.float64) + pd["A1"].astype(np.float64)) @ Wd.T, rtol=1e-6,
+                       atol=1e-6 * np.abs(Yd).max())
