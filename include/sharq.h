@@ -8,7 +8,8 @@
  *   sharq_linear           sparse + dense block-scaled FP4 GEMMs into one accumulator, bf16 epilogue
  * plus sharq_linear_grouped (the same over the row ranges of E experts, MoE), sharq_prepare_add
  * (sharq_prepare with the residual-stream add fused in front of the norm), host-only size / plan queries
- * (sharq_weight_sizes, sharq_act_sizes, sharq_linear_workspace, sharq_linear_plan), sharq_act_init and the test
+ * (sharq_weight_sizes, sharq_act_sizes, sharq_linear_workspace, sharq_linear_plan), sharq_act_init, the Table 5
+ * path combinations (sharq_act_sizes_paths, sharq_prepare_paths, sharq_linear_paths) and the test
  * helpers sharq_untile_sf / sharq_untile_meta.  The tensor-pipe probe lives in sharq_diag.h.
  *
  * Conventions
@@ -185,6 +186,30 @@ sharq_status sharq_linear_grouped(const sharq_config* cfg, int32_t E, const int3
                                   const void* w_sf_sparse_view, const void* w_sf_dense_view,
                                   const float* w_tensor_scale, void* Y, int64_t ldy, int32_t out_dtype,
                                   void* workspace, size_t workspace_bytes, void* stream);
+
+/* ---- Table 5 path combinations ----------------------------------
+ * The paper's ablation replaces SharQ's sparse + dense pair by two paths of ONE kind, the second quantised from
+ * the residual of the first exactly as in Eq. 8, one row tensor scale for both:
+ *   path 3  Dense + Dense    a0 = dense FP4 of X, a1 = dense FP4 of R = X - D(a0)
+ *   path 4  Sparse + Sparse  a0 = SharQ's sparse backbone, a1 = sparse FP4 of R under its own pairwise 4:8 mask
+ *                            (score on the fp32 magnitudes of R, same tie rule)
+ * (paths 0 / 1 / 2 -- SharQ, sparse only, dense only -- are sharq_prepare + sharq_linear's `path`.)
+ * NVFP4 / MXFP4, pairwise mask.  Operand shapes, per operand: dense: codes [T, K/2], sf [T, K/16] (MXFP4 K/32),
+ * meta unused (NULL); sparse: codes [T, K/4], sf [T, K/32], meta [T, K/16].  sf / meta follow cfg->layout;
+ * sharq_linear_paths needs TILED.  Both operands accumulate into the same TMEM tile (two K-loops of one kernel
+ * launch, W streamed twice: an ablation, not a tuned path). */
+sharq_status sharq_act_sizes_paths(const sharq_config* cfg, int32_t path, int64_t T, int64_t K, size_t* a_codes,
+                                   size_t* a_sf, size_t* a_meta, size_t* row_scale);
+sharq_status sharq_prepare_paths(const sharq_config* cfg, int32_t path, const void* x, int64_t T, int64_t K,
+                                 int64_t ldx, const void* gamma, const void* beta, const float* x_tensor_scale,
+                                 void* a0_codes, void* a0_sf, void* a0_meta, void* a1_codes, void* a1_sf,
+                                 void* a1_meta, float* row_scale, void* stream);
+sharq_status sharq_linear_paths(const sharq_config* cfg, int32_t path, int64_t T, int64_t D, int64_t K,
+                                const void* a0_codes, const void* a0_sf, const void* a0_meta,
+                                const void* a1_codes, const void* a1_sf, const void* a1_meta,
+                                const float* row_scale, const void* w_codes, const void* w_sf_sparse_view,
+                                const void* w_sf_dense_view, const float* w_tensor_scale, const void* bias,
+                                void* Y, int64_t ldy, int32_t out_dtype, void* stream);
 
 /* ---- sharq_act_init: one-time initialisation of TILED activation scale / metadata buffers ----------
  * Fills sp_sf and dn_sf with zero scales and sp_meta with the valid nibble 0x4 (pairs 0 and 1) for all

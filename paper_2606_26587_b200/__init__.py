@@ -20,7 +20,7 @@ NVFP4, MXFP4, HIF4 = 0, 1, 2
 MASK_PAIR48, MASK_24 = 0, 1
 NORM_NONE, NORM_RMS, NORM_LAYER = 0, 1, 2
 LAYOUT_CANONICAL, LAYOUT_TILED = 0, 1
-PATH_SHARQ, PATH_SPARSE_ONLY, PATH_DENSE_ONLY = 0, 1, 2
+PATH_SHARQ, PATH_SPARSE_ONLY, PATH_DENSE_ONLY, PATH_DENSE_DENSE, PATH_SPARSE_SPARSE = 0, 1, 2, 3, 4
 _STATUS = {0: "SHARQ_OK", 1: "SHARQ_EINVAL", 2: "SHARQ_ESHAPE", 3: "SHARQ_EWORKSPACE", 4: "SHARQ_EARCH",
            5: "SHARQ_ECUDA"}
 
@@ -63,6 +63,10 @@ def _load() -> ctypes.CDLL:
     lib.sharq_linear_grouped.argtypes = [CFG, c_int32, P, c_int64, c_int64, c_int64, P, P, P, P, P, P, P, P,
                                          P, P, P, c_int64, c_int32, P, c_size_t, P]
     lib.sharq_act_init.argtypes = [CFG, c_int64, c_int64, P, P, P, P]
+    lib.sharq_act_sizes_paths.argtypes = [CFG, c_int32, c_int64, c_int64, SZ, SZ, SZ, SZ]
+    lib.sharq_prepare_paths.argtypes = [CFG, c_int32, P, c_int64, c_int64, c_int64, P, P, P, P, P, P, P, P, P, P, P]
+    lib.sharq_linear_paths.argtypes = [CFG, c_int32, c_int64, c_int64, c_int64, P, P, P, P, P, P, P, P, P, P, P, P, P,
+                                       c_int64, c_int32, P]
     lib.sharq_linear_plan.argtypes = [CFG, c_int64, c_int64, c_int64, c_int32, ctypes.c_char_p, c_size_t]
     lib.sharq_untile_sf.argtypes = [P, c_int64, c_int64, P, P]
     lib.sharq_untile_meta.argtypes = [P, c_int64, c_int64, P, P]
@@ -75,7 +79,8 @@ def _load() -> ctypes.CDLL:
 # every symbol include/sharq.h declares, then include/sharq_diag.h's
 EXPORTS = ("sharq_version", "sharq_weight_sizes", "sharq_act_sizes", "sharq_linear_workspace",
            "sharq_quantize_weight", "sharq_prepare", "sharq_prepare_add", "sharq_linear", "sharq_linear_grouped",
-           "sharq_act_init", "sharq_linear_plan", "sharq_untile_sf", "sharq_untile_meta", "sharq_mma_peak_launch")
+           "sharq_act_init", "sharq_linear_plan", "sharq_untile_sf", "sharq_untile_meta", "sharq_act_sizes_paths",
+           "sharq_prepare_paths", "sharq_linear_paths", "sharq_mma_peak_launch")
 capi = _load()
 
 
@@ -203,6 +208,40 @@ def prepare_add(cfg: Config, x, residual, gamma=None, beta=None, x_tensor_scale=
                                   _ptr(out["sp_codes"]), _ptr(out["sp_sf"]), _ptr(out["sp_meta"]), _ptr(out["dn_codes"]),
                                   _ptr(out["dn_sf"]), _ptr(out["row_scale"]), _stream()), "sharq_prepare_add")
     return out, sum_out
+
+
+def prepare_paths(cfg: Config, path: int, x, gamma=None, beta=None, x_tensor_scale=None):
+    """Table 5 combination (PATH_DENSE_DENSE / PATH_SPARSE_SPARSE): returns dict(a0_codes, a0_sf, a0_meta, a1_*,
+    row_scale, T, K, path)."""
+    import torch
+    T, K = x.shape
+    s = [c_size_t() for _ in range(4)]
+    _check(capi.sharq_act_sizes_paths(ctypes.byref(cfg), path, T, K, *[ctypes.byref(v) for v in s]), "sharq_act_sizes_paths")
+    n_codes, n_sf, n_meta, _ = (v.value for v in s)
+    dev = x.device
+    out = dict(T=T, K=K, path=path, row_scale=torch.empty(max(T, 1), dtype=torch.float32, device=dev))
+    for i in (0, 1):
+        out[f"a{i}_codes"] = _bytes(n_codes, dev)
+        out[f"a{i}_sf"] = torch.zeros(max(n_sf, 16), dtype=torch.uint8, device=dev)            # pad rows: zero scales
+        out[f"a{i}_meta"] = torch.full((max(n_meta, 16),), 0x44, dtype=torch.uint8, device=dev) if n_meta else None
+    _check(capi.sharq_prepare_paths(ctypes.byref(cfg), path, _ptr(x), T, K, x.stride(0), _ptr(gamma), _ptr(beta),
+                                    _ptr(x_tensor_scale), _ptr(out["a0_codes"]), _ptr(out["a0_sf"]), _ptr(out["a0_meta"]),
+                                    _ptr(out["a1_codes"]), _ptr(out["a1_sf"]), _ptr(out["a1_meta"]), _ptr(out["row_scale"]),
+                                    _stream()), "sharq_prepare_paths")
+    return out
+
+
+def linear_paths(cfg: Config, act: dict, wq: dict, bias=None, out_dtype="bf16", Y=None):
+    import torch
+    T, K, D = act["T"], act["K"], wq["D"]
+    if Y is None:
+        Y = torch.empty((T, D), dtype=torch.bfloat16 if out_dtype == "bf16" else torch.float32, device=act["a0_codes"].device)
+    _check(capi.sharq_linear_paths(ctypes.byref(cfg), act["path"], T, D, K, _ptr(act["a0_codes"]), _ptr(act["a0_sf"]),
+                                   _ptr(act["a0_meta"]), _ptr(act["a1_codes"]), _ptr(act["a1_sf"]), _ptr(act["a1_meta"]),
+                                   _ptr(act["row_scale"]), _ptr(wq["codes"]), _ptr(wq["sf_sp"]), _ptr(wq["sf_dn"]),
+                                   _ptr(wq["ts_w"]), _ptr(bias), _ptr(Y), Y.stride(0), 0 if Y.dtype == torch.bfloat16 else 1,
+                                   _stream()), "sharq_linear_paths")
+    return Y
 
 
 def act_slot(cfg: Config, act: dict, row0: int, T: int) -> dict:

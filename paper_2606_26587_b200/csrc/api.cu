@@ -10,7 +10,8 @@ namespace sharq {
 cudaError_t launch_prepare(const sharq_config* cfg, const void* x, int64_t T, int64_t K, int64_t ldx,
                            const void* gamma, const void* beta, const float* x_ts, void* sp_codes, void* sp_sf,
                            void* sp_meta, void* dn_codes, void* dn_sf, float* row_scale, int num_sms,
-                           cudaStream_t st, const void* residual, int64_t ldr, void* sum_out, int64_t ldo);
+                           cudaStream_t st, const void* residual, int64_t ldr, void* sum_out, int64_t ldo,
+                           int combo, void* dn_meta);
 cudaError_t launch_quantize_weight(const sharq_config* cfg, const void* W, int64_t D, int64_t K, int64_t ldw,
                                    void* codes, void* sf_sp, void* sf_dn, float* ts, void* workspace,
                                    cudaStream_t st);
@@ -137,7 +138,7 @@ sharq_status sharq_prepare(const sharq_config* cfg, const void* x, int64_t T, in
   DeviceInfo di{};
   if ((s = device_info(&di)) != SHARQ_OK) return s;
   cudaError_t e = launch_prepare(cfg, x, T, K, ldx, gamma, beta, x_tensor_scale, sp_codes, sp_sf, sp_meta, dn_codes,
-                                 dn_sf, row_scale, di.sms, (cudaStream_t)stream, nullptr, 0, nullptr, 0);
+                                 dn_sf, row_scale, di.sms, (cudaStream_t)stream, nullptr, 0, nullptr, 0, 0, nullptr);
   return e == cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
 }
 
@@ -162,7 +163,7 @@ sharq_status sharq_prepare_add(const sharq_config* cfg, const void* x, const voi
   DeviceInfo di{};
   if ((s = device_info(&di)) != SHARQ_OK) return s;
   cudaError_t e = launch_prepare(cfg, x, T, K, ldx, gamma, beta, x_tensor_scale, sp_codes, sp_sf, sp_meta, dn_codes,
-                                 dn_sf, row_scale, di.sms, (cudaStream_t)stream, residual, ldr, sum_out, ldo);
+                                 dn_sf, row_scale, di.sms, (cudaStream_t)stream, residual, ldr, sum_out, ldo, 0, nullptr);
   return e == cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
 }
 
@@ -173,7 +174,7 @@ static sharq_status check_linear(const sharq_config* cfg, int64_t D, int64_t K, 
   if (cfg->fmt != SHARQ_HIF4 && cfg->mask != SHARQ_MASK_PAIR48) return SHARQ_ESHAPE;   // no element-wise 2:4 FP4 MMA
   if (cfg->layout != SHARQ_LAYOUT_TILED && cfg->fmt != SHARQ_HIF4) return SHARQ_EINVAL;
   if (D <= 0 || D % 128 != 0 || K <= 0 || K % 256 != 0 || ldy < D || ldy % 8 != 0) return SHARQ_ESHAPE;
-  if (out_dtype < 0 || out_dtype > 1 || path < 0 || path > 2) return SHARQ_EINVAL;
+  if (out_dtype < 0 || out_dtype > 1 || path < 0 || path > 4) return SHARQ_EINVAL;
   for (int i = 0; i < n; ++i)
     if (!ptrs[i] || !aligned16(ptrs[i])) return SHARQ_EINVAL;
   return SHARQ_OK;
@@ -194,9 +195,72 @@ sharq_status sharq_linear(const sharq_config* cfg, int64_t T, int64_t D, int64_t
   if (workspace_bytes < linear_workspace_bytes(cfg, T, D, K, 0)) return SHARQ_EWORKSPACE;
   DeviceInfo di{};
   if ((s = device_info(&di)) != SHARQ_OK) return s;
-  LinearArgs a{T, D, K, sp_codes, sp_sf, sp_meta, dn_codes, dn_sf, row_scale, w_codes, w_sf_sparse_view,
+  if (path > 2) return SHARQ_EINVAL;                       // the two-operand combinations go through sharq_linear_paths
+  LinearArgs a{T, D, K, sp_codes, sp_sf, sp_meta, dn_codes, dn_sf, nullptr, row_scale, w_codes, w_sf_sparse_view,
                w_sf_dense_view, w_tensor_scale, bias, Y, ldy, out_dtype, path};
   return launch_linear(cfg, a, 0, nullptr, workspace, workspace_bytes, di.sms, di.dev, (cudaStream_t)stream, nullptr);
+}
+
+// ---- Table 5 path combinations --------------------------------------------------------------
+static bool combo_ok(const sharq_config* cfg, int32_t path) {
+  return (path == 3 || path == 4) && cfg->fmt != SHARQ_HIF4 && cfg->mask == SHARQ_MASK_PAIR48;
+}
+
+sharq_status sharq_act_sizes_paths(const sharq_config* cfg, int32_t path, int64_t T, int64_t K, size_t* a_codes,
+                                   size_t* a_sf, size_t* a_meta, size_t* row_scale) {
+  sharq_status s = check_cfg(cfg);
+  if (s != SHARQ_OK) return s;
+  if (!combo_ok(cfg, path)) return SHARQ_EINVAL;
+  if (T < 0 || K <= 0 || K % 256 != 0) return SHARQ_ESHAPE;
+  const bool dense = path == 3;
+  if (a_codes) *a_codes = (size_t)T * (size_t)(dense ? K / 2 : K / 4);
+  if (a_sf) *a_sf = sf_bytes(cfg, T, dense ? sf_cols(cfg->fmt, true, K) : K / 32);
+  if (a_meta) *a_meta = dense ? 0 : sf_bytes(cfg, T, K / 16);
+  if (row_scale) *row_scale = (size_t)T * sizeof(float);
+  return SHARQ_OK;
+}
+
+sharq_status sharq_prepare_paths(const sharq_config* cfg, int32_t path, const void* x, int64_t T, int64_t K, int64_t ldx,
+                                 const void* gamma, const void* beta, const float* x_tensor_scale, void* a0_codes,
+                                 void* a0_sf, void* a0_meta, void* a1_codes, void* a1_sf, void* a1_meta,
+                                 float* row_scale, void* stream) {
+  sharq_status s = check_cfg(cfg);
+  if (s != SHARQ_OK) return s;
+  if (!combo_ok(cfg, path)) return SHARQ_EINVAL;
+  if (T < 0 || K <= 0 || K % 256 != 0 || ldx < K || ldx % 8 != 0 || K > 100 * 1024) return SHARQ_ESHAPE;
+  if (T == 0) return SHARQ_OK;
+  if (!x || !a0_codes || !a0_sf || !a1_codes || !a1_sf || !row_scale) return SHARQ_EINVAL;
+  if (path == 4 && (!a0_meta || !a1_meta)) return SHARQ_EINVAL;
+  if (cfg->norm != SHARQ_NORM_NONE && !gamma) return SHARQ_EINVAL;
+  if (!aligned16(x) || !aligned16(a0_codes) || !aligned16(a0_sf) || !aligned16(a1_codes) || !aligned16(a1_sf) ||
+      (a0_meta && !aligned16(a0_meta)) || (a1_meta && !aligned16(a1_meta)) || (gamma && !aligned16(gamma)) ||
+      (beta && !aligned16(beta)))
+    return SHARQ_EINVAL;
+  DeviceInfo di{};
+  if ((s = device_info(&di)) != SHARQ_OK) return s;
+  cudaError_t e = launch_prepare(cfg, x, T, K, ldx, gamma, beta, x_tensor_scale, a0_codes, a0_sf, a0_meta, a1_codes,
+                                 a1_sf, row_scale, di.sms, (cudaStream_t)stream, nullptr, 0, nullptr, 0, path, a1_meta);
+  return e == cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
+}
+
+sharq_status sharq_linear_paths(const sharq_config* cfg, int32_t path, int64_t T, int64_t D, int64_t K,
+                                const void* a0_codes, const void* a0_sf, const void* a0_meta, const void* a1_codes,
+                                const void* a1_sf, const void* a1_meta, const float* row_scale, const void* w_codes,
+                                const void* w_sf_sparse_view, const void* w_sf_dense_view, const float* w_tensor_scale,
+                                const void* bias, void* Y, int64_t ldy, int32_t out_dtype, void* stream) {
+  if (!cfg || !combo_ok(cfg, path)) return SHARQ_EINVAL;
+  const void* ptrs[] = {a0_codes, a0_sf, a1_codes, a1_sf, w_codes, w_sf_sparse_view, w_sf_dense_view, Y};
+  sharq_status s = check_linear(cfg, D, K, ptrs, T == 0 ? 0 : 8, ldy, out_dtype, path);
+  if (s != SHARQ_OK) return s;
+  if (T < 0 || T >= (int64_t)1 << 30) return SHARQ_ESHAPE;
+  if (T == 0) return SHARQ_OK;
+  if (!row_scale || !w_tensor_scale) return SHARQ_EINVAL;
+  if (path == 4 && (!a0_meta || !a1_meta || !aligned16(a0_meta) || !aligned16(a1_meta))) return SHARQ_EINVAL;
+  DeviceInfo di{};
+  if ((s = device_info(&di)) != SHARQ_OK) return s;
+  LinearArgs a{T, D, K, a0_codes, a0_sf, a0_meta, a1_codes, a1_sf, a1_meta, row_scale, w_codes, w_sf_sparse_view,
+               w_sf_dense_view, w_tensor_scale, bias, Y, ldy, out_dtype, path};
+  return launch_linear(cfg, a, 0, nullptr, nullptr, 0, di.sms, di.dev, (cudaStream_t)stream, nullptr);
 }
 
 sharq_status sharq_linear_grouped(const sharq_config* cfg, int32_t E, const int32_t* offsets, int64_t padded_rows,
@@ -216,8 +280,8 @@ sharq_status sharq_linear_grouped(const sharq_config* cfg, int32_t E, const int3
   if (padded_rows == 0) return SHARQ_OK;
   DeviceInfo di{};
   if ((s = device_info(&di)) != SHARQ_OK) return s;
-  LinearArgs a{padded_rows, D, K, sp_codes, sp_sf, sp_meta, dn_codes, dn_sf, row_scale, w_codes, w_sf_sparse_view,
-               w_sf_dense_view, w_tensor_scale, nullptr, Y, ldy, out_dtype, 0};
+  LinearArgs a{padded_rows, D, K, sp_codes, sp_sf, sp_meta, dn_codes, dn_sf, nullptr, row_scale, w_codes,
+               w_sf_sparse_view, w_sf_dense_view, w_tensor_scale, nullptr, Y, ldy, out_dtype, 0};
   return launch_linear(cfg, a, E, offsets, workspace, workspace_bytes, di.sms, di.dev, (cudaStream_t)stream, nullptr);
 }
 
@@ -232,7 +296,7 @@ sharq_status sharq_linear_plan(const sharq_config* cfg, int64_t T, int64_t D, in
   LinearPlan pl{};
   pl.kind = -1;
   LinearArgs a{T, D, K, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr,
-               nullptr, nullptr, D, 0, 0};
+               nullptr, nullptr, nullptr, D, 0, 0};
   if (T > 0) {
     s = launch_linear(cfg, a, E, nullptr, nullptr, 0, di.sms, di.dev, nullptr, &pl);
     if (s != SHARQ_OK) return s;

@@ -61,6 +61,10 @@ struct KParams {
                                    // both are replaced inside the kernel by the values the expert table gives
   const int32_t* offsets;          // grouped: device int32[E + 1] (nullptr otherwise)
   int32_t E;
+  // Table 5 combinations (path 3 = dense + dense, 4 = sparse + sparse): the tile runs the K-loop twice
+  // into the same accumulator, the second time on the SECOND operand of the same kind (tensor map tm_alt, scale
+  // factors sf2, metadata meta2); W is streamed twice
+  const uint8_t *sf2, *meta2;
   int32_t a_rows;     // rows of the activation TMA boxes: 128, or roundup(T, 8) when T < 128 (out-of-bounds
                       // rows are zero-filled slowly; rows beyond the box keep stale smem, which only feeds
                       // accumulator rows that are never stored)
@@ -134,7 +138,7 @@ __device__ __forceinline__ Unit decode_unit(const KParams& p, const GroupTab& g,
   } else {
     u.rows_valid = min(BM, p.T - u.m_blk * BM);
   }
-  const int num_kb = p.K / BK;
+  const int num_kb = (p.K / BK) * (p.path >= 3 ? 2 : 1);   // combinations: second pass = k-blocks num_kb .. 2 num_kb - 1
   u.kb0 = (int)((int64_t)rank * num_kb / splits);
   u.kb1 = (int)((int64_t)(rank + 1) * num_kb / splits);
   return u;
@@ -169,7 +173,8 @@ __device__ __forceinline__ void store_row(const KParams& p, int64_t row, int col
 template <int BN, int FMT, bool SPLIT, int AR, bool MC = false>
 __global__ void __launch_bounds__(kThreads, 1)
 sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_constant__ CUtensorMap tm_a_dn,
-                    const __grid_constant__ CUtensorMap tm_w, const KParams p) {
+                    const __grid_constant__ CUtensorMap tm_w, const __grid_constant__ CUtensorMap tm_alt,
+                    const KParams p) {
   using S = Stage<BN, FMT, SPLIT, AR>;
   constexpr bool NV = (FMT == SHARQ_NVFP4);
   extern __shared__ uint8_t smem_raw[];
@@ -185,7 +190,7 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   if (warp == 0) SHARQ_TS(0);
-  const bool do_sp = p.path != 2, do_dn = p.path != 1;
+  const bool do_sp = p.path == 0 || p.path == 1 || p.path == 4, do_dn = p.path == 0 || p.path == 2 || p.path == 3;
   // work distribution: SPLIT -> one tile per cluster, this CTA's k-slice; else persistent round-robin
   static_assert(!(SPLIT && MC), "split-K clusters and multicast clusters are separate variants");
   const int crank = (SPLIT || MC) ? (int)tc::cluster_ctarank() : 0;
@@ -287,7 +292,9 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
         const uint8_t* sfa_dn = p.dn_sf + (size_t)u.m_blk * (Kc / 256) * (S::SF_DN_BYTES);
         const uint8_t* meta = p.sp_meta + (size_t)u.m_blk * (Kc / 256) * 2048;
         // weight side of k-block kb (codes + both scale views): independent of the preceding kernel
-        auto load_w = [&](int kb, uint32_t st, uint32_t fb) {
+        const int nkb = (int)(Kc / BK);
+        auto load_w = [&](int kbv, uint32_t st, uint32_t fb) {
+          const int kb = kbv >= nkb ? kbv - nkb : kbv;   // second pass of a combination: the same W k-blocks again
           if (lead) tc::tma_load_2d(st + S::W, &tm_w, fb, kb * 128, w_row0, pol_w);
           for (int nb = 0; nb < S::NB; ++nb) {
             if (do_sp && lead)
@@ -300,7 +307,9 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
           }
         };
         // activation side: written by sharq_prepare, only after griddepcontrol.wait
-        auto load_a = [&](int kb, uint32_t st, uint32_t fb) {
+        auto load_a = [&](int kbv, uint32_t st, uint32_t fb) {
+          const bool alt = kbv >= nkb;                   // combinations: the second operand
+          const int kb = alt ? kbv - nkb : kbv;
           if constexpr (MC) {
             // same 128-row block in both CTAs: CTA 0 fetches the dense side, CTA 1 the sparse side, for both
             if (do_sp && crank == 1) {
@@ -315,13 +324,16 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
             return;
           }
           if (do_sp) {
-            if (lead) tc::tma_load_2d(st + S::A_SP, &tm_a_sp, fb, kb * 64, u.m_blk * BM, pol_act);
-            if (lead) tc::bulk_load(st + S::META, meta + (size_t)kb * 2048, 2048, fb, pol_act);
-            if (lead) tc::bulk_load(st + S::SFA_SP, sfa_sp + (size_t)kb * 1024, 1024, fb, pol_act);
+            const size_t mo = (size_t)u.m_blk * (Kc / 256) * 2048 + (size_t)kb * 2048;
+            const size_t so = (size_t)u.m_blk * (Kc / 128) * 512 + (size_t)kb * 1024;
+            if (lead) tc::tma_load_2d(st + S::A_SP, alt ? &tm_alt : &tm_a_sp, fb, kb * 64, u.m_blk * BM, pol_act);
+            if (lead) tc::bulk_load(st + S::META, (alt ? p.meta2 : p.sp_meta) + mo, 2048, fb, pol_act);
+            if (lead) tc::bulk_load(st + S::SFA_SP, (alt ? p.sf2 : p.sp_sf) + so, 1024, fb, pol_act);
           }
           if (do_dn) {
-            if (lead) tc::tma_load_2d(st + S::A_DN, &tm_a_dn, fb, kb * 128, u.m_blk * BM, pol_act);
-            if (lead) tc::bulk_load(st + S::SFA_DN, sfa_dn + (size_t)kb * S::SF_DN_BYTES, S::SF_DN_BYTES, fb, pol_act);
+            const size_t so = ((size_t)u.m_blk * (Kc / 256) + (size_t)kb) * S::SF_DN_BYTES;
+            if (lead) tc::tma_load_2d(st + S::A_DN, alt ? &tm_alt : &tm_a_dn, fb, kb * 128, u.m_blk * BM, pol_act);
+            if (lead) tc::bulk_load(st + S::SFA_DN, (alt ? p.sf2 : p.dn_sf) + so, S::SF_DN_BYTES, fb, pol_act);
           }
         };
         int kb = u.kb0;
@@ -878,10 +890,11 @@ inline void fill_plan(LinearPlan* pl, int kind, int bn, int ar, int splits, int 
 
 template <int BN, int FMT, int AR>
 sharq_status launch_1cta(const LinearArgs& a, const KParams& p, const CUtensorMap& tm_sp,
-                         const CUtensorMap& tm_dn, const CUtensorMap& tm_w, int64_t tiles, const LaunchEnv& env) {
+                         const CUtensorMap& tm_dn, const CUtensorMap& tm_w, const CUtensorMap& tm_alt, int64_t tiles,
+                         const LaunchEnv& env) {
   constexpr bool kSplitFits = !(BN == 256 && AR == 128);   // no room for the exchange buffers; never needed there
   int splits = 1;
-  if constexpr (kSplitFits) if (p.E == 0) splits = choose_splits<BN, FMT, AR>(tiles, (int)(a.K / BK), env.num_sms, env.dev);
+  if constexpr (kSplitFits) if (p.E == 0 && p.path < 3) splits = choose_splits<BN, FMT, AR>(tiles, (int)(a.K / BK), env.num_sms, env.dev);
   cudaLaunchConfig_t lc{};
   cudaLaunchAttribute attr[2];
   attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
@@ -903,7 +916,7 @@ sharq_status launch_1cta(const LinearArgs& a, const KParams& p, const CUtensorMa
     attr[1].val.clusterDim.y = 1;
     attr[1].val.clusterDim.z = 1;
     lc.numAttrs = 2;
-    return cudaLaunchKernelEx(&lc, kfn, tm_sp, tm_dn, tm_w, p) == cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
+    return cudaLaunchKernelEx(&lc, kfn, tm_sp, tm_dn, tm_w, tm_alt, p) == cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
   }
   using S = Stage<BN, FMT, false, AR>;
   auto kfn = sharq_linear_kernel<BN, FMT, false, AR>;
@@ -914,7 +927,7 @@ sharq_status launch_1cta(const LinearArgs& a, const KParams& p, const CUtensorMa
   if (set_smem_once(smem_set, (const void*)kfn, S::SMEM, env.dev) != cudaSuccess) return SHARQ_ECUDA;
   lc.gridDim = dim3((unsigned)grid);
   lc.dynamicSmemBytes = S::SMEM;
-  return cudaLaunchKernelEx(&lc, kfn, tm_sp, tm_dn, tm_w, p) == cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
+  return cudaLaunchKernelEx(&lc, kfn, tm_sp, tm_dn, tm_w, tm_alt, p) == cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
 }
 
 // grouped GEMM: persistent clusters of two CTAs on neighbouring n-tiles, activation operands multicast
@@ -941,7 +954,7 @@ sharq_status launch_mc(const KParams& p, const CUtensorMap& tm_sp, const CUtenso
   lc.gridDim = dim3((unsigned)(2 * clusters));
   lc.dynamicSmemBytes = S::SMEM;
   lc.stream = env.st;
-  return cudaLaunchKernelEx(&lc, kfn, tm_sp, tm_dn, tm_w, p) == cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
+  return cudaLaunchKernelEx(&lc, kfn, tm_sp, tm_dn, tm_w, tm_sp, p) == cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
 }
 
 // scale-factor / metadata array as a 2-D tensor of 1024-byte rows (256 x u32), boxes of `box_rows` rows
@@ -1003,22 +1016,29 @@ template <int BN, int FMT>
 sharq_status launch_tiles(const LinearArgs& a, int64_t rows_total, int64_t m_blocks, int E, const int32_t* offsets,
                           const LaunchEnv& env) {
   const int num_sms = env.num_sms;
-  CUtensorMap tm_sp, tm_dn, tm_w;
+  CUtensorMap tm_sp, tm_dn, tm_w, tm_alt;
   const int64_t w_rows = (int64_t)(E > 0 ? E : 1) * a.D;
   const uint32_t a_rows = (E == 0 && m_blocks == 1 && rows_total < BM) ? (uint32_t)((rows_total + 7) / 8 * 8) : BM;
+  // combinations: both operands are of one kind, the first in the sp_* (path 4) / dn_* (path 3) slots of the kernel
+  const bool dd = a.path == 3, ss = a.path == 4;
+  const void* first_dn = dd ? a.sp_codes : a.dn_codes;     // path 3: operand 0 arrives in the "sp" arguments of the ABI
   if (!env.plan_only &&
-      (!make_map(&tm_sp, a.sp_codes, (uint64_t)rows_total, (uint64_t)a.K / 4, 64, a_rows) ||
-       !make_map(&tm_dn, a.dn_codes, (uint64_t)rows_total, (uint64_t)a.K / 2, 128, a_rows) ||
+      (!make_map(&tm_sp, dd ? a.dn_codes : a.sp_codes, (uint64_t)rows_total, (uint64_t)a.K / (dd ? 2 : 4), dd ? 128 : 64, a_rows) ||
+       !make_map(&tm_dn, ss ? a.sp_codes : first_dn, (uint64_t)rows_total, (uint64_t)a.K / (ss ? 4 : 2), ss ? 64 : 128, a_rows) ||
+       !make_map(&tm_alt, a.dn_codes, (uint64_t)rows_total, (uint64_t)a.K / (ss ? 4 : 2), ss ? 64 : 128, a_rows) ||
        !make_map(&tm_w, a.w_codes, (uint64_t)w_rows, (uint64_t)a.K / 2, 128, BN < 256 ? BN : 256)))
     return SHARQ_ECUDA;
   const int64_t n_tiles = a.D / BN;
   const int64_t tiles = m_blocks * n_tiles;                  // grouped: an upper bound (the kernel knows the real count)
-  KParams p{(const uint8_t*)a.sp_sf, (const uint8_t*)a.sp_meta, (const uint8_t*)a.dn_sf, (const uint8_t*)a.w_sf_sp,
-            (const uint8_t*)a.w_sf_dn, a.row_scale, a.w_ts, (const uint16_t*)a.bias, a.Y, a.ldy,
+  // path 3: kernel slots dn_sf = operand 0's scales (ABI: sp_sf), sf2 = operand 1's (ABI: dn_sf)
+  // path 4: kernel slots sp_sf / sp_meta = operand 0, sf2 / meta2 = operand 1 (ABI: dn_sf / dn_meta)
+  KParams p{(const uint8_t*)a.sp_sf, (const uint8_t*)a.sp_meta, (const uint8_t*)(dd ? a.sp_sf : a.dn_sf),
+            (const uint8_t*)a.w_sf_sp, (const uint8_t*)a.w_sf_dn, a.row_scale, a.w_ts, (const uint16_t*)a.bias, a.Y, a.ldy,
             (int32_t)a.T, (int32_t)a.D, (int32_t)a.K, a.out_dtype, a.path, (int32_t)m_blocks,
-            (int32_t)(E > 0 ? n_tiles : tiles), offsets, (int32_t)E, (int32_t)a_rows};
+            (int32_t)(E > 0 ? n_tiles : tiles), offsets, (int32_t)E, (const uint8_t*)a.dn_sf, (const uint8_t*)a.dn_meta,
+            (int32_t)a_rows};
   const bool pair_worth = ((m_blocks + 1) / 2) * (a.D / 256) >= num_sms / 4 || debug_env().force_pair;
-  if (E == 0 && m_blocks >= 2 && BN == 128 && pair_worth && !debug_env().no_pair) {
+  if (E == 0 && m_blocks >= 2 && BN == 128 && pair_worth && !debug_env().no_pair && a.path < 3) {
     // tile width by a cost model fitted on the box over the eight Llama / Qwen prefill shapes at T = 2048 ..
     // 8192 (us per round of 74 tiles): 256-wide 0.54 per k-block + 4.5 (one TMEM accumulator: drain and pipeline
     // refill exposed), 192-wide 0.50 per k-block + 1.5 (drain hidden by the second accumulator, but more
@@ -1036,9 +1056,9 @@ sharq_status launch_tiles(const LinearArgs& a, int64_t rows_total, int64_t m_blo
     // experts: n-tiles of one 128-row block are consecutive (decode_unit), so tiles 2j and 2j+1 share activations
     if (E > 0 && n_tiles % 2 == 0 && !debug_env().no_mc) return launch_mc<FMT>(p, tm_sp, tm_dn, tm_w, tiles, env);
   }
-  if (a_rows <= 16) return launch_1cta<BN, FMT, 16>(a, p, tm_sp, tm_dn, tm_w, tiles, env);
-  if (a_rows <= 64) return launch_1cta<BN, FMT, 64>(a, p, tm_sp, tm_dn, tm_w, tiles, env);
-  return launch_1cta<BN, FMT, 128>(a, p, tm_sp, tm_dn, tm_w, tiles, env);
+  if (a_rows <= 16) return launch_1cta<BN, FMT, 16>(a, p, tm_sp, tm_dn, tm_w, tm_alt, tiles, env);
+  if (a_rows <= 64) return launch_1cta<BN, FMT, 64>(a, p, tm_sp, tm_dn, tm_w, tm_alt, tiles, env);
+  return launch_1cta<BN, FMT, 128>(a, p, tm_sp, tm_dn, tm_w, tm_alt, tiles, env);
 }
 
 }  // namespace
@@ -1080,7 +1100,7 @@ sharq_status launch_linear(const sharq_config* cfg, const LinearArgs& a, int32_t
   // (the decode launches are bound by tensor-pipe issue per k-block, not by HBM)
   // ... and only pays when the 128-wide tiles would need a second round on the SMs (measured: with fewer
   // tiles than SMs the narrower tiles + deeper K-split win)
-  if (E == 0 && a.T <= debug_env().wide_t && a.D % 256 == 0 && a.D / 128 > num_sms && !debug_env().no_wide) {
+  if (E == 0 && a.path < 3 && a.T <= debug_env().wide_t && a.D % 256 == 0 && a.D / 128 > num_sms && !debug_env().no_wide) {
     if (cfg->fmt == SHARQ_NVFP4) return launch_tiles<256, SHARQ_NVFP4>(a, rows_total, m_blocks, E, offsets, env);
     return launch_tiles<256, SHARQ_MXFP4>(a, rows_total, m_blocks, E, offsets, env);
   }

@@ -6,7 +6,8 @@ namespace sharq {
 
 struct LinearArgs {
   int64_t T, D, K;              // T = rows (grouped: row capacity of the padded activation buffers)
-  const void *sp_codes, *sp_sf, *sp_meta, *dn_codes, *dn_sf;
+  const void *sp_codes, *sp_sf, *sp_meta, *dn_codes, *dn_sf;   // paths 3 / 4: operand 0 (sp_*) and operand 1 (dn_*)
+  const void* dn_meta;                                          // path 4 only: metadata of the second sparse operand
   const float* row_scale;
   const void *w_codes, *w_sf_sp, *w_sf_dn;
   const float* w_ts;

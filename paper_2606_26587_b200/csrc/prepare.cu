@@ -150,7 +150,8 @@ __global__ void __launch_bounds__(512) sharq_prepare_kernel(const PrepParams p) 
       if (FMT == SHARQ_HIF4) {
         quantize_block_hif4(p, row, (uint32_t)k0, X, lane, act);
       } else if (act) {
-        if (p.mask24) quantize_block_e2m1_24<FMT>(p, row, (uint32_t)k0, X, ts, inv_ts);
+        if (p.combo) quantize_block_combo<FMT>(p, row, (uint32_t)k0, X, ts, inv_ts);
+        else if (p.mask24) quantize_block_e2m1_24<FMT>(p, row, (uint32_t)k0, X, ts, inv_ts);
         else quantize_block_e2m1<FMT>(p, row, (uint32_t)k0, X, ts, inv_ts);
       }
     }
@@ -286,8 +287,10 @@ static cudaError_t launch_norm(int norm, const PrepParams& p, dim3 grid, dim3 bl
 cudaError_t launch_prepare(const sharq_config* cfg, const void* x, int64_t T, int64_t K, int64_t ldx,
                            const void* gamma, const void* beta, const float* x_ts, void* sp_codes, void* sp_sf,
                            void* sp_meta, void* dn_codes, void* dn_sf, float* row_scale, int num_sms,
-                           cudaStream_t st, const void* residual, int64_t ldr, void* sum_out, int64_t ldo) {
+                           cudaStream_t st, const void* residual, int64_t ldr, void* sum_out, int64_t ldo,
+                           int combo, void* dn_meta) {
   PrepParams p;
+  p.combo = combo; p.dn_meta = (uint8_t*)dn_meta;
   p.res = (const uint16_t*)residual; p.sum_out = (uint16_t*)sum_out; p.ldr = ldr; p.ldo = ldo;
   p.x = (const uint16_t*)x; p.ldx = ldx; p.T = T; p.K = K;
   p.gamma = (const uint16_t*)gamma; p.beta = (const uint16_t*)beta; p.x_ts = x_ts;
@@ -300,8 +303,8 @@ cudaError_t launch_prepare(const sharq_config* cfg, const void* x, int64_t T, in
   // the row kernel reads 32 bytes per load: rows must start on 32-byte boundaries, otherwise (16-byte aligned
   // input, the C ABI's minimum) the warp-per-row kernel with its 16-byte cp.async takes the call
   const bool wide_ok = ((uintptr_t)x % 32 == 0) && (ldx % 16 == 0);
-  if (residual && (!wide_ok || K > 1024 * kRowMaxWarps || p.mask24)) return cudaErrorInvalidValue;   // checked by the C ABI
-  if (K <= 1024 * kRowMaxWarps && wide_ok && !p.mask24 && (!debug_env().old_prepare || residual)) {
+  if (residual && (!wide_ok || K > 1024 * kRowMaxWarps || p.mask24 || combo)) return cudaErrorInvalidValue;   // checked by the C ABI
+  if (K <= 1024 * kRowMaxWarps && wide_ok && !p.mask24 && !combo && (!debug_env().old_prepare || residual)) {
     p.nbuf = 0;
     if (cfg->fmt == SHARQ_NVFP4) return launch_row_chunks<SHARQ_NVFP4>(cfg->norm, p, num_sms, st);
     if (cfg->fmt == SHARQ_MXFP4) return launch_row_chunks<SHARQ_MXFP4>(cfg->norm, p, num_sms, st);
