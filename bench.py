@@ -588,6 +588,27 @@ def prefill_extras(sq, wl, pk, steps, mp=None):
                                                unfused_us=round(ms_u * 1e3, 1),
                                                unfused_note="torch bf16 add_ kernel + sharq_prepare (two launches)")}
     del xs, rs, acts
+    # SURVEY.md 8(f) N1, second fusion: SiLU(gate) * up in front of the down projection's preparation
+    # (sharq_prepare_swiglu) against torch's silu * mul kernels + sharq_prepare.  Algorithmic bytes of the fused pass:
+    # the prepare bytes + 2 (the second input) per element; h never goes to HBM.
+    Tp, K = 8192, 14336
+    cfg = wl.cfg["down"]
+    gus = [device_activations(Tp, 2 * K, BASE_SEED + 110 + j, outlier_mult=5.0) for j in range(2)]    # [T, 2K] gate | up
+    acts = [sq.alloc_act(cfg, Tp, K, "cuda") for _ in gus]
+    ms_f = timed([lambda j=j: sq.prepare_swiglu(cfg, gus[j][:, :K], gus[j][:, K:], out=acts[j]) for j in range(2)],
+                 max(steps, 12), 3, lambda: None)
+    hbuf = torch.empty((Tp, K), dtype=torch.bfloat16, device="cuda")
+
+    def unfused_swiglu(j):
+        torch.mul(torch.nn.functional.silu(gus[j][:, :K]), gus[j][:, K:], out=hbuf)
+        sq.prepare(cfg, hbuf, out=acts[j])
+    ms_u = timed([lambda j=j: unfused_swiglu(j) for j in range(2)], max(steps, 12), 3, lambda: None)
+    by = prepare_bytes(Tp, K) + 2.0 * Tp * K
+    out["prepare_swiglu"] = {f"T{Tp}_K{K}": dict(us=round(ms_f * 1e3, 1), GBps=round(by / (ms_f * 1e-3) / 1e9, 1),
+                                                 frac_of_hbm=round(by / (ms_f * 1e-3) / 1e9 / pk["hbm"], 4),
+                                                 unfused_us=round(ms_u * 1e3, 1),
+                                                 unfused_note="torch silu + mul kernels (MUFU exp, not bit-restatable) + sharq_prepare")}
+    del gus, acts, hbuf
     return out
 
 

@@ -7,7 +7,8 @@
  *   sharq_prepare          per call: norm -> N:M mask -> sparse FP4 backbone -> residual -> dense FP4
  *   sharq_linear           sparse + dense block-scaled FP4 GEMMs into one accumulator, bf16 epilogue
  * plus sharq_linear_grouped (the same over the row ranges of E experts, MoE), sharq_prepare_add
- * (sharq_prepare with the residual-stream add fused in front of the norm), host-only size / plan queries
+ * (sharq_prepare with the residual-stream add fused in front of the norm), sharq_prepare_swiglu (with
+ * SiLU(gate) * up fused in front of it), host-only size / plan queries
  * (sharq_weight_sizes, sharq_act_sizes, sharq_linear_workspace, sharq_linear_plan), sharq_act_init, the Table 5
  * path combinations (sharq_act_sizes_paths, sharq_prepare_paths, sharq_linear_paths) and the test
  * helpers sharq_untile_sf / sharq_untile_meta.  The tensor-pipe probe lives in sharq_diag.h.
@@ -144,6 +145,18 @@ sharq_status sharq_prepare_add(const sharq_config* cfg, const void* x, const voi
                                const float* x_tensor_scale, void* sp_codes, void* sp_sf,
                                void* sp_meta, void* dn_codes, void* dn_sf, float* row_scale,
                                void* stream);
+
+/* ---- sharq_prepare_swiglu (second fusion) -------------------------------------
+ * sharq_prepare for the down projection with the SwiGLU elementwise operator fused in front of it:
+ *     h[t,k] = bf16( silu(gate[t,k]) * up[t,k] ),   silu(g) = g / (1 + exp(-g))
+ * computed in fp32 by a fixed algorithm (degree-5 polynomial exp, IEEE reciprocal; R18) that the oracle
+ * restates bit for bit; h never goes to HBM and is the activation norm -> mask -> backbone -> residual see.
+ * gate / up: bf16 [T, K] (ldg / ldu elements between rows: the two halves of a [T, 2K] gate+up output work),
+ * 32-byte aligned, ldg / ldu multiples of 16, K <= 32768; otherwise SHARQ_EINVAL / SHARQ_ESHAPE. */
+sharq_status sharq_prepare_swiglu(const sharq_config* cfg, const void* gate, const void* up, int64_t T, int64_t K,
+                                  int64_t ldg, int64_t ldu, const void* gamma, const void* beta,
+                                  const float* x_tensor_scale, void* sp_codes, void* sp_sf, void* sp_meta,
+                                  void* dn_codes, void* dn_sf, float* row_scale, void* stream);
 
 /* ---- sharq_linear (Eq. 9) -----------------------------------------------
  * Y[T,D] = (A_sp . W^T through the sparse view  +  A_dn . W^T through the dense view)

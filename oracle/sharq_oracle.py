@@ -82,6 +82,48 @@ def residual_add(x_u16, r_u16):
 
 
 # --------------------------------------------------------------------------------------------
+# SwiGLU in front of the down-projection's preparation (R18)
+# --------------------------------------------------------------------------------------------
+# fp32 constants of the exp contract, as bit patterns so that both sides hold the same numbers
+NEG_LOG2E = np.array([0xBFB8AA3B], dtype=U32).view(F32)[0]          # -RN(log2 e)
+EXP2_POLY = np.array([0x3F800000, 0x3F317218, 0x3E75FDF0, 0x3D635847, 0x3C1D955B, 0x3AAEC3FF],
+                     dtype=U32).view(F32)                            # RN(ln2^k / k!), k = 0..5
+RINT_MAGIC = F32(12582912.0)                                         # 1.5 * 2^23: (t + M) - M = RNE integer of t
+
+
+def exp_neg_contract(g):
+    """e ~= exp(-g) for fp32 g by a fixed, restatable algorithm (every step ONE fp32 RN operation, no FMA):
+       t = clamp(RN(g * (-log2e)), -126, 126);  n = (t + M) - M (RNE integer);  f = RN(t - n)  in [-1/2, 1/2]
+       p = Horner_5(f) with c_k = RN(ln2^k / k!), each step RN(RN(p * f) + c_k);  e = RN(p * 2^n)
+    Relative error <= 3.5e-6 + |g| 1.3e-7 (degree-5 Taylor remainder 2.4e-6, roundings of log2e and of t),
+    pinned against math.exp."""
+    g = np.asarray(g, dtype=F32)
+    t = np.clip(g * NEG_LOG2E, F32(-126.0), F32(126.0)).astype(F32)
+    n = ((t + RINT_MAGIC) - RINT_MAGIC).astype(F32)
+    f = (t - n).astype(F32)
+    p = np.full(g.shape, EXP2_POLY[5], dtype=F32)
+    for k in (4, 3, 2, 1, 0):
+        p = ((p * f).astype(F32) + EXP2_POLY[k]).astype(F32)
+    two_n = ((n.astype(np.int32) + 127).astype(U32) << U32(23)).view(F32)
+    return (p * two_n).astype(F32)
+
+
+def swiglu(gate_u16, up_u16):
+    """h = bf16( silu(gate) * up ), silu(g) = g * sigmoid(g) = g / (1 + exp(-g)): the elementwise operator between
+    the gate/up projection and the down projection, which `sharq_prepare_swiglu` folds in front of the
+    preparation (the paper's lever is folding the neighbouring operator into the prep kernel).
+    fp32 steps, one RN each: e = exp_neg_contract(g); den = 1 + e; sig = 1 / den; s = g * sig; a = s * u;
+    one rounding to bf16 at the end (R18; definition unpinned by the paper)."""
+    g = bf16_to_f32(np.asarray(gate_u16, dtype=U16))
+    u = bf16_to_f32(np.asarray(up_u16, dtype=U16))
+    e = exp_neg_contract(g)
+    den = (F32(1.0) + e).astype(F32)
+    sig = (F32(1.0) / den).astype(F32)
+    s = (g * sig).astype(F32)
+    return f32_to_bf16((s * u).astype(F32))
+
+
+# --------------------------------------------------------------------------------------------
 # element / scale codecs
 # --------------------------------------------------------------------------------------------
 def e2m1_encode(v: np.ndarray) -> np.ndarray:

@@ -58,6 +58,7 @@ def _load() -> ctypes.CDLL:
     lib.sharq_quantize_weight.argtypes = [CFG, P, c_int64, c_int64, c_int64, P, P, P, P, P, c_size_t, P]
     lib.sharq_prepare.argtypes = [CFG, P, c_int64, c_int64, c_int64, P, P, P, P, P, P, P, P, P, P]
     lib.sharq_prepare_add.argtypes = [CFG, P, P, c_int64, c_int64, c_int64, c_int64, P, c_int64, P, P, P, P, P, P, P, P, P, P]
+    lib.sharq_prepare_swiglu.argtypes = [CFG, P, P, c_int64, c_int64, c_int64, c_int64, P, P, P, P, P, P, P, P, P, P]
     lib.sharq_linear.argtypes = [CFG, c_int64, c_int64, c_int64, P, P, P, P, P, P, P, P, P, P, P, P, c_int64,
                                  c_int32, c_int32, P, c_size_t, P]
     lib.sharq_linear_grouped.argtypes = [CFG, c_int32, P, c_int64, c_int64, c_int64, P, P, P, P, P, P, P, P,
@@ -78,7 +79,7 @@ def _load() -> ctypes.CDLL:
 
 # every symbol include/sharq.h declares, then include/sharq_diag.h's
 EXPORTS = ("sharq_version", "sharq_weight_sizes", "sharq_act_sizes", "sharq_linear_workspace",
-           "sharq_quantize_weight", "sharq_prepare", "sharq_prepare_add", "sharq_linear", "sharq_linear_grouped",
+           "sharq_quantize_weight", "sharq_prepare", "sharq_prepare_add", "sharq_prepare_swiglu", "sharq_linear", "sharq_linear_grouped",
            "sharq_act_init", "sharq_linear_plan", "sharq_untile_sf", "sharq_untile_meta", "sharq_act_sizes_paths",
            "sharq_prepare_paths", "sharq_linear_paths", "sharq_mma_peak_launch")
 capi = _load()
@@ -242,6 +243,19 @@ def linear_paths(cfg: Config, act: dict, wq: dict, bias=None, out_dtype="bf16", 
                                    _ptr(wq["ts_w"]), _ptr(bias), _ptr(Y), Y.stride(0), 0 if Y.dtype == torch.bfloat16 else 1,
                                    _stream()), "sharq_linear_paths")
     return Y
+
+
+def prepare_swiglu(cfg: Config, gate, up, gamma=None, beta=None, x_tensor_scale=None, out=None):
+    """sharq_prepare_swiglu: the preparation path on h = bf16(silu(gate) * up); gate / up may be the two column halves
+    of one [T, 2K] tensor."""
+    T, K = gate.shape
+    if out is None:
+        out = alloc_act(cfg, T, K, gate.device)
+    _check(capi.sharq_prepare_swiglu(ctypes.byref(cfg), _ptr(gate), _ptr(up), T, K, gate.stride(0), up.stride(0),
+                                     _ptr(gamma), _ptr(beta), _ptr(x_tensor_scale), _ptr(out["sp_codes"]), _ptr(out["sp_sf"]),
+                                     _ptr(out["sp_meta"]), _ptr(out["dn_codes"]), _ptr(out["dn_sf"]), _ptr(out["row_scale"]),
+                                     _stream()), "sharq_prepare_swiglu")
+    return out
 
 
 def act_slot(cfg: Config, act: dict, row0: int, T: int) -> dict:

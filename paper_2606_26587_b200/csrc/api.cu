@@ -167,6 +167,31 @@ sharq_status sharq_prepare_add(const sharq_config* cfg, const void* x, const voi
   return e == cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
 }
 
+// sharq_prepare with h = bf16(silu(gate) * up) computed on the fly (the row kernel's fused-operand path with no
+// sum_out: the activation never goes to HBM)
+sharq_status sharq_prepare_swiglu(const sharq_config* cfg, const void* gate, const void* up, int64_t T, int64_t K,
+                                  int64_t ldg, int64_t ldu, const void* gamma, const void* beta,
+                                  const float* x_tensor_scale, void* sp_codes, void* sp_sf, void* sp_meta,
+                                  void* dn_codes, void* dn_sf, float* row_scale, void* stream) {
+  sharq_status s = check_cfg(cfg);
+  if (s != SHARQ_OK) return s;
+  if (T < 0 || K <= 0 || K % 256 != 0 || K > 32768) return SHARQ_ESHAPE;
+  if (cfg->fmt != SHARQ_HIF4 && cfg->mask != SHARQ_MASK_PAIR48) return SHARQ_EINVAL;
+  if (ldg < K || ldu < K || ldg % 16 != 0 || ldu % 16 != 0) return SHARQ_ESHAPE;
+  if (T == 0) return SHARQ_OK;
+  if (!gate || !up || !sp_codes || !sp_sf || !sp_meta || !dn_codes || !dn_sf || !row_scale) return SHARQ_EINVAL;
+  if (cfg->norm != SHARQ_NORM_NONE && !gamma) return SHARQ_EINVAL;
+  if (((uintptr_t)gate & 31u) || ((uintptr_t)up & 31u)) return SHARQ_EINVAL;
+  if (!aligned16(sp_codes) || !aligned16(sp_sf) || !aligned16(sp_meta) || !aligned16(dn_codes) || !aligned16(dn_sf) ||
+      (gamma && !aligned16(gamma)) || (beta && !aligned16(beta)))
+    return SHARQ_EINVAL;
+  DeviceInfo di{};
+  if ((s = device_info(&di)) != SHARQ_OK) return s;
+  cudaError_t e = launch_prepare(cfg, gate, T, K, ldg, gamma, beta, x_tensor_scale, sp_codes, sp_sf, sp_meta, dn_codes,
+                                 dn_sf, row_scale, di.sms, (cudaStream_t)stream, up, ldu, nullptr, 0, 0, nullptr);
+  return e == cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
+}
+
 static sharq_status check_linear(const sharq_config* cfg, int64_t D, int64_t K, const void* const* ptrs, int n,
                                  int64_t ldy, int32_t out_dtype, int32_t path) {
   sharq_status s = check_cfg(cfg);

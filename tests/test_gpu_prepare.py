@@ -219,3 +219,25 @@ def test_tiled_pad_rows_are_initialised(sq):
     meta = sq.untile_meta(act["sp_meta"], 128, K).cpu().numpy()
     assert (sf[T:] == 0).all() and (dn[T:] == 0).all() and (meta[T:] == 0x44).all()
     assert (meta[:T] != 0).all()
+
+
+@pytest.mark.parametrize("fmt,T,K,halves", [(0, 16, 14336, True), (0, 700, 4096, False), (1, 33, 3584, True), (2, 9, 768, False),
+                                            (0, 300, 18944, True)])
+def test_prepare_swiglu_bit_exact(sq, fmt, T, K, halves):
+    """sharq_prepare_swiglu: every prepared output equals the oracle's preparation of
+    h = bf16(silu(gate) * up) computed by the restatable exp contract (R18); gate / up given as two tensors
+    or as the two column halves of one [T, 2K] gate+up output."""
+    g_bits = si.activations(T, K, config=4, outlier_mult=5.0, extra=T + 1)
+    u_bits = si.activations(T, K, config=5, outlier_mult=50.0, extra=K + 2)
+    g_bits[0, :8] = si.to_bf16_bits(np.array([0.0, -0.0, 40.0, -40.0, 100.0, -100.0, 1e-30, -88.0], np.float32))
+    cfg = sq.make_config(fmt, sq.NORM_NONE, 1e-6, sq.LAYOUT_CANONICAL if fmt == 2 else sq.LAYOUT_TILED)
+    if halves:
+        both = torch.cat([to_dev(g_bits), to_dev(u_bits)], dim=1)
+        gd, ud = both[:, :K], both[:, K:]
+    else:
+        gd, ud = to_dev(g_bits), to_dev(u_bits)
+    act = sq.prepare_swiglu(cfg, gd, ud)
+    torch.cuda.synchronize()
+    h = so.swiglu(g_bits, u_bits)
+    p = so.prepare(h, fmt=fmt, mask=cfg.mask, norm=so.NORM_NONE)
+    _compare_act(act_to_canonical(sq, cfg, act, T, K), p, f"swiglu fmt{fmt} T{T} K{K}")

@@ -464,3 +464,50 @@ def test_sparse_sparse_paths_and_table5_ordering(fmt):
     Yd = so.linear_paths(pd, wq)
     assert np.allclose(Yd, (pd["A0"].astype(np.float64) + pd["A1"].astype(np.float64)) @ Wd.T, rtol=1e-6,
                        atol=1e-6 * np.abs(Yd).max())
+
+
+# ------------------------------------------------------------------ SwiGLU contract (R18)
+def test_exp_contract_against_math_exp_and_special_values():
+    """exp_neg_contract(g) ~= exp(-g): constants are RN of their definitions, relative error <= 3e-6 against
+    math.exp over the whole useful range, exact at g = 0 and at g = -k ln 2 up to the rounding of t."""
+    assert so.NEG_LOG2E == F32(-math.log2(math.e))
+    for k in range(6):
+        assert so.EXP2_POLY[k] == F32(math.log(2.0) ** k / math.factorial(k)), k
+    assert so.exp_neg_contract(np.zeros(3, F32)).tolist() == [1.0, 1.0, 1.0]
+    g = np.concatenate([np.linspace(-80, 80, 20001), np.random.default_rng(0).standard_normal(20000) * 8]).astype(F32)
+    e = so.exp_neg_contract(g).astype(np.float64)
+    ref = np.array([math.exp(-float(v)) for v in g])
+    # degree-5 remainder 2.4e-6 + roundings; + the rounding of the constant log2e and of t = g * log2e (each up to
+    # |g| 2^-24 relative in e)
+    bound = 3.5e-6 + np.abs(g.astype(np.float64)) * 1.3e-7
+    assert (np.abs(e - ref) <= bound * ref).all(), float((np.abs(e - ref) / ref / bound).max())
+    # monotone non-increasing in g on a fine grid (a sign or index slip in the reduction would break it)
+    gs = np.sort(g)
+    es = so.exp_neg_contract(gs)
+    assert (np.diff(es.astype(np.float64)) <= 2e-6 * es[:-1]).all()
+    # clamp: no inf / nan at the ends, limits of the sigmoid
+    big = so.exp_neg_contract(np.array([-1e4, 1e4], F32))
+    assert np.isfinite(big).all() and big[0] >= 2.0 ** 125 and big[1] <= 2.0 ** -125
+
+
+def test_swiglu_against_fp64_definition():
+    """h = bf16(silu(g) * u): always one of the two bf16 neighbours of the exact value, equal to its RNE whenever the
+    exact value is not within 1e-5 (relative) of a rounding boundary; exact special cases by hand."""
+    rng = np.random.default_rng(1)
+    g = so.f32_to_bf16((rng.standard_normal(200000) * 4).astype(F32))
+    u = so.f32_to_bf16((rng.standard_normal(200000) * 2).astype(F32))
+    h = so.bf16_to_f32(so.swiglu(g, u)).astype(np.float64)
+    gf, uf = so.bf16_to_f32(g).astype(np.float64), so.bf16_to_f32(u).astype(np.float64)
+    exact = gf / (1.0 + np.exp(-gf)) * uf
+    rne = so.bf16_to_f32(so.f32_to_bf16(exact.astype(F32))).astype(np.float64)
+    ulp = 2.0 ** (np.floor(np.log2(np.maximum(np.abs(exact), 1e-300))) - 7)
+    assert (np.abs(h - exact) <= ulp * (0.5 + 1e-3) + 1e-38).all()               # a neighbour of the exact value
+    away = np.abs(np.abs(exact - rne) - ulp / 2) > 2e-5 * np.abs(exact)           # not near a tie of the bf16 grid
+    assert (h[away] == rne[away]).all()
+    assert away.mean() > 0.99
+    # by hand: g = 0 -> silu = 0; g = 40 -> sigmoid = 1 exactly in fp32 -> h = bf16(40 u); g = -40 -> ~ -40 e^-40 u
+    hh = so.bf16_to_f32(so.swiglu(so.f32_to_bf16(np.array([0.0, 40.0, -40.0, 1.0], F32)),
+                                  so.f32_to_bf16(np.array([3.0, 1.5, 2.0, 1.0], F32))))
+    assert hh[0] == 0.0 and hh[1] == 60.0
+    assert abs(hh[2] / (-40 * math.exp(-40) * 2.0) - 1) < 2.0 ** -8
+    assert hh[3] == so.bf16_to_f32(so.f32_to_bf16(np.array([1 / (1 + math.exp(-1))], F32)))[0]
