@@ -344,9 +344,16 @@ def run_ours(args):
                     algorithmic_flop_per_launch=round(2.0 * flops / n_lin), share_of_step=round(ms_lin / ms_step, 3))
     if mp is not None:
         q_dn, q_sp = mp["dense"]["sustained"], mp["sparse"]["sustained"]
+        r_dn, r_sp = mp["dense_random_operands"]["sustained"], mp["sparse_random_operands"]["sustained"]
         roofline.update(peak_probe=round(comb(q_dn, q_sp), 1), frac_probe=round(ach / comb(q_dn, q_sp), 4),
                         peak_probe_definition="same formula with P_dense / P_sparse measured on this GPU by the MMA issue "
-                                              "probe (sharq_diag.h), sustained; SURVEY.md 8(d) names this the applicable peak",
+                                              "probe (sharq_diag.h), sustained, CONSTANT operand bytes; SURVEY.md 8(d) names "
+                                              "the probe the applicable peak",
+                        peak_probe_random=round(comb(r_dn, r_sp), 1), frac_probe_random=round(ach / comb(r_dn, r_sp), 4),
+                        peak_probe_random_definition="the same probe fed pseudo-random operand bits: the GPU is power capped "
+                                                     "(clocks line), and a tensor pipe switching real data bits sustains a "
+                                                     "lower clock than one fed constants; real FP4 activations / weights "
+                                                     "lie between the two",
                         mma_issue_probe_tflops=mp)
     gbs = wl.prepare_bytes() / (ms_prep * 1e-3) / 1e9
     roofline_prepare = dict(kernel="sharq_prepare_row_kernel (the 4 sharq_prepare launches of the step)", bound="hbm",
@@ -522,7 +529,8 @@ def mma_issue_peaks(sq):
     import torch
     n_sm = torch.cuda.get_device_properties(0).multi_processor_count
     out = {}
-    for name, mode in (("dense", 1), ("sparse", 2), ("fused_with_sf_copies", 7)):
+    for name, mode in (("dense", 1), ("sparse", 2), ("fused_with_sf_copies", 7), ("dense_random_operands", 9),
+                       ("sparse_random_operands", 10), ("fused_random_operands", 15)):
         paths = (1 if mode & 1 else 0) + (1 if mode & 2 else 0)
         res = {}
         for kind, iters, secs in (("burst", 4000, 0.0), ("sustained", 40000, 1.5)):

@@ -5,7 +5,10 @@
  * that loop, and bench.py is its only caller.
  * Launches, on every SM pair, `iters` repetitions of the per-k-block (256 logical k) instruction sequence of the
  * CTA-pair GEMM on shared-memory-resident bytes: mode bit 1 = the 4 dense block-scaled MMAs, bit 2 = the 2 sparse
- * MMAs, bit 4 = the scale-factor / metadata tcgen05.cp copies; M = 256, N = 256 per pair, no loads, no epilogue.
+ * MMAs, bit 4 = the scale-factor / metadata tcgen05.cp copies, bit 8 = pseudo-random operand bits instead of constant
+ * bytes (the GPU is power capped: a pipe fed constants runs at higher clocks than one fed data, so the constant-
+ * operand rate is an upper bound of the applicable peak and the random-operand rate a lower bound); M = 256, N = 256
+ * per pair, no loads, no epilogue.
  * The caller times it (CUDA events): nominal flop per path = 2 * 128 * 256 * 256 * iters * (number of SMs). */
 #ifndef SHARQ_DIAG_H_
 #define SHARQ_DIAG_H_
