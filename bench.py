@@ -295,6 +295,9 @@ def run_ours(args):
     # ---- headline: BASELINE configs[2], the four Llama prefill linears at T = 8192 (the shapes the north-star
     # targets are quoted on): prepare + linear per layer, device-timed, CUDA-graph replay, MEAN of the steps ----
     wl = Workload(sq, rank, LLAMA, [T], n_sets)
+    if args.decode_only:                                  # short run for ncu: the configs[1] step alone
+        print(json.dumps({"decode_only": True, "decode_configs1": decode_extras(sq, wl, pk, steps, rank)}))
+        return
     if args.extras_only:
         ex = prefill_extras(sq, wl, pk, steps)
         if not args.short_extras:
@@ -810,6 +813,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--headline-only", action="store_true",
                     help="time only the whole-step region (short run for ncu launch lists / captures)")
+    ap.add_argument("--decode-only", action="store_true", help="only the configs[1] decode step (short run for ncu)")
     ap.add_argument("--short-extras", action="store_true", help="with --extras-only: skip configs 3-5")
     ap.add_argument("--extras-only", action="store_true",
                     help="only the prefill (T=4096) linear and T=8192 prepare measurements (short run for ncu)")

@@ -101,7 +101,9 @@ sharq_status sharq_linear_workspace(const sharq_config* cfg, int64_t T, int64_t 
  *   sf_sparse_view  [D, K/32] e4m3|e8m0     one scale per 32 k   (HiF4: [D, K/64] uint32 words)
  *   sf_dense_view   [D, K/16] e4m3          every sparse-view scale repeated for its two
  *                                           16-groups (MXFP4: [D,K/32], equal to the sparse
- *                                           view; HiF4: equal to the sparse view)
+ *                                           view; HiF4: bf16 [D, K], the EXACT dequantisation of
+ *                                           the payload -- every HiF4 value has <= 6 significant
+ *                                           bits -- which the bf16 tensor path multiplies with)
  *   tensor_scale    1 float                 NVFP4: max|W| / 2688; otherwise 1
  *   workspace       >= sharq_weight_sizes(...workspace) bytes; used for the max|W| reduction
  * Scale views follow cfg->layout.  Two kernels (amax, quantize); not on the timed path. */
@@ -167,8 +169,9 @@ sharq_status sharq_prepare_swiglu(const sharq_config* cfg, const void* gate, con
  * out_dtype: 0 = bf16, 1 = fp32.  bias bf16 [D] or NULL.  ldy in elements.
  * path: 0 = sparse + dense (SharQ), 1 = sparse only, 2 = dense only (Table 5 rows).
  * HiF4 (layout CANONICAL): tcgen05 has no S1P2 / E6M2 formats, so the operands are dequantised to bf16
- * (exact: every HiF4 value has <= 6 significant bits) into `workspace` and multiplied by a dense bf16
- * tensor-core GEMM with fp32 accumulation; workspace >= sharq_linear_workspace(...) bytes is required.
+ * (exact: every HiF4 value has <= 6 significant bits): the weight once, by sharq_quantize_weight (its
+ * sf_dense_view), the activation operands per call into `workspace`, and multiplied by a dense bf16 tensor-core
+ * GEMM with fp32 accumulation; workspace >= sharq_linear_workspace(...) bytes is required.
  * NVFP4 / MXFP4 need no workspace (it may be NULL).  Kernels are launched with programmatic dependent
  * launch: the weight stream of sharq_linear may start while the preceding kernel of the stream (normally
  * sharq_prepare) is still draining; all reads of activation operands wait for it to complete. */

@@ -74,7 +74,8 @@ sharq_status sharq_weight_sizes(const sharq_config* cfg, int64_t D, int64_t K, s
   if (D < 0 || K <= 0 || K % 256 != 0) return SHARQ_ESHAPE;
   if (codes) *codes = (size_t)D * (size_t)(K / 2);
   if (sf_sparse_view) *sf_sparse_view = sf_bytes(cfg, D, sf_cols(cfg->fmt, false, K));
-  if (sf_dense_view) *sf_dense_view = sf_bytes(cfg, D, sf_cols(cfg->fmt, true, K));
+  if (sf_dense_view)                                       // HiF4: the exact bf16 dequantisation [D, K] (the GEMM-side view)
+    *sf_dense_view = cfg->fmt == SHARQ_HIF4 ? (size_t)D * (size_t)K * 2 : sf_bytes(cfg, D, sf_cols(cfg->fmt, true, K));
   if (workspace) *workspace = 256;
   return SHARQ_OK;
 }

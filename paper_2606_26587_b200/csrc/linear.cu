@@ -65,6 +65,7 @@ struct KParams {
   // into the same accumulator, the second time on the SECOND operand of the same kind (tensor map tm_alt, scale
   // factors sf2, metadata meta2); W is streamed twice
   const uint8_t *sf2, *meta2;
+  int32_t group_m;    // pair kernel: 256-row blocks per supertile (tile order, see pair_tile)
   int32_t a_rows;     // rows of the activation TMA boxes: 128, or roundup(T, 8) when T < 128 (out-of-bounds
                       // rows are zero-filled slowly; rows beyond the box keep stale smem, which only feeds
                       // accumulator rows that are never stored)
@@ -601,6 +602,22 @@ struct PairStage {
   static_assert(SF0 + 76 <= 512, "tensor memory");
 };
 
+// Tile order of the pair kernel.  Tiles run m-fastest inside a SUPERTILE of `gm` 256-row blocks x all n-tiles: the
+// concurrently running clusters then touch gm activation blocks (which stay in L2 for the whole supertile, read from
+// DRAM once) and one or two W tiles at a time.  gm = all row blocks reproduces the plain m-fastest order (right when
+// the whole activation operand fits in L2); with a long K and many tokens (down projection at T = 8192: 106 MB of
+// activation operands) the plain order cycled the whole operand through L2 once per two n-tiles: 782 MB of DRAM
+// reads for 137 MB of operands (profiles/linear_pair_r2_ncu_full.md).
+__device__ __forceinline__ void pair_tile(int tile, int m_pairs, int n_tiles, int gm, int& m_pair, int& n_blk) {
+  const int per_group = gm * n_tiles;
+  const int g = tile / per_group;
+  const int g0 = g * gm;
+  const int rows = min(gm, m_pairs - g0);              // the last supertile may be shorter
+  const int within = tile - g * per_group;
+  m_pair = g0 + within % rows;
+  n_blk = within / rows;
+}
+
 template <int FMT, int PBN>
 __global__ void __launch_bounds__(kThreads, 1)
 sharq_linear_pair_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_constant__ CUtensorMap tm_a_dn,
@@ -624,7 +641,9 @@ sharq_linear_pair_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __gr
   const bool do_sp = p.path != 2, do_dn = p.path != 1;
   const int num_kb = p.K / BK;
   const int m_pairs = (p.m_blocks + 1) / 2;
-  const int total = m_pairs * ((p.D + S::BN - 1) / S::BN);      // the last tile may be ragged in N
+  const int n_tiles = (p.D + S::BN - 1) / S::BN;                // the last tile may be ragged in N
+  const int total = m_pairs * n_tiles;
+  const int gm = p.group_m > 0 && p.group_m < m_pairs ? p.group_m : m_pairs;
   const int tile0 = (int)tc::cluster_id_x(), tile_step = (int)(gridDim.x >> 1);
 
   if (warp == 0 && lane == 0) {
@@ -672,7 +691,9 @@ sharq_linear_pair_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __gr
       const int kq = p.K / 256;
       uint32_t it = 0;
       for (int tile = tile0; tile < total; tile += tile_step) {
-        const int m_blk = 2 * (tile % m_pairs) + rank, n_blk = tile / m_pairs;
+        int m_pair, n_blk;
+        pair_tile(tile, m_pairs, n_tiles, gm, m_pair, n_blk);
+        const int m_blk = 2 * m_pair + rank;
         const int m_sf = min(m_blk, p.m_blocks - 1);       // a ragged pair's second CTA: valid memory, unused rows
         const int n0 = n_blk * S::BN;
         const int wblk0 = n0 / 128;
@@ -709,7 +730,9 @@ sharq_linear_pair_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __gr
       for (int tile = tile0; tile < total; tile += tile_step, ++n_unit) {
         const uint32_t as = n_unit % S::ACC_STAGES;
         const uint32_t acc = tmem_base + as * S::BN;
-        const uint32_t sfb_shift = (uint32_t)((((tile / m_pairs) * S::BN) % 128) / 32);   // tile starts inside a 128-row atom
+        int m_pair_u, n_blk_u;
+        pair_tile(tile, m_pairs, n_tiles, gm, m_pair_u, n_blk_u);
+        const uint32_t sfb_shift = (uint32_t)(((n_blk_u * S::BN) % 128) / 32);   // tile starts inside a 128-row atom
         tc::mbar_wait(tmem_empty_bar(as), ((n_unit / S::ACC_STAGES) & 1u) ^ 1u);   // both CTAs' epilogues drained it
         tc::tc_fence_after();
         uint32_t accumulate = 0;
@@ -772,7 +795,9 @@ sharq_linear_pair_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __gr
     const uint32_t lane_addr = tmem_base + ((uint32_t)(sub * 32) << 16);
     uint32_t n_unit = 0;
     for (int tile = tile0; tile < total; tile += tile_step, ++n_unit) {
-      const int m_blk = 2 * (tile % m_pairs) + rank, n_blk = tile / m_pairs;
+      int m_pair, n_blk;
+      pair_tile(tile, m_pairs, n_tiles, gm, m_pair, n_blk);
+      const int m_blk = 2 * m_pair + rank;
       const int64_t row = (int64_t)m_blk * BM + r_local;
       const bool row_ok = row < p.T;
       const float scale = row_ok ? __fmul_rn(p.row_scale[row], p.w_ts[0]) : 0.0f;
@@ -1036,7 +1061,7 @@ sharq_status launch_tiles(const LinearArgs& a, int64_t rows_total, int64_t m_blo
             (const uint8_t*)a.w_sf_sp, (const uint8_t*)a.w_sf_dn, a.row_scale, a.w_ts, (const uint16_t*)a.bias, a.Y, a.ldy,
             (int32_t)a.T, (int32_t)a.D, (int32_t)a.K, a.out_dtype, a.path, (int32_t)m_blocks,
             (int32_t)(E > 0 ? n_tiles : tiles), offsets, (int32_t)E, (const uint8_t*)a.dn_sf, (const uint8_t*)a.dn_meta,
-            (int32_t)a_rows};
+            0, (int32_t)a_rows};
   const bool pair_worth = ((m_blocks + 1) / 2) * (a.D / 256) >= num_sms / 4 || debug_env().force_pair;
   if (E == 0 && m_blocks >= 2 && BN == 128 && pair_worth && !debug_env().no_pair && a.path < 3) {
     // tile width by a cost model fitted on the box over the eight Llama / Qwen prefill shapes at T = 2048 ..
@@ -1049,6 +1074,16 @@ sharq_status launch_tiles(const LinearArgs& a, int64_t rows_total, int64_t m_blo
     const double cost256 = (double)((m_pairs * ((a.D + 255) / 256) + clusters - 1) / clusters) * (0.5375 * kb + 4.5);
     int width = (a.D % 256 != 0 || cost192 < cost256) ? 192 : 256;
     if (debug_env().pair_bn > 0) width = (debug_env().pair_bn == 256 && a.D % 256 == 0) ? 256 : 192;
+    // supertile height: the whole activation operand when it sits comfortably in L2 beside the streamed W tiles,
+    // otherwise as many 256-row blocks as fit beside (the resident part of) W in ~72 MB of the 126 MB L2
+    const double a_pair = 256.0 * (double)a.K * 0.90625, a_total = a_pair * (double)m_pairs;
+    const double w_total = (double)a.D * (double)a.K * 0.59375;
+    if (a_total > 48e6) {
+      const double room = 72e6 - (w_total < 40e6 ? w_total : 40e6);
+      int64_t gm = (int64_t)(room / a_pair);
+      p.group_m = (int32_t)(gm < 1 ? 1 : gm > m_pairs ? m_pairs : gm);
+    }
+    if (debug_env().pair_gm > 0) p.group_m = debug_env().pair_gm;
     if (width == 256) return launch_pair<FMT, 256>(a, p, tm_sp, tm_dn, m_blocks, env);
     return launch_pair<FMT, 192>(a, p, tm_sp, tm_dn, m_blocks, env);
   }

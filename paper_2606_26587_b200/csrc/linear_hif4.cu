@@ -4,7 +4,8 @@
 // HiF4 value E6M2 * 2^(E1_8 + E1_16) * S1P2 = (4 + m) * k * 2^(E - 52 + shift) with (4 + m) * k <= 49
 // has at most 6 significant bits, i.e. it is EXACT in bf16.  The path is therefore:
 //   1. hif4_dequant_*  : codes + 32-bit unit metadata -> bf16 (exact), activations as [T, 2K] =
-//                        [backbone with zeros at dropped positions | residual], weights as [D, K];
+//                        [backbone with zeros at dropped positions | residual] on every call, weights as [D, K]
+//                        ONCE, by sharq_quantize_weight (the HiF4 "dense view" of the payload is this bf16 tensor);
 //   2. hif4_gemm_kernel: dense bf16 tcgen05.mma (kind::f16, fp32 accumulate) over the 2K-long rows, the
 //                        W tile reused for both halves (k and k + K read the same weight columns):
 //                        Y = A_sp W^T + A_dn W^T in one accumulator.
@@ -283,9 +284,19 @@ sharq_status launch_gemm(const CUtensorMap& tm_a, const CUtensorMap& tm_w, const
 
 }  // namespace
 
-size_t hif4_linear_workspace_bytes(int64_t T, int64_t D, int64_t K) {
+size_t hif4_linear_workspace_bytes(int64_t T, int64_t, int64_t K) {
   const int64_t Tp = round_up(T, 128);
-  return (size_t)Tp * (size_t)(2 * K) * 2 + (size_t)D * (size_t)K * 2 + 256;
+  return (size_t)Tp * (size_t)(2 * K) * 2 + 256;       // the bf16 copy of the activation operands [T, 2K]
+}
+
+// offline, once per weight (sharq_quantize_weight): the bf16 view of the HiF4 payload
+cudaError_t launch_hif4_dequant_weight(const void* codes, const void* sf, void* W_bf16, int64_t D, int64_t K,
+                                       cudaStream_t st) {
+  const int64_t nw = D * (K >> 3);
+  if (nw == 0) return cudaSuccess;
+  hif4_dequant_weight_kernel<<<(unsigned)((nw + 255) / 256 < 16384 ? (nw + 255) / 256 : 16384), 256, 0, st>>>(
+      (const uint8_t*)codes, (const uint32_t*)sf, (uint16_t*)W_bf16, D, K);
+  return cudaGetLastError();
 }
 
 sharq_status launch_linear_hif4(const LinearArgs& a, void* workspace, size_t workspace_bytes, int num_sms,
@@ -294,13 +305,11 @@ sharq_status launch_linear_hif4(const LinearArgs& a, void* workspace, size_t wor
   if (a.K > (int64_t)1 << 24 || a.D > (int64_t)1 << 24 || a.T > (int64_t)1 << 30) return SHARQ_ESHAPE;
   const int64_t Tp = round_up(a.T, 128);
   uint16_t* A = reinterpret_cast<uint16_t*>((reinterpret_cast<uintptr_t>(workspace) + 127) & ~(uintptr_t)127);
-  uint16_t* W = A + (size_t)Tp * (size_t)(2 * a.K);
-  const int64_t na = a.T * (a.K >> 3), nw = a.D * (a.K >> 3);
+  const uint16_t* W = reinterpret_cast<const uint16_t*>(a.w_sf_dn);   // bf16 [D, K], written by sharq_quantize_weight
+  const int64_t na = a.T * (a.K >> 3);
   hif4_dequant_act_kernel<<<(unsigned)((na + 255) / 256 < 8192 ? (na + 255) / 256 : 8192), 256, 0, st>>>(
       (const uint8_t*)a.sp_codes, (const uint32_t*)a.sp_sf, (const uint8_t*)a.sp_meta, (const uint8_t*)a.dn_codes,
       (const uint32_t*)a.dn_sf, A, a.T, a.K, a.path);
-  hif4_dequant_weight_kernel<<<(unsigned)((nw + 255) / 256 < 16384 ? (nw + 255) / 256 : 16384), 256, 0, st>>>(
-      (const uint8_t*)a.w_codes, (const uint32_t*)a.w_sf_sp, W, a.D, a.K);
   if (cudaGetLastError() != cudaSuccess) return SHARQ_ECUDA;
   CUtensorMap tm_a, tm_w;
   const bool wide = a.D % 256 == 0;

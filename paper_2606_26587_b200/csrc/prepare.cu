@@ -387,11 +387,8 @@ __global__ void weight_quant_kernel(const uint16_t* W, int64_t D, int64_t K, int
     const uint32_t word = hif4_meta_word(hs.e6m2, e8b, e16b, lane);
     if (!act) return;
     *reinterpret_cast<uint4*>(codes + d * (K >> 1) + (k0 >> 1)) = make_uint4(c[0], c[1], c[2], c[3]);
-    if ((lane & 1) == 0) {
-      reinterpret_cast<uint32_t*>(sf_sp)[d * (K >> 6) + (k0 >> 6)] = word;
-      reinterpret_cast<uint32_t*>(sf_dn)[d * (K >> 6) + (k0 >> 6)] = word;
-    }
-    return;
+    if ((lane & 1) == 0) reinterpret_cast<uint32_t*>(sf_sp)[d * (K >> 6) + (k0 >> 6)] = word;
+    return;                                         // the dense view (exact bf16 values) is written by a second kernel
   }
   if (!act) return;
   uint32_t amax = 0;
@@ -423,6 +420,8 @@ __global__ void weight_quant_kernel(const uint16_t* W, int64_t D, int64_t K, int
   }
 }
 
+cudaError_t launch_hif4_dequant_weight(const void* codes, const void* sf, void* W_bf16, int64_t D, int64_t K, cudaStream_t st);
+
 cudaError_t launch_quantize_weight(const sharq_config* cfg, const void* W, int64_t D, int64_t K, int64_t ldw,
                                    void* codes, void* sf_sp, void* sf_dn, float* ts, void* workspace,
                                    cudaStream_t st) {
@@ -442,7 +441,10 @@ cudaError_t launch_quantize_weight(const sharq_config* cfg, const void* W, int64
   else if (cfg->fmt == SHARQ_MXFP4) SHARQ_WQ(SHARQ_MXFP4);
   else SHARQ_WQ(SHARQ_HIF4);
 #undef SHARQ_WQ
-  return cudaGetLastError();
+  if ((e = cudaGetLastError()) != cudaSuccess) return e;
+  // HiF4: the GEMM-side ("dense") view of the payload is its exact bf16 dequantisation, made once here
+  if (cfg->fmt == SHARQ_HIF4) return launch_hif4_dequant_weight(codes, sf_sp, sf_dn, D, K, st);
+  return cudaSuccess;
 }
 
 // ---- test helpers: TILED -> canonical (include/sharq.h "Output layouts"); pure index maps --------------------------

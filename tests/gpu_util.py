@@ -63,7 +63,7 @@ def weight_to_canonical(sq, cfg, wq, D, K):
     out = dict(codes=host(wq["codes"], D * K // 2).reshape(D, K // 2), ts_w=float(host(wq["ts_w"])[0]))
     if cfg.fmt == sq.HIF4:
         out["sf_sp"] = host(wq["sf_sp"], D * K // 16).view(np.uint32).reshape(D, K // 64)
-        out["sf_dn"] = host(wq["sf_dn"], D * K // 16).view(np.uint32).reshape(D, K // 64)
+        out["w_bf16"] = host(wq["sf_dn"], D * K * 2).view(np.uint16).reshape(D, K)      # HiF4 dense view: exact bf16 values
         return out
     Cd = K // 16 if cfg.fmt == sq.NVFP4 else K // 32
     if cfg.layout == sq.LAYOUT_TILED:

@@ -41,6 +41,7 @@ def test_sizes_follow_the_header(sq):
     cfg_m = sq.make_config(sq.MXFP4, layout=sq.LAYOUT_CANONICAL)
     assert sq.act_sizes(cfg_m, T, K)[4] == T * K // 32
     cfg_h = sq.make_config(sq.HIF4)
+    assert sq.weight_sizes(cfg_h, D, K)[:3] == (D * K // 2, D * K // 16, D * K * 2)      # dense view = bf16 [D, K]
     assert sq.act_sizes(cfg_h, T, K) == (T * K // 4, T * K // 16, T * K // 8, T * K // 2, T * K // 16, T * 4)
 
 

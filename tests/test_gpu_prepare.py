@@ -93,8 +93,11 @@ def test_quantize_weight_bit_exact(sq, fmt, layout, D, K):
     torch.cuda.synchronize()
     ref = so.quantize_weight(w, fmt)
     got = weight_to_canonical(sq, cfg, wq, D, K)
-    for key in ("codes", "sf_sp", "sf_dn"):
+    for key in ("codes", "sf_sp") + (("sf_dn",) if fmt != 2 else ()):
         assert np.array_equal(got[key], ref[key]), key
+    if fmt == 2:      # the GEMM-side view of a HiF4 payload is its exact bf16 dequantisation (Eq. 15)
+        w64 = so.dequant_weight(ref)
+        assert np.array_equal(so.bf16_to_f32(got["w_bf16"]).astype(np.float64), w64)
     assert np.float32(got["ts_w"]) == ref["ts_w"]
 
 
