@@ -28,7 +28,8 @@
  *   - bf16 tensors are row-major; "code" tensors hold two 4-bit codes per byte, the element
  *     with the lower k in the low nibble.
  *   - Shapes: K % 256 == 0 (8-chunks, 32/64 scale groups, MMA-K 128, 256-wide metadata tile),
- *     D % 128 == 0 for sharq_linear, T >= 0 (T == 0 returns SHARQ_OK without a launch), T < 2^30.
+ *     D % 8 == 0 for sharq_linear (D % 128 == 0 for HiF4 and for sharq_linear_grouped), T >= 0 (T == 0 returns
+ *     SHARQ_OK without a launch), T < 2^30.
  *   - Inputs must be finite; NaN/Inf behaviour is deterministic but unspecified.
  *
  * Output layouts (config.layout)

@@ -98,7 +98,8 @@ sharq_status sharq_linear_workspace(const sharq_config* cfg, int64_t T, int64_t 
                                     size_t* workspace) {
   sharq_status s = check_cfg(cfg);
   if (s != SHARQ_OK) return s;
-  if (T < 0 || D <= 0 || D % 128 != 0 || K <= 0 || K % 256 != 0 || E < 0) return SHARQ_ESHAPE;
+  if (T < 0 || D <= 0 || D % 8 != 0 || K <= 0 || K % 256 != 0 || E < 0) return SHARQ_ESHAPE;
+  if ((cfg->fmt == SHARQ_HIF4 || E > 0) && D % 128 != 0) return SHARQ_ESHAPE;
   if (cfg->fmt != SHARQ_HIF4 && cfg->mask != SHARQ_MASK_PAIR48) return SHARQ_ESHAPE;
   if (workspace) *workspace = linear_workspace_bytes(cfg, T, D, K, E);
   return SHARQ_OK;
@@ -199,7 +200,8 @@ static sharq_status check_linear(const sharq_config* cfg, int64_t D, int64_t K, 
   if (s != SHARQ_OK) return s;
   if (cfg->fmt != SHARQ_HIF4 && cfg->mask != SHARQ_MASK_PAIR48) return SHARQ_ESHAPE;   // no element-wise 2:4 FP4 MMA
   if (cfg->layout != SHARQ_LAYOUT_TILED && cfg->fmt != SHARQ_HIF4) return SHARQ_EINVAL;
-  if (D <= 0 || D % 128 != 0 || K <= 0 || K % 256 != 0 || ldy < D || ldy % 8 != 0) return SHARQ_ESHAPE;
+  if (D <= 0 || D % 8 != 0 || K <= 0 || K % 256 != 0 || ldy < D || ldy % 8 != 0) return SHARQ_ESHAPE;
+  if (cfg->fmt == SHARQ_HIF4 && D % 128 != 0) return SHARQ_ESHAPE;     // the bf16 emulation tiles D by 128
   if (out_dtype < 0 || out_dtype > 1 || path < 0 || path > 4) return SHARQ_EINVAL;
   for (int i = 0; i < n; ++i)
     if (!ptrs[i] || !aligned16(ptrs[i])) return SHARQ_EINVAL;

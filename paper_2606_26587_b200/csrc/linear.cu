@@ -145,26 +145,32 @@ __device__ __forceinline__ Unit decode_unit(const KParams& p, const GroupTab& g,
   return u;
 }
 
-// y = acc * scale (+ bias) for N consecutive output features of one row, bf16 or fp32 store
+// y = acc * scale (+ bias) for N consecutive output features of one row, bf16 or fp32 store.  Columns at or beyond D
+// (the ragged last n-tile: D % 8 == 0, any multiple of 8) are neither computed with bias nor stored.
 template <int N>
 __device__ __forceinline__ void store_row(const KParams& p, int64_t row, int col0, float scale, float (&f)[N]) {
+  const int ncols = p.D - col0;                       // >= N for every tile but the last
+  if (ncols <= 0) return;
 #pragma unroll
   for (int i = 0; i < N; ++i) f[i] = __fmul_rn(f[i], scale);
   if (p.bias) {
     const uint16_t* b = p.bias + col0;
 #pragma unroll
-    for (int i = 0; i < N; ++i) f[i] = __fadd_rn(f[i], __uint_as_float((uint32_t)b[i] << 16));
+    for (int i = 0; i < N; ++i)
+      if (i < ncols) f[i] = __fadd_rn(f[i], __uint_as_float((uint32_t)b[i] << 16));
   }
   if (p.out_fp32) {
     float4* dst = reinterpret_cast<float4*>(static_cast<float*>(p.Y) + row * p.ldy + col0);
 #pragma unroll
-    for (int i = 0; i < N / 4; ++i) dst[i] = make_float4(f[4 * i], f[4 * i + 1], f[4 * i + 2], f[4 * i + 3]);
+    for (int i = 0; i < N / 4; ++i)
+      if (4 * i < ncols) dst[i] = make_float4(f[4 * i], f[4 * i + 1], f[4 * i + 2], f[4 * i + 3]);
   } else {
     uint4* dst = reinterpret_cast<uint4*>(static_cast<uint16_t*>(p.Y) + row * p.ldy + col0);
 #pragma unroll
     for (int i = 0; i < N / 8; ++i)
-      dst[i] = make_uint4(pack_bf16x2_rn(f[8 * i], f[8 * i + 1]), pack_bf16x2_rn(f[8 * i + 2], f[8 * i + 3]),
-                          pack_bf16x2_rn(f[8 * i + 4], f[8 * i + 5]), pack_bf16x2_rn(f[8 * i + 6], f[8 * i + 7]));
+      if (8 * i < ncols)
+        dst[i] = make_uint4(pack_bf16x2_rn(f[8 * i], f[8 * i + 1]), pack_bf16x2_rn(f[8 * i + 2], f[8 * i + 3]),
+                            pack_bf16x2_rn(f[8 * i + 4], f[8 * i + 5]), pack_bf16x2_rn(f[8 * i + 6], f[8 * i + 7]));
   }
 }
 
@@ -1053,7 +1059,8 @@ sharq_status launch_tiles(const LinearArgs& a, int64_t rows_total, int64_t m_blo
        !make_map(&tm_alt, a.dn_codes, (uint64_t)rows_total, (uint64_t)a.K / (ss ? 4 : 2), ss ? 64 : 128, a_rows) ||
        !make_map(&tm_w, a.w_codes, (uint64_t)w_rows, (uint64_t)a.K / 2, 128, BN < 256 ? BN : 256)))
     return SHARQ_ECUDA;
-  const int64_t n_tiles = a.D / BN;
+  const int64_t n_tiles = (a.D + BN - 1) / BN;               // the last n-tile may be ragged (D % 8 == 0): W rows beyond D
+                                                             // are zero-filled by TMA, their columns never stored
   const int64_t tiles = m_blocks * n_tiles;                  // grouped: an upper bound (the kernel knows the real count)
   // path 3: kernel slots dn_sf = operand 0's scales (ABI: sp_sf), sf2 = operand 1's (ABI: dn_sf)
   // path 4: kernel slots sp_sf / sp_meta = operand 0, sf2 / meta2 = operand 1 (ABI: dn_sf / dn_meta)
@@ -1062,7 +1069,7 @@ sharq_status launch_tiles(const LinearArgs& a, int64_t rows_total, int64_t m_blo
             (int32_t)a.T, (int32_t)a.D, (int32_t)a.K, a.out_dtype, a.path, (int32_t)m_blocks,
             (int32_t)(E > 0 ? n_tiles : tiles), offsets, (int32_t)E, (const uint8_t*)a.dn_sf, (const uint8_t*)a.dn_meta,
             0, (int32_t)a_rows};
-  const bool pair_worth = ((m_blocks + 1) / 2) * (a.D / 256) >= num_sms / 4 || debug_env().force_pair;
+  const bool pair_worth = ((m_blocks + 1) / 2) * ((a.D + 255) / 256) >= num_sms / 4 || debug_env().force_pair;
   if (E == 0 && m_blocks >= 2 && BN == 128 && pair_worth && !debug_env().no_pair && a.path < 3) {
     // tile width by a cost model fitted on the box over the eight Llama / Qwen prefill shapes at T = 2048 ..
     // 8192 (us per round of 74 tiles): 256-wide 0.54 per k-block + 4.5 (one TMEM accumulator: drain and pipeline
@@ -1130,7 +1137,8 @@ sharq_status launch_linear(const sharq_config* cfg, const LinearArgs& a, int32_t
     rows_total = m_blocks * BM;
     if (m_blocks == 0) return SHARQ_OK;
   }
-  if (m_blocks * (a.D / 128) > (int64_t)1 << 30) return SHARQ_ESHAPE;
+  if (m_blocks * ((a.D + 127) / 128) > (int64_t)1 << 30) return SHARQ_ESHAPE;
+  if (E > 0 && a.D % 128 != 0) return SHARQ_ESHAPE;       // stacked expert weights: whole 128-row scale atoms per expert
   // T <= 128 (one m-block): 128 x 256 tiles halve the per-column cost of the scale-factor copies and of the M = 128 MMA
   // (the decode launches are bound by tensor-pipe issue per k-block, not by HBM)
   // ... and only pays when the 128-wide tiles would need a second round on the SMs (measured: with fewer

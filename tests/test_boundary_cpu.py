@@ -92,4 +92,7 @@ def test_argument_validation_returns_codes_without_touching_cuda(sq):
     with pytest.raises(sq.SharqError):
         sq.act_sizes(cfg, 16, 1000)
     with pytest.raises(sq.SharqError):
-        sq.linear_workspace(cfg, 16, 100, 1024)          # D % 128
+        sq.linear_workspace(cfg, 16, 100, 1024)          # D % 8
+    assert sq.linear_workspace(cfg, 16, 200, 1024) == 0  # any multiple of 8
+    with pytest.raises(sq.SharqError):
+        sq.linear_workspace(sq.make_config(sq.HIF4), 16, 200, 1024)      # HiF4 emulation: D % 128

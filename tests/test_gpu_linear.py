@@ -370,3 +370,60 @@ def test_moe_config5_down_projection_sampled(sq):
         y64 = so.linear(so.prepare(x[offsets[e]: offsets[e + 1]], norm=0), so.quantize_weight(ws[e]))
         got = Y[pad_off[e]: pad_off[e] + counts[e]]
         assert rel_err(got, y64).max() <= TOL, f"expert {e}"
+
+
+@pytest.mark.parametrize("fmt,T,K,D", [(0, 16, 1024, 200), (0, 300, 512, 328), (1, 130, 768, 136), (0, 1, 4096, 4104),
+                                       (0, 512, 1024, 9480)])
+def test_linear_any_multiple_of_8_columns(sq, fmt, T, K, D):
+    """D % 8 == 0.  The last n-tile is ragged: W rows beyond D are zero-filled by TMA, columns beyond
+    D are neither stored nor touched (sentinel columns), in the split-K, persistent and CTA-pair variants."""
+    x, w, bias = si.activations(T, K, config=3, extra=D), si.weight(D, K, 3, extra=D + 1), si.beta(D, 3)
+    cfg = sq.make_config(fmt, sq.NORM_NONE, 1e-6, sq.LAYOUT_TILED)
+    wq, act = sq.quantize_weight(cfg, to_dev(w)), sq.prepare(cfg, to_dev(x))
+    big = torch.full((T, D + 24), 7.0, dtype=torch.float32, device="cuda")
+    sq.linear(cfg, act, wq, bias=to_dev(bias), Y=big[:, :D])
+    y16 = sq.linear(cfg, act, wq, bias=to_dev(bias), out_dtype="bf16")
+    torch.cuda.synchronize()
+    assert (big[:, D:] == 7.0).all(), "columns beyond D were written"
+    p, q = so.prepare(x, fmt=fmt, norm=0), so.quantize_weight(w, fmt=fmt)
+    assert rel_err(big[:, :D].cpu().numpy(), so.linear(p, q, bias_u16=bias)).max() <= TOL
+    assert torch.equal(y16, big[:, :D].to(torch.bfloat16))
+
+
+def test_outputs_are_repeatable_and_stay_inside_their_buffers(sq):
+    """compute-sanitizer is closed on this GPU pool, so the races / stray writes it would look for are hunted with what
+    can run here: every kernel variant 12 times on the same inputs must give bit-identical outputs (the split-K DSMEM
+    exchange, the multicast grouped clusters, the CTA pairs and the lagged prepare loop all order their sums), and
+    sentinel bytes around every output buffer must survive."""
+    def guarded(n, dtype=torch.uint8):
+        buf = torch.full((n + 512,), 0x5A if dtype == torch.uint8 else 7.0, dtype=dtype, device="cuda")
+        return buf, buf[256: 256 + n]
+    cases = [(1, 4096, 4096), (16, 14336, 4096), (130, 1024, 384), (256, 4096, 28672), (700, 9216, 512)]
+    cfg = sq.make_config(sq.NVFP4, sq.NORM_RMS, 1e-6, sq.LAYOUT_TILED)
+    for T, K, D in cases:
+        x, g, w = si.activations(T, K, config=2, extra=T), si.gamma(K, 2), si.weight(D, K, 2, extra=K)
+        wq = sq.quantize_weight(cfg, to_dev(w))
+        xd, gd = to_dev(x), to_dev(g)
+        n = sq.act_sizes(cfg, T, K)
+        first = None
+        for rep in range(12):
+            bufs = {k: guarded(sz) for k, sz in zip(("sp_codes", "sp_sf", "sp_meta", "dn_codes", "dn_sf"), n[:5])}
+            rs_full, rs = guarded(T, torch.float32)
+            act = dict({k: v[1] for k, v in bufs.items()}, row_scale=rs, T=T, K=K)
+            sq.capi.sharq_act_init(__import__("ctypes").byref(cfg), T, K, act["sp_sf"].data_ptr(), act["sp_meta"].data_ptr(),
+                                   act["dn_sf"].data_ptr(), torch.cuda.current_stream().cuda_stream)
+            sq.prepare(cfg, xd, gd, out=act)
+            y_full, y = guarded(T * D, torch.float32)
+            Y = y.view(T, D)
+            sq.linear(cfg, act, wq, Y=Y)
+            torch.cuda.synchronize()
+            for k, (full, view) in bufs.items():
+                assert (full[:256] == 0x5A).all() and (full[256 + view.numel():] == 0x5A).all(), f"{k} T{T} K{K}"
+            assert (rs_full[:256] == 7.0).all() and (rs_full[256 + T:] == 7.0).all()
+            assert (y_full[:256] == 7.0).all() and (y_full[256 + T * D:] == 7.0).all()
+            snap = [act[k].clone() for k in ("sp_codes", "sp_sf", "sp_meta", "dn_codes", "dn_sf")] + [Y.clone()]
+            if first is None:
+                first = snap
+            else:
+                for a, b in zip(first, snap):
+                    assert torch.equal(a, b), f"run {rep} differs (T{T} K{K} D{D})"
