@@ -493,6 +493,11 @@ def decode_extras(sq, wl0, pk, steps, rank):
             ms = timed(reps, max(steps, 12), 3, lambda: None)
             w_mb = K * D * (0.5 + 1 / 32 + 1 / 16) / 1e6
             out["layers"][f"{n}_T{T}"] = dict(us=round(ms * 1e3, 2), weights="cold" if 3 * w_mb > 126 else "partly L2-resident")
+            if T <= 8:   # the same layer as ONE fused launch (sharq_prepare_linear single_launch = 1)
+                reps1, _ = replays_of([lambda r=r, T=T, n=n, K=K, norm=norm: sq.prepare_linear(
+                    wl.cfg[n], wl.x[T, n], wl.wq[r][n], wl.gamma[K] if norm else None, act=wl.act[T, n], Y=wl.Y[T, n],
+                    single_launch=True) for r in range(wl.n_sets)])
+                out["layers"][f"{n}_T{T}"]["single_launch_us"] = round(timed(reps1, max(steps, 12), 3, lambda: None) * 1e3, 2)
     del wl
     torch.cuda.empty_cache()
     return out

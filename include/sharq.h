@@ -8,7 +8,8 @@
  *   sharq_linear           sparse + dense block-scaled FP4 GEMMs into one accumulator, bf16 epilogue
  * plus sharq_linear_grouped (the same over the row ranges of E experts, MoE), sharq_prepare_add
  * (sharq_prepare with the residual-stream add fused in front of the norm), sharq_prepare_swiglu (with
- * SiLU(gate) * up fused in front of it), host-only size / plan queries
+ * SiLU(gate) * up fused in front of it), sharq_prepare_linear (both calls as one, a single launch for decode
+ * shapes), host-only size / plan queries
  * (sharq_weight_sizes, sharq_act_sizes, sharq_linear_workspace, sharq_linear_plan), sharq_act_init, the Table 5
  * path combinations (sharq_act_sizes_paths, sharq_prepare_paths, sharq_linear_paths) and the test
  * helpers sharq_untile_sf / sharq_untile_meta.  The tensor-pipe probe lives in sharq_diag.h.
@@ -183,6 +184,27 @@ sharq_status sharq_linear(const sharq_config* cfg, int64_t T, int64_t D, int64_t
                           const void* w_sf_dense_view, const float* w_tensor_scale,
                           const void* bias, void* Y, int64_t ldy, int32_t out_dtype, int32_t path,
                           void* workspace, size_t workspace_bytes, void* stream);
+
+/* ---- sharq_prepare_linear (decode is where the method's gain shows) ----------------
+ * sharq_prepare followed by sharq_linear (path 0) as ONE call with the arguments of both; the activation buffers
+ * (sp_codes ... row_scale) are still the caller's and hold sharq_prepare's outputs afterwards.
+ * single_launch = 0 (recommended): the two kernels, chained by programmatic dependent launch -- the preparation runs
+ *   while the GEMM's CTAs are scheduled, set up their barriers / tensor memory and fill their weight ring.
+ * single_launch = 1: for T <= 8 rows, K <= 16384, NVFP4 / MXFP4, TILED layout, norm NONE / RMS and a 32-byte aligned
+ *   x with ldx % 16 == 0, ONE launch: every CTA of the GEMM prepares the T rows itself with extra warps while its
+ *   producer warp streams the weights (no cross-CTA wait).  Measured 4-6 us per layer SLOWER than the chained pair
+ *   on B200: a fused launch cannot start its 1.6 us prologue before the previous launch's CTAs leave
+ *   the SMs, the chained pair hides exactly that behind the preparation.  Kept as the measured alternative; other
+ *   shapes fall back to the two launches.
+ * Results are bit-identical to the two calls either way. */
+sharq_status sharq_prepare_linear(const sharq_config* cfg, const void* x, int64_t T, int64_t K, int64_t ldx,
+                                  const void* gamma, const void* beta, const float* x_tensor_scale,
+                                  void* sp_codes, void* sp_sf, void* sp_meta, void* dn_codes, void* dn_sf,
+                                  float* row_scale, int64_t D, const void* w_codes,
+                                  const void* w_sf_sparse_view, const void* w_sf_dense_view,
+                                  const float* w_tensor_scale, const void* bias, void* Y, int64_t ldy,
+                                  int32_t out_dtype, int32_t single_launch, void* workspace,
+                                  size_t workspace_bytes, void* stream);
 
 /* ---- sharq_linear_grouped (MoE expert linears) -----------------------------
  * E experts (E <= 1024); `offsets` is a DEVICE int32[E+1] array (e.g. the router's output, no host copy and no

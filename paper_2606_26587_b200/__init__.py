@@ -61,6 +61,8 @@ def _load() -> ctypes.CDLL:
     lib.sharq_prepare_swiglu.argtypes = [CFG, P, P, c_int64, c_int64, c_int64, c_int64, P, P, P, P, P, P, P, P, P, P]
     lib.sharq_linear.argtypes = [CFG, c_int64, c_int64, c_int64, P, P, P, P, P, P, P, P, P, P, P, P, c_int64,
                                  c_int32, c_int32, P, c_size_t, P]
+    lib.sharq_prepare_linear.argtypes = [CFG, P, c_int64, c_int64, c_int64, P, P, P, P, P, P, P, P, P, c_int64, P, P, P, P, P,
+                                         P, c_int64, c_int32, c_int32, P, c_size_t, P]
     lib.sharq_linear_grouped.argtypes = [CFG, c_int32, P, c_int64, c_int64, c_int64, P, P, P, P, P, P, P, P,
                                          P, P, P, c_int64, c_int32, P, c_size_t, P]
     lib.sharq_act_init.argtypes = [CFG, c_int64, c_int64, P, P, P, P]
@@ -79,7 +81,7 @@ def _load() -> ctypes.CDLL:
 
 # every symbol include/sharq.h declares, then include/sharq_diag.h's
 EXPORTS = ("sharq_version", "sharq_weight_sizes", "sharq_act_sizes", "sharq_linear_workspace",
-           "sharq_quantize_weight", "sharq_prepare", "sharq_prepare_add", "sharq_prepare_swiglu", "sharq_linear", "sharq_linear_grouped",
+           "sharq_quantize_weight", "sharq_prepare", "sharq_prepare_add", "sharq_prepare_swiglu", "sharq_prepare_linear", "sharq_linear", "sharq_linear_grouped",
            "sharq_act_init", "sharq_linear_plan", "sharq_untile_sf", "sharq_untile_meta", "sharq_act_sizes_paths",
            "sharq_prepare_paths", "sharq_linear_paths", "sharq_mma_peak_launch")
 capi = _load()
@@ -284,6 +286,26 @@ def linear(cfg: Config, act: dict, wq: dict, bias=None, out_dtype="bf16", path=P
                              _ptr(Y), Y.stride(0), 0 if Y.dtype == torch.bfloat16 else 1, path, _ptr(workspace), n_ws,
                              _stream()), "sharq_linear")
     return Y
+
+
+def prepare_linear(cfg: Config, x, wq: dict, gamma=None, beta=None, x_tensor_scale=None, bias=None, out_dtype="bf16",
+                   act=None, Y=None, single_launch=False):
+    """sharq_prepare_linear: prepare + linear as one call; single_launch=True asks for the fused launch (T <= 8, see
+    sharq.h: measured slower than the chained pair).  Returns (Y, act)."""
+    import torch
+    T, K = x.shape
+    D = wq["D"]
+    if act is None:
+        act = alloc_act(cfg, T, K, x.device)
+    if Y is None:
+        Y = torch.empty((T, D), dtype=torch.bfloat16 if out_dtype == "bf16" else torch.float32, device=x.device)
+    _check(capi.sharq_prepare_linear(ctypes.byref(cfg), _ptr(x), T, K, x.stride(0), _ptr(gamma), _ptr(beta),
+                                     _ptr(x_tensor_scale), _ptr(act["sp_codes"]), _ptr(act["sp_sf"]), _ptr(act["sp_meta"]),
+                                     _ptr(act["dn_codes"]), _ptr(act["dn_sf"]), _ptr(act["row_scale"]), D, _ptr(wq["codes"]),
+                                     _ptr(wq["sf_sp"]), _ptr(wq["sf_dn"]), _ptr(wq["ts_w"]), _ptr(bias), _ptr(Y), Y.stride(0),
+                                     0 if Y.dtype == torch.bfloat16 else 1, 1 if single_launch else 0, None, 0, _stream()),
+           "sharq_prepare_linear")
+    return Y, act
 
 
 def linear_grouped(cfg: Config, offsets, act: dict, wq: dict, D: int, out_dtype="bf16", Y=None, workspace=None):

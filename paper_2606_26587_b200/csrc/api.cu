@@ -5,6 +5,7 @@
 
 #include "common.cuh"
 #include "linear_args.h"
+#include "prepare_device.cuh"
 
 namespace sharq {
 cudaError_t launch_prepare(const sharq_config* cfg, const void* x, int64_t T, int64_t K, int64_t ldx,
@@ -17,7 +18,10 @@ cudaError_t launch_quantize_weight(const sharq_config* cfg, const void* W, int64
                                    cudaStream_t st);
 sharq_status launch_linear(const sharq_config* cfg, const LinearArgs& a, int32_t E, const int32_t* offsets,
                            void* workspace, size_t workspace_bytes, int num_sms, int dev, cudaStream_t st,
-                           LinearPlan* plan_only);
+                           LinearPlan* plan_only, const FusedArgs* fz = nullptr);
+PrepParams make_prep_params(const sharq_config* cfg, const void* x, int64_t T, int64_t K, int64_t ldx, const void* gamma,
+                            const void* beta, const float* x_ts, void* sp_codes, void* sp_sf, void* sp_meta,
+                            void* dn_codes, void* dn_sf, float* row_scale);
 cudaError_t launch_untile(const void* tiled, int64_t R, int64_t C, void* canonical, int meta, cudaStream_t st);
 size_t linear_workspace_bytes(const sharq_config* cfg, int64_t T, int64_t D, int64_t K, int32_t E);
 }  // namespace sharq
@@ -229,6 +233,48 @@ sharq_status sharq_linear(const sharq_config* cfg, int64_t T, int64_t D, int64_t
   return launch_linear(cfg, a, 0, nullptr, workspace, workspace_bytes, di.sms, di.dev, (cudaStream_t)stream, nullptr);
 }
 
+// ---- sharq_prepare_linear --------------------------------------------------------------
+sharq_status sharq_prepare_linear(const sharq_config* cfg, const void* x, int64_t T, int64_t K, int64_t ldx,
+                                  const void* gamma, const void* beta, const float* x_tensor_scale, void* sp_codes,
+                                  void* sp_sf, void* sp_meta, void* dn_codes, void* dn_sf, float* row_scale, int64_t D,
+                                  const void* w_codes, const void* w_sf_sparse_view, const void* w_sf_dense_view,
+                                  const float* w_tensor_scale, const void* bias, void* Y, int64_t ldy, int32_t out_dtype,
+                                  int32_t single_launch, void* workspace, size_t workspace_bytes, void* stream) {
+  // single_launch = 0: the two calls it stands for, chained by programmatic dependent launch (measured faster: the
+  // prepare kernel runs while the GEMM's CTAs are being scheduled and fill their weight ring); 1: one fused launch
+  // when the shape allows it
+  sharq_status s = check_cfg(cfg);
+  if (s != SHARQ_OK) return s;
+  if (single_launch < 0 || single_launch > 1) return SHARQ_EINVAL;
+  const bool fusable = single_launch == 1 && cfg->fmt != SHARQ_HIF4 && cfg->mask == SHARQ_MASK_PAIR48 && cfg->layout == SHARQ_LAYOUT_TILED &&
+                       cfg->norm != SHARQ_NORM_LAYER && T >= 1 && T <= 8 && K > 0 && K % 256 == 0 && K <= 16384 &&
+                       ldx >= K && ldx % 16 == 0 && x && ((uintptr_t)x & 31u) == 0;
+  if (!fusable) {
+    s = sharq_prepare(cfg, x, T, K, ldx, gamma, beta, x_tensor_scale, sp_codes, sp_sf, sp_meta, dn_codes, dn_sf, row_scale,
+                      stream);
+    if (s != SHARQ_OK) return s;
+    return sharq_linear(cfg, T, D, K, sp_codes, sp_sf, sp_meta, dn_codes, dn_sf, row_scale, w_codes, w_sf_sparse_view,
+                        w_sf_dense_view, w_tensor_scale, bias, Y, ldy, out_dtype, 0, workspace, workspace_bytes, stream);
+  }
+  // the argument checks of the two calls
+  if (!sp_codes || !sp_sf || !sp_meta || !dn_codes || !dn_sf || !row_scale) return SHARQ_EINVAL;
+  if (cfg->norm != SHARQ_NORM_NONE && !gamma) return SHARQ_EINVAL;
+  if (!aligned16(sp_codes) || !aligned16(sp_sf) || !aligned16(sp_meta) || !aligned16(dn_codes) || !aligned16(dn_sf) ||
+      (gamma && !aligned16(gamma)))
+    return SHARQ_EINVAL;
+  const void* ptrs[] = {sp_codes, sp_sf, sp_meta, dn_codes, dn_sf, w_codes, w_sf_sparse_view, w_sf_dense_view, Y};
+  if ((s = check_linear(cfg, D, K, ptrs, 9, ldy, out_dtype, 0)) != SHARQ_OK) return s;
+  if (!w_tensor_scale) return SHARQ_EINVAL;
+  DeviceInfo di{};
+  if ((s = device_info(&di)) != SHARQ_OK) return s;
+  const PrepParams pp = make_prep_params(cfg, x, T, K, ldx, gamma, beta, x_tensor_scale, sp_codes, sp_sf, sp_meta, dn_codes,
+                                         dn_sf, row_scale);
+  const FusedArgs fz{&pp, cfg->norm, (int32_t)((K + 1023) / 1024)};
+  LinearArgs a{T, D, K, sp_codes, sp_sf, sp_meta, dn_codes, dn_sf, nullptr, row_scale, w_codes, w_sf_sparse_view,
+               w_sf_dense_view, w_tensor_scale, bias, Y, ldy, out_dtype, 0};
+  return launch_linear(cfg, a, 0, nullptr, workspace, workspace_bytes, di.sms, di.dev, (cudaStream_t)stream, nullptr, &fz);
+}
+
 // ---- Table 5 path combinations --------------------------------------------------------------
 static bool combo_ok(const sharq_config* cfg, int32_t path) {
   return (path == 3 || path == 4) && cfg->fmt != SHARQ_HIF4 && cfg->mask == SHARQ_MASK_PAIR48;
@@ -329,7 +375,7 @@ sharq_status sharq_linear_plan(const sharq_config* cfg, int64_t T, int64_t D, in
     s = launch_linear(cfg, a, E, nullptr, nullptr, 0, di.sms, di.dev, nullptr, &pl);
     if (s != SHARQ_OK) return s;
   }
-  static const char* const kinds[] = {"tile", "pair", "grouped-mc", "hif4-bf16"};
+  static const char* const kinds[] = {"tile", "pair", "grouped-mc", "hif4-bf16", "tile+prepare"};
   if (pl.kind < 0) snprintf(buf, n, "none");
   else snprintf(buf, n, "%s bn=%d act_rows=%d splits=%d stages=%d tiles=%lld grid=%lld cluster=%d", kinds[pl.kind],
                 pl.bn, pl.act_rows, pl.splits, pl.stages, (long long)pl.tiles, (long long)pl.grid, pl.cluster);

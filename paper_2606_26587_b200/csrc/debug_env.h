@@ -19,11 +19,12 @@ struct DebugEnv {
   int row_per_sm;      // SHARQ_DEBUG_ROW_PER_SM: prepare grid = this many CTAs per SM (0 = default)
   int old_prepare;     // SHARQ_DEBUG_OLD_PREPARE: warp-per-row prepare kernel for every K
   int pair_gm;         // SHARQ_DEBUG_PAIR_GM: supertile height of the pair GEMM in 256-row blocks (0 = by L2 footprint)
+  int skip_prep;       // SHARQ_DEBUG_SKIP_PREP: fused decode launch without its in-kernel prepare (timing experiment)
   int prep_chunk_rows; // SHARQ_DEBUG_PREP_CHUNK_ROWS: rows per launch of the row-per-CTA prepare kernel (tests; 0 = 2^31 / width)
 };
 
 #ifndef SHARQ_EXPERIMENTS
-constexpr DebugEnv kNoDebug{0, 0, 0, 0, 0, 0, 0, 128, 0, 0, 0, 0, 0};
+constexpr DebugEnv kNoDebug{0, 0, 0, 0, 0, 0, 0, 128, 0, 0, 0, 0, 0, 0};
 inline constexpr const DebugEnv& debug_env() { return kNoDebug; }
 #else
 inline const DebugEnv& debug_env() {
@@ -46,6 +47,7 @@ inline const DebugEnv& debug_env() {
     d.row_per_sm = num("SHARQ_DEBUG_ROW_PER_SM", 0);
     d.old_prepare = flag("SHARQ_DEBUG_OLD_PREPARE");
     d.pair_gm = num("SHARQ_DEBUG_PAIR_GM", 0);
+    d.skip_prep = flag("SHARQ_DEBUG_SKIP_PREP");
     d.prep_chunk_rows = num("SHARQ_DEBUG_PREP_CHUNK_ROWS", 0);
     return d;
   }();

@@ -22,6 +22,7 @@
 #include "common.cuh"
 #include "debug_env.h"
 #include "linear_args.h"
+#include "prepare_device.cuh"
 #include "tc_ptx.cuh"
 
 namespace sharq {
@@ -79,7 +80,12 @@ struct KParams {
 // and a smaller reservation leaves room for more ring stages, i.e. more weight bytes in flight per SM (the
 // decode shapes are bound by exactly that).  The MMA still reads 128 rows; rows beyond the loaded ones are
 // whatever follows in shared memory and only reach accumulator rows that are never stored.
-template <int BN, int FMT, bool SPLIT, int AR>
+// sharq_prepare_linear (N2): shared memory of the in-kernel sharq_prepare rows (prepare_rows' layout for up to 16
+// warps with gamma staged) and the widest row the fused kernel takes
+constexpr int kPrepWarpsMax = 16;                 // K <= 16384
+constexpr int kPrepSmem = kPrepWarpsMax * 1024 + 256 + 16 + 64 + kPrepWarpsMax * 32 * 64 + 128;
+
+template <int BN, int FMT, bool SPLIT, int AR, int EXTRA = 0>
 struct Stage {
   static constexpr int NB = (BN + 127) / 128;                         // 128-row scale atoms of W per tile
   static constexpr int SF_DN_BYTES = (FMT == SHARQ_NVFP4) ? 2048 : 1024;  // per 128 rows per k-block
@@ -99,9 +105,9 @@ struct Stage {
   static constexpr int RECV = SPLIT ? (NSL + 2) * AR * 64 : 0;        // [src][slot][AR rows][16 fp32]; S*ceil(NSL/S) <= NSL+2 for S in {2,3,4,8}
   static constexpr int PAD = AR < 128 ? 128 * 128 : 0;               // the MMA's over-read behind the last stage
   static constexpr int GRP = (!SPLIT && AR == 128 && BN == 128) ? 2 * (kMaxExperts + 1) * 4 + 8 : 0;   // expert table (grouped)
-  static constexpr int FIT = (232448 - 1024 - 256 - RECV - PAD - GRP) / BYTES;
+  static constexpr int FIT = (232448 - 1024 - 256 - RECV - PAD - GRP - EXTRA) / BYTES;
   static constexpr int STAGES = FIT > 8 ? 8 : FIT;
-  static constexpr int SMEM = STAGES * BYTES + PAD + RECV + 1024 /*alignment slack*/ + 256 /*barriers*/ + GRP;
+  static constexpr int SMEM = STAGES * BYTES + PAD + RECV + 1024 /*alignment slack*/ + 256 /*barriers*/ + GRP + EXTRA;
   // tensor-memory columns: two accumulator stages, then metadata and scale factors
   static constexpr int SFB_COLS = NB * 4;          // columns one MMA's B scales occupy
   static constexpr int ACC_STAGES = BN > 128 ? 1 : 2;
@@ -177,12 +183,21 @@ __device__ __forceinline__ void store_row(const KParams& p, int64_t row, int col
 // MC = true (grouped GEMM): a cluster of two CTAs works on two neighbouring n-tiles of the same 128-row block in
 // lock step; each CTA fetches half of the shared activation operands and multicasts them to both (the many
 // short tiles of the expert GEMMs are bound by L2 -> SM traffic, 60 % of which is the activation side).
-template <int BN, int FMT, bool SPLIT, int AR, bool MC = false>
-__global__ void __launch_bounds__(kThreads, 1)
+//
+// FUSED = true (sharq_prepare_linear, SURVEY.md 8(f) N2, T <= 8): warps 6 .. of EVERY CTA run sharq_prepare for all T
+// rows (prepare_rows on named barrier 2: the row-per-CTA kernel's body, one warp per 1024 elements of a row) while
+// warp 0 already streams the weights.  Every CTA prepares the rows itself: no cross-CTA wait (an earlier version
+// released the producers through a device-scope counter and lost 4-6 us waiting for the last CTA to be scheduled).
+// The prepared operands go to the caller's activation buffers in global memory -- all CTAs write the same bytes --
+// and come back through the same TMA loads as in the two-launch path, after this CTA's own stores are fenced
+// (__threadfence + fence.proxy.async) and its `act_bar` mbarrier has completed.
+template <int BN, int FMT, bool SPLIT, int AR, bool MC = false, bool FUSED = false>
+__global__ void __launch_bounds__(FUSED ? kThreads + 32 * kPrepWarpsMax : kThreads, 1)
 sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_constant__ CUtensorMap tm_a_dn,
                     const __grid_constant__ CUtensorMap tm_w, const __grid_constant__ CUtensorMap tm_alt,
-                    const KParams p) {
-  using S = Stage<BN, FMT, SPLIT, AR>;
+                    const KParams p, const PrepParams pp, const int prep_norm) {
+  using S = Stage<BN, FMT, SPLIT, AR, FUSED ? kPrepSmem : 0>;
+  static_assert(!(FUSED && MC), "the fused kernel is for single-problem launches");
   constexpr bool NV = (FMT == SHARQ_NVFP4);
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
@@ -193,7 +208,9 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
   auto tmem_full_bar = [&](int a) { return bars + 8u * (2 * S::STAGES + a); };
   auto tmem_empty_bar = [&](int a) { return bars + 8u * (2 * S::STAGES + 2 + a); };
   const uint32_t tmem_ptr_smem = bars + 8u * (2 * S::STAGES + 4);
+  const uint32_t act_bar = bars + 8u * (2 * S::STAGES + 5);          // FUSED: this CTA's prepared operands are in memory
   int32_t* grp_tab = reinterpret_cast<int32_t*>(smem_raw + (bars + 256u - smem_u32(smem_raw)));   // offs[E+1], pref[E+1]
+  uint8_t* prep_smem = smem_raw + (bars + 256u + (uint32_t)S::GRP - smem_u32(smem_raw));          // FUSED: prepare_rows' scratch
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   if (warp == 0) SHARQ_TS(0);
@@ -221,6 +238,7 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
       tc::mbar_init(tmem_full_bar(a), 1);
       tc::mbar_init(tmem_empty_bar(a), 4);          // one arrival per epilogue warp
     }
+    if constexpr (FUSED) tc::mbar_init(act_bar, 1);
     tc::fence_mbar_init();
   }
   if (warp == 2) tc::tmem_alloc<kTmemCols>(tmem_ptr_smem);
@@ -354,6 +372,10 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
           }
           SHARQ_TS(2);
           tc::grid_dependency_wait();
+          if constexpr (FUSED) {                         // the rows prepared by this CTA's own warps 6 .. are in memory
+            tc::mbar_wait(act_bar, 0);
+            asm volatile("fence.proxy.async;" ::: "memory");
+          }
           SHARQ_TS(3);
           dep_synced = true;
           for (int i = 0; i < n_early; ++i) load_a(kb + i, smem_base + i * S::BYTES, full_bar(i));
@@ -445,9 +467,10 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
         if (lead) tc::tc_commit(tmem_full_bar(as));                // accumulator complete
       }
     }
-  } else {
+  } else if (warp < 6) {
     // =========================== epilogue ====================================================
     tc::grid_dependency_wait();                          // row_scale is sharq_prepare's; Y may still be read
+    if constexpr (FUSED) tc::mbar_wait(act_bar, 0);      // ... here: this launch's own prepare warps write it
     const int sub = warp & 3;                            // TMEM sub-partition this warp may read
     const int r_local = sub * 32 + lane;
     const uint32_t lane_addr = tmem_base + ((uint32_t)(sub * 32) << 16);
@@ -458,7 +481,7 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
         const uint32_t as = n_unit % S::ACC_STAGES;
         const int64_t row = (int64_t)u.m_blk * BM + r_local;
         const bool row_ok = r_local < u.rows_valid;
-        const float scale = row_ok ? __fmul_rn(p.row_scale[row], p.w_ts[u.expert]) : 0.0f;
+        const float scale = row_ok ? __fmul_rn(FUSED ? __ldcg(p.row_scale + row) : p.row_scale[row], p.w_ts[u.expert]) : 0.0f;
         tc::mbar_wait(tmem_full_bar(as), (n_unit / S::ACC_STAGES) & 1u);
         tc::tc_fence_after();
 #pragma unroll 1
@@ -483,7 +506,10 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
       const bool row_ok = r_local < u.rows_valid;
       const int slots = (BN / 16 + splits - 1) / splits;
       // the output scale of this thread's row, fetched while the main loop runs (used after the exchange)
-      if (row_ok) split_scale = __fmul_rn(p.row_scale[(int64_t)u.m_blk * BM + r_local], p.w_ts[u.expert]);
+      if (row_ok) {
+        const float* rs = p.row_scale + (int64_t)u.m_blk * BM + r_local;
+        split_scale = __fmul_rn(FUSED ? __ldcg(rs) : *rs, p.w_ts[u.expert]);
+      }
       tc::mbar_wait(tmem_full_bar(0), 0);
       if (warp == 2) SHARQ_TS(6);
       tc::tc_fence_after();
@@ -520,13 +546,27 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
       }
       tc::tc_fence_before();
     }
+  } else {
+    // =========================== in-kernel sharq_prepare (FUSED only: warps 6 ..) ==================
+    if constexpr (FUSED) {
+      tc::grid_dependency_wait();                        // x belongs to the kernels before this one
+      const int ptid = (int)threadIdx.x - kThreads, pthreads = (int)blockDim.x - kThreads;
+      if (prep_norm == SHARQ_NORM_RMS) prepare_rows<FMT, SHARQ_NORM_RMS, 2, false>(pp, prep_smem, ptid, pthreads, 0, 1);
+#ifdef SHARQ_EXPERIMENTS
+      else if (prep_norm == 99) { }                      // timing experiment: no in-kernel prepare at all
+#endif
+      else prepare_rows<FMT, SHARQ_NORM_NONE, 2, false>(pp, prep_smem, ptid, pthreads, 0, 1);
+      __threadfence();                                   // every thread's stores, device scope
+      named_bar_sync<2>(pthreads);
+      if (ptid == 0) tc::mbar_arrive(act_bar);
+    }
   }
   if constexpr (SPLIT) {
     __syncwarp();
     if (warp == 2) SHARQ_TS(7);
     tc::cluster_sync_all();                              // partial slices have landed in their owners
     if (warp == 2) SHARQ_TS(8);
-    if (warp >= 2) {
+    if (warp >= 2 && warp < 6) {
       const Unit u = decode_unit(p, g, m_blocks, total_tiles, tile0, rank, splits);
       const int r_local = (warp & 3) * 32 + lane;
       if (r_local < u.rows_valid) {
@@ -911,7 +951,7 @@ int choose_splits(int64_t tiles, int num_kb, int num_sms, int dev) {
   return 1;
 }
 
-struct LaunchEnv { int num_sms; int dev; cudaStream_t st; LinearPlan* plan_only; };
+struct LaunchEnv { int num_sms; int dev; cudaStream_t st; LinearPlan* plan_only; const FusedArgs* fz; };
 
 inline void fill_plan(LinearPlan* pl, int kind, int bn, int ar, int splits, int stages, int64_t tiles, int64_t grid,
                       int cluster) {
@@ -919,12 +959,14 @@ inline void fill_plan(LinearPlan* pl, int kind, int bn, int ar, int splits, int 
   pl->grid = grid; pl->cluster = cluster;
 }
 
-template <int BN, int FMT, int AR>
-sharq_status launch_1cta(const LinearArgs& a, const KParams& p, const CUtensorMap& tm_sp,
-                         const CUtensorMap& tm_dn, const CUtensorMap& tm_w, const CUtensorMap& tm_alt, int64_t tiles,
-                         const LaunchEnv& env) {
+template <int BN, int FMT, int AR, bool FUSED>
+sharq_status launch_1cta_impl(const LinearArgs& a, const KParams& p, const CUtensorMap& tm_sp,
+                              const CUtensorMap& tm_dn, const CUtensorMap& tm_w, const CUtensorMap& tm_alt, int64_t tiles,
+                              const LaunchEnv& env) {
   constexpr bool kSplitFits = !(BN == 256 && AR == 128);   // no room for the exchange buffers; never needed there
+  constexpr int kExtra = FUSED ? kPrepSmem : 0;
   int splits = 1;
+  // (the fused kernel takes the cluster size the plain kernel would: one CTA per SM either way)
   if constexpr (kSplitFits) if (p.E == 0 && p.path < 3) splits = choose_splits<BN, FMT, AR>(tiles, (int)(a.K / BK), env.num_sms, env.dev);
   cudaLaunchConfig_t lc{};
   cudaLaunchAttribute attr[2];
@@ -932,12 +974,15 @@ sharq_status launch_1cta(const LinearArgs& a, const KParams& p, const CUtensorMa
   attr[0].val.programmaticStreamSerializationAllowed = debug_env().no_pdl ? 0 : 1;
   lc.attrs = attr;
   lc.numAttrs = 1;
-  lc.blockDim = dim3(kThreads);
+  lc.blockDim = dim3(FUSED ? kThreads + 32 * env.fz->warps : kThreads);
   lc.stream = env.st;
+  PrepParams pp{};
+  int norm = 0;
+  if constexpr (FUSED) { pp = *env.fz->pp; norm = env.fz->norm; if (debug_env().skip_prep) norm = 99; }
   if constexpr (kSplitFits) if (splits > 1) {
-    using S = Stage<BN, FMT, true, AR>;
-    auto kfn = sharq_linear_kernel<BN, FMT, true, AR>;
-    if (env.plan_only) { fill_plan(env.plan_only, 0, BN, AR, splits, S::STAGES, tiles, tiles * splits, splits); return SHARQ_OK; }
+    using S = Stage<BN, FMT, true, AR, kExtra>;
+    auto kfn = sharq_linear_kernel<BN, FMT, true, AR, false, FUSED>;
+    if (env.plan_only) { fill_plan(env.plan_only, FUSED ? 4 : 0, BN, AR, splits, S::STAGES, tiles, tiles * splits, splits); return SHARQ_OK; }
     static std::atomic<uint64_t> smem_set{0};
     if (set_smem_once(smem_set, (const void*)kfn, S::SMEM, env.dev) != cudaSuccess) return SHARQ_ECUDA;
     lc.gridDim = dim3((unsigned)(tiles * splits));
@@ -947,18 +992,28 @@ sharq_status launch_1cta(const LinearArgs& a, const KParams& p, const CUtensorMa
     attr[1].val.clusterDim.y = 1;
     attr[1].val.clusterDim.z = 1;
     lc.numAttrs = 2;
-    return cudaLaunchKernelEx(&lc, kfn, tm_sp, tm_dn, tm_w, tm_alt, p) == cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
+    return cudaLaunchKernelEx(&lc, kfn, tm_sp, tm_dn, tm_w, tm_alt, p, pp, norm) == cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
   }
-  using S = Stage<BN, FMT, false, AR>;
-  auto kfn = sharq_linear_kernel<BN, FMT, false, AR>;
+  using S = Stage<BN, FMT, false, AR, kExtra>;
+  auto kfn = sharq_linear_kernel<BN, FMT, false, AR, false, FUSED>;
   int64_t grid = tiles < env.num_sms ? tiles : env.num_sms;      // persistent: one CTA per SM
   if (debug_env().grid > 0) grid = debug_env().grid;
-  if (env.plan_only) { fill_plan(env.plan_only, 0, BN, AR, 1, S::STAGES, tiles, grid, 1); return SHARQ_OK; }
+  if (env.plan_only) { fill_plan(env.plan_only, FUSED ? 4 : 0, BN, AR, 1, S::STAGES, tiles, grid, 1); return SHARQ_OK; }
   static std::atomic<uint64_t> smem_set{0};
   if (set_smem_once(smem_set, (const void*)kfn, S::SMEM, env.dev) != cudaSuccess) return SHARQ_ECUDA;
   lc.gridDim = dim3((unsigned)grid);
   lc.dynamicSmemBytes = S::SMEM;
-  return cudaLaunchKernelEx(&lc, kfn, tm_sp, tm_dn, tm_w, tm_alt, p) == cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
+  return cudaLaunchKernelEx(&lc, kfn, tm_sp, tm_dn, tm_w, tm_alt, p, pp, norm) == cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
+}
+
+template <int BN, int FMT, int AR>
+sharq_status launch_1cta(const LinearArgs& a, const KParams& p, const CUtensorMap& tm_sp,
+                         const CUtensorMap& tm_dn, const CUtensorMap& tm_w, const CUtensorMap& tm_alt, int64_t tiles,
+                         const LaunchEnv& env) {
+  if constexpr (AR == 16) {                                // the fused decode launch exists for T <= 8 (8-row boxes) only
+    if (env.fz) return launch_1cta_impl<BN, FMT, AR, true>(a, p, tm_sp, tm_dn, tm_w, tm_alt, tiles, env);
+  }
+  return launch_1cta_impl<BN, FMT, AR, false>(a, p, tm_sp, tm_dn, tm_w, tm_alt, tiles, env);
 }
 
 // grouped GEMM: persistent clusters of two CTAs on neighbouring n-tiles, activation operands multicast
@@ -985,7 +1040,7 @@ sharq_status launch_mc(const KParams& p, const CUtensorMap& tm_sp, const CUtenso
   lc.gridDim = dim3((unsigned)(2 * clusters));
   lc.dynamicSmemBytes = S::SMEM;
   lc.stream = env.st;
-  return cudaLaunchKernelEx(&lc, kfn, tm_sp, tm_dn, tm_w, tm_sp, p) == cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
+  return cudaLaunchKernelEx(&lc, kfn, tm_sp, tm_dn, tm_w, tm_sp, p, PrepParams{}, 0) == cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
 }
 
 // scale-factor / metadata array as a 2-D tensor of 1024-byte rows (256 x u32), boxes of `box_rows` rows
@@ -1117,7 +1172,7 @@ size_t linear_workspace_bytes(const sharq_config* cfg, int64_t T, int64_t D, int
 // plan_only != nullptr: fill it with the launch configuration this call would use and launch nothing.
 sharq_status launch_linear(const sharq_config* cfg, const LinearArgs& a, int32_t E, const int32_t* offsets,
                            void* workspace, size_t workspace_bytes, int num_sms, int dev, cudaStream_t st,
-                           LinearPlan* plan_only) {
+                           LinearPlan* plan_only, const FusedArgs* fz) {
   if (cfg->fmt == SHARQ_HIF4) {                           // no FP4-rate tensor path: exact bf16 emulation
     if (E > 0) return SHARQ_EINVAL;
     if (plan_only) {
@@ -1129,7 +1184,7 @@ sharq_status launch_linear(const sharq_config* cfg, const LinearArgs& a, int32_t
     return launch_linear_hif4(a, workspace, workspace_bytes, num_sms, st);
   }
   if (a.K > (int64_t)1 << 24 || a.D > (int64_t)1 << 24 || a.T > (int64_t)1 << 30) return SHARQ_ESHAPE;
-  const LaunchEnv env{num_sms, dev, st, plan_only};
+  const LaunchEnv env{num_sms, dev, st, plan_only, fz};
   int64_t rows_total = a.T, m_blocks = (a.T + BM - 1) / BM;
   if (E > 0) {
     if (E > kMaxExperts) return SHARQ_ESHAPE;

@@ -15,6 +15,14 @@ struct LinearArgs {
   void* Y; int64_t ldy; int out_dtype; int path;
 };
 
+// sharq_prepare_linear (N2): the in-kernel prepare of the fused decode launch; nullptr = plain sharq_linear
+struct PrepParams;
+struct FusedArgs {
+  const PrepParams* pp;
+  int32_t norm;        // SHARQ_NORM_NONE or SHARQ_NORM_RMS
+  int32_t warps;       // prepare warps per CTA = ceil(K / 1024)
+};
+
 // what a sharq_linear call launches (sharq_linear_plan): kind 0 = 128-row tiles, one CTA per tile (persistent, or a
 // split-K cluster of `splits` CTAs per tile); 1 = CTA-pair tiles (256 rows x bn); 2 = grouped GEMM, multicast
 // clusters of two CTAs; 3 = HiF4 bf16 emulation

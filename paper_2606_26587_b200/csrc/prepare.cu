@@ -283,23 +283,34 @@ static cudaError_t launch_norm(int norm, const PrepParams& p, dim3 grid, dim3 bl
 #undef SHARQ_LAUNCH
 }
 
-// Host launcher, called by the C ABI in api.cu after argument validation.
-cudaError_t launch_prepare(const sharq_config* cfg, const void* x, int64_t T, int64_t K, int64_t ldx,
-                           const void* gamma, const void* beta, const float* x_ts, void* sp_codes, void* sp_sf,
-                           void* sp_meta, void* dn_codes, void* dn_sf, float* row_scale, int num_sms,
-                           cudaStream_t st, const void* residual, int64_t ldr, void* sum_out, int64_t ldo,
-                           int combo, void* dn_meta) {
+// Kernel parameters of a plain sharq_prepare (also used by sharq_prepare_linear's in-kernel rows, linear.cu)
+PrepParams make_prep_params(const sharq_config* cfg, const void* x, int64_t T, int64_t K, int64_t ldx, const void* gamma,
+                            const void* beta, const float* x_ts, void* sp_codes, void* sp_sf, void* sp_meta,
+                            void* dn_codes, void* dn_sf, float* row_scale) {
   PrepParams p;
-  p.combo = combo; p.dn_meta = (uint8_t*)dn_meta;
-  p.res = (const uint16_t*)residual; p.sum_out = (uint16_t*)sum_out; p.ldr = ldr; p.ldo = ldo;
+  p.res = nullptr; p.sum_out = nullptr; p.ldr = 0; p.ldo = 0;
   p.x = (const uint16_t*)x; p.ldx = ldx; p.T = T; p.K = K;
   p.gamma = (const uint16_t*)gamma; p.beta = (const uint16_t*)beta; p.x_ts = x_ts;
   p.sp_codes = (uint8_t*)sp_codes; p.sp_sf = (uint8_t*)sp_sf; p.sp_meta = (uint8_t*)sp_meta;
   p.dn_codes = (uint8_t*)dn_codes; p.dn_sf = (uint8_t*)dn_sf; p.row_scale = row_scale;
   p.eps = cfg->eps; p.tiled = (cfg->layout == SHARQ_LAYOUT_TILED);
   p.row_bytes = (uint32_t)(K * 2);
+  p.nbuf = 0;
   p.idx_tags = 0x0004080Cu;
   p.mask24 = (cfg->fmt != SHARQ_HIF4 && cfg->mask == SHARQ_MASK_24) ? 1 : 0;
+  p.combo = 0; p.dn_meta = nullptr;
+  return p;
+}
+
+// Host launcher, called by the C ABI in api.cu after argument validation.
+cudaError_t launch_prepare(const sharq_config* cfg, const void* x, int64_t T, int64_t K, int64_t ldx,
+                           const void* gamma, const void* beta, const float* x_ts, void* sp_codes, void* sp_sf,
+                           void* sp_meta, void* dn_codes, void* dn_sf, float* row_scale, int num_sms,
+                           cudaStream_t st, const void* residual, int64_t ldr, void* sum_out, int64_t ldo,
+                           int combo, void* dn_meta) {
+  PrepParams p = make_prep_params(cfg, x, T, K, ldx, gamma, beta, x_ts, sp_codes, sp_sf, sp_meta, dn_codes, dn_sf, row_scale);
+  p.combo = combo; p.dn_meta = (uint8_t*)dn_meta;
+  p.res = (const uint16_t*)residual; p.sum_out = (uint16_t*)sum_out; p.ldr = ldr; p.ldo = ldo;
   // the row kernel reads 32 bytes per load: rows must start on 32-byte boundaries, otherwise (16-byte aligned
   // input, the C ABI's minimum) the warp-per-row kernel with its 16-byte cp.async takes the call
   const bool wide_ok = ((uintptr_t)x % 32 == 0) && (ldx % 16 == 0);

@@ -427,3 +427,26 @@ def test_outputs_are_repeatable_and_stay_inside_their_buffers(sq):
             else:
                 for a, b in zip(first, snap):
                     assert torch.equal(a, b), f"run {rep} differs (T{T} K{K} D{D})"
+
+
+@pytest.mark.parametrize("fmt,norm,T,K,D", [(0, 1, 1, 4096, 4096), (0, 1, 8, 4096, 6144), (0, 0, 3, 14336, 4096), (0, 1, 2, 4096, 28672),
+                                            (1, 1, 4, 3584, 512), (0, 1, 16, 4096, 4096), (0, 2, 2, 1024, 256)])
+def test_prepare_linear_one_call(sq, fmt, norm, T, K, D):
+    """sharq_prepare_linear: the chained pair (default) and, for T <= 8, the single fused launch (every
+    GEMM CTA prepares the rows with extra warps); either way the activation operands and Y are bit-identical to
+    sharq_prepare followed by sharq_linear, which the other tests compare with the oracle."""
+    x = si.activations(T, K, config=2, outlier_mult=50.0, extra=T + K + D)
+    g, b, w, bias = si.gamma(K, 2), si.beta(K, 2), si.weight(D, K, 2, extra=D), si.beta(D, 2)
+    cfg = sq.make_config(fmt, norm, 1e-6, sq.LAYOUT_TILED)
+    wq = sq.quantize_weight(cfg, to_dev(w))
+    xd, gd, bd = to_dev(x), to_dev(g) if norm else None, to_dev(b) if norm == 2 else None
+    act_ref = sq.prepare(cfg, xd, gd, bd)
+    y_ref = sq.linear(cfg, act_ref, wq, bias=to_dev(bias), out_dtype="fp32")
+    for rep in range(4):                                 # repeated: the fused launch re-reads what its own warps wrote
+        y, act = sq.prepare_linear(cfg, xd, wq, gd, bd, bias=to_dev(bias), out_dtype="fp32", single_launch=rep != 3)
+        torch.cuda.synchronize()
+        for k in ("sp_codes", "sp_sf", "sp_meta", "dn_codes", "dn_sf", "row_scale"):
+            assert torch.equal(act[k], act_ref[k]), f"{k} (rep {rep})"
+        assert torch.equal(y, y_ref), f"Y (rep {rep})"
+    p, q = so.prepare(x, fmt=fmt, norm=norm, gamma_u16=g, beta_u16=b if norm == 2 else None), so.quantize_weight(w, fmt=fmt)
+    assert rel_err(y.cpu().numpy(), so.linear(p, q, bias_u16=bias)).max() <= TOL
