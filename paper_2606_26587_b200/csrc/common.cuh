@@ -26,6 +26,21 @@ __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)_
 __device__ __forceinline__ float bf16lo_to_f32(uint32_t packed) { return __uint_as_float(packed << 16); }
 __device__ __forceinline__ float bf16hi_to_f32(uint32_t packed) { return __uint_as_float(packed & 0xFFFF0000u); }
 
+// The same widenings on the FMA pipe (FHFMA.BF16: x * 1 + (-0), exact for every finite x and both zeros): sharq_prepare
+// is bound by the ALU pipe (shifts, logic, min / max, conversions), the FMA pipe has room
+__device__ __forceinline__ void bf16x2_to_f32_fma(uint32_t packed, float& lo, float& hi) {
+#ifdef SHARQ_UNPACK_ALU
+  lo = bf16lo_to_f32(packed); hi = bf16hi_to_f32(packed);
+#else
+  asm("{ .reg .b16 l, h, one;\n\t"
+      "mov.b32 {l, h}, %2;\n\t"
+      "mov.b16 one, 0x3F80;\n\t"
+      "fma.rn.f32.bf16 %0, l, one, %3;\n\t"
+      "fma.rn.f32.bf16 %1, h, one, %3; }"
+      : "=f"(lo), "=f"(hi) : "r"(packed), "f"(-0.0f));
+#endif
+}
+
 // fp32 pair -> packed bf16x2 (lo in the low half), round-to-nearest-even
 __device__ __forceinline__ uint32_t pack_bf16x2_rn(float lo, float hi) {
   uint32_t r;

@@ -175,3 +175,33 @@ def test_hif4_round_trip_on_grid_and_threshold_predicates():
     sat = (c & 7) == 7
     X = so.bf16_to_f32(xb).astype(np.float64)
     assert (np.abs(X - d)[~sat] <= step[~sat] * (0.5 + 2.0 ** -6) * 1.3).all()
+
+
+def test_hif4_significands_and_the_fp8_question():
+    """SURVEY.md 8(f) N4 (the FP8-rate HiF4 study), the arithmetic behind DESIGN.md's conclusion.  Every HiF4 value is
+    +-(4 + m) * k * 2^p (E6M2 mantissa 1.m, S1P2 magnitude k / 4, the E1 shifts and the exponent in p; Eq. 15 P:467,
+    Table 7): its significand (4 + m) * k <= 49 needs at most 6 bits, so bf16 (8 bits) holds every value
+    exactly -- what the B200 path relies on -- while FP8 does not: e4m3 (4 bits) represents only 21 of the 28 nonzero
+    (m, k) combinations, e5m2 (3 bits) 16.  An exact FP8 path therefore needs a two-term split of BOTH operands (four
+    FP8 GEMMs at twice the bf16 rate = twice the bf16 time); the per-unit mantissa cannot go into a block scale either,
+    because tcgen05's FP8 block scales are powers of two (UE8M0)."""
+    def sig_bits(n):
+        while n % 2 == 0:
+            n //= 2
+        return n.bit_length()
+    pairs = [(m, k) for m in range(4) for k in range(1, 8)]
+    need = [sig_bits((4 + m) * k) for m, k in pairs]
+    assert max(need) == 6 and max((4 + m) * k for m, k in pairs) == 49
+    assert sum(b <= 4 for b in need) == 21 and sum(b <= 3 for b in need) == 16 and sum(b <= 8 for b in need) == 28
+    # the oracle's decode agrees: every decoded value of random units has an odd part below 2^6, and e4m3 misses some
+    rng = np.random.default_rng(3)
+    codes = rng.integers(0, 16, (64, 64)).astype(np.uint8)
+    meta = (rng.integers(0x80, 0xF0, 64).astype(np.uint32) | (rng.integers(0, 1 << 24, 64).astype(np.uint32) << 8))
+    v = np.abs(ho.hif4_decode_units(codes, meta).astype(np.float64)).ravel()
+    v = v[v > 0]
+    mant, _ = np.frexp(v)
+    sig = (mant * 2.0 ** 6)
+    assert (sig == np.round(sig)).all()                                   # 6 bits suffice
+    exact_e4m3 = np.array(v, np.float32).astype(ml_dtypes.float8_e4m3fn).astype(np.float64) == v
+    in_range = (v <= 448) & (v >= 2.0 ** -6)
+    assert 0.5 < exact_e4m3[in_range].mean() < 0.95                       # ... and four bits do not
