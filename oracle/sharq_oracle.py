@@ -10,7 +10,7 @@ Only `tests/`, `__graft_entry__.smoke()` and `bench.py`'s cpu_baseline / `--impl
 legs may import this module.  It shares no code with the CUDA path (paper_2606_26587_b200/) and
 never imports it.  SharQ is an approximation / encoding, so the oracle follows the paper's
 algorithm step by step; where the paper is silent the reading is the one listed in DESIGN.md
-("Readings", R1..R16) and named in the docstrings below.
+("Readings", R1..R18) and named in the docstrings below.
 
 Numerics contract (R1): every fp32 step below is ONE IEEE-754 binary32 operation,
 round-to-nearest-even, no fused multiply-add, no flush-to-zero.  numpy float32 ufuncs do exactly
