@@ -142,7 +142,8 @@ sharq_status sharq_prepare(const sharq_config* cfg, const void* x, int64_t T, in
  * element is read and written by the same thread) but not x.  One kernel, one pass: 2 + 2 B/element
  * more HBM traffic than sharq_prepare, against a separate add kernel's 6 B/element plus a launch.
  * x, residual, sum_out: 32-byte aligned, ldx / ldr / ldo multiples of 16 (256-bit accesses), else
- * SHARQ_EINVAL / SHARQ_ESHAPE; K <= 32768 (one row per CTA), else SHARQ_ESHAPE. */
+ * SHARQ_EINVAL / SHARQ_ESHAPE; K <= 32768 (one row per CTA; NVFP4 with LayerNorm: K <= 25600), else SHARQ_ESHAPE.
+ * The alias check on sum_out is pointer equality with x: partially overlapping buffers are the caller's error. */
 sharq_status sharq_prepare_add(const sharq_config* cfg, const void* x, const void* residual,
                                int64_t T, int64_t K, int64_t ldx, int64_t ldr, void* sum_out,
                                int64_t ldo, const void* gamma, const void* beta,

@@ -180,6 +180,14 @@ __global__ void __launch_bounds__(MAXT, MINB) sharq_prepare_row_kernel(const Pre
 template <int FMT>
 static cudaError_t launch_row_kernel(int norm, const PrepParams& p, int num_sms, cudaStream_t st);
 
+// dynamic shared memory of the row-per-CTA kernel for rows of `warps` 1024-element blocks (prepare_rows' layout)
+static size_t row_kernel_smem(int fmt, int norm, int warps) {
+  return (size_t)warps * 1024 + 256 + 16 + 64                                                         // leaves, amax, stat, mask table
+         + (size_t)warps * 32 * (norm == SHARQ_NORM_LAYER ? 128 : norm == SHARQ_NORM_RMS ? 64 : 0)    // gamma, beta
+         + (fmt == SHARQ_NVFP4 && warps > 8 ? (size_t)warps * 32 * 128 + 512 + 16 : 0);   // lagged loop: parked row (2 stages), amax slots, mbarriers
+}
+constexpr size_t kRowKernelSmemMax = 227 * 1024;   // opt-in limit per CTA on sm_100
+
 // The row kernel indexes with 32 bits: at most 2^31 / max(ldx, K) rows (a multiple of 128, so the tiled
 // layouts split at tile boundaries) per launch; larger problems run as several launches on row ranges.
 template <int FMT>
@@ -230,9 +238,7 @@ static cudaError_t launch_row_kernel(int norm, const PrepParams& p, int num_sms,
   attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
   attr[0].val.programmaticStreamSerializationAllowed = debug_env().no_pdl ? 0 : 1;
   lc.gridDim = grid; lc.blockDim = block; lc.stream = st; lc.attrs = attr; lc.numAttrs = 1;
-  lc.dynamicSmemBytes = (size_t)warps * 1024 + 256 + 16 + 64                                           // leaves, amax, stat, mask table
-                        + (size_t)warps * 32 * (norm == SHARQ_NORM_LAYER ? 128 : norm == SHARQ_NORM_RMS ? 64 : 0)    // gamma, beta
-                        + (FMT == SHARQ_NVFP4 && warps > 8 ? (size_t)warps * 32 * 128 + 512 + 16 : 0);   // lagged loop: parked row (2 stages), amax slots, mbarriers
+  lc.dynamicSmemBytes = row_kernel_smem(FMT, norm, warps);
   cudaError_t err = cudaSuccess;
 #define SHARQ_ROW(N, MAXT, MINB)                                                                              \
   do {                                                                                                        \
@@ -314,8 +320,12 @@ cudaError_t launch_prepare(const sharq_config* cfg, const void* x, int64_t T, in
   // the row kernel reads 32 bytes per load: rows must start on 32-byte boundaries, otherwise (16-byte aligned
   // input, the C ABI's minimum) the warp-per-row kernel with its 16-byte cp.async takes the call
   const bool wide_ok = ((uintptr_t)x % 32 == 0) && (ldx % 16 == 0);
-  if (residual && (!wide_ok || K > 1024 * kRowMaxWarps || p.mask24 || combo)) return cudaErrorInvalidValue;   // checked by the C ABI
-  if (K <= 1024 * kRowMaxWarps && wide_ok && !p.mask24 && !combo && (!debug_env().old_prepare || residual)) {
+  // NVFP4 + LayerNorm on the widest rows (K > 25600): gamma, beta and the lagged loop's parked row together exceed the
+  // shared memory of one CTA; those shapes go to the warp-per-row kernel (the fused-operand calls refuse them)
+  const bool row_fits = K <= 1024 * kRowMaxWarps &&
+                        row_kernel_smem(cfg->fmt, cfg->norm, (int)((K + 1023) / 1024)) <= kRowKernelSmemMax;
+  if (residual && (!wide_ok || !row_fits || p.mask24 || combo)) return cudaErrorInvalidValue;   // checked by the C ABI
+  if (row_fits && wide_ok && !p.mask24 && !combo && (!debug_env().old_prepare || residual)) {
     p.nbuf = 0;
     if (cfg->fmt == SHARQ_NVFP4) return launch_row_chunks<SHARQ_NVFP4>(cfg->norm, p, num_sms, st);
     if (cfg->fmt == SHARQ_MXFP4) return launch_row_chunks<SHARQ_MXFP4>(cfg->norm, p, num_sms, st);

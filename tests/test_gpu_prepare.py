@@ -34,6 +34,7 @@ CASES = [
     (2, 1, 0, 16, 4096, 50.0), (2, 0, 0, 33, 3584, 200.0), (2, 2, 0, 7, 768, 10.0), (2, 1, 0, 3, 18944, 50.0),
     # the widest row one CTA covers (32 warps) and the first K beyond it (warp-per-row kernel, row in smem)
     (0, 1, 1, 3, 32768, 50.0), (0, 1, 1, 3, 33792, 50.0), (0, 2, 0, 150, 33792, 50.0), (1, 0, 0, 2, 33792, 200.0),
+    (0, 2, 1, 5, 32768, 50.0), (0, 2, 0, 4, 25600, 50.0), (0, 2, 0, 4, 26624, 50.0),   # NVFP4 + LayerNorm around the one-CTA shared-memory limit
     (2, 1, 0, 2, 33792, 50.0),
 ]
 
