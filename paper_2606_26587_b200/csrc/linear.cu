@@ -305,9 +305,15 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
       const uint64_t pol_act = SPLIT ? tc::policy_evict_last() : tc::policy_evict_normal();
       const uint64_t pol_w = SPLIT ? tc::policy_evict_first() : tc::policy_evict_normal();
       const int64_t Kc = p.K;
+      // W codes + W's scales.  MXFP4: the dense view IS the sparse view, one load feeds both paths.  NVFP4: the dense
+      // view (every sparse-view scale repeated, P:130 / R7) is read as its own tensor: expanding it from the sparse
+      // atoms in shared memory (tried in the MMA warp: LDS / PRMT / STS + fence.proxy.async per k-block) saved 5 % of
+      // the DRAM bytes and cost 1-2 us per decode launch, whose k-block issue sequence is the critical path.
+      constexpr bool kSharedSfb = !NV;
       uint32_t tx = BN * 128;
-      if (do_sp) tx += p.a_rows * 64 + 2048 + 1024 + S::NB * 1024;
-      if (do_dn) tx += p.a_rows * 128 + S::SF_DN_BYTES + S::NB * S::SF_DN_BYTES;
+      if (do_sp || (kSharedSfb && do_dn)) tx += S::NB * 1024;
+      if (do_sp) tx += p.a_rows * 64 + 2048 + 1024;
+      if (do_dn) tx += p.a_rows * 128 + S::SF_DN_BYTES + (kSharedSfb ? 0 : S::NB * S::SF_DN_BYTES);
       uint32_t it = 0;                                   // k-blocks issued so far (ring position)
       for (int tile = tile0; tile < total_tiles; tile += tile_step) {
         const Unit u = decode_unit(p, g, m_blocks, total_tiles, tile, rank, splits);
@@ -322,10 +328,10 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
           const int kb = kbv >= nkb ? kbv - nkb : kbv;   // second pass of a combination: the same W k-blocks again
           if (lead) tc::tma_load_2d(st + S::W, &tm_w, fb, kb * 128, w_row0, pol_w);
           for (int nb = 0; nb < S::NB; ++nb) {
-            if (do_sp && lead)
+            if ((do_sp || (kSharedSfb && do_dn)) && lead)
               tc::bulk_load(st + S::SFB_SP + nb * 1024,
                             p.w_sf_sp + ((size_t)(wblk0 + nb) * (Kc / 128) + (size_t)kb * 2) * 512, 1024, fb, pol_w);
-            if (do_dn && lead)
+            if (!kSharedSfb && do_dn && lead)
               tc::bulk_load(st + S::SFB_DN + nb * S::SF_DN_BYTES,
                             p.w_sf_dn + ((size_t)(wblk0 + nb) * (Kc / 256) + (size_t)kb) * S::SF_DN_BYTES,
                             S::SF_DN_BYTES, fb, pol_w);
@@ -442,9 +448,9 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
             for (int a = 0; a < ATOMS; ++a) {
               if (lead) tc::tc_cp_sf(tmem_base + S::SFA_DN_COL + 4 * a, tc::smem_desc(st + S::SFA_DN + 512 * a, 128, 0));
 #pragma unroll
-              for (int nb = 0; nb < S::NB; ++nb)
+              for (int nb = 0; nb < S::NB; ++nb)      // MXFP4: the dense view IS the sparse view (same atoms)
                 if (lead) tc::tc_cp_sf(tmem_base + S::SFB_DN_COL + S::SFB_COLS * a + 4 * nb,
-                             tc::smem_desc(st + S::SFB_DN + nb * S::SF_DN_BYTES + 512 * a, 128, 0));
+                             tc::smem_desc(st + (NV ? S::SFB_DN + nb * S::SF_DN_BYTES : S::SFB_SP + nb * 1024) + 512 * a, 128, 0));
             }
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
