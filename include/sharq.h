@@ -157,7 +157,8 @@ sharq_status sharq_prepare_add(const sharq_config* cfg, const void* x, const voi
  * computed in fp32 by a fixed algorithm (degree-5 polynomial exp, IEEE reciprocal; R18) that the oracle
  * restates bit for bit; h never goes to HBM and is the activation norm -> mask -> backbone -> residual see.
  * gate / up: bf16 [T, K] (ldg / ldu elements between rows: the two halves of a [T, 2K] gate+up output work),
- * 32-byte aligned, ldg / ldu multiples of 16, K <= 32768; otherwise SHARQ_EINVAL / SHARQ_ESHAPE. */
+ * 32-byte aligned, ldg / ldu multiples of 16, K <= 32768; cfg->norm must be SHARQ_NORM_NONE (the down projection's input is
+ * not normalised; gamma / beta are ignored); otherwise SHARQ_EINVAL / SHARQ_ESHAPE. */
 sharq_status sharq_prepare_swiglu(const sharq_config* cfg, const void* gate, const void* up, int64_t T, int64_t K,
                                   int64_t ldg, int64_t ldu, const void* gamma, const void* beta,
                                   const float* x_tensor_scale, void* sp_codes, void* sp_sf, void* sp_meta,

@@ -183,7 +183,7 @@ sharq_status sharq_prepare_swiglu(const sharq_config* cfg, const void* gate, con
   sharq_status s = check_cfg(cfg);
   if (s != SHARQ_OK) return s;
   if (T < 0 || K <= 0 || K % 256 != 0 || K > 32768) return SHARQ_ESHAPE;
-  if (cfg->fmt == SHARQ_NVFP4 && cfg->norm == SHARQ_NORM_LAYER && K > 25600) return SHARQ_ESHAPE;
+  if (cfg->norm != SHARQ_NORM_NONE) return SHARQ_EINVAL;   // the down projection's input is not normalised
   if (cfg->fmt != SHARQ_HIF4 && cfg->mask != SHARQ_MASK_PAIR48) return SHARQ_EINVAL;
   if (ldg < K || ldu < K || ldg % 16 != 0 || ldu % 16 != 0) return SHARQ_ESHAPE;
   if (T == 0) return SHARQ_OK;

@@ -155,10 +155,29 @@ __device__ __forceinline__ Unit decode_unit(const KParams& p, const GroupTab& g,
 // (the ragged last n-tile: D % 8 == 0, any multiple of 8) are neither computed with bias nor stored.
 template <int N>
 __device__ __forceinline__ void store_row(const KParams& p, int64_t row, int col0, float scale, float (&f)[N]) {
-  const int ncols = p.D - col0;                       // >= N for every tile but the last
+  const int ncols = p.D - col0;                       // >= N for every tile but a ragged last one
   if (ncols <= 0) return;
 #pragma unroll
   for (int i = 0; i < N; ++i) f[i] = __fmul_rn(f[i], scale);
+  if (ncols >= N) {                                   // the common case, no per-column predicates
+    if (p.bias) {
+      const uint16_t* b = p.bias + col0;
+#pragma unroll
+      for (int i = 0; i < N; ++i) f[i] = __fadd_rn(f[i], __uint_as_float((uint32_t)b[i] << 16));
+    }
+    if (p.out_fp32) {
+      float4* dst = reinterpret_cast<float4*>(static_cast<float*>(p.Y) + row * p.ldy + col0);
+#pragma unroll
+      for (int i = 0; i < N / 4; ++i) dst[i] = make_float4(f[4 * i], f[4 * i + 1], f[4 * i + 2], f[4 * i + 3]);
+    } else {
+      uint4* dst = reinterpret_cast<uint4*>(static_cast<uint16_t*>(p.Y) + row * p.ldy + col0);
+#pragma unroll
+      for (int i = 0; i < N / 8; ++i)
+        dst[i] = make_uint4(pack_bf16x2_rn(f[8 * i], f[8 * i + 1]), pack_bf16x2_rn(f[8 * i + 2], f[8 * i + 3]),
+                            pack_bf16x2_rn(f[8 * i + 4], f[8 * i + 5]), pack_bf16x2_rn(f[8 * i + 6], f[8 * i + 7]));
+    }
+    return;
+  }
   if (p.bias) {
     const uint16_t* b = p.bias + col0;
 #pragma unroll
@@ -191,13 +210,16 @@ __device__ __forceinline__ void store_row(const KParams& p, int64_t row, int col
 // The prepared operands go to the caller's activation buffers in global memory -- all CTAs write the same bytes --
 // and come back through the same TMA loads as in the two-launch path, after this CTA's own stores are fenced
 // (__threadfence + fence.proxy.async) and its `act_bar` mbarrier has completed.
-template <int BN, int FMT, bool SPLIT, int AR, bool MC = false, bool FUSED = false>
-__global__ void __launch_bounds__(FUSED ? kThreads + 32 * kPrepWarpsMax : kThreads, 1)
-sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_constant__ CUtensorMap tm_a_dn,
-                    const __grid_constant__ CUtensorMap tm_w, const __grid_constant__ CUtensorMap tm_alt,
-                    const KParams p, const PrepParams pp, const int prep_norm) {
+// COMBO = true: the Table 5 combinations (path 3 / 4): second K-loop on the second operand (tm_alt, sf2, meta2).
+// The body is shared; the __global__ wrappers below differ in their parameter lists, so that the plain kernel --
+// every decode and MoE launch -- carries neither the fourth tensor map nor the prepare parameters.
+template <int BN, int FMT, bool SPLIT, int AR, bool MC, bool FUSED, bool COMBO>
+__device__ __forceinline__ void linear_body(const CUtensorMap* tm_a_sp_p, const CUtensorMap* tm_a_dn_p,
+                                            const CUtensorMap* tm_w_p, const CUtensorMap* tm_alt_p, const KParams& p,
+                                            const PrepParams* pp_p, const int prep_norm) {
   using S = Stage<BN, FMT, SPLIT, AR, FUSED ? kPrepSmem : 0>;
   static_assert(!(FUSED && MC), "the fused kernel is for single-problem launches");
+  static_assert(!(COMBO && (SPLIT || MC || FUSED)), "combinations run on the persistent single-problem variant");
   constexpr bool NV = (FMT == SHARQ_NVFP4);
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
@@ -225,9 +247,9 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
   GroupTab g{nullptr, nullptr, 0};
 
   if (warp == 0 && lane == 0) {
-    tc::prefetch_tmap(&tm_a_sp);
-    tc::prefetch_tmap(&tm_a_dn);
-    tc::prefetch_tmap(&tm_w);
+    tc::prefetch_tmap(tm_a_sp_p);
+    tc::prefetch_tmap(tm_a_dn_p);
+    tc::prefetch_tmap(tm_w_p);
   }
   if (warp == 1 && lane == 0) {
     for (int s = 0; s < S::STAGES; ++s) {
@@ -325,8 +347,8 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
         // weight side of k-block kb (codes + both scale views): independent of the preceding kernel
         const int nkb = (int)(Kc / BK);
         auto load_w = [&](int kbv, uint32_t st, uint32_t fb) {
-          const int kb = kbv >= nkb ? kbv - nkb : kbv;   // second pass of a combination: the same W k-blocks again
-          if (lead) tc::tma_load_2d(st + S::W, &tm_w, fb, kb * 128, w_row0, pol_w);
+          const int kb = (COMBO && kbv >= nkb) ? kbv - nkb : kbv;   // second pass of a combination: the same W k-blocks again
+          if (lead) tc::tma_load_2d(st + S::W, tm_w_p, fb, kb * 128, w_row0, pol_w);
           for (int nb = 0; nb < S::NB; ++nb) {
             if ((do_sp || (kSharedSfb && do_dn)) && lead)
               tc::bulk_load(st + S::SFB_SP + nb * 1024,
@@ -339,32 +361,44 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
         };
         // activation side: written by sharq_prepare, only after griddepcontrol.wait
         auto load_a = [&](int kbv, uint32_t st, uint32_t fb) {
-          const bool alt = kbv >= nkb;                   // combinations: the second operand
+          const bool alt = COMBO && kbv >= nkb;          // combinations: the second operand
           const int kb = alt ? kbv - nkb : kbv;
           if constexpr (MC) {
             // same 128-row block in both CTAs: CTA 0 fetches the dense side, CTA 1 the sparse side, for both
             if (do_sp && crank == 1) {
-              if (lead) tc::tma_load_2d_mc(st + S::A_SP, &tm_a_sp, fb, kb * 64, u.m_blk * BM, 3, pol_act);
+              if (lead) tc::tma_load_2d_mc(st + S::A_SP, tm_a_sp_p, fb, kb * 64, u.m_blk * BM, 3, pol_act);
               if (lead) tc::bulk_load_mc(st + S::META, meta + (size_t)kb * 2048, 2048, fb, 3, pol_act);
               if (lead) tc::bulk_load_mc(st + S::SFA_SP, sfa_sp + (size_t)kb * 1024, 1024, fb, 3, pol_act);
             }
             if (do_dn && crank == 0) {
-              if (lead) tc::tma_load_2d_mc(st + S::A_DN, &tm_a_dn, fb, kb * 128, u.m_blk * BM, 3, pol_act);
+              if (lead) tc::tma_load_2d_mc(st + S::A_DN, tm_a_dn_p, fb, kb * 128, u.m_blk * BM, 3, pol_act);
               if (lead) tc::bulk_load_mc(st + S::SFA_DN, sfa_dn + (size_t)kb * S::SF_DN_BYTES, S::SF_DN_BYTES, fb, 3, pol_act);
+            }
+            return;
+          }
+          if (!COMBO || !alt) {                          // SharQ and the single-path modes: everything but a combination's second pass
+            if (do_sp) {
+              if (lead) tc::tma_load_2d(st + S::A_SP, tm_a_sp_p, fb, kb * 64, u.m_blk * BM, pol_act);
+              if (lead) tc::bulk_load(st + S::META, meta + (size_t)kb * 2048, 2048, fb, pol_act);
+              if (lead) tc::bulk_load(st + S::SFA_SP, sfa_sp + (size_t)kb * 1024, 1024, fb, pol_act);
+            }
+            if (do_dn) {
+              if (lead) tc::tma_load_2d(st + S::A_DN, tm_a_dn_p, fb, kb * 128, u.m_blk * BM, pol_act);
+              if (lead) tc::bulk_load(st + S::SFA_DN, sfa_dn + (size_t)kb * S::SF_DN_BYTES, S::SF_DN_BYTES, fb, pol_act);
             }
             return;
           }
           if (do_sp) {
             const size_t mo = (size_t)u.m_blk * (Kc / 256) * 2048 + (size_t)kb * 2048;
             const size_t so = (size_t)u.m_blk * (Kc / 128) * 512 + (size_t)kb * 1024;
-            if (lead) tc::tma_load_2d(st + S::A_SP, alt ? &tm_alt : &tm_a_sp, fb, kb * 64, u.m_blk * BM, pol_act);
-            if (lead) tc::bulk_load(st + S::META, (alt ? p.meta2 : p.sp_meta) + mo, 2048, fb, pol_act);
-            if (lead) tc::bulk_load(st + S::SFA_SP, (alt ? p.sf2 : p.sp_sf) + so, 1024, fb, pol_act);
+            if (lead) tc::tma_load_2d(st + S::A_SP, tm_alt_p, fb, kb * 64, u.m_blk * BM, pol_act);
+            if (lead) tc::bulk_load(st + S::META, p.meta2 + mo, 2048, fb, pol_act);
+            if (lead) tc::bulk_load(st + S::SFA_SP, p.sf2 + so, 1024, fb, pol_act);
           }
           if (do_dn) {
             const size_t so = ((size_t)u.m_blk * (Kc / 256) + (size_t)kb) * S::SF_DN_BYTES;
-            if (lead) tc::tma_load_2d(st + S::A_DN, alt ? &tm_alt : &tm_a_dn, fb, kb * 128, u.m_blk * BM, pol_act);
-            if (lead) tc::bulk_load(st + S::SFA_DN, (alt ? p.sf2 : p.dn_sf) + so, S::SF_DN_BYTES, fb, pol_act);
+            if (lead) tc::tma_load_2d(st + S::A_DN, tm_alt_p, fb, kb * 128, u.m_blk * BM, pol_act);
+            if (lead) tc::bulk_load(st + S::SFA_DN, p.sf2 + so, S::SF_DN_BYTES, fb, pol_act);
           }
         };
         int kb = u.kb0;
@@ -557,11 +591,11 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
     if constexpr (FUSED) {
       tc::grid_dependency_wait();                        // x belongs to the kernels before this one
       const int ptid = (int)threadIdx.x - kThreads, pthreads = (int)blockDim.x - kThreads;
-      if (prep_norm == SHARQ_NORM_RMS) prepare_rows<FMT, SHARQ_NORM_RMS, 2, false>(pp, prep_smem, ptid, pthreads, 0, 1);
+      if (prep_norm == SHARQ_NORM_RMS) prepare_rows<FMT, SHARQ_NORM_RMS, 2, false>(*pp_p, prep_smem, ptid, pthreads, 0, 1);
 #ifdef SHARQ_EXPERIMENTS
       else if (prep_norm == 99) { }                      // timing experiment: no in-kernel prepare at all
 #endif
-      else prepare_rows<FMT, SHARQ_NORM_NONE, 2, false>(pp, prep_smem, ptid, pthreads, 0, 1);
+      else prepare_rows<FMT, SHARQ_NORM_NONE, 2, false>(*pp_p, prep_smem, ptid, pthreads, 0, 1);
       __threadfence();                                   // every thread's stores, device scope
       named_bar_sync<2>(pthreads);
       if (ptid == 0) tc::mbar_arrive(act_bar);
@@ -621,6 +655,29 @@ sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_co
     tc::tc_fence_after();
     tc::tmem_dealloc<kTmemCols>(tmem_base);
   }
+}
+
+template <int BN, int FMT, bool SPLIT, int AR, bool MC = false>
+__global__ void __launch_bounds__(kThreads, 1)
+sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_constant__ CUtensorMap tm_a_dn,
+                    const __grid_constant__ CUtensorMap tm_w, const KParams p) {
+  linear_body<BN, FMT, SPLIT, AR, MC, false, false>(&tm_a_sp, &tm_a_dn, &tm_w, nullptr, p, nullptr, 0);
+}
+
+template <int BN, int FMT, int AR>
+__global__ void __launch_bounds__(kThreads, 1)
+sharq_linear_combo_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_constant__ CUtensorMap tm_a_dn,
+                          const __grid_constant__ CUtensorMap tm_w, const __grid_constant__ CUtensorMap tm_alt,
+                          const KParams p) {
+  linear_body<BN, FMT, false, AR, false, false, true>(&tm_a_sp, &tm_a_dn, &tm_w, &tm_alt, p, nullptr, 0);
+}
+
+template <int BN, int FMT, bool SPLIT, int AR>
+__global__ void __launch_bounds__(kThreads + 32 * kPrepWarpsMax, 1)
+sharq_linear_fused_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_constant__ CUtensorMap tm_a_dn,
+                          const __grid_constant__ CUtensorMap tm_w, const KParams p,
+                          const __grid_constant__ PrepParams pp, const int prep_norm) {
+  linear_body<BN, FMT, SPLIT, AR, false, true, false>(&tm_a_sp, &tm_a_dn, &tm_w, nullptr, p, &pp, prep_norm);
 }
 
 // ---- CTA-pair kernel (cta_group::2): 256 x 256 output tile per cluster of two CTAs ---------------------
@@ -987,10 +1044,8 @@ sharq_status launch_1cta_impl(const LinearArgs& a, const KParams& p, const CUten
   if constexpr (FUSED) { pp = *env.fz->pp; norm = env.fz->norm; if (debug_env().skip_prep) norm = 99; }
   if constexpr (kSplitFits) if (splits > 1) {
     using S = Stage<BN, FMT, true, AR, kExtra>;
-    auto kfn = sharq_linear_kernel<BN, FMT, true, AR, false, FUSED>;
     if (env.plan_only) { fill_plan(env.plan_only, FUSED ? 4 : 0, BN, AR, splits, S::STAGES, tiles, tiles * splits, splits); return SHARQ_OK; }
     static std::atomic<uint64_t> smem_set{0};
-    if (set_smem_once(smem_set, (const void*)kfn, S::SMEM, env.dev) != cudaSuccess) return SHARQ_ECUDA;
     lc.gridDim = dim3((unsigned)(tiles * splits));
     lc.dynamicSmemBytes = S::SMEM;
     attr[1].id = cudaLaunchAttributeClusterDimension;
@@ -998,18 +1053,39 @@ sharq_status launch_1cta_impl(const LinearArgs& a, const KParams& p, const CUten
     attr[1].val.clusterDim.y = 1;
     attr[1].val.clusterDim.z = 1;
     lc.numAttrs = 2;
-    return cudaLaunchKernelEx(&lc, kfn, tm_sp, tm_dn, tm_w, tm_alt, p, pp, norm) == cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
+    if constexpr (FUSED) {
+      auto kfn = sharq_linear_fused_kernel<BN, FMT, true, AR>;
+      if (set_smem_once(smem_set, (const void*)kfn, S::SMEM, env.dev) != cudaSuccess) return SHARQ_ECUDA;
+      return cudaLaunchKernelEx(&lc, kfn, tm_sp, tm_dn, tm_w, p, pp, norm) == cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
+    } else {
+      auto kfn = sharq_linear_kernel<BN, FMT, true, AR>;
+      if (set_smem_once(smem_set, (const void*)kfn, S::SMEM, env.dev) != cudaSuccess) return SHARQ_ECUDA;
+      return cudaLaunchKernelEx(&lc, kfn, tm_sp, tm_dn, tm_w, p) == cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
+    }
   }
   using S = Stage<BN, FMT, false, AR, kExtra>;
-  auto kfn = sharq_linear_kernel<BN, FMT, false, AR, false, FUSED>;
   int64_t grid = tiles < env.num_sms ? tiles : env.num_sms;      // persistent: one CTA per SM
   if (debug_env().grid > 0) grid = debug_env().grid;
   if (env.plan_only) { fill_plan(env.plan_only, FUSED ? 4 : 0, BN, AR, 1, S::STAGES, tiles, grid, 1); return SHARQ_OK; }
-  static std::atomic<uint64_t> smem_set{0};
-  if (set_smem_once(smem_set, (const void*)kfn, S::SMEM, env.dev) != cudaSuccess) return SHARQ_ECUDA;
   lc.gridDim = dim3((unsigned)grid);
   lc.dynamicSmemBytes = S::SMEM;
-  return cudaLaunchKernelEx(&lc, kfn, tm_sp, tm_dn, tm_w, tm_alt, p, pp, norm) == cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
+  if constexpr (FUSED) {
+    static std::atomic<uint64_t> smem_set{0};
+    auto kfn = sharq_linear_fused_kernel<BN, FMT, false, AR>;
+    if (set_smem_once(smem_set, (const void*)kfn, S::SMEM, env.dev) != cudaSuccess) return SHARQ_ECUDA;
+    return cudaLaunchKernelEx(&lc, kfn, tm_sp, tm_dn, tm_w, p, pp, norm) == cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
+  } else {
+    if (p.path >= 3) {                                           // Table 5 combinations: second K-loop, fourth tensor map
+      static std::atomic<uint64_t> smem_set{0};
+      auto kfn = sharq_linear_combo_kernel<BN, FMT, AR>;
+      if (set_smem_once(smem_set, (const void*)kfn, S::SMEM, env.dev) != cudaSuccess) return SHARQ_ECUDA;
+      return cudaLaunchKernelEx(&lc, kfn, tm_sp, tm_dn, tm_w, tm_alt, p) == cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
+    }
+    static std::atomic<uint64_t> smem_set{0};
+    auto kfn = sharq_linear_kernel<BN, FMT, false, AR>;
+    if (set_smem_once(smem_set, (const void*)kfn, S::SMEM, env.dev) != cudaSuccess) return SHARQ_ECUDA;
+    return cudaLaunchKernelEx(&lc, kfn, tm_sp, tm_dn, tm_w, p) == cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
+  }
 }
 
 template <int BN, int FMT, int AR>
@@ -1046,7 +1122,7 @@ sharq_status launch_mc(const KParams& p, const CUtensorMap& tm_sp, const CUtenso
   lc.gridDim = dim3((unsigned)(2 * clusters));
   lc.dynamicSmemBytes = S::SMEM;
   lc.stream = env.st;
-  return cudaLaunchKernelEx(&lc, kfn, tm_sp, tm_dn, tm_w, tm_sp, p, PrepParams{}, 0) == cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
+  return cudaLaunchKernelEx(&lc, kfn, tm_sp, tm_dn, tm_w, p) == cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
 }
 
 // scale-factor / metadata array as a 2-D tensor of 1024-byte rows (256 x u32), boxes of `box_rows` rows

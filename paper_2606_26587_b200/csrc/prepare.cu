@@ -167,14 +167,14 @@ __global__ void __launch_bounds__(512) sharq_prepare_kernel(const PrepParams p) 
 }
 
 // ---- row-per-CTA kernel (K <= 32768): body in prepare_device.cuh --------------------------------------
-template <int FMT, int NORM, int MAXT, int MINB>
+template <int FMT, int NORM, int MAXT, int MINB, bool SWIGLU = false>
 __global__ void __launch_bounds__(MAXT, MINB) sharq_prepare_row_kernel(const PrepParams p) {
   extern __shared__ __align__(16) uint8_t row_smem[];
   // programmatic dependent launch: let the GEMM that follows start streaming its weights now; our own
   // inputs (and the operand buffers we overwrite) belong to the kernels before us
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   asm volatile("griddepcontrol.wait;" ::: "memory");
-  prepare_rows<FMT, NORM, 0, (MAXT >= 512)>(p, row_smem, (int)threadIdx.x, (int)blockDim.x, (int64_t)blockIdx.x, (int64_t)gridDim.x);
+  prepare_rows<FMT, NORM, 0, (MAXT >= 512), SWIGLU>(p, row_smem, (int)threadIdx.x, (int)blockDim.x, (int64_t)blockIdx.x, (int64_t)gridDim.x);
 }
 
 template <int FMT>
@@ -240,6 +240,7 @@ static cudaError_t launch_row_kernel(int norm, const PrepParams& p, int num_sms,
   lc.gridDim = grid; lc.blockDim = block; lc.stream = st; lc.attrs = attr; lc.numAttrs = 1;
   lc.dynamicSmemBytes = row_kernel_smem(FMT, norm, warps);
   cudaError_t err = cudaSuccess;
+  const bool swiglu = p.res != nullptr && p.sum_out == nullptr;        // sharq_prepare_swiglu (norm NONE only, checked by the C ABI)
 #define SHARQ_ROW(N, MAXT, MINB)                                                                              \
   do {                                                                                                        \
     auto kfn = sharq_prepare_row_kernel<FMT, N, MAXT, MINB>;                                                  \
@@ -247,9 +248,17 @@ static cudaError_t launch_row_kernel(int norm, const PrepParams& p, int num_sms,
       err = cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)lc.dynamicSmemBytes); \
     if (err == cudaSuccess) err = cudaLaunchKernelEx(&lc, kfn, p);                                            \
   } while (0)
+#define SHARQ_ROW_SWIGLU(MAXT, MINB)                                                                         \
+  do {                                                                                                        \
+    auto kfn = sharq_prepare_row_kernel<FMT, SHARQ_NORM_NONE, MAXT, MINB, true>;                              \
+    if (lc.dynamicSmemBytes > 48 * 1024)                                                                      \
+      err = cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)lc.dynamicSmemBytes); \
+    if (err == cudaSuccess) err = cudaLaunchKernelEx(&lc, kfn, p);                                            \
+  } while (0)
 #define SHARQ_ROW_N(MAXT, MINB)                                              \
   {                                                                          \
-    if (norm == SHARQ_NORM_NONE) SHARQ_ROW(SHARQ_NORM_NONE, MAXT, MINB);     \
+    if (swiglu) SHARQ_ROW_SWIGLU(MAXT, MINB);                                \
+    else if (norm == SHARQ_NORM_NONE) SHARQ_ROW(SHARQ_NORM_NONE, MAXT, MINB); \
     else if (norm == SHARQ_NORM_RMS) SHARQ_ROW(SHARQ_NORM_RMS, MAXT, MINB);  \
     else SHARQ_ROW(SHARQ_NORM_LAYER, MAXT, MINB);                            \
   }
@@ -269,6 +278,7 @@ static cudaError_t launch_row_kernel(int norm, const PrepParams& p, int num_sms,
   else if (warps <= 16) SHARQ_ROW_N(512, SHARQ_ROW_MINB_512)
   else SHARQ_ROW_N(1024, 1)                      // <= 64 registers
 #undef SHARQ_ROW_N
+#undef SHARQ_ROW_SWIGLU
 #undef SHARQ_ROW
   return err;
 }
