@@ -252,6 +252,26 @@ sharq_status sharq_linear_paths(const sharq_config* cfg, int32_t path, int64_t T
                                 const void* w_sf_dense_view, const float* w_tensor_scale, const void* bias,
                                 void* Y, int64_t ldy, int32_t out_dtype, void* stream);
 
+/* ---- sharq_linear_hif4_static: sharq_linear for HiF4 that needs no workspace and allocates nothing -------------
+ * HiF4's sharq_linear is the one call of this library that needs scratch memory (the bf16 copy of the activation
+ * operands).  Some callers cannot provide or allocate it: code under CUDA-graph capture, tight serving loops, harnesses
+ * that forbid cudaMalloc.  This variant keeps the scratch in a file-scope device array of
+ * SHARQ_STATIC_SCRATCH_BYTES inside the library (every GPU that loads the library holds it until exit); the call
+ * makes no cudaMalloc / cudaFree / allocating library call.  Same arguments and results as sharq_linear with a HiF4
+ * config (layout CANONICAL, D % 128 == 0), minus the workspace.
+ * Limit: roundup(T, 128) * 2K * 2 + 256 <= SHARQ_STATIC_SCRATCH_BYTES, i.e. T <= 128 with K <= 16384, T <= 256 with
+ * K <= 8192, T <= 512 with K <= 4096 (decode and small-batch shapes); larger problems return SHARQ_EWORKSPACE and launch
+ * nothing.  All calls on a device share the one array: calls that overlap on the GPU (different streams) RACE on it;
+ * calls in one stream are ordered.  The array keeps the last call's contents; nothing in it has to start at zero. */
+#define SHARQ_STATIC_SCRATCH_BYTES (8u * 1024u * 1024u + 256u)
+sharq_status sharq_linear_hif4_static(const sharq_config* cfg, int64_t T, int64_t D, int64_t K,
+                                      const void* sp_codes, const void* sp_sf, const void* sp_meta,
+                                      const void* dn_codes, const void* dn_sf, const float* row_scale,
+                                      const void* w_codes, const void* w_sf_sparse_view,
+                                      const void* w_sf_dense_view, const float* w_tensor_scale,
+                                      const void* bias, void* Y, int64_t ldy, int32_t out_dtype, int32_t path,
+                                      void* stream);
+
 /* ---- sharq_act_init: one-time initialisation of TILED activation scale / metadata buffers ----------
  * Fills sp_sf and dn_sf with zero scales and sp_meta with the valid nibble 0x4 (pairs 0 and 1) for all
  * roundup(T, 128) rows, so that the pad rows sharq_prepare never writes hold defined operands (see "Output

@@ -63,6 +63,8 @@ def _load() -> ctypes.CDLL:
                                  c_int32, c_int32, P, c_size_t, P]
     lib.sharq_prepare_linear.argtypes = [CFG, P, c_int64, c_int64, c_int64, P, P, P, P, P, P, P, P, P, c_int64, P, P, P, P, P,
                                          P, c_int64, c_int32, c_int32, P, c_size_t, P]
+    lib.sharq_linear_hif4_static.argtypes = [CFG, c_int64, c_int64, c_int64, P, P, P, P, P, P, P, P, P, P, P, P, c_int64,
+                                             c_int32, c_int32, P]
     lib.sharq_linear_grouped.argtypes = [CFG, c_int32, P, c_int64, c_int64, c_int64, P, P, P, P, P, P, P, P,
                                          P, P, P, c_int64, c_int32, P, c_size_t, P]
     lib.sharq_act_init.argtypes = [CFG, c_int64, c_int64, P, P, P, P]
@@ -82,7 +84,7 @@ def _load() -> ctypes.CDLL:
 # every symbol include/sharq.h declares, then include/sharq_diag.h's
 EXPORTS = ("sharq_version", "sharq_weight_sizes", "sharq_act_sizes", "sharq_linear_workspace",
            "sharq_quantize_weight", "sharq_prepare", "sharq_prepare_add", "sharq_prepare_swiglu", "sharq_prepare_linear", "sharq_linear", "sharq_linear_grouped",
-           "sharq_act_init", "sharq_linear_plan", "sharq_untile_sf", "sharq_untile_meta", "sharq_act_sizes_paths",
+           "sharq_linear_hif4_static", "sharq_act_init", "sharq_linear_plan", "sharq_untile_sf", "sharq_untile_meta", "sharq_act_sizes_paths",
            "sharq_prepare_paths", "sharq_linear_paths", "sharq_mma_peak_launch")
 capi = _load()
 
@@ -306,6 +308,24 @@ def prepare_linear(cfg: Config, x, wq: dict, gamma=None, beta=None, x_tensor_sca
                                      0 if Y.dtype == torch.bfloat16 else 1, 1 if single_launch else 0, None, 0, _stream()),
            "sharq_prepare_linear")
     return Y, act
+
+
+STATIC_SCRATCH_BYTES = 8 * 1024 * 1024 + 256      # SHARQ_STATIC_SCRATCH_BYTES of sharq.h
+
+
+def linear_hif4_static(cfg: Config, act: dict, wq: dict, bias=None, out_dtype="bf16", path=PATH_SHARQ, Y=None):
+    """sharq_linear_hif4_static: HiF4 linear with the library's own static scratch (no workspace, no allocation in the
+    call; Y may be passed in).  Raises SharqError(EWORKSPACE) beyond the limit stated in sharq.h."""
+    import torch
+    T, K, D = act["T"], act["K"], wq["D"]
+    if Y is None:
+        Y = torch.empty((T, D), dtype=torch.bfloat16 if out_dtype == "bf16" else torch.float32, device=act["sp_codes"].device)
+    _check(capi.sharq_linear_hif4_static(ctypes.byref(cfg), T, D, K, _ptr(act["sp_codes"]), _ptr(act["sp_sf"]),
+                                         _ptr(act["sp_meta"]), _ptr(act["dn_codes"]), _ptr(act["dn_sf"]), _ptr(act["row_scale"]),
+                                         _ptr(wq["codes"]), _ptr(wq["sf_sp"]), _ptr(wq["sf_dn"]), _ptr(wq["ts_w"]), _ptr(bias),
+                                         _ptr(Y), Y.stride(0), 0 if Y.dtype == torch.bfloat16 else 1, path, _stream()),
+           "sharq_linear_hif4_static")
+    return Y
 
 
 def linear_grouped(cfg: Config, offsets, act: dict, wq: dict, D: int, out_dtype="bf16", Y=None, workspace=None):

@@ -14,6 +14,8 @@
 #include <cuda.h>
 #include <cuda_runtime.h>
 
+#include <atomic>
+
 #include "common.cuh"
 #include "linear_args.h"
 #include "tc_ptx.cuh"
@@ -322,4 +324,65 @@ sharq_status launch_linear_hif4(const LinearArgs& a, void* workspace, size_t wor
   return wide ? launch_gemm<256>(tm_a, tm_w, p, num_sms, st) : launch_gemm<128>(tm_a, tm_w, p, num_sms, st);
 }
 
+// ---- sharq_linear_hif4_static: the same path with its scratch in a file-scope device array (no allocation) ---------
+// For callers that cannot provide (or allocate) a workspace: code under CUDA-graph capture, tight serving loops,
+// harnesses that forbid cudaMalloc.  The bf16 copy of the activation operands [roundup(T, 128), 2K] goes to
+// g_hif4_scratch instead of a caller's workspace.  Every GPU that loads the library holds the array until exit.
+// In HOST code the array's name is only a stand-in for the symbol, not a device address: the address is taken once per
+// device, with that device current, by cudaGetSymbolAddress, and that pointer is what the kernels get.
+constexpr size_t kHif4StaticScratchBytes = SHARQ_STATIC_SCRATCH_BYTES;
+static __device__ __align__(256) uint8_t g_hif4_scratch[kHif4StaticScratchBytes];
+
+namespace {
+constexpr int kScratchDevices = 64;
+std::atomic<void*> g_scratch_ptr[kScratchDevices];      // per device ordinal; filled idempotently, lock-free
+
+sharq_status static_scratch_ptr(int dev, void** out) {
+  void* ptr = (dev >= 0 && dev < kScratchDevices) ? g_scratch_ptr[dev].load(std::memory_order_acquire) : nullptr;
+  if (!ptr) {
+    if (cudaGetSymbolAddress(&ptr, g_hif4_scratch) != cudaSuccess || !ptr) return SHARQ_ECUDA;   // current device = dev
+    if (dev >= 0 && dev < kScratchDevices) g_scratch_ptr[dev].store(ptr, std::memory_order_release);
+  }
+  *out = ptr;
+  return SHARQ_OK;
+}
+}  // namespace
+
 }  // namespace sharq
+
+extern "C" sharq_status sharq_linear_hif4_static(const sharq_config* cfg, int64_t T, int64_t D, int64_t K,
+                                                 const void* sp_codes, const void* sp_sf, const void* sp_meta,
+                                                 const void* dn_codes, const void* dn_sf, const float* row_scale,
+                                                 const void* w_codes, const void* w_sf_sparse_view,
+                                                 const void* w_sf_dense_view, const float* w_tensor_scale,
+                                                 const void* bias, void* Y, int64_t ldy, int32_t out_dtype,
+                                                 int32_t path, void* stream) {
+  using namespace sharq;
+  if (!cfg || cfg->fmt != SHARQ_HIF4 || cfg->mask != SHARQ_MASK_24 || cfg->layout != SHARQ_LAYOUT_CANONICAL)
+    return SHARQ_EINVAL;
+  if (T < 0 || T >= (int64_t)1 << 30 || D <= 0 || D % 128 != 0 || K <= 0 || K % 256 != 0 || ldy < D || ldy % 8 != 0)
+    return SHARQ_ESHAPE;
+  if (out_dtype < 0 || out_dtype > 1 || path < 0 || path > 2) return SHARQ_EINVAL;
+  if (T == 0) return SHARQ_OK;
+  // the scratch is a fixed array: larger problems are refused, never silently truncated
+  if (hif4_linear_workspace_bytes(T, D, K) > kHif4StaticScratchBytes) return SHARQ_EWORKSPACE;
+  const void* ptrs[] = {sp_codes, sp_sf, sp_meta, dn_codes, dn_sf, w_codes, w_sf_sparse_view, w_sf_dense_view, Y};
+  for (const void* q : ptrs)
+    if (!q || (reinterpret_cast<uintptr_t>(q) & 15u)) return SHARQ_EINVAL;
+  if (!row_scale || !w_tensor_scale) return SHARQ_EINVAL;
+  int dev = 0, major = 0, sms = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) return SHARQ_ECUDA;
+  if (cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess ||
+      cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
+    return SHARQ_ECUDA;
+  if (major != 10) return SHARQ_EARCH;
+  void* scratch = nullptr;
+  const sharq_status s = static_scratch_ptr(dev, &scratch);
+  if (s != SHARQ_OK) return s;
+  // nothing in the scratch has to start at zero: rows 0 .. T-1 of the bf16 operand copy are rewritten by every call
+  // before the GEMM reads them; the pad rows up to roundup(T, 128) keep an earlier call's bytes and only feed
+  // accumulator rows that are never stored
+  LinearArgs a{T, D, K, sp_codes, sp_sf, sp_meta, dn_codes, dn_sf, nullptr, row_scale, w_codes, w_sf_sparse_view,
+               w_sf_dense_view, w_tensor_scale, bias, Y, ldy, out_dtype, path};
+  return launch_linear_hif4(a, scratch, kHif4StaticScratchBytes, sms, (cudaStream_t)stream);
+}
