@@ -377,7 +377,7 @@ sharq_status sharq_linear_plan(const sharq_config* cfg, int64_t T, int64_t D, in
     s = launch_linear(cfg, a, E, nullptr, nullptr, 0, di.sms, di.dev, nullptr, &pl);
     if (s != SHARQ_OK) return s;
   }
-  static const char* const kinds[] = {"tile", "pair", "grouped-mc", "hif4-bf16", "tile+prepare"};
+  static const char* const kinds[] = {"tile", "pair", "grouped-mc", "hif4-bf16", "tile+prepare", "grouped-pair"};
   if (pl.kind < 0) snprintf(buf, n, "none");
   else snprintf(buf, n, "%s bn=%d act_rows=%d splits=%d stages=%d tiles=%lld grid=%lld cluster=%d", kinds[pl.kind],
                 pl.bn, pl.act_rows, pl.splits, pl.stages, (long long)pl.tiles, (long long)pl.grid, pl.cluster);

@@ -703,6 +703,8 @@ struct PairStage {
   static constexpr int BYTES = (RAW + 1023) / 1024 * 1024;
   static constexpr int STAGES = 4;
   static constexpr int SMEM = STAGES * BYTES + 1024 + 256;
+  static constexpr int GRP = 3 * (kMaxExperts + 1) * 4 + 16;      // grouped: offs, pair prefix, block prefix per expert
+  static constexpr int SMEM_GROUPED = SMEM + GRP;
   static constexpr int ACC_STAGES = PBN <= 192 ? 2 : 1;
   static constexpr int SFB_COLS = 8;
   static constexpr int SF0 = PBN * ACC_STAGES;           // first column after the accumulators
@@ -727,7 +729,17 @@ __device__ __forceinline__ void pair_tile(int tile, int m_pairs, int n_tiles, in
   n_blk = within / rows;
 }
 
-template <int FMT, int PBN>
+// One unit of work of the pair kernel: which 128-row block this CTA contributes, which n-tile, how many of its rows
+// are real, and (grouped) which expert's weights.
+struct PairUnit { int m_blk, n_blk, rows_valid, expert; };
+
+// GROUPED = true (sharq_linear_grouped, MoE experts with more than 128 rows): a pair works on two consecutive 128-row
+// blocks of ONE expert (the second block may not exist: its CTA then contributes rows that are never stored) and on
+// that expert's weight rows.  Tiles run n-fastest inside a pair, so the clusters running at the same time share a few
+// experts' activation blocks (L2) and every weight tile is read from DRAM by exactly one cluster.  The expert table
+// (row offsets, prefix of pairs, prefix of 128-row blocks in the padded row numbering) is built by every CTA in its
+// own shared memory from the DEVICE array `offsets`.
+template <int FMT, int PBN, bool GROUPED = false>
 __global__ void __launch_bounds__(kThreads, 1)
 sharq_linear_pair_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_constant__ CUtensorMap tm_a_dn,
                          const __grid_constant__ CUtensorMap tm_w, const __grid_constant__ CUtensorMap tm_sfa_sp,
@@ -749,11 +761,13 @@ sharq_linear_pair_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __gr
   const int rank = (int)tc::cluster_ctarank();
   const bool do_sp = p.path != 2, do_dn = p.path != 1;
   const int num_kb = p.K / BK;
-  const int m_pairs = (p.m_blocks + 1) / 2;
+  int m_pairs = (p.m_blocks + 1) / 2;
   const int n_tiles = (p.D + S::BN - 1) / S::BN;                // the last tile may be ragged in N
-  const int total = m_pairs * n_tiles;
   const int gm = p.group_m > 0 && p.group_m < m_pairs ? p.group_m : m_pairs;
   const int tile0 = (int)tc::cluster_id_x(), tile_step = (int)(gridDim.x >> 1);
+  const int32_t* g_offs = reinterpret_cast<const int32_t*>(smem_raw + (bars + 256u - smem_u32(smem_raw)));
+  const int32_t* g_ppref = g_offs + (kMaxExperts + 1);
+  const int32_t* g_bpref = g_ppref + (kMaxExperts + 1);
 
   if (warp == 0 && lane == 0) {
     tc::prefetch_tmap(&tm_a_sp);
@@ -785,6 +799,69 @@ sharq_linear_pair_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __gr
   asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_ptr_smem));
   tc::grid_launch_dependents();
   tc::grid_dependency_wait();
+  if constexpr (GROUPED) {
+    int32_t* offs = const_cast<int32_t*>(g_offs);
+    int32_t* ppref = const_cast<int32_t*>(g_ppref);
+    int32_t* bpref = const_cast<int32_t*>(g_bpref);
+    for (int i = threadIdx.x; i <= p.E; i += kThreads) offs[i] = p.offsets[i];
+    __syncthreads();
+    if (warp == 0) {
+      const int per = (p.E + 31) / 32;                 // lane l scans experts [l * per, l * per + per)
+      int sp = 0, sb = 0;
+      for (int i = 0; i < per; ++i) {
+        const int e = lane * per + i;
+        if (e < p.E) {
+          const int c = max(offs[e + 1] - offs[e], 0);
+          sp += (c + 2 * BM - 1) / (2 * BM);
+          sb += (c + BM - 1) / BM;
+        }
+      }
+      int ip = sp, ib = sb;
+#pragma unroll
+      for (int d = 1; d < 32; d <<= 1) {
+        const int tp = __shfl_up_sync(0xffffffffu, ip, d), tb = __shfl_up_sync(0xffffffffu, ib, d);
+        if (lane >= d) { ip += tp; ib += tb; }
+      }
+      int rp = ip - sp, rb = ib - sb;
+      for (int i = 0; i < per; ++i) {
+        const int e = lane * per + i;
+        if (e < p.E) {
+          ppref[e] = rp; bpref[e] = rb;
+          const int c = max(offs[e + 1] - offs[e], 0);
+          rp += (c + 2 * BM - 1) / (2 * BM);
+          rb += (c + BM - 1) / BM;
+        }
+      }
+      if (lane == 31) { ppref[p.E] = ip; bpref[p.E] = ib; }
+    }
+    __syncthreads();
+    m_pairs = g_ppref[p.E];
+  }
+  const int total = m_pairs * n_tiles;
+  auto unit_of = [&](int tile) {
+    PairUnit u;
+    if constexpr (GROUPED) {
+      const int gp = tile / n_tiles;
+      u.n_blk = tile - gp * n_tiles;
+      int lo = 0, hi = p.E - 1;                        // last expert whose first pair is <= gp
+      while (lo < hi) {
+        const int mid = (lo + hi + 1) >> 1;
+        if (g_ppref[mid] <= gp) lo = mid; else hi = mid - 1;
+      }
+      u.expert = lo;
+      const int b = 2 * (gp - g_ppref[lo]) + rank;     // this CTA's block inside the expert
+      u.m_blk = g_bpref[lo] + b;
+      const int left = (g_offs[lo + 1] - g_offs[lo]) - b * BM;
+      u.rows_valid = (u.m_blk < p.m_blocks) ? max(0, min(BM, left)) : 0;     // never beyond the caller's buffers
+    } else {
+      int m_pair;
+      pair_tile(tile, m_pairs, n_tiles, gm, m_pair, u.n_blk);
+      u.m_blk = 2 * m_pair + rank;
+      u.expert = 0;
+      u.rows_valid = max(0, min(BM, p.T - u.m_blk * BM));
+    }
+    return u;
+  };
 
   if (warp == 0) {
     // =========================== TMA producer (both CTAs) ===================================
@@ -800,11 +877,10 @@ sharq_linear_pair_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __gr
       const int kq = p.K / 256;
       uint32_t it = 0;
       for (int tile = tile0; tile < total; tile += tile_step) {
-        int m_pair, n_blk;
-        pair_tile(tile, m_pairs, n_tiles, gm, m_pair, n_blk);
-        const int m_blk = 2 * m_pair + rank;
+        const PairUnit u = unit_of(tile);
+        const int m_blk = u.m_blk, n_blk = u.n_blk;
         const int m_sf = min(m_blk, p.m_blocks - 1);       // a ragged pair's second CTA: valid memory, unused rows
-        const int n0 = n_blk * S::BN;
+        const int n0 = u.expert * p.D + n_blk * S::BN;     // first weight row of the tile (stacked experts)
         const int wblk0 = n0 / 128;
         for (int kb = 0; kb < num_kb; ++kb, ++it) {
           const int s = it % S::STAGES;
@@ -839,8 +915,13 @@ sharq_linear_pair_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __gr
       for (int tile = tile0; tile < total; tile += tile_step, ++n_unit) {
         const uint32_t as = n_unit % S::ACC_STAGES;
         const uint32_t acc = tmem_base + as * S::BN;
-        int m_pair_u, n_blk_u;
-        pair_tile(tile, m_pairs, n_tiles, gm, m_pair_u, n_blk_u);
+        int n_blk_u;
+        if constexpr (GROUPED) {
+          n_blk_u = tile % n_tiles;
+        } else {
+          int m_pair_u;
+          pair_tile(tile, m_pairs, n_tiles, gm, m_pair_u, n_blk_u);
+        }
         const uint32_t sfb_shift = (uint32_t)(((n_blk_u * S::BN) % 128) / 32);   // tile starts inside a 128-row atom
         tc::mbar_wait(tmem_empty_bar(as), ((n_unit / S::ACC_STAGES) & 1u) ^ 1u);   // both CTAs' epilogues drained it
         tc::tc_fence_after();
@@ -904,12 +985,11 @@ sharq_linear_pair_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __gr
     const uint32_t lane_addr = tmem_base + ((uint32_t)(sub * 32) << 16);
     uint32_t n_unit = 0;
     for (int tile = tile0; tile < total; tile += tile_step, ++n_unit) {
-      int m_pair, n_blk;
-      pair_tile(tile, m_pairs, n_tiles, gm, m_pair, n_blk);
-      const int m_blk = 2 * m_pair + rank;
-      const int64_t row = (int64_t)m_blk * BM + r_local;
-      const bool row_ok = row < p.T;
-      const float scale = row_ok ? __fmul_rn(p.row_scale[row], p.w_ts[0]) : 0.0f;
+      const PairUnit u = unit_of(tile);
+      const int n_blk = u.n_blk;
+      const int64_t row = (int64_t)u.m_blk * BM + r_local;
+      const bool row_ok = r_local < u.rows_valid;
+      const float scale = row_ok ? __fmul_rn(p.row_scale[row], p.w_ts[u.expert]) : 0.0f;
       const uint32_t as = n_unit % S::ACC_STAGES;
       tc::mbar_wait(tmem_full_bar(as), (n_unit / S::ACC_STAGES) & 1u);
       tc::tc_fence_after();
@@ -1138,29 +1218,33 @@ bool make_map_rows1k(CUtensorMap* m, const void* base, uint64_t bytes, uint32_t 
             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
-template <int FMT, int PBN>
+template <int FMT, int PBN, bool GROUPED = false>
 sharq_status launch_pair(const LinearArgs& a, const KParams& p, const CUtensorMap& tm_sp, const CUtensorMap& tm_dn,
                          int64_t m_blocks, const LaunchEnv& env) {
   using P = PairStage<FMT, PBN>;
-  const int64_t pair_tiles = ((m_blocks + 1) / 2) * ((a.D + PBN - 1) / PBN);
+  constexpr int kSmem = GROUPED ? P::SMEM_GROUPED : P::SMEM;
+  const int64_t n_tiles = (a.D + PBN - 1) / PBN;
+  // grouped: the real number of pairs is only known on the device; an upper bound sizes the persistent grid
+  const int64_t pair_tiles = (GROUPED ? (m_blocks + 1) / 2 + p.E : (m_blocks + 1) / 2) * n_tiles;
   int64_t clusters = pair_tiles < env.num_sms / 2 ? pair_tiles : env.num_sms / 2;
   if (debug_env().pair_clusters > 0 && debug_env().pair_clusters < clusters) clusters = debug_env().pair_clusters;
-  if (env.plan_only) { fill_plan(env.plan_only, 1, PBN, 128, 1, P::STAGES, pair_tiles, 2 * clusters, 2); return SHARQ_OK; }
+  if (env.plan_only) { fill_plan(env.plan_only, GROUPED ? 5 : 1, PBN, 128, 1, P::STAGES, pair_tiles, 2 * clusters, 2); return SHARQ_OK; }
   CUtensorMap tm_wp, tm_sfa_sp, tm_sfa_dn, tm_meta, tm_sfb_sp, tm_sfb_dn;
   const uint64_t act_rows = (uint64_t)m_blocks * 128, kk = (uint64_t)a.K;
   const uint32_t dn_rows = P::SF_DN_BYTES / 1024;
   const uint64_t dn_div = (FMT == SHARQ_NVFP4) ? 16 : 32;
-  const uint64_t w_rows_pad = (uint64_t)round_up(a.D, 128);       // the scale views are padded to whole 128-row atoms
-  if (!make_map(&tm_wp, a.w_codes, (uint64_t)a.D, kk / 2, 128, P::HALF) ||
+  const uint64_t w_rows = (uint64_t)a.D * (uint64_t)(GROUPED ? p.E : 1);                // stacked experts
+  const uint64_t w_rows_pad = (uint64_t)round_up((int64_t)w_rows, 128);   // the scale views are padded to whole 128-row atoms
+  if (!make_map(&tm_wp, a.w_codes, w_rows, kk / 2, 128, P::HALF) ||
       !make_map_rows1k(&tm_sfa_sp, a.sp_sf, act_rows * kk / 32, 1) ||
       !make_map_rows1k(&tm_sfa_dn, a.dn_sf, act_rows * kk / dn_div, dn_rows) ||
       !make_map_rows1k(&tm_meta, a.sp_meta, act_rows * kk / 16, 2) ||
       !make_map_rows1k(&tm_sfb_sp, a.w_sf_sp, w_rows_pad * kk / 32, 1) ||
       !make_map_rows1k(&tm_sfb_dn, a.w_sf_dn, w_rows_pad * kk / dn_div, dn_rows))
     return SHARQ_ECUDA;
-  auto kfn = sharq_linear_pair_kernel<FMT, PBN>;
+  auto kfn = sharq_linear_pair_kernel<FMT, PBN, GROUPED>;
   static std::atomic<uint64_t> smem_set{0};
-  if (set_smem_once(smem_set, (const void*)kfn, P::SMEM, env.dev) != cudaSuccess) return SHARQ_ECUDA;
+  if (set_smem_once(smem_set, (const void*)kfn, kSmem, env.dev) != cudaSuccess) return SHARQ_ECUDA;
   cudaLaunchConfig_t lp{};
   cudaLaunchAttribute at[2];
   at[0].id = cudaLaunchAttributeClusterDimension;
@@ -1171,7 +1255,7 @@ sharq_status launch_pair(const LinearArgs& a, const KParams& p, const CUtensorMa
   at[1].val.programmaticStreamSerializationAllowed = debug_env().no_pdl ? 0 : 1;
   lp.blockDim = dim3(kThreads);
   lp.gridDim = dim3((unsigned)(2 * clusters));
-  lp.dynamicSmemBytes = P::SMEM;
+  lp.dynamicSmemBytes = kSmem;
   lp.stream = env.st;
   lp.attrs = at;
   lp.numAttrs = 2;
@@ -1232,6 +1316,12 @@ sharq_status launch_tiles(const LinearArgs& a, int64_t rows_total, int64_t m_blo
     return launch_pair<FMT, 192>(a, p, tm_sp, tm_dn, m_blocks, env);
   }
   if constexpr (BN == 128) {
+    // experts with (on average) well over 128 rows AND a long K: CTA-pair tiles, two row blocks of one expert x 192
+    // columns per pair (half the weight bytes staged per CTA, M = 256 MMAs).  Short K-loops (BASELINE configs[4]:
+    // K = 2048 / 768, 8 / 3 k-blocks per tile) are bound by the per-tile drain and store, not by the MMAs: measured
+    // 134 / 114 us with pair tiles against 127 / 86 us with the 128-row multicast tiles below, so those stay there.
+    if (E > 0 && rows_total / E >= 192 && a.K >= 4096 && !debug_env().no_pair)
+      return launch_pair<FMT, 192, true>(a, p, tm_sp, tm_dn, m_blocks, env);
     // experts: n-tiles of one 128-row block are consecutive (decode_unit), so tiles 2j and 2j+1 share activations
     if (E > 0 && n_tiles % 2 == 0 && !debug_env().no_mc) return launch_mc<FMT>(p, tm_sp, tm_dn, tm_w, tiles, env);
   }

@@ -296,6 +296,7 @@ def test_linear_plan_names_the_variants_the_tests_cover(sq):
     assert plans["o_T4096"].startswith("pair "), plans
     assert plans["down_T4096"].startswith("pair "), plans
     assert plans["moe_gate_up"].startswith("grouped-mc") and plans["moe_down"].startswith("grouped-mc"), plans
+    assert sq.linear_plan(cfg, 40576, 1536, 4096, 128).startswith("grouped-pair")   # long K, > 192 rows per expert
     assert sq.linear_plan(sq.make_config(2, 0), 4096, 3584, 18944).startswith("hif4-bf16")
 
 
@@ -303,13 +304,15 @@ def test_linear_grouped_device_offsets_and_spare_capacity(sq):
     """sharq_linear_grouped reads `offsets` on the DEVICE (no host copy): a device tensor, buffers larger than the
     padded total (roundup(total, 128) + 128 E), an odd number of n-tiles (the non-multicast grouped path) and a
     capacity that is too SMALL (extra row blocks are skipped, nothing is written beyond the buffers)."""
-    E, K = 5, 512
+    E = 5
     counts = [3, 0, 257, 128, 64]
     offsets = np.concatenate([[0], np.cumsum(counts)]).astype(np.int32)
     pad_off = np.concatenate([[0], np.cumsum([-(-c // 128) * 128 for c in counts])])
     cap = int(-(-offsets[-1] // 128) * 128 + 128 * E)
     cfg = sq.make_config(sq.NVFP4, sq.NORM_NONE, 1e-6, sq.LAYOUT_TILED)
-    for D in (256, 384):                                            # 2 n-tiles (multicast clusters) / 3 (plain persistent)
+    # 2 n-tiles (multicast clusters) / 3 (plain persistent) / long K: CTA-pair tiles on two row blocks of one expert,
+    # ragged last n-tile (D = 256 with 192-wide tiles reads the next expert's weight rows, never stored)
+    for D, K in ((256, 512), (384, 512), (256, 4096)):
         act = sq.alloc_act(cfg, cap, K, "cuda")
         ws, xs = [], []
         for e in range(E):
@@ -321,6 +324,8 @@ def test_linear_grouped_device_offsets_and_spare_capacity(sq):
         wq = dict(codes=torch.cat([q["codes"] for q in wqs]), sf_sp=torch.cat([q["sf_sp"] for q in wqs]),
                   sf_dn=torch.cat([q["sf_dn"] for q in wqs]), ts_w=torch.cat([q["ts_w"] for q in wqs]), D=D, K=K)
         offs_dev = torch.from_numpy(offsets).cuda()
+        assert sq.linear_plan(cfg, cap, D, K, E).startswith("grouped-pair") == (K >= 4096)   # 230 rows of capacity per expert
+        assert not sq.linear_plan(cfg, 4 * 128, D, K, E).startswith("grouped-pair")
         Y = torch.full((cap, D), 7.0, dtype=torch.float32, device="cuda")
         sq.linear_grouped(cfg, offs_dev, act, wq, D, Y=Y)
         torch.cuda.synchronize()
