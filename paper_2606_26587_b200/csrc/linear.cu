@@ -41,6 +41,7 @@ __device__ long long g_dbg_ts[1024 * 16];
 #define SHARQ_TS(i) do { } while (0)
 #endif
 constexpr int kTmemCols = 512;
+constexpr int kStageBytes = 4 * 4096;      // epilogue staging: 4 KB for each of the four epilogue warps
 
 // Grouped (MoE) launches: the expert table is built by every CTA in its own shared memory from the DEVICE array
 // `offsets` (no host copy of the routing result, no device -> host synchronisation after the router):
@@ -105,9 +106,10 @@ struct Stage {
   static constexpr int RECV = SPLIT ? (NSL + 2) * AR * 64 : 0;        // [src][slot][AR rows][16 fp32]; S*ceil(NSL/S) <= NSL+2 for S in {2,3,4,8}
   static constexpr int PAD = AR < 128 ? 128 * 128 : 0;               // the MMA's over-read behind the last stage
   static constexpr int GRP = (!SPLIT && AR == 128 && BN == 128) ? 2 * (kMaxExperts + 1) * 4 + 8 : 0;   // expert table (grouped)
-  static constexpr int FIT = (232448 - 1024 - 256 - RECV - PAD - GRP - EXTRA) / BYTES;
+  static constexpr int STG = SPLIT ? 0 : kStageBytes;                  // epilogue staging (persistent variants)
+  static constexpr int FIT = (232448 - 1024 - 256 - RECV - PAD - GRP - EXTRA - STG) / BYTES;
   static constexpr int STAGES = FIT > 8 ? 8 : FIT;
-  static constexpr int SMEM = STAGES * BYTES + PAD + RECV + 1024 /*alignment slack*/ + 256 /*barriers*/ + GRP + EXTRA;
+  static constexpr int SMEM = STAGES * BYTES + PAD + RECV + 1024 /*alignment slack*/ + 256 /*barriers*/ + GRP + EXTRA + STG;
   // tensor-memory columns: two accumulator stages, then metadata and scale factors
   static constexpr int SFB_COLS = NB * 4;          // columns one MMA's B scales occupy
   static constexpr int ACC_STAGES = BN > 128 ? 1 : 2;
@@ -199,6 +201,78 @@ __device__ __forceinline__ void store_row(const KParams& p, int64_t row, int col
   }
 }
 
+// ---- epilogue through shared memory (persistent tiles and CTA pairs) ------------------------------------------
+// tcgen05.ld hands every thread 32 consecutive columns of ITS row, so direct stores are 32 rows x 16 bytes per warp
+// instruction: 32 half-filled sectors, and the LSU becomes the bound of short-K tiles (MoE experts: the tile's stores
+// cost 31 % of the down projection).  Instead each epilogue warp stages 128 bytes per row (64 bf16 or 32 fp32 columns)
+// of its 32 rows in its own 4 KB of shared memory (16-byte chunks XOR-swizzled by the row, conflict free both ways)
+// and writes them back transposed: one warp instruction = 4 rows x one full 128-byte line.
+
+__device__ __forceinline__ uint32_t stg_addr(uint32_t base, int r, int ch) {
+  return base + (uint32_t)r * 128u + ((uint32_t)(ch ^ (r & 7)) << 4);
+}
+
+// y = acc * scale (+ bias) for the 32 columns col0 .. col0 + 31 of this thread's row, into the staging row `lane`;
+// slot = which half of the 128 staged bytes a bf16 chunk takes (fp32: the whole row)
+__device__ __forceinline__ void epilogue_stage32(const KParams& p, uint32_t stg, int lane, int col0, int slot, float scale,
+                                                 const uint32_t (&v)[32]) {
+  float f[32];
+#pragma unroll
+  for (int i = 0; i < 32; ++i) f[i] = __fmul_rn(__uint_as_float(v[i]), scale);
+  if (p.bias) {
+    const int ncols = p.D - col0;                     // < 32 only on a ragged last n-tile
+    const uint16_t* b = p.bias + col0;
+#pragma unroll
+    for (int i = 0; i < 32; ++i)
+      if (i < ncols) f[i] = __fadd_rn(f[i], __uint_as_float((uint32_t)b[i] << 16));
+  }
+  if (p.out_fp32) {
+#pragma unroll
+    for (int j = 0; j < 8; ++j) tc::st_shared_v4(stg_addr(stg, lane, j), f[4 * j], f[4 * j + 1], f[4 * j + 2], f[4 * j + 3]);
+  } else {
+#pragma unroll
+    for (int j = 0; j < 4; ++j)
+      tc::st_shared_v4(stg_addr(stg, lane, 4 * slot + j),
+                       __uint_as_float(pack_bf16x2_rn(f[8 * j], f[8 * j + 1])), __uint_as_float(pack_bf16x2_rn(f[8 * j + 2], f[8 * j + 3])),
+                       __uint_as_float(pack_bf16x2_rn(f[8 * j + 4], f[8 * j + 5])), __uint_as_float(pack_bf16x2_rn(f[8 * j + 6], f[8 * j + 7])));
+  }
+}
+
+// the staged 32 rows x 128 bytes -> Y: rows row0 .. row0 + rows_ok - 1, columns from colbase, D-guarded per 16 bytes
+__device__ __forceinline__ void epilogue_flush(const KParams& p, uint32_t stg, int lane, int64_t row0, int rows_ok, int colbase) {
+  const int ch = lane & 7;
+  const int col = colbase + ch * (p.out_fp32 ? 4 : 8);
+  uint8_t* ybase = static_cast<uint8_t*>(p.Y) + (size_t)col * (p.out_fp32 ? 4 : 2);
+  const size_t pitch = (size_t)p.ldy * (p.out_fp32 ? 4 : 2);
+#pragma unroll
+  for (int i = 0; i < 8; ++i) {
+    const int rr = 4 * i + (lane >> 3);
+    if (rr < rows_ok && col < p.D) {
+      const float4 t = tc::ld_shared_v4(stg_addr(stg, rr, ch));
+      *reinterpret_cast<float4*>(ybase + (size_t)(row0 + rr) * pitch) = t;
+    }
+  }
+}
+
+// all BN columns of one accumulator stage of this warp's 32 rows
+template <int BN>
+__device__ __forceinline__ void epilogue_tile(const KParams& p, uint32_t taddr, uint32_t stg, int lane, int64_t row0, int rows_ok,
+                                              int n0, float scale) {
+#pragma unroll 1
+  for (int c = 0; c < BN / 32; ++c) {
+    uint32_t v[32];
+    tc::tmem_ld32(taddr + c * 32, v);
+    tc::tmem_ld_wait();
+    const bool second = !p.out_fp32 && (c & 1);
+    epilogue_stage32(p, stg, lane, n0 + c * 32, second ? 1 : 0, scale, v);
+    if (p.out_fp32 || second) {
+      __syncwarp();
+      epilogue_flush(p, stg, lane, row0, rows_ok, n0 + (second ? c - 1 : c) * 32);
+      __syncwarp();
+    }
+  }
+}
+
 // MC = true (grouped GEMM): a cluster of two CTAs works on two neighbouring n-tiles of the same 128-row block in
 // lock step; each CTA fetches half of the shared activation operands and multicasts them to both (the many
 // short tiles of the expert GEMMs are bound by L2 -> SM traffic, 60 % of which is the activation side).
@@ -233,6 +307,7 @@ __device__ __forceinline__ void linear_body(const CUtensorMap* tm_a_sp_p, const 
   const uint32_t act_bar = bars + 8u * (2 * S::STAGES + 5);          // FUSED: this CTA's prepared operands are in memory
   int32_t* grp_tab = reinterpret_cast<int32_t*>(smem_raw + (bars + 256u - smem_u32(smem_raw)));   // offs[E+1], pref[E+1]
   uint8_t* prep_smem = smem_raw + (bars + 256u + (uint32_t)S::GRP - smem_u32(smem_raw));          // FUSED: prepare_rows' scratch
+  const uint32_t stg_base = bars + 256u + (uint32_t)S::GRP + (FUSED ? (uint32_t)kPrepSmem : 0u);     // epilogue staging
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   if (warp == 0) SHARQ_TS(0);
@@ -524,18 +599,8 @@ __device__ __forceinline__ void linear_body(const CUtensorMap* tm_a_sp_p, const 
         const float scale = row_ok ? __fmul_rn(FUSED ? __ldcg(p.row_scale + row) : p.row_scale[row], p.w_ts[u.expert]) : 0.0f;
         tc::mbar_wait(tmem_full_bar(as), (n_unit / S::ACC_STAGES) & 1u);
         tc::tc_fence_after();
-#pragma unroll 1
-        for (int c = 0; c < BN / 32; ++c) {
-          uint32_t v[32];
-          tc::tmem_ld32(lane_addr + as * BN + c * 32, v);
-          tc::tmem_ld_wait();
-          if (row_ok) {
-            float f[32];
-#pragma unroll
-            for (int i = 0; i < 32; ++i) f[i] = __uint_as_float(v[i]);
-            store_row<32>(p, row, u.n_blk * BN + c * 32, scale, f);
-          }
-        }
+        epilogue_tile<BN>(p, lane_addr + as * BN, stg_base + (uint32_t)sub * 4096u, lane, (int64_t)u.m_blk * BM + sub * 32,
+                          min(32, max(0, u.rows_valid - sub * 32)), u.n_blk * BN, scale);
         tc::tc_fence_before();
         __syncwarp();
         if (lane == 0) tc::mbar_arrive(tmem_empty_bar(as));
@@ -702,7 +767,7 @@ struct PairStage {
   static constexpr int RAW = SFB_DN + 2 * SF_DN_BYTES;
   static constexpr int BYTES = (RAW + 1023) / 1024 * 1024;
   static constexpr int STAGES = 4;
-  static constexpr int SMEM = STAGES * BYTES + 1024 + 256;
+  static constexpr int SMEM = STAGES * BYTES + 1024 + 256 + kStageBytes;
   static constexpr int GRP = 3 * (kMaxExperts + 1) * 4 + 16;      // grouped: offs, pair prefix, block prefix per expert
   static constexpr int SMEM_GROUPED = SMEM + GRP;
   static constexpr int ACC_STAGES = PBN <= 192 ? 2 : 1;
@@ -765,7 +830,8 @@ sharq_linear_pair_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __gr
   const int n_tiles = (p.D + S::BN - 1) / S::BN;                // the last tile may be ragged in N
   const int gm = p.group_m > 0 && p.group_m < m_pairs ? p.group_m : m_pairs;
   const int tile0 = (int)tc::cluster_id_x(), tile_step = (int)(gridDim.x >> 1);
-  const int32_t* g_offs = reinterpret_cast<const int32_t*>(smem_raw + (bars + 256u - smem_u32(smem_raw)));
+  const uint32_t stg_base = bars + 256u;                                    // epilogue staging, then the grouped tables
+  const int32_t* g_offs = reinterpret_cast<const int32_t*>(smem_raw + (bars + 256u + (uint32_t)kStageBytes - smem_u32(smem_raw)));
   const int32_t* g_ppref = g_offs + (kMaxExperts + 1);
   const int32_t* g_bpref = g_ppref + (kMaxExperts + 1);
 
@@ -993,18 +1059,8 @@ sharq_linear_pair_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __gr
       const uint32_t as = n_unit % S::ACC_STAGES;
       tc::mbar_wait(tmem_full_bar(as), (n_unit / S::ACC_STAGES) & 1u);
       tc::tc_fence_after();
-#pragma unroll 1
-      for (int c = 0; c < S::BN / 32; ++c) {
-        uint32_t v[32];
-        tc::tmem_ld32(lane_addr + as * S::BN + c * 32, v);
-        tc::tmem_ld_wait();
-        if (row_ok && n_blk * S::BN + c * 32 < p.D) {
-          float f[32];
-#pragma unroll
-          for (int i = 0; i < 32; ++i) f[i] = __uint_as_float(v[i]);
-          store_row<32>(p, row, n_blk * S::BN + c * 32, scale, f);
-        }
-      }
+      epilogue_tile<S::BN>(p, lane_addr + as * S::BN, stg_base + (uint32_t)sub * 4096u, lane, (int64_t)u.m_blk * BM + sub * 32,
+                           min(32, max(0, u.rows_valid - sub * 32)), n_blk * S::BN, scale);
       tc::tc_fence_before();
       __syncwarp();
       if (lane == 0) tc::mbar_arrive_cluster(tc::map_to_cta(tmem_empty_bar(as), 0));
