@@ -24,6 +24,7 @@
 #include "linear_args.h"
 #include "prepare_device.cuh"
 #include "tc_ptx.cuh"
+#include "epilogue.cuh"
 
 namespace sharq {
 
@@ -41,7 +42,6 @@ __device__ long long g_dbg_ts[1024 * 16];
 #define SHARQ_TS(i) do { } while (0)
 #endif
 constexpr int kTmemCols = 512;
-constexpr int kStageBytes = 4 * 4096;      // epilogue staging: 4 KB for each of the four epilogue warps
 
 // Grouped (MoE) launches: the expert table is built by every CTA in its own shared memory from the DEVICE array
 // `offsets` (no host copy of the routing result, no device -> host synchronisation after the router):
@@ -198,78 +198,6 @@ __device__ __forceinline__ void store_row(const KParams& p, int64_t row, int col
       if (8 * i < ncols)
         dst[i] = make_uint4(pack_bf16x2_rn(f[8 * i], f[8 * i + 1]), pack_bf16x2_rn(f[8 * i + 2], f[8 * i + 3]),
                             pack_bf16x2_rn(f[8 * i + 4], f[8 * i + 5]), pack_bf16x2_rn(f[8 * i + 6], f[8 * i + 7]));
-  }
-}
-
-// ---- epilogue through shared memory (persistent tiles and CTA pairs) ------------------------------------------
-// tcgen05.ld hands every thread 32 consecutive columns of ITS row, so direct stores are 32 rows x 16 bytes per warp
-// instruction: 32 half-filled sectors, and the LSU becomes the bound of short-K tiles (MoE experts: the tile's stores
-// cost 31 % of the down projection).  Instead each epilogue warp stages 128 bytes per row (64 bf16 or 32 fp32 columns)
-// of its 32 rows in its own 4 KB of shared memory (16-byte chunks XOR-swizzled by the row, conflict free both ways)
-// and writes them back transposed: one warp instruction = 4 rows x one full 128-byte line.
-
-__device__ __forceinline__ uint32_t stg_addr(uint32_t base, int r, int ch) {
-  return base + (uint32_t)r * 128u + ((uint32_t)(ch ^ (r & 7)) << 4);
-}
-
-// y = acc * scale (+ bias) for the 32 columns col0 .. col0 + 31 of this thread's row, into the staging row `lane`;
-// slot = which half of the 128 staged bytes a bf16 chunk takes (fp32: the whole row)
-__device__ __forceinline__ void epilogue_stage32(const KParams& p, uint32_t stg, int lane, int col0, int slot, float scale,
-                                                 const uint32_t (&v)[32]) {
-  float f[32];
-#pragma unroll
-  for (int i = 0; i < 32; ++i) f[i] = __fmul_rn(__uint_as_float(v[i]), scale);
-  if (p.bias) {
-    const int ncols = p.D - col0;                     // < 32 only on a ragged last n-tile
-    const uint16_t* b = p.bias + col0;
-#pragma unroll
-    for (int i = 0; i < 32; ++i)
-      if (i < ncols) f[i] = __fadd_rn(f[i], __uint_as_float((uint32_t)b[i] << 16));
-  }
-  if (p.out_fp32) {
-#pragma unroll
-    for (int j = 0; j < 8; ++j) tc::st_shared_v4(stg_addr(stg, lane, j), f[4 * j], f[4 * j + 1], f[4 * j + 2], f[4 * j + 3]);
-  } else {
-#pragma unroll
-    for (int j = 0; j < 4; ++j)
-      tc::st_shared_v4(stg_addr(stg, lane, 4 * slot + j),
-                       __uint_as_float(pack_bf16x2_rn(f[8 * j], f[8 * j + 1])), __uint_as_float(pack_bf16x2_rn(f[8 * j + 2], f[8 * j + 3])),
-                       __uint_as_float(pack_bf16x2_rn(f[8 * j + 4], f[8 * j + 5])), __uint_as_float(pack_bf16x2_rn(f[8 * j + 6], f[8 * j + 7])));
-  }
-}
-
-// the staged 32 rows x 128 bytes -> Y: rows row0 .. row0 + rows_ok - 1, columns from colbase, D-guarded per 16 bytes
-__device__ __forceinline__ void epilogue_flush(const KParams& p, uint32_t stg, int lane, int64_t row0, int rows_ok, int colbase) {
-  const int ch = lane & 7;
-  const int col = colbase + ch * (p.out_fp32 ? 4 : 8);
-  uint8_t* ybase = static_cast<uint8_t*>(p.Y) + (size_t)col * (p.out_fp32 ? 4 : 2);
-  const size_t pitch = (size_t)p.ldy * (p.out_fp32 ? 4 : 2);
-#pragma unroll
-  for (int i = 0; i < 8; ++i) {
-    const int rr = 4 * i + (lane >> 3);
-    if (rr < rows_ok && col < p.D) {
-      const float4 t = tc::ld_shared_v4(stg_addr(stg, rr, ch));
-      *reinterpret_cast<float4*>(ybase + (size_t)(row0 + rr) * pitch) = t;
-    }
-  }
-}
-
-// all BN columns of one accumulator stage of this warp's 32 rows
-template <int BN>
-__device__ __forceinline__ void epilogue_tile(const KParams& p, uint32_t taddr, uint32_t stg, int lane, int64_t row0, int rows_ok,
-                                              int n0, float scale) {
-#pragma unroll 1
-  for (int c = 0; c < BN / 32; ++c) {
-    uint32_t v[32];
-    tc::tmem_ld32(taddr + c * 32, v);
-    tc::tmem_ld_wait();
-    const bool second = !p.out_fp32 && (c & 1);
-    epilogue_stage32(p, stg, lane, n0 + c * 32, second ? 1 : 0, scale, v);
-    if (p.out_fp32 || second) {
-      __syncwarp();
-      epilogue_flush(p, stg, lane, row0, rows_ok, n0 + (second ? c - 1 : c) * 32);
-      __syncwarp();
-    }
   }
 }
 
@@ -777,22 +705,6 @@ struct PairStage {
                        SFB_DN_COL = SF0 + 44;
   static_assert(SF0 + 76 <= 512, "tensor memory");
 };
-
-// Tile order of the pair kernel.  Tiles run m-fastest inside a SUPERTILE of `gm` 256-row blocks x all n-tiles: the
-// concurrently running clusters then touch gm activation blocks (which stay in L2 for the whole supertile, read from
-// DRAM once) and one or two W tiles at a time.  gm = all row blocks reproduces the plain m-fastest order (right when
-// the whole activation operand fits in L2); with a long K and many tokens (down projection at T = 8192: 106 MB of
-// activation operands) the plain order cycled the whole operand through L2 once per two n-tiles: 782 MB of DRAM
-// reads for 137 MB of operands (profiles/linear_pair_r2_ncu_full.md).
-__device__ __forceinline__ void pair_tile(int tile, int m_pairs, int n_tiles, int gm, int& m_pair, int& n_blk) {
-  const int per_group = gm * n_tiles;
-  const int g = tile / per_group;
-  const int g0 = g * gm;
-  const int rows = min(gm, m_pairs - g0);              // the last supertile may be shorter
-  const int within = tile - g * per_group;
-  m_pair = g0 + within % rows;
-  n_blk = within / rows;
-}
 
 // One unit of work of the pair kernel: which 128-row block this CTA contributes, which n-tile, how many of its rows
 // are real, and (grouped) which expert's weights.

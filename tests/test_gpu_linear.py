@@ -43,6 +43,7 @@ CASES = [
     (1, 1, 16, 4096, 4096, 50.0), (1, 0, 130, 3584, 4608, 200.0), (1, 1, 5, 768, 2048, 10.0),
     # HiF4: exact bf16 emulation path (128- and 256-wide tiles, ragged T)
     (2, 1, 16, 4096, 4096, 50.0), (2, 0, 130, 768, 384, 10.0), (2, 1, 300, 3584, 512, 200.0),
+    (2, 0, 600, 768, 3328, 50.0),      # HiF4 CTA-pair bf16 tiles: 5 row blocks (ragged pair, ragged T) x 13 n-tiles
     (0, 1, 5, 33792, 256, 50.0),       # K beyond one prepare CTA; 132 k-blocks
 ]
 
