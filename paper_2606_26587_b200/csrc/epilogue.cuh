@@ -48,7 +48,8 @@ __device__ __forceinline__ void epilogue_stage32(const P& p, uint32_t stg, int l
 
 // the staged 32 rows x 128 bytes -> Y: rows row0 .. row0 + rows_ok - 1, columns from colbase, D-guarded per 16 bytes
 template <class P>
-__device__ __forceinline__ void epilogue_flush(const P& p, uint32_t stg, int lane, int64_t row0, int rows_ok, int colbase) {
+__device__ __forceinline__ void epilogue_flush(const P& p, uint32_t stg, int lane, int64_t row0, int rows_ok, int colbase,
+                                               int col_end) {
   const int ch = lane & 7;
   const int col = colbase + ch * (p.out_fp32 ? 4 : 8);
   uint8_t* ybase = static_cast<uint8_t*>(p.Y) + (size_t)col * (p.out_fp32 ? 4 : 2);
@@ -56,7 +57,7 @@ __device__ __forceinline__ void epilogue_flush(const P& p, uint32_t stg, int lan
 #pragma unroll
   for (int i = 0; i < 8; ++i) {
     const int rr = 4 * i + (lane >> 3);
-    if (rr < rows_ok && col < p.D) {
+    if (rr < rows_ok && col < col_end) {
       const float4 t = tc::ld_shared_v4(stg_addr(stg, rr, ch));
       *reinterpret_cast<float4*>(ybase + (size_t)(row0 + rr) * pitch) = t;
     }
@@ -74,9 +75,9 @@ __device__ __forceinline__ void epilogue_tile(const P& p, uint32_t taddr, uint32
     tc::tmem_ld_wait();
     const bool second = !p.out_fp32 && (c & 1);
     epilogue_stage32(p, stg, lane, n0 + c * 32, second ? 1 : 0, scale, v);
-    if (p.out_fp32 || second) {
+    if (p.out_fp32 || second || c == BN / 32 - 1) {   // (a tile of an odd number of 32-column chunks: half a staged row)
       __syncwarp();
-      epilogue_flush(p, stg, lane, row0, rows_ok, n0 + (second ? c - 1 : c) * 32);
+      epilogue_flush(p, stg, lane, row0, rows_ok, n0 + (second ? c - 1 : c) * 32, min(p.D, n0 + (c + 1) * 32));
       __syncwarp();
     }
   }

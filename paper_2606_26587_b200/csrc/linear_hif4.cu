@@ -384,6 +384,230 @@ hif4_gemm_pair_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_con
   }
 }
 
+// ---- 2:4-sparse backbone: tcgen05.mma.sp kind::f16 (SURVEY.md 8(a) S12 as written) --------------------------------
+// The backbone half of a HiF4 activation is 2:4 sparse by construction: instead of multiplying a dense
+// [T, K] bf16 matrix with explicit zeros, the survivors go in compressed, [T, K/2] bf16 in ascending k (exactly the order
+// of sp_codes), and the 2-bit indices of sharq_prepare's metadata nibbles (i0 | i1 << 2 per 4 elements) tell the
+// tensor core where they belong: half the A bytes and half the MMA time of the dense emulation for that half.
+// Metadata layout the sparse bf16 MMA expects (CUTLASS sm1xx_sparse_config.inl, TensorEAtom_MMA_F16, used as a hardware
+// spec): one 2048-byte atom per 128 rows x 128 logical k; byte of (row m, logical k) inside the atom =
+//   16 (m % 8) + 2 ((m / 8) % 2) + 256 (m / 16) + 128 ((k / 16) % 2) + 4 (k / 32) + (k % 16) / 8,
+// so that one tcgen05.cp.128x128b puts the four 32-bit columns of the four K = 32 MMAs of the atom into tensor memory.
+__global__ void hif4_dequant_act_sparse_kernel(const uint8_t* __restrict__ sp_codes, const uint32_t* __restrict__ sp_sf,
+                                               const uint8_t* __restrict__ sp_meta, const uint8_t* __restrict__ dn_codes,
+                                               const uint32_t* __restrict__ dn_sf, uint16_t* __restrict__ Asp,
+                                               uint16_t* __restrict__ Adn, uint8_t* __restrict__ E, int64_t T, int64_t Tp,
+                                               int64_t K, int path) {
+  tc::grid_dependency_wait();
+  const int64_t n8 = K >> 3;
+  for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < Tp * n8;
+       idx += (int64_t)gridDim.x * blockDim.x) {
+    const int64_t t = idx / n8, c = idx % n8;          // k = 8c .. 8c+7
+    const uint32_t unit_i = (uint32_t)((8 * c) & 63);
+    uint32_t sp[4] = {0u, 0u, 0u, 0u}, dn[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) dn[i] = 0u;
+    uint32_t meta = 0x44u;                             // pad rows: a valid nibble, zero values
+    if (t < T) {
+      meta = sp_meta[t * (K >> 3) + c];                // two nibbles: 4-groups 2c, 2c+1
+      if (path != 2) {
+        const uint32_t word = sp_sf[t * (K >> 6) + (c >> 3)];
+        const uint32_t codes = *reinterpret_cast<const uint16_t*>(sp_codes + t * (K >> 2) + 2 * c);
+#pragma unroll
+        for (int g = 0; g < 2; ++g) {
+          const uint32_t nib = (meta >> (4 * g)) & 15u, i0 = nib & 3u, i1 = nib >> 2;
+          const uint32_t byte = (codes >> (8 * g)) & 255u;
+          sp[2 * g] = hif4_to_bf16(byte & 15u, word, unit_i + 4 * g + i0);
+          sp[2 * g + 1] = hif4_to_bf16(byte >> 4, word, unit_i + 4 * g + i1);
+        }
+      }
+      if (path != 1) {
+        const uint32_t word = dn_sf[t * (K >> 6) + (c >> 3)];
+        const uint32_t codes = *reinterpret_cast<const uint32_t*>(dn_codes + t * (K >> 1) + 4 * c);
+#pragma unroll
+        for (int e = 0; e < 8; ++e) dn[e] = hif4_to_bf16((codes >> (4 * e)) & 15u, word, unit_i + e);
+      }
+    }
+    *reinterpret_cast<uint2*>(Asp + t * (K >> 1) + 4 * c) = make_uint2(sp[0] | sp[1] << 16, sp[2] | sp[3] << 16);
+    *reinterpret_cast<uint4*>(Adn + t * K + 8 * c) =
+        make_uint4(dn[0] | dn[1] << 16, dn[2] | dn[3] << 16, dn[4] | dn[5] << 16, dn[6] | dn[7] << 16);
+    const int64_t m = t & 127, kk = (8 * c) & 127;
+    const int64_t atom = (t >> 7) * (K >> 7) + ((8 * c) >> 7);
+    E[atom * 2048 + 16 * (m & 7) + 2 * ((m >> 3) & 1) + 256 * (m >> 4) + 128 * ((kk >> 4) & 1) + 4 * (kk >> 5) + ((kk & 15) >> 3)] =
+        (uint8_t)meta;
+  }
+}
+
+__device__ __forceinline__ void mma_bf16_sparse_pair(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc,
+                                                     uint32_t meta_tmem, uint32_t accumulate) {
+  asm volatile("{ .reg .pred p;\n\t"
+               "setp.ne.b32 p, %4, 0;\n\t"
+               "tcgen05.mma.sp.cta_group::2.kind::f16 [%0], %1, %2, [%5], %3, p; }"
+               ::"r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate), "r"(meta_tmem) : "memory");
+}
+
+// One pipeline stage = 128 logical k.  Sparse step: A_sp 128 rows x 64 stored bf16 (16 KB) + metadata atom (2 KB) + this
+// CTA's half of the W tile as two 64-k sub-tiles; dense step: two A sub-tiles (32 KB) + the same W bytes.
+template <int BN>
+struct SpStage {
+  static constexpr int HALF = BN / 2;
+  static constexpr int A0 = 0, A1 = 16384, META = 16384, B0 = 32768, B1 = B0 + HALF * 128;
+  static constexpr int BYTES = (B1 + HALF * 128 + 1023) / 1024 * 1024;
+  static constexpr int STAGES = 3;
+  static constexpr int E_COL = 2 * BN;                     // two accumulator stages, then four metadata columns
+  static constexpr int SMEM = STAGES * BYTES + 1024 + 256 + kStageBytes;
+  static_assert(E_COL + 4 <= 512, "tensor memory");
+};
+
+template <int BN>
+__global__ void __launch_bounds__(kGemmThreads, 1)
+hif4_gemm_sp_pair_kernel(const __grid_constant__ CUtensorMap tm_asp, const __grid_constant__ CUtensorMap tm_adn,
+                         const __grid_constant__ CUtensorMap tm_w, const __grid_constant__ CUtensorMap tm_e,
+                         const GemmParams p, const int path) {
+  using S = SpStage<BN>;
+  extern __shared__ uint8_t smem_raw[];
+  const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+  const uint32_t bars = smem_base + S::STAGES * S::BYTES;
+  auto full_bar = [&](int s) { return bars + 8u * s; };                       // leader CTA
+  auto empty_bar = [&](int s) { return bars + 8u * (S::STAGES + s); };
+  auto tmem_full_bar = [&](int a) { return bars + 8u * (2 * S::STAGES + a); };
+  auto tmem_empty_bar = [&](int a) { return bars + 8u * (2 * S::STAGES + 2 + a); };   // leader CTA
+  const uint32_t tmem_ptr_smem = bars + 8u * (2 * S::STAGES + 4);
+  const uint32_t stg_base = bars + 256u;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int rank = (int)tc::cluster_ctarank();
+  const int ksteps = p.K / 128;                                    // per phase
+  const int sp_steps = path != 2 ? ksteps : 0, dn_steps = path != 1 ? ksteps : 0;
+  const int m_pairs = (p.m_blocks + 1) / 2, n_tiles = (p.D + BN - 1) / BN, total = m_pairs * n_tiles;
+  const int gm = p.group_m > 0 && p.group_m < m_pairs ? p.group_m : m_pairs;
+  const int tile0 = (int)tc::cluster_id_x(), tile_step = (int)(gridDim.x >> 1);
+
+  if (warp == 0 && lane == 0) {
+    tc::prefetch_tmap(&tm_asp);
+    tc::prefetch_tmap(&tm_adn);
+    tc::prefetch_tmap(&tm_w);
+    tc::prefetch_tmap(&tm_e);
+  }
+  if (warp == 1 && lane == 0) {
+    for (int s = 0; s < S::STAGES; ++s) {
+      tc::mbar_init(full_bar(s), 1);
+      tc::mbar_init(empty_bar(s), 1);
+    }
+    for (int a = 0; a < 2; ++a) {
+      tc::mbar_init(tmem_full_bar(a), 1);
+      tc::mbar_init(tmem_empty_bar(a), 8);
+    }
+    tc::fence_mbar_init();
+  }
+  if (warp == 2) tc::tmem_alloc_pair<512>(tmem_ptr_smem);
+  tc::tc_fence_before();
+  __syncwarp();
+  tc::cluster_sync_all();
+  tc::tc_fence_after();
+  uint32_t tmem_base;
+  asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_ptr_smem));
+  tc::grid_dependency_wait();
+
+  if (warp == 0) {
+    const bool lead = tc::elect_one() != 0;
+    const uint64_t pol = tc::policy_evict_normal();
+    const uint32_t w_bytes = 2u * S::HALF * 128u;
+    uint32_t it = 0;
+    for (int tile = tile0; tile < total; tile += tile_step) {
+      int m_pair, n_blk;
+      pair_tile(tile, m_pairs, n_tiles, gm, m_pair, n_blk);
+      const int m_blk = 2 * m_pair + rank;
+      const int m_e = min(m_blk, p.m_blocks - 1);                  // a ragged pair's second CTA: valid memory, unused rows
+      const int w_row = n_blk * BN + rank * S::HALF;
+      for (int ks = 0; ks < sp_steps + dn_steps; ++ks, ++it) {
+        const int s = it % S::STAGES;
+        tc::mbar_wait(empty_bar(s), ((it / S::STAGES) & 1) ^ 1);
+        const uint32_t st = smem_base + s * S::BYTES;
+        const uint32_t fb = full_bar(s);
+        const bool sparse = ks < sp_steps;
+        const int k128 = sparse ? ks : ks - sp_steps;
+        if (lead && rank == 0) tc::mbar_expect_tx(fb, 2u * (w_bytes + (sparse ? 16384u + 2048u : 32768u)));
+        if (lead) tc::tma_load_2d_pair(st + S::B0, &tm_w, fb, k128 * 128, w_row, pol);
+        if (lead) tc::tma_load_2d_pair(st + S::B1, &tm_w, fb, k128 * 128 + 64, w_row, pol);
+        if (sparse) {
+          if (lead) tc::tma_load_2d_pair(st + S::A0, &tm_asp, fb, k128 * 64, m_blk * GM, pol);
+          if (lead) tc::tma_load_2d_pair(st + S::META, &tm_e, fb, 0, (m_e * ksteps + k128) * 2, pol);
+        } else {
+          if (lead) tc::tma_load_2d_pair(st + S::A0, &tm_adn, fb, k128 * 128, m_blk * GM, pol);
+          if (lead) tc::tma_load_2d_pair(st + S::A1, &tm_adn, fb, k128 * 128 + 64, m_blk * GM, pol);
+        }
+      }
+    }
+  } else if (warp == 1) {
+    if (rank == 0) {
+      const bool lead = tc::elect_one() != 0;
+      const uint32_t idesc = idesc_bf16(256, BN), idesc_sp = idesc | (1u << 2);
+      uint32_t it = 0, n_unit = 0;
+      for (int tile = tile0; tile < total; tile += tile_step, ++n_unit) {
+        const uint32_t as = n_unit & 1u;
+        const uint32_t acc = tmem_base + as * BN;
+        tc::mbar_wait(tmem_empty_bar(as), ((n_unit >> 1) & 1u) ^ 1u);
+        tc::tc_fence_after();
+        uint32_t accumulate = 0;
+        for (int ks = 0; ks < sp_steps + dn_steps; ++ks, ++it) {
+          const int s = it % S::STAGES;
+          tc::mbar_wait(full_bar(s), (it / S::STAGES) & 1);
+          tc::tc_fence_after();
+          const uint32_t st = smem_base + s * S::BYTES;
+          if (ks < sp_steps) {
+            if (lead) tc::tc_cp_meta_pair(tmem_base + S::E_COL, tc::smem_desc(st + S::META, 128, 0));
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {                  // K = 32 logical = 16 stored bf16 (32 bytes of A) per MMA
+              // the metadata address is an EVEN tensor-memory column; bit 0 of the instruction descriptor ("sparse id")
+              // selects the even or the odd column of the pair
+              if (lead) mma_bf16_sparse_pair(acc, tc::smem_desc(st + S::A0 + 32 * j, 1024, 2),
+                                             tc::smem_desc(st + (j < 2 ? S::B0 : S::B1) + 64 * (j & 1), 1024, 2),
+                                             idesc_sp | (uint32_t)(j & 1), tmem_base + S::E_COL + (j & ~1), accumulate);
+              accumulate = 1;
+            }
+          } else {
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {                  // K = 16 per MMA
+              if (lead) mma_bf16_pair(acc, tc::smem_desc(st + (j < 4 ? S::A0 : S::A1) + 32 * (j & 3), 1024, 2),
+                                      tc::smem_desc(st + (j < 4 ? S::B0 : S::B1) + 32 * (j & 3), 1024, 2), idesc, accumulate);
+              accumulate = 1;
+            }
+          }
+          if (lead) tc::tc_commit_pair(empty_bar(s), 3);
+        }
+        if (lead) tc::tc_commit_pair(tmem_full_bar(as), 3);
+      }
+    }
+  } else {
+    const int sub = warp & 3, r_local = sub * 32 + lane;
+    const uint32_t lane_addr = tmem_base + ((uint32_t)(sub * 32) << 16);
+    uint32_t n_unit = 0;
+    for (int tile = tile0; tile < total; tile += tile_step, ++n_unit) {
+      int m_pair, n_blk;
+      pair_tile(tile, m_pairs, n_tiles, gm, m_pair, n_blk);
+      const int m_blk = 2 * m_pair + rank;
+      const uint32_t as = n_unit & 1u;
+      const int64_t row = (int64_t)m_blk * GM + r_local;
+      const float scale = row < p.T ? __fmul_rn(p.row_scale[row], p.w_ts[0]) : 0.0f;
+      tc::mbar_wait(tmem_full_bar(as), (n_unit >> 1) & 1u);
+      tc::tc_fence_after();
+      const int rows_ok = (int)min((int64_t)32, max((int64_t)0, (int64_t)p.T - ((int64_t)m_blk * GM + sub * 32)));
+      epilogue_tile<BN>(p, lane_addr + as * BN, stg_base + (uint32_t)sub * 4096u, lane, (int64_t)m_blk * GM + sub * 32, rows_ok,
+                        n_blk * BN, scale);
+      tc::tc_fence_before();
+      __syncwarp();
+      if (lane == 0) tc::mbar_arrive_cluster(tc::map_to_cta(tmem_empty_bar(as), 0));
+    }
+  }
+  tc::tc_fence_before();
+  __syncwarp();
+  tc::cluster_sync_all();
+  if (warp == 2) {
+    tc::tc_fence_after();
+    tc::tmem_dealloc_pair<512>(tmem_base);
+  }
+}
+
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
@@ -436,6 +660,69 @@ cudaError_t launch_hif4_dequant_weight(const void* codes, const void* sf, void* 
   return cudaGetLastError();
 }
 
+namespace {
+// [rows1k][256 u32] view of a byte buffer, boxes of `box_rows` 1024-byte rows (the metadata atoms: 2 rows each)
+bool make_rows1k_map(CUtensorMap* m, const void* base, uint64_t bytes, uint32_t box_rows) {
+  void* f = nullptr;
+  cudaDriverEntryPointQueryResult q;
+  if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &f, cudaEnableDefault, &q) != cudaSuccess ||
+      q != cudaDriverEntryPointSuccess || bytes % 1024 != 0)
+    return false;
+  cuuint64_t dims[2] = {256, bytes / 1024};
+  cuuint64_t strides[1] = {1024};
+  cuuint32_t box[2] = {256, box_rows};
+  cuuint32_t estr[2] = {1, 1};
+  return reinterpret_cast<EncodeTiledFn>(f)(m, CU_TENSOR_MAP_DATA_TYPE_UINT32, 2, const_cast<void*>(base), dims, strides, box, estr,
+                                            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                            CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+template <int BN>
+sharq_status launch_sp_pair(const LinearArgs& a, void* workspace, int64_t Tp, int64_t m_blocks, int num_sms, cudaStream_t st) {
+  using S = SpStage<BN>;
+  // workspace: A_sp bf16 [Tp, K/2] | A_dn bf16 [Tp, K] | metadata atoms [Tp/128][K/128][2048]  (3.125 Tp K bytes of the 4 Tp K)
+  uint8_t* base = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(workspace) + 127) & ~(uintptr_t)127);
+  uint16_t* Asp = reinterpret_cast<uint16_t*>(base);
+  uint16_t* Adn = reinterpret_cast<uint16_t*>(base + (size_t)Tp * (size_t)a.K);
+  uint8_t* E = base + (size_t)Tp * (size_t)a.K * 3;
+  const uint16_t* W = reinterpret_cast<const uint16_t*>(a.w_sf_dn);
+  const int64_t na = Tp * (a.K >> 3);
+  hif4_dequant_act_sparse_kernel<<<(unsigned)((na + 255) / 256 < 8192 ? (na + 255) / 256 : 8192), 256, 0, st>>>(
+      (const uint8_t*)a.sp_codes, (const uint32_t*)a.sp_sf, (const uint8_t*)a.sp_meta, (const uint8_t*)a.dn_codes,
+      (const uint32_t*)a.dn_sf, Asp, Adn, E, a.T, Tp, a.K, a.path);
+  if (cudaGetLastError() != cudaSuccess) return SHARQ_ECUDA;
+  CUtensorMap tm_asp, tm_adn, tm_w, tm_e;
+  if (!make_bf16_map(&tm_asp, Asp, (uint64_t)Tp, (uint64_t)(a.K / 2), GM) ||
+      !make_bf16_map(&tm_adn, Adn, (uint64_t)Tp, (uint64_t)a.K, GM) ||
+      !make_bf16_map(&tm_w, W, (uint64_t)a.D, (uint64_t)a.K, S::HALF) ||
+      !make_rows1k_map(&tm_e, E, (uint64_t)Tp * (uint64_t)a.K / 8, 2))
+    return SHARQ_ECUDA;
+  const int64_t m_pairs = (m_blocks + 1) / 2, n_tiles = (a.D + BN - 1) / BN;
+  GemmParams pp{a.row_scale, a.w_ts, (const uint16_t*)a.bias, a.Y, a.ldy, (int32_t)a.T, (int32_t)a.D, (int32_t)a.K,
+                a.out_dtype, (int32_t)m_blocks, (int32_t)(m_pairs * n_tiles), 0};
+  const double a_pair = 256.0 * 1.5 * (double)a.K * 2.0;         // bf16 bytes of one 256-row block of both operands
+  if (a_pair * (double)m_pairs > 48e6) {
+    int64_t gm = (int64_t)(64e6 / a_pair);
+    pp.group_m = (int32_t)(gm < 1 ? 1 : gm > m_pairs ? m_pairs : gm);
+  }
+  auto kfn = hif4_gemm_sp_pair_kernel<BN>;
+  if (cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, S::SMEM) != cudaSuccess) return SHARQ_ECUDA;
+  const int64_t tiles = m_pairs * n_tiles;
+  const int64_t clusters = tiles < num_sms / 2 ? tiles : num_sms / 2;
+  cudaLaunchConfig_t lp{};
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeClusterDimension;
+  at[0].val.clusterDim.x = 2; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+  lp.blockDim = dim3(kGemmThreads);
+  lp.gridDim = dim3((unsigned)(2 * clusters));
+  lp.dynamicSmemBytes = S::SMEM;
+  lp.stream = st;
+  lp.attrs = at;
+  lp.numAttrs = 1;
+  return cudaLaunchKernelEx(&lp, kfn, tm_asp, tm_adn, tm_w, tm_e, pp, (int)a.path) == cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
+}
+}  // namespace
+
 sharq_status launch_linear_hif4(const LinearArgs& a, void* workspace, size_t workspace_bytes, int num_sms,
                                 cudaStream_t st) {
   if (!workspace || workspace_bytes < hif4_linear_workspace_bytes(a.T, a.D, a.K)) return SHARQ_EWORKSPACE;
@@ -444,6 +731,12 @@ sharq_status launch_linear_hif4(const LinearArgs& a, void* workspace, size_t wor
   uint16_t* A = reinterpret_cast<uint16_t*>((reinterpret_cast<uintptr_t>(workspace) + 127) & ~(uintptr_t)127);
   const uint16_t* W = reinterpret_cast<const uint16_t*>(a.w_sf_dn);   // bf16 [D, K], written by sharq_quantize_weight
   const int64_t na = a.T * (a.K >> 3);
+  {
+    const int64_t mb = Tp / 128;
+    if (mb >= 2 && ((mb + 1) / 2) * ((a.D + 223) / 224) >= num_sms / 4 && a.K % 128 == 0)
+      return a.D % 192 == 0 && a.D % 224 != 0 ? launch_sp_pair<192>(a, workspace, Tp, mb, num_sms, st)
+                                              : launch_sp_pair<224>(a, workspace, Tp, mb, num_sms, st);
+  }
   hif4_dequant_act_kernel<<<(unsigned)((na + 255) / 256 < 8192 ? (na + 255) / 256 : 8192), 256, 0, st>>>(
       (const uint8_t*)a.sp_codes, (const uint32_t*)a.sp_sf, (const uint8_t*)a.sp_meta, (const uint8_t*)a.dn_codes,
       (const uint32_t*)a.dn_sf, A, a.T, a.K, a.path);

@@ -456,3 +456,22 @@ def test_prepare_linear_one_call(sq, fmt, norm, T, K, D):
         assert torch.equal(y, y_ref), f"Y (rep {rep})"
     p, q = so.prepare(x, fmt=fmt, norm=norm, gamma_u16=g, beta_u16=b if norm == 2 else None), so.quantize_weight(w, fmt=fmt)
     assert rel_err(y.cpu().numpy(), so.linear(p, q, bias_u16=bias)).max() <= TOL
+
+
+@pytest.mark.parametrize("T,K,D", [(600, 768, 3328), (1000, 1024, 2304)])
+def test_hif4_sparse_backbone_paths(sq, T, K, D):
+    """HiF4 on the 2:4-sparse bf16 tensor path (tcgen05.mma.sp kind::f16 on the compressed survivors + metadata, dense
+    MMAs on the residual; 224- and 192-wide CTA-pair tiles, ragged last n-tile, ragged T, odd number of row blocks):
+    SharQ, sparse-only and dense-only against the oracle's fp64 products of the same dequantized operands."""
+    x, g, w = si.activations(T, K, config=4, outlier_mult=50.0, extra=T), si.gamma(K, 4), si.weight(D, K, 4, extra=D)
+    cfg = sq.make_config(sq.HIF4, sq.NORM_RMS, 1e-6)
+    wq = sq.quantize_weight(cfg, to_dev(w))
+    act = sq.prepare(cfg, to_dev(x), to_dev(g))
+    p, q = so.prepare(x, fmt=so.HIF4, norm=1, gamma_u16=g), so.quantize_weight(w, so.HIF4)
+    for path in (0, 1, 2):
+        y = sq.linear(cfg, act, wq, out_dtype="fp32", path=path)
+        torch.cuda.synchronize()
+        err = rel_err(y.cpu().numpy(), path_reference(p, q, path))
+        assert err.max() <= TOL, f"path {path}: {err.max():.3e} at {np.unravel_index(err.argmax(), err.shape)}"
+    y16 = sq.linear(cfg, act, wq, out_dtype="bf16")
+    assert torch.equal(y16, sq.linear(cfg, act, wq, out_dtype="fp32").to(torch.bfloat16))
