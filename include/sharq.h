@@ -172,10 +172,11 @@ sharq_status sharq_prepare_swiglu(const sharq_config* cfg, const void* gate, con
  * same TMEM tile in one kernel ("accumulates directly into this output").
  * out_dtype: 0 = bf16, 1 = fp32.  bias bf16 [D] or NULL.  ldy in elements.
  * path: 0 = sparse + dense (SharQ), 1 = sparse only, 2 = dense only (Table 5 rows).
- * HiF4 (layout CANONICAL): tcgen05 has no S1P2 / E6M2 formats, so the operands are dequantised to bf16
- * (exact: every HiF4 value has <= 6 significant bits): the weight once, by sharq_quantize_weight (its
- * sf_dense_view), the activation operands per call into `workspace`, and multiplied by a dense bf16 tensor-core
- * GEMM with fp32 accumulation; workspace >= sharq_linear_workspace(...) bytes is required.
+ * HiF4 (layout CANONICAL): tcgen05 has no S1P2 / E6M2 formats, so the operands are dequantised to bf16 (exact: every
+ * HiF4 value has <= 6 significant bits): the weight once, by sharq_quantize_weight (its sf_dense_view), the activation
+ * operands per call into `workspace` (backbone compressed [T, K/2] + its 2:4 metadata re-tiled for the tensor core,
+ * residual [T, K]), and multiplied on the bf16 tensor path with fp32 accumulation: 2:4-sparse MMAs for the backbone,
+ * dense MMAs for the residual.  workspace >= sharq_linear_workspace(...) bytes is required.
  * NVFP4 / MXFP4 need no workspace (it may be NULL).  Kernels are launched with programmatic dependent
  * launch: the weight stream of sharq_linear may start while the preceding kernel of the stream (normally
  * sharq_prepare) is still draining; all reads of activation operands wait for it to complete. */
