@@ -3,14 +3,14 @@
 // B200's tcgen05 has no S1P2 element / E6M2 scale format, so HiF4 has no FP4-rate tensor path.  Every
 // HiF4 value E6M2 * 2^(E1_8 + E1_16) * S1P2 = (4 + m) * k * 2^(E - 52 + shift) with (4 + m) * k <= 49
 // has at most 6 significant bits, i.e. it is EXACT in bf16.  The path is therefore:
-//   1. hif4_dequant_*  : codes + 32-bit unit metadata -> bf16 (exact), activations as [T, 2K] =
-//                        [backbone with zeros at dropped positions | residual] on every call, weights as [D, K]
-//                        ONCE, by sharq_quantize_weight (the HiF4 "dense view" of the payload is this bf16 tensor);
-//   2. hif4_gemm_kernel: dense bf16 tcgen05.mma (kind::f16, fp32 accumulate) over the 2K-long rows, the
-//                        W tile reused for both halves (k and k + K read the same weight columns):
-//                        Y = A_sp W^T + A_dn W^T in one accumulator.
-// Roofline denominator: the measured bf16 tensor peak.  The 2:4 sparse bf16 MMA for the backbone half
-// (which would save a quarter of the MMA time) is not used yet: the zeros are multiplied densely.
+//   1. weights: bf16 [D, K] ONCE, by sharq_quantize_weight (the HiF4 "dense view" of the payload is this bf16 tensor);
+//   2. activations, per call (hif4_dequant_act_sparse_kernel): backbone compressed [T, K/2] bf16 + 2:4 metadata in the
+//      tensor core's tiling, residual [T, K] bf16;
+//   3. hif4_gemm_sp_pair_kernel: CTA-pair tiles, tcgen05.mma.sp kind::f16 on the backbone, dense tcgen05.mma kind::f16
+//      on the residual, one fp32 accumulator: Y = A_sp W^T + A_dn W^T.
+// Small launches keep the first version: activations as [T, 2K] = [backbone with zeros | residual] and a dense bf16
+// GEMM over the 2K-long rows (hif4_gemm_kernel / hif4_gemm_pair_kernel).
+// Roofline denominator: the measured bf16 tensor peak.
 #include <cuda.h>
 #include <cuda_runtime.h>
 
