@@ -846,7 +846,6 @@ sharq_linear_pair_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __gr
     {
       const bool lead = tc::elect_one() != 0;
       const uint64_t pol = tc::policy_evict_normal();
-      const int64_t Kc = p.K;
       // every load of the pair (tiles, scale-factor atoms, metadata) is a cta_group::2 tensor copy whose
       // complete_tx lands on the LEADER's full barrier: no cross-CTA hand-off inside the ring
       const uint32_t tx = 2u * (S::HALF * 128 + (do_sp ? BM * 64 + 2048 + 1024 + 2 * 1024 : 0) +

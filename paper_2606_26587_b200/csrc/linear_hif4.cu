@@ -9,7 +9,7 @@
 //   3. hif4_gemm_sp_pair_kernel: CTA-pair tiles, tcgen05.mma.sp kind::f16 on the backbone, dense tcgen05.mma kind::f16
 //      on the residual, one fp32 accumulator: Y = A_sp W^T + A_dn W^T.
 // Small launches keep the first version: activations as [T, 2K] = [backbone with zeros | residual] and a dense bf16
-// GEMM over the 2K-long rows (hif4_gemm_kernel / hif4_gemm_pair_kernel).
+// GEMM over the 2K-long rows (hif4_gemm_kernel).
 // Roofline denominator: the measured bf16 tensor peak.
 #include <cuda.h>
 #include <cuda_runtime.h>
@@ -251,137 +251,14 @@ hif4_gemm_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant
   }
 }
 
-// ---- CTA-pair version (cta_group::2): 256 x 256 tile per cluster of two CTAs -----------------------------------
-// Each CTA stages its own 128 rows of A and HALF of the 256-row W tile per k-step (32 KB instead of 48 KB for twice
-// the MMA work of a 128 x 256 tile), one tcgen05.mma.cta_group::2 of M = 256 consumes both CTAs' shared memory.  The
-// bf16 path needs no scale-factor columns, so both 256-column accumulator stages fit in tensor memory: the epilogue of
-// tile i (through shared memory, full-line stores) overlaps the main loop of tile i + 1.
+// ---- CTA-pair MMAs (cta_group::2): each CTA stages its own 128 rows of A and HALF of the W tile, one tcgen05.mma of
+// M = 256 consumes both CTAs' shared memory --------------------------------------------------------------------
 __device__ __forceinline__ void mma_bf16_pair(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc,
                                               uint32_t accumulate) {
   asm volatile("{ .reg .pred p;\n\t"
                "setp.ne.b32 p, %4, 0;\n\t"
                "tcgen05.mma.cta_group::2.kind::f16 [%0], %1, %2, %3, p; }"
                ::"r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate) : "memory");
-}
-
-constexpr int kPairStages = 6, kPairStageBytes = GM * 128 + 128 * 128;          // A 16 KB + half of B 16 KB
-constexpr int kPairSmem = kPairStages * kPairStageBytes + 1024 + 256 + kStageBytes;
-
-__global__ void __launch_bounds__(kGemmThreads, 1)
-hif4_gemm_pair_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant__ CUtensorMap tm_w,
-                      const GemmParams p) {
-  constexpr int BN = 256, STAGES = kPairStages, STAGE = kPairStageBytes, A_BYTES = GM * 128;
-  extern __shared__ uint8_t smem_raw[];
-  const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
-  const uint32_t bars = smem_base + STAGES * STAGE;
-  auto full_bar = [&](int s) { return bars + 8u * s; };                       // leader CTA
-  auto empty_bar = [&](int s) { return bars + 8u * (STAGES + s); };
-  auto tmem_full_bar = [&](int a) { return bars + 8u * (2 * STAGES + a); };
-  auto tmem_empty_bar = [&](int a) { return bars + 8u * (2 * STAGES + 2 + a); };   // leader CTA
-  const uint32_t tmem_ptr_smem = bars + 8u * (2 * STAGES + 4);
-  const uint32_t stg_base = bars + 256u;
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int rank = (int)tc::cluster_ctarank();
-  const int num_kb = 2 * p.K / GK, half_kb = p.K / GK;
-  const int m_pairs = (p.m_blocks + 1) / 2, n_tiles = p.D / BN, total = m_pairs * n_tiles;
-  const int gm = p.group_m > 0 && p.group_m < m_pairs ? p.group_m : m_pairs;
-  const int tile0 = (int)tc::cluster_id_x(), tile_step = (int)(gridDim.x >> 1);
-
-  if (warp == 0 && lane == 0) {
-    tc::prefetch_tmap(&tm_a);
-    tc::prefetch_tmap(&tm_w);
-  }
-  if (warp == 1 && lane == 0) {
-    for (int s = 0; s < STAGES; ++s) {
-      tc::mbar_init(full_bar(s), 1);
-      tc::mbar_init(empty_bar(s), 1);
-    }
-    for (int a = 0; a < 2; ++a) {
-      tc::mbar_init(tmem_full_bar(a), 1);
-      tc::mbar_init(tmem_empty_bar(a), 8);       // four epilogue warps in each CTA
-    }
-    tc::fence_mbar_init();
-  }
-  if (warp == 2) tc::tmem_alloc_pair<512>(tmem_ptr_smem);
-  tc::tc_fence_before();
-  __syncwarp();
-  tc::cluster_sync_all();
-  tc::tc_fence_after();
-  uint32_t tmem_base;
-  asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_ptr_smem));
-  tc::grid_dependency_wait();                            // A was dequantised by the kernel before us
-
-  if (warp == 0) {
-    const bool lead = tc::elect_one() != 0;
-    const uint64_t pol = tc::policy_evict_normal();
-    uint32_t it = 0;
-    for (int tile = tile0; tile < total; tile += tile_step) {
-      int m_pair, n_blk;
-      pair_tile(tile, m_pairs, n_tiles, gm, m_pair, n_blk);
-      const int m_blk = 2 * m_pair + rank;
-      for (int kb = 0; kb < num_kb; ++kb, ++it) {
-        const int s = it % STAGES;
-        tc::mbar_wait(empty_bar(s), ((it / STAGES) & 1) ^ 1);
-        const uint32_t st = smem_base + s * STAGE;
-        if (lead && rank == 0) tc::mbar_expect_tx(full_bar(s), 2u * STAGE);
-        if (lead) tc::tma_load_2d_pair(st, &tm_a, full_bar(s), kb * GK, m_blk * GM, pol);    // rows beyond the map: zero fill
-        if (lead) tc::tma_load_2d_pair(st + A_BYTES, &tm_w, full_bar(s), (kb % half_kb) * GK, n_blk * BN + rank * 128, pol);
-      }
-    }
-  } else if (warp == 1) {
-    if (rank == 0) {
-      const bool lead = tc::elect_one() != 0;
-      const uint32_t idesc = idesc_bf16(256, BN);
-      uint32_t it = 0, n_unit = 0;
-      for (int tile = tile0; tile < total; tile += tile_step, ++n_unit) {
-        const uint32_t as = n_unit & 1u;
-        tc::mbar_wait(tmem_empty_bar(as), ((n_unit >> 1) & 1u) ^ 1u);
-        tc::tc_fence_after();
-        uint32_t accumulate = 0;
-        for (int kb = 0; kb < num_kb; ++kb, ++it) {
-          const int s = it % STAGES;
-          tc::mbar_wait(full_bar(s), (it / STAGES) & 1);
-          tc::tc_fence_after();
-          const uint32_t st = smem_base + s * STAGE;
-#pragma unroll
-          for (int j = 0; j < GK / 16; ++j) {
-            if (lead) mma_bf16_pair(tmem_base + as * BN, tc::smem_desc(st + 32 * j, 1024, 2),
-                                    tc::smem_desc(st + A_BYTES + 32 * j, 1024, 2), idesc, accumulate);
-            accumulate = 1;
-          }
-          if (lead) tc::tc_commit_pair(empty_bar(s), 3);
-        }
-        if (lead) tc::tc_commit_pair(tmem_full_bar(as), 3);
-      }
-    }
-  } else {
-    const int sub = warp & 3, r_local = sub * 32 + lane;
-    const uint32_t lane_addr = tmem_base + ((uint32_t)(sub * 32) << 16);
-    uint32_t n_unit = 0;
-    for (int tile = tile0; tile < total; tile += tile_step, ++n_unit) {
-      int m_pair, n_blk;
-      pair_tile(tile, m_pairs, n_tiles, gm, m_pair, n_blk);
-      const int m_blk = 2 * m_pair + rank;
-      const uint32_t as = n_unit & 1u;
-      const int64_t row = (int64_t)m_blk * GM + r_local;
-      const float scale = row < p.T ? __fmul_rn(p.row_scale[row], p.w_ts[0]) : 0.0f;
-      tc::mbar_wait(tmem_full_bar(as), (n_unit >> 1) & 1u);
-      tc::tc_fence_after();
-      const int rows_ok = (int)min((int64_t)32, max((int64_t)0, (int64_t)p.T - ((int64_t)m_blk * GM + sub * 32)));
-      epilogue_tile<BN>(p, lane_addr + as * BN, stg_base + (uint32_t)sub * 4096u, lane, (int64_t)m_blk * GM + sub * 32, rows_ok,
-                        n_blk * BN, scale);
-      tc::tc_fence_before();
-      __syncwarp();
-      if (lane == 0) tc::mbar_arrive_cluster(tc::map_to_cta(tmem_empty_bar(as), 0));
-    }
-  }
-  tc::tc_fence_before();
-  __syncwarp();
-  tc::cluster_sync_all();
-  if (warp == 2) {
-    tc::tc_fence_after();
-    tc::tmem_dealloc_pair<512>(tmem_base);
-  }
 }
 
 // ---- 2:4-sparse backbone: tcgen05.mma.sp kind::f16 (SURVEY.md 8(a) S12 as written) --------------------------------
@@ -747,35 +624,6 @@ sharq_status launch_linear_hif4(const LinearArgs& a, void* workspace, size_t wor
       !make_bf16_map(&tm_w, W, (uint64_t)a.D, (uint64_t)a.K, wide ? 256 : 128))
     return SHARQ_ECUDA;
   const int64_t m_blocks = Tp / 128;
-  if (wide && m_blocks >= 2 && ((m_blocks + 1) / 2) * (a.D / 256) >= num_sms / 4) {
-    // CTA-pair tiles; W map with 128-row boxes (each CTA stages half of the 256-row tile)
-    CUtensorMap tm_wh;
-    if (!make_bf16_map(&tm_wh, W, (uint64_t)a.D, (uint64_t)a.K, 128)) return SHARQ_ECUDA;
-    const int64_t m_pairs = (m_blocks + 1) / 2;
-    GemmParams pp{a.row_scale, a.w_ts, (const uint16_t*)a.bias, a.Y, a.ldy, (int32_t)a.T, (int32_t)a.D, (int32_t)a.K,
-                  a.out_dtype, (int32_t)m_blocks, (int32_t)(m_pairs * (a.D / 256)), 0};
-    // supertile height: as many 256-row blocks of A (bf16 [256, 2K]) as fit beside W's tiles in ~64 MB of L2
-    const double a_pair = 256.0 * 2.0 * (double)a.K * 2.0;
-    if (a_pair * (double)m_pairs > 48e6) {
-      int64_t gm = (int64_t)(64e6 / a_pair);
-      pp.group_m = (int32_t)(gm < 1 ? 1 : gm > m_pairs ? m_pairs : gm);
-    }
-    if (cudaFuncSetAttribute(hif4_gemm_pair_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kPairSmem) != cudaSuccess)
-      return SHARQ_ECUDA;
-    const int64_t tiles = m_pairs * (a.D / 256);
-    const int64_t clusters = tiles < num_sms / 2 ? tiles : num_sms / 2;
-    cudaLaunchConfig_t lp{};
-    cudaLaunchAttribute at[1];
-    at[0].id = cudaLaunchAttributeClusterDimension;
-    at[0].val.clusterDim.x = 2; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
-    lp.blockDim = dim3(kGemmThreads);
-    lp.gridDim = dim3((unsigned)(2 * clusters));
-    lp.dynamicSmemBytes = kPairSmem;
-    lp.stream = st;
-    lp.attrs = at;
-    lp.numAttrs = 1;
-    return cudaLaunchKernelEx(&lp, hif4_gemm_pair_kernel, tm_a, tm_wh, pp) == cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
-  }
   GemmParams p{a.row_scale, a.w_ts, (const uint16_t*)a.bias, a.Y, a.ldy, (int32_t)a.T, (int32_t)a.D, (int32_t)a.K,
                a.out_dtype, (int32_t)m_blocks, (int32_t)(m_blocks * (a.D / (wide ? 256 : 128))), 0};
   return wide ? launch_gemm<256>(tm_a, tm_w, p, num_sms, st) : launch_gemm<128>(tm_a, tm_w, p, num_sms, st);
