@@ -16,8 +16,8 @@ and every Y copied back to the host inside the timed region.  N > 1: one process
 `extras`: configs[1] (decode, T <= 256: us per layer, HBM roofline of the weight stream), configs[2] at
 T = 2048 / 4096, configs[3] (Qwen shapes x NVFP4 / MXFP4 / HiF4), configs[4] (MoE grouped), stream-mode host cost.
 
-`--impl reference` times the CPU oracle (oracle/, as it stands) on a bounded sample of the same
-workload on the host cores.  The oracle is never on the product path.
+`--impl reference` times the CPU oracle (the compiled C one, oracle/sharq_oracle_c.c, as it stands) on a bounded sample
+of the same workload on the host cores.  The oracle is never on the product path.
 """
 from __future__ import annotations
 
@@ -734,52 +734,68 @@ def config_extras(sq, wl, pk, steps, mp=None):
 
 
 # ---- CPU oracle legs (the only places bench.py executes oracle/) ---------------------------------------
-SAMPLE_T, SAMPLE_COLS = 16, 1024
-SAMPLE_DESC = (f"bounded sample of the headline workload (configs[2] shapes qkv/o/gate_up/down): {SAMPLE_T} of the 8192 rows and "
-               f"{SAMPLE_COLS} seeded output features per layer, oracle prepare + fp64 linear as they stand (numpy; the fp64 "
-               "GEMM runs on the BLAS thread pool = `cores`, the prepare half is single-threaded numpy); weight "
-               "quantization (offline) not timed; value = nominal 2TKD of the sample / time")
+# the baseline IS the oracle, compiled (-O2, no fast-math, no FMA contraction), rows parallel over
+# the host cores: oracle/sharq_oracle_c.c, which tests/test_oracle_c.py holds byte-identical to the numpy oracle.
 
 
-def oracle_sample_setup():
+def sample_desc(t_prep, t_lin):
+    return (f"headline workload (configs[2] shapes qkv/o/gate_up/down, T = {HEADLINE_T}): the compiled C oracle "
+            f"(oracle/sharq_oracle_c.c, gcc -O2 -ffp-contract=off -fno-fast-math, OpenMP over rows) as it stands; "
+            f"prepare timed on {t_prep} of the {HEADLINE_T} rows of every layer, the fp64 linear on {t_lin} seeded full "
+            f"rows x all D output features of every layer; value = the whole step's nominal 2TKD / (each part's time "
+            f"scaled linearly to {HEADLINE_T} rows) -- EXTRAPOLATED from the sample; weight quantization (offline) not timed")
+
+
+def oracle_sample_setup(t_prep, t_lin):
     import sharq_inputs as si
-    from oracle import sharq_oracle as so
+    from oracle import c_oracle as co
     rng = np.random.Generator(np.random.Philox(BASE_SEED))
     items = []
     for i, (n, K, D, norm) in enumerate(LLAMA):
-        x, g = si.activations(SAMPLE_T, K, config=2, extra=i), si.gamma(K, 2)
-        cols = np.sort(rng.choice(D, size=SAMPLE_COLS, replace=False))
-        w = si.weight(SAMPLE_COLS, K, config=2, extra=i)            # the sampled rows of W stand for W[cols]
-        items.append((n, K, norm, x, g, so.quantize_weight(w)))
-    return so, items
+        x, g = si.activations(t_prep, K, config=2, extra=i), si.gamma(K, 2)
+        rows = np.sort(rng.choice(t_prep, size=t_lin, replace=False))
+        wq = co.quantize_weight(si.weight(D, K, config=2, extra=i))
+        items.append((n, K, D, norm, x, g, rows, wq))
+    return co, items
 
 
-def oracle_sample_step(so, items):
-    for n, K, norm, x, g, wq in items:
-        p = so.prepare(x, norm=norm, gamma_u16=g if norm else None)
-        so.linear(p, wq)
+def oracle_sample_step(co, items):
+    """One bounded sample of the step.  Returns (prepare seconds, linear seconds, threads used)."""
+    tp = tl = 0.0
+    nt = 1
+    for n, K, D, norm, x, g, rows, wq in items:
+        t0 = time.perf_counter()
+        p = co.prepare(x, co.NVFP4, norm, g if norm else None, want_X=False)
+        t1 = time.perf_counter()
+        co.linear(p, wq, rows=rows)
+        tl += time.perf_counter() - t1
+        tp += t1 - t0
+        nt = p["threads"]
+    return tp, tl, nt
 
 
-def oracle_threads():
-    try:
-        from threadpoolctl import threadpool_info
-        return max([int(i.get("num_threads", 1)) for i in threadpool_info()] or [1])
-    except Exception:
-        return 1
+def oracle_value(tp, tl, t_prep, t_lin):
+    """Whole-step TFLOP/s with each part scaled linearly to the full row count."""
+    est = tp * HEADLINE_T / t_prep + tl * HEADLINE_T / t_lin
+    fl = sum(layer_flops(HEADLINE_T, K, D) for _, K, D, _ in LLAMA)
+    return fl / est / 1e12, est
 
 
-def cpu_baseline_sample():
-    so, items = oracle_sample_setup()
-    oracle_sample_step(so, items)                                    # warm
+def cpu_baseline_sample(t_prep=HEADLINE_T, t_lin=32):
+    co, items = oracle_sample_setup(t_prep, t_lin)
+    oracle_sample_step(co, items)                                    # warm
     t0 = time.perf_counter()
-    reps = 0
-    while reps < 2 or time.perf_counter() - t0 < 10.0:
-        oracle_sample_step(so, items)
+    acc, reps = [0.0, 0.0], 0
+    while reps < 1 or time.perf_counter() - t0 < 10.0:
+        tp, tl, nt = oracle_sample_step(co, items)
+        acc[0] += tp
+        acc[1] += tl
         reps += 1
-    dt = (time.perf_counter() - t0) / reps
-    fl = sum(layer_flops(SAMPLE_T, K, SAMPLE_COLS) for _, K, _, _ in LLAMA)
-    return dict(value=round(fl / dt / 1e12, 6), unit="TFLOP/s", cores=oracle_threads(), kind="oracle",
-                sample=SAMPLE_DESC, host_cores=os.cpu_count(), s_per_sample_step=round(dt, 3))
+    tp, tl = acc[0] / reps, acc[1] / reps
+    v, est = oracle_value(tp, tl, t_prep, t_lin)
+    return dict(value=round(v, 6), unit="TFLOP/s", cores=nt, kind="oracle", sample=sample_desc(t_prep, t_lin),
+                host_cores=os.cpu_count(), prepare_s=round(tp, 3), linear_sample_s=round(tl, 3),
+                extrapolated_step_s=round(est, 1), extrapolated=True)
 
 
 def run_reference(args):
@@ -787,31 +803,36 @@ def run_reference(args):
     if rank != 0:
         return
     world = int(os.environ.get("WORLD_SIZE", "1"))
-    so, items = oracle_sample_setup()
+    t_prep, t_lin = 1024, 8                                           # a step of about a second: 30 + 5 steps in minutes
+    co, items = oracle_sample_setup(t_prep, t_lin)
     steps, warmup = args.steps, args.warmup
     budget = 150.0                                                    # seconds: keep the whole run to minutes
     t_all = time.perf_counter()
     for _ in range(warmup):
-        oracle_sample_step(so, items)
+        oracle_sample_step(co, items)
         if time.perf_counter() - t_all > budget / 3:
             break
     t0 = time.perf_counter()
-    done = 0
+    acc, done, nt = [0.0, 0.0], 0, 1
     for _ in range(steps):
-        oracle_sample_step(so, items)
+        tp, tl, nt = oracle_sample_step(co, items)
+        acc[0] += tp
+        acc[1] += tl
         done += 1
         if time.perf_counter() - t0 > budget:
             break
     dt = (time.perf_counter() - t0) / done
-    fl = sum(layer_flops(SAMPLE_T, K, SAMPLE_COLS) for _, K, _, _ in LLAMA)
-    v = round(fl / dt / 1e12, 6)
+    v, est = oracle_value(acc[0] / done, acc[1] / done, t_prep, t_lin)
+    v = round(v, 6)
+    desc = sample_desc(t_prep, t_lin)
     print(json.dumps({
         "impl": "reference", "metric": "sharq_layer_effective_tflops", "value": v, "unit": "TFLOP/s",
         "n_gpus": world, "steps": done, "warmup": warmup, "ms_per_step": round(dt * 1e3, 3), "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": "BASELINE configs[2] (bounded sample): " + SAMPLE_DESC},
-        "cpu_baseline": dict(value=v, unit="TFLOP/s", kind="oracle", cores=oracle_threads(), sample=SAMPLE_DESC,
-                             host_cores=os.cpu_count()),
+        "config": {"workload": "BASELINE configs[2] (bounded sample per step; ms_per_step is the sample's wall time, "
+                               "value is extrapolated to the whole step): " + desc},
+        "cpu_baseline": dict(value=v, unit="TFLOP/s", kind="oracle", cores=nt, sample=desc, host_cores=os.cpu_count(),
+                             extrapolated_step_s=round(est, 1), extrapolated=True),
         "e2e": {"value": v, "unit": "TFLOP/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0}), flush=True)
 

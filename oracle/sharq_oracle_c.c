@@ -1,0 +1,387 @@
+/* SharQ CPU oracle in plain C -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+ *
+ * A second, independent restatement of the SharQ per-linear-layer hot path (arxiv/paper_2606_26587; "P:n" = line n of
+ * /root/reference/PAPER.md), written from the paper and DESIGN.md's readings R1-R8, NOT from oracle/sharq_oracle.py and
+ * not from the CUDA sources: it shares no code with either.  It exists for two reasons:
+ *   1. a cross-pin: tests/test_oracle_c.py requires this file and the numpy oracle to agree byte for byte on every
+ *      prepared output (two independent implementations of one specification), and to 1e-12 on the fp64 linear;
+ *   2. the CPU baseline BASELINE.md section 3 asks for: the oracle compiled with -O2 (no fast-math, no FMA contraction),
+ *      rows parallelised over the host cores with OpenMP.  Never tuned beyond that.
+ * Scope: NVFP4 and MXFP4, pairwise 4:8 mask, norm none / RMS / Layer, dynamic or static tensor scale, weights, Eq. 9 in
+ * fp64.  (HiF4 lives in the numpy oracle only.)
+ *
+ * Numerics contract (R1-R8): every float operation below is ONE IEEE-754 binary32 operation, round to nearest
+ * even; build with -O2 -ffp-contract=off -fno-fast-math (oracle/build_c.py).  bf16 values travel as uint16 bit patterns.
+ * Only tests/, __graft_entry__ (build / smoke) and bench.py's cpu_baseline / --impl reference legs may load this library.
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+enum { FMT_NVFP4 = 0, FMT_MXFP4 = 1 };
+enum { NORM_NONE = 0, NORM_RMS = 1, NORM_LAYER = 2 };
+
+/* ---- bit-level helpers ------------------------------------------------------------------------------------------ */
+static inline float bits_f32(uint32_t u) { float f; memcpy(&f, &u, 4); return f; }
+static inline uint32_t f32_bits(float f) { uint32_t u; memcpy(&u, &f, 4); return u; }
+static inline float bf16_to_f32(uint16_t h) { return bits_f32((uint32_t)h << 16); }
+/* fp32 -> bf16, round to nearest, ties to even (finite inputs) */
+static inline uint16_t f32_to_bf16(float f) {
+  uint32_t u = f32_bits(f);
+  uint32_t lsb = (u >> 16) & 1u;
+  return (uint16_t)((u + 0x7FFFu + lsb) >> 16);
+}
+
+/* E2M1: magnitudes {0, .5, 1, 1.5, 2, 3, 4, 6}; nearest, ties to the even code, saturating; the sign bit of the
+ * input survives even when the magnitude rounds to zero */
+static inline uint8_t e2m1_encode(float v) {
+  static const float grid[8] = {0.0f, 0.5f, 1.0f, 1.5f, 2.0f, 3.0f, 4.0f, 6.0f};
+  float a = fabsf(v);
+  int code = 7;
+  if (a < 6.0f) {
+    code = 0;
+    while (code < 7 && a >= grid[code + 1]) ++code;          /* grid[code] <= a < grid[code + 1] */
+    float lo = a - grid[code], hi = grid[code + 1] - a;       /* both exact: small dyadic numbers */
+    if (hi < lo || (hi == lo && (code & 1))) ++code;          /* nearer neighbour; a tie goes to the even code */
+  }
+  return (uint8_t)(code | ((f32_bits(v) >> 31) << 3));
+}
+static inline float e2m1_decode(uint8_t c) {
+  static const float grid[8] = {0.0f, 0.5f, 1.0f, 1.5f, 2.0f, 3.0f, 4.0f, 6.0f};
+  float m = grid[c & 7];
+  return (c & 8) ? -m : m;
+}
+
+/* E4M3: bias 7, 3 mantissa bits, subnormals down to 2^-9, largest finite 448; x >= 0; RNE, saturating */
+static inline float e4m3_decode(uint8_t c) {
+  int e = (c >> 3) & 15, m = c & 7;
+  return e == 0 ? ldexpf((float)m, -9) : ldexpf((float)(8 + m), e - 10);
+}
+static inline uint8_t e4m3_encode(float x) {
+  if (!(x > 0.0f)) return 0;
+  if (x >= 448.0f) return 0x7E;
+  /* walk the 127 finite codes: the grid is monotone in the code, so bisect for the last code whose value is <= x */
+  int lo = 0, hi = 0x7E;
+  while (lo < hi) {
+    int mid = (lo + hi + 1) >> 1;
+    if (e4m3_decode((uint8_t)mid) <= x) lo = mid; else hi = mid - 1;
+  }
+  if (lo == 0x7E) return 0x7E;
+  double below = (double)e4m3_decode((uint8_t)lo), above = (double)e4m3_decode((uint8_t)(lo + 1));
+  double dl = (double)x - below, dh = above - (double)x;      /* exact in double */
+  if (dh < dl || (dh == dl && (lo & 1))) ++lo;                /* ties to the even code (even mantissa) */
+  return (uint8_t)lo;
+}
+
+/* E8M0: smallest power of two >= x (x >= 0), exponent clamped to [-127, 127]; x == 0 -> 2^-127 (R8) */
+static inline uint8_t e8m0_encode_up(float x) {
+  if (!(x > 0.0f)) return 0;
+  int e;
+  float m = frexpf(x, &e);                                    /* x = m 2^e, m in [0.5, 1) */
+  int up = (m == 0.5f) ? e - 1 : e;
+  if (up < -127) up = -127;
+  if (up > 127) up = 127;
+  return (uint8_t)(up + 127);
+}
+static inline float e8m0_decode(uint8_t c) { return ldexpf(1.0f, (int)c - 127); }
+
+static const uint32_t kC6bits = 0x3E2AAAABu;                  /* RN(1/6), R6 */
+
+/* block scale (Eq. 3; R6, R8): code, effective scale and its reciprocal for a group maximum a */
+static inline void block_scale(float a, int fmt, float ts, float inv_ts, uint8_t* code, float* s_eff, float* inv) {
+  float q = a * bits_f32(kC6bits);
+  if (fmt == FMT_NVFP4) {
+    float sf = q * inv_ts;
+    *code = e4m3_encode(sf);
+    *s_eff = e4m3_decode(*code) * ts;
+  } else {
+    *code = e8m0_encode_up(q);
+    *s_eff = e8m0_decode(*code);
+  }
+  *inv = (*s_eff == 0.0f) ? 0.0f : 1.0f / *s_eff;
+}
+
+/* ---- O1 normalisation (R1, R3) --------------------------------------------------------------- */
+/* canonical fp32 sum of t[0..K) (or of RN(t*t)), in R1's order, defined on the column index k */
+static float canonical_sum(const float* t, int64_t K, int squares) {
+  float P[32];
+  for (int l = 0; l < 32; ++l) P[l] = 0.0f;
+  int64_t blocks = (K + 1023) / 1024;
+  for (int64_t b = 0; b < blocks; ++b)
+    for (int j = 0; j < 4; ++j)
+      for (int l = 0; l < 32; ++l) {
+        float leaf = 0.0f;
+        for (int i = 0; i < 8; ++i) {
+          int64_t k = b * 1024 + l * 32 + j * 8 + i;
+          float v = k < K ? t[k] : 0.0f;                     /* columns beyond K do not exist: +0 */
+          if (squares) v = v * v;
+          leaf = leaf + v;
+        }
+        P[l] = P[l] + leaf;
+      }
+  for (int delta = 16; delta >= 1; delta >>= 1) {
+    float Q[32];
+    for (int l = 0; l < 32; ++l) Q[l] = P[l] + P[l ^ delta];
+    memcpy(P, Q, sizeof P);
+  }
+  return P[0];
+}
+
+/* X (bf16 bits) = norm(x) for one row; c is scratch of K floats */
+static void normalize_row(const uint16_t* x, int64_t K, int norm, const uint16_t* gamma, const uint16_t* beta, float eps,
+                          uint16_t* X, float* c) {
+  if (norm == NORM_NONE) { memcpy(X, x, (size_t)K * 2); return; }
+  for (int64_t k = 0; k < K; ++k) c[k] = bf16_to_f32(x[k]);
+  float Kf = (float)K;
+  if (norm == NORM_LAYER) {
+    float mu = canonical_sum(c, K, 0) / Kf;
+    for (int64_t k = 0; k < K; ++k) c[k] = c[k] - mu;
+  }
+  float S = canonical_sum(c, K, 1);
+  float ms = S / Kf;
+  float v = ms + eps;
+  float rstd = 1.0f / sqrtf(v);
+  for (int64_t k = 0; k < K; ++k) {
+    uint16_t h = f32_to_bf16(c[k] * rstd);                                        /* first rounding: h = bf16(x rstd) */
+    uint16_t g = f32_to_bf16(bf16_to_f32(h) * bf16_to_f32(gamma[k]));             /* second: X = bf16(h gamma) */
+    if (norm == NORM_LAYER && beta) g = f32_to_bf16(bf16_to_f32(g) + bf16_to_f32(beta[k]));
+    X[k] = g;
+  }
+}
+
+/* ---- O3 pairwise 4:8 mask (R2, R4) ---------------------------------------------------------------------- */
+/* one chunk of 8 bf16 values -> the two kept pair indices i0 < i1 */
+static void top2_pairs(const uint16_t* X8, int* i0, int* i1) {
+  int score[4];
+  for (int p = 0; p < 4; ++p) {
+    int a = X8[2 * p] & 0x7FFF, b = X8[2 * p + 1] & 0x7FFF;
+    score[p] = a > b ? a : b;
+  }
+  /* best, then second best; a later pair wins only when strictly larger, so ties go to the lower index */
+  int first = 0;
+  for (int p = 1; p < 4; ++p) if (score[p] > score[first]) first = p;
+  int second = -1;
+  for (int p = 0; p < 4; ++p) {
+    if (p == first) continue;
+    if (second < 0 || score[p] > score[second]) second = p;
+  }
+  *i0 = first < second ? first : second;
+  *i1 = first < second ? second : first;
+}
+
+/* ---- sharq_prepare, one row (Fig. 2) ----------------------------------------------------------- */
+static void prepare_row(const uint16_t* x, int64_t K, int fmt, int norm, const uint16_t* gamma, const uint16_t* beta,
+                        float eps, const float* static_ts, uint8_t* sp_codes, uint8_t* sp_sf, uint8_t* sp_meta,
+                        uint8_t* dn_codes, uint8_t* dn_sf, float* ts_out, uint16_t* X_out, uint16_t* X, float* c,
+                        float* R, uint8_t* keep) {
+  normalize_row(x, K, norm, gamma, beta, eps, X, c);
+  if (X_out) memcpy(X_out, X, (size_t)K * 2);
+  /* O2 tensor scale (R5) */
+  float ts = 1.0f;
+  if (fmt == FMT_NVFP4) {
+    if (static_ts) ts = *static_ts;
+    else {
+      uint16_t m = 0;
+      for (int64_t k = 0; k < K; ++k) { uint16_t a = X[k] & 0x7FFF; if (a > m) m = a; }
+      float a_row = bf16_to_f32(m);
+      ts = a_row == 0.0f ? 1.0f : a_row / 2688.0f;
+    }
+  }
+  float inv_ts = 1.0f / ts;
+  *ts_out = ts;
+  /* O3 mask */
+  for (int64_t ch = 0; ch < K / 8; ++ch) {
+    int i0, i1;
+    top2_pairs(X + ch * 8, &i0, &i1);
+    uint8_t nib = (uint8_t)(i0 | (i1 << 2));
+    if (ch & 1) sp_meta[ch / 2] |= (uint8_t)(nib << 4); else sp_meta[ch / 2] = nib;
+    for (int p = 0; p < 4; ++p) keep[ch * 8 + 2 * p] = keep[ch * 8 + 2 * p + 1] = (p == i0 || p == i1);
+  }
+  /* O4 backbone + O5 residual, one group of 32 logical k at a time (Eq. 7, Eq. 8) */
+  int64_t ns = 0;                                             /* survivors written so far */
+  for (int64_t g = 0; g < K / 32; ++g) {
+    float a = 0.0f;
+    for (int i = 0; i < 32; ++i)
+      if (keep[g * 32 + i]) { float v = fabsf(bf16_to_f32(X[g * 32 + i])); if (v > a) a = v; }
+    float s_eff, inv;
+    block_scale(a, fmt, ts, inv_ts, &sp_sf[g], &s_eff, &inv);
+    for (int i = 0; i < 32; ++i) {
+      int64_t k = g * 32 + i;
+      float xv = bf16_to_f32(X[k]);
+      if (!keep[k]) { R[k] = xv; continue; }
+      uint8_t code = e2m1_encode(xv * inv);
+      float d = e2m1_decode(code) * s_eff;
+      R[k] = xv - d;
+      if (ns & 1) sp_codes[ns / 2] |= (uint8_t)(code << 4); else sp_codes[ns / 2] = code;
+      ++ns;
+    }
+  }
+  /* O6 residual, dense groups */
+  int Gd = fmt == FMT_NVFP4 ? 16 : 32;
+  for (int64_t g = 0; g < K / Gd; ++g) {
+    float a = 0.0f;
+    for (int i = 0; i < Gd; ++i) { float v = fabsf(R[g * Gd + i]); if (v > a) a = v; }
+    float s_eff, inv;
+    block_scale(a, fmt, ts, inv_ts, &dn_sf[g], &s_eff, &inv);
+    for (int i = 0; i < Gd; ++i) {
+      int64_t k = g * Gd + i;
+      uint8_t code = e2m1_encode(R[k] * inv);
+      if (k & 1) dn_codes[k / 2] |= (uint8_t)(code << 4); else dn_codes[k / 2] = code;
+    }
+  }
+}
+
+static int pick_threads(int nthreads) {
+#ifdef _OPENMP
+  return nthreads > 0 ? nthreads : omp_get_max_threads();
+#else
+  (void)nthreads;
+  return 1;
+#endif
+}
+
+/* Canonical (row-major) outputs: sp_codes [T,K/4], sp_sf [T,K/32], sp_meta [T,K/16], dn_codes [T,K/2],
+ * dn_sf [T,K/Gd] (Gd = 16 NVFP4 / 32 MXFP4), ts [T]; X_out [T,K] bf16 bits or NULL.  static_ts NULL = dynamic per-row.
+ * Returns the number of threads used, or -1 on a bad argument. */
+int so_prepare(const uint16_t* x, int64_t T, int64_t K, int fmt, int norm, const uint16_t* gamma, const uint16_t* beta,
+               float eps, const float* static_ts, uint8_t* sp_codes, uint8_t* sp_sf, uint8_t* sp_meta,
+               uint8_t* dn_codes, uint8_t* dn_sf, float* ts, uint16_t* X_out, int nthreads) {
+  if (K <= 0 || K % 256 || T < 0 || (fmt != FMT_NVFP4 && fmt != FMT_MXFP4) || norm < 0 || norm > 2) return -1;
+  if (norm != NORM_NONE && !gamma) return -1;
+  int nt = pick_threads(nthreads);
+  int64_t Gd = fmt == FMT_NVFP4 ? 16 : 32;
+#pragma omp parallel num_threads(nt)
+  {
+    uint16_t* X = (uint16_t*)malloc((size_t)K * 2);
+    float* c = (float*)malloc((size_t)K * 4);
+    float* R = (float*)malloc((size_t)K * 4);
+    uint8_t* keep = (uint8_t*)malloc((size_t)K);
+#pragma omp for schedule(static)
+    for (int64_t t = 0; t < T; ++t)
+      prepare_row(x + t * K, K, fmt, norm, gamma, beta, eps, static_ts, sp_codes + t * (K / 4), sp_sf + t * (K / 32),
+                  sp_meta + t * (K / 16), dn_codes + t * (K / 2), dn_sf + t * (K / Gd), ts + t,
+                  X_out ? X_out + t * K : NULL, X, c, R, keep);
+    free(X); free(c); free(R); free(keep);
+  }
+  return nt;
+}
+
+/* ---- sharq_quantize_weight (Fig. 2 caption; R7) ---------------------------------------------------- */
+/* codes [D,K/2], sf_sp [D,K/32], sf_dn [D,K/16] (NVFP4: every scale twice) or [D,K/32] (MXFP4), ts_w scalar */
+int so_quantize_weight(const uint16_t* w, int64_t D, int64_t K, int fmt, uint8_t* codes, uint8_t* sf_sp, uint8_t* sf_dn,
+                       float* ts_w, int nthreads) {
+  if (K <= 0 || K % 256 || D < 0 || (fmt != FMT_NVFP4 && fmt != FMT_MXFP4)) return -1;
+  int nt = pick_threads(nthreads);
+  float ts = 1.0f;
+  if (fmt == FMT_NVFP4) {
+    uint16_t m = 0;
+    for (int64_t i = 0; i < D * K; ++i) { uint16_t a = w[i] & 0x7FFF; if (a > m) m = a; }
+    float a = bf16_to_f32(m);
+    ts = a == 0.0f ? 1.0f : a / 2688.0f;
+  }
+  float inv_ts = 1.0f / ts;
+  *ts_w = ts;
+#pragma omp parallel for schedule(static) num_threads(nt)
+  for (int64_t d = 0; d < D; ++d) {
+    const uint16_t* row = w + d * K;
+    for (int64_t g = 0; g < K / 32; ++g) {
+      float a = 0.0f;
+      for (int i = 0; i < 32; ++i) { float v = fabsf(bf16_to_f32(row[g * 32 + i])); if (v > a) a = v; }
+      uint8_t code; float s_eff, inv;
+      block_scale(a, fmt, ts, inv_ts, &code, &s_eff, &inv);
+      sf_sp[d * (K / 32) + g] = code;
+      if (fmt == FMT_NVFP4) sf_dn[d * (K / 16) + 2 * g] = sf_dn[d * (K / 16) + 2 * g + 1] = code;
+      else sf_dn[d * (K / 32) + g] = code;
+      for (int i = 0; i < 32; ++i) {
+        int64_t k = g * 32 + i;
+        uint8_t c4 = e2m1_encode(bf16_to_f32(row[k]) * inv);
+        if (k & 1) codes[d * (K / 2) + k / 2] |= (uint8_t)(c4 << 4); else codes[d * (K / 2) + k / 2] = c4;
+      }
+    }
+  }
+  return nt;
+}
+
+/* ---- O7 the linear layer in fp64 (Eq. 9) ------------------------------------------------------------------ */
+static inline double sf_value(uint8_t code, int fmt) {
+  return fmt == FMT_NVFP4 ? (double)e4m3_decode(code) : (double)e8m0_decode(code);
+}
+
+/* Y[i, j] = ( sum_k Asp[rows[i], k] Wsp[cols[j], k] + sum_k Adn[rows[i], k] Wdn[cols[j], k] ) ts[rows[i]] ts_w  in fp64,
+ * from the STORED canonical outputs only (what the GEMMs see): the backbone is scattered back to its logical positions
+ * through the metadata and read through the weight's sparse (group-32) scale view, the residual through the dense view.
+ * rows / cols NULL = all.  Every product code*sf*code*sf is exact in fp64; sums run in ascending k, backbone first. */
+int so_linear(int64_t T, int64_t K, int64_t D, int fmt, const uint8_t* sp_codes, const uint8_t* sp_sf,
+              const uint8_t* sp_meta, const uint8_t* dn_codes, const uint8_t* dn_sf, const float* ts,
+              const uint8_t* w_codes, const uint8_t* w_sf_sp, const uint8_t* w_sf_dn, float ts_w,
+              const int64_t* rows, int64_t n_rows, const int64_t* cols, int64_t n_cols, double* Y, int nthreads) {
+  if (K <= 0 || K % 256 || (fmt != FMT_NVFP4 && fmt != FMT_MXFP4)) return -1;
+  if (!rows) n_rows = T;
+  if (!cols) n_cols = D;
+  int nt = pick_threads(nthreads);
+  int64_t Gd = fmt == FMT_NVFP4 ? 16 : 32;
+  double* Asp = (double*)calloc((size_t)(n_rows * K), sizeof(double));
+  double* Adn = (double*)malloc((size_t)(n_rows * K) * sizeof(double));
+  if (!Asp || !Adn) { free(Asp); free(Adn); return -2; }
+#pragma omp parallel for schedule(static) num_threads(nt)
+  for (int64_t i = 0; i < n_rows; ++i) {
+    int64_t t = rows ? rows[i] : i;
+    double* asp = Asp + i * K;
+    double* adn = Adn + i * K;
+    int64_t ns = 0;
+    for (int64_t ch = 0; ch < K / 8; ++ch) {
+      uint8_t byte = sp_meta[t * (K / 16) + ch / 2];
+      int nib = (ch & 1) ? byte >> 4 : byte & 15;
+      int idx[2] = {nib & 3, (nib >> 2) & 3};
+      for (int s = 0; s < 2; ++s)
+        for (int e = 0; e < 2; ++e) {
+          int64_t k = ch * 8 + idx[s] * 2 + e;
+          uint8_t b = sp_codes[t * (K / 4) + ns / 2];
+          uint8_t code = (ns & 1) ? b >> 4 : b & 15;
+          ++ns;
+          asp[k] = (double)e2m1_decode(code) * sf_value(sp_sf[t * (K / 32) + k / 32], fmt);
+        }
+    }
+    for (int64_t k = 0; k < K; ++k) {
+      uint8_t b = dn_codes[t * (K / 2) + k / 2];
+      uint8_t code = (k & 1) ? b >> 4 : b & 15;
+      adn[k] = (double)e2m1_decode(code) * sf_value(dn_sf[t * (K / Gd) + k / Gd], fmt);
+    }
+  }
+#pragma omp parallel num_threads(nt)
+  {
+    double* wsp = (double*)malloc((size_t)K * sizeof(double));
+    double* wdn = (double*)malloc((size_t)K * sizeof(double));
+#pragma omp for schedule(static)
+    for (int64_t j = 0; j < n_cols; ++j) {
+      int64_t d = cols ? cols[j] : j;
+      for (int64_t k = 0; k < K; ++k) {
+        uint8_t b = w_codes[d * (K / 2) + k / 2];
+        double v = (double)e2m1_decode((k & 1) ? b >> 4 : b & 15);
+        wsp[k] = v * sf_value(w_sf_sp[d * (K / 32) + k / 32], fmt);
+        wdn[k] = v * sf_value(w_sf_dn[d * (K / Gd) + k / Gd], fmt);
+      }
+      for (int64_t i = 0; i < n_rows; ++i) {
+        const double* asp = Asp + i * K;
+        const double* adn = Adn + i * K;
+        double acc = 0.0;
+        for (int64_t k = 0; k < K; ++k) acc += asp[k] * wsp[k];
+        for (int64_t k = 0; k < K; ++k) acc += adn[k] * wdn[k];
+        int64_t t = rows ? rows[i] : i;
+        Y[i * n_cols + j] = acc * (double)ts[t] * (double)ts_w;
+      }
+    }
+    free(wsp); free(wdn);
+  }
+  free(Asp); free(Adn);
+  return nt;
+}
+
+int so_max_threads(void) { return pick_threads(0); }
+
+/* R1's reduction alone (tests compare it with the numpy oracle on order-sensitive inputs) */
+float so_canonical_sum(const float* t, int64_t K, int squares) { return canonical_sum(t, K, squares); }
