@@ -803,7 +803,7 @@ def run_reference(args):
     if rank != 0:
         return
     world = int(os.environ.get("WORLD_SIZE", "1"))
-    t_prep, t_lin = 1024, 8                                           # a step of about a second: 30 + 5 steps in minutes
+    t_prep, t_lin = HEADLINE_T, 32                                    # the cpu_baseline leg's sample: 1.3 s per step on the box's 16 cores
     co, items = oracle_sample_setup(t_prep, t_lin)
     steps, warmup = args.steps, args.warmup
     budget = 150.0                                                    # seconds: keep the whole run to minutes
