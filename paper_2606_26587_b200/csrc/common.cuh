@@ -58,6 +58,33 @@ __device__ __forceinline__ uint32_t add_bf16x2_rn(uint32_t a, uint32_t b) {
   asm("add.rn.bf16x2 %0, %1, %2;" : "=r"(r) : "r"(a), "r"(b));
   return r;
 }
+__device__ __forceinline__ uint32_t sub_bf16x2_rn(uint32_t a, uint32_t b) {
+  uint32_t r;
+  asm("sub.rn.bf16x2 %0, %1, %2;" : "=r"(r) : "r"(a), "r"(b));
+  return r;
+}
+// a * b + c per half: the exact product and sum, ONE RNE rounding to bf16
+__device__ __forceinline__ uint32_t fma_bf16x2_rn(uint32_t a, uint32_t b, uint32_t c) {
+  uint32_t r;
+  asm("fma.rn.bf16x2 %0, %1, %2, %3;" : "=r"(r) : "r"(a), "r"(b), "r"(c));
+  return r;
+}
+__device__ __forceinline__ uint32_t min_bf16x2(uint32_t a, uint32_t b) {
+  uint32_t r;
+  asm("min.bf16x2 %0, %1, %2;" : "=r"(r) : "r"(a), "r"(b));
+  return r;
+}
+__device__ __forceinline__ uint32_t abs_bf16x2(uint32_t a) {          // FMA pipe (a LOP3 would take an ALU slot)
+  uint32_t r;
+  asm("abs.bf16x2 %0, %1;" : "=r"(r) : "r"(a));
+  return r;
+}
+// per half: magnitude = max(|a|, |b|), sign = sign(a) xor sign(b)
+__device__ __forceinline__ uint32_t max_abs_bf16x2(uint32_t a, uint32_t b) {
+  uint32_t r;
+  asm("max.xorsign.abs.bf16x2 %0, %1, %2;" : "=r"(r) : "r"(a), "r"(b));
+  return r;
+}
 // two fp32 -> one byte of two E2M1 codes (lo in the low nibble), RNE, saturating
 __device__ __forceinline__ uint32_t cvt_e2m1x2(float lo, float hi) {
   uint32_t r;

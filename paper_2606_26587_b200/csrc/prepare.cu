@@ -414,7 +414,7 @@ __global__ void weight_quant_kernel(const uint16_t* W, int64_t D, int64_t K, int
     vmax = fmaxf(vmax, __shfl_xor_sync(0xffffffffu, vmax, 1));
     const Hif4Scale hs = hif4_scale(vmax);
     uint32_t c[4], e8b, e16b;
-    hif4_quant32<false>(X, v16, hs, c, e8b, e16b, nullptr, nullptr);
+    hif4_quant32<false>(X, v16, hs, c, e8b, e16b, nullptr, nullptr, nullptr, nullptr);
     const uint32_t word = hif4_meta_word(hs.e6m2, e8b, e16b, lane);
     if (!act) return;
     *reinterpret_cast<uint4*>(codes + d * (K >> 1) + (k0 >> 1)) = make_uint4(c[0], c[1], c[2], c[3]);
