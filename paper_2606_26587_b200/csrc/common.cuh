@@ -79,10 +79,21 @@ __device__ __forceinline__ uint32_t abs_bf16x2(uint32_t a) {          // FMA pip
   asm("abs.bf16x2 %0, %1;" : "=r"(r) : "r"(a));
   return r;
 }
-// per half: magnitude = max(|a|, |b|), sign = sign(a) xor sign(b)
-__device__ __forceinline__ uint32_t max_abs_bf16x2(uint32_t a, uint32_t b) {
+// byte permute, integer multiply-add and (a & mask) | c as single instructions
+__device__ __forceinline__ uint32_t prmt(uint32_t a, uint32_t b, uint32_t sel) {   // only sel[15:0] is read
   uint32_t r;
-  asm("max.xorsign.abs.bf16x2 %0, %1, %2;" : "=r"(r) : "r"(a), "r"(b));
+  asm("prmt.b32 %0, %1, %2, %3;" : "=r"(r) : "r"(a), "r"(b), "r"(sel));
+  return r;
+}
+
+__device__ __forceinline__ uint32_t mad_lo_u32(uint32_t a, uint32_t b, uint32_t c) {   // IMAD: FMA pipe
+  uint32_t r;
+  asm("mad.lo.u32 %0, %1, %2, %3;" : "=r"(r) : "r"(a), "r"(b), "r"(c));
+  return r;
+}
+__device__ __forceinline__ uint32_t lop3_and_or(uint32_t a, uint32_t mask, uint32_t c) {   // (a & mask) | c
+  uint32_t r;
+  asm("lop3.b32 %0, %1, %2, %3, 0xF8;" : "=r"(r) : "r"(c), "r"(mask), "r"(a));
   return r;
 }
 // two fp32 -> one byte of two E2M1 codes (lo in the low nibble), RNE, saturating

@@ -270,48 +270,89 @@ __device__ __forceinline__ void mma_bf16_pair(uint32_t d_tmem, uint64_t adesc, u
 // spec): one 2048-byte atom per 128 rows x 128 logical k; byte of (row m, logical k) inside the atom =
 //   16 (m % 8) + 2 ((m / 8) % 2) + 256 (m / 16) + 128 ((k / 16) % 2) + 4 (k / 32) + (k % 16) / 8,
 // so that one tcgen05.cp.128x128b puts the four 32-bit columns of the four K = 32 MMAs of the atom into tensor memory.
-__global__ void hif4_dequant_act_sparse_kernel(const uint8_t* __restrict__ sp_codes, const uint32_t* __restrict__ sp_sf,
-                                               const uint8_t* __restrict__ sp_meta, const uint8_t* __restrict__ dn_codes,
-                                               const uint32_t* __restrict__ dn_sf, uint16_t* __restrict__ Asp,
-                                               uint16_t* __restrict__ Adn, uint8_t* __restrict__ E, int64_t T, int64_t Tp,
-                                               int64_t K, int path) {
+//
+// The decode itself is packed bf16x2 (the values are exact in bf16): value = m qup, m the 3 magnitude bits of the code,
+// qup = 0.25 * E6M2 * 2^(E1_8 + E1_16) a bf16 number whose bits are the E6M2 code shifted into place plus exponent-field
+// offsets.  The code nibbles of two neighbouring elements go into the low mantissa bits of 128.0 (0x4300 | m per half),
+// one fma.rn.bf16x2 (128 + m) qup - 128 qup gives m qup exactly, the sign nibble bits are OR-ed in.
+struct Hif4Qup { uint32_t qa, nqa, qb, nqb; };   // qup and -128 qup (bf16x2 splats) of the thread's two 4-groups
+
+// `word` = E6M2 | E1_8 << 8 | E1_16 << 16 of the unit, g8 = index of the thread's 8 elements inside the 64-element unit
+__device__ __forceinline__ Hif4Qup hif4_qup(uint32_t word, uint32_t g8) {
+  const uint32_t base = ((word & 0xFFu) << 5) + (79u << 7) - 0x100u;        // bf16 bits of 0.25 * E6M2 (R11: bias 48)
+  const uint32_t e8 = (word >> (8 + g8)) & 1u, e16 = (word >> (16 + 2 * g8)) & 3u;
+  Hif4Qup q;
+  q.qa = (base + ((e8 + (e16 & 1u)) << 7)) * 0x10001u;
+  q.qb = (base + ((e8 + (e16 >> 1)) << 7)) * 0x10001u;
+  q.nqa = q.qa + 0x83808380u;                                                // exponent + 7, sign set: no carry between halves
+  q.nqb = q.qb + 0x83808380u;
+  return q;
+}
+
+// elements 2j, 2j + 1 of a word of code nibbles (ascending k) -> bf16x2
+__device__ __forceinline__ uint32_t hif4_decode2(uint32_t L, uint32_t H, uint32_t Se, uint32_t So, int j, uint32_t q,
+                                                 uint32_t nq) {
+  const uint32_t sel = 0x4400u + 0x1111u * (uint32_t)j;                      // bytes [lo_j, lo_j, hi_j, hi_j]
+  const uint32_t tq = lop3_and_or(prmt(L, H, sel), 0x00FF00FFu, 0x43004300u);
+  return lop3_and_or(prmt(Se, So, sel), 0x80008000u, fma_bf16x2_rn(tq, q, nq));
+}
+
+// grid: x over the K / 8 element groups of a row (one thread each), y over blocks of kDqRows consecutive rows: the
+// thread keeps its column-derived offsets and walks down the rows with pointer increments
+constexpr int kDqRows = 8;                             // Tp is a multiple of 128
+
+__global__ void __launch_bounds__(128)
+hif4_dequant_act_sparse_kernel(const uint8_t* __restrict__ sp_codes, const uint32_t* __restrict__ sp_sf,
+                               const uint8_t* __restrict__ sp_meta, const uint8_t* __restrict__ dn_codes,
+                               const uint32_t* __restrict__ dn_sf, uint16_t* __restrict__ Asp,
+                               uint16_t* __restrict__ Adn, uint8_t* __restrict__ E, int64_t T, int64_t Tp,
+                               int64_t K, int path) {
   tc::grid_dependency_wait();
-  const int64_t n8 = K >> 3;
-  for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < Tp * n8;
-       idx += (int64_t)gridDim.x * blockDim.x) {
-    const int64_t t = idx / n8, c = idx % n8;          // k = 8c .. 8c+7
-    const uint32_t unit_i = (uint32_t)((8 * c) & 63);
-    uint32_t sp[4] = {0u, 0u, 0u, 0u}, dn[8];
-#pragma unroll
-    for (int i = 0; i < 8; ++i) dn[i] = 0u;
-    uint32_t meta = 0x44u;                             // pad rows: a valid nibble, zero values
-    if (t < T) {
-      meta = sp_meta[t * (K >> 3) + c];                // two nibbles: 4-groups 2c, 2c+1
+  const uint32_t c = blockIdx.x * blockDim.x + threadIdx.x;                  // k = 8c .. 8c + 7: one E1_8 group
+  if (c >= (uint32_t)(K >> 3)) return;
+  const uint32_t g8 = c & 7u, kk = (8u * c) & 127u;
+  for (int64_t t0 = (int64_t)blockIdx.y * kDqRows; t0 < Tp; t0 += (int64_t)gridDim.y * kDqRows) {
+  // row-invariant offsets; all rows of the block lie in one 128-row metadata atom row (kDqRows divides 128)
+  const uint8_t* p_meta = sp_meta + t0 * (K >> 3) + c;
+  const uint32_t* p_spsf = sp_sf + t0 * (K >> 6) + (c >> 3);
+  const uint32_t* p_dnsf = dn_sf + t0 * (K >> 6) + (c >> 3);
+  const uint8_t* p_spc = sp_codes + t0 * (K >> 2) + 2 * c;
+  const uint8_t* p_dnc = dn_codes + t0 * (K >> 1) + 4 * c;
+  uint16_t* p_asp = Asp + t0 * (K >> 1) + 4 * c;
+  uint16_t* p_adn = Adn + t0 * K + 8 * c;
+  uint8_t* p_e = E + ((t0 >> 7) * (K >> 7) + (c >> 4)) * 2048 + 128u * ((kk >> 4) & 1u) + 4u * (kk >> 5) + ((kk & 15u) >> 3);
+  const int64_t rows_valid = T - t0;                   // rows >= T are pad rows: a valid nibble, zero values
+#pragma unroll 4
+  for (int i = 0; i < kDqRows; ++i) {
+    uint2 sp = make_uint2(0u, 0u);
+    uint4 dn = make_uint4(0u, 0u, 0u, 0u);
+    uint32_t meta = 0x44u;
+    if (i < rows_valid) {
+      meta = p_meta[(int64_t)i * (K >> 3)];            // two nibbles: 4-groups 2c, 2c+1
       if (path != 2) {
-        const uint32_t word = sp_sf[t * (K >> 6) + (c >> 3)];
-        const uint32_t codes = *reinterpret_cast<const uint16_t*>(sp_codes + t * (K >> 2) + 2 * c);
-#pragma unroll
-        for (int g = 0; g < 2; ++g) {
-          const uint32_t nib = (meta >> (4 * g)) & 15u, i0 = nib & 3u, i1 = nib >> 2;
-          const uint32_t byte = (codes >> (8 * g)) & 255u;
-          sp[2 * g] = hif4_to_bf16(byte & 15u, word, unit_i + 4 * g + i0);
-          sp[2 * g + 1] = hif4_to_bf16(byte >> 4, word, unit_i + 4 * g + i1);
-        }
+        const Hif4Qup q = hif4_qup(p_spsf[(int64_t)i * (K >> 6)], g8);
+        // two bytes: the survivors i0 < i1 of each 4-group, ascending k, exactly the compressed operand's order
+        const uint32_t codes = *reinterpret_cast<const uint16_t*>(p_spc + (int64_t)i * (K >> 2));
+        const uint32_t L = codes & 0x0707u, H = (codes >> 4) & 0x0707u, Se = (codes << 4) & 0x8080u, So = codes & 0x8080u;
+        sp.x = hif4_decode2(L, H, Se, So, 0, q.qa, q.nqa);
+        sp.y = hif4_decode2(L, H, Se, So, 1, q.qb, q.nqb);
       }
       if (path != 1) {
-        const uint32_t word = dn_sf[t * (K >> 6) + (c >> 3)];
-        const uint32_t codes = *reinterpret_cast<const uint32_t*>(dn_codes + t * (K >> 1) + 4 * c);
-#pragma unroll
-        for (int e = 0; e < 8; ++e) dn[e] = hif4_to_bf16((codes >> (4 * e)) & 15u, word, unit_i + e);
+        const Hif4Qup q = hif4_qup(p_dnsf[(int64_t)i * (K >> 6)], g8);
+        const uint32_t codes = *reinterpret_cast<const uint32_t*>(p_dnc + (int64_t)i * (K >> 1));
+        const uint32_t L = codes & 0x07070707u, H = (codes >> 4) & 0x07070707u;
+        const uint32_t Se = (codes << 4) & 0x80808080u, So = codes & 0x80808080u;
+        dn.x = hif4_decode2(L, H, Se, So, 0, q.qa, q.nqa);
+        dn.y = hif4_decode2(L, H, Se, So, 1, q.qa, q.nqa);
+        dn.z = hif4_decode2(L, H, Se, So, 2, q.qb, q.nqb);
+        dn.w = hif4_decode2(L, H, Se, So, 3, q.qb, q.nqb);
       }
     }
-    *reinterpret_cast<uint2*>(Asp + t * (K >> 1) + 4 * c) = make_uint2(sp[0] | sp[1] << 16, sp[2] | sp[3] << 16);
-    *reinterpret_cast<uint4*>(Adn + t * K + 8 * c) =
-        make_uint4(dn[0] | dn[1] << 16, dn[2] | dn[3] << 16, dn[4] | dn[5] << 16, dn[6] | dn[7] << 16);
-    const int64_t m = t & 127, kk = (8 * c) & 127;
-    const int64_t atom = (t >> 7) * (K >> 7) + ((8 * c) >> 7);
-    E[atom * 2048 + 16 * (m & 7) + 2 * ((m >> 3) & 1) + 256 * (m >> 4) + 128 * ((kk >> 4) & 1) + 4 * (kk >> 5) + ((kk & 15) >> 3)] =
-        (uint8_t)meta;
+    *reinterpret_cast<uint2*>(p_asp + (int64_t)i * (K >> 1)) = sp;
+    *reinterpret_cast<uint4*>(p_adn + (int64_t)i * K) = dn;
+    const uint32_t m = ((uint32_t)t0 + (uint32_t)i) & 127u;
+    p_e[16 * (m & 7) + 2 * ((m >> 3) & 1) + 256 * (m >> 4)] = (uint8_t)meta;
+  }
   }
 }
 
@@ -563,8 +604,8 @@ sharq_status launch_sp_pair(const LinearArgs& a, void* workspace, int64_t Tp, in
   uint16_t* Adn = reinterpret_cast<uint16_t*>(base + (size_t)Tp * (size_t)a.K);
   uint8_t* E = base + (size_t)Tp * (size_t)a.K * 3;
   const uint16_t* W = reinterpret_cast<const uint16_t*>(a.w_sf_dn);
-  const int64_t na = Tp * (a.K >> 3);
-  hif4_dequant_act_sparse_kernel<<<(unsigned)((na + 255) / 256 < 8192 ? (na + 255) / 256 : 8192), 256, 0, st>>>(
+  const dim3 dq_grid((unsigned)(((a.K >> 3) + 127) / 128), (unsigned)(Tp / kDqRows < 65535 ? Tp / kDqRows : 65535));
+  hif4_dequant_act_sparse_kernel<<<dq_grid, 128, 0, st>>>(
       (const uint8_t*)a.sp_codes, (const uint32_t*)a.sp_sf, (const uint8_t*)a.sp_meta, (const uint8_t*)a.dn_codes,
       (const uint32_t*)a.dn_sf, Asp, Adn, E, a.T, Tp, a.K, a.path);
   if (cudaGetLastError() != cudaSuccess) return SHARQ_ECUDA;
