@@ -64,18 +64,22 @@ __device__ __forceinline__ void epilogue_flush(const P& p, uint32_t stg, int lan
   }
 }
 
-// all BN columns of one accumulator stage of this warp's 32 rows
+// all BN columns of one accumulator stage of this warp's 32 rows.  The tensor-memory load of chunk c + 1 is issued
+// before chunk c is scaled, staged and stored (two register buffers, loop fully unrolled): the load latency of every
+// chunk but the first runs under the previous chunk's work instead of in front of its own.
 template <int BN, class P>
 __device__ __forceinline__ void epilogue_tile(const P& p, uint32_t taddr, uint32_t stg, int lane, int64_t row0, int rows_ok,
                                               int n0, float scale) {
-#pragma unroll 1
-  for (int c = 0; c < BN / 32; ++c) {
-    uint32_t v[32];
-    tc::tmem_ld32(taddr + c * 32, v);
-    tc::tmem_ld_wait();
+  constexpr int NC = BN / 32;
+  uint32_t v[2][32];
+  tc::tmem_ld32(taddr, v[0]);
+#pragma unroll
+  for (int c = 0; c < NC; ++c) {
+    tc::tmem_ld_wait(v[c & 1]);                       // chunk c has arrived (tcgen05.wait::ld covers every earlier load)
+    if (c + 1 < NC) tc::tmem_ld32(taddr + (c + 1) * 32, v[(c + 1) & 1]);
     const bool second = !p.out_fp32 && (c & 1);
-    epilogue_stage32(p, stg, lane, n0 + c * 32, second ? 1 : 0, scale, v);
-    if (p.out_fp32 || second || c == BN / 32 - 1) {   // (a tile of an odd number of 32-column chunks: half a staged row)
+    epilogue_stage32(p, stg, lane, n0 + c * 32, second ? 1 : 0, scale, v[c & 1]);
+    if (p.out_fp32 || second || c == NC - 1) {        // (a tile of an odd number of 32-column chunks: half a staged row)
       __syncwarp();
       epilogue_flush(p, stg, lane, row0, rows_ok, n0 + (second ? c - 1 : c) * 32, min(p.D, n0 + (c + 1) * 32));
       __syncwarp();
