@@ -215,11 +215,11 @@ __device__ __forceinline__ void store_row(const KParams& p, int64_t row, int col
 // COMBO = true: the Table 5 combinations (path 3 / 4): second K-loop on the second operand (tm_alt, sf2, meta2).
 // The body is shared; the __global__ wrappers below differ in their parameter lists, so that the plain kernel --
 // every decode and MoE launch -- carries neither the fourth tensor map nor the prepare parameters.
-template <int BN, int FMT, bool SPLIT, int AR, bool MC, bool FUSED, bool COMBO>
+template <int BN, int FMT, bool SPLIT, int AR, int MC, bool FUSED, bool COMBO>
 __device__ __forceinline__ void linear_body(const CUtensorMap* tm_a_sp_p, const CUtensorMap* tm_a_dn_p,
                                             const CUtensorMap* tm_w_p, const CUtensorMap* tm_alt_p, const KParams& p,
                                             const PrepParams* pp_p, const int prep_norm) {
-  using S = Stage<BN, FMT, SPLIT, AR, FUSED ? kPrepSmem : 0>;
+  using S = Stage<BN, FMT, SPLIT, AR, FUSED ? kPrepSmem : (MC == 2 ? kStageBytes : 0)>;   // MC == 2: staging for 8 epilogue warps
   static_assert(!(FUSED && MC), "the fused kernel is for single-problem launches");
   static_assert(!(COMBO && (SPLIT || MC || FUSED)), "combinations run on the persistent single-problem variant");
   constexpr bool NV = (FMT == SHARQ_NVFP4);
@@ -235,8 +235,12 @@ __device__ __forceinline__ void linear_body(const CUtensorMap* tm_a_sp_p, const 
   const uint32_t act_bar = bars + 8u * (2 * S::STAGES + 5);          // FUSED: this CTA's prepared operands are in memory
   int32_t* grp_tab = reinterpret_cast<int32_t*>(smem_raw + (bars + 256u - smem_u32(smem_raw)));   // offs[E+1], pref[E+1]
   uint8_t* prep_smem = smem_raw + (bars + 256u + (uint32_t)S::GRP - smem_u32(smem_raw));          // FUSED: prepare_rows' scratch
-  const uint32_t stg_base = bars + 256u + (uint32_t)S::GRP + (FUSED ? (uint32_t)kPrepSmem : 0u);     // epilogue staging
+  const uint32_t stg_base = bars + 256u + (uint32_t)S::GRP + (FUSED ? (uint32_t)kPrepSmem : 0u);     // epilogue staging (MC == 2: EXTRA + STG)
 
+  // MC == 2 (320 threads; the short-K expert GEMMs are bound by draining and storing the tiles): eight epilogue warps,
+  // two per tensor-memory sub-partition, each taking half of the tile's columns; their staging costs a pipeline stage
+  // (3 instead of 4), which tiles of <= 4 k-blocks do not miss.  Long-K launches keep MC == 1: four warps, 4 stages.
+  constexpr int kEpiWarps = MC == 2 ? 8 : 4;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   if (warp == 0) SHARQ_TS(0);
   const bool do_sp = p.path == 0 || p.path == 1 || p.path == 4, do_dn = p.path == 0 || p.path == 2 || p.path == 3;
@@ -261,7 +265,7 @@ __device__ __forceinline__ void linear_body(const CUtensorMap* tm_a_sp_p, const 
     }
     for (int a = 0; a < 2; ++a) {
       tc::mbar_init(tmem_full_bar(a), 1);
-      tc::mbar_init(tmem_empty_bar(a), 4);          // one arrival per epilogue warp
+      tc::mbar_init(tmem_empty_bar(a), kEpiWarps);  // one arrival per epilogue warp
     }
     if constexpr (FUSED) tc::mbar_init(act_bar, 1);
     tc::fence_mbar_init();
@@ -510,7 +514,7 @@ __device__ __forceinline__ void linear_body(const CUtensorMap* tm_a_sp_p, const 
         if (lead) tc::tc_commit(tmem_full_bar(as));                // accumulator complete
       }
     }
-  } else if (warp < 6) {
+  } else if (warp < 2 + kEpiWarps) {
     // =========================== epilogue ====================================================
     tc::grid_dependency_wait();                          // row_scale is sharq_prepare's; Y may still be read
     if constexpr (FUSED) tc::mbar_wait(act_bar, 0);      // ... here: this launch's own prepare warps write it
@@ -527,8 +531,15 @@ __device__ __forceinline__ void linear_body(const CUtensorMap* tm_a_sp_p, const 
         const float scale = row_ok ? __fmul_rn(FUSED ? __ldcg(p.row_scale + row) : p.row_scale[row], p.w_ts[u.expert]) : 0.0f;
         tc::mbar_wait(tmem_full_bar(as), (n_unit / S::ACC_STAGES) & 1u);
         tc::tc_fence_after();
-        epilogue_tile<BN>(p, lane_addr + as * BN, stg_base + (uint32_t)sub * 4096u, lane, (int64_t)u.m_blk * BM + sub * 32,
-                          min(32, max(0, u.rows_valid - sub * 32)), u.n_blk * BN, scale);
+        if constexpr (MC == 2) {
+          const int half = (warp - 2) >> 2;                // columns [half BN / 2, (half + 1) BN / 2)
+          epilogue_tile<BN / 2>(p, lane_addr + as * BN + half * (BN / 2), stg_base + (uint32_t)(sub + 4 * half) * 4096u, lane,
+                                (int64_t)u.m_blk * BM + sub * 32, min(32, max(0, u.rows_valid - sub * 32)),
+                                u.n_blk * BN + half * (BN / 2), scale);
+        } else {
+          epilogue_tile<BN>(p, lane_addr + as * BN, stg_base + (uint32_t)sub * 4096u, lane, (int64_t)u.m_blk * BM + sub * 32,
+                            min(32, max(0, u.rows_valid - sub * 32)), u.n_blk * BN, scale);
+        }
         tc::tc_fence_before();
         __syncwarp();
         if (lane == 0) tc::mbar_arrive(tmem_empty_bar(as));
@@ -650,8 +661,8 @@ __device__ __forceinline__ void linear_body(const CUtensorMap* tm_a_sp_p, const 
   }
 }
 
-template <int BN, int FMT, bool SPLIT, int AR, bool MC = false>
-__global__ void __launch_bounds__(kThreads, 1)
+template <int BN, int FMT, bool SPLIT, int AR, int MC = 0>
+__global__ void __launch_bounds__(MC == 2 ? kThreads + 128 : kThreads, 1)
 sharq_linear_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __grid_constant__ CUtensorMap tm_a_dn,
                     const __grid_constant__ CUtensorMap tm_w, const KParams p) {
   linear_body<BN, FMT, SPLIT, AR, MC, false, false>(&tm_a_sp, &tm_a_dn, &tm_w, nullptr, p, nullptr, 0);
@@ -1146,11 +1157,11 @@ sharq_status launch_1cta(const LinearArgs& a, const KParams& p, const CUtensorMa
 }
 
 // grouped GEMM: persistent clusters of two CTAs on neighbouring n-tiles, activation operands multicast
-template <int FMT>
-sharq_status launch_mc(const KParams& p, const CUtensorMap& tm_sp, const CUtensorMap& tm_dn,
+template <int FMT, int MC>
+sharq_status launch_mc_impl(const KParams& p, const CUtensorMap& tm_sp, const CUtensorMap& tm_dn,
                        const CUtensorMap& tm_w, int64_t tiles, const LaunchEnv& env) {
-  using S = Stage<128, FMT, false, 128>;
-  auto kfn = sharq_linear_kernel<128, FMT, false, 128, true>;
+  using S = Stage<128, FMT, false, 128, MC == 2 ? kStageBytes : 0>;
+  auto kfn = sharq_linear_kernel<128, FMT, false, 128, MC>;
   const int64_t clusters = tiles / 2 < env.num_sms / 2 ? tiles / 2 : env.num_sms / 2;
   if (env.plan_only) { fill_plan(env.plan_only, 2, 128, 128, 1, S::STAGES, tiles, 2 * clusters, 2); return SHARQ_OK; }
   static std::atomic<uint64_t> smem_set{0};
@@ -1165,11 +1176,19 @@ sharq_status launch_mc(const KParams& p, const CUtensorMap& tm_sp, const CUtenso
   attr[1].val.clusterDim.z = 1;
   lc.attrs = attr;
   lc.numAttrs = 2;
-  lc.blockDim = dim3(kThreads);
+  lc.blockDim = dim3(MC == 2 ? kThreads + 128 : kThreads);
   lc.gridDim = dim3((unsigned)(2 * clusters));
   lc.dynamicSmemBytes = S::SMEM;
   lc.stream = env.st;
   return cudaLaunchKernelEx(&lc, kfn, tm_sp, tm_dn, tm_w, p) == cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
+}
+
+template <int FMT>
+sharq_status launch_mc(const KParams& p, const CUtensorMap& tm_sp, const CUtensorMap& tm_dn,
+                       const CUtensorMap& tm_w, int64_t tiles, const LaunchEnv& env) {
+  // tiles of at most four k-blocks are bound by their drain and stores: eight epilogue warps, three stages
+  return p.K <= 1024 ? launch_mc_impl<FMT, 2>(p, tm_sp, tm_dn, tm_w, tiles, env)
+                     : launch_mc_impl<FMT, 1>(p, tm_sp, tm_dn, tm_w, tiles, env);
 }
 
 // scale-factor / metadata array as a 2-D tensor of 1024-byte rows (256 x u32), boxes of `box_rows` rows
