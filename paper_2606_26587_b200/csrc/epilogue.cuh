@@ -64,25 +64,44 @@ __device__ __forceinline__ void epilogue_flush(const P& p, uint32_t stg, int lan
   }
 }
 
-// all BN columns of one accumulator stage of this warp's 32 rows.  The tensor-memory load of chunk c + 1 is issued
-// before chunk c is scaled, staged and stored (two register buffers, loop fully unrolled): the load latency of every
-// chunk but the first runs under the previous chunk's work instead of in front of its own.
-template <int BN, class P>
+// all BN columns of one accumulator stage of this warp's 32 rows.  PIPE: the tensor-memory load of chunk c + 1 is
+// issued before chunk c is scaled, staged and stored (two register buffers, two chunks per loop iteration), so the load
+// latency of every chunk but the first runs under the previous chunk's work.  (A FULLY unrolled version cost the decode
+// launches, whose CTAs drain one or two tiles in their life, ~1 us each in cold instruction fetches.)
+template <int BN, bool PIPE = true, class P>
 __device__ __forceinline__ void epilogue_tile(const P& p, uint32_t taddr, uint32_t stg, int lane, int64_t row0, int rows_ok,
                                               int n0, float scale) {
   constexpr int NC = BN / 32;
-  uint32_t v[2][32];
-  tc::tmem_ld32(taddr, v[0]);
-#pragma unroll
-  for (int c = 0; c < NC; ++c) {
-    tc::tmem_ld_wait(v[c & 1]);                       // chunk c has arrived (tcgen05.wait::ld covers every earlier load)
-    if (c + 1 < NC) tc::tmem_ld32(taddr + (c + 1) * 32, v[(c + 1) & 1]);
+  auto finish = [&](int c, const uint32_t (&v)[32]) {
     const bool second = !p.out_fp32 && (c & 1);
-    epilogue_stage32(p, stg, lane, n0 + c * 32, second ? 1 : 0, scale, v[c & 1]);
+    epilogue_stage32(p, stg, lane, n0 + c * 32, second ? 1 : 0, scale, v);
     if (p.out_fp32 || second || c == NC - 1) {        // (a tile of an odd number of 32-column chunks: half a staged row)
       __syncwarp();
       epilogue_flush(p, stg, lane, row0, rows_ok, n0 + (second ? c - 1 : c) * 32, min(p.D, n0 + (c + 1) * 32));
       __syncwarp();
+    }
+  };
+  if constexpr (PIPE) {
+    uint32_t v0[32], v1[32];
+    tc::tmem_ld32(taddr, v0);
+#pragma unroll 1
+    for (int c = 0; c < NC; c += 2) {                 // two chunks per iteration: compact code, two register buffers
+      tc::tmem_ld_wait(v0);                           // chunk c has arrived (tcgen05.wait::ld covers every earlier load)
+      if (c + 1 < NC) tc::tmem_ld32(taddr + (c + 1) * 32, v1);
+      finish(c, v0);
+      if (c + 1 < NC) {
+        tc::tmem_ld_wait(v1);
+        if (c + 2 < NC) tc::tmem_ld32(taddr + (c + 2) * 32, v0);
+        finish(c + 1, v1);
+      }
+    }
+  } else {
+#pragma unroll 1
+    for (int c = 0; c < NC; ++c) {
+      uint32_t v[32];
+      tc::tmem_ld32(taddr + c * 32, v);
+      tc::tmem_ld_wait();
+      finish(c, v);
     }
   }
 }

@@ -523,6 +523,7 @@ __device__ __forceinline__ void linear_body(const CUtensorMap* tm_a_sp_p, const 
     const uint32_t lane_addr = tmem_base + ((uint32_t)(sub * 32) << 16);
     if constexpr (!SPLIT) {
       uint32_t n_unit = 0;
+      const bool one_shot = total_tiles <= tile_step;      // every CTA drains at most one tile (decode launches)
       for (int tile = tile0; tile < total_tiles; tile += tile_step, ++n_unit) {
         const Unit u = decode_unit(p, g, m_blocks, total_tiles, tile, 0, 1);
         const uint32_t as = n_unit % S::ACC_STAGES;
@@ -536,6 +537,9 @@ __device__ __forceinline__ void linear_body(const CUtensorMap* tm_a_sp_p, const 
           epilogue_tile<BN / 2>(p, lane_addr + as * BN + half * (BN / 2), stg_base + (uint32_t)(sub + 4 * half) * 4096u, lane,
                                 (int64_t)u.m_blk * BM + sub * 32, min(32, max(0, u.rows_valid - sub * 32)),
                                 u.n_blk * BN + half * (BN / 2), scale);
+        } else if (one_shot) {
+          epilogue_tile<BN, false>(p, lane_addr + as * BN, stg_base + (uint32_t)sub * 4096u, lane, (int64_t)u.m_blk * BM + sub * 32,
+                                   min(32, max(0, u.rows_valid - sub * 32)), u.n_blk * BN, scale);
         } else {
           epilogue_tile<BN>(p, lane_addr + as * BN, stg_base + (uint32_t)sub * 4096u, lane, (int64_t)u.m_blk * BM + sub * 32,
                             min(32, max(0, u.rows_valid - sub * 32)), u.n_blk * BN, scale);
@@ -981,8 +985,12 @@ sharq_linear_pair_kernel(const __grid_constant__ CUtensorMap tm_a_sp, const __gr
       const uint32_t as = n_unit % S::ACC_STAGES;
       tc::mbar_wait(tmem_full_bar(as), (n_unit / S::ACC_STAGES) & 1u);
       tc::tc_fence_after();
-      epilogue_tile<S::BN>(p, lane_addr + as * S::BN, stg_base + (uint32_t)sub * 4096u, lane, (int64_t)u.m_blk * BM + sub * 32,
-                           min(32, max(0, u.rows_valid - sub * 32)), n_blk * S::BN, scale);
+      if (total <= tile_step)                        // one tile per pair in its life (T <= 256): the rolled loop
+        epilogue_tile<S::BN, false>(p, lane_addr + as * S::BN, stg_base + (uint32_t)sub * 4096u, lane,
+                                    (int64_t)u.m_blk * BM + sub * 32, min(32, max(0, u.rows_valid - sub * 32)), n_blk * S::BN, scale);
+      else
+        epilogue_tile<S::BN>(p, lane_addr + as * S::BN, stg_base + (uint32_t)sub * 4096u, lane, (int64_t)u.m_blk * BM + sub * 32,
+                             min(32, max(0, u.rows_valid - sub * 32)), n_blk * S::BN, scale);
       tc::tc_fence_before();
       __syncwarp();
       if (lane == 0) tc::mbar_arrive_cluster(tc::map_to_cta(tmem_empty_bar(as), 0));
