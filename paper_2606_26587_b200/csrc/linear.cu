@@ -105,20 +105,20 @@ struct Stage {
   static constexpr int NSL = BN / 16;                                 // 16-column slices of the accumulator
   static constexpr int RECV = SPLIT ? (NSL + 2) * AR * 64 : 0;        // [src][slot][AR rows][16 fp32]; S*ceil(NSL/S) <= NSL+2 for S in {2,3,4,8}
   static constexpr int PAD = AR < 128 ? 128 * 128 : 0;               // the MMA's over-read behind the last stage
-  static constexpr int GRP = (!SPLIT && AR == 128 && BN == 128) ? 2 * (kMaxExperts + 1) * 4 + 8 : 0;   // expert table (grouped)
+  static constexpr int GRP = (!SPLIT && AR == 128 && (BN == 128 || BN == 192)) ? 2 * (kMaxExperts + 1) * 4 + 8 : 0;   // expert table (grouped)
   static constexpr int STG = SPLIT ? 0 : kStageBytes;                  // epilogue staging (persistent variants)
   static constexpr int FIT = (232448 - 1024 - 256 - RECV - PAD - GRP - EXTRA - STG) / BYTES;
   static constexpr int STAGES = FIT > 8 ? 8 : FIT;
   static constexpr int SMEM = STAGES * BYTES + PAD + RECV + 1024 /*alignment slack*/ + 256 /*barriers*/ + GRP + EXTRA + STG;
   // tensor-memory columns: two accumulator stages, then metadata and scale factors
   static constexpr int SFB_COLS = NB * 4;          // columns one MMA's B scales occupy
-  static constexpr int ACC_STAGES = BN > 128 ? 1 : 2;
-  static constexpr int E_COL = 256;
-  static constexpr int SFA_SP_COL = 260;           // 2 MMAs x 4
-  static constexpr int SFA_DN_COL = 268;           // 4 MMAs x 4
-  static constexpr int SFB_SP_COL = 284;           // 2 MMAs x SFB_COLS (<= 16)
-  static constexpr int SFB_DN_COL = 300;           // 4 MMAs x SFB_COLS (<= 32)
-  static_assert(BN * ACC_STAGES <= 256, "accumulator stages overlap the scale-factor columns");
+  static constexpr int ACC_STAGES = 2 * BN + 76 <= 512 ? 2 : 1;      // 128- and 192-wide tiles: drain overlaps the next tile
+  static constexpr int E_COL = BN * ACC_STAGES > 256 ? BN * ACC_STAGES : 256;   // first column after the accumulators
+  static constexpr int SFA_SP_COL = E_COL + 4;     // 2 MMAs x 4
+  static constexpr int SFA_DN_COL = E_COL + 12;    // 4 MMAs x 4
+  static constexpr int SFB_SP_COL = E_COL + 28;    // 2 MMAs x SFB_COLS (<= 16)
+  static constexpr int SFB_DN_COL = E_COL + 44;    // 4 MMAs x SFB_COLS (<= 32)
+  static_assert(SFB_DN_COL + 32 <= 512, "tensor memory");
   static_assert(STAGES >= 2, "shared memory: fewer than two ring stages");
 };
 
@@ -450,7 +450,7 @@ __device__ __forceinline__ void linear_body(const CUtensorMap* tm_a_sp_p, const 
       uint32_t it = 0, n_unit = 0;
       for (int tile = tile0; tile < total_tiles; tile += tile_step, ++n_unit) {
         const Unit u = decode_unit(p, g, m_blocks, total_tiles, tile, rank, splits);
-        const uint32_t sfb_shift = (BN < 128) ? (uint32_t)(((u.n_blk * BN) % 128) / 32) : 0u;   // sub-atom N tiles
+        const uint32_t sfb_shift = (uint32_t)(((u.n_blk * BN) % 128) / 32);   // tiles that start inside a 128-row scale atom
         const uint32_t as = n_unit % S::ACC_STAGES;                       // accumulator stage
         const uint32_t acc = tmem_base + as * BN;
         tc::mbar_wait(tmem_empty_bar(as), ((n_unit / S::ACC_STAGES) & 1u) ^ 1u);   // epilogue has drained this stage
@@ -1165,13 +1165,13 @@ sharq_status launch_1cta(const LinearArgs& a, const KParams& p, const CUtensorMa
 }
 
 // grouped GEMM: persistent clusters of two CTAs on neighbouring n-tiles, activation operands multicast
-template <int FMT, int MC>
+template <int BN, int FMT, int MC>
 sharq_status launch_mc_impl(const KParams& p, const CUtensorMap& tm_sp, const CUtensorMap& tm_dn,
                        const CUtensorMap& tm_w, int64_t tiles, const LaunchEnv& env) {
-  using S = Stage<128, FMT, false, 128, MC == 2 ? kStageBytes : 0>;
-  auto kfn = sharq_linear_kernel<128, FMT, false, 128, MC>;
+  using S = Stage<BN, FMT, false, 128, MC == 2 ? kStageBytes : 0>;
+  auto kfn = sharq_linear_kernel<BN, FMT, false, 128, MC>;
   const int64_t clusters = tiles / 2 < env.num_sms / 2 ? tiles / 2 : env.num_sms / 2;
-  if (env.plan_only) { fill_plan(env.plan_only, 2, 128, 128, 1, S::STAGES, tiles, 2 * clusters, 2); return SHARQ_OK; }
+  if (env.plan_only) { fill_plan(env.plan_only, 2, BN, 128, 1, S::STAGES, tiles, 2 * clusters, 2); return SHARQ_OK; }
   static std::atomic<uint64_t> smem_set{0};
   if (set_smem_once(smem_set, (const void*)kfn, S::SMEM, env.dev) != cudaSuccess) return SHARQ_ECUDA;
   cudaLaunchConfig_t lc{};
@@ -1191,12 +1191,14 @@ sharq_status launch_mc_impl(const KParams& p, const CUtensorMap& tm_sp, const CU
   return cudaLaunchKernelEx(&lc, kfn, tm_sp, tm_dn, tm_w, p) == cudaSuccess ? SHARQ_OK : SHARQ_ECUDA;
 }
 
-template <int FMT>
+template <int BN, int FMT>
 sharq_status launch_mc(const KParams& p, const CUtensorMap& tm_sp, const CUtensorMap& tm_dn,
                        const CUtensorMap& tm_w, int64_t tiles, const LaunchEnv& env) {
-  // tiles of at most four k-blocks are bound by their drain and stores: eight epilogue warps, three stages
-  return p.K <= 1024 ? launch_mc_impl<FMT, 2>(p, tm_sp, tm_dn, tm_w, tiles, env)
-                     : launch_mc_impl<FMT, 1>(p, tm_sp, tm_dn, tm_w, tiles, env);
+  if constexpr (BN == 128) {
+    // tiles of at most four k-blocks are bound by their drain and stores: eight epilogue warps, three stages
+    if (p.K <= 1024) return launch_mc_impl<128, FMT, 2>(p, tm_sp, tm_dn, tm_w, tiles, env);
+  }
+  return launch_mc_impl<BN, FMT, 1>(p, tm_sp, tm_dn, tm_w, tiles, env);
 }
 
 // scale-factor / metadata array as a 2-D tensor of 1024-byte rows (256 x u32), boxes of `box_rows` rows
@@ -1317,11 +1319,15 @@ sharq_status launch_tiles(const LinearArgs& a, int64_t rows_total, int64_t m_blo
     if (E > 0 && rows_total / E >= 192 && a.K >= 4096 && !debug_env().no_pair)
       return launch_pair<FMT, 192, true>(a, p, tm_sp, tm_dn, m_blocks, env);
     // experts: n-tiles of one 128-row block are consecutive (decode_unit), so tiles 2j and 2j+1 share activations
-    if (E > 0 && n_tiles % 2 == 0 && !debug_env().no_mc) return launch_mc<FMT>(p, tm_sp, tm_dn, tm_w, tiles, env);
+    if (E > 0 && n_tiles % 2 == 0 && !debug_env().no_mc) return launch_mc<128, FMT>(p, tm_sp, tm_dn, tm_w, tiles, env);
   }
+  if constexpr (BN == 192) {                               // launch_linear sends only grouped calls with an even n-tile count here
+    return launch_mc<192, FMT>(p, tm_sp, tm_dn, tm_w, tiles, env);
+  } else {
   if (a_rows <= 16) return launch_1cta<BN, FMT, 16>(a, p, tm_sp, tm_dn, tm_w, tm_alt, tiles, env);
   if (a_rows <= 64) return launch_1cta<BN, FMT, 64>(a, p, tm_sp, tm_dn, tm_w, tm_alt, tiles, env);
   return launch_1cta<BN, FMT, 128>(a, p, tm_sp, tm_dn, tm_w, tm_alt, tiles, env);
+  }
 }
 
 }  // namespace
@@ -1367,6 +1373,14 @@ sharq_status launch_linear(const sharq_config* cfg, const LinearArgs& a, int32_t
   if (E == 0 && a.path < 3 && a.T <= debug_env().wide_t && a.D % 256 == 0 && a.D / 128 > num_sms && !debug_env().no_wide) {
     if (cfg->fmt == SHARQ_NVFP4) return launch_tiles<256, SHARQ_NVFP4>(a, rows_total, m_blocks, E, offsets, env);
     return launch_tiles<256, SHARQ_MXFP4>(a, rows_total, m_blocks, E, offsets, env);
+  }
+  // experts with a medium K-loop (more than four k-blocks per tile, too short for the grouped pair tiles): 128 x 192
+  // tiles in multicast clusters.  Those launches are bound by the bytes each SM takes in per k-block (~85 GB/s per SM:
+  // operands of a 128 x 128 tile 48 KB, of a 128 x 192 tile 59 KB for 1.5 x the flop)
+  const bool pair_grouped = E > 0 && rows_total / E >= 192 && a.K >= 4096 && !debug_env().no_pair;
+  if (E > 0 && a.D % 384 == 0 && a.K > 1024 && !pair_grouped && !debug_env().no_mc) {
+    if (cfg->fmt == SHARQ_NVFP4) return launch_tiles<192, SHARQ_NVFP4>(a, rows_total, m_blocks, E, offsets, env);
+    return launch_tiles<192, SHARQ_MXFP4>(a, rows_total, m_blocks, E, offsets, env);
   }
   if (cfg->fmt == SHARQ_NVFP4) return launch_tiles<128, SHARQ_NVFP4>(a, rows_total, m_blocks, E, offsets, env);
   return launch_tiles<128, SHARQ_MXFP4>(a, rows_total, m_blocks, E, offsets, env);

@@ -313,7 +313,8 @@ def test_linear_grouped_device_offsets_and_spare_capacity(sq):
     cfg = sq.make_config(sq.NVFP4, sq.NORM_NONE, 1e-6, sq.LAYOUT_TILED)
     # 2 n-tiles (multicast clusters) / 3 (plain persistent) / long K: CTA-pair tiles on two row blocks of one expert,
     # ragged last n-tile (D = 256 with 192-wide tiles reads the next expert's weight rows, never stored)
-    for D, K in ((256, 512), (384, 512), (256, 4096)):
+    # ... and medium K with D % 384 == 0: 128 x 192 multicast tiles (tiles that start inside a 128-row scale atom)
+    for D, K in ((256, 512), (384, 512), (256, 4096), (384, 2048), (768, 1280)):
         act = sq.alloc_act(cfg, cap, K, "cuda")
         ws, xs = [], []
         for e in range(E):
