@@ -360,9 +360,12 @@ def run_ours(args):
                                                      "lie between the two",
                         mma_issue_probe_tflops=mp)
     gbs = wl.prepare_bytes() / (ms_prep * 1e-3) / 1e9
+    ptraffic, ptraffic_commit = committed_traffic("prepare_traffic_r2.json")
     roofline_prepare = dict(kernel="sharq_prepare_row_kernel (the 4 sharq_prepare launches of the step)", bound="hbm",
                             achieved=round(gbs, 1), peak=pk["hbm"], unit="GB/s", frac=round(gbs / pk["hbm"], 4),
-                            traffic=None, peak_source=pk["source"], launches_per_step=n_lin,
+                            traffic=ptraffic,
+                            traffic_source=("ncu --set full capture at commit " + str(ptraffic_commit)) if ptraffic else None,
+                            peak_source=pk["source"], launches_per_step=n_lin,
                             avg_launch_us=round(ms_prep * 1e3 / n_lin, 2),
                             algorithmic_bytes_per_launch=round(wl.prepare_bytes() / n_lin),
                             share_of_step=round(ms_prep / ms_step, 3),
