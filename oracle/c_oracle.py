@@ -43,6 +43,8 @@ def lib():
         _lib = ctypes.CDLL(build())
         _lib.so_max_threads.restype = ctypes.c_int
         _lib.so_canonical_sum.restype = ctypes.c_float
+        _lib.so_exp_neg.restype = ctypes.c_float
+        _lib.so_exp_neg.argtypes = [ctypes.c_float]
     return _lib
 
 
@@ -113,3 +115,23 @@ def linear(prep, wq, rows=None, cols=None, nthreads=0):
     if rc < 0:
         raise ValueError(f"so_linear failed ({rc})")
     return Y
+
+
+def residual_add(x_u16, r_u16):
+    """h = bf16(x + r), elementwise (bf16 bit patterns)."""
+    x, r = _u16(x_u16), _u16(r_u16)
+    h = np.empty_like(x)
+    lib().so_residual_add(_p(x), _p(r), ctypes.c_int64(x.size), _p(h))
+    return h
+
+
+def swiglu(gate_u16, up_u16, nthreads=0):
+    """h = bf16(silu(gate) * up) with DESIGN.md R18's exp contract."""
+    g, u = _u16(gate_u16), _u16(up_u16)
+    h = np.empty_like(g)
+    lib().so_swiglu(_p(g), _p(u), ctypes.c_int64(g.size), _p(h), int(nthreads))
+    return h
+
+
+def exp_neg(g: float) -> np.float32:
+    return np.float32(lib().so_exp_neg(ctypes.c_float(g)))

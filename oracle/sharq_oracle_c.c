@@ -385,3 +385,43 @@ int so_max_threads(void) { return pick_threads(0); }
 
 /* R1's reduction alone (tests compare it with the numpy oracle on order-sensitive inputs) */
 float so_canonical_sum(const float* t, int64_t K, int squares) { return canonical_sum(t, K, squares); }
+
+/* ---- operators folded in front of the preparation (R18) -------------- */
+/* h = bf16(x + r): the residual-stream add; the fp32 sum then RNE to bf16 */
+void so_residual_add(const uint16_t* x, const uint16_t* r, int64_t n, uint16_t* h) {
+  for (int64_t i = 0; i < n; ++i) h[i] = f32_to_bf16(bf16_to_f32(x[i]) + bf16_to_f32(r[i]));
+}
+
+/* e ~ exp(-g) by R18's fixed algorithm: every step one binary32 RN operation, no FMA; constants as bit patterns */
+static float exp_neg_contract(float g) {
+  static const uint32_t kPoly[6] = {0x3F800000u, 0x3F317218u, 0x3E75FDF0u, 0x3D635847u, 0x3C1D955Bu, 0x3AAEC3FFu};  /* RN(ln2^k / k!) */
+  const float magic = 12582912.0f;                            /* 1.5 * 2^23 */
+  float t = g * bits_f32(0xBFB8AA3Bu);                        /* -RN(log2 e) */
+  if (t < -126.0f) t = -126.0f;
+  if (t > 126.0f) t = 126.0f;
+  volatile float tm = t + magic;                              /* volatile: the compiler must not fold (t + M) - M */
+  float n = tm - magic;                                       /* RNE integer of t */
+  float f = t - n;
+  float p = bits_f32(kPoly[5]);
+  for (int k = 4; k >= 0; --k) {
+    float pf = p * f;
+    p = pf + bits_f32(kPoly[k]);
+  }
+  return p * bits_f32((uint32_t)((int32_t)n + 127) << 23);    /* p * 2^n */
+}
+
+/* h = bf16( silu(g) u ): e = exp_neg(g); den = 1 + e; sig = 1 / den; s = g sig; a = s u; one rounding to bf16 */
+void so_swiglu(const uint16_t* gate, const uint16_t* up, int64_t n, uint16_t* h, int nthreads) {
+  int nt = pick_threads(nthreads);
+#pragma omp parallel for schedule(static) num_threads(nt)
+  for (int64_t i = 0; i < n; ++i) {
+    float g = bf16_to_f32(gate[i]), u = bf16_to_f32(up[i]);
+    float e = exp_neg_contract(g);
+    float den = 1.0f + e;
+    float sig = 1.0f / den;
+    float s = g * sig;
+    h[i] = f32_to_bf16(s * u);
+  }
+}
+
+float so_exp_neg(float g) { return exp_neg_contract(g); }

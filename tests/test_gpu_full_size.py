@@ -79,3 +79,34 @@ def test_linear_whole_rows_at_full_size(sq, fmt, norm, T, K, D):
     got = y[torch.from_numpy(rows).cuda()].cpu().numpy().astype(np.float64)
     err = np.abs(got - y64) / np.maximum(np.abs(y64), 1e-2 * np.sqrt((y64 ** 2).mean()))       # DESIGN.md R15
     assert err.max() <= 1e-3, (err.max(), np.unravel_index(err.argmax(), err.shape))
+
+
+def test_prepare_add_full_tensor_every_byte(sq):
+    """sharq_prepare_add at the size bench.py times (T = 8192, K = 4096, RMSNorm, in place): the whole new residual
+    stream and every prepared byte."""
+    T, K = 8192, 4096
+    x = si.activations(T, K, config=4, outlier_mult=50.0, extra=T)
+    r = si.activations(T, K, config=5, outlier_mult=10.0, extra=K)
+    g = si.gamma(K, 4)
+    cfg = sq.make_config(0, 1, 1e-6, sq.LAYOUT_TILED)
+    act, h_dev = sq.prepare_add(cfg, to_dev(x), to_dev(r), to_dev(g))
+    torch.cuda.synchronize()
+    h = co.residual_add(x, r)
+    assert np.array_equal(h_dev.view(torch.int16).cpu().numpy().view(np.uint16), h), "residual stream"
+    ref = co.prepare(h, 0, 1, g, eps=1e-6, want_X=False)
+    _all_equal(act_to_canonical(sq, cfg, act, T, K), ref, ("sp_meta", "sp_sf", "sp_codes", "dn_sf", "dn_codes"), "prepare_add")
+
+
+def test_prepare_swiglu_full_tensor_every_byte(sq):
+    """sharq_prepare_swiglu at the size bench.py times (T = 8192, K = 14336, gate / up as the halves of one [T, 2K]
+    gate+up output): every prepared byte against the C oracle's restatement of the exp contract (R18)."""
+    T, K = 8192, 14336
+    g_bits = si.activations(T, K, config=4, outlier_mult=5.0, extra=T + 1)
+    u_bits = si.activations(T, K, config=5, outlier_mult=50.0, extra=K + 2)
+    cfg = sq.make_config(0, sq.NORM_NONE, 1e-6, sq.LAYOUT_TILED)
+    both = torch.cat([to_dev(g_bits), to_dev(u_bits)], dim=1)
+    act = sq.prepare_swiglu(cfg, both[:, :K], both[:, K:])
+    torch.cuda.synchronize()
+    ref = co.prepare(co.swiglu(g_bits, u_bits), 0, 0, want_X=False)
+    _all_equal(act_to_canonical(sq, cfg, act, T, K), ref, ("sp_meta", "sp_sf", "sp_codes", "dn_sf", "dn_codes"), "prepare_swiglu")
+    assert np.array_equal(act_to_canonical(sq, cfg, act, T, K)["ts"].view(np.uint32), ref["ts"].view(np.uint32))

@@ -106,6 +106,20 @@ def test_codec_tables_exhaustive():
               so.prepare(xb, fmt=fmt, norm=so.NORM_NONE, x_tensor_scale=None if fmt else 1.0 / 512))
 
 
+def test_front_end_operators_agree():
+    # N1 (R18): the residual-stream add and SiLU(gate) * up, bit for bit; the exp contract on a sweep incl. both clamps
+    rng = np.random.default_rng(23)
+    x = si.to_bf16_bits((rng.standard_normal(5000) * np.exp2(rng.integers(-20, 8, 5000))).astype(np.float32))
+    r = si.to_bf16_bits((rng.standard_normal(5000) * np.exp2(rng.integers(-20, 8, 5000))).astype(np.float32))
+    assert np.array_equal(co.residual_add(x, r), so.residual_add(x, r))
+    g = si.to_bf16_bits(np.concatenate([np.linspace(-100, 100, 4001), rng.standard_normal(4000) * 4]).astype(np.float32))
+    u = si.to_bf16_bits(rng.standard_normal(g.size).astype(np.float32))
+    assert np.array_equal(co.swiglu(g, u), so.swiglu(g, u))
+    assert np.array_equal(co.swiglu(g, u, nthreads=1), so.swiglu(g, u))
+    for v in (-200.0, -88.0, -1.0, -1e-8, 0.0, 0.5, 17.3, 87.3, 88.0, 200.0):
+        assert co.exp_neg(v).tobytes() == np.float32(so.exp_neg_contract(np.float32(v))).tobytes(), v
+
+
 def test_rejects_bad_arguments():
     x = np.zeros((2, 100), np.uint16)
     with pytest.raises(ValueError):
