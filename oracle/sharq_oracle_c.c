@@ -8,7 +8,8 @@
  *   2. the CPU baseline BASELINE.md section 3 asks for: the oracle compiled with -O2 (no fast-math, no FMA contraction),
  *      rows parallelised over the host cores with OpenMP.  Never tuned beyond that.
  * Scope: NVFP4 and MXFP4, pairwise 4:8 mask, norm none / RMS / Layer, dynamic or static tensor scale, weights, Eq. 9 in
- * fp64.  (HiF4 lives in the numpy oracle only.)
+ * fp64, and the two operators folded in front of the preparation (residual add, SiLU(gate) * up: R18).  (HiF4, the
+ * element-wise 2:4 mask and the Table 5 path combinations live in the numpy oracle only.)
  *
  * Numerics contract (R1-R8): every float operation below is ONE IEEE-754 binary32 operation, round to nearest
  * even; build with -O2 -ffp-contract=off -fno-fast-math (oracle/build_c.py).  bf16 values travel as uint16 bit patterns.
