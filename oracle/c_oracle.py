@@ -135,3 +135,47 @@ def swiglu(gate_u16, up_u16, nthreads=0):
 
 def exp_neg(g: float) -> np.float32:
     return np.float32(lib().so_exp_neg(ctypes.c_float(g)))
+
+
+def prepare_hif4(x_u16, norm=NORM_RMS, gamma_u16=None, beta_u16=None, eps=1e-6, nthreads=0):
+    """Same stored outputs as the numpy oracle's `prepare_hif4` (2:4 mask, Algorithm 1 on backbone and residual)."""
+    x = _u16(x_u16)
+    T, K = x.shape
+    out = dict(sp_codes=np.empty((T, K // 4), np.uint8), sp_sf=np.empty((T, K // 64), np.uint32),
+               sp_meta=np.empty((T, K // 8), np.uint8), dn_codes=np.empty((T, K // 2), np.uint8),
+               dn_sf=np.empty((T, K // 64), np.uint32), ts=np.ones(T, np.float32))
+    g, b = _u16(gamma_u16), _u16(beta_u16)
+    rc = lib().so_prepare_hif4(_p(x), ctypes.c_int64(T), ctypes.c_int64(K), int(norm), _p(g), _p(b), ctypes.c_float(eps),
+                               _p(out["sp_codes"]), _p(out["sp_sf"]), _p(out["sp_meta"]), _p(out["dn_codes"]),
+                               _p(out["dn_sf"]), int(nthreads))
+    if rc < 0:
+        raise ValueError(f"so_prepare_hif4 rejected its arguments ({rc})")
+    out.update(fmt=2, threads=rc, T=T, K=K)
+    return out
+
+
+def quantize_weight_hif4(w_u16, nthreads=0):
+    w = _u16(w_u16)
+    D, K = w.shape
+    out = dict(codes=np.empty((D, K // 2), np.uint8), sf_sp=np.empty((D, K // 64), np.uint32))
+    rc = lib().so_quantize_weight_hif4(_p(w), ctypes.c_int64(D), ctypes.c_int64(K), _p(out["codes"]), _p(out["sf_sp"]),
+                                       int(nthreads))
+    if rc < 0:
+        raise ValueError(f"so_quantize_weight_hif4 rejected its arguments ({rc})")
+    out.update(fmt=2, threads=rc, D=D, K=K)
+    return out
+
+
+def linear_hif4(prep, wq, rows=None, cols=None, nthreads=0):
+    T, K, D = prep["T"], prep["K"], wq["D"]
+    r = None if rows is None else np.ascontiguousarray(rows, dtype=np.int64)
+    c = None if cols is None else np.ascontiguousarray(cols, dtype=np.int64)
+    nr, nc = (T if r is None else len(r)), (D if c is None else len(c))
+    Y = np.empty((nr, nc), np.float64)
+    rc = lib().so_linear_hif4(ctypes.c_int64(T), ctypes.c_int64(K), ctypes.c_int64(D), _p(prep["sp_codes"]),
+                              _p(prep["sp_sf"]), _p(prep["sp_meta"]), _p(prep["dn_codes"]), _p(prep["dn_sf"]),
+                              _p(wq["codes"]), _p(wq["sf_sp"]), _p(r), ctypes.c_int64(nr), _p(c), ctypes.c_int64(nc),
+                              _p(Y), int(nthreads))
+    if rc < 0:
+        raise ValueError(f"so_linear_hif4 failed ({rc})")
+    return Y

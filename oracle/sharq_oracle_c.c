@@ -8,8 +8,9 @@
  *   2. the CPU baseline BASELINE.md section 3 asks for: the oracle compiled with -O2 (no fast-math, no FMA contraction),
  *      rows parallelised over the host cores with OpenMP.  Never tuned beyond that.
  * Scope: NVFP4 and MXFP4, pairwise 4:8 mask, norm none / RMS / Layer, dynamic or static tensor scale, weights, Eq. 9 in
- * fp64, and the two operators folded in front of the preparation (residual add, SiLU(gate) * up: R18).  (HiF4, the
- * element-wise 2:4 mask and the Table 5 path combinations live in the numpy oracle only.)
+ * fp64, the two operators folded in front of the preparation (residual add, SiLU(gate) * up: R18), and HiF4 (Algorithm 1,
+ * 2:4 mask, R9-R12) at the end of the file.  (The element-wise 2:4 mask on E2M1 formats and the Table 5 path combinations
+ * live in the numpy oracle only.)
  *
  * Numerics contract (R1-R8): every float operation below is ONE IEEE-754 binary32 operation, round to nearest
  * even; build with -O2 -ffp-contract=off -fno-fast-math (oracle/build_c.py).  bf16 values travel as uint16 bit patterns.
@@ -426,3 +427,204 @@ void so_swiglu(const uint16_t* gate, const uint16_t* up, int64_t n, uint16_t* h,
 }
 
 float so_exp_neg(float g) { return exp_neg_contract(g); }
+
+/* ==== HiF4 (Appendix A.2; R9-R12, R16) ======================================================= */
+/* A unit = 64 S1P2 elements + one 32-bit word E6M2 | E1_8 << 8 | E1_16 << 16.  Conversion from BF16 = Algorithm 1
+ * (P:496-528), RNE everywhere (R9), BF16 intermediates (R10). */
+
+/* E6M2 (Table 7): value(c) = 2^((c >> 2) - 48) (1 + (c & 3) / 4), codes 0x00 .. 0xFE */
+static inline float e6m2_value(int c) { return ldexpf(1.0f + (float)(c & 3) * 0.25f, (c >> 2) - 48); }
+/* nearest code, ties to the even mantissa, clamped to [2^-48, 1.5 * 2^15]; by bisection over the monotone grid */
+static int e6m2_encode(float sf) {
+  if (!(sf >= e6m2_value(0))) return 0;                       /* below the minimum, and 0 (R11) */
+  if (sf >= e6m2_value(0xFE)) return 0xFE;
+  int lo = 0, hi = 0xFE;
+  while (lo < hi) {
+    int mid = (lo + hi + 1) >> 1;
+    if (e6m2_value(mid) <= sf) lo = mid; else hi = mid - 1;
+  }
+  double dl = (double)sf - (double)e6m2_value(lo), dh = (double)e6m2_value(lo + 1) - (double)sf;
+  if (dh < dl || (dh == dl && (lo & 1))) ++lo;
+  return lo;
+}
+/* E6M2_REC_to_BF16: bf16(1 / 1.M) from a 4-entry table, exponent negated */
+static inline float e6m2_reciprocal(int c) {
+  static const float lut[4] = {1.0f, 0.80078125f, 0.66796875f, 0.5703125f};
+  return ldexpf(lut[c & 3], -((c >> 2) - 48));
+}
+static inline float round_bf16(float x) { return bf16_to_f32(f32_to_bf16(x)); }
+
+/* Algorithm 1 on one unit: V = 64 bf16 bit patterns -> 64 S1P2 codes (bit 3 sign, 3 bits of |.| in quarters) + word */
+static void hif4_encode_unit(const uint16_t* V, uint8_t* codes, uint32_t* word) {
+  float v16[16], v8[8], vmax = 0.0f;
+  for (int j = 0; j < 16; ++j) {                              /* stage 1: three-level tree of maxima (lines 1-8) */
+    float m = 0.0f;
+    for (int i = 0; i < 4; ++i) { float a = fabsf(bf16_to_f32(V[4 * j + i])); if (a > m) m = a; }
+    v16[j] = m;
+  }
+  for (int g = 0; g < 8; ++g) { v8[g] = v16[2 * g] > v16[2 * g + 1] ? v16[2 * g] : v16[2 * g + 1]; if (v8[g] > vmax) vmax = v8[g]; }
+  float sf = round_bf16(vmax * 0.142578125f);                 /* line 10: (1/7) in bf16, bf16 multiply */
+  int e6 = e6m2_encode(sf);                                   /* line 11 */
+  float rec = e6m2_reciprocal(e6);                            /* line 12 */
+  uint32_t w = (uint32_t)e6;
+  float s8[8], s16[16];
+  for (int g = 0; g < 8; ++g) {                               /* line 13 */
+    int b = v8[g] * rec >= 4.0f;
+    s8[g] = b ? 0.5f : 1.0f;
+    w |= (uint32_t)b << (8 + g);
+  }
+  for (int j = 0; j < 16; ++j) {                              /* line 14 */
+    int b = (v16[j] * rec) * s8[j / 2] >= 2.0f;
+    s16[j] = b ? 0.5f : 1.0f;
+    w |= (uint32_t)b << (16 + j);
+  }
+  for (int i = 0; i < 64; ++i) {                              /* lines 17-21: scale (a BF16 value, R10), then S1P2 */
+    float scaled = (round_bf16(bf16_to_f32(V[i]) * rec) * s8[i / 8]) * s16[i / 4];
+    float q = nearbyintf(fabsf(scaled) * 4.0f);               /* RNE (default rounding mode) */
+    int mag = q > 7.0f ? 7 : (int)q;
+    codes[i] = (uint8_t)(mag | ((f32_bits(scaled) >> 31) << 3));
+  }
+  *word = w;
+}
+/* Eq. 15, 0-based integer division (R16): V_i = E6M2 2^(E1_8[i / 8] + E1_16[i / 4]) S1P2_i; exact in fp32 */
+static inline float hif4_decode(uint8_t code, uint32_t word, int i) {
+  float mag = (float)(code & 7) * 0.25f;
+  int sh = (int)((word >> (8 + i / 8)) & 1u) + (int)((word >> (16 + i / 4)) & 1u);
+  float v = ldexpf(mag, sh) * e6m2_value((int)(word & 0xFFu));
+  return (code & 8) ? -v : v;
+}
+
+/* 2:4: the two largest |x| of four, ties to the lower index */
+static void top2_of4(const uint16_t* X4, int* i0, int* i1) {
+  int first = 0, second = -1;
+  for (int p = 1; p < 4; ++p) if ((X4[p] & 0x7FFF) > (X4[first] & 0x7FFF)) first = p;
+  for (int p = 0; p < 4; ++p) {
+    if (p == first) continue;
+    if (second < 0 || (X4[p] & 0x7FFF) > (X4[second] & 0x7FFF)) second = p;
+  }
+  *i0 = first < second ? first : second;
+  *i1 = first < second ? second : first;
+}
+
+/* sharq_prepare with HiF4: sp_codes [T,K/4], sp_sf u32 [T,K/64], sp_meta [T,K/8] (one nibble per 4 elements),
+ * dn_codes [T,K/2], dn_sf u32 [T,K/64]; ts = 1 */
+int so_prepare_hif4(const uint16_t* x, int64_t T, int64_t K, int norm, const uint16_t* gamma, const uint16_t* beta,
+                    float eps, uint8_t* sp_codes, uint32_t* sp_sf, uint8_t* sp_meta, uint8_t* dn_codes, uint32_t* dn_sf,
+                    int nthreads) {
+  if (K <= 0 || K % 256 || T < 0 || norm < 0 || norm > 2 || (norm != NORM_NONE && !gamma)) return -1;
+  int nt = pick_threads(nthreads);
+#pragma omp parallel num_threads(nt)
+  {
+    uint16_t* X = (uint16_t*)malloc((size_t)K * 2);
+    uint16_t* Xsp = (uint16_t*)malloc((size_t)K * 2);
+    uint16_t* Rb = (uint16_t*)malloc((size_t)K * 2);
+    float* c = (float*)malloc((size_t)K * 4);
+    uint8_t* keep = (uint8_t*)malloc((size_t)K);
+    uint8_t* code = (uint8_t*)malloc((size_t)K);
+#pragma omp for schedule(static)
+    for (int64_t t = 0; t < T; ++t) {
+      normalize_row(x + t * K, K, norm, gamma, beta, eps, X, c);
+      for (int64_t q = 0; q < K / 4; ++q) {                   /* mask; M (.) X has +0 at dropped positions */
+        int i0, i1;
+        top2_of4(X + 4 * q, &i0, &i1);
+        uint8_t nib = (uint8_t)(i0 | (i1 << 2));
+        uint8_t* m = sp_meta + t * (K / 8) + q / 2;
+        if (q & 1) *m |= (uint8_t)(nib << 4); else *m = nib;
+        for (int p = 0; p < 4; ++p) { keep[4 * q + p] = (p == i0 || p == i1); Xsp[4 * q + p] = keep[4 * q + p] ? X[4 * q + p] : 0; }
+      }
+      int64_t ns = 0;
+      for (int64_t u = 0; u < K / 64; ++u) {                  /* backbone: Alg. 1 on 64 LOGICAL positions (R12) */
+        uint32_t w;
+        hif4_encode_unit(Xsp + 64 * u, code + 64 * u, &w);
+        sp_sf[t * (K / 64) + u] = w;
+        for (int i = 0; i < 64; ++i) {
+          int64_t k = 64 * u + i;
+          float xf = bf16_to_f32(X[k]);
+          float r = xf;
+          if (keep[k]) {
+            r = xf - hif4_decode(code[k], w, i);              /* Eq. 8 */
+            uint8_t* dst = sp_codes + t * (K / 4) + ns / 2;
+            if (ns & 1) *dst |= (uint8_t)(code[k] << 4); else *dst = code[k];
+            ++ns;
+          }
+          Rb[k] = f32_to_bf16(r);                             /* Alg. 1 takes BF16 input */
+        }
+      }
+      for (int64_t u = 0; u < K / 64; ++u) {                  /* residual */
+        uint32_t w;
+        hif4_encode_unit(Rb + 64 * u, code + 64 * u, &w);
+        dn_sf[t * (K / 64) + u] = w;
+        for (int i = 0; i < 64; i += 2) dn_codes[t * (K / 2) + (64 * u + i) / 2] = (uint8_t)(code[64 * u + i] | (code[64 * u + i + 1] << 4));
+      }
+    }
+    free(X); free(Xsp); free(Rb); free(c); free(keep); free(code);
+  }
+  return nt;
+}
+
+int so_quantize_weight_hif4(const uint16_t* w, int64_t D, int64_t K, uint8_t* codes, uint32_t* sf, int nthreads) {
+  if (K <= 0 || K % 256 || D < 0) return -1;
+  int nt = pick_threads(nthreads);
+#pragma omp parallel for schedule(static) num_threads(nt)
+  for (int64_t d = 0; d < D; ++d)
+    for (int64_t u = 0; u < K / 64; ++u) {
+      uint8_t c[64];
+      hif4_encode_unit(w + d * K + 64 * u, c, &sf[d * (K / 64) + u]);
+      for (int i = 0; i < 64; i += 2) codes[d * (K / 2) + (64 * u + i) / 2] = (uint8_t)(c[i] | (c[i + 1] << 4));
+    }
+  return nt;
+}
+
+/* Eq. 9 in fp64 for HiF4 from the stored arrays (backbone scattered through the 2:4 metadata) */
+int so_linear_hif4(int64_t T, int64_t K, int64_t D, const uint8_t* sp_codes, const uint32_t* sp_sf, const uint8_t* sp_meta,
+                   const uint8_t* dn_codes, const uint32_t* dn_sf, const uint8_t* w_codes, const uint32_t* w_sf,
+                   const int64_t* rows, int64_t n_rows, const int64_t* cols, int64_t n_cols, double* Y, int nthreads) {
+  if (K <= 0 || K % 256) return -1;
+  if (!rows) n_rows = T;
+  if (!cols) n_cols = D;
+  int nt = pick_threads(nthreads);
+  double* A = (double*)calloc((size_t)(n_rows * K), sizeof(double));     /* backbone at its logical positions, 0 elsewhere */
+  double* B = (double*)malloc((size_t)(n_rows * K) * sizeof(double));     /* residual */
+  if (!A || !B) { free(A); free(B); return -2; }
+#pragma omp parallel for schedule(static) num_threads(nt)
+  for (int64_t i = 0; i < n_rows; ++i) {
+    int64_t t = rows ? rows[i] : i, ns = 0;
+    for (int64_t q = 0; q < K / 4; ++q) {
+      uint8_t byte = sp_meta[t * (K / 8) + q / 2];
+      int nib = (q & 1) ? byte >> 4 : byte & 15;
+      int idx[2] = {nib & 3, (nib >> 2) & 3};
+      for (int s = 0; s < 2; ++s) {
+        int64_t k = 4 * q + idx[s];
+        uint8_t b = sp_codes[t * (K / 4) + ns / 2];
+        uint8_t code = (ns & 1) ? b >> 4 : b & 15;
+        ++ns;
+        A[i * K + k] = (double)hif4_decode(code, sp_sf[t * (K / 64) + k / 64], (int)(k % 64));
+      }
+    }
+    for (int64_t k = 0; k < K; ++k) {
+      uint8_t b = dn_codes[t * (K / 2) + k / 2];
+      B[i * K + k] = (double)hif4_decode((k & 1) ? b >> 4 : b & 15, dn_sf[t * (K / 64) + k / 64], (int)(k % 64));
+    }
+  }
+#pragma omp parallel num_threads(nt)
+  {
+    double* wv = (double*)malloc((size_t)K * sizeof(double));
+#pragma omp for schedule(static)
+    for (int64_t j = 0; j < n_cols; ++j) {
+      int64_t d = cols ? cols[j] : j;
+      for (int64_t k = 0; k < K; ++k) {
+        uint8_t b = w_codes[d * (K / 2) + k / 2];
+        wv[k] = (double)hif4_decode((k & 1) ? b >> 4 : b & 15, w_sf[d * (K / 64) + k / 64], (int)(k % 64));
+      }
+      for (int64_t i = 0; i < n_rows; ++i) {
+        double acc = 0.0;
+        for (int64_t k = 0; k < K; ++k) acc += A[i * K + k] * wv[k];
+        for (int64_t k = 0; k < K; ++k) acc += B[i * K + k] * wv[k];
+        Y[i * n_cols + j] = acc;
+      }
+    }
+    free(wv);
+  }
+  free(A); free(B);
+  return nt;
+}

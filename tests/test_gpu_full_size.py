@@ -110,3 +110,37 @@ def test_prepare_swiglu_full_tensor_every_byte(sq):
     ref = co.prepare(co.swiglu(g_bits, u_bits), 0, 0, want_X=False)
     _all_equal(act_to_canonical(sq, cfg, act, T, K), ref, ("sp_meta", "sp_sf", "sp_codes", "dn_sf", "dn_codes"), "prepare_swiglu")
     assert np.array_equal(act_to_canonical(sq, cfg, act, T, K)["ts"].view(np.uint32), ref["ts"].view(np.uint32))
+
+
+@pytest.mark.parametrize("norm,T,K", [(1, 4096, 3584), (0, 4096, 18944)])
+def test_hif4_prepare_full_tensor_every_byte(sq, norm, T, K):
+    """HiF4 sharq_prepare (packed bf16x2 Algorithm 1) at configs[3]'s sizes: every stored byte of every row against the
+    C oracle's scalar restatement of Algorithm 1."""
+    x, g = si.activations(T, K, config=4, outlier_mult=50.0, extra=T + K), si.gamma(K, 4)
+    cfg = sq.make_config(sq.HIF4, norm, 1e-6, sq.LAYOUT_CANONICAL)
+    act = sq.prepare(cfg, to_dev(x), to_dev(g) if norm else None)
+    torch.cuda.synchronize()
+    ref = co.prepare_hif4(x, norm, g if norm else None, eps=1e-6)
+    _all_equal(act_to_canonical(sq, cfg, act, T, K), ref, ("sp_meta", "sp_sf", "sp_codes", "dn_sf", "dn_codes"), f"hif4 norm{norm} K{K}")
+
+
+def test_hif4_weight_and_linear_whole_rows_at_full_size(sq):
+    """configs[3] Qwen qkv in HiF4 (T = 4096, 3584 -> 4608): the whole weight payload byte for byte, its bf16 GEMM-side
+    view equal to the decoded values, and every output feature of 40 seeded rows of the sparse + dense bf16 GEMM."""
+    T, K, D = 4096, 3584, 4608
+    x, g, w = si.activations(T, K, config=4, extra=T + D), si.gamma(K, 4), si.weight(D, K, config=4, extra=D)
+    cfg = sq.make_config(sq.HIF4, 1, 1e-6, sq.LAYOUT_CANONICAL)
+    wq = sq.quantize_weight(cfg, to_dev(w))
+    act = sq.prepare(cfg, to_dev(x), to_dev(g))
+    y = sq.linear(cfg, act, wq, out_dtype="fp32")
+    torch.cuda.synchronize()
+    wc = co.quantize_weight_hif4(w)
+    got_w = weight_to_canonical(sq, cfg, wq, D, K)
+    assert np.array_equal(got_w["codes"], wc["codes"]) and np.array_equal(got_w["sf_sp"], wc["sf_sp"])
+    rows = np.random.default_rng(T + D).choice(T, 40, replace=False)
+    rows[:6] = (0, 1, 127, T - 128, T - 2, T - 1)
+    rows = np.unique(rows)
+    y64 = co.linear_hif4(co.prepare_hif4(x, 1, g, eps=1e-6), wc, rows=rows)
+    got = y[torch.from_numpy(rows).cuda()].cpu().numpy().astype(np.float64)
+    err = np.abs(got - y64) / np.maximum(np.abs(y64), 1e-2 * np.sqrt((y64 ** 2).mean()))
+    assert err.max() <= 1e-3, (err.max(), np.unravel_index(err.argmax(), err.shape))

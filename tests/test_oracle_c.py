@@ -120,6 +120,52 @@ def test_front_end_operators_agree():
         assert co.exp_neg(v).tobytes() == np.float32(so.exp_neg_contract(np.float32(v))).tobytes(), v
 
 
+@pytest.mark.parametrize("norm", [so.NORM_NONE, so.NORM_RMS, so.NORM_LAYER])
+@pytest.mark.parametrize("K", [256, 768, 3584])
+def test_hif4_prepare_agrees_byte_for_byte(norm, K):
+    # Algorithm 1, 2:4 mask, residual: every stored byte, incl. zero rows, ties, 1e-30 .. 1e30 magnitudes
+    T = 12
+    x = si.activations(T, K, config=2, outlier_mult=200.0, extra=K + norm)
+    x[2] = 0
+    x[3, :64] = si.to_bf16_bits(np.full(64, -0.75, np.float32))
+    xf = si.bf16_bits_to_f32(x).copy()
+    xf[4] *= 1e-30; xf[5] *= 1e30; xf[6] *= 2.0 ** -50; xf[7] *= 2.0 ** 14
+    x = si.to_bf16_bits(xf) if norm == so.NORM_NONE else x
+    g, b = si.gamma(K, 2), si.beta(K, 2)
+    pc = co.prepare_hif4(x, norm, g, b if norm == so.NORM_LAYER else None, eps=1e-5)
+    pn = so.prepare(x, fmt=so.HIF4, mask=so.MASK_24, norm=norm, gamma_u16=g, beta_u16=b if norm == so.NORM_LAYER else None,
+                    eps=1e-5)
+    for k in ("sp_meta", "sp_codes", "sp_sf", "dn_codes", "dn_sf"):
+        assert pc[k].dtype == pn[k].dtype and np.array_equal(pc[k], pn[k]), k
+
+
+def test_hif4_weights_and_linear_agree():
+    T, K, D = 6, 512, 24
+    x, g, w = si.activations(T, K, config=4), si.gamma(K, 4), si.weight(D, K, 4)
+    wc, wn = co.quantize_weight_hif4(w), so.quantize_weight(w, fmt=so.HIF4)
+    assert np.array_equal(wc["codes"], wn["codes"]) and np.array_equal(wc["sf_sp"], wn["sf_sp"])
+    pc = co.prepare_hif4(x, so.NORM_RMS, g)
+    pn = so.prepare(x, fmt=so.HIF4, mask=so.MASK_24, norm=so.NORM_RMS, gamma_u16=g)
+    Yc, Yn = co.linear_hif4(pc, wc), so.linear(pn, wn)
+    assert np.abs(Yc - Yn).max() <= 1e-12 * np.sqrt((Yn ** 2).mean())
+    rows, cols = np.array([4, 1]), np.array([23, 0, 7])
+    assert np.array_equal(co.linear_hif4(pc, wc, rows=rows, cols=cols, nthreads=2), Yc[np.ix_(rows, cols)])
+
+
+def test_hif4_scale_codec_sweep():
+    # every E6M2 rounding decision: units whose maximum sweeps 7 * (a fine grid over three octaves and both clamps)
+    vals = np.concatenate([np.linspace(1.0, 8.0, 1793), [2.0 ** -60, 2.0 ** -49, 2.0 ** -48, 1.2 * 2.0 ** 17, 1e37]]).astype(np.float32)
+    x = np.zeros((len(vals), 256), np.float32)
+    x[:, 0] = vals * 7
+    x[:, 1] = -vals * 3.3
+    x[:, 5] = vals * 0.9
+    x[:, 70] = vals
+    xb = si.to_bf16_bits(x)
+    pc, pn = co.prepare_hif4(xb, so.NORM_NONE), so.prepare(xb, fmt=so.HIF4, mask=so.MASK_24, norm=so.NORM_NONE)
+    for k in ("sp_meta", "sp_codes", "sp_sf", "dn_codes", "dn_sf"):
+        assert np.array_equal(pc[k], pn[k]), k
+
+
 def test_rejects_bad_arguments():
     x = np.zeros((2, 100), np.uint16)
     with pytest.raises(ValueError):
